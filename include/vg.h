@@ -1,0 +1,152 @@
+/*
+ * vg.h -- C ABI of libvg: batched solid-geometry navigation queries on one NVIDIA B200 (sm_100a).
+ *
+ * The operations are the three questions the paper asks of the geometry for every particle
+ * (sec. III.C):
+ *     "Is the particle inside or outside the solid?"                                   -> vg_inside
+ *     "What is the minimal distance between the particle and the border of the solid?" -> vg_safety_to_in/out
+ *     "What is the maximal step length for a particle with a given velocity and
+ *      direction?"                                                                     -> vg_distance_to_in/out
+ * and the navigation step that uses them (the distance to the geometric border
+ * competes with the physics step; "coordinate transformations and distance calculations")
+ *                                                                                      -> vg_compute_step.
+ * The paper defines no solid and no formula; the exact meaning of every query is the reading
+ * R1-R21 of SURVEY.md sec. 8(c), restated in DESIGN.md sec. 3.  In one line each:
+ *   Inside        VG_INSIDE if sdf(p) < -kTol, VG_OUTSIDE if sdf(p) > +kTol, else VG_SURFACE (kTol = 1e-9)
+ *   SafetyToIn    +sdf(p), SafetyToOut  -sdf(p): exact signed Euclidean distance to the surface
+ *   DistanceToIn  -1 if p is inside; else the first t > 0 with p + t d on the surface; +inf if none or > step_max
+ *   DistanceToOut -1 if p is outside; else likewise
+ *   ComputeStep   lexicographic min of (distance, index) over the mother's DistanceToOut (index -1) and every
+ *                 daughter's DistanceToIn in its local frame p_i = R_i p + b_i, d_i = R_i d; (step_max, -2)
+ *                 if the physics step step_max is shorter.
+ *
+ * Conventions for every entry point
+ *   - Track arrays x, y, z, dx, dy, dz and every output array are DEVICE pointers owned by the caller,
+ *     n elements each, FP64 struct-of-arrays (six separate arrays), 8-byte aligned.  When all of them
+ *     are 16-byte aligned the 128-bit vectorised path is taken; otherwise a 64-bit path (never an
+ *     error, never a host fallback).  Outputs must not alias inputs.
+ *   - Shape parameters and placement matrices are HOST pointers, read during the create call only.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls enqueue
+ *     work and return; they never synchronise.  The caller keeps the arrays alive until the stream
+ *     has passed the call.
+ *   - Directions must be unit vectors to rounding (not checked, not renormalised).
+ *   - Return value: VG_OK or a negative vg_status; vg_last_error() gives a thread-local message.
+ *     n == 0 is VG_OK and launches nothing.  No exceptions, no abort, no output to stdout/stderr.
+ *   - Handles are immutable after create and may be used concurrently from several host threads
+ *     and streams.  A handle belongs to the CUDA device that was current when it was created.
+ *   - There is no CPU implementation behind this interface: without a CUDA device every compute
+ *     call returns VG_ERR_CUDA.
+ */
+#ifndef VG_H
+#define VG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vg_shape vg_shape;   /* opaque solid; owned by the library until vg_shape_destroy          */
+typedef struct vg_volume vg_volume; /* opaque mother + placed daughters; does NOT own the vg_shape objects */
+
+typedef enum { VG_BOX = 0, VG_ORB = 1, VG_TUBE = 2, VG_CONE = 3, VG_TRD = 4, VG_POLYCONE = 5 } vg_kind;
+
+enum { VG_OUTSIDE = 0, VG_SURFACE = 1, VG_INSIDE = 2 }; /* values written by vg_inside */
+
+typedef enum {
+    VG_OK = 0,
+    VG_ERR_ARG = -1,   /* null pointer, negative n, misaligned (not 8-byte) array, bad step_max      */
+    VG_ERR_PARAM = -2, /* shape / volume parameters rejected by validation                           */
+    VG_ERR_ALIGN = -3, /* reserved                                                                   */
+    VG_ERR_CUDA = -4,  /* CUDA runtime error (no device, launch failure); message has the CUDA text  */
+    VG_ERR_NOMEM = -5  /* host or device allocation failed                                           */
+} vg_status;
+
+#define VG_KTOLERANCE 1e-9   /* BASELINE.json: kTolerance; half-width of the surface band (R6)        */
+#define VG_MAX_ZPLANES 32    /* polycone                                                              */
+#define VG_MAX_DAUGHTERS 256 /* per volume                                                            */
+#define VG_HIT_MOTHER (-1)   /* vg_compute_step: the mother's boundary limits the step                */
+#define VG_HIT_STEPMAX (-2)  /* vg_compute_step: step_max (the physics step) limits it   */
+
+/*
+ * vg_shape_create -- build a solid (solids as closed point sets, sec. 8(c) c.1).
+ * `params` (HOST, nparams doubles, lengths unitless, angles in radians):
+ *   VG_BOX      [hx, hy, hz]                               half-lengths, |x|<=hx, |y|<=hy, |z|<=hz
+ *   VG_ORB      [r]                                        x^2+y^2+z^2 <= r^2
+ *   VG_TUBE     [rmin, rmax, dz, sphi, dphi]               |z|<=dz, rmin<=rho<=rmax, phi in [sphi, sphi+dphi]
+ *   VG_CONE     [rmin1, rmax1, rmin2, rmax2, dz, sphi, dphi]  radii linear in z, index 1 at z=-dz, 2 at z=+dz
+ *   VG_TRD      [dx1, dx2, dy1, dy2, dz]                   half-lengths, index 1 at z=-dz, 2 at z=+dz
+ *   VG_POLYCONE [sphi, dphi, nz, z_0, rmin_0, rmax_0, ..., z_{nz-1}, rmin_{nz-1}, rmax_{nz-1}]
+ *               radii linear between consecutive z-planes, z strictly increasing, 2 <= nz <= VG_MAX_ZPLANES
+ *   dphi >= 2 pi (as FP64) means the full revolution.
+ * Validation (VG_ERR_PARAM): wrong nparams, non-finite values, lengths <= 0, rmin < 0, rmin >= rmax at any
+ * plane, dphi <= 0, nz out of range or not an integer, z not strictly increasing.
+ * On success *out receives a handle; derived constants are computed once here on the host.
+ */
+int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **out);
+void vg_shape_destroy(vg_shape *shape); /* NULL is allowed */
+int vg_shape_kind(const vg_shape *shape); /* the vg_kind, or VG_ERR_ARG for NULL */
+
+/* Inside classification of n points.  cls: DEVICE int32[n]. */
+int vg_inside(const vg_shape *shape, const double *x, const double *y, const double *z, int64_t n, int32_t *cls,
+              void *stream);
+
+/* DistanceToIn / DistanceToOut of n tracks.
+ * step_max >= 0, may be +inf; a crossing farther than step_max is reported as +inf.  dist: DEVICE double[n]. */
+int vg_distance_to_in(const vg_shape *shape, const double *x, const double *y, const double *z, const double *dx,
+                      const double *dy, const double *dz, double step_max, int64_t n, double *dist, void *stream);
+int vg_distance_to_out(const vg_shape *shape, const double *x, const double *y, const double *z, const double *dx,
+                       const double *dy, const double *dz, double step_max, int64_t n, double *dist, void *stream);
+
+/* SafetyToIn = +sdf, SafetyToOut = -sdf of n points (exact, signed).
+ * safety: DEVICE double[n]. */
+int vg_safety_to_in(const vg_shape *shape, const double *x, const double *y, const double *z, int64_t n,
+                    double *safety, void *stream);
+int vg_safety_to_out(const vg_shape *shape, const double *x, const double *y, const double *z, int64_t n,
+                     double *safety, void *stream);
+
+/*
+ * vg_volume_create -- a mother solid holding ndaughters placed solids ("coordinate
+ * transformations"; BASELINE.json configs[4]).  `xforms` (HOST): ndaughters * 12 doubles, row-major 3x4
+ * [R | b] per daughter, mother -> daughter-local: p_loc = R p + b, d_loc = R d (reading R12).  R is
+ * expected to be orthonormal (checked to 1e-9: VG_ERR_PARAM otherwise).  0 <= ndaughters <= VG_MAX_DAUGHTERS.
+ * Daughter kinds: box, orb, tube, cone, trd (a polycone daughter gives VG_ERR_ARG in this build).
+ * The shapes' constants are copied; the vg_shape handles may be destroyed afterwards.
+ */
+int vg_volume_create(const vg_shape *mother, int ndaughters, const vg_shape *const *daughters, const double *xforms,
+                     vg_volume **out);
+void vg_volume_destroy(vg_volume *volume); /* NULL is allowed */
+
+/*
+ * vg_compute_step -- navigation step of n tracks.
+ * step: DEVICE double[n]; hit: DEVICE int32[n] in {VG_HIT_STEPMAX, VG_HIT_MOTHER, 0 .. ndaughters-1}.
+ * Ties go to the lowest index, the mother first.  Tracks are expected inside the mother and outside every
+ * daughter; a track outside the mother gets (-1, VG_HIT_MOTHER), a daughter the track is inside of is skipped.
+ */
+int vg_compute_step(const vg_volume *volume, const double *x, const double *y, const double *z, const double *dx,
+                    const double *dy, const double *dz, double step_max, int64_t n, double *step, int32_t *hit,
+                    void *stream);
+
+/*
+ * vg_volume_safety -- isotropic safety of the navigation state of n points (PAPER.md:113 at the level of
+ * placed volumes): min( SafetyToOut_mother(p), min_i SafetyToIn_i(R_i p + b_i) ).  safety: DEVICE double[n].
+ */
+int vg_volume_safety(const vg_volume *volume, const double *x, const double *y, const double *z, int64_t n,
+                     double *safety, void *stream);
+
+/* Thread-local message of the last failing call on this host thread ("" if none). Static storage. */
+const char *vg_last_error(void);
+
+/* ---- measurement helpers (used by bench.py for the roofline denominators; not part of the method) ---- */
+
+/* Runs `launches` back-to-back launches of a register-resident chain of independent FP64 FMAs that fills the
+ * device, timed with CUDA events on `stream`; writes the achieved FP64 rate in FMA instructions (lanes) per
+ * second to *fma_per_s (HOST).  Synchronises the stream. */
+int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *stream);
+/* Enqueues `launches` empty kernels (launch-latency floor for the small-N end of configs[3]). */
+int vg_probe_empty_launch(int launches, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VG_H */

@@ -1,0 +1,658 @@
+/*
+ * vg_oracle.c -- ORACLE.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, scalar CPU implementation of what the hot path computes:
+ * the three geometry questions of the paper (sec. III.C:
+ * "Is the particle inside or outside the solid?", "What is the minimal
+ * distance between the particle and the border of the solid?", "What is the
+ * maximal step length for a particle with a given velocity and direction?")
+ * for box / orb / tube segment / cone segment / trd / polycone, and the
+ * one-level navigation step (distance to the geometric
+ * border against the physics step; "coordinate transformations and distance
+ * calculations").
+ *
+ * The paper gives no formula for any solid.  Every query here is the PLAIN
+ * DEFINITION written out as brute force over the boundary patches of the
+ * solid, following the readings R1-R21 of SURVEY.md sec. 8(c) (listed again in
+ * DESIGN.md):
+ *   - solids as closed point sets ................ SURVEY.md 8(c) c.1
+ *   - Inside / Safety / Cross / Distance / Step ... SURVEY.md 8(c) c.2
+ *   - exact signed Euclidean distance per solid ... SURVEY.md 8(c) c.3
+ *   - first boundary crossing per solid ........... SURVEY.md 8(c) c.4
+ * No early-outs, no symmetry tricks, no direction filters, IEEE divides and
+ * square roots, atan2 for the phi wedge.  Compile with -O2 -ffp-contract=off.
+ *
+ * Independence: this file shares NO code, header, table or constant
+ * generator with paper_1512_06637_b200/csrc (the CUDA path) and includes
+ * nothing from include/.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may load it.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): closed forms and hand-worked
+ * examples E1-E21 (tests/golden/worked_examples.txt), brute-force surface
+ * sampling for every sdf, the eikonal property, sphere tracing and ray
+ * marching for every first crossing, special-case reductions between solids
+ * (trd==box, cone==tube, polycone==cone==tube, inserted collinear z-plane),
+ * rigid-motion and permutation invariance of the navigation step, and the
+ * 80-bit long-double build of this same file (-DORC_LONG_DOUBLE).
+ * Parity unpinned: nothing under readings R1-R21; behaviour INSIDE the
+ * kTol surface band (R7) is outside the parity contract.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifdef ORC_LONG_DOUBLE
+typedef long double real;
+#define R_SQRT sqrtl
+#define R_ATAN2 atan2l
+#define R_FABS fabsl
+#define R_FMOD fmodl
+#define R_COS cosl
+#define R_SIN sinl
+#define R_PI 3.14159265358979323846264338327950288L
+#else
+typedef double real;
+#define R_SQRT sqrt
+#define R_ATAN2 atan2
+#define R_FABS fabs
+#define R_FMOD fmod
+#define R_COS cos
+#define R_SIN sin
+#define R_PI 3.14159265358979323846
+#endif
+
+#define ORC_KTOL ((real)1e-9)      /* BASELINE.json: kTolerance = 1e-9; reading R6 */
+#define ORC_INF ((real)INFINITY)   /* reading R5: a miss is IEEE +inf            */
+#define ORC_MAXZ 32                /* polycone: at most 32 z-planes               */
+#define ORC_MAXV (2 * ORC_MAXZ)
+
+enum { ORC_BOX = 0, ORC_ORB = 1, ORC_TUBE = 2, ORC_CONE = 3, ORC_TRD = 4, ORC_POLYCONE = 5 };
+enum { ORC_OUTSIDE = 0, ORC_SURFACE = 1, ORC_INSIDE = 2 };
+
+typedef struct {
+    int kind;
+    real h[3];                 /* box half-lengths                                      */
+    real r;                    /* orb radius                                            */
+    real trd[5];               /* dx1 dx2 dy1 dy2 dz                                    */
+    real pn[6][3], ph[6];      /* trd: six half-spaces n.p <= h, unit normals           */
+    real fv[6][4][3];          /* trd: the four corners of each face, in order          */
+    int nv;                    /* RZ polygon (tube, cone, polycone): vertex count       */
+    real pr[ORC_MAXV], pz[ORC_MAXV];
+    real sphi, dphi;
+    int full;                  /* dphi >= 2 pi                                          */
+    real e[2][2];              /* unit vectors of the two phi planes (cos, sin)         */
+} orc_shape;
+
+typedef struct {
+    const orc_shape *mother;
+    int nd;
+    const orc_shape **daughter;
+    real *xf;                  /* nd * 12, row-major [R | b], mother -> local (R12)     */
+} orc_volume;
+
+static real rmin2(real a, real b) { return a < b ? a : b; }
+static real rmax2(real a, real b) { return a > b ? a : b; }
+
+/* ------------------------------------------------------------------ create */
+
+static int finite_all(const double *p, int n)
+{
+    for (int i = 0; i < n; ++i)
+        if (!isfinite(p[i])) return 0;
+    return 1;
+}
+
+static void set_wedge(orc_shape *s, real sphi, real dphi)
+{
+    s->sphi = sphi;
+    s->dphi = dphi;
+    /* "dphi >= 2 pi means full": 2 pi is the FP64 value in both builds */
+    s->full = (dphi >= (real)(2.0 * 3.14159265358979323846));
+    /* reading R11: cos/sin of the phi planes evaluated once at create */
+    s->e[0][0] = R_COS(sphi);
+    s->e[0][1] = R_SIN(sphi);
+    s->e[1][0] = R_COS(sphi + dphi);
+    s->e[1][1] = R_SIN(sphi + dphi);
+}
+
+static void trd_setup(orc_shape *s)
+{
+    /* SURVEY.md 8(c) c.3 "trd": six half-spaces with unit normals. */
+    real dx1 = s->trd[0], dx2 = s->trd[1], dy1 = s->trd[2], dy2 = s->trd[3], dz = s->trd[4];
+    real fx = (dx2 - dx1) / (2 * dz), mx = (dx1 + dx2) / 2, cx = R_SQRT(1 + fx * fx);
+    real fy = (dy2 - dy1) / (2 * dz), my = (dy1 + dy2) / 2, cy = R_SQRT(1 + fy * fy);
+    real n[6][3] = { { 0, 0, -1 }, { 0, 0, 1 }, { 1 / cx, 0, -fx / cx }, { -1 / cx, 0, -fx / cx },
+                     { 0, 1 / cy, -fy / cy }, { 0, -1 / cy, -fy / cy } };
+    real h[6] = { dz, dz, mx / cx, mx / cx, my / cy, my / cy };
+    memcpy(s->pn, n, sizeof n);
+    memcpy(s->ph, h, sizeof h);
+    /* corners: (+-dx1, +-dy1, -dz), (+-dx2, +-dy2, +dz) */
+    real f[6][4][3] = {
+        { { -dx1, -dy1, -dz }, { dx1, -dy1, -dz }, { dx1, dy1, -dz }, { -dx1, dy1, -dz } },   /* -z */
+        { { -dx2, -dy2, dz }, { dx2, -dy2, dz }, { dx2, dy2, dz }, { -dx2, dy2, dz } },       /* +z */
+        { { dx1, -dy1, -dz }, { dx1, dy1, -dz }, { dx2, dy2, dz }, { dx2, -dy2, dz } },       /* +x */
+        { { -dx1, -dy1, -dz }, { -dx1, dy1, -dz }, { -dx2, dy2, dz }, { -dx2, -dy2, dz } },   /* -x */
+        { { -dx1, dy1, -dz }, { dx1, dy1, -dz }, { dx2, dy2, dz }, { -dx2, dy2, dz } },       /* +y */
+        { { -dx1, -dy1, -dz }, { dx1, -dy1, -dz }, { dx2, -dy2, dz }, { -dx2, -dy2, dz } },   /* -y */
+    };
+    memcpy(s->fv, f, sizeof f);
+}
+
+/* Parameter layouts: SURVEY.md 8(b).  Returns NULL for invalid parameters. */
+orc_shape *orc_shape_create(int kind, const double *par, int np)
+{
+    if (!par || np <= 0 || !finite_all(par, np)) return NULL;
+    orc_shape *s = (orc_shape *)calloc(1, sizeof *s);
+    if (!s) return NULL;
+    s->kind = kind;
+    s->full = 1;
+    int ok = 0;
+    switch (kind) {
+    case ORC_BOX:
+        if (np == 3 && par[0] > 0 && par[1] > 0 && par[2] > 0) {
+            for (int i = 0; i < 3; ++i) s->h[i] = par[i];
+            ok = 1;
+        }
+        break;
+    case ORC_ORB:
+        if (np == 1 && par[0] > 0) { s->r = par[0]; ok = 1; }
+        break;
+    case ORC_TUBE: /* rmin rmax dz sphi dphi : rectangle in (r, z), c.1 */
+        if (np == 5 && par[0] >= 0 && par[1] > par[0] && par[2] > 0 && par[4] > 0) {
+            real rmin = par[0], rmax = par[1], dz = par[2];
+            s->nv = 4;
+            s->pr[0] = rmin; s->pz[0] = -dz;
+            s->pr[1] = rmax; s->pz[1] = -dz;
+            s->pr[2] = rmax; s->pz[2] = dz;
+            s->pr[3] = rmin; s->pz[3] = dz;
+            set_wedge(s, par[3], par[4]);
+            ok = 1;
+        }
+        break;
+    case ORC_CONE: /* rmin1 rmax1 rmin2 rmax2 dz sphi dphi : quadrilateral, c.1 */
+        if (np == 7 && par[0] >= 0 && par[1] > par[0] && par[2] >= 0 && par[3] > par[2] && par[4] > 0 &&
+            par[6] > 0) {
+            real dz = par[4];
+            s->nv = 4;
+            s->pr[0] = par[0]; s->pz[0] = -dz;
+            s->pr[1] = par[1]; s->pz[1] = -dz;
+            s->pr[2] = par[3]; s->pz[2] = dz;
+            s->pr[3] = par[2]; s->pz[3] = dz;
+            set_wedge(s, par[5], par[6]);
+            ok = 1;
+        }
+        break;
+    case ORC_TRD:
+        if (np == 5 && par[0] > 0 && par[1] > 0 && par[2] > 0 && par[3] > 0 && par[4] > 0) {
+            for (int i = 0; i < 5; ++i) s->trd[i] = par[i];
+            trd_setup(s);
+            ok = 1;
+        }
+        break;
+    case ORC_POLYCONE: { /* sphi dphi nz (z rmin rmax)*nz : 2n-gon, c.1; reading R18 */
+        if (np < 3) break;
+        int nz = (int)par[2];
+        if ((double)nz != par[2] || nz < 2 || nz > ORC_MAXZ || np != 3 + 3 * nz || !(par[1] > 0)) break;
+        ok = 1;
+        for (int i = 0; i < nz; ++i) {
+            double z = par[3 + 3 * i], rmin = par[4 + 3 * i], rmax = par[5 + 3 * i];
+            if (rmin < 0 || rmax <= rmin) ok = 0;
+            if (i > 0 && !(z > par[3 + 3 * (i - 1)])) ok = 0;
+            /* (rmin_0,z_0) ... (rmin_{n-1},z_{n-1}), (rmax_{n-1},z_{n-1}) ... (rmax_0,z_0) */
+            s->pr[i] = rmin; s->pz[i] = z;
+            s->pr[2 * nz - 1 - i] = rmax; s->pz[2 * nz - 1 - i] = z;
+        }
+        s->nv = 2 * nz;
+        set_wedge(s, par[0], par[1]);
+        break;
+    }
+    default:
+        break;
+    }
+    if (!ok) { free(s); return NULL; }
+    return s;
+}
+
+void orc_shape_destroy(orc_shape *s) { free(s); }
+
+/* -------------------------------------------- RZ polygon + phi wedge (c.3) */
+
+static int edge_on_axis(const orc_shape *s, int i)
+{
+    int j = (i + 1) % s->nv;
+    return s->pr[i] == 0 && s->pr[j] == 0;
+}
+
+/* even-odd point-in-polygon in the (r, z) half plane */
+static int in_poly(const orc_shape *s, real u, real v)
+{
+    int in = 0;
+    for (int i = 0; i < s->nv; ++i) {
+        int j = (i + 1) % s->nv;
+        real ri = s->pr[i], zi = s->pz[i], rj = s->pr[j], zj = s->pz[j];
+        if ((zi > v) != (zj > v)) {
+            real ucross = ri + (v - zi) * (rj - ri) / (zj - zi);
+            if (u < ucross) in = !in;
+        }
+    }
+    return in;
+}
+
+static real seg_d2(real u, real v, real r0, real z0, real r1, real z1)
+{
+    real eu = r1 - r0, ev = z1 - z0, wu = u - r0, wv = v - z0;
+    real L2 = eu * eu + ev * ev;
+    real t = L2 > 0 ? (wu * eu + wv * ev) / L2 : 0;
+    if (t < 0) t = 0;
+    if (t > 1) t = 1;
+    real du = wu - t * eu, dv = wv - t * ev;
+    return du * du + dv * dv;
+}
+
+/* min squared distance to the polygon edges; axis edges are not a surface */
+static real poly_d2(const orc_shape *s, real u, real v, int skip_axis)
+{
+    real best = ORC_INF;
+    for (int i = 0; i < s->nv; ++i) {
+        if (skip_axis && edge_on_axis(s, i)) continue;
+        int j = (i + 1) % s->nv;
+        best = rmin2(best, seg_d2(u, v, s->pr[i], s->pz[i], s->pr[j], s->pz[j]));
+    }
+    return best;
+}
+
+static int in_phi(const orc_shape *s, real x, real y)
+{
+    if (s->full) return 1;
+    real phi = R_ATAN2(y, x);
+    real d = R_FMOD(phi - s->sphi, 2 * R_PI);
+    if (d < 0) d += 2 * R_PI;
+    return d <= s->dphi;
+}
+
+static real sdf_rz(const orc_shape *s, real x, real y, real z)
+{
+    real rho = R_SQRT(x * x + y * y);
+    int inphi = in_phi(s, x, y);
+    int inside = inphi && in_poly(s, rho, z);
+    real D2 = ORC_INF;
+    if (inphi) D2 = poly_d2(s, rho, z, 1);
+    if (!s->full) {
+        for (int k = 0; k < 2; ++k) {
+            real ex = s->e[k][0], ey = s->e[k][1];
+            real u = x * ex + y * ey;
+            real w = -x * ey + y * ex;
+            real dF2 = in_poly(s, u, z) ? 0 : poly_d2(s, u, z, 0);
+            D2 = rmin2(D2, w * w + dF2);
+        }
+    }
+    real D = R_SQRT(D2);
+    return inside ? -D : D;
+}
+
+/* --------------------------------------------------------------- trd (c.3) */
+
+static real seg3_d2(const real p[3], const real a[3], const real b[3])
+{
+    real e[3], w[3], L2 = 0, we = 0;
+    for (int i = 0; i < 3; ++i) { e[i] = b[i] - a[i]; w[i] = p[i] - a[i]; L2 += e[i] * e[i]; we += w[i] * e[i]; }
+    real t = L2 > 0 ? we / L2 : 0;
+    if (t < 0) t = 0;
+    if (t > 1) t = 1;
+    real d2 = 0;
+    for (int i = 0; i < 3; ++i) { real d = w[i] - t * e[i]; d2 += d * d; }
+    return d2;
+}
+
+/* exact distance from p to a planar convex quad (corners q[0..3] in order, unit normal n, offset h) */
+static real quad_dist(const real p[3], const real q[4][3], const real n[3], real h)
+{
+    real dist = n[0] * p[0] + n[1] * p[1] + n[2] * p[2] - h;
+    real f[3] = { p[0] - dist * n[0], p[1] - dist * n[1], p[2] - dist * n[2] };
+    /* foot inside the quad <=> same side of all four edges */
+    int pos = 0, neg = 0;
+    for (int i = 0; i < 4; ++i) {
+        int j = (i + 1) & 3;
+        real e[3] = { q[j][0] - q[i][0], q[j][1] - q[i][1], q[j][2] - q[i][2] };
+        real w[3] = { f[0] - q[i][0], f[1] - q[i][1], f[2] - q[i][2] };
+        real c[3] = { e[1] * w[2] - e[2] * w[1], e[2] * w[0] - e[0] * w[2], e[0] * w[1] - e[1] * w[0] };
+        real sgn = c[0] * n[0] + c[1] * n[1] + c[2] * n[2];
+        if (sgn > 0) pos++;
+        if (sgn < 0) neg++;
+    }
+    if (pos == 0 || neg == 0) return R_FABS(dist);
+    real best = ORC_INF;
+    for (int i = 0; i < 4; ++i) best = rmin2(best, seg3_d2(p, q[i], q[(i + 1) & 3]));
+    return R_SQRT(best);
+}
+
+static real sdf_trd(const orc_shape *s, real x, real y, real z)
+{
+    real p[3] = { x, y, z };
+    real g = -ORC_INF;
+    for (int j = 0; j < 6; ++j)
+        g = rmax2(g, s->pn[j][0] * x + s->pn[j][1] * y + s->pn[j][2] * z - s->ph[j]);
+    if (g <= 0) return g; /* exact inside a convex polyhedron */
+    real best = ORC_INF;
+    for (int j = 0; j < 6; ++j) best = rmin2(best, quad_dist(p, s->fv[j], s->pn[j], s->ph[j]));
+    return best;
+}
+
+/* -------------------------------------------------------------- sdf (c.3) */
+
+static real sdf(const orc_shape *s, real x, real y, real z)
+{
+    switch (s->kind) {
+    case ORC_BOX: {
+        real qx = R_FABS(x) - s->h[0], qy = R_FABS(y) - s->h[1], qz = R_FABS(z) - s->h[2];
+        real ax = rmax2(qx, 0), ay = rmax2(qy, 0), az = rmax2(qz, 0);
+        return R_SQRT(ax * ax + ay * ay + az * az) + rmin2(rmax2(qx, rmax2(qy, qz)), 0);
+    }
+    case ORC_ORB:
+        return R_SQRT(x * x + y * y + z * z) - s->r;
+    case ORC_TRD:
+        return sdf_trd(s, x, y, z);
+    default:
+        return sdf_rz(s, x, y, z);
+    }
+}
+
+/* c.2: Inside */
+static int inside(const orc_shape *s, real x, real y, real z)
+{
+    real d = sdf(s, x, y, z);
+    if (d < -ORC_KTOL) return ORC_INSIDE;
+    if (d > ORC_KTOL) return ORC_OUTSIDE;
+    return ORC_SURFACE;
+}
+
+/* ------------------------------------------------- first crossing (c.4) */
+
+/* a t^2 + 2 b t + c = 0; D = b^2 - a c; D <= 0 => no crossing (reading R8) */
+static int quad_roots(real a, real b, real c, real t[2])
+{
+    real D = b * b - a * c;
+    if (!(D > 0)) return 0;
+    real sq = R_SQRT(D);
+    real q = (b >= 0) ? -(b + sq) : -(b - sq); /* sgn(0) = +1, reading R9 */
+    int n = 0;
+    if (a != 0) t[n++] = q / a;
+    if (q != 0) t[n++] = c / q;
+    return n;
+}
+
+static real cross_box(const orc_shape *s, int is_inside, const real p[3], const real d[3])
+{
+    real tin = -ORC_INF, tout = ORC_INF;
+    for (int i = 0; i < 3; ++i) {
+        real h = s->h[i];
+        if (d[i] != 0) {
+            real sg = d[i] > 0 ? 1 : -1;
+            real t1 = (-sg * h - p[i]) / d[i];
+            real t2 = (sg * h - p[i]) / d[i];
+            tin = rmax2(tin, t1);
+            tout = rmin2(tout, t2);
+        } else if (R_FABS(p[i]) >= h) {
+            return ORC_INF;
+        }
+    }
+    if (is_inside) return tout;
+    return (tin < tout && tout > 0) ? tin : ORC_INF;
+}
+
+static real cross_convex(const orc_shape *s, int is_inside, const real p[3], const real d[3])
+{
+    real tin = -ORC_INF, tout = ORC_INF;
+    for (int j = 0; j < 6; ++j) {
+        real num = s->ph[j] - (s->pn[j][0] * p[0] + s->pn[j][1] * p[1] + s->pn[j][2] * p[2]);
+        real den = s->pn[j][0] * d[0] + s->pn[j][1] * d[1] + s->pn[j][2] * d[2];
+        if (den > 0) tout = rmin2(tout, num / den);
+        else if (den < 0) tin = rmax2(tin, num / den);
+        else if (num < 0) return ORC_INF;
+    }
+    if (is_inside) return tout;
+    return (tin < tout && tout > 0) ? tin : ORC_INF;
+}
+
+static real cross_orb(const orc_shape *s, const real p[3], const real d[3])
+{
+    real t[2], best = ORC_INF;
+    real b = p[0] * d[0] + p[1] * d[1] + p[2] * d[2];
+    real c = p[0] * p[0] + p[1] * p[1] + p[2] * p[2] - s->r * s->r;
+    int n = quad_roots(1, b, c, t);
+    for (int i = 0; i < n; ++i)
+        if (t[i] > 0) best = rmin2(best, t[i]);
+    return best;
+}
+
+static real cross_rz(const orc_shape *s, const real p[3], const real d[3])
+{
+    real best = ORC_INF;
+    real x = p[0], y = p[1], z = p[2], dx = d[0], dy = d[1], dz = d[2];
+    for (int i = 0; i < s->nv; ++i) {
+        if (edge_on_axis(s, i)) continue;
+        int j = (i + 1) % s->nv;
+        real r0 = s->pr[i], z0 = s->pz[i], r1 = s->pr[j], z1 = s->pz[j];
+        if (z0 != z1) { /* frustum (cylinder if r0 == r1) */
+            real B = (r1 - r0) / (z1 - z0), A = r0 - B * z0, k = A + B * z;
+            real a = dx * dx + dy * dy - B * B * dz * dz;
+            real b = x * dx + y * dy - B * dz * k;
+            real c = x * x + y * y - k * k;
+            real t[2];
+            int n = quad_roots(a, b, c, t);
+            for (int m = 0; m < n; ++m) {
+                if (!(t[m] > 0)) continue;
+                real zh = z + t[m] * dz;
+                if (zh < rmin2(z0, z1) || zh > rmax2(z0, z1)) continue;
+                if (!in_phi(s, x + t[m] * dx, y + t[m] * dy)) continue;
+                best = rmin2(best, t[m]);
+            }
+        } else if (dz != 0) { /* cap annulus */
+            real t = (z0 - z) / dz;
+            if (!(t > 0)) continue;
+            real hx = x + t * dx, hy = y + t * dy, rh2 = hx * hx + hy * hy;
+            real rlo = rmin2(r0, r1), rhi = rmax2(r0, r1);
+            if (rh2 < rlo * rlo || rh2 > rhi * rhi) continue;
+            if (!in_phi(s, hx, hy)) continue;
+            best = rmin2(best, t);
+        }
+    }
+    if (!s->full) {
+        for (int k = 0; k < 2; ++k) {
+            real ex = s->e[k][0], ey = s->e[k][1];
+            real nx = -ey, ny = ex;
+            real nd = nx * dx + ny * dy;
+            if (nd == 0) continue;
+            real t = -(nx * x + ny * y) / nd;
+            if (!(t > 0)) continue;
+            real hx = x + t * dx, hy = y + t * dy;
+            if (!in_poly(s, ex * hx + ey * hy, z + t * dz)) continue;
+            best = rmin2(best, t);
+        }
+    }
+    return best;
+}
+
+static real cross(const orc_shape *s, int is_inside, const real p[3], const real d[3])
+{
+    switch (s->kind) {
+    case ORC_BOX: return cross_box(s, is_inside, p, d);
+    case ORC_ORB: return cross_orb(s, p, d);
+    case ORC_TRD: return cross_convex(s, is_inside, p, d);
+    default: return cross_rz(s, p, d);
+    }
+}
+
+/* c.2: DistanceToIn / DistanceToOut (readings R4, R5) */
+static real distance_to_in(const orc_shape *s, const real p[3], const real d[3], real step_max)
+{
+    if (inside(s, p[0], p[1], p[2]) == ORC_INSIDE) return -1;
+    real t = cross(s, 0, p, d);
+    return t <= step_max ? t : ORC_INF;
+}
+
+static real distance_to_out(const orc_shape *s, const real p[3], const real d[3], real step_max)
+{
+    if (inside(s, p[0], p[1], p[2]) == ORC_OUTSIDE) return -1;
+    real t = cross(s, 1, p, d);
+    return t <= step_max ? t : ORC_INF;
+}
+
+/* ------------------------------------------------------------ batch entry */
+
+double orc_ktol(void) { return 1e-9; }
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+void orc_sdf(const orc_shape *s, const double *x, const double *y, const double *z, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) out[i] = (double)sdf(s, x[i], y[i], z[i]);
+}
+
+void orc_inside(const orc_shape *s, const double *x, const double *y, const double *z, int64_t n, int32_t *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) out[i] = inside(s, x[i], y[i], z[i]);
+}
+
+/* c.2: SafetyToIn = +sdf, SafetyToOut = -sdf; exact and signed (readings R2, R3) */
+void orc_safety_to_in(const orc_shape *s, const double *x, const double *y, const double *z, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) out[i] = (double)sdf(s, x[i], y[i], z[i]);
+}
+
+void orc_safety_to_out(const orc_shape *s, const double *x, const double *y, const double *z, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) out[i] = (double)(-sdf(s, x[i], y[i], z[i]));
+}
+
+void orc_distance_to_in(const orc_shape *s, const double *x, const double *y, const double *z, const double *dx,
+                        const double *dy, const double *dz, double step_max, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] };
+        out[i] = (double)distance_to_in(s, p, d, step_max);
+    }
+}
+
+void orc_distance_to_out(const orc_shape *s, const double *x, const double *y, const double *z, const double *dx,
+                         const double *dy, const double *dz, double step_max, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] };
+        out[i] = (double)distance_to_out(s, p, d, step_max);
+    }
+}
+
+/* the raw first crossing Cross(p, d) of c.2, exposed for the pins */
+void orc_cross(const orc_shape *s, const double *x, const double *y, const double *z, const double *dx,
+               const double *dy, const double *dz, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] };
+        int in = inside(s, p[0], p[1], p[2]) != ORC_OUTSIDE;
+        out[i] = (double)cross(s, in, p, d);
+    }
+}
+
+/* ---------------------------------------------------------- navigation */
+
+orc_volume *orc_volume_create(const orc_shape *mother, int nd, const orc_shape *const *daughters, const double *xf)
+{
+    if (!mother || nd < 0 || (nd > 0 && (!daughters || !xf))) return NULL;
+    orc_volume *v = (orc_volume *)calloc(1, sizeof *v);
+    if (!v) return NULL;
+    v->mother = mother;
+    v->nd = nd;
+    v->daughter = (const orc_shape **)calloc((size_t)(nd > 0 ? nd : 1), sizeof *v->daughter);
+    v->xf = (real *)calloc((size_t)(nd > 0 ? nd : 1) * 12, sizeof *v->xf);
+    for (int i = 0; i < nd; ++i) {
+        v->daughter[i] = daughters[i];
+        for (int k = 0; k < 12; ++k) v->xf[12 * i + k] = xf[12 * i + k];
+    }
+    return v;
+}
+
+void orc_volume_destroy(orc_volume *v)
+{
+    if (!v) return;
+    free((void *)v->daughter);
+    free(v->xf);
+    free(v);
+}
+
+static void to_local(const real *m, const real p[3], const real d[3], real pl[3], real dl[3])
+{
+    /* reading R12: p_loc = R p + b, d_loc = R d, row-major [R | b] */
+    for (int r = 0; r < 3; ++r) {
+        pl[r] = m[4 * r + 0] * p[0] + m[4 * r + 1] * p[1] + m[4 * r + 2] * p[2] + m[4 * r + 3];
+        dl[r] = m[4 * r + 0] * d[0] + m[4 * r + 1] * d[1] + m[4 * r + 2] * d[2];
+    }
+}
+
+/* c.2 ComputeStep; tie-break reading R13; (stepMax, -2) when the physics step wins */
+void orc_compute_step(const orc_volume *v, const double *x, const double *y, const double *z, const double *dx,
+                      const double *dy, const double *dz, double step_max, int64_t n, double *step, int32_t *hit)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] };
+        real best = distance_to_out(v->mother, p, d, ORC_INF);
+        int32_t who = -1;
+        for (int k = 0; k < v->nd; ++k) {
+            real pl[3], dl[3];
+            to_local(v->xf + 12 * k, p, d, pl, dl);
+            real t = distance_to_in(v->daughter[k], pl, dl, ORC_INF);
+            if (t >= 0 && t < best) { best = t; who = k; }
+        }
+        if (best > step_max) { best = step_max; who = -2; }
+        step[i] = (double)best;
+        hit[i] = who;
+    }
+}
+
+/*
+ * Isotropic safety of the navigation state (widening of PAPER.md:113 to the
+ * placed-volume level): min( SafetyToOut_mother(p), min_i SafetyToIn_i(R_i p + b_i) ).
+ * Positive for a point inside the mother and outside every daughter.
+ */
+void orc_volume_safety(const orc_volume *v, const double *x, const double *y, const double *z, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d0[3] = { 0, 0, 0 };
+        real best = -sdf(v->mother, p[0], p[1], p[2]);
+        for (int k = 0; k < v->nd; ++k) {
+            real pl[3], dl[3];
+            to_local(v->xf + 12 * k, p, d0, pl, dl);
+            best = rmin2(best, sdf(v->daughter[k], pl[0], pl[1], pl[2]));
+        }
+        out[i] = (double)best;
+    }
+}

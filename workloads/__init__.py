@@ -1,0 +1,209 @@
+"""Seeded synthetic workloads: the five configurations of BASELINE.json (`configs[0..4]`).
+
+This module serves BOTH the oracle tests and the CUDA path (tests, bench.py, smoke) and holds
+none of the method's arithmetic: it only draws numbers (numpy Philox) and lays out parameters.
+The one geometric decision the recipe needs -- rejecting points that lie in the 1e-6 surface
+band (BASELINE.json configs[0]) -- is taken by a callback the caller
+supplies (`band(x, y, z) -> bool mask of points to redraw`), so that the oracle legs reject with
+the oracle's sdf and the product legs with the library's own safety query.
+
+Recipe (SURVEY.md sec. 8(d) "Generator"; the paper's workload is "randomly placed particles with
+random speed"): points c + (2u-1) h per axis in the sampling box, directions
+dz = 2u1-1, phi = 2 pi u2, d = (sqrt(1-dz^2) cos phi, sqrt(1-dz^2) sin phi, dz), renormalised once.
+"""
+import math
+
+import numpy as np
+
+# shape kinds: the enumeration of include/vg.h (and, independently, of the oracle)
+BOX, ORB, TUBE, CONE, TRD, POLYCONE = range(6)
+KIND_NAME = {BOX: "box", ORB: "orb", TUBE: "tube", CONE: "cone", TRD: "trd", POLYCONE: "polycone"}
+
+BASE_SEED = 1512066370          # + k for config k, + 100 * shape_index for a second shape of the config
+SURFACE_BAND = 1e-6             # generators keep |sdf| >= 1e-6 (BASELINE.json configs[0], R17)
+STEP_MAX = 1e30                 # BASELINE.json configs[0], [4]
+TWO_PI = 2.0 * math.pi
+
+QUERIES5 = ("inside", "distance_to_in", "distance_to_out", "safety_to_in", "safety_to_out")
+
+
+def config_seed(k, shape_index=0):
+    return BASE_SEED + k + 100 * shape_index
+
+
+def _rng(seed):
+    return np.random.Generator(np.random.Philox(int(seed)))
+
+
+def draw_tracks(seed, n, center, half, band=None, max_rounds=64):
+    """n tracks as six float64 arrays (x, y, z, dx, dy, dz).
+
+    `band(x, y, z)` returns True for points to be redrawn (inside the surface band, or outside the
+    region the config allows); redraws come from the continuing stream until none remain.
+    """
+    rng = _rng(seed)
+    n = int(n)
+    c = np.asarray(center, dtype=np.float64)
+    h = np.asarray(half, dtype=np.float64)
+    u = rng.random((n, 3))
+    p = c + (2.0 * u - 1.0) * h
+    v = rng.random((n, 2))
+    dz = 2.0 * v[:, 0] - 1.0
+    phi = TWO_PI * v[:, 1]
+    s = np.sqrt(np.maximum(0.0, 1.0 - dz * dz))
+    dx = s * np.cos(phi)
+    dy = s * np.sin(phi)
+    norm = np.sqrt(dx * dx + dy * dy + dz * dz)
+    dx, dy, dz = dx / norm, dy / norm, dz / norm
+    x, y, z = (np.ascontiguousarray(p[:, i]) for i in range(3))
+    if band is not None and n > 0:
+        bad = np.flatnonzero(np.asarray(band(x, y, z), dtype=bool))
+        rounds = 0
+        while bad.size:
+            rounds += 1
+            if rounds > max_rounds:
+                raise RuntimeError("draw_tracks: rejection did not terminate")
+            q = c + (2.0 * rng.random((bad.size, 3)) - 1.0) * h
+            x[bad], y[bad], z[bad] = q[:, 0], q[:, 1], q[:, 2]
+            still = np.asarray(band(x[bad], y[bad], z[bad]), dtype=bool)
+            bad = bad[still]
+    return x, y, z, np.ascontiguousarray(dx), np.ascontiguousarray(dy), np.ascontiguousarray(dz)
+
+
+# --------------------------------------------------------------------------- shapes of the configs
+
+def bounding_half(kind, params):
+    """Centre and half-extent of the axis-aligned box of the FULL-phi solid (reading R16)."""
+    p = list(params)
+    if kind == BOX:
+        return (0.0, 0.0, 0.0), (p[0], p[1], p[2])
+    if kind == ORB:
+        return (0.0, 0.0, 0.0), (p[0], p[0], p[0])
+    if kind == TUBE:
+        return (0.0, 0.0, 0.0), (p[1], p[1], p[2])
+    if kind == CONE:
+        r = max(p[1], p[3])
+        return (0.0, 0.0, 0.0), (r, r, p[4])
+    if kind == TRD:
+        return (0.0, 0.0, 0.0), (max(p[0], p[1]), max(p[2], p[3]), p[4])
+    if kind == POLYCONE:
+        nz = int(p[2])
+        zs = [p[3 + 3 * i] for i in range(nz)]
+        r = max(p[5 + 3 * i] for i in range(nz))
+        return (0.0, 0.0, 0.5 * (zs[0] + zs[-1])), (r, r, 0.5 * (zs[-1] - zs[0]))
+    raise ValueError(kind)
+
+
+def polycone_params(seed, nz=10):
+    """configs[3]: z uniform-sorted in [-50,50], rmin uniform [0,5], rmax uniform [10,30], full phi."""
+    rng = _rng(seed + 7)
+    z = np.sort(rng.uniform(-50.0, 50.0, nz))
+    rmin = rng.uniform(0.0, 5.0, nz)
+    rmax = rng.uniform(10.0, 30.0, nz)
+    out = [0.0, TWO_PI, float(nz)]
+    for i in range(nz):
+        out += [float(z[i]), float(rmin[i]), float(rmax[i])]
+    return out
+
+
+class ShapeCase:
+    """One (shape, sampling box, seed) of a config."""
+
+    def __init__(self, cfg, name, kind, params, center, half, seed, sizes, queries):
+        self.cfg, self.name, self.kind = cfg, name, kind
+        self.params = [float(v) for v in params]
+        self.center, self.half = tuple(center), tuple(half)
+        self.seed, self.sizes, self.queries = seed, tuple(sizes), tuple(queries)
+
+    def tracks(self, n=None, band=None):
+        return draw_tracks(self.seed, self.sizes[-1] if n is None else n, self.center, self.half, band)
+
+
+def _scaled(kind, params, scale=1.5):
+    c, h = bounding_half(kind, params)
+    return c, tuple(scale * v for v in h)
+
+
+def shape_cases(k):
+    """The ShapeCase list of BASELINE.json configs[k], k = 0..3 (config 4 is `navigator_case`)."""
+    if k == 0:
+        par = [5.0, 5.0, 5.0]
+        return [ShapeCase(0, "box", BOX, par, (0, 0, 0), (10, 10, 10), config_seed(0), [65536], QUERIES5)]
+    if k == 1:
+        par = [5.0, 10.0, 15.0, 0.0, 4.0 * math.pi / 3.0]
+        c, h = _scaled(TUBE, par)
+        return [ShapeCase(1, "tube", TUBE, par, c, h, config_seed(1), [1048576], QUERIES5)]
+    if k == 2:
+        cone = [2.0, 6.0, 4.0, 12.0, 20.0, 0.0, TWO_PI]
+        trd = [5.0, 10.0, 7.0, 3.0, 15.0]
+        c0, h0 = _scaled(CONE, cone)
+        c1, h1 = _scaled(TRD, trd)
+        return [ShapeCase(2, "cone", CONE, cone, c0, h0, config_seed(2, 0), [4194304], QUERIES5),
+                ShapeCase(2, "trd", TRD, trd, c1, h1, config_seed(2, 1), [4194304], QUERIES5)]
+    if k == 3:
+        sizes = [2 ** 10, 2 ** 14, 2 ** 18, 2 ** 22, 2 ** 24]
+        pc = polycone_params(config_seed(3, 0))
+        orb = [20.0]
+        c0, h0 = _scaled(POLYCONE, pc)
+        c1, h1 = _scaled(ORB, orb)
+        q = ("distance_to_in", "safety_to_in")
+        return [ShapeCase(3, "polycone", POLYCONE, pc, c0, h0, config_seed(3, 0), sizes, q),
+                ShapeCase(3, "orb", ORB, orb, c1, h1, config_seed(3, 1), sizes, q)]
+    raise ValueError("config %r has no shape cases" % (k,))
+
+
+# ------------------------------------------------------------------------------ navigator (configs[4])
+
+def quaternion_to_matrix(q):
+    """Rotation matrix (local -> mother) of a unit quaternion (x, y, z, w)."""
+    x, y, z, w = q
+    return np.array([[1 - 2 * (y * y + z * z), 2 * (x * y - z * w), 2 * (x * z + y * w)],
+                     [2 * (x * y + z * w), 1 - 2 * (x * x + z * z), 2 * (y * z - x * w)],
+                     [2 * (x * z - y * w), 2 * (y * z + x * w), 1 - 2 * (x * x + y * y)]], dtype=np.float64)
+
+
+def placement(Q, c):
+    """3x4 row-major mother -> local transform [R | b] of a daughter centred at c with local -> mother
+    rotation Q: R = Q^T, b = -Q^T c (reading R12)."""
+    R = np.asarray(Q, dtype=np.float64).T
+    b = -R @ np.asarray(c, dtype=np.float64)
+    return np.concatenate([R, b[:, None]], axis=1).reshape(12)
+
+
+class NavigatorCase:
+    """configs[4]: mother box (100,100,100), 64 daughters on a 4x4x4 grid (readings R14, R15)."""
+
+    def __init__(self, seed=None, n=4194304, grid=4, pitch=50.0, mother_half=100.0, dhalf=8.0):
+        self.cfg = 4
+        self.seed = config_seed(4) if seed is None else seed
+        self.sizes = (n,)
+        self.mother_kind, self.mother_params = BOX, [mother_half] * 3
+        self.center, self.half = (0.0, 0.0, 0.0), (mother_half,) * 3
+        rng = _rng(self.seed + 7)
+        kinds, params, xf, centers = [], [], [], []
+        off = 0.5 * (grid - 1) * pitch
+        for iz in range(grid):
+            for iy in range(grid):
+                for ix in range(grid):
+                    c = (ix * pitch - off, iy * pitch - off, iz * pitch - off)
+                    u1, u2, u3 = rng.random(3)
+                    q = (math.sqrt(1 - u1) * math.sin(TWO_PI * u2), math.sqrt(1 - u1) * math.cos(TWO_PI * u2),
+                         math.sqrt(u1) * math.sin(TWO_PI * u3), math.sqrt(u1) * math.cos(TWO_PI * u3))
+                    if (ix + iy + iz) % 2 == 0:
+                        kinds.append(BOX)
+                        params.append([dhalf, dhalf, dhalf])
+                    else:
+                        kinds.append(TUBE)
+                        params.append([0.0, dhalf, dhalf, 0.0, TWO_PI])
+                    xf.append(placement(quaternion_to_matrix(q), c))
+                    centers.append(c)
+        self.daughter_kinds, self.daughter_params = kinds, params
+        self.xforms = np.ascontiguousarray(np.stack(xf))
+        self.centers = np.asarray(centers)
+
+    def tracks(self, n=None, band=None):
+        return draw_tracks(self.seed, self.sizes[-1] if n is None else n, self.center, self.half, band)
+
+
+def navigator_case(**kw):
+    return NavigatorCase(**kw)
