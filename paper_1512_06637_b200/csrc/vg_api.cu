@@ -1,0 +1,439 @@
+// vg_api.cu -- the C ABI of include/vg.h: handle registry, parameter validation, derived constants
+// (SURVEY.md sec. 8(a) A0, sec. 8(b)), argument checks and kernel dispatch.  Host code only; every step of the
+// path runs in the kernels of vg_k_*.cu / vg_nav.cu.
+#include "../../include/vg.h"
+#include "vg_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace vg;
+
+struct vg_shape {
+    int kind;
+    union {
+        BoxP box;
+        OrbP orb;
+        TubeP tube;
+        ConeP cone;
+        TrdP trd;
+        PolyconeP pcon;
+    } u;
+};
+
+struct vg_volume {
+    SolidU mother;
+    int nd;
+    Daughter *table_dev;
+};
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+static int fail_cuda(cudaError_t e, const char *what)
+{
+    return fail(VG_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+extern "C" const char *vg_last_error(void) { return g_err; }
+
+// ------------------------------------------------------------------------------------------- derived constants
+
+static const double kTwoPi = 2.0 * 3.14159265358979323846;
+
+static Wedge make_wedge(double sphi, double dphi)
+{
+    Wedge w;
+    w.full = dphi >= kTwoPi;
+    w.wide = dphi > 0.5 * kTwoPi;
+    w.e0x = std::cos(sphi);
+    w.e0y = std::sin(sphi);
+    w.e1x = std::cos(sphi + dphi);
+    w.e1y = std::sin(sphi + dphi);
+    return w;
+}
+
+static Frustum make_frustum(double z0, double r0, double z1, double r1)
+{
+    Frustum f;
+    f.B = (r1 - r0) / (z1 - z0);
+    f.A = r0 - f.B * z0;
+    f.sec = std::sqrt(1.0 + f.B * f.B);
+    f.r0 = r0;
+    f.er = r1 - r0;
+    f.inv_l2 = 1.0 / (f.er * f.er + (z1 - z0) * (z1 - z0));
+    return f;
+}
+
+static bool all_finite(const double *p, int n)
+{
+    for (int i = 0; i < n; ++i)
+        if (!std::isfinite(p[i])) return false;
+    return true;
+}
+
+static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
+{
+    s->kind = kind;
+    switch (kind) {
+    case VG_BOX:
+        if (np != 3) return fail(VG_ERR_PARAM, "box: 3 parameters expected, got %d", np);
+        if (!(p[0] > 0 && p[1] > 0 && p[2] > 0)) return fail(VG_ERR_PARAM, "box: half-lengths must be > 0");
+        s->u.box = BoxP{ p[0], p[1], p[2] };
+        return VG_OK;
+    case VG_ORB:
+        if (np != 1) return fail(VG_ERR_PARAM, "orb: 1 parameter expected, got %d", np);
+        if (!(p[0] > 0)) return fail(VG_ERR_PARAM, "orb: r must be > 0");
+        s->u.orb.r = p[0];
+        s->u.orb.r2 = p[0] * p[0];
+        s->u.orb.rin2 = p[0] > kTol ? (p[0] - kTol) * (p[0] - kTol) : 0.0;
+        s->u.orb.rout2 = (p[0] + kTol) * (p[0] + kTol);
+        return VG_OK;
+    case VG_TUBE: {
+        if (np != 5) return fail(VG_ERR_PARAM, "tube: 5 parameters expected, got %d", np);
+        double rmin = p[0], rmax = p[1], dz = p[2];
+        if (!(rmin >= 0 && rmax > rmin && dz > 0 && p[4] > 0))
+            return fail(VG_ERR_PARAM, "tube: need 0 <= rmin < rmax, dz > 0, dphi > 0");
+        TubeP &t = s->u.tube;
+        t.rmin = rmin;
+        t.rmax = rmax;
+        t.dz = dz;
+        t.rmin2 = rmin * rmin;
+        t.rmax2 = rmax * rmax;
+        t.rmin_in2 = (rmin + kTol) * (rmin + kTol);
+        t.rmax_in2 = (rmax - kTol) * (rmax - kTol);
+        t.rmin_out2 = rmin > kTol ? (rmin - kTol) * (rmin - kTol) : 0.0;
+        t.rmax_out2 = (rmax + kTol) * (rmax + kTol);
+        t.w = make_wedge(p[3], p[4]);
+        t.hollow = rmin > 0;
+        return VG_OK;
+    }
+    case VG_CONE: {
+        if (np != 7) return fail(VG_ERR_PARAM, "cone: 7 parameters expected, got %d", np);
+        double rmin1 = p[0], rmax1 = p[1], rmin2 = p[2], rmax2 = p[3], dz = p[4];
+        if (!(rmin1 >= 0 && rmax1 > rmin1 && rmin2 >= 0 && rmax2 > rmin2 && dz > 0 && p[6] > 0))
+            return fail(VG_ERR_PARAM, "cone: need 0 <= rmin < rmax at both ends, dz > 0, dphi > 0");
+        ConeP &c = s->u.cone;
+        c.dz = dz;
+        c.out = make_frustum(-dz, rmax1, dz, rmax2);
+        c.in = make_frustum(-dz, rmin1, dz, rmin2);
+        c.rmin1 = rmin1;
+        c.rmax1 = rmax1;
+        c.rmin2 = rmin2;
+        c.rmax2 = rmax2;
+        c.w = make_wedge(p[5], p[6]);
+        c.hollow = rmin1 > 0 || rmin2 > 0;
+        return VG_OK;
+    }
+    case VG_TRD: {
+        if (np != 5) return fail(VG_ERR_PARAM, "trd: 5 parameters expected, got %d", np);
+        for (int i = 0; i < 5; ++i)
+            if (!(p[i] > 0)) return fail(VG_ERR_PARAM, "trd: half-lengths must be > 0");
+        TrdP &t = s->u.trd;
+        t.dx1 = p[0];
+        t.dx2 = p[1];
+        t.dy1 = p[2];
+        t.dy2 = p[3];
+        t.dz = p[4];
+        t.fx = (t.dx2 - t.dx1) / (2 * t.dz);
+        t.mx = (t.dx1 + t.dx2) / 2;
+        t.cx = std::sqrt(1 + t.fx * t.fx);
+        t.icx = 1 / t.cx;
+        t.fy = (t.dy2 - t.dy1) / (2 * t.dz);
+        t.my = (t.dy1 + t.dy2) / 2;
+        t.cy = std::sqrt(1 + t.fy * t.fy);
+        t.icy = 1 / t.cy;
+        // slanted edge of the +x face: half-widths dy1 -> dy2 over the slant height 2 dz cx; likewise +y
+        t.inv_kx = 1 / ((t.dy2 - t.dy1) * (t.dy2 - t.dy1) + 4 * t.dz * t.dz * t.cx * t.cx);
+        t.inv_ky = 1 / ((t.dx2 - t.dx1) * (t.dx2 - t.dx1) + 4 * t.dz * t.dz * t.cy * t.cy);
+        return VG_OK;
+    }
+    case VG_POLYCONE: {
+        if (np < 3) return fail(VG_ERR_PARAM, "polycone: at least 3 parameters expected");
+        int nz = int(p[2]);
+        if (double(nz) != p[2] || nz < 2 || nz > VG_MAX_ZPLANES)
+            return fail(VG_ERR_PARAM, "polycone: nz must be an integer in [2, %d]", VG_MAX_ZPLANES);
+        if (np != 3 + 3 * nz) return fail(VG_ERR_PARAM, "polycone: %d parameters expected, got %d", 3 + 3 * nz, np);
+        if (!(p[1] > 0)) return fail(VG_ERR_PARAM, "polycone: dphi must be > 0");
+        const double *zp = p + 3;
+        for (int i = 0; i < nz; ++i) {
+            if (!(zp[3 * i + 1] >= 0 && zp[3 * i + 2] > zp[3 * i + 1]))
+                return fail(VG_ERR_PARAM, "polycone: need 0 <= rmin < rmax at plane %d", i);
+            if (i > 0 && !(zp[3 * i] > zp[3 * (i - 1)]))
+                return fail(VG_ERR_PARAM, "polycone: z must be strictly increasing (plane %d)", i);
+        }
+        PolyconeP &c = s->u.pcon;
+        std::memset(&c, 0, sizeof c);
+        c.nsec = nz - 1;
+        c.w = make_wedge(p[0], p[1]);
+        c.zlo = zp[0];
+        c.zhi = zp[3 * (nz - 1)];
+        c.cap_lo_rmin = zp[1];
+        c.cap_lo_rmax = zp[2];
+        c.cap_hi_rmin = zp[3 * (nz - 1) + 1];
+        c.cap_hi_rmax = zp[3 * (nz - 1) + 2];
+        for (int k = 0; k < nz - 1; ++k) {
+            const double *a = zp + 3 * k, *b = zp + 3 * (k + 1);
+            c.sec[k].z0 = a[0];
+            c.sec[k].z1 = b[0];
+            c.sec[k].out = make_frustum(a[0], a[2], b[0], b[2]);
+            c.sec[k].in = make_frustum(a[0], a[1], b[0], b[1]);
+            if (a[1] > 0 || b[1] > 0) c.inner_mask |= 1u << k;
+        }
+        return VG_OK;
+    }
+    }
+    return fail(VG_ERR_PARAM, "unknown shape kind %d", int(kind));
+}
+
+extern "C" int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **out)
+{
+    if (!out) return fail(VG_ERR_ARG, "vg_shape_create: out is NULL");
+    *out = nullptr;
+    if (!params || nparams <= 0) return fail(VG_ERR_ARG, "vg_shape_create: params is NULL or empty");
+    if (!all_finite(params, nparams)) return fail(VG_ERR_PARAM, "vg_shape_create: non-finite parameter");
+    vg_shape *s = new (std::nothrow) vg_shape;
+    if (!s) return fail(VG_ERR_NOMEM, "vg_shape_create: out of host memory");
+    std::memset(s, 0, sizeof *s);
+    int rc = fill_shape(s, kind, params, nparams);
+    if (rc != VG_OK) {
+        delete s;
+        return rc;
+    }
+    *out = s;
+    return VG_OK;
+}
+
+extern "C" void vg_shape_destroy(vg_shape *s) { delete s; }
+
+extern "C" int vg_shape_kind(const vg_shape *s) { return s ? s->kind : fail(VG_ERR_ARG, "vg_shape_kind: NULL"); }
+
+// ------------------------------------------------------------------------------------------------- queries
+
+static bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+static int check_arrays(const char *fn, const void *const *ptrs, int count, size_t out_align, const void *out,
+                        int64_t n, bool *vec)
+{
+    if (n < 0) return fail(VG_ERR_ARG, "%s: n < 0", fn);
+    bool v = true;
+    for (int i = 0; i < count; ++i) {
+        if (!ptrs[i]) return fail(VG_ERR_ARG, "%s: NULL track array", fn);
+        if (!aligned(ptrs[i], 8)) return fail(VG_ERR_ARG, "%s: track array not 8-byte aligned", fn);
+        v = v && aligned(ptrs[i], 16);
+    }
+    if (!out) return fail(VG_ERR_ARG, "%s: NULL output array", fn);
+    if (!aligned(out, out_align)) return fail(VG_ERR_ARG, "%s: output array misaligned", fn);
+    v = v && aligned(out, 2 * out_align);
+    *vec = v;
+    return VG_OK;
+}
+
+static int run_query(const char *fn, int q, const vg_shape *s, const double *x, const double *y, const double *z,
+                     const double *dx, const double *dy, const double *dz, double step_max, int64_t n, void *out,
+                     void *stream)
+{
+    if (!s) return fail(VG_ERR_ARG, "%s: shape is NULL", fn);
+    bool dir = (q == qDistIn || q == qDistOut);
+    const void *ptrs[6] = { x, y, z, dx, dy, dz };
+    bool vec = false;
+    int rc = check_arrays(fn, ptrs, dir ? 6 : 3, q == qInside ? 4 : 8, out, n, &vec);
+    if (rc != VG_OK) return rc;
+    if (dir && !(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
+    if (n == 0) return VG_OK;
+    Tracks t{ x, y, z, dx, dy, dz };
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (s->kind) {
+    case VG_BOX: e = launch_box(q, s->u.box, t, step_max, n, out, vec, st); break;
+    case VG_ORB: e = launch_orb(q, s->u.orb, t, step_max, n, out, vec, st); break;
+    case VG_TUBE: e = launch_tube(q, s->u.tube, t, step_max, n, out, vec, st); break;
+    case VG_CONE: e = launch_cone(q, s->u.cone, t, step_max, n, out, vec, st); break;
+    case VG_TRD: e = launch_trd(q, s->u.trd, t, step_max, n, out, vec, st); break;
+    case VG_POLYCONE: e = launch_polycone(q, s->u.pcon, t, step_max, n, out, vec, st); break;
+    }
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+extern "C" int vg_inside(const vg_shape *s, const double *x, const double *y, const double *z, int64_t n, int32_t *cls,
+                         void *stream)
+{
+    return run_query("vg_inside", qInside, s, x, y, z, nullptr, nullptr, nullptr, 0.0, n, cls, stream);
+}
+
+extern "C" int vg_distance_to_in(const vg_shape *s, const double *x, const double *y, const double *z, const double *dx,
+                                 const double *dy, const double *dz, double step_max, int64_t n, double *dist,
+                                 void *stream)
+{
+    return run_query("vg_distance_to_in", qDistIn, s, x, y, z, dx, dy, dz, step_max, n, dist, stream);
+}
+
+extern "C" int vg_distance_to_out(const vg_shape *s, const double *x, const double *y, const double *z,
+                                  const double *dx, const double *dy, const double *dz, double step_max, int64_t n,
+                                  double *dist, void *stream)
+{
+    return run_query("vg_distance_to_out", qDistOut, s, x, y, z, dx, dy, dz, step_max, n, dist, stream);
+}
+
+extern "C" int vg_safety_to_in(const vg_shape *s, const double *x, const double *y, const double *z, int64_t n,
+                               double *safety, void *stream)
+{
+    return run_query("vg_safety_to_in", qSafeIn, s, x, y, z, nullptr, nullptr, nullptr, 0.0, n, safety, stream);
+}
+
+extern "C" int vg_safety_to_out(const vg_shape *s, const double *x, const double *y, const double *z, int64_t n,
+                                double *safety, void *stream)
+{
+    return run_query("vg_safety_to_out", qSafeOut, s, x, y, z, nullptr, nullptr, nullptr, 0.0, n, safety, stream);
+}
+
+// ---------------------------------------------------------------------------------------------- navigation
+
+static int to_solid(const vg_shape *s, SolidU *o, const char *what)
+{
+    std::memset(o, 0, sizeof *o);
+    o->kind = s->kind;
+    switch (s->kind) {
+    case VG_BOX: o->u.box = s->u.box; return VG_OK;
+    case VG_ORB: o->u.orb = s->u.orb; return VG_OK;
+    case VG_TUBE: o->u.tube = s->u.tube; return VG_OK;
+    case VG_CONE: o->u.cone = s->u.cone; return VG_OK;
+    case VG_TRD: o->u.trd = s->u.trd; return VG_OK;
+    default: return fail(VG_ERR_ARG, "vg_volume_create: a polycone %s is not supported in this build", what);
+    }
+}
+
+extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
+                                vg_volume **out)
+{
+    if (!out) return fail(VG_ERR_ARG, "vg_volume_create: out is NULL");
+    *out = nullptr;
+    if (!mother) return fail(VG_ERR_ARG, "vg_volume_create: mother is NULL");
+    if (nd < 0 || nd > VG_MAX_DAUGHTERS)
+        return fail(VG_ERR_PARAM, "vg_volume_create: ndaughters must be in [0, %d]", VG_MAX_DAUGHTERS);
+    if (nd > 0 && (!daughters || !xforms)) return fail(VG_ERR_ARG, "vg_volume_create: NULL daughters or xforms");
+    vg_volume *v = new (std::nothrow) vg_volume;
+    if (!v) return fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
+    v->nd = nd;
+    v->table_dev = nullptr;
+    int rc = to_solid(mother, &v->mother, "mother");
+    Daughter *host = nullptr;
+    if (rc == VG_OK && nd > 0) {
+        host = new (std::nothrow) Daughter[nd];
+        if (!host) rc = fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
+    }
+    for (int i = 0; rc == VG_OK && i < nd; ++i) {
+        if (!daughters[i]) {
+            rc = fail(VG_ERR_ARG, "vg_volume_create: daughter %d is NULL", i);
+            break;
+        }
+        std::memset(&host[i], 0, sizeof(Daughter));
+        const double *m = xforms + 12 * i;
+        if (!all_finite(m, 12)) {
+            rc = fail(VG_ERR_PARAM, "vg_volume_create: non-finite transform of daughter %d", i);
+            break;
+        }
+        for (int r = 0; r < 3 && rc == VG_OK; ++r)
+            for (int c = 0; c < 3; ++c) {
+                double dot = m[4 * r] * m[4 * c] + m[4 * r + 1] * m[4 * c + 1] + m[4 * r + 2] * m[4 * c + 2];
+                if (std::fabs(dot - (r == c ? 1.0 : 0.0)) > 1e-9) {
+                    rc = fail(VG_ERR_PARAM, "vg_volume_create: rotation of daughter %d is not orthonormal", i);
+                    break;
+                }
+            }
+        if (rc != VG_OK) break;
+        std::memcpy(host[i].m, m, 12 * sizeof(double));
+        rc = to_solid(daughters[i], &host[i].s, "daughter");
+    }
+    if (rc == VG_OK) {
+        size_t bytes = sizeof(Daughter) * size_t(nd > 0 ? nd : 1);
+        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&v->table_dev), bytes);
+        if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMalloc");
+        if (rc == VG_OK && nd > 0) {
+            e = cudaMemcpy(v->table_dev, host, sizeof(Daughter) * size_t(nd), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMemcpy");
+        }
+    }
+    delete[] host;
+    if (rc != VG_OK) {
+        if (v->table_dev) cudaFree(v->table_dev);
+        delete v;
+        return rc;
+    }
+    *out = v;
+    return VG_OK;
+}
+
+extern "C" void vg_volume_destroy(vg_volume *v)
+{
+    if (!v) return;
+    if (v->table_dev) cudaFree(v->table_dev);
+    delete v;
+}
+
+extern "C" int vg_compute_step(const vg_volume *v, const double *x, const double *y, const double *z, const double *dx,
+                               const double *dy, const double *dz, double step_max, int64_t n, double *step,
+                               int32_t *hit, void *stream)
+{
+    const char *fn = "vg_compute_step";
+    if (!v) return fail(VG_ERR_ARG, "%s: volume is NULL", fn);
+    const void *ptrs[6] = { x, y, z, dx, dy, dz };
+    bool vec = false;
+    int rc = check_arrays(fn, ptrs, 6, 8, step, n, &vec);
+    if (rc != VG_OK) return rc;
+    if (!hit || !aligned(hit, 4)) return fail(VG_ERR_ARG, "%s: hit array NULL or misaligned", fn);
+    if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
+    if (n == 0) return VG_OK;
+    Tracks t{ x, y, z, dx, dy, dz };
+    cudaError_t e = launch_compute_step(v->mother, v->table_dev, v->nd, t, step_max, n, step, hit,
+                                        static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const double *y, const double *z, int64_t n,
+                                double *safety, void *stream)
+{
+    const char *fn = "vg_volume_safety";
+    if (!v) return fail(VG_ERR_ARG, "%s: volume is NULL", fn);
+    const void *ptrs[3] = { x, y, z };
+    bool vec = false;
+    int rc = check_arrays(fn, ptrs, 3, 8, safety, n, &vec);
+    if (rc != VG_OK) return rc;
+    if (n == 0) return VG_OK;
+    Tracks t{ x, y, z, nullptr, nullptr, nullptr };
+    cudaError_t e = launch_volume_safety(v->mother, v->table_dev, v->nd, t, n, safety, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+// -------------------------------------------------------------------------------------------------- probes
+
+extern "C" int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *stream)
+{
+    if (!fma_per_s || launches <= 0) return fail(VG_ERR_ARG, "vg_probe_fp64_fma_rate: bad arguments");
+    *fma_per_s = 0.0;
+    cudaError_t e = probe_fp64_fma_rate(launches, fma_per_s, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "vg_probe_fp64_fma_rate");
+    return VG_OK;
+}
+
+extern "C" int vg_probe_empty_launch(int launches, void *stream)
+{
+    if (launches < 0) return fail(VG_ERR_ARG, "vg_probe_empty_launch: launches < 0");
+    cudaError_t e = probe_empty_launch(launches, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "vg_probe_empty_launch");
+    return VG_OK;
+}

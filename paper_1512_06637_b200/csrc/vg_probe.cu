@@ -1,0 +1,66 @@
+// vg_probe.cu -- measurement helpers for the roofline denominators ("FP64 peak: measure it
+// in the same run"; hard parts H2, H9).  Not part of the method.
+#include "vg_kernels.cuh"
+
+namespace vg {
+
+constexpr int kProbeIters = 4096;
+constexpr int kProbeChains = 8;
+
+// register-resident chains of independent DFMAs: kProbeChains x kProbeIters FMA per thread
+__global__ void __launch_bounds__(256) fma_chain_kernel(double seed, double *sink)
+{
+    double a[kProbeChains];
+#pragma unroll
+    for (int j = 0; j < kProbeChains; ++j) a[j] = seed + j + threadIdx.x * 1e-9;
+    double m = 1.0 + seed * 1e-12, c = seed * 1e-13;
+#pragma unroll 1
+    for (int it = 0; it < kProbeIters; it += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int j = 0; j < kProbeChains; ++j) a[j] = fma(a[j], m, c);
+    }
+    double s = 0;
+#pragma unroll
+    for (int j = 0; j < kProbeChains; ++j) s += a[j];
+    if (s == 12345.678) *sink = s; // never true; keeps the chains alive
+}
+
+__global__ void empty_kernel() {}
+
+cudaError_t probe_fp64_fma_rate(int launches, double *fma_per_s, cudaStream_t s)
+{
+    int dev = 0, sms = 0;
+    cudaError_t err;
+    if ((err = cudaGetDevice(&dev)) != cudaSuccess) return err;
+    if ((err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return err;
+    double *sink = nullptr;
+    if ((err = cudaMalloc(&sink, sizeof(double))) != cudaSuccess) return err;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    unsigned grid = unsigned(sms) * 8 * 4; // 4 waves of 8 resident 256-thread CTAs per SM
+    fma_chain_kernel<<<grid, 256, 0, s>>>(1.0, sink); // warm-up
+    cudaEventRecord(e0, s);
+    for (int i = 0; i < launches; ++i) fma_chain_kernel<<<grid, 256, 0, s>>>(1.0 + i, sink);
+    cudaEventRecord(e1, s);
+    err = cudaEventSynchronize(e1);
+    float ms = 0;
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    if (err == cudaSuccess && ms > 0)
+        *fma_per_s = double(launches) * double(grid) * 256.0 * kProbeChains * kProbeIters / (ms * 1e-3);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (err == cudaSuccess) err = cudaGetLastError();
+    return err;
+}
+
+cudaError_t probe_empty_launch(int launches, cudaStream_t s)
+{
+    for (int i = 0; i < launches; ++i) empty_kernel<<<1, 32, 0, s>>>();
+    return cudaGetLastError();
+}
+
+} // namespace vg

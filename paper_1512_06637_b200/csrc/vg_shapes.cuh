@@ -1,0 +1,770 @@
+// vg_shapes.cuh -- per-solid device code: Inside, exact signed distance (safeties), DistanceToIn, DistanceToOut.
+//
+// Semantics: SURVEY.md sec. 8(c) c.1-c.4 and readings R1-R21 (the paper names the three questions only,
+// PAPER.md:110-114).  Unlike the oracle (brute force over every boundary patch, both roots, atan2), the code
+// here is specialised per solid and evaluates only the crossings that CAN be the answer:
+//   * DistanceToIn looks only at crossings in the entering sense, DistanceToOut only in the leaving sense
+//     (for a surface F(t) = a t^2 + 2 b t + c with the material on the F < 0 side, the entering root is
+//     (-b - sqrt(D))/a and the leaving root (-b + sqrt(D))/a for either sign of a);
+//   * the phi test is two cross products with the stored plane vectors instead of atan2;
+//   * everything is select-based (no data-dependent branch inside a solid), zero direction components are
+//     replaced by +-1e-300 so that no 0/0 or inf-inf can arise (R9, hard part H4);
+//   * `valid` flags are conjunctions of positive comparisons, so a NaN candidate is always discarded.
+// Inside uses per-surface tolerance tests (an L-infinity band); it equals the oracle's Euclidean band except
+// for points within [kTol, sqrt(3) kTol] of an edge, which the parity contract excludes (R6, R7).
+#pragma once
+#include "vg_math.cuh"
+#include "vg_params.h"
+
+namespace vg {
+
+enum : int { cOutside = 0, cSurface = 1, cInside = 2 };
+
+VG_DEV int classify(bool in, bool out) { return in ? cInside : (out ? cOutside : cSurface); }
+
+// ------------------------------------------------------------------------------------------------ phi wedge
+
+struct WedgeEval {
+    double c0, c1; // signed distances into the segment from plane 0 / plane 1 (>= 0 on the material side)
+    double u0, u1; // coordinates along the two bounding half-planes (>= 0 on the half-plane itself)
+};
+
+VG_DEV WedgeEval wedge_eval(const Wedge &w, double x, double y)
+{
+    WedgeEval e;
+    e.c0 = fma(w.e0x, y, -w.e0y * x);
+    e.c1 = fma(w.e1y, x, -w.e1x * y);
+    e.u0 = fma(w.e0x, x, w.e0y * y);
+    e.u1 = fma(w.e1x, x, w.e1y * y);
+    return e;
+}
+
+VG_DEV bool wedge_member(const Wedge &w, double c0, double c1)
+{
+    return w.wide ? (c0 >= 0.0 || c1 >= 0.0) : (c0 >= 0.0 && c1 >= 0.0);
+}
+
+VG_DEV bool in_wedge(const Wedge &w, double x, double y)
+{
+    double c0 = fma(w.e0x, y, -w.e0y * x);
+    double c1 = fma(w.e1y, x, -w.e1x * y);
+    return wedge_member(w, c0, c1);
+}
+
+// squared distance from (x, y) to the nearer of the two bounding half-planes (not the full planes)
+VG_DEV double wedge_clear2(const WedgeEval &e, double rho2)
+{
+    double f0 = e.u0 >= 0.0 ? e.c0 * e.c0 : rho2;
+    double f1 = e.u1 >= 0.0 ? e.c1 * e.c1 : rho2;
+    return dmin(f0, f1);
+}
+
+VG_DEV void wedge_classify(const Wedge &w, double x, double y, double rho2, bool &in, bool &out)
+{
+    WedgeEval e = wedge_eval(w, x, y);
+    bool mem = wedge_member(w, e.c0, e.c1);
+    bool clear = wedge_clear2(e, rho2) > kTol * kTol;
+    in = in && mem && clear;
+    out = out || (!mem && clear);
+}
+
+// squared distance from (u, v) to the segment (r0, z0) + t (er, ez), t in [0, 1]
+VG_DEV double seg_d2(double u, double v, double r0, double z0, double er, double ez, double inv_l2)
+{
+    double wu = u - r0, wv = v - z0;
+    double t = fma(wu, er, wv * ez) * inv_l2;
+    t = dmin(dmax(t, 0.0), 1.0);
+    double du = fma(-t, er, wu), dv = fma(-t, ez, wv);
+    return fma(du, du, dv * dv);
+}
+
+// one root of a t^2 + 2 b t + c = 0 chosen by the sign of F' there: leaving = false gives the root with
+// F' < 0 ((-b - s)/a), leaving = true the root with F' > 0 ((-b + s)/a).  Evaluated as q/a or c/q with
+// q = -(b + sgn(b) s), whichever does not cancel, so it stays accurate for a -> 0 (ray along a generator).
+// Returns NaN/inf garbage when D <= 0; the caller tests D > 0.
+VG_DEV double quad_root(double a, double b, double c, double s, bool leaving)
+{
+    bool bpos = b >= 0.0;
+    double q = -(b + copysign_bits(s, b));
+    // bpos: q = -(b+s): (-b - s)/a = q/a, (-b + s)/a = c/q.   !bpos: q = -b + s: (-b + s)/a = q/a, (-b - s)/a = c/q
+    bool use_qa = (bpos != leaving);
+    double num = use_qa ? q : c;
+    double den = use_qa ? a : q;
+    return num * rcp(den);
+}
+
+// ------------------------------------------------------------------------------------------------------ box
+
+struct Box {
+    using P = BoxP;
+
+    VG_DEV static void slack(const P &p, double x, double y, double z, double &m, double &s2)
+    {
+        double qx = fabs(x) - p.hx, qy = fabs(y) - p.hy, qz = fabs(z) - p.hz;
+        m = dmax(dmax(qx, qy), qz);
+        double ax = dmax(qx, 0.0), ay = dmax(qy, 0.0), az = dmax(qz, 0.0);
+        s2 = fma(ax, ax, fma(ay, ay, az * az));
+    }
+    VG_DEV static int inside(const P &p, double x, double y, double z)
+    {
+        double m, s2;
+        slack(p, x, y, z, m, s2);
+        return classify(m < -kTol, s2 > kTol * kTol);
+    }
+    // c.3: sdf = |max(q, 0)| + min(max(qx, qy, qz), 0)
+    VG_DEV static double safety(const P &p, double x, double y, double z)
+    {
+        double m, s2;
+        slack(p, x, y, z, m, s2);
+        return m > 0.0 ? sqrt_pos(s2) : m;
+    }
+    // c.4 slabs, written for the direction folded to d >= 0: t1 = (-h - p s)/|d|, t2 = (h - p s)/|d|
+    VG_DEV static void slabs(const P &p, double x, double y, double z, double dx, double dy, double dz, double &tin,
+                             double &tout)
+    {
+        double ix = rcp(fabs(nonzero(dx))), iy = rcp(fabs(nonzero(dy))), iz = rcp(fabs(nonzero(dz)));
+        double px = flipsign_bits(x, dx), py = flipsign_bits(y, dy), pz = flipsign_bits(z, dz);
+        double hx = p.hx * ix, hy = p.hy * iy, hz = p.hz * iz;
+        double t1x = fma(-px, ix, -hx), t2x = fma(-px, ix, hx);
+        double t1y = fma(-py, iy, -hy), t2y = fma(-py, iy, hy);
+        double t1z = fma(-pz, iz, -hz), t2z = fma(-pz, iz, hz);
+        tin = dmax(dmax(t1x, t1y), t1z);
+        tout = dmin(dmin(t2x, t2y), t2z);
+    }
+    VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        double m, s2, tin, tout;
+        slack(p, x, y, z, m, s2);
+        slabs(p, x, y, z, dx, dy, dz, tin, tout);
+        double t = (tin < tout && tout > 0.0) ? tin : inf();
+        return m < -kTol ? -1.0 : t;
+    }
+    VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        double m, s2, tin, tout;
+        slack(p, x, y, z, m, s2);
+        slabs(p, x, y, z, dx, dy, dz, tin, tout);
+        return s2 > kTol * kTol ? -1.0 : tout;
+    }
+};
+
+// ------------------------------------------------------------------------------------------------------ orb
+
+struct Orb {
+    using P = OrbP;
+
+    VG_DEV static int inside(const P &p, double x, double y, double z)
+    {
+        double pp = fma(x, x, fma(y, y, z * z));
+        return classify(pp < p.rin2, pp > p.rout2);
+    }
+    VG_DEV static double safety(const P &p, double x, double y, double z)
+    {
+        double pp = fma(x, x, fma(y, y, z * z));
+        return sqrt_nn(pp) - p.r;
+    }
+    // c.4: a = 1, b = p.d, c = p.p - r^2; smallest root > 0
+    VG_DEV static double first_root(const P &p, double pp, double b)
+    {
+        double c = pp - p.r2;
+        double D = fma(b, b, -c);
+        double s = sqrt_pos(D);
+        double q = -(b + copysign_bits(s, b));
+        double t1 = q, t2 = c * rcp(q);
+        double lo = dmin(t1, t2), hi = dmax(t1, t2);
+        double t = lo > 0.0 ? lo : (hi > 0.0 ? hi : inf());
+        return D > 0.0 ? t : inf();
+    }
+    VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        double pp = fma(x, x, fma(y, y, z * z));
+        double b = fma(x, dx, fma(y, dy, z * dz));
+        double t = first_root(p, pp, b);
+        return pp < p.rin2 ? -1.0 : t;
+    }
+    VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        double pp = fma(x, x, fma(y, y, z * z));
+        double b = fma(x, dx, fma(y, dy, z * dz));
+        double t = first_root(p, pp, b);
+        return pp > p.rout2 ? -1.0 : t;
+    }
+};
+
+// ----------------------------------------------------------------------------------------------------- tube
+
+struct Tube {
+    using P = TubeP;
+
+    VG_DEV static void classify_pt(const P &p, double x, double y, double z, bool &in, bool &out)
+    {
+        double rho2 = fma(x, x, y * y), az = fabs(z);
+        in = az < p.dz - kTol && rho2 < p.rmax_in2;
+        out = az > p.dz + kTol || rho2 > p.rmax_out2;
+        if (p.hollow) {
+            in = in && rho2 > p.rmin_in2;
+            out = out || rho2 < p.rmin_out2;
+        }
+        if (!p.w.full) wedge_classify(p.w, x, y, rho2, in, out);
+    }
+    VG_DEV static int inside(const P &p, double x, double y, double z)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        return classify(in, out);
+    }
+    // c.3 for the rectangle [rmin, rmax] x [-dz, dz] in (rho, z) cut by the phi segment
+    VG_DEV static double safety(const P &p, double x, double y, double z)
+    {
+        double rho2 = fma(x, x, y * y);
+        double rho = sqrt_nn(rho2);
+        double qr = rho - p.rmax;
+        if (p.hollow) qr = dmax(qr, p.rmin - rho);
+        double qz = fabs(z) - p.dz;
+        double ar = dmax(qr, 0.0), az = dmax(qz, 0.0);
+        double out2 = fma(ar, ar, az * az);
+        double m = dmax(qr, qz);
+        bool in_rect = m < 0.0;
+        if (p.w.full) return in_rect ? m : sqrt_nn(out2);
+        double D2 = in_rect ? m * m : out2;
+        WedgeEval e = wedge_eval(p.w, x, y);
+        bool mem = wedge_member(p.w, e.c0, e.c1);
+        D2 = mem ? D2 : inf();
+        // the two phi faces: filled rectangle [rmin, rmax] x [-dz, dz] in the half-plane (u >= 0)
+        double q0 = dmax(dmax(e.u0 - p.rmax, p.rmin - e.u0), 0.0);
+        double q1 = dmax(dmax(e.u1 - p.rmax, p.rmin - e.u1), 0.0);
+        double az2 = az * az;
+        D2 = dmin(D2, fma(e.c0, e.c0, fma(q0, q0, az2)));
+        D2 = dmin(D2, fma(e.c1, e.c1, fma(q1, q1, az2)));
+        double D = sqrt_nn(D2);
+        return (mem && in_rect) ? -D : D;
+    }
+
+    VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        double rho2 = fma(x, x, y * y);
+        double a = fma(dx, dx, dy * dy);
+        double b = fma(x, dx, y * dy);
+        double inv_a = rcp(nonzero(a));
+        double best = inf();
+        // outer cylinder, entering root
+        {
+            double D = fma(b, b, -a * (rho2 - p.rmax2));
+            double t = (-b - sqrt_pos(D)) * inv_a;
+            double zh = fma(t, dz, z);
+            bool ok = D > 0.0 && t > 0.0 && fabs(zh) <= p.dz;
+            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            best = ok ? t : best;
+        }
+        // inner cylinder: the ray enters the material where it LEAVES the bore
+        if (p.hollow) {
+            double D = fma(b, b, -a * (rho2 - p.rmin2));
+            double t = (-b + sqrt_pos(D)) * inv_a;
+            double zh = fma(t, dz, z);
+            bool ok = D > 0.0 && t > 0.0 && fabs(zh) <= p.dz;
+            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            best = (ok && t < best) ? t : best;
+        }
+        // the cap the ray moves towards, only from beyond it
+        {
+            double az = fabs(z);
+            double t = (az - p.dz) * rcp(fabs(nonzero(dz)));
+            double hx = fma(t, dx, x), hy = fma(t, dy, y);
+            double rh2 = fma(hx, hx, hy * hy);
+            bool ok = az > p.dz && z * dz < 0.0 && t > 0.0 && rh2 >= p.rmin2 && rh2 <= p.rmax2;
+            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            best = (ok && t < best) ? t : best;
+        }
+        // phi faces, entering sense: c_k(p) < 0 and c_k(d) > 0
+        if (!p.w.full) {
+            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+            {
+                double t = -ep.c0 * rcp(ed.c0);
+                double uh = fma(t, ed.u0, ep.u0), zh = fma(t, dz, z);
+                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && t > 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(zh) <= p.dz;
+                best = (ok && t < best) ? t : best;
+            }
+            {
+                double t = -ep.c1 * rcp(ed.c1);
+                double uh = fma(t, ed.u1, ep.u1), zh = fma(t, dz, z);
+                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && t > 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(zh) <= p.dz;
+                best = (ok && t < best) ? t : best;
+            }
+        }
+        return in ? -1.0 : best;
+    }
+
+    VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        double rho2 = fma(x, x, y * y);
+        double a = fma(dx, dx, dy * dy);
+        double b = fma(x, dx, y * dy);
+        double inv_a = rcp(nonzero(a));
+        double best = inf();
+        {
+            double D = fma(b, b, -a * (rho2 - p.rmax2));
+            double t = (-b + sqrt_pos(D)) * inv_a;
+            best = (D > 0.0 && t > 0.0) ? t : best;
+        }
+        if (p.hollow) {
+            double D = fma(b, b, -a * (rho2 - p.rmin2));
+            double t = (-b - sqrt_pos(D)) * inv_a;
+            best = (D > 0.0 && b < 0.0 && t > 0.0 && t < best) ? t : best;
+        }
+        {
+            double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(nonzero(dz)));
+            best = (t > 0.0 && t < best) ? t : best;
+        }
+        if (!p.w.full) {
+            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+            {
+                double t = -ep.c0 * rcp(ed.c0);
+                bool ok = ed.c0 < 0.0 && t > 0.0 && fma(t, ed.u0, ep.u0) >= 0.0;
+                best = (ok && t < best) ? t : best;
+            }
+            {
+                double t = -ep.c1 * rcp(ed.c1);
+                bool ok = ed.c1 < 0.0 && t > 0.0 && fma(t, ed.u1, ep.u1) >= 0.0;
+                best = (ok && t < best) ? t : best;
+            }
+        }
+        return out ? -1.0 : best;
+    }
+};
+
+// ------------------------------------------------------------------------------- conical patches (cone, polycone)
+
+// coefficients of F(t) = rho(t)^2 - k(t)^2 on the ray, k = A + B z (c.4 "slanted or vertical edge")
+struct RayRZ {
+    double rho2, a_xy, b_xy; // x^2+y^2, dx^2+dy^2, x dx + y dy
+};
+
+VG_DEV double frustum_root(const Frustum &f, const RayRZ &r, double z, double dz, bool leaving, bool &ok)
+{
+    double k = fma(f.B, z, f.A);
+    double Bd = f.B * dz;
+    double a = fma(-Bd, Bd, r.a_xy);
+    double b = fma(-Bd, k, r.b_xy);
+    double c = fma(-k, k, r.rho2);
+    double D = fma(b, b, -a * c);
+    double t = quad_root(a, b, c, sqrt_pos(D), leaving);
+    ok = D > 0.0 && t > 0.0;
+    return t;
+}
+
+// ----------------------------------------------------------------------------------------------------- cone
+
+struct Cone {
+    using P = ConeP;
+
+    VG_DEV static void classify_pt(const P &p, double x, double y, double z, bool &in, bool &out)
+    {
+        double rho2 = fma(x, x, y * y), az = fabs(z);
+        double ro = fma(p.out.B, z, p.out.A), to = kTol * p.out.sec;
+        double ro_in = ro - to, ro_out = ro + to;
+        in = az < p.dz - kTol && ro_in > 0.0 && rho2 < ro_in * ro_in;
+        out = az > p.dz + kTol || rho2 > ro_out * ro_out;
+        if (p.hollow) {
+            double ri = fma(p.in.B, z, p.in.A), ti = kTol * p.in.sec;
+            double ri_in = ri + ti, ri_out = ri - ti;
+            in = in && (ri_in < 0.0 || rho2 > ri_in * ri_in);
+            out = out || (ri_out > 0.0 && rho2 < ri_out * ri_out);
+        }
+        if (!p.w.full) wedge_classify(p.w, x, y, rho2, in, out);
+    }
+    VG_DEV static int inside(const P &p, double x, double y, double z)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        return classify(in, out);
+    }
+    // squared distance from (u, v) to the outline of the quadrilateral; `axis` adds the edge on the axis
+    // (part of a phi face, not of the surface of revolution) when rmin1 = rmin2 = 0
+    VG_DEV static double outline_d2(const P &p, double u, double v, bool axis)
+    {
+        double ez = 2.0 * p.dz;
+        double d2 = seg_d2(u, v, p.out.r0, -p.dz, p.out.er, ez, p.out.inv_l2);
+        if (p.hollow || axis) d2 = dmin(d2, seg_d2(u, v, p.in.r0, -p.dz, p.in.er, ez, p.in.inv_l2));
+        double b1 = dmax(dmax(p.rmin1 - u, u - p.rmax1), 0.0), v1 = v + p.dz;
+        double b2 = dmax(dmax(p.rmin2 - u, u - p.rmax2), 0.0), v2 = v - p.dz;
+        d2 = dmin(d2, fma(b1, b1, v1 * v1));
+        d2 = dmin(d2, fma(b2, b2, v2 * v2));
+        return d2;
+    }
+    VG_DEV static bool in_quad(const P &p, double u, double v)
+    {
+        double ro = fma(p.out.B, v, p.out.A), ri = fma(p.in.B, v, p.in.A);
+        return fabs(v) < p.dz && u < ro && u > ri;
+    }
+    VG_DEV static double safety(const P &p, double x, double y, double z)
+    {
+        double rho2 = fma(x, x, y * y);
+        double rho = sqrt_nn(rho2);
+        double ro = fma(p.out.B, z, p.out.A), ri = fma(p.in.B, z, p.in.A);
+        bool in2d = fabs(z) < p.dz && rho < ro && (rho > ri || !p.hollow);
+        double D2 = outline_d2(p, rho, z, false);
+        if (p.w.full) {
+            double D = sqrt_nn(D2);
+            return in2d ? -D : D;
+        }
+        WedgeEval e = wedge_eval(p.w, x, y);
+        bool mem = wedge_member(p.w, e.c0, e.c1);
+        D2 = mem ? D2 : inf();
+        double f0 = in_quad(p, e.u0, z) ? 0.0 : outline_d2(p, e.u0, z, true);
+        double f1 = in_quad(p, e.u1, z) ? 0.0 : outline_d2(p, e.u1, z, true);
+        D2 = dmin(D2, fma(e.c0, e.c0, f0));
+        D2 = dmin(D2, fma(e.c1, e.c1, f1));
+        double D = sqrt_nn(D2);
+        return (mem && in2d) ? -D : D;
+    }
+
+    VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        RayRZ r;
+        r.rho2 = fma(x, x, y * y);
+        r.a_xy = fma(dx, dx, dy * dy);
+        r.b_xy = fma(x, dx, y * dy);
+        double best = inf();
+        {
+            bool ok;
+            double t = frustum_root(p.out, r, z, dz, false, ok);
+            ok = ok && fabs(fma(t, dz, z)) <= p.dz;
+            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            best = ok ? t : best;
+        }
+        if (p.hollow) {
+            bool ok;
+            double t = frustum_root(p.in, r, z, dz, true, ok);
+            ok = ok && fabs(fma(t, dz, z)) <= p.dz;
+            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            best = (ok && t < best) ? t : best;
+        }
+        {
+            double az = fabs(z);
+            double t = (az - p.dz) * rcp(fabs(nonzero(dz)));
+            double hx = fma(t, dx, x), hy = fma(t, dy, y);
+            double rh2 = fma(hx, hx, hy * hy);
+            bool top = z > 0.0;
+            double rlo = top ? p.rmin2 : p.rmin1, rhi = top ? p.rmax2 : p.rmax1;
+            bool ok = az > p.dz && z * dz < 0.0 && t > 0.0 && rh2 >= rlo * rlo && rh2 <= rhi * rhi;
+            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            best = (ok && t < best) ? t : best;
+        }
+        if (!p.w.full) {
+            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+            {
+                double t = -ep.c0 * rcp(ed.c0);
+                double uh = fma(t, ed.u0, ep.u0), zh = fma(t, dz, z);
+                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && t > 0.0 && fabs(zh) <= p.dz &&
+                          uh >= fma(p.in.B, zh, p.in.A) && uh <= fma(p.out.B, zh, p.out.A);
+                best = (ok && t < best) ? t : best;
+            }
+            {
+                double t = -ep.c1 * rcp(ed.c1);
+                double uh = fma(t, ed.u1, ep.u1), zh = fma(t, dz, z);
+                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && t > 0.0 && fabs(zh) <= p.dz &&
+                          uh >= fma(p.in.B, zh, p.in.A) && uh <= fma(p.out.B, zh, p.out.A);
+                best = (ok && t < best) ? t : best;
+            }
+        }
+        return in ? -1.0 : best;
+    }
+
+    VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        RayRZ r;
+        r.rho2 = fma(x, x, y * y);
+        r.a_xy = fma(dx, dx, dy * dy);
+        r.b_xy = fma(x, dx, y * dy);
+        double best = inf();
+        {
+            bool ok;
+            double t = frustum_root(p.out, r, z, dz, true, ok);
+            best = ok ? t : best;
+        }
+        if (p.hollow) {
+            bool ok;
+            double t = frustum_root(p.in, r, z, dz, false, ok);
+            // the mirror nappe (k < 0) lies beyond a cap, but guard the apex-at-the-cap case
+            ok = ok && fma(p.in.B, fma(t, dz, z), p.in.A) >= 0.0;
+            best = (ok && t < best) ? t : best;
+        }
+        {
+            double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(nonzero(dz)));
+            best = (t > 0.0 && t < best) ? t : best;
+        }
+        if (!p.w.full) {
+            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+            {
+                double t = -ep.c0 * rcp(ed.c0);
+                bool ok = ed.c0 < 0.0 && t > 0.0 && fma(t, ed.u0, ep.u0) >= 0.0;
+                best = (ok && t < best) ? t : best;
+            }
+            {
+                double t = -ep.c1 * rcp(ed.c1);
+                bool ok = ed.c1 < 0.0 && t > 0.0 && fma(t, ed.u1, ep.u1) >= 0.0;
+                best = (ok && t < best) ? t : best;
+            }
+        }
+        return out ? -1.0 : best;
+    }
+};
+
+// ------------------------------------------------------------------------------------------------------ trd
+
+struct Trd {
+    using P = TrdP;
+
+    // max over the six planes of the signed plane distance (exact sdf inside a convex body)
+    VG_DEV static double gmax(const P &p, double ax, double ay, double z, double &gx, double &gy)
+    {
+        gx = (fma(-p.fx, z, ax) - p.mx) * p.icx;
+        gy = (fma(-p.fy, z, ay) - p.my) * p.icy;
+        return dmax(dmax(gx, gy), fabs(z) - p.dz);
+    }
+    VG_DEV static int inside(const P &p, double x, double y, double z)
+    {
+        double gx, gy;
+        double g = gmax(p, fabs(x), fabs(y), z, gx, gy);
+        return classify(g < -kTol, g > kTol);
+    }
+    // squared in-plane distance from (v, s), v >= 0, to the filled symmetric trapezoid with half-widths r1 at
+    // s = -he and r2 at s = +he; 0 inside.  inv_k = 1 / ((r2-r1)^2 + (2 he)^2).
+    VG_DEV static double trapezoid_d2(double v, double s, double r1, double r2, double he, double inv_k)
+    {
+        double rc = s < 0.0 ? r1 : r2;
+        double cax = dmax(v - rc, 0.0), cay = fabs(s) - he;
+        double k2x = r2 - r1, k2y = 2.0 * he;
+        double h = fma(r2 - v, k2x, (he - s) * k2y) * inv_k;
+        h = dmin(dmax(h, 0.0), 1.0);
+        double cbx = fma(k2x, h, v - r2), cby = fma(k2y, h, s - he);
+        double d2 = dmin(fma(cax, cax, cay * cay), fma(cbx, cbx, cby * cby));
+        return (cbx < 0.0 && cay < 0.0) ? 0.0 : d2;
+    }
+    VG_DEV static double safety(const P &p, double x, double y, double z)
+    {
+        double ax = fabs(x), ay = fabs(y), gx, gy;
+        double g = gmax(p, ax, ay, z, gx, gy);
+        // the two z faces: rectangles
+        double zx1 = dmax(ax - p.dx1, 0.0), zy1 = dmax(ay - p.dy1, 0.0), zz1 = z + p.dz;
+        double zx2 = dmax(ax - p.dx2, 0.0), zy2 = dmax(ay - p.dy2, 0.0), zz2 = z - p.dz;
+        double D2 = dmin(fma(zx1, zx1, fma(zy1, zy1, zz1 * zz1)), fma(zx2, zx2, fma(zy2, zy2, zz2 * zz2)));
+        // +x face: foot of the perpendicular, in-plane coordinates (|y|, slant coordinate)
+        {
+            double zf = fma(gx * p.icx, p.fx, z);
+            D2 = dmin(D2, fma(gx, gx, trapezoid_d2(ay, zf * p.cx, p.dy1, p.dy2, p.dz * p.cx, p.inv_kx)));
+        }
+        {
+            double zf = fma(gy * p.icy, p.fy, z);
+            D2 = dmin(D2, fma(gy, gy, trapezoid_d2(ax, zf * p.cy, p.dx1, p.dx2, p.dz * p.cy, p.inv_ky)));
+        }
+        return g > 0.0 ? sqrt_nn(D2) : g;
+    }
+    // c.4 generic convex clip over the six half-spaces (normals need not be unit: num/den is scale free)
+    VG_DEV static void clip(double num, double den, double &tin, double &tout)
+    {
+        double dn = nonzero(den); // den = +-0 -> +-1e-300: t = -+huge decides hit / miss like the oracle's branch
+        double t = num * rcp(dn);
+        tout = (dn > 0.0 && t < tout) ? t : tout;
+        tin = (dn < 0.0 && t > tin) ? t : tin;
+    }
+    VG_DEV static void clip_all(const P &p, double x, double y, double z, double dx, double dy, double dz, double &tin,
+                                double &tout)
+    {
+        tin = -inf();
+        tout = inf();
+        double sx = fma(p.fx, z, p.mx), sdx = p.fx * dz; // X(z) and its rate along the ray
+        double sy = fma(p.fy, z, p.my), sdy = p.fy * dz;
+        clip(sx - x, dx - sdx, tin, tout);
+        clip(sx + x, -dx - sdx, tin, tout);
+        clip(sy - y, dy - sdy, tin, tout);
+        clip(sy + y, -dy - sdy, tin, tout);
+        clip(p.dz - z, dz, tin, tout);
+        clip(p.dz + z, -dz, tin, tout);
+    }
+    VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        double gx, gy, tin, tout;
+        double g = gmax(p, fabs(x), fabs(y), z, gx, gy);
+        clip_all(p, x, y, z, dx, dy, dz, tin, tout);
+        double t = (tin < tout && tout > 0.0) ? tin : inf();
+        return g < -kTol ? -1.0 : t;
+    }
+    VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        double gx, gy, tin, tout;
+        double g = gmax(p, fabs(x), fabs(y), z, gx, gy);
+        clip_all(p, x, y, z, dx, dy, dz, tin, tout);
+        return g > kTol ? -1.0 : tout;
+    }
+};
+
+// ------------------------------------------------------------------------------------------------- polycone
+
+struct Polycone {
+    using P = PolyconeP;
+
+    VG_DEV static bool has_inner(const P &p, int k) { return (p.inner_mask >> k) & 1u; }
+
+    // membership of (u, v) in the (r, z) outline (closed), by section
+    VG_DEV static bool in_outline(const P &p, double u, double v)
+    {
+        bool mem = false;
+#pragma unroll 1
+        for (int k = 0; k < p.nsec; ++k) {
+            const PconSec &s = p.sec[k];
+            double ro = fma(s.out.B, v, s.out.A), ri = fma(s.in.B, v, s.in.A);
+            mem = mem || (v >= s.z0 && v <= s.z1 && u <= ro && u >= ri);
+        }
+        return mem;
+    }
+    VG_DEV static void classify_pt(const P &p, double x, double y, double z, bool &in, bool &out)
+    {
+        double rho2 = fma(x, x, y * y);
+        double rho = sqrt_nn(rho2);
+        bool any_in = false, any_near = false;
+#pragma unroll 1
+        for (int k = 0; k < p.nsec; ++k) {
+            const PconSec &s = p.sec[k];
+            double ro = fma(s.out.B, z, s.out.A), ri = fma(s.in.B, z, s.in.A);
+            double to = kTol * s.out.sec, ti = kTol * s.in.sec;
+            bool zin = z >= s.z0 && z <= s.z1;
+            bool znear = z >= s.z0 - kTol && z <= s.z1 + kTol;
+            bool inner = has_inner(p, k);
+            any_in = any_in || (zin && rho < ro - to && (!inner || rho > ri + ti));
+            any_near = any_near || (znear && rho <= ro + to && (!inner || rho >= ri - ti));
+        }
+        in = any_in && z > p.zlo + kTol && z < p.zhi - kTol;
+        out = !any_near;
+        if (!p.w.full) wedge_classify(p.w, x, y, rho2, in, out);
+    }
+    VG_DEV static int inside(const P &p, double x, double y, double z)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        return classify(in, out);
+    }
+    VG_DEV static double outline_d2(const P &p, double u, double v, bool axis)
+    {
+        double b1 = dmax(dmax(p.cap_lo_rmin - u, u - p.cap_lo_rmax), 0.0), v1 = v - p.zlo;
+        double b2 = dmax(dmax(p.cap_hi_rmin - u, u - p.cap_hi_rmax), 0.0), v2 = v - p.zhi;
+        double d2 = dmin(fma(b1, b1, v1 * v1), fma(b2, b2, v2 * v2));
+#pragma unroll 1
+        for (int k = 0; k < p.nsec; ++k) {
+            const PconSec &s = p.sec[k];
+            double ez = s.z1 - s.z0;
+            d2 = dmin(d2, seg_d2(u, v, s.out.r0, s.z0, s.out.er, ez, s.out.inv_l2));
+            double di = seg_d2(u, v, s.in.r0, s.z0, s.in.er, ez, s.in.inv_l2);
+            d2 = (has_inner(p, k) || axis) ? dmin(d2, di) : d2;
+        }
+        return d2;
+    }
+    VG_DEV static double safety(const P &p, double x, double y, double z)
+    {
+        double rho2 = fma(x, x, y * y);
+        double rho = sqrt_nn(rho2);
+        bool in2d = in_outline(p, rho, z);
+        double D2 = outline_d2(p, rho, z, false);
+        if (p.w.full) {
+            double D = sqrt_nn(D2);
+            return in2d ? -D : D;
+        }
+        WedgeEval e = wedge_eval(p.w, x, y);
+        bool mem = wedge_member(p.w, e.c0, e.c1);
+        D2 = mem ? D2 : inf();
+        double f0 = in_outline(p, e.u0, z) ? 0.0 : outline_d2(p, e.u0, z, true);
+        double f1 = in_outline(p, e.u1, z) ? 0.0 : outline_d2(p, e.u1, z, true);
+        D2 = dmin(D2, fma(e.c0, e.c0, f0));
+        D2 = dmin(D2, fma(e.c1, e.c1, f1));
+        double D = sqrt_nn(D2);
+        return (mem && in2d) ? -D : D;
+    }
+
+    // first crossing in the entering (leaving = false) or leaving (leaving = true) sense over all patches
+    VG_DEV static double cross(const P &p, double x, double y, double z, double dx, double dy, double dz, bool leaving)
+    {
+        RayRZ r;
+        r.rho2 = fma(x, x, y * y);
+        r.a_xy = fma(dx, dx, dy * dy);
+        r.b_xy = fma(x, dx, y * dy);
+        double best = inf();
+#pragma unroll 1
+        for (int k = 0; k < p.nsec; ++k) {
+            const PconSec &s = p.sec[k];
+            {
+                bool ok;
+                double t = frustum_root(s.out, r, z, dz, leaving, ok);
+                double zh = fma(t, dz, z);
+                ok = ok && zh >= s.z0 && zh <= s.z1;
+                if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+                best = (ok && t < best) ? t : best;
+            }
+            if (has_inner(p, k)) {
+                bool ok;
+                double t = frustum_root(s.in, r, z, dz, !leaving, ok);
+                double zh = fma(t, dz, z);
+                ok = ok && zh >= s.z0 && zh <= s.z1;
+                if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+                best = (ok && t < best) ? t : best;
+            }
+        }
+        // end caps: entering from beyond, leaving from within
+        double idz = rcp(nonzero(dz));
+        {
+            double t = (p.zlo - z) * idz;
+            double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);
+            bool sense = leaving ? dz < 0.0 : dz > 0.0;
+            bool ok = sense && t > 0.0 && rh2 >= p.cap_lo_rmin * p.cap_lo_rmin && rh2 <= p.cap_lo_rmax * p.cap_lo_rmax;
+            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            best = (ok && t < best) ? t : best;
+        }
+        {
+            double t = (p.zhi - z) * idz;
+            double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);
+            bool sense = leaving ? dz > 0.0 : dz < 0.0;
+            bool ok = sense && t > 0.0 && rh2 >= p.cap_hi_rmin * p.cap_hi_rmin && rh2 <= p.cap_hi_rmax * p.cap_hi_rmax;
+            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            best = (ok && t < best) ? t : best;
+        }
+        if (!p.w.full) {
+            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+            {
+                double t = -ep.c0 * rcp(ed.c0);
+                bool sense = leaving ? ed.c0 < 0.0 : ed.c0 > 0.0;
+                bool ok = sense && t > 0.0 && in_outline(p, fma(t, ed.u0, ep.u0), fma(t, dz, z));
+                best = (ok && t < best) ? t : best;
+            }
+            {
+                double t = -ep.c1 * rcp(ed.c1);
+                bool sense = leaving ? ed.c1 < 0.0 : ed.c1 > 0.0;
+                bool ok = sense && t > 0.0 && in_outline(p, fma(t, ed.u1, ep.u1), fma(t, dz, z));
+                best = (ok && t < best) ? t : best;
+            }
+        }
+        return best;
+    }
+    VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        double t = cross(p, x, y, z, dx, dy, dz, false);
+        return in ? -1.0 : t;
+    }
+    VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
+    {
+        bool in, out;
+        classify_pt(p, x, y, z, in, out);
+        double t = cross(p, x, y, z, dx, dy, dz, true);
+        return out ? -1.0 : t;
+    }
+};
+
+} // namespace vg
