@@ -134,6 +134,29 @@ int vg_compute_step(const vg_volume *volume, const double *x, const double *y, c
 int vg_volume_safety(const vg_volume *volume, const double *x, const double *y, const double *z, int64_t n,
                      double *safety, void *stream);
 
+/* ---- host-buffer entry points (the scheduler hands baskets of tracks to the geometry every step;
+ *      the GPU pays off once transfers are amortised) ----
+ *
+ * Same operations as above, but every track array and every output array is a HOST pointer (pageable or
+ * pinned; pinned memory makes the copies asynchronous).  The library cuts the arrays into chunks and pipelines
+ * host->device copy, the same kernels, device->host copy over several internal streams and per-device staging
+ * memory allocated once on first use.  The call returns when the outputs are complete (it synchronises its own
+ * streams only).  Calls on one device are serialised by a lock.
+ *
+ * vg_query_host: `query` is a vg_query; out is int32[n] for VG_Q_INSIDE, double[n] otherwise; dx, dy, dz are
+ * read only by the two distance queries (may be NULL otherwise), step_max likewise. */
+typedef enum {
+    VG_Q_INSIDE = 0,
+    VG_Q_DISTANCE_TO_IN = 1,
+    VG_Q_DISTANCE_TO_OUT = 2,
+    VG_Q_SAFETY_TO_IN = 3,
+    VG_Q_SAFETY_TO_OUT = 4
+} vg_query;
+int vg_query_host(const vg_shape *shape, int query, const double *x, const double *y, const double *z,
+                  const double *dx, const double *dy, const double *dz, double step_max, int64_t n, void *out);
+int vg_compute_step_host(const vg_volume *volume, const double *x, const double *y, const double *z, const double *dx,
+                         const double *dy, const double *dz, double step_max, int64_t n, double *step, int32_t *hit);
+
 /* Thread-local message of the last failing call on this host thread ("" if none). Static storage. */
 const char *vg_last_error(void);
 
@@ -145,6 +168,8 @@ const char *vg_last_error(void);
 int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *stream);
 /* Enqueues `launches` empty kernels (launch-latency floor for the small-N end of configs[3]). */
 int vg_probe_empty_launch(int launches, void *stream);
+/* Number of kernel launches the library has made in this process (all threads). */
+int64_t vg_launch_count(void);
 
 #ifdef __cplusplus
 }

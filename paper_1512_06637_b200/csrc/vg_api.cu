@@ -4,6 +4,7 @@
 #include "../../include/vg.h"
 #include "vg_kernels.cuh"
 
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -47,6 +48,14 @@ static int fail_cuda(cudaError_t e, const char *what)
 }
 
 extern "C" const char *vg_last_error(void) { return g_err; }
+
+// for the other host translation units of the library (vg_host.cu)
+extern "C" int vg_set_error(int code, const char *msg) { return fail(code, "%s", msg); }
+
+namespace vg {
+std::atomic<int64_t> g_launches{ 0 };
+}
+extern "C" int64_t vg_launch_count(void) { return vg::g_launches.load(); }
 
 // ------------------------------------------------------------------------------------------- derived constants
 
@@ -227,6 +236,8 @@ static int check_arrays(const char *fn, const void *const *ptrs, int count, size
                         int64_t n, bool *vec)
 {
     if (n < 0) return fail(VG_ERR_ARG, "%s: n < 0", fn);
+    *vec = false;
+    if (n == 0) return VG_OK; // nothing is read or written: pointers are not inspected
     bool v = true;
     for (int i = 0; i < count; ++i) {
         if (!ptrs[i]) return fail(VG_ERR_ARG, "%s: NULL track array", fn);
@@ -393,9 +404,9 @@ extern "C" int vg_compute_step(const vg_volume *v, const double *x, const double
     bool vec = false;
     int rc = check_arrays(fn, ptrs, 6, 8, step, n, &vec);
     if (rc != VG_OK) return rc;
+    if (n == 0) return VG_OK;
     if (!hit || !aligned(hit, 4)) return fail(VG_ERR_ARG, "%s: hit array NULL or misaligned", fn);
     if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
-    if (n == 0) return VG_OK;
     Tracks t{ x, y, z, dx, dy, dz };
     cudaError_t e = launch_compute_step(v->mother, v->table_dev, v->nd, t, step_max, n, step, hit,
                                         static_cast<cudaStream_t>(stream));

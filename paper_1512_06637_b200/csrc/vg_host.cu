@@ -1,0 +1,155 @@
+// vg_host.cu -- host-buffer entry points: tracks arrive from a host scheduler every step (PAPER.md:61 the
+// scheduler hands baskets to the geometry; PAPER.md:122 the GPU only pays off once the transfer is amortised;
+// SURVEY.md sec. 8(f) f4).  The arrays are cut into chunks; chunk c uses slot c % kSlots = {a CUDA stream, a
+// device staging area}: H2D copies of the six (or three) coordinate arrays, the SAME kernel the device entry
+// points launch, D2H copy of the result.  Operations of one slot are ordered by its stream, different slots
+// overlap, so that the two copy engines and the SMs work at the same time when the host memory is pinned.
+// Staging memory is allocated once per device on first use (never per call).
+#include "../../include/vg.h"
+#include "vg_kernels.cuh"
+
+#include <cstdio>
+#include <mutex>
+
+namespace vg {
+
+constexpr int kSlots = 4;
+constexpr int64_t kMaxChunk = int64_t(1) << 20; // tracks per chunk: 8 MiB per coordinate array
+constexpr int64_t kMinChunk = int64_t(1) << 16;
+constexpr int kMaxDev = 16;
+
+struct HostPipe {
+    bool ready = false;
+    cudaStream_t st[kSlots];
+    double *in[kSlots];   // 6 * kMaxChunk doubles
+    double *outd[kSlots]; // kMaxChunk doubles
+    int32_t *outi[kSlots]; // kMaxChunk int32
+    std::mutex mu;
+};
+
+static HostPipe g_pipe[kMaxDev];
+
+static cudaError_t pipe_slot(HostPipe **out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+    *out = &g_pipe[dev];
+    return cudaSuccess;
+}
+
+// called with p.mu held
+static cudaError_t pipe_init(HostPipe &p)
+{
+    cudaError_t e;
+    if (!p.ready) {
+        for (int s = 0; s < kSlots; ++s) {
+            if ((e = cudaStreamCreateWithFlags(&p.st[s], cudaStreamNonBlocking)) != cudaSuccess) return e;
+            if ((e = cudaMalloc(&p.in[s], 6 * kMaxChunk * sizeof(double))) != cudaSuccess) return e;
+            if ((e = cudaMalloc(&p.outd[s], kMaxChunk * sizeof(double))) != cudaSuccess) return e;
+            if ((e = cudaMalloc(&p.outi[s], kMaxChunk * sizeof(int32_t))) != cudaSuccess) return e;
+        }
+        p.ready = true;
+    }
+    return cudaSuccess;
+}
+
+static int64_t pick_chunk(int64_t n)
+{
+    int64_t c = (n + 2 * kSlots - 1) / (2 * kSlots); // about two rounds over the slots
+    c = (c + 4095) / 4096 * 4096;
+    if (c < kMinChunk) c = kMinChunk;
+    if (c > kMaxChunk) c = kMaxChunk;
+    return c;
+}
+
+} // namespace vg
+
+using namespace vg;
+
+extern "C" int vg_set_error(int code, const char *msg); // vg_api.cu
+
+static int cuda_fail(cudaError_t e, const char *fn)
+{
+    char buf[256];
+    snprintf(buf, sizeof buf, "%s: %s", fn, cudaGetErrorString(e));
+    return vg_set_error(VG_ERR_CUDA, buf);
+}
+
+// shape != NULL: query q of the shape; volume != NULL: ComputeStep
+static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volume, int q, const double *const h[6],
+                    double step_max, int64_t n, void *out, int32_t *hit)
+{
+    bool dir = volume || q == qDistIn || q == qDistOut;
+    int na = dir ? 6 : 3;
+    if (n < 0) return vg_set_error(VG_ERR_ARG, "host entry: n < 0");
+    for (int a = 0; a < na; ++a)
+        if (!h[a]) return vg_set_error(VG_ERR_ARG, "host entry: NULL track array");
+    if (!out || (volume && !hit)) return vg_set_error(VG_ERR_ARG, "host entry: NULL output array");
+    if (n == 0) return VG_OK;
+    HostPipe *p = nullptr;
+    cudaError_t e = pipe_slot(&p);
+    if (e != cudaSuccess) return cuda_fail(e, fn);
+    std::lock_guard<std::mutex> lock(p->mu);
+    if ((e = pipe_init(*p)) != cudaSuccess) return cuda_fail(e, fn);
+    int64_t chunk = pick_chunk(n);
+    int rc = VG_OK;
+    int c = 0;
+    for (int64_t o = 0; o < n && rc == VG_OK; o += chunk, ++c) {
+        int s = c % kSlots;
+        int64_t m = n - o < chunk ? n - o : chunk;
+        cudaStream_t st = p->st[s];
+        double *d[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
+        for (int a = 0; a < na; ++a) {
+            d[a] = p->in[s] + a * kMaxChunk;
+            e = cudaMemcpyAsync(d[a], h[a] + o, m * sizeof(double), cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return cuda_fail(e, fn);
+        }
+        if (volume) {
+            rc = vg_compute_step(volume, d[0], d[1], d[2], d[3], d[4], d[5], step_max, m, p->outd[s], p->outi[s], st);
+            if (rc != VG_OK) break;
+            e = cudaMemcpyAsync(static_cast<double *>(out) + o, p->outd[s], m * sizeof(double), cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(hit + o, p->outi[s], m * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        } else if (q == qInside) {
+            rc = vg_inside(shape, d[0], d[1], d[2], m, p->outi[s], st);
+            if (rc != VG_OK) break;
+            e = cudaMemcpyAsync(static_cast<int32_t *>(out) + o, p->outi[s], m * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        } else {
+            switch (q) {
+            case qDistIn: rc = vg_distance_to_in(shape, d[0], d[1], d[2], d[3], d[4], d[5], step_max, m, p->outd[s], st); break;
+            case qDistOut: rc = vg_distance_to_out(shape, d[0], d[1], d[2], d[3], d[4], d[5], step_max, m, p->outd[s], st); break;
+            case qSafeIn: rc = vg_safety_to_in(shape, d[0], d[1], d[2], m, p->outd[s], st); break;
+            case qSafeOut: rc = vg_safety_to_out(shape, d[0], d[1], d[2], m, p->outd[s], st); break;
+            default: rc = vg_set_error(VG_ERR_ARG, "vg_query_host: unknown query");
+            }
+            if (rc != VG_OK) break;
+            e = cudaMemcpyAsync(static_cast<double *>(out) + o, p->outd[s], m * sizeof(double), cudaMemcpyDeviceToHost, st);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, fn);
+    }
+    for (int s = 0; s < kSlots; ++s) {
+        e = cudaStreamSynchronize(p->st[s]);
+        if (e != cudaSuccess && rc == VG_OK) rc = cuda_fail(e, fn);
+    }
+    return rc;
+}
+
+extern "C" int vg_query_host(const vg_shape *shape, int query, const double *x, const double *y, const double *z,
+                             const double *dx, const double *dy, const double *dz, double step_max, int64_t n, void *out)
+{
+    if (!shape) return vg_set_error(VG_ERR_ARG, "vg_query_host: shape is NULL");
+    if (query < qInside || query > qSafeOut) return vg_set_error(VG_ERR_ARG, "vg_query_host: unknown query");
+    const double *h[6] = { x, y, z, dx, dy, dz };
+    return run_host("vg_query_host", shape, nullptr, query, h, step_max, n, out, nullptr);
+}
+
+extern "C" int vg_compute_step_host(const vg_volume *volume, const double *x, const double *y, const double *z,
+                                    const double *dx, const double *dy, const double *dz, double step_max, int64_t n,
+                                    double *step, int32_t *hit)
+{
+    if (!volume) return vg_set_error(VG_ERR_ARG, "vg_compute_step_host: volume is NULL");
+    const double *h[6] = { x, y, z, dx, dy, dz };
+    return run_host("vg_compute_step_host", nullptr, volume, -1, h, step_max, n, step, hit);
+}

@@ -9,6 +9,8 @@
 #pragma once
 #include "vg_shapes.cuh"
 
+#include <atomic>
+
 namespace vg {
 
 struct Tracks {
@@ -16,6 +18,8 @@ struct Tracks {
 };
 
 constexpr int kBlock = 256;
+
+extern std::atomic<int64_t> g_launches; // kernel launches made by the library (vg_launch_count)
 
 template <class S, int Q>
 VG_DEV void eval_store(const typename S::P &p, double x, double y, double z, double dx, double dy, double dz,
@@ -87,6 +91,7 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
         unsigned grid = unsigned((n + kBlock - 1) / kBlock);
         query_kernel<S, Q, 1><<<grid, kBlock, 0, stream>>>(p, t, step_max, n, out);
     }
+    g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError();
 }
 

@@ -171,6 +171,7 @@ static cudaError_t launch_nav(const SolidU &mother, const Daughter *table_dev, i
     int64_t cap = int64_t(sm_count) * per_sm; // persistent: one resident wave, a multiple of the SM count
     unsigned grid = unsigned(want < cap ? want : cap);
     nav_kernel<kStep><<<grid, kNavBlock, smem, s>>>(mother, table_dev, nd, t, step_max, n, out, hit);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
     return cudaGetLastError();
 }
 

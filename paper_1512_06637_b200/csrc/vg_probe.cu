@@ -44,6 +44,7 @@ cudaError_t probe_fp64_fma_rate(int launches, double *fma_per_s, cudaStream_t s)
     fma_chain_kernel<<<grid, 256, 0, s>>>(1.0, sink); // warm-up
     cudaEventRecord(e0, s);
     for (int i = 0; i < launches; ++i) fma_chain_kernel<<<grid, 256, 0, s>>>(1.0 + i, sink);
+    g_launches.fetch_add(launches + 1, std::memory_order_relaxed);
     cudaEventRecord(e1, s);
     err = cudaEventSynchronize(e1);
     float ms = 0;
@@ -60,6 +61,7 @@ cudaError_t probe_fp64_fma_rate(int launches, double *fma_per_s, cudaStream_t s)
 cudaError_t probe_empty_launch(int launches, cudaStream_t s)
 {
     for (int i = 0; i < launches; ++i) empty_kernel<<<1, 32, 0, s>>>();
+    g_launches.fetch_add(launches, std::memory_order_relaxed);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,33 @@
+"""Parity policy GPU vs oracle (BASELINE.json north_star):
+Inside classes and hit indices bit-exact; +inf and -1 sentinels bit-exact; finite distances / safeties pass iff
+|g - o| <= max(1e-9, 1e-12 |o|).  No whitelist."""
+import numpy as np
+
+ABS_TOL = 1e-9   # BASELINE.json: "within 1e-12 relative or 1e-9 absolute"
+REL_TOL = 1e-12
+
+
+def assert_int_equal(g, o, what):
+    g, o = np.asarray(g), np.asarray(o)
+    assert g.shape == o.shape, what
+    bad = np.flatnonzero(g != o)
+    assert bad.size == 0, "%s: %d of %d differ, first at %d: gpu %r oracle %r" % (
+        what, bad.size, g.size, bad[0] if bad.size else -1, g[bad[:5]], o[bad[:5]])
+
+
+def assert_real_close(g, o, what):
+    g, o = np.asarray(g, dtype=np.float64), np.asarray(o, dtype=np.float64)
+    assert g.shape == o.shape, what
+    assert not np.isnan(g).any(), "%s: NaN in the GPU result" % what
+    for name, sentinel in (("+inf", np.inf), ("-1", -1.0)):
+        mg, mo = g == sentinel, o == sentinel
+        bad = np.flatnonzero(mg != mo)
+        assert bad.size == 0, "%s: %s masks differ at %d of %d tracks, first %d: gpu %r oracle %r" % (
+            what, name, bad.size, g.size, bad[0] if bad.size else -1, g[bad[:5]], o[bad[:5]])
+    fin = np.isfinite(o)
+    err = np.abs(g[fin] - o[fin])
+    tol = np.maximum(ABS_TOL, REL_TOL * np.abs(o[fin]))
+    bad = np.flatnonzero(err > tol)
+    assert bad.size == 0, "%s: %d of %d finite values out of tolerance, worst |err| %.3e (gpu %r oracle %r)" % (
+        what, bad.size, int(fin.sum()), err.max() if err.size else 0.0, g[fin][bad[:3]], o[fin][bad[:3]])
+    return float(err.max()) if err.size else 0.0

@@ -1,0 +1,185 @@
+"""CPU-side checks of the boundary (no GPU): libvg.so loads, exports every symbol include/vg.h declares, validates
+parameters, treats n == 0 as a no-op and FAILS LOUDLY (VG_ERR_CUDA) when asked to compute without a CUDA device;
+plus the world_size-2 gloo test of the track sharding."""
+import ctypes as C
+import math
+import os
+import re
+import socket
+
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "vg.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(vg_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_1512_06637_b200 as vg
+    lib = C.CDLL(vg.LIB_PATH)
+    names = declared_symbols()
+    assert len(names) >= 18 and "vg_compute_step" in names and "vg_query_host" in names
+    for name in names:
+        assert hasattr(lib, name), "libvg.so does not export %s" % name
+
+
+def test_oracle_and_cuda_path_share_no_code():
+    """Neither side includes or imports the other (the independence the parity claim rests on)."""
+    csrc = os.path.join(ROOT, "paper_1512_06637_b200", "csrc")
+    for f in os.listdir(csrc):
+        for inc in re.findall(r'#include\s*[<"]([^>"]+)[>"]', open(os.path.join(csrc, f)).read()):
+            assert "oracle" not in inc.lower(), (f, inc)
+            if "/" in inc:
+                assert inc == "../../include/vg.h", (f, inc)
+    for f in ("__init__.py", "build.py", "shard.py"):
+        src = open(os.path.join(ROOT, "paper_1512_06637_b200", f)).read()
+        assert "import oracle" not in src and "from oracle" not in src
+    osrc = open(os.path.join(ROOT, "oracle", "vg_oracle.c")).read()
+    assert "vg.h" not in osrc and "csrc" not in re.sub(r"/\*.*?\*/", "", osrc, flags=re.S)
+    opy = open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "paper_1512_06637_b200" not in opy.split('"""', 2)[2]
+
+
+BAD = [
+    (0, [5, 5]), (0, [5, -1, 5]), (0, [5, 0, 5]), (0, [5, math.nan, 5]), (0, [5, math.inf, 5]),
+    (1, [0]), (1, [-2]), (1, [1, 2]),
+    (2, [5, 4, 15, 0, 1]), (2, [-1, 4, 15, 0, 1]), (2, [1, 4, 0, 0, 1]), (2, [1, 4, 15, 0, 0]), (2, [1, 4, 15, 0]),
+    (3, [2, 1, 4, 12, 20, 0, 1]), (3, [2, 6, 4, 3, 20, 0, 1]), (3, [2, 6, 4, 12, -20, 0, 1]), (3, [2, 6, 4, 12, 20, 0, -1]),
+    (4, [5, 10, 7, 3, 0]), (4, [5, 10, 7, 3]), (4, [0, 10, 7, 3, 15]),
+    (5, [0, 6.3, 1, 0, 0, 5]), (5, [0, 6.3, 2, 0, 0, 5, 0, 0, 5]), (5, [0, 6.3, 2, 1, 0, 5, 0, 0, 5]),
+    (5, [0, 6.3, 2, 0, 6, 5, 1, 0, 5]), (5, [0, 6.3, 2.5, 0, 0, 5, 1, 0, 5]), (5, [0, 6.3, 3, 0, 0, 5, 1, 0, 5]),
+    (5, [0, 6.3, 33] + [v for i in range(33) for v in (float(i), 0.0, 5.0)]), (9, [1, 2, 3]),
+]
+
+
+@pytest.mark.parametrize("kind,params", BAD)
+def test_invalid_shape_parameters_are_rejected(kind, params):
+    import paper_1512_06637_b200 as vg
+    with pytest.raises(vg.VgError) as e:
+        vg.Shape(kind, params)
+    assert e.value.code in (vg.ERR_PARAM, vg.ERR_ARG)
+
+
+GOOD = [(0, [5, 5, 5]), (1, [20]), (2, [5, 10, 15, 0, 4 * math.pi / 3]), (2, [0, 10, 15, 0, 7]),
+        (3, [2, 6, 4, 12, 20, 0, 2 * math.pi]), (3, [0, 6, 0, 12, 20, 1, 2]), (4, [5, 10, 7, 3, 15]),
+        (5, [0, 6.3, 2, -1, 0, 5, 1, 0, 5]),
+        (5, [0, 6.3, 32] + [v for i in range(32) for v in (float(i), 0.0, 5.0)])]
+
+
+@pytest.mark.parametrize("kind,params", GOOD)
+def test_valid_shapes_create_without_a_gpu(kind, params):
+    import paper_1512_06637_b200 as vg
+    s = vg.Shape(kind, params)
+    assert vg._lib.vg_shape_kind(s._h) == kind
+
+
+def test_null_handles_and_zero_tracks():
+    import paper_1512_06637_b200 as vg
+    lib = vg._lib
+    s = vg.Shape(vg.BOX, [5, 5, 5])
+    null = C.c_void_p(0)
+    assert lib.vg_inside(s._h, null, null, null, 0, null, null) == vg.OK         # n == 0: nothing inspected
+    assert lib.vg_distance_to_in(s._h, null, null, null, null, null, null, 1e30, 0, null, null) == vg.OK
+    assert lib.vg_inside(null, null, null, null, 0, null, null) == vg.ERR_ARG    # NULL shape
+    assert lib.vg_inside(s._h, null, null, null, 4, null, null) == vg.ERR_ARG    # NULL arrays with n > 0
+    assert lib.vg_inside(s._h, null, null, null, -1, null, null) == vg.ERR_ARG
+    assert b"NULL" in lib.vg_last_error() or b"n < 0" in lib.vg_last_error()
+    odd = C.c_void_p(0x1004)
+    assert lib.vg_safety_to_in(s._h, odd, odd, odd, 4, odd, null) == vg.ERR_ARG  # not 8-byte aligned
+    lib.vg_shape_destroy(null)
+    lib.vg_volume_destroy(null)
+    assert lib.vg_shape_kind(null) == vg.ERR_ARG
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the behaviour WITHOUT a CUDA device")
+def test_compute_calls_fail_loudly_without_a_gpu():
+    """No CPU fallback behind the interface (include/vg.h): a launch without a device is VG_ERR_CUDA."""
+    import paper_1512_06637_b200 as vg
+    lib = vg._lib
+    s = vg.Shape(vg.BOX, [5, 5, 5])
+    fake = C.c_void_p(0x10000)  # never dereferenced on the host
+    assert lib.vg_inside(s._h, fake, fake, fake, 16, fake, C.c_void_p(0)) == vg.ERR_CUDA
+    assert lib.vg_last_error() != b""
+    x = torch.zeros(4, dtype=torch.float64)
+    with pytest.raises(TypeError):
+        s.inside(x, x, x)
+    with pytest.raises(vg.VgError):
+        s.query_host("inside", x, x, x, out=torch.zeros(4, dtype=torch.int32))
+    m = vg.Shape(vg.BOX, [10, 10, 10])
+    with pytest.raises(vg.VgError):
+        vg.Volume(m, [s], [[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]])  # needs device memory for the table
+
+
+# ------------------------------------------------------------------------------------------ sharding (gloo)
+
+def test_track_ranges_partition_the_tracks():
+    from paper_1512_06637_b200.shard import track_range
+    for n in (0, 1, 7, 65536, 4194304, 4194305):
+        for world in (1, 2, 3, 8):
+            r = [track_range(n, g, world) for g in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == n
+            assert all(r[g][1] == r[g + 1][0] for g in range(world - 1))
+            sizes = [b - a for a, b in r]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        track_range(10, 2, 2)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    return port
+
+
+def _worker(rank, world, port, n, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import numpy as np
+    import oracle as O
+    import workloads as W
+    from paper_1512_06637_b200.shard import barrier, max_over_ranks, sum_over_ranks, track_range
+    sc = W.shape_cases(0)[0]
+    t = sc.tracks(n)                       # every rank draws the same seeded tracks ...
+    lo, hi = track_range(n, rank, world)   # ... and answers its own contiguous range, no exchange
+    s = O.Shape(sc.kind, sc.params)        # (the oracle stands in for the kernels on this CPU-only test)
+    part = s.distance_to_in(*[a[lo:hi] for a in t], 1e30)
+    barrier()
+    tmax = max_over_ranks(0.5 + rank)
+    total = sum_over_ranks(hi - lo)
+    q.put((rank, lo, hi, part, tmax, total))
+    dist.destroy_process_group()
+
+
+def test_two_ranks_shard_without_exchange_and_reduce_the_timing():
+    import numpy as np
+    import sys
+    sys.path.insert(0, ROOT)
+    import oracle as O
+    import workloads as W
+    n, world = 10001, 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, n, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted([q.get(timeout=120) for _ in range(world)], key=lambda r: r[0])
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    sc = W.shape_cases(0)[0]
+    t = sc.tracks(n)
+    whole = O.Shape(sc.kind, sc.params).distance_to_in(*t, 1e30)
+    assert got[0][1] == 0 and got[0][2] == got[1][1] and got[1][2] == n
+    assert np.array_equal(np.concatenate([got[0][3], got[1][3]]), whole)
+    assert all(r[4] == 1.5 for r in got) and all(r[5] == n for r in got)

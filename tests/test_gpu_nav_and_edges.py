@@ -1,0 +1,366 @@
+"""GPU parity, part 2: the hand-worked examples through the CUDA path, degenerate rays, step_max, the navigation
+step of BASELINE.json configs[4], the host-buffer entry points, streams."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+from parity import assert_int_equal, assert_real_close
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TWO_PI = 2 * math.pi
+PI = math.pi
+
+
+@pytest.fixture(scope="module")
+def vg():
+    import paper_1512_06637_b200 as m
+    assert torch.cuda.is_available(), "the CUDA path needs a GPU; there is no fallback"
+    return m
+
+
+def dev(arrs):
+    return [torch.from_numpy(np.ascontiguousarray(np.asarray(a, dtype=np.float64))).cuda() for a in arrs]
+
+
+def oracle_band(s):
+    return lambda x, y, z: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND
+
+
+# ------------------------------------------------------------- worked examples E1-E21 (tests/golden) on the GPU
+
+def _parse_golden():
+    path = os.path.join(os.path.dirname(__file__), "golden", "worked_examples.txt")
+    names = {"box": W.BOX, "orb": W.ORB, "tube": W.TUBE, "cone": W.CONE, "trd": W.TRD}
+    sym = {"4PI3": 4 * PI / 3, "2PI": 2 * PI, "inf": math.inf}
+    val = lambda t: sym[t] if t in sym else float(t)
+    rows = []
+    for line in open(path):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        eid, shape, p, d, res = [f.strip() for f in line.split("|")]
+        st = shape.split()
+        rows.append((eid, names[st[0]], [val(t) for t in st[1:]], [val(t) for t in p.split()],
+                     None if d == "-" else [val(t) for t in d.split()],
+                     {k: val(v) for k, v in (kv.split("=") for kv in res.split())}))
+    return rows
+
+
+@pytest.mark.parametrize("row", _parse_golden(), ids=lambda r: r[0])
+def test_worked_examples_on_gpu(vg, row):
+    eid, kind, par, p, d, res = row
+    s = vg.Shape(kind, par)
+    pt = dev([[v] for v in p])
+    dt = dev([[v] for v in d]) if d is not None else None
+    for q, want in res.items():
+        if q == "inside":
+            got = float(s.inside(*pt).cpu()[0])
+        elif q.startswith("safety"):
+            got = float(getattr(s, q)(*pt).cpu()[0])
+        else:
+            got = float(getattr(s, q)(*pt, *dt, 1e30).cpu()[0])
+        if math.isinf(want):
+            assert got == want, (eid, q, got)
+        else:
+            assert abs(got - want) <= max(1e-9, 1e-12 * abs(want)), (eid, q, got, want)
+
+
+# ------------------------------------------------------------------------------------------- degenerate rays
+
+SHAPES = {
+    "box": (W.BOX, [5.0, 5.0, 5.0]),
+    "orb": (W.ORB, [20.0]),
+    "tube": (W.TUBE, [5.0, 10.0, 15.0, 0.0, 4 * PI / 3]),
+    "cone": (W.CONE, [2.0, 6.0, 4.0, 12.0, 20.0, 0.0, TWO_PI]),
+    "trd": (W.TRD, [5.0, 10.0, 7.0, 3.0, 15.0]),
+    "polycone": (W.POLYCONE, W.polycone_params(W.config_seed(3, 0))),
+}
+
+
+@pytest.mark.parametrize("name", list(SHAPES))
+def test_axis_aligned_and_planar_directions(vg, name):
+    """Directions with one or two components exactly zero (hard part H4): the select-based
+    kernels must give what the oracle's explicit branches give."""
+    kind, par = SHAPES[name]
+    so, sg = O.Shape(kind, par), vg.Shape(kind, par)
+    c, h = W.bounding_half(kind, par)
+    x, y, z, dx, dy, dz = W.draw_tracks(5, 60000, c, tuple(1.5 * v for v in h), oracle_band(so))
+    n = len(x)
+    rng = np.random.default_rng(1)
+    mode = rng.integers(0, 9, n)
+    sgn = rng.choice([-1.0, 1.0], n)
+    ang = rng.uniform(0, TWO_PI, n)
+    for m, (a, b, c_) in enumerate([(1, 0, 0), (0, 1, 0), (0, 0, 1)]):
+        k = mode == m
+        dx[k], dy[k], dz[k] = a * sgn[k], b * sgn[k], c_ * sgn[k]
+    k = mode == 3
+    dx[k], dy[k], dz[k] = np.cos(ang[k]), np.sin(ang[k]), 0.0
+    k = mode == 4
+    dx[k], dy[k], dz[k] = np.cos(ang[k]), 0.0, np.sin(ang[k])
+    k = mode == 5
+    dx[k], dy[k], dz[k] = 0.0, np.cos(ang[k]), np.sin(ang[k])
+    k = mode == 6  # negative zeros
+    dx[k], dy[k], dz[k] = -0.0, sgn[k], -0.0
+    t = (x, y, z, dx, dy, dz)
+    dt = dev(t)
+    for q in ("distance_to_in", "distance_to_out"):
+        o = getattr(so, q)(*t, W.STEP_MAX)
+        g = getattr(sg, q)(*dt, W.STEP_MAX).cpu().numpy()
+        assert_real_close(g, o, "%s %s degenerate directions" % (name, q))
+
+
+@pytest.mark.parametrize("name", list(SHAPES))
+def test_points_on_symmetry_axes_and_planes(vg, name):
+    """Points with exactly zero coordinates (rho = 0 on the axis of a solid of revolution, the mid-planes)."""
+    kind, par = SHAPES[name]
+    so, sg = O.Shape(kind, par), vg.Shape(kind, par)
+    c, h = W.bounding_half(kind, par)
+    x, y, z, dx, dy, dz = W.draw_tracks(6, 40000, c, tuple(1.5 * v for v in h))
+    rng = np.random.default_rng(2)
+    mode = rng.integers(0, 6, len(x))
+    x[(mode == 0) | (mode == 3)] = 0.0
+    y[(mode == 1) | (mode == 3)] = 0.0
+    z[mode == 2] = c[2]
+    keep = np.abs(so.sdf(x, y, z)) >= W.SURFACE_BAND
+    t = tuple(a[keep] for a in (x, y, z, dx, dy, dz))
+    dt = dev(t)
+    for q in W.QUERIES5:
+        if q.startswith("distance"):
+            o = getattr(so, q)(*t, W.STEP_MAX)
+            g = getattr(sg, q)(*dt, W.STEP_MAX).cpu().numpy()
+            assert_real_close(g, o, "%s %s axis points" % (name, q))
+        elif q == "inside":
+            assert_int_equal(sg.inside(*dt[:3]).cpu().numpy(), so.inside(*t[:3]), "%s inside axis points" % name)
+        else:
+            assert_real_close(getattr(sg, q)(*dt[:3]).cpu().numpy(), getattr(so, q)(*t[:3]), "%s %s axis points" % (name, q))
+
+
+@pytest.mark.parametrize("name", list(SHAPES))
+def test_step_max_turns_far_hits_into_misses(vg, name):
+    kind, par = SHAPES[name]
+    so, sg = O.Shape(kind, par), vg.Shape(kind, par)
+    c, h = W.bounding_half(kind, par)
+    t = W.draw_tracks(8, 50001, c, tuple(1.5 * v for v in h), oracle_band(so))
+    dt = dev(t)
+    for step_max in (0.0, 3.0, 11.5, math.inf):
+        for q in ("distance_to_in", "distance_to_out"):
+            o = getattr(so, q)(*t, step_max)
+            g = getattr(sg, q)(*dt, step_max).cpu().numpy()
+            assert_real_close(g, o, "%s %s step_max=%r" % (name, q, step_max))
+
+
+def test_permuting_tracks_permutes_results(vg):
+    """the geometry calculations of different particles are independent of each other."""
+    kind, par = SHAPES["tube"]
+    sg = vg.Shape(kind, par)
+    c, h = W.bounding_half(kind, par)
+    t = W.draw_tracks(9, 70001, c, tuple(1.5 * v for v in h))
+    perm = np.random.default_rng(3).permutation(len(t[0]))
+    a = sg.distance_to_in(*dev(t), 1e30).cpu().numpy()
+    b = sg.distance_to_in(*dev([v[perm] for v in t]), 1e30).cpu().numpy()
+    assert np.array_equal(a[perm], b)
+
+
+def test_non_default_stream_and_concurrent_handles(vg):
+    kind, par = SHAPES["cone"]
+    so, sg = O.Shape(kind, par), vg.Shape(kind, par)
+    c, h = W.bounding_half(kind, par)
+    t = W.draw_tracks(10, 300001, c, tuple(1.5 * v for v in h), oracle_band(so))
+    dt = dev(t)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(s1):
+        a = sg.distance_to_in(*dt, 1e30)
+    with torch.cuda.stream(s2):
+        b = sg.safety_to_in(*dt[:3])
+    c_ = sg.distance_to_out(*dt, 1e30, stream=s1)
+    torch.cuda.synchronize()
+    assert_real_close(a.cpu().numpy(), so.distance_to_in(*t, 1e30), "stream s1")
+    assert_real_close(b.cpu().numpy(), so.safety_to_in(*t[:3]), "stream s2")
+    assert_real_close(c_.cpu().numpy(), so.distance_to_out(*t, 1e30), "explicit stream")
+
+
+def test_bad_arguments_raise(vg):
+    sg = vg.Shape(W.BOX, [5, 5, 5])
+    x = torch.zeros(8, dtype=torch.float64, device="cuda")
+    with pytest.raises(TypeError):
+        sg.inside(x.float(), x, x)
+    with pytest.raises(ValueError):
+        sg.inside(x, x[:4], x)
+    with pytest.raises(TypeError):
+        sg.inside(x.cpu(), x.cpu(), x.cpu())
+    with pytest.raises(vg.VgError):
+        sg.distance_to_in(x, x, x, x, x, x, step_max=-1.0)
+    with pytest.raises(vg.VgError):
+        sg.distance_to_in(x, x, x, x, x, x, step_max=float("nan"))
+
+
+# ------------------------------------------------------------------------------ navigation (configs[4])
+
+def build_volumes(vg, nav, order=None, nd=None):
+    idx = list(range(len(nav.daughter_kinds))) if order is None else list(order)
+    if nd is not None:
+        idx = idx[:nd]
+    mo = O.Shape(nav.mother_kind, nav.mother_params)
+    mg = vg.Shape(nav.mother_kind, nav.mother_params)
+    do = [O.Shape(nav.daughter_kinds[i], nav.daughter_params[i]) for i in idx]
+    dg = [vg.Shape(nav.daughter_kinds[i], nav.daughter_params[i]) for i in idx]
+    xf = nav.xforms[idx] if idx else np.zeros((0, 12))
+    return O.Volume(mo, do, xf), vg.Volume(mg, dg, xf)
+
+
+def nav_tracks(nav, vol, n, seed=None):
+    band = lambda x, y, z: vol.safety(x, y, z) < W.SURFACE_BAND
+    return W.draw_tracks(nav.seed if seed is None else seed, n, nav.center, nav.half, band)
+
+
+def check_step(vo, vgv, t, step_max, what):
+    so, ho = vo.compute_step(*t, step_max)
+    sg, hg = vgv.compute_step(*dev(t), step_max)
+    torch.cuda.synchronize()
+    assert_int_equal(hg.cpu().numpy(), ho, what + " hit")
+    assert_real_close(sg.cpu().numpy(), so, what + " step")
+    return so, ho
+
+
+def test_config4_full_size(vg):
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    t = nav_tracks(nav, vo, nav.sizes[-1])
+    so, ho = check_step(vo, vgv, t, W.STEP_MAX, "cfg4")
+    frac = (ho >= 0).mean()
+    assert 0.15 < frac < 0.30 and len(set(ho.tolist())) == 65  # every daughter and the mother are hit
+
+
+@pytest.mark.parametrize("n", [1, 2, 127, 128, 129, 100003])
+def test_config4_ragged(vg, n):
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    t = nav_tracks(nav, vo, n, seed=nav.seed + 1)
+    check_step(vo, vgv, t, W.STEP_MAX, "cfg4 n=%d" % n)
+
+
+@pytest.mark.parametrize("step_max", [0.0, 5.0, 40.0, 150.0, math.inf])
+def test_physics_step_limits_the_geometric_step(vg, step_max):
+    """the smaller of the physics step and the distance to the border wins (hit = -2)."""
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    t = nav_tracks(nav, vo, 200001, seed=nav.seed + 2)
+    so, ho = check_step(vo, vgv, t, step_max, "cfg4 step_max=%r" % step_max)
+    if step_max < 100:
+        assert (ho == -2).any()
+
+
+@pytest.mark.parametrize("nd", [0, 1, 2, 7, 33])
+def test_fewer_daughters_and_permuted_order(vg, nd):
+    nav = W.navigator_case()
+    order = np.random.default_rng(4).permutation(64)
+    vo, vgv = build_volumes(vg, nav, order=order, nd=nd)
+    t = nav_tracks(nav, vo, 150001, seed=nav.seed + 3)
+    check_step(vo, vgv, t, W.STEP_MAX, "nd=%d" % nd)
+
+
+def test_tracks_that_break_the_contract(vg):
+    """Tracks outside the mother get (-1, -1); a daughter the track is inside of is skipped (R13)."""
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    x, y, z, dx, dy, dz = W.draw_tracks(99, 120001, (0, 0, 0), (130, 130, 130))
+    keep = (np.abs(vo.mother.sdf(x, y, z)) >= 1e-6)
+    for d, xf in zip(vo.daughters, vo.xforms):
+        M = xf.reshape(3, 4)
+        lx, ly, lz = (M[i, 0] * x + M[i, 1] * y + M[i, 2] * z + M[i, 3] for i in range(3))
+        keep &= np.abs(d.sdf(lx, ly, lz)) >= 1e-6
+    t = tuple(a[keep] for a in (x, y, z, dx, dy, dz))
+    so, ho = check_step(vo, vgv, t, W.STEP_MAX, "contract violations")
+    assert (so == -1.0).any()
+
+
+def test_mixed_daughter_kinds_and_mothers(vg):
+    """Daughters of every supported kind (box, orb, tube segment, cone segment, trd) in a tube mother."""
+    rng = np.random.default_rng(12)
+    kinds = [W.BOX, W.ORB, W.TUBE, W.CONE, W.TRD, W.TUBE, W.CONE, W.ORB]
+    pars = [[3, 4, 5], [5], [2, 5, 4, 0.3, 4.0], [1, 3, 2, 5, 4, 0.0, TWO_PI], [2, 4, 3, 1, 5], [0, 4, 6, 0, TWO_PI],
+            [0, 3, 2, 5, 4, 1.0, 2.5], [3]]
+    centers = [(-20, -20, -20), (20, -20, -20), (-20, 20, -20), (20, 20, -20), (-20, -20, 20), (20, -20, 20),
+               (-20, 20, 20), (20, 20, 20)]
+    xf = []
+    for c in centers:
+        u1, u2, u3 = rng.random(3)
+        q = (math.sqrt(1 - u1) * math.sin(TWO_PI * u2), math.sqrt(1 - u1) * math.cos(TWO_PI * u2),
+             math.sqrt(u1) * math.sin(TWO_PI * u3), math.sqrt(u1) * math.cos(TWO_PI * u3))
+        xf.append(W.placement(W.quaternion_to_matrix(q), c))
+    xf = np.stack(xf)
+    for mk, mp in ((W.TUBE, [0, 45, 40, 0, TWO_PI]), (W.ORB, [50]), (W.TRD, [40, 45, 42, 38, 40]),
+                   (W.CONE, [0, 45, 0, 50, 40, 0, TWO_PI])):
+        vo = O.Volume(O.Shape(mk, mp), [O.Shape(k, p) for k, p in zip(kinds, pars)], xf)
+        vgv = vg.Volume(vg.Shape(mk, mp), [vg.Shape(k, p) for k, p in zip(kinds, pars)], xf)
+        t = W.draw_tracks(31, 120001, (0, 0, 0), (36, 36, 36), lambda x, y, z: vo.safety(x, y, z) < 1e-6)
+        so, ho = check_step(vo, vgv, t, W.STEP_MAX, "mixed kinds mother=%d" % mk)
+        assert len(set(ho.tolist())) == 9
+        sg = vgv.safety(*dev(t[:3])).cpu().numpy()
+        assert_real_close(sg, vo.safety(*t[:3]), "volume safety mother=%d" % mk)
+
+
+def test_volume_safety_config4(vg):
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    t = nav_tracks(nav, vo, 300001, seed=nav.seed + 5)
+    assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), vo.safety(*t[:3]), "volume safety")
+
+
+def test_volume_create_rejects_bad_input(vg):
+    m = vg.Shape(W.BOX, [10, 10, 10])
+    d = vg.Shape(W.BOX, [1, 1, 1])
+    bad = [[2, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]]
+    with pytest.raises(vg.VgError):
+        vg.Volume(m, [d], bad)
+    pc = vg.Shape(W.POLYCONE, W.polycone_params(1))
+    with pytest.raises(vg.VgError):
+        vg.Volume(m, [pc], [[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]])
+
+
+# ------------------------------------------------------------------------------- host-buffer entry points
+
+@pytest.mark.parametrize("n", [1, 4097, 65536, 1048576 + 3, 3 * 1048576 + 11])
+def test_host_entry_points_match_the_oracle(vg, n):
+    sc = W.shape_cases(1)[0]
+    so, sg = O.Shape(sc.kind, sc.params), vg.Shape(sc.kind, sc.params)
+    t = sc.tracks(n, band=oracle_band(so))
+    ht = [torch.from_numpy(a).pin_memory() for a in t]
+    for q in W.QUERIES5:
+        g = sg.query_host(q, *ht, step_max=W.STEP_MAX).numpy()
+        if q.startswith("distance"):
+            assert_real_close(g, getattr(so, q)(*t, W.STEP_MAX), "host %s" % q)
+        elif q == "inside":
+            assert_int_equal(g, so.inside(*t[:3]), "host inside")
+        else:
+            assert_real_close(g, getattr(so, q)(*t[:3]), "host %s" % q)
+    # pageable memory works as well
+    g = sg.query_host("distance_to_in", *[torch.from_numpy(a) for a in t], step_max=W.STEP_MAX,
+                      out=torch.empty(n, dtype=torch.float64)).numpy()
+    assert_real_close(g, so.distance_to_in(*t, W.STEP_MAX), "host pageable")
+
+
+def test_host_compute_step(vg):
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    t = nav_tracks(nav, vo, 2 * 1048576 + 5, seed=nav.seed + 6)
+    so, ho = vo.compute_step(*t, W.STEP_MAX)
+    sg, hg = vgv.compute_step_host(*[torch.from_numpy(a).pin_memory() for a in t], step_max=W.STEP_MAX)
+    assert_int_equal(hg.numpy(), ho, "host compute_step hit")
+    assert_real_close(sg.numpy(), so, "host compute_step step")
+
+
+def test_library_launch_counter_counts_kernels(vg):
+    sg = vg.Shape(W.BOX, [5, 5, 5])
+    x = torch.zeros(1000, dtype=torch.float64, device="cuda")
+    before = vg.vg_launch_count()
+    for _ in range(7):
+        sg.safety_to_in(x, x, x)
+    assert vg.vg_launch_count() - before == 7
