@@ -1,0 +1,464 @@
+#!/usr/bin/env python
+"""bench.py -- tracks/s per query on one B200 (BASELINE.json `metric`) for the geometry hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-detail]
+
+A "step" is one pass of the hot path over one batch of synthetic tracks of BASELINE.json configs[1] (tube segment
+rmin 5, rmax 10, dz 15, phi 0..4pi/3, N = 1,048,576 tracks): Inside, DistanceToIn, DistanceToOut, SafetyToIn and
+SafetyToOut, five kernel launches through the C ABI.  `value` = tracks x queries / second with the tracks resident
+in HBM; every launch reads a different copy of the batch (rotating buffer sets whose total size is several times
+the 126 MB L2), so no launch finds its inputs in L2.  The K timed steps are replays of CUDA graphs captured from
+the same C-ABI calls (the launches are microseconds long; eager launches would time the Python interpreter).
+`e2e` is the same step through the host-buffer entry points (pinned host arrays in, host arrays out, copies
+inside the timed region).  `detail` adds every (config, shape, query) of BASELINE.json with its roofline fraction.
+`--impl reference` times the oracle (oracle/, plain scalar CPU code) on the host cores for the same step.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402  (seeded input generators; no arithmetic of the method)
+
+METRIC = "tracks/sec per query per shape (1 B200) and fraction of HBM / FP64 roofline"
+UNIT = "track-queries/s"
+# algorithmic bytes per track: SoA inputs read once + one result written once
+BYTES = {"inside": 24 + 4, "safety_to_in": 24 + 8, "safety_to_out": 24 + 8, "distance_to_in": 48 + 8,
+         "distance_to_out": 48 + 8, "compute_step": 48 + 12}
+L2_BYTES = 126e6
+HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------- clock sampler
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the GPU is under the bench load."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+        self.marks = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0, t1, load0, load1):
+        def pick(a, b):
+            return [r for ts, r in self.rows if a <= ts <= b and len(r) >= 7]
+        rows, window = pick(t0, t1), "timed region"
+        if len(rows) < 3:
+            rows, window = pick(load0, load1), "bench load phase (timed region shorter than the sampling period)"
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "window": "nvidia-smi unavailable"}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows), "window": window}
+
+
+# ------------------------------------------------------------------------------------ device-resident cases
+
+class Case:
+    """One solid (or the navigation volume) with its seeded tracks resident in HBM as `nsets` rotating copies."""
+
+    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None):
+        self.vg, self.torch, self.name, self.n, self.queries = vg, torch, name, int(n), tuple(queries)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        if nav is not None:
+            self.kind = "navigator"
+            mother = vg.Shape(nav.mother_kind, nav.mother_params)
+            daughters = [vg.Shape(k, p) for k, p in zip(nav.daughter_kinds, nav.daughter_params)]
+            self.handle = vg.Volume(mother, daughters, nav.xforms)
+            seed, center, half = nav.seed + seed_shift, nav.center, nav.half
+            # surface-band rejection with the library's own safety (the product path never touches oracle/)
+            band = lambda x, y, z: self._gpu3(self.handle.safety, x, y, z) < W.SURFACE_BAND
+        else:
+            self.kind = W.KIND_NAME[shape.kind]
+            self.handle = vg.Shape(shape.kind, shape.params)
+            seed, center, half = shape.seed + seed_shift, shape.center, shape.half
+            band = lambda x, y, z: np.abs(self._gpu3(self.handle.safety_to_in, x, y, z)) < W.SURFACE_BAND
+        self.host = W.draw_tracks(seed, self.n, center, half, band)
+        per_set = 48 * self.n
+        self.nsets = int(min(16, max(2, -(-int(4 * L2_BYTES) // per_set))))
+        self.cold = self.nsets * per_set >= 2 * L2_BYTES
+        base = [torch.from_numpy(a).to(dev) for a in self.host]
+        self.sets = [base] + [[a.clone() for a in base] for _ in range(self.nsets - 1)]
+        self.outd = [torch.empty(self.n, dtype=torch.float64, device=dev) for _ in range(self.nsets)]
+        self.outi = [torch.empty(self.n, dtype=torch.int32, device=dev) for _ in range(self.nsets)]
+        self.cursor = 0
+
+    def _gpu3(self, fn, x, y, z):
+        t = self.torch
+        d = [t.from_numpy(np.ascontiguousarray(a)).cuda() for a in (x, y, z)]
+        return fn(*d).cpu().numpy()
+
+    def launch(self, q):
+        """One C-ABI call of query `q` on the next buffer set (enqueue only)."""
+        k = self.cursor
+        self.cursor = (k + 1) % self.nsets
+        s = self.sets[k]
+        if q == "compute_step":
+            self.handle.compute_step(*s, step_max=W.STEP_MAX, step=self.outd[k], hit=self.outi[k])
+        elif q == "inside":
+            self.handle.inside(*s[:3], out=self.outi[k])
+        elif q in ("distance_to_in", "distance_to_out"):
+            self.handle.query(q, *s, step_max=W.STEP_MAX, out=self.outd[k])
+        else:
+            self.handle.query(q, *s[:3], out=self.outd[k])
+
+    def step(self):
+        for q in self.queries:
+            self.launch(q)
+
+
+def capture_steps(torch, case, with_events):
+    """CUDA graphs of one step each, as many as it takes for the buffer-set rotation to come round; every kernel
+    node is bracketed by external timing events when the torch build supports them."""
+    nq = len(case.queries)
+    ngraphs = case.nsets  # after nsets steps every launch position has used every set
+    graphs, events = [], []
+    case.cursor = 0
+    case.step()  # eager warm-up before capture (lazy attribute / occupancy queries happen here)
+    torch.cuda.synchronize()
+    case.cursor = 0
+    for _ in range(ngraphs):
+        g = torch.cuda.CUDAGraph()
+        ev = [torch.cuda.Event(enable_timing=True, external=True) for _ in range(nq + 1)] if with_events else []
+        with torch.cuda.graph(g):
+            for j, q in enumerate(case.queries):
+                if with_events:
+                    ev[j].record()
+                case.launch(q)
+            if with_events:
+                ev[nq].record()
+        graphs.append(g)
+        events.append(ev)
+    return graphs, events
+
+
+def time_query_alone(torch, case, q, min_ms=30.0):
+    """Average duration of one launch of `q` (cold inputs): a graph of nsets launches over the rotating sets,
+    replayed between two CUDA events on the launching stream until >= min_ms have been timed."""
+    case.cursor = 0
+    case.launch(q)
+    torch.cuda.synchronize()
+    case.cursor = 0
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for _ in range(case.nsets):
+            case.launch(q)
+    for _ in range(3):
+        g.replay()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps, ms = 4, 0.0
+    while True:
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(reps):
+            g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        if ms >= min_ms or reps >= 4096:
+            break
+        reps *= 4
+    return ms * 1e-3 / (reps * case.nsets)
+
+
+# ------------------------------------------------------------------------------------------ the oracle legs
+
+def oracle_step(O, shape, tracks, queries):
+    for q in queries:
+        if q in ("distance_to_in", "distance_to_out"):
+            getattr(shape, q)(*tracks, W.STEP_MAX)
+        else:
+            getattr(shape, q)(*tracks[:3])
+
+
+def cpu_baseline(seconds=10.0):
+    """The oracle as it stands, timed on this box's host cores on the tracks of configs[1] (all five queries)."""
+    import oracle as O
+    sc = W.shape_cases(1)[0]
+    s = O.Shape(sc.kind, sc.params)
+    t = sc.tracks(sc.sizes[-1], band=lambda x, y, z: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND)
+    oracle_step(O, s, t, sc.queries)  # warm-up (thread pool, page faults)
+    reps, t0 = 0, time.perf_counter()
+    while True:
+        oracle_step(O, s, t, sc.queries)
+        reps += 1
+        el = time.perf_counter() - t0
+        if el >= seconds:
+            break
+    return {"value": len(sc.queries) * len(t[0]) * reps / el, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": "%d repetitions of the five queries over all %d tracks of configs[1] (%.1f s of wall time, "
+                      "gcc -O2 -ffp-contract=off, OpenMP static)" % (reps, len(t[0]), el)}
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle on the host cores, same config / metric / unit (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle as O
+    sc = W.shape_cases(1)[0]
+    s = O.Shape(sc.kind, sc.params)
+    full = sc.tracks(sc.sizes[-1], band=lambda x, y, z: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND)
+    probe = [a[:65536] for a in full]
+    oracle_step(O, s, probe, sc.queries)
+    t0 = time.perf_counter()
+    oracle_step(O, s, probe, sc.queries)
+    per_track = (time.perf_counter() - t0) / 65536
+    budget = 120.0  # seconds for the whole --steps + --warmup run
+    n = int(min(len(full[0]), max(4096, budget / ((args.steps + args.warmup) * per_track))))
+    t = [np.ascontiguousarray(a[:n]) for a in full]
+    for _ in range(args.warmup):
+        oracle_step(O, s, t, sc.queries)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_step(O, s, t, sc.queries)
+    el = time.perf_counter() - t0
+    value = len(sc.queries) * n * args.steps / el
+    sample = "each step = the five queries over the first %d of the %d tracks of configs[1]" % (n, len(full[0]))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": el * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1]: tube segment rmin=5 rmax=10 dz=15 phi 0..4pi/3, five queries", "n_tracks": n,
+                       "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------- our arm
+
+# Algorithmic FP64 operations per track of the ALU-bound rows (DESIGN.md sec. 6 derives them from the formulas:
+# +, -, x, compare/min/max/select = 1, FMA = 2, divide / sqrt = 1), used for `bound: "alu"` entries of `detail`.
+ALGO_FLOP = {("polycone", "distance_to_in"): None, ("polycone", "safety_to_in"): None, ("navigator", "compute_step"): None}
+
+
+def roofline_entry(shape_kind, q, n, seconds, hbm_peak, fp64_fma_per_s):
+    gbs = BYTES[q] * n / seconds / 1e9
+    e = {"tracks_per_s": n / seconds, "us_per_launch": seconds * 1e6, "hbm_gbs": gbs, "hbm_frac": gbs / hbm_peak}
+    flop = ALGO_FLOP.get((shape_kind, q))
+    if flop:
+        e["bound"] = "alu"
+        e["fp64_tflops"] = flop * n / seconds / 1e12
+        e["fp64_frac"] = e["fp64_tflops"] * 1e12 / (2.0 * fp64_fma_per_s)
+    else:
+        e["bound"] = "hbm"
+    return e
+
+
+def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
+    """Every (config, shape, query) of BASELINE.json configs[0..4], each launch timed alone on cold inputs."""
+    rows = []
+    plan = []
+    for k in (0, 1, 2, 3):
+        for i, sc in enumerate(W.shape_cases(k)):
+            for n in sc.sizes:
+                plan.append((k, sc, n))
+    for k, sc, n in plan:
+        case = main_case if (k == 1) else Case(vg, torch, sc.name, n, sc.queries, shape=sc)
+        for q in sc.queries:
+            sec = time_query_alone(torch, case, q)
+            e = roofline_entry(case.kind, q, n, sec, hbm_peak, fma_rate)
+            e.update({"config": k, "shape": sc.name, "query": q, "n": n, "cold_inputs": case.cold})
+            rows.append(e)
+        if case is not main_case:
+            del case
+            torch.cuda.empty_cache()
+    nav = W.navigator_case()
+    case = Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step",), nav=nav)
+    sec = time_query_alone(torch, case, "compute_step")
+    e = roofline_entry("navigator", "compute_step", case.n, sec, hbm_peak, fma_rate)
+    e.update({"config": 4, "shape": "box(100)+64 daughters", "query": "compute_step", "n": case.n, "cold_inputs": case.cold})
+    rows.append(e)
+    return rows
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback "
+                         "(use --impl reference for the oracle on the host cores)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    import paper_1512_06637_b200 as vg
+    from paper_1512_06637_b200.shard import barrier, max_over_ranks, sum_over_ranks
+
+    hbm_peak, hbm_src = measured_peaks()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    load0 = time.time()
+    fma_rate = vg.vg_probe_fp64_fma_rate(30)
+
+    # weak scaling: every rank owns one full configs[1] batch (its own seed); no data-path collective
+    sc = W.shape_cases(1)[0]
+    case = Case(vg, torch, sc.name, sc.sizes[-1], sc.queries, seed_shift=1000 * rank, shape=sc)
+    try:
+        graphs, events = capture_steps(torch, case, True)
+        kernel_timing = "external CUDA events recorded around every kernel node of the timed graphs"
+    except Exception:
+        torch.cuda.synchronize()
+        graphs, events = capture_steps(torch, case, False)
+        kernel_timing = None
+    for i in range(max(args.warmup, 3)):
+        graphs[i % len(graphs)].replay()
+    torch.cuda.synchronize()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record()
+    for i in range(args.steps):
+        graphs[i % len(graphs)].replay()
+    e1.record()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    barrier()
+    ms = max_over_ranks(e0.elapsed_time(e1), "cuda")
+    tracks_all = sum_over_ranks(case.n, "cuda")
+    nq = len(case.queries)
+    value = tracks_all * nq * args.steps / (ms * 1e-3)
+
+    # per-kernel durations inside the timed region (the last replay of every graph that ran)
+    per_q = {}
+    used = range(min(len(graphs), args.steps))
+    if kernel_timing:
+        try:
+            for j, q in enumerate(case.queries):
+                per_q[q] = float(np.mean([events[g][j].elapsed_time(events[g][j + 1]) for g in used])) * 1e-3
+        except Exception:
+            per_q, kernel_timing = {}, None
+    if not kernel_timing:
+        kernel_timing = "each query alone: graph of nsets launches between two CUDA events (events inside graphs unsupported)"
+        for q in case.queries:
+            per_q[q] = time_query_alone(torch, case, q)
+
+    per_query = {q: roofline_entry(case.kind, q, case.n, per_q[q], hbm_peak, fma_rate) for q in case.queries}
+    dom = max(case.queries, key=lambda q: per_q[q])
+    roof = {"bound": "hbm", "kernel": "query_kernel<Tube, %s>" % dom, "achieved": per_query[dom]["hbm_gbs"],
+            "peak": hbm_peak, "unit": "GB/s", "frac": per_query[dom]["hbm_gbs"] / hbm_peak, "peak_source": hbm_src,
+            "traffic": None, "algorithmic_bytes_per_launch": BYTES[dom] * case.n,
+            "us_per_launch": per_q[dom] * 1e6, "share_of_step": per_q[dom] / sum(per_q.values()),
+            "kernel_timing": kernel_timing,
+            "step_hbm_frac": sum(BYTES[q] for q in case.queries) * case.n / (ms * 1e-3 / args.steps) / 1e9 / hbm_peak}
+
+    # end to end: pinned host arrays -> C-ABI host entry points -> host results, copies inside the timed region
+    host = [torch.from_numpy(a).pin_memory() for a in case.host]
+    hout_d = torch.empty(case.n, dtype=torch.float64).pin_memory()
+    hout_i = torch.empty(case.n, dtype=torch.int32).pin_memory()
+
+    def e2e_step():
+        for q in case.queries:
+            case.handle.query_host(q, *host, step_max=W.STEP_MAX, out=hout_i if q == "inside" else hout_d)
+
+    for _ in range(3):
+        e2e_step()
+    ke = max(3, min(args.steps, 20))
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(ke):
+        e2e_step()
+    w1 = time.perf_counter()
+    barrier()
+    e2e_s = max_over_ranks(w1 - w0, "cuda")
+    h2d = sum((48 if q.startswith("distance") else 24) for q in case.queries) * case.n
+    d2h = sum((4 if q == "inside" else 8) for q in case.queries) * case.n
+    e2e = {"value": tracks_all * nq * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+           "steps": ke, "ms_per_step": e2e_s * 1e3 / ke,
+           "api": "vg_query_host x5 (pinned host SoA in, pinned host result out, chunked copy/compute overlap)"}
+
+    launches_per_step = nq
+    detail = None
+    if world == 1 and not args.no_detail:
+        detail = detail_sweep(vg, torch, hbm_peak, fma_rate, case)
+    load1 = time.time()
+    sampler.stop()
+    clocks = sampler.summary(t0, t1, load0, load1)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "configs[1]: tube segment rmin=5 rmax=10 dz=15 phi 0..4pi/3, N=%d tracks per GPU, "
+                                       "Inside + DistanceToIn + DistanceToOut + SafetyToIn + SafetyToOut per step" % case.n,
+                           "n_tracks_per_gpu": case.n, "queries_per_step": nq, "step_max": W.STEP_MAX,
+                           "l2_policy": "inputs larger than L2: every launch reads the next of %d copies of the batch "
+                                        "(%d MB of inputs in rotation, L2 = 126 MB)" % (case.nsets, case.nsets * 48 * case.n // 10 ** 6),
+                           "launch": "CUDA graphs captured from the C-ABI calls, one graph per step",
+                           "parallelism": "tracks sharded over ranks, no collective" if world > 1 else "1 GPU"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+                "roofline": roof, "per_query": per_query,
+                "fp64_peak": {"fma_per_s": fma_rate, "tflops": 2 * fma_rate / 1e12,
+                              "how": "register-resident DFMA chains, vg_probe_fp64_fma_rate, same run"}}
+        if world == 1:
+            line["cpu_baseline"] = cpu_baseline()
+        if detail is not None:
+            line["detail"] = detail
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5000)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-detail", action="store_true", help="skip the per-config sweep (configs[0..4])")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world != args.gpus and world == 1 and args.gpus > 1:
+        raise SystemExit("bench.py: --gpus %d needs torchrun (one rank per GPU); see the module docstring" % args.gpus)
+    run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
