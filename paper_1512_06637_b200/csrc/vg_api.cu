@@ -27,8 +27,8 @@ struct vg_shape {
 
 struct vg_volume {
     SolidU mother;
-    int nd;
-    Daughter *table_dev;
+    NavMeta meta;
+    unsigned char *table_dev; // the blob described in vg_params.h
 };
 
 static thread_local char g_err[512] = "";
@@ -312,6 +312,24 @@ extern "C" int vg_safety_to_out(const vg_shape *s, const double *x, const double
 
 // ---------------------------------------------------------------------------------------------- navigation
 
+// radius of a sphere about the local origin that contains the solid (phi cuts ignored)
+static double bounding_radius(const SolidU &s)
+{
+    switch (s.kind) {
+    case kBox: return std::sqrt(s.u.box.hx * s.u.box.hx + s.u.box.hy * s.u.box.hy + s.u.box.hz * s.u.box.hz);
+    case kOrb: return s.u.orb.r;
+    case kTube: return std::sqrt(s.u.tube.rmax2 + s.u.tube.dz * s.u.tube.dz);
+    case kCone: {
+        double r = std::fmax(s.u.cone.rmax1, s.u.cone.rmax2);
+        return std::sqrt(r * r + s.u.cone.dz * s.u.cone.dz);
+    }
+    default: {
+        double a = std::fmax(s.u.trd.dx1, s.u.trd.dx2), b = std::fmax(s.u.trd.dy1, s.u.trd.dy2);
+        return std::sqrt(a * a + b * b + s.u.trd.dz * s.u.trd.dz);
+    }
+    }
+}
+
 static int to_solid(const vg_shape *s, SolidU *o, const char *what)
 {
     std::memset(o, 0, sizeof *o);
@@ -337,20 +355,31 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
     if (nd > 0 && (!daughters || !xforms)) return fail(VG_ERR_ARG, "vg_volume_create: NULL daughters or xforms");
     vg_volume *v = new (std::nothrow) vg_volume;
     if (!v) return fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
-    v->nd = nd;
-    v->table_dev = nullptr;
+    std::memset(v, 0, sizeof *v);
     int rc = to_solid(mother, &v->mother, "mother");
-    Daughter *host = nullptr;
-    if (rc == VG_OK && nd > 0) {
-        host = new (std::nothrow) Daughter[nd];
+    NavMeta &mt = v->meta;
+    mt.nd = nd;
+    mt.nchunks = (nd + 63) / 64;
+    int ndp = (nd + kCullUnroll - 1) / kCullUnroll * kCullUnroll;
+    mt.off_d = unsigned(16 * ndp);
+    mt.bytes = (mt.off_d + unsigned(nd) * unsigned(kDaughterStride) + 15u) / 16u * 16u;
+    if (mt.bytes == 0) mt.bytes = 16;
+    unsigned char *host = nullptr;
+    if (rc == VG_OK) {
+        host = new (std::nothrow) unsigned char[mt.bytes];
         if (!host) rc = fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
+        else std::memset(host, 0, mt.bytes);
+    }
+    double r_mother = rc == VG_OK ? bounding_radius(v->mother) : 0.0;
+    for (int i = 0; rc == VG_OK && i < ndp; ++i) { // padding entries of the cull table: never hit
+        float pad[4] = { 0.f, 0.f, 0.f, -1.f };
+        std::memcpy(host + 16 * i, pad, 16);
     }
     for (int i = 0; rc == VG_OK && i < nd; ++i) {
         if (!daughters[i]) {
             rc = fail(VG_ERR_ARG, "vg_volume_create: daughter %d is NULL", i);
             break;
         }
-        std::memset(&host[i], 0, sizeof(Daughter));
         const double *m = xforms + 12 * i;
         if (!all_finite(m, 12)) {
             rc = fail(VG_ERR_PARAM, "vg_volume_create: non-finite transform of daughter %d", i);
@@ -365,15 +394,31 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
                 }
             }
         if (rc != VG_OK) break;
-        std::memcpy(host[i].m, m, 12 * sizeof(double));
-        rc = to_solid(daughters[i], &host[i].s, "daughter");
+        Daughter d;
+        std::memset(&d, 0, sizeof d);
+        std::memcpy(d.m, m, 12 * sizeof(double));
+        rc = to_solid(daughters[i], &d.s, "daughter");
+        if (rc != VG_OK) break;
+        std::memcpy(host + mt.off_d + size_t(i) * kDaughterStride, &d, sizeof d);
+        mt.kmask[d.s.kind][i / 64] |= 1ull << (i % 64);
+        // bounding sphere in the mother frame: centre c = -R^T b, radius r of the solid about its local origin.
+        // The cull runs in FP32; with S >= |c - p| + r for every p in the mother the FP32 evaluation of
+        // |c - p|^2 - ((c - p).d)^2 is off by < 30 u S^2 (u = 2^-24), so the squared radius is inflated by
+        // 64 u S^2 on top of a relative 1e-6 and rounded UP to float: a daughter the ray can touch is never culled.
+        double cx = -(m[0] * m[3] + m[4] * m[7] + m[8] * m[11]);
+        double cy = -(m[1] * m[3] + m[5] * m[7] + m[9] * m[11]);
+        double cz = -(m[2] * m[3] + m[6] * m[7] + m[10] * m[11]);
+        double r = bounding_radius(d.s);
+        double S = r_mother + std::sqrt(cx * cx + cy * cy + cz * cz) + r;
+        double r2 = r * r * (1.0 + 1e-6) + 64.0 * std::ldexp(1.0, -24) * S * S;
+        float e[4] = { float(cx), float(cy), float(cz), std::nextafterf(float(r2), INFINITY) };
+        std::memcpy(host + 16 * i, e, 16);
     }
     if (rc == VG_OK) {
-        size_t bytes = sizeof(Daughter) * size_t(nd > 0 ? nd : 1);
-        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&v->table_dev), bytes);
+        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&v->table_dev), mt.bytes);
         if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMalloc");
-        if (rc == VG_OK && nd > 0) {
-            e = cudaMemcpy(v->table_dev, host, sizeof(Daughter) * size_t(nd), cudaMemcpyHostToDevice);
+        if (rc == VG_OK) {
+            e = cudaMemcpy(v->table_dev, host, mt.bytes, cudaMemcpyHostToDevice);
             if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMemcpy");
         }
     }
@@ -408,7 +453,7 @@ extern "C" int vg_compute_step(const vg_volume *v, const double *x, const double
     if (!hit || !aligned(hit, 4)) return fail(VG_ERR_ARG, "%s: hit array NULL or misaligned", fn);
     if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
     Tracks t{ x, y, z, dx, dy, dz };
-    cudaError_t e = launch_compute_step(v->mother, v->table_dev, v->nd, t, step_max, n, step, hit,
+    cudaError_t e = launch_compute_step(v->mother, v->table_dev, v->meta, t, step_max, n, step, hit,
                                         static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
@@ -425,7 +470,7 @@ extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const doubl
     if (rc != VG_OK) return rc;
     if (n == 0) return VG_OK;
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
-    cudaError_t e = launch_volume_safety(v->mother, v->table_dev, v->nd, t, n, safety, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_volume_safety(v->mother, v->table_dev, v->meta, t, n, safety, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }

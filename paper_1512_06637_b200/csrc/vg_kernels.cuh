@@ -17,7 +17,13 @@ struct Tracks {
     const double *x, *y, *z, *dx, *dy, *dz;
 };
 
-constexpr int kBlock = 256;
+#ifndef VG_BLOCK
+#define VG_BLOCK 256
+#endif
+#ifndef VG_MINB
+#define VG_MINB 1
+#endif
+constexpr int kBlock = VG_BLOCK;
 
 extern std::atomic<int64_t> g_launches; // kernel launches made by the library (vg_launch_count)
 
@@ -38,7 +44,7 @@ VG_DEV void eval_store(const typename S::P &p, double x, double y, double z, dou
 }
 
 template <class S, int Q, int TPT>
-__global__ void __launch_bounds__(kBlock) query_kernel(const __grid_constant__ typename S::P p, Tracks t,
+__global__ void __launch_bounds__(kBlock, VG_MINB) query_kernel(const __grid_constant__ typename S::P p, Tracks t,
                                                        double step_max, int64_t n, void *out)
 {
     constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
@@ -83,6 +89,9 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
                          cudaStream_t stream)
 {
     if (n <= 0) return cudaSuccess;
+#ifdef VG_FORCE_TPT1
+    vec = false;
+#endif
     if (vec) {
         int64_t threads = (n + 1) / 2;
         unsigned grid = unsigned((threads + kBlock - 1) / kBlock);
@@ -124,9 +133,9 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const Tracks &t, double s
                             cudaStream_t s);
 
 // navigation (vg_nav.cu)
-cudaError_t launch_compute_step(const SolidU &mother, const Daughter *table_dev, int nd, const Tracks &t,
+cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                 double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s);
-cudaError_t launch_volume_safety(const SolidU &mother, const Daughter *table_dev, int nd, const Tracks &t, int64_t n,
+cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t, int64_t n,
                                  double *safety, cudaStream_t s);
 
 // probes (vg_probe.cu)

@@ -87,11 +87,28 @@ struct SolidU {
     } u;
 };
 
-// navigation: one placed daughter; sizeof is a multiple of 16 so that the table moves by one TMA bulk copy
-struct alignas(16) Daughter {
+// navigation: one placed daughter
+struct Daughter {
     double m[12]; // row-major [R | b], mother -> local (reading R12)
     SolidU s;
 };
-static_assert(sizeof(Daughter) % 16 == 0, "daughter table entries must be 16-byte multiples");
+
+// The daughter table is ONE blob in device memory that a CTA stages into shared memory with a single TMA bulk copy:
+//   [0, 16 ndp)                float4 {cx, cy, cz, r2}: bounding sphere of daughter k in the MOTHER frame, in FP32 with
+//                              the radius inflated by the FP32 error bound (conservative cull, see vg_nav.cu);
+//                              ndp = nd rounded up to a multiple of kCullUnroll, padding entries have r2 = -1
+//   [off_d, off_d + nd stride) the Daughter records, stride = sizeof(Daughter) rounded up to an ODD number of 8-byte
+//                              words so that lanes reading different daughters spread over the shared-memory banks
+//   total rounded up to a multiple of 16 bytes (bulk-copy granularity)
+constexpr int kCullUnroll = 8;
+constexpr int kDaughterStride = int(sizeof(Daughter)) + (((sizeof(Daughter) / 8) % 2 == 0) ? 8 : 0);
+constexpr int kNavChunks = 4; // 64 daughters per chunk, VG_MAX_DAUGHTERS = 256
+constexpr int kNavKinds = 5;  // every kind except the polycone
+
+struct NavMeta {
+    int nd, nchunks;
+    unsigned off_d, bytes;
+    unsigned long long kmask[kNavKinds][kNavChunks]; // bit j of kmask[kind][c]: daughter 64 c + j is of that kind
+};
 
 } // namespace vg
