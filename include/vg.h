@@ -157,6 +157,14 @@ int vg_query_host(const vg_shape *shape, int query, const double *x, const doubl
 int vg_compute_step_host(const vg_volume *volume, const double *x, const double *y, const double *z, const double *dx,
                          const double *dy, const double *dz, double step_max, int64_t n, double *step, int32_t *hit);
 
+/* ---- launch policy (process-wide; does not change any result) ----
+ * VG_OPT_PIPE_MIN_N: queries over at least this many tracks whose arrays are all 16-byte aligned run as the
+ * persistent TMA-pipelined kernel (track tiles staged global -> shared memory by bulk copies);
+ * shorter or misaligned batches run as the plain one-pass kernel.  INT64_MAX switches the pipelined form off. */
+typedef enum { VG_OPT_PIPE_MIN_N = 0 } vg_option;
+int vg_set_option(int option, int64_t value);
+int64_t vg_get_option(int option); /* the value, or VG_ERR_ARG for an unknown option */
+
 /* Thread-local message of the last failing call on this host thread ("" if none). Static storage. */
 const char *vg_last_error(void);
 

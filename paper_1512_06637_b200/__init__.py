@@ -55,11 +55,27 @@ def _load():
     lib.vg_probe_fp64_fma_rate.argtypes = [C.c_int, _PD, _VP]
     lib.vg_probe_empty_launch.argtypes = [C.c_int, _VP]
     lib.vg_launch_count.restype = C.c_int64
+    lib.vg_set_option.argtypes = [C.c_int, C.c_int64]
+    lib.vg_get_option.argtypes = [C.c_int]
+    lib.vg_get_option.restype = C.c_int64
     return lib
 
 
 _lib = _load()
 LIB_PATH = _build.LIB
+
+
+OPT_PIPE_MIN_N = 0
+INT64_MAX = 2 ** 63 - 1
+
+
+def vg_set_option(option, value):
+    """Launch policy (vg.h): OPT_PIPE_MIN_N = batch size from which the TMA-pipelined kernel is used."""
+    _check(_lib.vg_set_option(int(option), int(value)))
+
+
+def vg_get_option(option):
+    return int(_lib.vg_get_option(int(option)))
 
 
 def _check(rc):

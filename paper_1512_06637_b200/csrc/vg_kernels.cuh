@@ -8,6 +8,7 @@
 // instantiation (TPT = 1) serves arrays that are only 8-byte aligned and the odd tail.
 #pragma once
 #include "vg_shapes.cuh"
+#include "vg_tma.cuh"
 
 #include <atomic>
 
@@ -84,6 +85,154 @@ __global__ void __launch_bounds__(kBlock, VG_MINB) query_kernel(const __grid_con
     }
 }
 
+// ---- the pipelined form of the same kernel (the default for 16-byte aligned arrays and n >= g_pipe_min_n) ----
+//
+// Why: the plain kernel above keeps a thread's loads in flight only until its own arithmetic starts; with 60-90
+// registers per thread (tube / cone / trd / polycone distances) the SM holds 2-3 CTAs, whose load and compute
+// phases do not overlap well: ncu showed DRAM and the FP64 pipe BOTH at 35-55 % (profiles/r1_*).  Here the track
+// tiles travel global -> shared memory as TMA bulk copies (cp.async.bulk, one 4 KiB copy per SoA array per tile)
+// issued by a producer warp into a kStages-deep ring guarded by full/empty mbarriers; kPipeWarps consumer warps
+// take two tracks per thread out of the ring with 128-bit shared loads, hand the slot back at once and evaluate.
+// Persistent CTAs (SM count x occupancy) walk the tiles round-robin: the bytes in flight per SM are set by the
+// ring (up to kStages x 24 KiB per CTA), not by the register file, and loads of later tiles overlap the FP64 work
+// of the current one.  Results leave as 128-bit streaming stores straight from registers.
+#ifndef VG_PIPE_WARPS
+#define VG_PIPE_WARPS 8
+#endif
+#ifndef VG_PIPE_STAGES
+#define VG_PIPE_STAGES 4
+#endif
+#ifndef VG_PIPE_MINB
+#define VG_PIPE_MINB 2
+#endif
+constexpr int kPipeWarps = VG_PIPE_WARPS;
+constexpr int kPipeStages = VG_PIPE_STAGES;
+constexpr int kPipeThreads = 32 * kPipeWarps + 32; // + the producer warp
+constexpr int kPipeTile = 64 * kPipeWarps;         // tracks per tile: two per consumer thread
+
+extern std::atomic<int64_t> g_pipe_min_n; // vg_set_option(VG_OPT_PIPE_MIN_N)
+
+template <class S, int Q>
+__global__ void __launch_bounds__(kPipeThreads, VG_PIPE_MINB)
+    query_pipe_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, void *out, int ntiles)
+{
+    constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
+    constexpr int kArr = kDir ? 6 : 3;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *ring = reinterpret_cast<double *>(smem_raw); // [kPipeStages][kArr][kPipeTile]
+    __shared__ __align__(8) uint64_t full[kPipeStages], empty[kPipeStages];
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < kPipeStages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kPipeWarps);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    if (warp == kPipeWarps) { // producer: one elected lane feeds the ring
+        if (lane != 0) return;
+        const double *src[6] = { t.x, t.y, t.z, t.dx, t.dy, t.dz };
+        int s = 0;
+        uint32_t ph = 1; // a fresh `empty` barrier lets the wait on parity 1 pass: every slot starts free
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            mbar_wait(&empty[s], ph);
+            const int64_t base = int64_t(tile) * kPipeTile;
+            const int64_t left = n - base;
+            const uint32_t cnt = left < kPipeTile ? uint32_t(left) : uint32_t(kPipeTile);
+            const uint32_t bytes = (cnt * 8u) & ~15u; // an odd last track is read by its consumer straight from global
+            if (bytes) {
+                mbar_expect_tx(&full[s], kArr * bytes);
+#pragma unroll
+                for (int a = 0; a < kArr; ++a) bulk_g2s(ring + (s * kArr + a) * kPipeTile, src[a] + base, bytes, &full[s]);
+            } else {
+                mbar_arrive(&full[s]);
+            }
+            if (++s == kPipeStages) {
+                s = 0;
+                ph ^= 1u;
+            }
+        }
+        return;
+    }
+
+    int s = 0;
+    uint32_t ph = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int64_t i = int64_t(tile) * kPipeTile + 2 * threadIdx.x;
+        const bool pair = i + 1 < n;
+        mbar_wait(&full[s], ph);
+        const double *st = ring + s * kArr * kPipeTile + 2 * threadIdx.x;
+        double2 x = make_double2(0, 0), y = x, z = x, dx = x, dy = x, dz = x;
+        if (pair) {
+            x = *reinterpret_cast<const double2 *>(st);
+            y = *reinterpret_cast<const double2 *>(st + kPipeTile);
+            z = *reinterpret_cast<const double2 *>(st + 2 * kPipeTile);
+            if (kDir) {
+                dx = *reinterpret_cast<const double2 *>(st + 3 * kPipeTile);
+                dy = *reinterpret_cast<const double2 *>(st + 4 * kPipeTile);
+                dz = *reinterpret_cast<const double2 *>(st + 5 * kPipeTile);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]); // the slot is free again as soon as the warp holds its tracks in registers
+        if (++s == kPipeStages) {
+            s = 0;
+            ph ^= 1u;
+        }
+        if (pair) {
+            double d0 = 0, d1 = 0;
+            int i0 = 0, i1 = 0;
+            eval_store<S, Q>(p, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max, d0, i0);
+            eval_store<S, Q>(p, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max, d1, i1);
+            if (Q == qInside)
+                stg2i(static_cast<int32_t *>(out) + i, i0, i1);
+            else
+                stg2(static_cast<double *>(out) + i, d0, d1);
+        } else if (i < n) { // odd last track
+            double x1 = ldg1(t.x + i), y1 = ldg1(t.y + i), z1 = ldg1(t.z + i);
+            double dx1 = 0, dy1 = 0, dz1 = 0;
+            if (kDir) {
+                dx1 = ldg1(t.dx + i);
+                dy1 = ldg1(t.dy + i);
+                dz1 = ldg1(t.dz + i);
+            }
+            double d0 = 0;
+            int i0 = 0;
+            eval_store<S, Q>(p, x1, y1, z1, dx1, dy1, dz1, step_max, d0, i0);
+            if (Q == qInside)
+                stg1i(static_cast<int32_t *>(out) + i, i0);
+            else
+                stg1(static_cast<double *>(out) + i, d0);
+        }
+    }
+}
+
+// resident CTAs of the pipelined kernel on the current device (configured once per device and instantiation)
+template <class S, int Q> cudaError_t pipe_capacity(int *cap, size_t *smem_out)
+{
+    constexpr int kMaxDev = 64;
+    constexpr int kArr = (Q == qDistIn || Q == qDistOut) ? 6 : 3;
+    constexpr size_t smem = size_t(kPipeStages) * kArr * kPipeTile * sizeof(double);
+    static std::atomic<int> cached[kMaxDev];
+    *smem_out = smem;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < kMaxDev && (*cap = cached[dev].load(std::memory_order_acquire)) > 0) return cudaSuccess;
+    int sms = 0, per_sm = 0;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(query_pipe_kernel<S, Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem))) != cudaSuccess)
+        return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, query_pipe_kernel<S, Q>, kPipeThreads, smem)) != cudaSuccess)
+        return e;
+    *cap = sms * (per_sm < 1 ? 1 : per_sm);
+    if (dev >= 0 && dev < kMaxDev) cached[dev].store(*cap, std::memory_order_release);
+    return cudaSuccess;
+}
+
 template <class S, int Q>
 cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
                          cudaStream_t stream)
@@ -92,7 +241,15 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
 #ifdef VG_FORCE_TPT1
     vec = false;
 #endif
-    if (vec) {
+    if (vec && n >= g_pipe_min_n.load(std::memory_order_relaxed)) {
+        int cap = 0;
+        size_t smem = 0;
+        cudaError_t e = pipe_capacity<S, Q>(&cap, &smem);
+        if (e != cudaSuccess) return e;
+        int64_t tiles = (n + kPipeTile - 1) / kPipeTile;
+        unsigned grid = unsigned(tiles < cap ? tiles : cap);
+        query_pipe_kernel<S, Q><<<grid, kPipeThreads, smem, stream>>>(p, t, step_max, n, out, int(tiles));
+    } else if (vec) {
         int64_t threads = (n + 1) / 2;
         unsigned grid = unsigned((threads + kBlock - 1) / kBlock);
         query_kernel<S, Q, 2><<<grid, kBlock, 0, stream>>>(p, t, step_max, n, out);

@@ -15,42 +15,17 @@
 // The tie-break of R13 (lowest index, mother first) is kept by comparing (t, k) pairs explicitly, because
 // candidates are not visited in index order.
 #include "vg_kernels.cuh"
+#include "vg_tma.cuh"
 
 namespace vg {
 
 constexpr int kNavBlock = 128;
 
-VG_DEV uint32_t smem_u32(const void *p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
-
 // one elected thread: arm the barrier with the byte count and issue the bulk copy global -> shared
 VG_DEV void tma_load_table(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
 {
-    uint32_t b = smem_u32(bar), d = smem_u32(dst_smem);
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b), "r"(bytes) : "memory");
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(d),
-                 "l"(src_gmem), "r"(bytes), "r"(b)
-                 : "memory");
-}
-
-VG_DEV void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-
-VG_DEV void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t b = smem_u32(bar), done = 0;
-    while (!done) { // try_wait suspends the thread in hardware for a bounded time; loop until the phase flips
-        asm volatile("{\n"
-                     ".reg .pred p;\n"
-                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-                     "selp.u32 %0, 1, 0, p;\n"
-                     "}\n"
-                     : "=r"(done)
-                     : "r"(b), "r"(parity)
-                     : "memory");
-    }
+    mbar_expect_tx(bar, bytes);
+    bulk_g2s(dst_smem, src_gmem, bytes, bar);
 }
 
 VG_DEV double solid_dist_in(const SolidU &s, double x, double y, double z, double dx, double dy, double dz)
@@ -135,7 +110,10 @@ __global__ void __launch_bounds__(kNavBlock) nav_kernel(const __grid_constant__ 
     const unsigned char *dtab = smem_raw + meta.off_d;
     const int nd = meta.nd;
 
-    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        mbar_fence_init();
+    }
     __syncthreads();
     if (threadIdx.x == 0 && nd > 0) tma_load_table(smem_raw, table, meta.bytes, &bar);
     bool waited = (nd == 0);

@@ -47,6 +47,19 @@ def test_oracle_and_cuda_path_share_no_code():
     assert "paper_1512_06637_b200" not in opy.split('"""', 2)[2]
 
 
+def test_options_round_trip_without_a_gpu():
+    import paper_1512_06637_b200 as vg
+    old = vg.vg_get_option(vg.OPT_PIPE_MIN_N)
+    assert old > 0
+    vg.vg_set_option(vg.OPT_PIPE_MIN_N, 12345)
+    assert vg.vg_get_option(vg.OPT_PIPE_MIN_N) == 12345
+    vg.vg_set_option(vg.OPT_PIPE_MIN_N, old)
+    with pytest.raises(vg.VgError):
+        vg.vg_set_option(vg.OPT_PIPE_MIN_N, -1)
+    with pytest.raises(vg.VgError):
+        vg.vg_set_option(99, 1)
+
+
 BAD = [
     (0, [5, 5]), (0, [5, -1, 5]), (0, [5, 0, 5]), (0, [5, math.nan, 5]), (0, [5, math.inf, 5]),
     (1, [0]), (1, [-2]), (1, [1, 2]),

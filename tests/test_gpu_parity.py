@@ -23,6 +23,15 @@ def vg():
     return m
 
 
+@pytest.fixture(params=["pipelined", "plain"])
+def kernel_form(request, vg):
+    """Force every 16-byte aligned batch through the TMA-pipelined kernel (whatever its size), or none."""
+    old = vg.vg_get_option(vg.OPT_PIPE_MIN_N)
+    vg.vg_set_option(vg.OPT_PIPE_MIN_N, 0 if request.param == "pipelined" else vg.INT64_MAX)
+    yield request.param
+    vg.vg_set_option(vg.OPT_PIPE_MIN_N, old)
+
+
 def dev(arrs):
     return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrs]
 
@@ -94,7 +103,7 @@ ALL_CASES = [(k, i) for k in (0, 1, 2, 3) for i in range(len(W.shape_cases(k)))]
 
 
 @pytest.mark.parametrize("k,i", ALL_CASES)
-def test_ragged_tail_and_misaligned_slices(vg, k, i):
+def test_ragged_tail_and_misaligned_slices(vg, kernel_form, k, i):
     """n spans many blocks and ends in a ragged tail; slices starting at element 1 are only 8-byte aligned and
     take the 64-bit path (include/vg.h: never an error, never a host fallback)."""
     sc = W.shape_cases(k)[i]
@@ -102,23 +111,23 @@ def test_ragged_tail_and_misaligned_slices(vg, k, i):
     n = 100003
     t = sc.tracks(n + 1, band=oracle_band(so))
     dt = dev(t)
-    for off, m in ((0, n), (1, n), (1, n - 1), (0, 513), (1, 511)):
+    for off, m in ((0, n), (1, n), (1, n - 1), (0, 513), (1, 511), (0, 1), (0, 2), (2, 1025), (2, 1024)):
         ts = [a[off:off + m] for a in t]
         ds = [a[off:off + m] for a in dt]
         for q in W.QUERIES5:
             o = run_oracle(so, q, ts, W.STEP_MAX)
             if q == "inside":
-                out = torch.empty(m + 1, dtype=torch.int32, device="cuda")[off:off + m]
+                out = torch.empty(m + off, dtype=torch.int32, device="cuda")[off:off + m]
                 sg.inside(*ds[:3], out=out)
                 assert_int_equal(out.cpu().numpy(), o, "%s inside off=%d" % (sc.name, off))
             else:
-                out = torch.empty(m + 1, dtype=torch.float64, device="cuda")[off:off + m]
+                out = torch.empty(m + off, dtype=torch.float64, device="cuda")[off:off + m]
                 sg.query(q, *ds, step_max=W.STEP_MAX, out=out)
                 assert_real_close(out.cpu().numpy(), o, "%s %s off=%d" % (sc.name, q, off))
 
 
-@pytest.mark.parametrize("n", [0, 1, 2, 3, 255, 256, 257, 511, 512, 513])
-def test_tiny_sizes(vg, n):
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 255, 256, 257, 511, 512, 513, 1023, 1025])
+def test_tiny_sizes(vg, kernel_form, n):
     sc = W.shape_cases(1)[0]
     so = O.Shape(sc.kind, sc.params)
     t = sc.tracks(n, band=oracle_band(so))
@@ -130,7 +139,7 @@ def test_tiny_sizes(vg, n):
     check_all(vg, sc.kind, sc.params, t, what="tiny")
 
 
-def test_outputs_do_not_overrun(vg):
+def test_outputs_do_not_overrun(vg, kernel_form):
     """Guard elements after the output must stay untouched for odd n on the 128-bit path."""
     sc = W.shape_cases(0)[0]
     sg = vg.Shape(sc.kind, sc.params)
