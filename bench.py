@@ -322,6 +322,8 @@ def run_profile(args):
     import paper_1512_06637_b200 as vg
     if args.pipe_min_n is not None:
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, args.pipe_min_n)
+    if args.no_pdl:
+        vg.vg_set_option(vg.OPT_PDL, 0)
     cases = []
     for k in (1, 2, 3):
         for sc in W.shape_cases(k):
@@ -351,6 +353,8 @@ def run_ours(args, rank, world, local_rank):
     from paper_1512_06637_b200.shard import barrier, max_over_ranks, sum_over_ranks
     if args.pipe_min_n is not None:
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, args.pipe_min_n)
+    if args.no_pdl:
+        vg.vg_set_option(vg.OPT_PDL, 0)
 
     hbm_peak, hbm_src = measured_peaks()
     sampler = ClockSampler(local_rank)
@@ -439,7 +443,7 @@ def run_ours(args, rank, world, local_rank):
                            "l2_policy": "inputs larger than L2: every launch reads the next of %d copies of the batch "
                                         "(%d MB of inputs in rotation, L2 = 126 MB)" % (case.nsets, case.nsets * 48 * case.n // 10 ** 6),
                            "launch": "CUDA graphs captured from the C-ABI calls, one graph per step",
-                           "pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N),
+                           "pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N), "pdl": vg.vg_get_option(vg.OPT_PDL),
                            "parallelism": "tracks sharded over ranks, no collective" if world > 1 else "1 GPU"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
                 "roofline": roof, "per_query": per_query,
@@ -465,6 +469,7 @@ def main():
     ap.add_argument("--pipe-min-n", type=int, default=None,
                     help="vg_set_option(VG_OPT_PIPE_MIN_N): batch size from which the TMA-pipelined kernel runs "
                          "(default: the library's); for A/B runs of the two kernel forms")
+    ap.add_argument("--no-pdl", action="store_true", help="vg_set_option(VG_OPT_PDL, 0): launch without programmatic dependent launch")
     ap.add_argument("--profile", action="store_true", help="eager launches of every kernel, for ncu; no timing")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

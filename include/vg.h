@@ -160,8 +160,12 @@ int vg_compute_step_host(const vg_volume *volume, const double *x, const double 
 /* ---- launch policy (process-wide; does not change any result) ----
  * VG_OPT_PIPE_MIN_N: queries over at least this many tracks whose arrays are all 16-byte aligned run as the
  * persistent TMA-pipelined kernel (track tiles staged global -> shared memory by bulk copies);
- * shorter or misaligned batches run as the plain one-pass kernel.  INT64_MAX switches the pipelined form off. */
-typedef enum { VG_OPT_PIPE_MIN_N = 0 } vg_option;
+ * shorter or misaligned batches run as the plain one-pass kernel.  INT64_MAX switches the pipelined form off.
+ * VG_OPT_PDL (default 1): kernels are launched with the programmatic-dependent-launch attribute, so that the launch
+ * latency and set-up of a kernel overlap the tail of the previous kernel in the same stream; every kernel still
+ * waits (griddepcontrol.wait) for its predecessor to complete before it touches global memory, so stream order is
+ * preserved exactly.  0 launches without the attribute. */
+typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1 } vg_option;
 int vg_set_option(int option, int64_t value);
 int64_t vg_get_option(int option); /* the value, or VG_ERR_ARG for an unknown option */
 

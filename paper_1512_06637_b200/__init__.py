@@ -66,6 +66,7 @@ LIB_PATH = _build.LIB
 
 
 OPT_PIPE_MIN_N = 0
+OPT_PDL = 1
 INT64_MAX = 2 ** 63 - 1
 
 

@@ -55,6 +55,7 @@ extern "C" int vg_set_error(int code, const char *msg) { return fail(code, "%s",
 namespace vg {
 std::atomic<int64_t> g_launches{ 0 };
 std::atomic<int64_t> g_pipe_min_n{ int64_t(1) << 17 };
+std::atomic<int64_t> g_pdl{ 1 };
 }
 extern "C" int64_t vg_launch_count(void) { return vg::g_launches.load(); }
 
@@ -65,6 +66,9 @@ extern "C" int vg_set_option(int option, int64_t value)
         if (value < 0) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_PIPE_MIN_N must be >= 0");
         vg::g_pipe_min_n.store(value);
         return VG_OK;
+    case VG_OPT_PDL:
+        vg::g_pdl.store(value != 0);
+        return VG_OK;
     }
     return fail(VG_ERR_ARG, "vg_set_option: unknown option %d", option);
 }
@@ -73,6 +77,7 @@ extern "C" int64_t vg_get_option(int option)
 {
     switch (option) {
     case VG_OPT_PIPE_MIN_N: return vg::g_pipe_min_n.load();
+    case VG_OPT_PDL: return vg::g_pdl.load();
     }
     return fail(VG_ERR_ARG, "vg_get_option: unknown option %d", option);
 }

@@ -27,6 +27,26 @@ struct Tracks {
 constexpr int kBlock = VG_BLOCK;
 
 extern std::atomic<int64_t> g_launches; // kernel launches made by the library (vg_launch_count)
+extern std::atomic<int64_t> g_pdl;      // vg_set_option(VG_OPT_PDL)
+
+// every kernel of the library is launched through this: optional programmatic-dependent-launch attribute
+template <class... KArgs, class... Args>
+cudaError_t launch_kernel(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream,
+                          Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = g_pdl.load(std::memory_order_relaxed) ? 1 : 0;
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
 
 template <class S, int Q>
 VG_DEV void eval_store(const typename S::P &p, double x, double y, double z, double dx, double dy, double dz,
@@ -50,6 +70,8 @@ __global__ void __launch_bounds__(kBlock, VG_MINB) query_kernel(const __grid_con
 {
     constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
     int64_t i = (int64_t(blockIdx.x) * kBlock + threadIdx.x) * TPT;
+    pdl_launch_dependents();
+    pdl_wait();
     if (i >= n) return;
     if (TPT == 2 && i + 1 < n) {
         double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
@@ -93,9 +115,12 @@ __global__ void __launch_bounds__(kBlock, VG_MINB) query_kernel(const __grid_con
 // tiles travel global -> shared memory as TMA bulk copies (cp.async.bulk, one 4 KiB copy per SoA array per tile)
 // issued by a producer warp into a kStages-deep ring guarded by full/empty mbarriers; kPipeWarps consumer warps
 // take two tracks per thread out of the ring with 128-bit shared loads, hand the slot back at once and evaluate.
-// Persistent CTAs (SM count x occupancy) walk the tiles round-robin: the bytes in flight per SM are set by the
-// ring (up to kStages x 24 KiB per CTA), not by the register file, and loads of later tiles overlap the FP64 work
-// of the current one.  Results leave as 128-bit streaming stores straight from registers.
+// The grid has one CTA per tile, but the CTAs that get to run are persistent: the producer takes over the block
+// index of a not yet launched CTA with cluster launch control (clusterlaunchcontrol.try_cancel, sm_100) for every
+// further tile, so tiles are handed out dynamically by the hardware scheduler (a static round-robin left the SMs
+// finishing 50 % apart, profiles/r1_*) and the ring never drains between tiles.  The bytes in flight per SM are set
+// by the ring (up to kStages x 24 KiB per CTA), not by the register file, and loads of later tiles overlap the
+// FP64 work of the current one.  Results leave as 128-bit streaming stores straight from registers.
 #ifndef VG_PIPE_WARPS
 #define VG_PIPE_WARPS 8
 #endif
@@ -114,31 +139,41 @@ extern std::atomic<int64_t> g_pipe_min_n; // vg_set_option(VG_OPT_PIPE_MIN_N)
 
 template <class S, int Q>
 __global__ void __launch_bounds__(kPipeThreads, VG_PIPE_MINB)
-    query_pipe_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, void *out, int ntiles)
+    query_pipe_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, void *out)
 {
     constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
     constexpr int kArr = kDir ? 6 : 3;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw); // [kPipeStages][kArr][kPipeTile]
-    __shared__ __align__(8) uint64_t full[kPipeStages], empty[kPipeStages];
+    __shared__ __align__(16) unsigned char clc_resp[16];
+    __shared__ __align__(8) uint64_t full[kPipeStages], empty[kPipeStages], clc_bar;
+    __shared__ int tile_of[kPipeStages];
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < kPipeStages; ++s) {
             mbar_init(&full[s], 1);
             mbar_init(&empty[s], kPipeWarps);
         }
+        mbar_init(&clc_bar, 1);
         mbar_fence_init();
     }
+    pdl_launch_dependents();
     __syncthreads();
+    pdl_wait(); // nothing above touches global memory: it overlaps the tail of the previous kernel in the stream
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-    if (warp == kPipeWarps) { // producer: one elected lane feeds the ring
+    if (warp == kPipeWarps) { // producer: one elected lane schedules tiles and feeds the ring
         if (lane != 0) return;
         const double *src[6] = { t.x, t.y, t.z, t.dx, t.dy, t.dz };
-        int s = 0;
+        int s = 0, tile = blockIdx.x;
         uint32_t ph = 1; // a fresh `empty` barrier lets the wait on parity 1 pass: every slot starts free
-        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        uint32_t clc_ph = 0;
+        while (true) {
+            // ask the hardware for the next tile (a not yet launched CTA of this grid) while this one is issued
+            mbar_expect_tx(&clc_bar, 16);
+            clc_try_cancel(clc_resp, &clc_bar);
             mbar_wait(&empty[s], ph);
+            tile_of[s] = tile;
             const int64_t base = int64_t(tile) * kPipeTile;
             const int64_t left = n - base;
             const uint32_t cnt = left < kPipeTile ? uint32_t(left) : uint32_t(kPipeTile);
@@ -154,16 +189,26 @@ __global__ void __launch_bounds__(kPipeThreads, VG_PIPE_MINB)
                 s = 0;
                 ph ^= 1u;
             }
+            mbar_wait(&clc_bar, clc_ph);
+            clc_ph ^= 1u;
+            tile = clc_decode_x(clc_resp);
+            fence_proxy_async_smem(); // the next response may overwrite clc_resp
+            if (tile < 0) break;
         }
+        mbar_wait(&empty[s], ph); // end marker for the consumers
+        tile_of[s] = -1;
+        mbar_arrive(&full[s]);
         return;
     }
 
     int s = 0;
     uint32_t ph = 0;
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    while (true) {
+        mbar_wait(&full[s], ph);
+        const int tile = tile_of[s];
+        if (tile < 0) break;
         const int64_t i = int64_t(tile) * kPipeTile + 2 * threadIdx.x;
         const bool pair = i + 1 < n;
-        mbar_wait(&full[s], ph);
         const double *st = ring + s * kArr * kPipeTile + 2 * threadIdx.x;
         double2 x = make_double2(0, 0), y = x, z = x, dx = x, dy = x, dz = x;
         if (pair) {
@@ -246,19 +291,17 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
         size_t smem = 0;
         cudaError_t e = pipe_capacity<S, Q>(&cap, &smem);
         if (e != cudaSuccess) return e;
-        int64_t tiles = (n + kPipeTile - 1) / kPipeTile;
-        unsigned grid = unsigned(tiles < cap ? tiles : cap);
-        query_pipe_kernel<S, Q><<<grid, kPipeThreads, smem, stream>>>(p, t, step_max, n, out, int(tiles));
-    } else if (vec) {
+        (void)cap;
+        int64_t tiles = (n + kPipeTile - 1) / kPipeTile; // one CTA per tile; running CTAs cancel and take over pending ones
+        return launch_kernel(query_pipe_kernel<S, Q>, unsigned(tiles), kPipeThreads, smem, stream, p, t, step_max, n, out);
+    }
+    if (vec) {
         int64_t threads = (n + 1) / 2;
         unsigned grid = unsigned((threads + kBlock - 1) / kBlock);
-        query_kernel<S, Q, 2><<<grid, kBlock, 0, stream>>>(p, t, step_max, n, out);
-    } else {
-        unsigned grid = unsigned((n + kBlock - 1) / kBlock);
-        query_kernel<S, Q, 1><<<grid, kBlock, 0, stream>>>(p, t, step_max, n, out);
+        return launch_kernel(query_kernel<S, Q, 2>, grid, kBlock, 0, stream, p, t, step_max, n, out);
     }
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return cudaGetLastError();
+    unsigned grid = unsigned((n + kBlock - 1) / kBlock);
+    return launch_kernel(query_kernel<S, Q, 1>, grid, kBlock, 0, stream, p, t, step_max, n, out);
 }
 
 template <class S>

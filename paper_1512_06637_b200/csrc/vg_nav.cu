@@ -114,7 +114,9 @@ __global__ void __launch_bounds__(kNavBlock) nav_kernel(const __grid_constant__ 
         mbar_init(&bar, 1);
         mbar_fence_init();
     }
+    pdl_launch_dependents();
     __syncthreads();
+    pdl_wait();
     if (threadIdx.x == 0 && nd > 0) tma_load_table(smem_raw, table, meta.bytes, &bar);
     bool waited = (nd == 0);
 
@@ -207,9 +209,7 @@ static cudaError_t launch_nav(const SolidU &mother, const unsigned char *table_d
     int64_t want = (n + kNavBlock - 1) / kNavBlock;
     int64_t cap = int64_t(sm_count) * per_sm; // persistent: one resident wave, a multiple of the SM count
     unsigned grid = unsigned(want < cap ? want : cap);
-    nav_kernel<kStep><<<grid, kNavBlock, smem, s>>>(mother, meta, table_dev, t, step_max, n, out, hit);
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return cudaGetLastError();
+    return launch_kernel(nav_kernel<kStep>, grid, kNavBlock, smem, s, mother, meta, table_dev, t, step_max, n, out, hit);
 }
 
 cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,

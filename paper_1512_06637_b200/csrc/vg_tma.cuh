@@ -69,4 +69,45 @@ VG_DEV uint64_t policy_evict_first()
     return p;
 }
 
+// ---- cluster launch control (sm_100): a running CTA asks the hardware scheduler to cancel a CTA of the same grid
+// that has not been launched yet and takes over its block index -- dynamic load balancing for persistent CTAs
+// without any global counter.  The 16-byte response lands in shared memory asynchronously (async proxy) and
+// completes 16 bytes on `bar`.  After the first failed request a CTA must not ask again.
+VG_DEV void clc_try_cancel(void *resp_smem16, uint64_t *bar)
+{
+    asm volatile("clusterlaunchcontrol.try_cancel.async.shared::cta.mbarrier::complete_tx::bytes.b128 [%0], [%1];" ::"r"(
+                     smem_u32(resp_smem16)),
+                 "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// decode a response: returns the stolen blockIdx.x, or -1 if nothing was left to cancel
+VG_DEV int clc_decode_x(const void *resp_smem16)
+{
+    uint32_t ok, bx;
+    asm volatile("{\n"
+                 ".reg .b128 r;\n"
+                 ".reg .pred p;\n"
+                 "ld.shared.b128 r, [%2];\n"
+                 "clusterlaunchcontrol.query_cancel.is_canceled.pred.b128 p, r;\n"
+                 "selp.u32 %0, 1, 0, p;\n"
+                 "@p clusterlaunchcontrol.query_cancel.get_first_ctaid::x.b32.b128 %1, r;\n"
+                 "@!p mov.u32 %1, 0;\n"
+                 "}\n"
+                 : "=r"(ok), "=r"(bx)
+                 : "r"(smem_u32(resp_smem16))
+                 : "memory");
+    return ok ? int(bx) : -1;
+}
+
+// ---- programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may be
+// scheduled while its predecessor in the stream is still draining; pdl_wait() blocks until the predecessor grid has
+// completed and its memory operations are visible, so everything before it (barrier set-up, index arithmetic, the
+// launch latency itself) overlaps the predecessor's tail.  Both are no-ops in a kernel launched without the attribute.
+VG_DEV void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+VG_DEV void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// orders this thread's generic-proxy accesses to shared memory before later async-proxy writes to it
+VG_DEV void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 } // namespace vg
