@@ -45,6 +45,22 @@ def measured_peaks():
         return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(solid, query, n):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of that kernel at that N, from the committed summary of
+    the last `ncu --set full` capture (profiles/traffic.csv); None when the capture has no such row."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                c = line.strip().split(",")
+                if len(c) >= 7 and c[1] == solid and c[2] == query and c[3] == str(n):
+                    return {"bytes": int(c[4]) + int(c[5]), "dram_read": int(c[4]), "dram_write": int(c[5]),
+                            "capture": "profiles/%s_full_capture.md" % c[6],
+                            "note": "results still sit in the 126 MB L2 when the kernel ends, so DRAM writes read low"}
+    except OSError:
+        pass
+    return None
+
+
 # ------------------------------------------------------------------------------------------- clock sampler
 
 class ClockSampler:
@@ -322,6 +338,8 @@ def run_profile(args):
     import paper_1512_06637_b200 as vg
     if args.pipe_min_n is not None:
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, args.pipe_min_n)
+    if args.form is not None:
+        vg.vg_set_option(vg.OPT_FORM, {"auto": vg.FORM_AUTO, "direct": vg.FORM_DIRECT, "pipelined": vg.FORM_PIPELINED}[args.form])
     if args.no_pdl:
         vg.vg_set_option(vg.OPT_PDL, 0)
     cases = []
@@ -353,6 +371,8 @@ def run_ours(args, rank, world, local_rank):
     from paper_1512_06637_b200.shard import barrier, max_over_ranks, sum_over_ranks
     if args.pipe_min_n is not None:
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, args.pipe_min_n)
+    if args.form is not None:
+        vg.vg_set_option(vg.OPT_FORM, {"auto": vg.FORM_AUTO, "direct": vg.FORM_DIRECT, "pipelined": vg.FORM_PIPELINED}[args.form])
     if args.no_pdl:
         vg.vg_set_option(vg.OPT_PDL, 0)
 
@@ -394,7 +414,8 @@ def run_ours(args, rank, world, local_rank):
     dom = max(case.queries, key=lambda q: per_q[q])
     roof = {"bound": "hbm", "kernel": "query_kernel<Tube, %s>" % dom, "achieved": per_query[dom]["hbm_gbs"],
             "peak": hbm_peak, "unit": "GB/s", "frac": per_query[dom]["hbm_gbs"] / hbm_peak, "peak_source": hbm_src,
-            "traffic": None, "algorithmic_bytes_per_launch": BYTES[dom] * case.n,
+            "traffic": (ncu_traffic("Tube", dom, case.n) or {}).get("bytes"), "traffic_detail": ncu_traffic("Tube", dom, case.n),
+            "algorithmic_bytes_per_launch": BYTES[dom] * case.n,
             "us_per_launch": per_q[dom] * 1e6, "share_of_step": per_q[dom] / sum(per_q.values()),
             "sum_of_kernels_us": sum(per_q.values()) * 1e6,
             "kernel_timing": kernel_timing,
@@ -443,7 +464,7 @@ def run_ours(args, rank, world, local_rank):
                            "l2_policy": "inputs larger than L2: every launch reads the next of %d copies of the batch "
                                         "(%d MB of inputs in rotation, L2 = 126 MB)" % (case.nsets, case.nsets * 48 * case.n // 10 ** 6),
                            "launch": "CUDA graphs captured from the C-ABI calls, one graph per step",
-                           "pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N), "pdl": vg.vg_get_option(vg.OPT_PDL),
+                           "pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N), "form": vg.vg_get_option(vg.OPT_FORM), "pdl": vg.vg_get_option(vg.OPT_PDL),
                            "parallelism": "tracks sharded over ranks, no collective" if world > 1 else "1 GPU"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
                 "roofline": roof, "per_query": per_query,
@@ -469,6 +490,8 @@ def main():
     ap.add_argument("--pipe-min-n", type=int, default=None,
                     help="vg_set_option(VG_OPT_PIPE_MIN_N): batch size from which the TMA-pipelined kernel runs "
                          "(default: the library's); for A/B runs of the two kernel forms")
+    ap.add_argument("--form", choices=["auto", "direct", "pipelined"], default=None,
+                    help="vg_set_option(VG_OPT_FORM): kernel form for A/B runs (default: the library's per-kernel choice)")
     ap.add_argument("--no-pdl", action="store_true", help="vg_set_option(VG_OPT_PDL, 0): launch without programmatic dependent launch")
     ap.add_argument("--profile", action="store_true", help="eager launches of every kernel, for ncu; no timing")
     args = ap.parse_args()

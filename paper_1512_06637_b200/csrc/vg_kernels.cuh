@@ -136,6 +136,13 @@ constexpr int kPipeThreads = 32 * kPipeWarps + 32; // + the producer warp
 constexpr int kPipeTile = 64 * kPipeWarps;         // tracks per tile: two per consumer thread
 
 extern std::atomic<int64_t> g_pipe_min_n; // vg_set_option(VG_OPT_PIPE_MIN_N)
+extern std::atomic<int64_t> g_form;       // vg_set_option(VG_OPT_FORM): 0 auto, 1 direct, 2 pipelined
+
+// VG_FORM_AUTO: the pairs whose pipelined form measured faster than the direct one at n >= 2^22 (profiles/):
+// only the heaviest straight-line kernel, where the direct form's registers leave too few warps to overlap its
+// loads with its FP64 work.  Everything lighter is faster direct (no ring hand-offs, four to eight CTAs per SM).
+template <class S, int Q> struct PipeByDefault { static constexpr bool value = false; };
+template <> struct PipeByDefault<Cone, qDistIn> { static constexpr bool value = true; };
 
 template <class S, int Q>
 __global__ void __launch_bounds__(kPipeThreads, VG_PIPE_MINB)
@@ -286,7 +293,9 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
 #ifdef VG_FORCE_TPT1
     vec = false;
 #endif
-    if (vec && n >= g_pipe_min_n.load(std::memory_order_relaxed)) {
+    const int64_t form = g_form.load(std::memory_order_relaxed);
+    const bool pipe = form == 2 || (form == 0 && PipeByDefault<S, Q>::value);
+    if (vec && pipe && n >= g_pipe_min_n.load(std::memory_order_relaxed)) {
         int cap = 0;
         size_t smem = 0;
         cudaError_t e = pipe_capacity<S, Q>(&cap, &smem);

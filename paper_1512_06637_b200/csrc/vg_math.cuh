@@ -4,7 +4,7 @@
 // (+ a slow-path branch), a sqrt MUFU.RSQ64H + 8.  The parity contract is
 // |gpu - oracle| <= max(1e-9, 1e-12 |oracle|) (BASELINE.json north_star), not correct rounding, so the
 // kernels use a third-order (cubic) refinement of the 20-bit MUFU seed: 3 FP64 instructions for a reciprocal,
-// 6 for a square root, relative error ~1e-16 (seed error e ~ 2^-18.5, the refinements leave O(e^3)).
+// 5 for a square root, relative error ~1e-16 (seed error e ~ 2^-18.5, the refinements leave O(e^3)).
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -38,6 +38,15 @@ VG_DEV double flipsign_bits(double v, double sgn)
     return __hiloint2double(__double2hiint(v) ^ (__double2hiint(sgn) & 0x80000000), __double2loint(v));
 }
 
+// Sign tests on the integer pipe: one ISETP on the high word instead of a DSETP, which would take an FP64-pipe
+// slot (the FP64 pipe is the scarce unit of these kernels).  They differ from the IEEE
+// compares only off the normal range: a +-NaN tests like a number of its sign (every caller ANDs in a real
+// compare or a discriminant test that a NaN fails), -0.0 tests negative, and denormals below 2^-1042 test as 0.
+VG_DEV bool is_pos(double x) { return __double2hiint(x) > 0; }                        // x > 0
+VG_DEV bool is_neg(double x) { return (unsigned)__double2hiint(x) > 0x80000000u; }    // x < 0
+VG_DEV bool not_neg(double x) { return __double2hiint(x) >= 0; }                      // x >= 0 (sign bit clear)
+VG_DEV bool sign_differs(double a, double b) { return (__double2hiint(a) ^ __double2hiint(b)) < 0; }
+
 // |a| < kTiny (incl. +-0)  ->  +-kTiny, so that 1/a and num/a stay finite-or-inf with the right sign and the
 // slab / plane formulas need no special case for rays parallel to a surface.
 VG_DEV double nonzero(double a) { return fabs(a) < kTiny ? copysign_bits(kTiny, a) : a; }
@@ -53,16 +62,16 @@ VG_DEV double rcp(double a)
     return fma(r, e, r);
 }
 
-// sqrt(a) for a > 0 (normal).  y = MUFU.RSQ64H seed; g = a y; r = (1 - a y^2)/2; sqrt = g (1 + r + 1.5 r^2).
+// sqrt(a) for a > 0 (normal).  y = MUFU.RSQ64H seed; g = a y; r = 1 - a y^2; sqrt = g (1 + r/2 + 3 r^2/8):
+// five FP64 instructions.
 VG_DEV double sqrt_pos(double a)
 {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
     double g = a * y;
-    double h = 0.5 * y;
-    double r = fma(-g, h, 0.5);
-    double p = fma(1.5 * r, r, r);
-    return fma(g, p, g);
+    double r = fma(-g, y, 1.0);
+    double q = fma(r, 0.375, 0.5);
+    return fma(g * r, q, g);
 }
 #else
 VG_DEV double rcp(double a) { return 1.0 / a; }

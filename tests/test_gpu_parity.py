@@ -26,10 +26,12 @@ def vg():
 @pytest.fixture(params=["pipelined", "plain"])
 def kernel_form(request, vg):
     """Force every 16-byte aligned batch through the TMA-pipelined kernel (whatever its size), or none."""
-    old = vg.vg_get_option(vg.OPT_PIPE_MIN_N)
-    vg.vg_set_option(vg.OPT_PIPE_MIN_N, 0 if request.param == "pipelined" else vg.INT64_MAX)
+    old = vg.vg_get_option(vg.OPT_PIPE_MIN_N), vg.vg_get_option(vg.OPT_FORM)
+    vg.vg_set_option(vg.OPT_PIPE_MIN_N, 0)
+    vg.vg_set_option(vg.OPT_FORM, vg.FORM_PIPELINED if request.param == "pipelined" else vg.FORM_DIRECT)
     yield request.param
-    vg.vg_set_option(vg.OPT_PIPE_MIN_N, old)
+    vg.vg_set_option(vg.OPT_PIPE_MIN_N, old[0])
+    vg.vg_set_option(vg.OPT_FORM, old[1])
 
 
 def dev(arrs):
