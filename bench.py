@@ -339,7 +339,7 @@ def run_profile(args):
     if args.pipe_min_n is not None:
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, args.pipe_min_n)
     if args.form is not None:
-        vg.vg_set_option(vg.OPT_FORM, {"auto": vg.FORM_AUTO, "direct": vg.FORM_DIRECT, "pipelined": vg.FORM_PIPELINED}[args.form])
+        vg.vg_set_option(vg.OPT_FORM, {"auto": vg.FORM_AUTO, "direct": vg.FORM_DIRECT, "pipelined": vg.FORM_PIPELINED, "streaming": vg.FORM_STREAMING}[args.form])
     if args.no_pdl:
         vg.vg_set_option(vg.OPT_PDL, 0)
     cases = []
@@ -372,7 +372,7 @@ def run_ours(args, rank, world, local_rank):
     if args.pipe_min_n is not None:
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, args.pipe_min_n)
     if args.form is not None:
-        vg.vg_set_option(vg.OPT_FORM, {"auto": vg.FORM_AUTO, "direct": vg.FORM_DIRECT, "pipelined": vg.FORM_PIPELINED}[args.form])
+        vg.vg_set_option(vg.OPT_FORM, {"auto": vg.FORM_AUTO, "direct": vg.FORM_DIRECT, "pipelined": vg.FORM_PIPELINED, "streaming": vg.FORM_STREAMING}[args.form])
     if args.no_pdl:
         vg.vg_set_option(vg.OPT_PDL, 0)
 
@@ -490,7 +490,7 @@ def main():
     ap.add_argument("--pipe-min-n", type=int, default=None,
                     help="vg_set_option(VG_OPT_PIPE_MIN_N): batch size from which the TMA-pipelined kernel runs "
                          "(default: the library's); for A/B runs of the two kernel forms")
-    ap.add_argument("--form", choices=["auto", "direct", "pipelined"], default=None,
+    ap.add_argument("--form", choices=["auto", "direct", "pipelined", "streaming"], default=None,
                     help="vg_set_option(VG_OPT_FORM): kernel form for A/B runs (default: the library's per-kernel choice)")
     ap.add_argument("--no-pdl", action="store_true", help="vg_set_option(VG_OPT_PDL, 0): launch without programmatic dependent launch")
     ap.add_argument("--profile", action="store_true", help="eager launches of every kernel, for ncu; no timing")

@@ -165,11 +165,13 @@ int vg_compute_step_host(const vg_volume *volume, const double *x, const double 
  * latency and set-up of a kernel overlap the tail of the previous kernel in the same stream; every kernel still
  * waits (griddepcontrol.wait) for its predecessor to complete before it touches global memory, so stream order is
  * preserved exactly.  0 launches without the attribute.
- * VG_OPT_FORM (default VG_FORM_AUTO): which of the two kernel forms a query runs as.  AUTO takes the pipelined form
- * only for the (solid, query) pairs where it measured faster (profiles/), DIRECT never, PIPELINED always (subject
- * to VG_OPT_PIPE_MIN_N and the alignment rule above). */
+ * VG_OPT_FORM (default VG_FORM_AUTO): which of the three kernel forms a query runs as (same arithmetic, same
+ * results).  DIRECT: one CTA per 512 tracks.  PIPELINED: the TMA ring above (subject to VG_OPT_PIPE_MIN_N and the
+ * alignment rule).  STREAMING: one resident wave of CTAs, each owning one contiguous range of tracks and loading its
+ * next pair of tracks while it evaluates the current one (16-byte aligned arrays only).  AUTO takes, per (solid,
+ * query), the form that measured fastest (profiles/). */
 typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2 } vg_option;
-enum { VG_FORM_AUTO = 0, VG_FORM_DIRECT = 1, VG_FORM_PIPELINED = 2 };
+enum { VG_FORM_AUTO = 0, VG_FORM_DIRECT = 1, VG_FORM_PIPELINED = 2, VG_FORM_STREAMING = 3 };
 int vg_set_option(int option, int64_t value);
 int64_t vg_get_option(int option); /* the value, or VG_ERR_ARG for an unknown option */
 

@@ -61,7 +61,7 @@ extern "C" int vg_set_option(int option, int64_t value)
         vg::g_pdl.store(value != 0);
         return VG_OK;
     case VG_OPT_FORM:
-        if (value < VG_FORM_AUTO || value > VG_FORM_PIPELINED) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_FORM must be 0, 1 or 2");
+        if (value < VG_FORM_AUTO || value > VG_FORM_STREAMING) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_FORM must be 0..3");
         vg::g_form.store(value);
         return VG_OK;
     }

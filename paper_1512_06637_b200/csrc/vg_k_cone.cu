@@ -1,12 +1,23 @@
-// vg_k_cone.cu -- instantiates the streaming query kernels of the cone (five queries x {128-bit, 64-bit} paths).
+// vg_k_cone.cu -- instantiates the query kernels of the cone: the run-time-flag form (pipelined kernel, navigator)
+// and one straight-line specialisation per (hollow, phi mode), picked here from the constants.
 #include "vg_kernels.cuh"
 
 namespace vg {
 
-cudaError_t launch_cone(int q, const ConeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
-                          cudaStream_t s)
+template <int WM>
+static cudaError_t launch_cone_w(int q, const ConeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
+                                 cudaStream_t s)
 {
-    return launch_any<Cone>(q, p, t, step_max, n, out, vec, s);
+    if (p.hollow) return launch_any<Cone, ConeT<solid_flags(true, WM)>>(q, p, t, step_max, n, out, vec, s);
+    return launch_any<Cone, ConeT<solid_flags(false, WM)>>(q, p, t, step_max, n, out, vec, s);
+}
+
+cudaError_t launch_cone(int q, const ConeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
+                        cudaStream_t s)
+{
+    if (p.w.full) return launch_cone_w<kWmFull>(q, p, t, step_max, n, out, vec, s);
+    if (p.w.wide) return launch_cone_w<kWmWide>(q, p, t, step_max, n, out, vec, s);
+    return launch_cone_w<kWmNarrow>(q, p, t, step_max, n, out, vec, s);
 }
 
 } // namespace vg

@@ -64,8 +64,30 @@ VG_DEV void eval_store(const typename S::P &p, double x, double y, double z, dou
     }
 }
 
+// Per-(solid, query) launch tuning, from the sweeps recorded in profiles/ (r1c_tuning.md):
+//   minb   -- minimum resident CTAs per SM of the direct kernel, i.e. its register cap (65536 / (256 minb)).  The
+//             straight-line distance code takes ~100 registers if allowed to, which leaves 2 CTAs per SM and too
+//             few warps to cover the FP64 latencies; capped at 64 registers (4 CTAs) it runs 15-25 % faster.
+//   stream -- VG_FORM_AUTO runs the persistent streaming form (below) instead of the direct one.
+template <class S, int Q> struct Tune {
+    static constexpr int minb = (Q == qDistIn || Q == qDistOut) ? 4 : VG_MINB;
+    static constexpr bool stream = false;
+};
+template <int F> struct Tune<TubeT<F>, qDistIn> {
+    static constexpr int minb = 4;
+    static constexpr bool stream = true;
+};
+template <> struct Tune<Trd, qSafeIn> {
+    static constexpr int minb = VG_MINB;
+    static constexpr bool stream = true;
+};
+template <> struct Tune<Trd, qSafeOut> {
+    static constexpr int minb = VG_MINB;
+    static constexpr bool stream = true;
+};
+
 template <class S, int Q, int TPT>
-__global__ void __launch_bounds__(kBlock, VG_MINB) query_kernel(const __grid_constant__ typename S::P p, Tracks t,
+__global__ void __launch_bounds__(kBlock, Tune<S, Q>::minb) query_kernel(const __grid_constant__ typename S::P p, Tracks t,
                                                        double step_max, int64_t n, void *out)
 {
     constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
@@ -136,13 +158,12 @@ constexpr int kPipeThreads = 32 * kPipeWarps + 32; // + the producer warp
 constexpr int kPipeTile = 64 * kPipeWarps;         // tracks per tile: two per consumer thread
 
 extern std::atomic<int64_t> g_pipe_min_n; // vg_set_option(VG_OPT_PIPE_MIN_N)
-extern std::atomic<int64_t> g_form;       // vg_set_option(VG_OPT_FORM): 0 auto, 1 direct, 2 pipelined
+extern std::atomic<int64_t> g_form;       // vg_set_option(VG_OPT_FORM): 0 auto, 1 direct, 2 pipelined, 3 streaming
 
 // VG_FORM_AUTO: the pairs whose pipelined form measured faster than the direct one at n >= 2^22 (profiles/):
 // only the heaviest straight-line kernel, where the direct form's registers leave too few warps to overlap its
 // loads with its FP64 work.  Everything lighter is faster direct (no ring hand-offs, four to eight CTAs per SM).
 template <class S, int Q> struct PipeByDefault { static constexpr bool value = false; };
-template <> struct PipeByDefault<Cone, qDistIn> { static constexpr bool value = true; };
 
 template <class S, int Q>
 __global__ void __launch_bounds__(kPipeThreads, VG_PIPE_MINB)
@@ -262,6 +283,99 @@ __global__ void __launch_bounds__(kPipeThreads, VG_PIPE_MINB)
     }
 }
 
+// ---- the persistent streaming form: one resident wave of CTAs, each owning ONE contiguous range of track pairs ----
+//
+// Why: with one CTA per 512 tracks the direct form runs n / 512 CTAs in waves of (SM count x CTAs per SM); at
+// n = 2^20 that is 2048 CTAs over e.g. 444 resident ones = 4.6 waves, so the last wave leaves 40 % of the SMs idle,
+// and inside a wave the CTAs of an SM load and compute in step.  Here the grid is exactly one resident wave, every
+// CTA gets the same number of pairs (rounded to a warp's 512-byte row), so every SM has the same work to within
+// one row, and each thread issues the 128-bit loads of its NEXT pair before it evaluates the current one (register
+// double buffering): the loads of iteration i+1 are in flight during the FP64 work of iteration i.
+#ifndef VG_SBLOCK
+#define VG_SBLOCK 256
+#endif
+#ifndef VG_SMINB
+#define VG_SMINB 2
+#endif
+constexpr int kSBlock = VG_SBLOCK;
+
+template <class S, int Q>
+__global__ void __launch_bounds__(kSBlock, VG_SMINB)
+    query_stream_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, void *out,
+                        int64_t pairs_per_cta)
+{
+    constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
+    using S_ = S;
+    pdl_launch_dependents();
+    pdl_wait();
+    const int64_t npairs = n >> 1;
+    const int64_t lo = int64_t(blockIdx.x) * pairs_per_cta;
+    const int64_t hi = lo + pairs_per_cta < npairs ? lo + pairs_per_cta : npairs;
+    int64_t j = lo + threadIdx.x;
+    // two register sets used in turn (the loop is unrolled by two so that no set is ever copied)
+    double2 xa = make_double2(0, 0), ya = xa, za = xa, dxa = xa, dya = xa, dza = xa;
+    double2 xb = xa, yb = xa, zb = xa, dxb = xa, dyb = xa, dzb = xa;
+#define VG_LOAD_PAIR(S, J)                                                                                           \
+    do {                                                                                                             \
+        x##S = ldg2(t.x + 2 * (J)), y##S = ldg2(t.y + 2 * (J)), z##S = ldg2(t.z + 2 * (J));                          \
+        if (kDir) dx##S = ldg2(t.dx + 2 * (J)), dy##S = ldg2(t.dy + 2 * (J)), dz##S = ldg2(t.dz + 2 * (J));          \
+    } while (0)
+#define VG_EVAL_PAIR(S, J)                                                                                           \
+    do {                                                                                                             \
+        double d0 = 0, d1 = 0;                                                                                       \
+        int i0 = 0, i1 = 0;                                                                                          \
+        eval_store<S_, Q>(p, x##S.x, y##S.x, z##S.x, dx##S.x, dy##S.x, dz##S.x, step_max, d0, i0);                   \
+        eval_store<S_, Q>(p, x##S.y, y##S.y, z##S.y, dx##S.y, dy##S.y, dz##S.y, step_max, d1, i1);                   \
+        if (Q == qInside)                                                                                            \
+            stg2i(static_cast<int32_t *>(out) + 2 * (J), i0, i1);                                                    \
+        else                                                                                                         \
+            stg2(static_cast<double *>(out) + 2 * (J), d0, d1);                                                      \
+    } while (0)
+    if (j < hi) VG_LOAD_PAIR(a, j);
+    while (j < hi) {
+        if (j + kSBlock < hi) VG_LOAD_PAIR(b, j + kSBlock);
+        VG_EVAL_PAIR(a, j);
+        j += kSBlock;
+        if (j >= hi) break;
+        if (j + kSBlock < hi) VG_LOAD_PAIR(a, j + kSBlock);
+        VG_EVAL_PAIR(b, j);
+        j += kSBlock;
+    }
+#undef VG_LOAD_PAIR
+#undef VG_EVAL_PAIR
+    if ((n & 1) && blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) { // odd last track
+        const int64_t i = n - 1;
+        double x1 = ldg1(t.x + i), y1 = ldg1(t.y + i), z1 = ldg1(t.z + i);
+        double dx1 = 0, dy1 = 0, dz1 = 0;
+        if (kDir) dx1 = ldg1(t.dx + i), dy1 = ldg1(t.dy + i), dz1 = ldg1(t.dz + i);
+        double d0 = 0;
+        int i0 = 0;
+        eval_store<S, Q>(p, x1, y1, z1, dx1, dy1, dz1, step_max, d0, i0);
+        if (Q == qInside)
+            stg1i(static_cast<int32_t *>(out) + i, i0);
+        else
+            stg1(static_cast<double *>(out) + i, d0);
+    }
+}
+
+// resident CTAs of the streaming kernel on the current device (queried once per device and instantiation)
+template <class S, int Q> cudaError_t stream_capacity(int *cap)
+{
+    constexpr int kMaxDev = 64;
+    static std::atomic<int> cached[kMaxDev];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < kMaxDev && (*cap = cached[dev].load(std::memory_order_acquire)) > 0) return cudaSuccess;
+    int sms = 0, per_sm = 0;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, query_stream_kernel<S, Q>, kSBlock, 0)) != cudaSuccess)
+        return e;
+    *cap = sms * (per_sm < 1 ? 1 : per_sm);
+    if (dev >= 0 && dev < kMaxDev) cached[dev].store(*cap, std::memory_order_release);
+    return cudaSuccess;
+}
+
 // resident CTAs of the pipelined kernel on the current device (configured once per device and instantiation)
 template <class S, int Q> cudaError_t pipe_capacity(int *cap, size_t *smem_out)
 {
@@ -285,7 +399,8 @@ template <class S, int Q> cudaError_t pipe_capacity(int *cap, size_t *smem_out)
     return cudaSuccess;
 }
 
-template <class S, int Q>
+// G = the run-time-flag form of the solid (pipelined kernel), S = the specialisation picked from the flags
+template <class G, class S, int Q>
 cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
                          cudaStream_t stream)
 {
@@ -294,15 +409,27 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
     vec = false;
 #endif
     const int64_t form = g_form.load(std::memory_order_relaxed);
-    const bool pipe = form == 2 || (form == 0 && PipeByDefault<S, Q>::value);
+    const bool pipe = form == 2 || (form == 0 && PipeByDefault<G, Q>::value);
     if (vec && pipe && n >= g_pipe_min_n.load(std::memory_order_relaxed)) {
         int cap = 0;
         size_t smem = 0;
-        cudaError_t e = pipe_capacity<S, Q>(&cap, &smem);
+        cudaError_t e = pipe_capacity<G, Q>(&cap, &smem);
         if (e != cudaSuccess) return e;
         (void)cap;
         int64_t tiles = (n + kPipeTile - 1) / kPipeTile; // one CTA per tile; running CTAs cancel and take over pending ones
-        return launch_kernel(query_pipe_kernel<S, Q>, unsigned(tiles), kPipeThreads, smem, stream, p, t, step_max, n, out);
+        return launch_kernel(query_pipe_kernel<G, Q>, unsigned(tiles), kPipeThreads, smem, stream, p, t, step_max, n, out);
+    }
+    if (vec && n >= 2 && (form == 3 || (form == 0 && Tune<S, Q>::stream))) {
+        int cap = 0;
+        cudaError_t e = stream_capacity<S, Q>(&cap);
+        if (e != cudaSuccess) return e;
+        const int64_t npairs = n >> 1;
+        int64_t grid = (npairs + kSBlock - 1) / kSBlock;
+        if (grid > cap) grid = cap;
+        int64_t per = (npairs + grid - 1) / grid;
+        per = (per + 31) / 32 * 32; // a warp's row of 32 pairs = 512 contiguous bytes per array
+        grid = (npairs + per - 1) / per;
+        return launch_kernel(query_stream_kernel<S, Q>, unsigned(grid), kSBlock, 0, stream, p, t, step_max, n, out, per);
     }
     if (vec) {
         int64_t threads = (n + 1) / 2;
@@ -313,16 +440,16 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
     return launch_kernel(query_kernel<S, Q, 1>, grid, kBlock, 0, stream, p, t, step_max, n, out);
 }
 
-template <class S>
+template <class G, class S = G>
 cudaError_t launch_any(int q, const typename S::P &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
                        cudaStream_t stream)
 {
     switch (q) {
-    case qInside: return launch_query<S, qInside>(p, t, step_max, n, out, vec, stream);
-    case qDistIn: return launch_query<S, qDistIn>(p, t, step_max, n, out, vec, stream);
-    case qDistOut: return launch_query<S, qDistOut>(p, t, step_max, n, out, vec, stream);
-    case qSafeIn: return launch_query<S, qSafeIn>(p, t, step_max, n, out, vec, stream);
-    case qSafeOut: return launch_query<S, qSafeOut>(p, t, step_max, n, out, vec, stream);
+    case qInside: return launch_query<G, S, qInside>(p, t, step_max, n, out, vec, stream);
+    case qDistIn: return launch_query<G, S, qDistIn>(p, t, step_max, n, out, vec, stream);
+    case qDistOut: return launch_query<G, S, qDistOut>(p, t, step_max, n, out, vec, stream);
+    case qSafeIn: return launch_query<G, S, qSafeIn>(p, t, step_max, n, out, vec, stream);
+    case qSafeOut: return launch_query<G, S, qSafeOut>(p, t, step_max, n, out, vec, stream);
     }
     return cudaErrorInvalidValue;
 }

@@ -23,12 +23,21 @@ enum : int { cOutside = 0, cSurface = 1, cInside = 2 };
 VG_DEV int classify(bool in, bool out) { return in ? cInside : (out ? cOutside : cSurface); }
 
 // ------------------------------------------------------------------------------------------------ phi wedge
+//
+// The solids with a phi cut (tube, cone, polycone) exist in a run-time form (flags read from the constants: the
+// navigator's daughters) and in compile-time specialisations that the streaming kernels are instantiated with, so
+// that their code is straight-line: WM = -1 reads w.full / w.wide, 0 = full (no cut), 1 = dphi <= pi, 2 = dphi > pi.
+constexpr int kWmRuntime = -1, kWmFull = 0, kWmNarrow = 1, kWmWide = 2;
+
+template <int WM> VG_DEV bool w_full(const Wedge &w) { return WM < 0 ? w.full != 0 : WM == kWmFull; }
+template <int WM> VG_DEV bool w_wide(const Wedge &w) { return WM < 0 ? w.wide != 0 : WM == kWmWide; }
 
 struct WedgeEval {
     double c0, c1; // signed distances into the segment from plane 0 / plane 1 (>= 0 on the material side)
     double u0, u1; // coordinates along the two bounding half-planes (>= 0 on the half-plane itself)
 };
 
+// linear in (x, y): the same function gives the rates of c and u along a direction
 VG_DEV WedgeEval wedge_eval(const Wedge &w, double x, double y)
 {
     WedgeEval e;
@@ -39,16 +48,15 @@ VG_DEV WedgeEval wedge_eval(const Wedge &w, double x, double y)
     return e;
 }
 
-VG_DEV bool wedge_member(const Wedge &w, double c0, double c1)
+template <int WM> VG_DEV bool wedge_member(const Wedge &w, double c0, double c1)
 {
-    return w.wide ? (c0 >= 0.0 || c1 >= 0.0) : (c0 >= 0.0 && c1 >= 0.0);
+    return w_wide<WM>(w) ? (c0 >= 0.0 || c1 >= 0.0) : (c0 >= 0.0 && c1 >= 0.0);
 }
 
-VG_DEV bool in_wedge(const Wedge &w, double x, double y)
+// is the point p + t d inside the segment?  c is linear along the ray: c(t) = c(p) + t c(d)
+template <int WM> VG_DEV bool wedge_member_at(const Wedge &w, const WedgeEval &ep, const WedgeEval &ed, double t)
 {
-    double c0 = fma(w.e0x, y, -w.e0y * x);
-    double c1 = fma(w.e1y, x, -w.e1x * y);
-    return wedge_member(w, c0, c1);
+    return wedge_member<WM>(w, fma(t, ed.c0, ep.c0), fma(t, ed.c1, ep.c1));
 }
 
 // squared distance from (x, y) to the nearer of the two bounding half-planes (not the full planes)
@@ -59,10 +67,9 @@ VG_DEV double wedge_clear2(const WedgeEval &e, double rho2)
     return dmin(f0, f1);
 }
 
-VG_DEV void wedge_classify(const Wedge &w, double x, double y, double rho2, bool &in, bool &out)
+template <int WM> VG_DEV void wedge_classify(const Wedge &w, const WedgeEval &e, double rho2, bool &in, bool &out)
 {
-    WedgeEval e = wedge_eval(w, x, y);
-    bool mem = wedge_member(w, e.c0, e.c1);
+    bool mem = wedge_member<WM>(w, e.c0, e.c1);
     bool clear = wedge_clear2(e, rho2) > kTol * kTol;
     in = in && mem && clear;
     out = out || (!mem && clear);
@@ -193,24 +200,34 @@ struct Orb {
 
 // ----------------------------------------------------------------------------------------------------- tube
 
-struct Tube {
-    using P = TubeP;
+// F = -1: flags read at run time (navigator daughters); F >= 0: bit 0 = hollow, bits 1.. = wedge mode (kWm*)
+constexpr int kFlagsRuntime = -1;
+constexpr int solid_flags(bool hollow, int wm) { return (hollow ? 1 : 0) | (wm << 1); }
 
-    VG_DEV static void classify_pt(const P &p, double x, double y, double z, bool &in, bool &out)
+template <int F> struct TubeT {
+    using P = TubeP;
+    static constexpr int WM = F < 0 ? kWmRuntime : (F >> 1);
+    VG_DEV static bool hollow(const P &p) { return F < 0 ? p.hollow != 0 : (F & 1) != 0; }
+    VG_DEV static bool full(const P &p) { return w_full<WM>(p.w); }
+
+    VG_DEV static void classify_pt(const P &p, double x, double y, double z, double rho2, const WedgeEval &ep, bool &in,
+                                   bool &out)
     {
-        double rho2 = fma(x, x, y * y), az = fabs(z);
+        double az = fabs(z);
         in = az < p.dz - kTol && rho2 < p.rmax_in2;
         out = az > p.dz + kTol || rho2 > p.rmax_out2;
-        if (p.hollow) {
+        if (hollow(p)) {
             in = in && rho2 > p.rmin_in2;
             out = out || rho2 < p.rmin_out2;
         }
-        if (!p.w.full) wedge_classify(p.w, x, y, rho2, in, out);
+        if (!full(p)) wedge_classify<WM>(p.w, ep, rho2, in, out);
     }
     VG_DEV static int inside(const P &p, double x, double y, double z)
     {
         bool in, out;
-        classify_pt(p, x, y, z, in, out);
+        WedgeEval ep = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y);
+        classify_pt(p, x, y, z, fma(x, x, y * y), ep, in, out);
         return classify(in, out);
     }
     // c.3 for the rectangle [rmin, rmax] x [-dz, dz] in (rho, z) cut by the phi segment
@@ -219,16 +236,16 @@ struct Tube {
         double rho2 = fma(x, x, y * y);
         double rho = sqrt_nn(rho2);
         double qr = rho - p.rmax;
-        if (p.hollow) qr = dmax(qr, p.rmin - rho);
+        if (hollow(p)) qr = dmax(qr, p.rmin - rho);
         double qz = fabs(z) - p.dz;
         double ar = dmax(qr, 0.0), az = dmax(qz, 0.0);
         double out2 = fma(ar, ar, az * az);
         double m = dmax(qr, qz);
         bool in_rect = m < 0.0;
-        if (p.w.full) return in_rect ? m : sqrt_nn(out2);
+        if (full(p)) return in_rect ? m : sqrt_nn(out2);
         double D2 = in_rect ? m * m : out2;
         WedgeEval e = wedge_eval(p.w, x, y);
-        bool mem = wedge_member(p.w, e.c0, e.c1);
+        bool mem = wedge_member<WM>(p.w, e.c0, e.c1);
         D2 = mem ? D2 : inf();
         // the two phi faces: filled rectangle [rmin, rmax] x [-dz, dz] in the half-plane (u >= 0)
         double q0 = dmax(dmax(e.u0 - p.rmax, p.rmin - e.u0), 0.0);
@@ -240,56 +257,58 @@ struct Tube {
         return (mem && in_rect) ? -D : D;
     }
 
+    // Every candidate carries its own validity tests, so a zero denominator needs no special case: rcp(0) is NaN
+    // after the refinement, the candidate's t is NaN and fails its tests (a ray parallel to a surface does not
+    // cross it, R8).  Hit points are tested against the phi segment with c(t) = c(p) + t c(d) (linear along the ray).
     VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {
         bool in, out;
-        classify_pt(p, x, y, z, in, out);
         double rho2 = fma(x, x, y * y);
+        WedgeEval ep = {}, ed = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        classify_pt(p, x, y, z, rho2, ep, in, out);
         double a = fma(dx, dx, dy * dy);
         double b = fma(x, dx, y * dy);
-        double inv_a = rcp(nonzero(a));
+        double inv_a = rcp(a);
         double best = inf();
         // outer cylinder, entering root
         {
             double D = fma(b, b, -a * (rho2 - p.rmax2));
             double t = (-b - sqrt_pos(D)) * inv_a;
-            double zh = fma(t, dz, z);
-            bool ok = D > 0.0 && t > 0.0 && fabs(zh) <= p.dz;
-            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            bool ok = D > 0.0 && t > 0.0 && fabs(fma(t, dz, z)) <= p.dz;
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = ok ? t : best;
         }
         // inner cylinder: the ray enters the material where it LEAVES the bore
-        if (p.hollow) {
+        if (hollow(p)) {
             double D = fma(b, b, -a * (rho2 - p.rmin2));
-            double t = (-b + sqrt_pos(D)) * inv_a;
-            double zh = fma(t, dz, z);
-            bool ok = D > 0.0 && t > 0.0 && fabs(zh) <= p.dz;
-            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            double t = (sqrt_pos(D) - b) * inv_a;
+            bool ok = D > 0.0 && t > 0.0 && fabs(fma(t, dz, z)) <= p.dz;
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
-        // the cap the ray moves towards, only from beyond it
+        // the cap the ray moves towards, only from beyond it (then t > 0 by construction);
+        // rho_hit^2 = rho^2 + 2 b t + a t^2
         {
             double az = fabs(z);
-            double t = (az - p.dz) * rcp(fabs(nonzero(dz)));
-            double hx = fma(t, dx, x), hy = fma(t, dy, y);
-            double rh2 = fma(hx, hx, hy * hy);
-            bool ok = az > p.dz && z * dz < 0.0 && t > 0.0 && rh2 >= p.rmin2 && rh2 <= p.rmax2;
-            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            double t = (az - p.dz) * rcp(fabs(dz));
+            double rh2 = fma(t, fma(t, a, b + b), rho2);
+            bool ok = az > p.dz && sign_differs(z, dz) && rh2 >= p.rmin2 && rh2 <= p.rmax2;
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
-        // phi faces, entering sense: c_k(p) < 0 and c_k(d) > 0
-        if (!p.w.full) {
-            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        // phi faces, entering sense: c_k(p) < 0 and c_k(d) > 0 (then t > 0 by construction)
+        if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
-                double uh = fma(t, ed.u0, ep.u0), zh = fma(t, dz, z);
-                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && t > 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(zh) <= p.dz;
+                double uh = fma(t, ed.u0, ep.u0);
+                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(fma(t, dz, z)) <= p.dz;
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
-                double uh = fma(t, ed.u1, ep.u1), zh = fma(t, dz, z);
-                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && t > 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(zh) <= p.dz;
+                double uh = fma(t, ed.u1, ep.u1);
+                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(fma(t, dz, z)) <= p.dz;
                 best = (ok && t < best) ? t : best;
             }
         }
@@ -299,28 +318,29 @@ struct Tube {
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {
         bool in, out;
-        classify_pt(p, x, y, z, in, out);
         double rho2 = fma(x, x, y * y);
+        WedgeEval ep = {}, ed = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        classify_pt(p, x, y, z, rho2, ep, in, out);
         double a = fma(dx, dx, dy * dy);
         double b = fma(x, dx, y * dy);
-        double inv_a = rcp(nonzero(a));
+        double inv_a = rcp(a);
         double best = inf();
         {
             double D = fma(b, b, -a * (rho2 - p.rmax2));
-            double t = (-b + sqrt_pos(D)) * inv_a;
+            double t = (sqrt_pos(D) - b) * inv_a;
             best = (D > 0.0 && t > 0.0) ? t : best;
         }
-        if (p.hollow) {
+        if (hollow(p)) {
             double D = fma(b, b, -a * (rho2 - p.rmin2));
             double t = (-b - sqrt_pos(D)) * inv_a;
             best = (D > 0.0 && b < 0.0 && t > 0.0 && t < best) ? t : best;
         }
         {
-            double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(nonzero(dz)));
+            double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(dz));
             best = (t > 0.0 && t < best) ? t : best;
         }
-        if (!p.w.full) {
-            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 bool ok = ed.c0 < 0.0 && t > 0.0 && fma(t, ed.u0, ep.u0) >= 0.0;
@@ -335,6 +355,7 @@ struct Tube {
         return out ? -1.0 : best;
     }
 };
+using Tube = TubeT<kFlagsRuntime>;
 
 // ------------------------------------------------------------------------------- conical patches (cone, polycone)
 
@@ -358,28 +379,34 @@ VG_DEV double frustum_root(const Frustum &f, const RayRZ &r, double z, double dz
 
 // ----------------------------------------------------------------------------------------------------- cone
 
-struct Cone {
+template <int F> struct ConeT {
     using P = ConeP;
+    static constexpr int WM = F < 0 ? kWmRuntime : (F >> 1);
+    VG_DEV static bool hollow(const P &p) { return F < 0 ? p.hollow != 0 : (F & 1) != 0; }
+    VG_DEV static bool full(const P &p) { return w_full<WM>(p.w); }
 
-    VG_DEV static void classify_pt(const P &p, double x, double y, double z, bool &in, bool &out)
+    VG_DEV static void classify_pt(const P &p, double x, double y, double z, double rho2, const WedgeEval &ep, bool &in,
+                                   bool &out)
     {
-        double rho2 = fma(x, x, y * y), az = fabs(z);
+        double az = fabs(z);
         double ro = fma(p.out.B, z, p.out.A), to = kTol * p.out.sec;
         double ro_in = ro - to, ro_out = ro + to;
         in = az < p.dz - kTol && ro_in > 0.0 && rho2 < ro_in * ro_in;
         out = az > p.dz + kTol || rho2 > ro_out * ro_out;
-        if (p.hollow) {
+        if (hollow(p)) {
             double ri = fma(p.in.B, z, p.in.A), ti = kTol * p.in.sec;
             double ri_in = ri + ti, ri_out = ri - ti;
             in = in && (ri_in < 0.0 || rho2 > ri_in * ri_in);
             out = out || (ri_out > 0.0 && rho2 < ri_out * ri_out);
         }
-        if (!p.w.full) wedge_classify(p.w, x, y, rho2, in, out);
+        if (!full(p)) wedge_classify<WM>(p.w, ep, rho2, in, out);
     }
     VG_DEV static int inside(const P &p, double x, double y, double z)
     {
         bool in, out;
-        classify_pt(p, x, y, z, in, out);
+        WedgeEval ep = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y);
+        classify_pt(p, x, y, z, fma(x, x, y * y), ep, in, out);
         return classify(in, out);
     }
     // squared distance from (u, v) to the outline of the quadrilateral; `axis` adds the edge on the axis
@@ -388,7 +415,7 @@ struct Cone {
     {
         double ez = 2.0 * p.dz;
         double d2 = seg_d2(u, v, p.out.r0, -p.dz, p.out.er, ez, p.out.inv_l2);
-        if (p.hollow || axis) d2 = dmin(d2, seg_d2(u, v, p.in.r0, -p.dz, p.in.er, ez, p.in.inv_l2));
+        if (hollow(p) || axis) d2 = dmin(d2, seg_d2(u, v, p.in.r0, -p.dz, p.in.er, ez, p.in.inv_l2));
         double b1 = dmax(dmax(p.rmin1 - u, u - p.rmax1), 0.0), v1 = v + p.dz;
         double b2 = dmax(dmax(p.rmin2 - u, u - p.rmax2), 0.0), v2 = v - p.dz;
         d2 = dmin(d2, fma(b1, b1, v1 * v1));
@@ -405,14 +432,14 @@ struct Cone {
         double rho2 = fma(x, x, y * y);
         double rho = sqrt_nn(rho2);
         double ro = fma(p.out.B, z, p.out.A), ri = fma(p.in.B, z, p.in.A);
-        bool in2d = fabs(z) < p.dz && rho < ro && (rho > ri || !p.hollow);
+        bool in2d = fabs(z) < p.dz && rho < ro && (rho > ri || !hollow(p));
         double D2 = outline_d2(p, rho, z, false);
-        if (p.w.full) {
+        if (full(p)) {
             double D = sqrt_nn(D2);
             return in2d ? -D : D;
         }
         WedgeEval e = wedge_eval(p.w, x, y);
-        bool mem = wedge_member(p.w, e.c0, e.c1);
+        bool mem = wedge_member<WM>(p.w, e.c0, e.c1);
         D2 = mem ? D2 : inf();
         double f0 = in_quad(p, e.u0, z) ? 0.0 : outline_d2(p, e.u0, z, true);
         double f1 = in_quad(p, e.u1, z) ? 0.0 : outline_d2(p, e.u1, z, true);
@@ -425,9 +452,11 @@ struct Cone {
     VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {
         bool in, out;
-        classify_pt(p, x, y, z, in, out);
         RayRZ r;
         r.rho2 = fma(x, x, y * y);
+        WedgeEval ep = {}, ed = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        classify_pt(p, x, y, z, r.rho2, ep, in, out);
         r.a_xy = fma(dx, dx, dy * dy);
         r.b_xy = fma(x, dx, y * dy);
         double best = inf();
@@ -435,40 +464,38 @@ struct Cone {
             bool ok;
             double t = frustum_root(p.out, r, z, dz, false, ok);
             ok = ok && fabs(fma(t, dz, z)) <= p.dz;
-            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = ok ? t : best;
         }
-        if (p.hollow) {
+        if (hollow(p)) {
             bool ok;
             double t = frustum_root(p.in, r, z, dz, true, ok);
             ok = ok && fabs(fma(t, dz, z)) <= p.dz;
-            if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
         {
             double az = fabs(z);
-            double t = (az - p.dz) * rcp(fabs(nonzero(dz)));
-            double hx = fma(t, dx, x), hy = fma(t, dy, y);
-            double rh2 = fma(hx, hx, hy * hy);
+            double t = (az - p.dz) * rcp(fabs(dz)); // > 0 from beyond the cap; NaN (rejected) for dz = 0
+            double rh2 = fma(t, fma(t, r.a_xy, r.b_xy + r.b_xy), r.rho2);
             bool top = z > 0.0;
             double rlo = top ? p.rmin2 : p.rmin1, rhi = top ? p.rmax2 : p.rmax1;
-            bool ok = az > p.dz && z * dz < 0.0 && t > 0.0 && rh2 >= rlo * rlo && rh2 <= rhi * rhi;
-            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            bool ok = az > p.dz && sign_differs(z, dz) && rh2 >= rlo * rlo && rh2 <= rhi * rhi;
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
-        if (!p.w.full) {
-            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 double uh = fma(t, ed.u0, ep.u0), zh = fma(t, dz, z);
-                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && t > 0.0 && fabs(zh) <= p.dz &&
+                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && fabs(zh) <= p.dz &&
                           uh >= fma(p.in.B, zh, p.in.A) && uh <= fma(p.out.B, zh, p.out.A);
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
                 double uh = fma(t, ed.u1, ep.u1), zh = fma(t, dz, z);
-                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && t > 0.0 && fabs(zh) <= p.dz &&
+                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && fabs(zh) <= p.dz &&
                           uh >= fma(p.in.B, zh, p.in.A) && uh <= fma(p.out.B, zh, p.out.A);
                 best = (ok && t < best) ? t : best;
             }
@@ -479,9 +506,11 @@ struct Cone {
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {
         bool in, out;
-        classify_pt(p, x, y, z, in, out);
         RayRZ r;
         r.rho2 = fma(x, x, y * y);
+        WedgeEval ep = {}, ed = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        classify_pt(p, x, y, z, r.rho2, ep, in, out);
         r.a_xy = fma(dx, dx, dy * dy);
         r.b_xy = fma(x, dx, y * dy);
         double best = inf();
@@ -490,7 +519,7 @@ struct Cone {
             double t = frustum_root(p.out, r, z, dz, true, ok);
             best = ok ? t : best;
         }
-        if (p.hollow) {
+        if (hollow(p)) {
             bool ok;
             double t = frustum_root(p.in, r, z, dz, false, ok);
             // the mirror nappe (k < 0) lies beyond a cap, but guard the apex-at-the-cap case
@@ -498,11 +527,10 @@ struct Cone {
             best = (ok && t < best) ? t : best;
         }
         {
-            double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(nonzero(dz)));
+            double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(dz));
             best = (t > 0.0 && t < best) ? t : best;
         }
-        if (!p.w.full) {
-            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 bool ok = ed.c0 < 0.0 && t > 0.0 && fma(t, ed.u0, ep.u0) >= 0.0;
@@ -517,6 +545,7 @@ struct Cone {
         return out ? -1.0 : best;
     }
 };
+using Cone = ConeT<kFlagsRuntime>;
 
 // ------------------------------------------------------------------------------------------------------ trd
 
@@ -609,8 +638,10 @@ struct Trd {
 
 // ------------------------------------------------------------------------------------------------- polycone
 
-struct Polycone {
+template <int F> struct PolyconeT {
     using P = PolyconeP;
+    static constexpr int WM = F < 0 ? kWmRuntime : (F >> 1);
+    VG_DEV static bool full(const P &p) { return w_full<WM>(p.w); }
 
     VG_DEV static bool has_inner(const P &p, int k) { return (p.inner_mask >> k) & 1u; }
 
@@ -644,7 +675,7 @@ struct Polycone {
         }
         in = any_in && z > p.zlo + kTol && z < p.zhi - kTol;
         out = !any_near;
-        if (!p.w.full) wedge_classify(p.w, x, y, rho2, in, out);
+        if (!full(p)) wedge_classify<WM>(p.w, wedge_eval(p.w, x, y), rho2, in, out);
     }
     VG_DEV static int inside(const P &p, double x, double y, double z)
     {
@@ -673,12 +704,12 @@ struct Polycone {
         double rho = sqrt_nn(rho2);
         bool in2d = in_outline(p, rho, z);
         double D2 = outline_d2(p, rho, z, false);
-        if (p.w.full) {
+        if (full(p)) {
             double D = sqrt_nn(D2);
             return in2d ? -D : D;
         }
         WedgeEval e = wedge_eval(p.w, x, y);
-        bool mem = wedge_member(p.w, e.c0, e.c1);
+        bool mem = wedge_member<WM>(p.w, e.c0, e.c1);
         D2 = mem ? D2 : inf();
         double f0 = in_outline(p, e.u0, z) ? 0.0 : outline_d2(p, e.u0, z, true);
         double f1 = in_outline(p, e.u1, z) ? 0.0 : outline_d2(p, e.u1, z, true);
@@ -695,6 +726,8 @@ struct Polycone {
         r.rho2 = fma(x, x, y * y);
         r.a_xy = fma(dx, dx, dy * dy);
         r.b_xy = fma(x, dx, y * dy);
+        WedgeEval ep = {}, ed = {};
+        if (!full(p)) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
         double best = inf();
 #pragma unroll 1
         for (int k = 0; k < p.nsec; ++k) {
@@ -704,7 +737,7 @@ struct Polycone {
                 double t = frustum_root(s.out, r, z, dz, leaving, ok);
                 double zh = fma(t, dz, z);
                 ok = ok && zh >= s.z0 && zh <= s.z1;
-                if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+                if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
                 best = (ok && t < best) ? t : best;
             }
             if (has_inner(p, k)) {
@@ -712,18 +745,18 @@ struct Polycone {
                 double t = frustum_root(s.in, r, z, dz, !leaving, ok);
                 double zh = fma(t, dz, z);
                 ok = ok && zh >= s.z0 && zh <= s.z1;
-                if (!p.w.full) ok = ok && in_wedge(p.w, fma(t, dx, x), fma(t, dy, y));
+                if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
                 best = (ok && t < best) ? t : best;
             }
         }
         // end caps: entering from beyond, leaving from within
-        double idz = rcp(nonzero(dz));
+        double idz = rcp(dz); // NaN for dz = 0: both caps rejected
         {
             double t = (p.zlo - z) * idz;
             double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);
             bool sense = leaving ? dz < 0.0 : dz > 0.0;
             bool ok = sense && t > 0.0 && rh2 >= p.cap_lo_rmin * p.cap_lo_rmin && rh2 <= p.cap_lo_rmax * p.cap_lo_rmax;
-            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
         {
@@ -731,11 +764,10 @@ struct Polycone {
             double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);
             bool sense = leaving ? dz > 0.0 : dz < 0.0;
             bool ok = sense && t > 0.0 && rh2 >= p.cap_hi_rmin * p.cap_hi_rmin && rh2 <= p.cap_hi_rmax * p.cap_hi_rmax;
-            if (!p.w.full) ok = ok && in_wedge(p.w, hx, hy);
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
-        if (!p.w.full) {
-            WedgeEval ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+        if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 bool sense = leaving ? ed.c0 < 0.0 : ed.c0 > 0.0;
@@ -766,5 +798,6 @@ struct Polycone {
         return out ? -1.0 : t;
     }
 };
+using Polycone = PolyconeT<kFlagsRuntime>;
 
 } // namespace vg

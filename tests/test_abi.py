@@ -57,11 +57,11 @@ def test_options_round_trip_without_a_gpu():
     with pytest.raises(vg.VgError):
         vg.vg_set_option(vg.OPT_PIPE_MIN_N, -1)
     assert vg.vg_get_option(vg.OPT_FORM) == vg.FORM_AUTO
-    for form in (vg.FORM_DIRECT, vg.FORM_PIPELINED, vg.FORM_AUTO):
+    for form in (vg.FORM_DIRECT, vg.FORM_PIPELINED, vg.FORM_STREAMING, vg.FORM_AUTO):
         vg.vg_set_option(vg.OPT_FORM, form)
         assert vg.vg_get_option(vg.OPT_FORM) == form
     with pytest.raises(vg.VgError):
-        vg.vg_set_option(vg.OPT_FORM, 3)
+        vg.vg_set_option(vg.OPT_FORM, 4)
     with pytest.raises(vg.VgError):
         vg.vg_set_option(99, 1)
 

@@ -23,12 +23,13 @@ def vg():
     return m
 
 
-@pytest.fixture(params=["pipelined", "plain"])
+@pytest.fixture(params=["pipelined", "plain", "streaming", "auto"])
 def kernel_form(request, vg):
-    """Force every 16-byte aligned batch through the TMA-pipelined kernel (whatever its size), or none."""
+    """Force every 16-byte aligned batch through one kernel form (whatever its size), or take the library's choice."""
     old = vg.vg_get_option(vg.OPT_PIPE_MIN_N), vg.vg_get_option(vg.OPT_FORM)
     vg.vg_set_option(vg.OPT_PIPE_MIN_N, 0)
-    vg.vg_set_option(vg.OPT_FORM, vg.FORM_PIPELINED if request.param == "pipelined" else vg.FORM_DIRECT)
+    vg.vg_set_option(vg.OPT_FORM, {"pipelined": vg.FORM_PIPELINED, "plain": vg.FORM_DIRECT, "streaming": vg.FORM_STREAMING,
+                                  "auto": vg.FORM_AUTO}[request.param])
     yield request.param
     vg.vg_set_option(vg.OPT_PIPE_MIN_N, old[0])
     vg.vg_set_option(vg.OPT_FORM, old[1])
