@@ -157,6 +157,11 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         c.cap_lo_rmax = zp[2];
         c.cap_hi_rmin = zp[3 * (nz - 1) + 1];
         c.cap_hi_rmax = zp[3 * (nz - 1) + 2];
+        {
+            double rb = 0;
+            for (int i = 0; i < nz; ++i) rb = std::fmax(rb, zp[3 * i + 2]);
+            c.rb2 = rb * rb * (1 + 2e-9);
+        }
         for (int k = 0; k < nz - 1; ++k) {
             const double *a = zp + 3 * k, *b = zp + 3 * (k + 1);
             c.sec[k].z0 = a[0];

@@ -1,13 +1,22 @@
-// vg_k_polycone.cu -- instantiates the query kernels of the polycone: the run-time-flag form and the full-phi
-// specialisation (configs[3]), picked here from the constants.
-#include "vg_kernels.cuh"
+// vg_k_polycone.cu -- instantiates the query kernels of the polycone: the run-time-flag form, the full-phi
+// specialisation, and the ordered-walk kernels (vg_pcon_walk.cuh) that serve DistanceToIn and the safeties of a
+// full-phi polycone when the arrays are 16-byte aligned (VG_FORM_AUTO; any forced form runs the generic kernels).
+#include "vg_pcon_walk.cuh"
 
 namespace vg {
 
 cudaError_t launch_polycone(int q, const PolyconeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
                             cudaStream_t s)
 {
-    if (p.w.full) return launch_any<Polycone, PolyconeT<solid_flags(false, kWmFull)>>(q, p, t, step_max, n, out, vec, s);
+    if (n <= 0) return cudaSuccess;
+    if (p.w.full) {
+        if (vec && g_form.load(std::memory_order_relaxed) == 0) {
+            if (q == qDistIn) return launch_pcon_walk<qDistIn>(p, t, step_max, n, static_cast<double *>(out), s);
+            if (q == qSafeIn) return launch_pcon_walk<qSafeIn>(p, t, step_max, n, static_cast<double *>(out), s);
+            if (q == qSafeOut) return launch_pcon_walk<qSafeOut>(p, t, step_max, n, static_cast<double *>(out), s);
+        }
+        return launch_any<Polycone, PolyconeT<solid_flags(false, kWmFull)>>(q, p, t, step_max, n, out, vec, s);
+    }
     return launch_any<Polycone>(q, p, t, step_max, n, out, vec, s);
 }
 

@@ -71,6 +71,7 @@ struct PolyconeP {
     Wedge w;
     double zlo, zhi;
     double cap_lo_rmin, cap_lo_rmax, cap_hi_rmin, cap_hi_rmax;
+    double rb2; // square of the largest rmax, inflated by 1e-9 relative: bounding cylinder of the ordered walk
     PconSec sec[kMaxSec];
 };
 

@@ -1,0 +1,244 @@
+// vg_pcon_walk.cuh -- ordered-walk kernels of the full-phi polycone (configs[3]: DistanceToIn, SafetyToIn/Out).
+//
+// The generic polycone code (vg_shapes.cuh) evaluates all 2 (nz - 1) conical patches for every track.  These
+// kernels give the same results (min over the same candidates) but visit only the sections that can hold it:
+//   DistanceToIn -- z(t) is monotonic along a ray and the sections are disjoint slabs in z, so the ray meets them in
+//                   z order; every crossing found in a section is earlier than every crossing of a later section.
+//                   The ray is first clipped against the bounding cylinder (largest rmax, [zlo, zhi]): a ray that
+//                   misses it is a miss; otherwise the walk starts in the section where the clipped ray starts and
+//                   stops at the first section that yields a valid crossing or where the clipped ray ends.
+//   Safety       -- the squared distance to a segment of section k is at least the squared z gap between the point
+//                   and the slab [z0_k, z1_k]; the walk goes outwards from the point's own section, up and down,
+//                   until the gap alone exceeds the best distance so far.
+// The walks are per-lane loops with lane-dependent section indices, so the section constants are staged in shared
+// memory (one compact record per section) instead of the constant bank, whose reads serialise on divergent indices.
+#pragma once
+#include "vg_kernels.cuh"
+
+namespace vg {
+
+struct PconWalkSec {          // 14 doubles, 16-byte aligned
+    double z0, z1;
+    double Ao, Bo, Ai, Bi;    // generators r = A + B z of the outer / inner patch
+    double ro0, ero, ilo;     // outer edge (r0, z0) -> (r0 + er, z1), 1 / |edge|^2
+    double ri0, eri, ili;     // inner edge
+    double seco, seci;        // sqrt(1 + B^2) of both patches (tolerance band of the Inside test)
+};
+
+constexpr int kWalkBlock = 256;
+
+VG_DEV void pcon_stage(const PolyconeP &p, PconWalkSec *tab)
+{
+    for (int k = threadIdx.x; k < p.nsec; k += blockDim.x) {
+        const PconSec &s = p.sec[k];
+        PconWalkSec w;
+        w.z0 = s.z0, w.z1 = s.z1;
+        w.Ao = s.out.A, w.Bo = s.out.B, w.Ai = s.in.A, w.Bi = s.in.B;
+        w.ro0 = s.out.r0, w.ero = s.out.er, w.ilo = s.out.inv_l2;
+        w.ri0 = s.in.r0, w.eri = s.in.er, w.ili = s.in.inv_l2;
+        w.seco = s.out.sec, w.seci = s.in.sec;
+        tab[k] = w;
+    }
+}
+
+// index of the section whose slab holds z: number of internal planes <= z (warp-uniform loop, constant-bank reads)
+VG_DEV int pcon_section_of(const PolyconeP &p, double z)
+{
+    int k = 0;
+#pragma unroll 1
+    for (int j = 1; j < p.nsec; ++j) k += (p.sec[j].z0 <= z) ? 1 : 0;
+    return k;
+}
+
+// three section indices in one warp-uniform pass over the internal planes
+VG_DEV void pcon_sections_of(const PolyconeP &p, double za, double zb, double zc, int &ka, int &kb, int &kc)
+{
+    ka = kb = kc = 0;
+#pragma unroll 1
+    for (int j = 1; j < p.nsec; ++j) {
+        const double zp = p.sec[j].z0;
+        ka += (zp <= za) ? 1 : 0;
+        kb += (zp <= zb) ? 1 : 0;
+        kc += (zp <= zc) ? 1 : 0;
+    }
+}
+
+// DistanceToIn of the full-phi polycone; same candidates and validity tests as PolyconeT::dist_in
+VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z, double dx,
+                                double dy, double dz)
+{
+    RayRZ r;
+    r.rho2 = fma(x, x, y * y);
+    r.a_xy = fma(dx, dx, dy * dy);
+    r.b_xy = fma(x, dx, y * dy);
+    const double a = r.a_xy, b = r.b_xy;
+
+    // clip the ray against the bounding cylinder rho^2 <= rb2, zlo - slack <= z <= zhi + slack
+    const double kSlack = 1e-7;
+    const double c = r.rho2 - p.rb2;
+    const double D = fma(b, b, -a * c);
+    const double s = sqrt_pos(D);
+    const double inv_a = rcp(a);
+    const bool vertical = !(a >= kTiny); // ray parallel to the axis
+    const double tr0 = vertical ? -inf() : (-b - s) * inv_a;
+    const double tr1 = vertical ? inf() : (s - b) * inv_a;
+    const bool rad_ok = vertical ? c <= 0.0 : D > 0.0;
+    const bool horizontal = !(fabs(dz) >= kTiny);
+    const double idz = rcp(dz);
+    const double ta = (p.zlo - z) * idz, tb = (p.zhi - z) * idz; // times of the two end planes
+    const double sl = kSlack * fabs(idz);
+    const bool up = not_neg(dz);
+    const double tz0 = horizontal ? -inf() : (up ? ta : tb) - sl;
+    const double tz1 = horizontal ? inf() : (up ? tb : ta) + sl;
+    const bool z_ok = horizontal ? (z >= p.zlo && z <= p.zhi) : true;
+    const double t0 = dmax(dmax(tr0, tz0), 0.0), t1 = dmin(tr1, tz1);
+    const double zs = fma(t0, dz, z), ze = fma(t1, dz, z);
+
+    int kz, k, kend;
+    pcon_sections_of(p, z, (up ? zs : ze) - kSlack, (up ? ze : zs) + kSlack, kz, k, kend);
+
+    // Inside (R6: strictly inside by kTol) on the point's own section
+    bool in;
+    {
+        const PconWalkSec &w = tab[kz];
+        const double ro = fma(w.Bo, z, w.Ao) - kTol * w.seco;
+        const double ri = fma(w.Bi, z, w.Ai) + kTol * w.seci;
+        const bool inner = (p.inner_mask >> kz) & 1u;
+        in = z > p.zlo + kTol && z < p.zhi - kTol && ro > 0.0 && r.rho2 < ro * ro && (!inner || ri < 0.0 || r.rho2 > ri * ri);
+    }
+
+    // a ray that starts beyond an end plane meets that cap before anything else
+    const double tc = up ? ta : tb;
+    const double rc2 = fma(tc, fma(tc, a, b + b), r.rho2);
+    const double clo = up ? p.cap_lo_rmin : p.cap_hi_rmin, chi = up ? p.cap_lo_rmax : p.cap_hi_rmax;
+    const bool beyond = up ? z < p.zlo : z > p.zhi;
+    const bool cap_hit = beyond && !horizontal && rc2 >= clo * clo && rc2 <= chi * chi;
+
+    double best = cap_hit ? tc : inf();
+    bool go = rad_ok && z_ok && t0 <= t1 && !in && !cap_hit;
+    if (!up) {
+        const int tmp = k;
+        k = kend;
+        kend = tmp;
+    }
+    const int step = up ? 1 : -1;
+    while (go) {
+        const PconWalkSec w = tab[k];
+        Frustum f;
+        bool ok;
+        f.A = w.Ao, f.B = w.Bo;
+        double t = frustum_root(f, r, z, dz, false, ok); // outer patch, entering root
+        double zh = fma(t, dz, z);
+        ok = ok && zh >= w.z0 && zh <= w.z1;
+        best = (ok && t < best) ? t : best;
+        f.A = w.Ai, f.B = w.Bi;
+        t = frustum_root(f, r, z, dz, true, ok); // inner patch: the ray enters where it leaves the bore
+        zh = fma(t, dz, z);
+        ok = ok && ((p.inner_mask >> k) & 1u) && zh >= w.z0 && zh <= w.z1;
+        best = (ok && t < best) ? t : best;
+        go = !(best < inf()) && k != kend;
+        k += step;
+    }
+    return in ? -1.0 : best;
+}
+
+// exact signed distance of the full-phi polycone; same segments as PolyconeT::safety
+VG_DEV double pcon_walk_sdf(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z)
+{
+    const double rho2 = fma(x, x, y * y);
+    const double rho = sqrt_nn(rho2);
+    const int kz = pcon_section_of(p, z);
+    bool in2d;
+    {
+        const PconWalkSec &w = tab[kz];
+        in2d = z >= p.zlo && z <= p.zhi && rho <= fma(w.Bo, z, w.Ao) && rho >= fma(w.Bi, z, w.Ai);
+    }
+    const double b1 = dmax(dmax(p.cap_lo_rmin - rho, rho - p.cap_lo_rmax), 0.0), v1 = z - p.zlo;
+    const double b2 = dmax(dmax(p.cap_hi_rmin - rho, rho - p.cap_hi_rmax), 0.0), v2 = z - p.zhi;
+    double d2 = dmin(fma(b1, b1, v1 * v1), fma(b2, b2, v2 * v2));
+    for (int k = kz; k < p.nsec; ++k) { // upwards
+        const PconWalkSec w = tab[k];
+        const double gap = dmax(w.z0 - z, 0.0);
+        if (gap * gap >= d2) break;
+        const double ez = w.z1 - w.z0;
+        d2 = dmin(d2, seg_d2(rho, z, w.ro0, w.z0, w.ero, ez, w.ilo));
+        const double di = seg_d2(rho, z, w.ri0, w.z0, w.eri, ez, w.ili);
+        d2 = ((p.inner_mask >> k) & 1u) ? dmin(d2, di) : d2;
+    }
+    for (int k = kz - 1; k >= 0; --k) { // downwards
+        const PconWalkSec w = tab[k];
+        const double gap = dmax(z - w.z1, 0.0);
+        if (gap * gap >= d2) break;
+        const double ez = w.z1 - w.z0;
+        d2 = dmin(d2, seg_d2(rho, z, w.ro0, w.z0, w.ero, ez, w.ilo));
+        const double di = seg_d2(rho, z, w.ri0, w.z0, w.eri, ez, w.ili);
+        d2 = ((p.inner_mask >> k) & 1u) ? dmin(d2, di) : d2;
+    }
+    const double dist = sqrt_nn(d2);
+    return in2d ? -dist : dist;
+}
+
+template <int Q> VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z,
+                                              double dx, double dy, double dz, double step_max)
+{
+    if (Q == qSafeIn) return pcon_walk_sdf(p, tab, x, y, z);
+    if (Q == qSafeOut) return -pcon_walk_sdf(p, tab, x, y, z);
+    const double t = pcon_walk_dist_in(p, tab, x, y, z, dx, dy, dz);
+    return t <= step_max ? t : inf();
+}
+
+#ifndef VG_WALK_MINB
+#define VG_WALK_MINB 3
+#endif
+
+// persistent CTAs striding over tiles of 512 tracks, two tracks per thread (128-bit loads; arrays 16-byte aligned)
+template <int Q>
+__global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
+    pcon_walk_kernel(const __grid_constant__ PolyconeP p, Tracks t, double step_max, int64_t n, double *out)
+{
+    constexpr bool kDir = (Q == qDistIn);
+    __shared__ __align__(16) PconWalkSec tab[kMaxSec];
+    pcon_stage(p, tab);
+    pdl_launch_dependents();
+    __syncthreads();
+    pdl_wait();
+    const int64_t npairs = (n + 1) >> 1;
+    for (int64_t j = int64_t(blockIdx.x) * kWalkBlock + threadIdx.x; j < npairs; j += int64_t(gridDim.x) * kWalkBlock) {
+        const int64_t i = 2 * j;
+        if (i + 1 < n) {
+            double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
+            double2 dx = make_double2(0, 0), dy = dx, dz = dx;
+            if (kDir) dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
+            const double r0 = pcon_walk_eval<Q>(p, tab, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max);
+            const double r1 = pcon_walk_eval<Q>(p, tab, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max);
+            stg2(out + i, r0, r1);
+        } else {
+            double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+            double dx = 0, dy = 0, dz = 0;
+            if (kDir) dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+            stg1(out + i, pcon_walk_eval<Q>(p, tab, x, y, z, dx, dy, dz, step_max));
+        }
+    }
+}
+
+template <int Q>
+cudaError_t launch_pcon_walk(const PolyconeP &p, const Tracks &t, double step_max, int64_t n, double *out, cudaStream_t s)
+{
+    static std::atomic<int> cap_cache{ 0 };
+    int cap = cap_cache.load(std::memory_order_acquire);
+    if (cap <= 0) {
+        int dev = 0, sms = 0, per_sm = 0;
+        cudaError_t e;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_walk_kernel<Q>, kWalkBlock, 0)) != cudaSuccess) return e;
+        cap = sms * (per_sm < 1 ? 1 : per_sm);
+        cap_cache.store(cap, std::memory_order_release);
+    }
+    const int64_t npairs = (n + 1) >> 1;
+    int64_t grid = (npairs + kWalkBlock - 1) / kWalkBlock;
+    if (grid > cap) grid = cap;
+    return launch_kernel(pcon_walk_kernel<Q>, unsigned(grid), kWalkBlock, 0, s, p, t, step_max, n, out);
+}
+
+} // namespace vg
