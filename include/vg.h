@@ -106,6 +106,18 @@ int vg_safety_to_out(const vg_shape *shape, const double *x, const double *y, co
                      double *safety, void *stream);
 
 /*
+ * vg_query_all -- the five answers of n tracks in one call (a basket of particles in one volume asks all three
+ * questions of PAPER.md:110-114 every step).  Same results, element by element, as the five
+ * calls above.  Any output pointer may be NULL (that answer is skipped; at least one must be given).  When all five
+ * are given and the solid is not a polycone, ONE fused kernel reads the six track arrays once (48 B per track
+ * instead of 168 B) and writes the five results; otherwise the call enqueues one kernel per requested answer.
+ * cls: DEVICE int32[n]; the other four: DEVICE double[n]; dx, dy, dz and step_max as for vg_distance_to_in.
+ */
+int vg_query_all(const vg_shape *shape, const double *x, const double *y, const double *z, const double *dx,
+                 const double *dy, const double *dz, double step_max, int64_t n, int32_t *cls, double *dist_in,
+                 double *dist_out, double *safety_in, double *safety_out, void *stream);
+
+/*
  * vg_volume_create -- a mother solid holding ndaughters placed solids ("coordinate
  * transformations"; BASELINE.json configs[4]).  `xforms` (HOST): ndaughters * 12 doubles, row-major 3x4
  * [R | b] per daughter, mother -> daughter-local: p_loc = R p + b, d_loc = R d (reading R12).  R is

@@ -45,6 +45,7 @@ def _load():
         getattr(lib, name).argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP]
     for name in ("vg_safety_to_in", "vg_safety_to_out"):
         getattr(lib, name).argtypes = [_VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
+    lib.vg_query_all.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64] + [_VP] * 5 + [_VP]
     lib.vg_volume_create.argtypes = [_VP, C.c_int, C.POINTER(_VP), _PD, C.POINTER(_VP)]
     lib.vg_volume_destroy.argtypes = [_VP]
     lib.vg_volume_destroy.restype = None
@@ -174,6 +175,19 @@ def vg_safety_to_in(shape, x, y, z, out=None, stream=None):
 
 def vg_safety_to_out(shape, x, y, z, out=None, stream=None):
     return _safe(_lib.vg_safety_to_out, shape, x, y, z, out, stream)
+
+
+def vg_query_all(shape, x, y, z, dx, dy, dz, step_max=math.inf, out=None, stream=None):
+    """All five answers in one call (one fused kernel for every solid but the polycone).  `out`: optional tuple
+    (cls int32, dist_in, dist_out, safety_in, safety_out) of preallocated tensors.  Returns that tuple."""
+    n, dev = _tracks((x, y, z, dx, dy, dz))
+    out = tuple(out) if out is not None else (None,) * 5
+    cls = _out(out[0], n, dev, torch.int32)
+    res = [_out(o, n, dev, torch.float64) for o in out[1:]]
+    with torch.cuda.device(dev):
+        _check(_lib.vg_query_all(_handle(shape), _p(x), _p(y), _p(z), _p(dx), _p(dy), _p(dz), float(step_max), n, _p(cls),
+                                 *[_p(r) for r in res], _stream(stream)))
+    return (cls, *res)
 
 
 def vg_volume_create(mother, daughters, xforms):
@@ -308,6 +322,9 @@ class Shape:
         if name in ("distance_to_in", "distance_to_out"):
             return getattr(self, name)(x, y, z, dx, dy, dz, step_max, **kw)
         return getattr(self, name)(x, y, z, **kw)
+
+    def query_all(self, x, y, z, dx, dy, dz, step_max=math.inf, **kw):
+        return vg_query_all(self, x, y, z, dx, dy, dz, step_max, **kw)
 
     def query_host(self, name, x, y, z, dx=None, dy=None, dz=None, step_max=math.inf, out=None):
         return vg_query_host(self, name, x, y, z, dx, dy, dz, step_max, out)

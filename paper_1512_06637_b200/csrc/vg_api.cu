@@ -182,6 +182,50 @@ extern "C" int vg_safety_to_out(const vg_shape *s, const double *x, const double
     return run_query("vg_safety_to_out", qSafeOut, s, x, y, z, nullptr, nullptr, nullptr, 0.0, n, safety, stream);
 }
 
+extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y, const double *z, const double *dx,
+                            const double *dy, const double *dz, double step_max, int64_t n, int32_t *cls,
+                            double *dist_in, double *dist_out, double *safety_in, double *safety_out, void *stream)
+{
+    const char *fn = "vg_query_all";
+    if (!s) return fail(VG_ERR_ARG, "%s: shape is NULL", fn);
+    const bool all = cls && dist_in && dist_out && safety_in && safety_out;
+    if (!all || s->kind == VG_POLYCONE) { // a subset, or no fused kernel for this solid: one launch per requested answer
+        if (!cls && !dist_in && !dist_out && !safety_in && !safety_out) return fail(VG_ERR_ARG, "%s: every output is NULL", fn);
+        int rc = VG_OK;
+        if (cls && rc == VG_OK) rc = vg_inside(s, x, y, z, n, cls, stream);
+        if (dist_in && rc == VG_OK) rc = vg_distance_to_in(s, x, y, z, dx, dy, dz, step_max, n, dist_in, stream);
+        if (dist_out && rc == VG_OK) rc = vg_distance_to_out(s, x, y, z, dx, dy, dz, step_max, n, dist_out, stream);
+        if (safety_in && rc == VG_OK) rc = vg_safety_to_in(s, x, y, z, n, safety_in, stream);
+        if (safety_out && rc == VG_OK) rc = vg_safety_to_out(s, x, y, z, n, safety_out, stream);
+        return rc;
+    }
+    const void *ptrs[6] = { x, y, z, dx, dy, dz };
+    bool vec = false, v2 = false;
+    int rc = check_arrays(fn, ptrs, 6, 4, cls, n, &vec);
+    if (rc != VG_OK) return rc;
+    double *outs[4] = { dist_in, dist_out, safety_in, safety_out };
+    for (int i = 0; i < 4; ++i) {
+        if ((rc = check_arrays(fn, ptrs, 6, 8, outs[i], n, &v2)) != VG_OK) return rc;
+        vec = vec && v2;
+    }
+    if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
+    if (n == 0) return VG_OK;
+    Tracks t{ x, y, z, dx, dy, dz };
+    AllOut o{ cls, dist_in, dist_out, safety_in, safety_out };
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (s->kind) {
+    case VG_BOX: e = launch_box_all(s->u.box, t, step_max, n, o, vec, st); break;
+    case VG_ORB: e = launch_orb_all(s->u.orb, t, step_max, n, o, vec, st); break;
+    case VG_TUBE: e = launch_tube_all(s->u.tube, t, step_max, n, o, vec, st); break;
+    case VG_CONE: e = launch_cone_all(s->u.cone, t, step_max, n, o, vec, st); break;
+    case VG_TRD: e = launch_trd_all(s->u.trd, t, step_max, n, o, vec, st); break;
+    default: break;
+    }
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
 // ---------------------------------------------------------------------------------------------- navigation
 
 // radius of a sphere about the local origin that contains the solid (phi cuts ignored)

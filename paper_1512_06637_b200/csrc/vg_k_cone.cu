@@ -20,4 +20,20 @@ cudaError_t launch_cone(int q, const ConeP &p, const Tracks &t, double step_max,
     return launch_cone_w<kWmNarrow>(q, p, t, step_max, n, out, vec, s);
 }
 
+template <int WM>
+static cudaError_t launch_cone_all_w(const ConeP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec,
+                                     cudaStream_t s)
+{
+    if (p.hollow) return launch_all<ConeT<solid_flags(true, WM)>>(p, t, step_max, n, o, vec, s);
+    return launch_all<ConeT<solid_flags(false, WM)>>(p, t, step_max, n, o, vec, s);
+}
+
+cudaError_t launch_cone_all(const ConeP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec,
+                            cudaStream_t s)
+{
+    if (p.w.full) return launch_cone_all_w<kWmFull>(p, t, step_max, n, o, vec, s);
+    if (p.w.wide) return launch_cone_all_w<kWmWide>(p, t, step_max, n, o, vec, s);
+    return launch_cone_all_w<kWmNarrow>(p, t, step_max, n, o, vec, s);
+}
+
 } // namespace vg

@@ -9,4 +9,10 @@ cudaError_t launch_trd(int q, const TrdP &p, const Tracks &t, double step_max, i
     return launch_any<Trd>(q, p, t, step_max, n, out, vec, s);
 }
 
+cudaError_t launch_trd_all(const TrdP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec,
+                           cudaStream_t s)
+{
+    return launch_all<Trd>(p, t, step_max, n, o, vec, s);
+}
+
 } // namespace vg

@@ -129,6 +129,80 @@ __global__ void __launch_bounds__(kBlock, Tune<S, Q>::minb) query_kernel(const _
     }
 }
 
+// ---- the fused "basket" kernel: all five answers of a track from one pass over its six coordinates ----
+//
+// A basket of particles in one volume asks all three questions of the paper every step (SURVEY.md
+// sec. 8(f) f1).  Five separate launches read 3 x 24 + 2 x 48 = 168 B and write 36 B per track and pay five launch
+// latencies; this kernel reads 48 B and writes 36 B once.  The per-solid functions are inlined into one
+// straight-line body, so the compiler shares their common subexpressions (rho^2, the classification, the phi terms).
+struct AllOut {
+    int32_t *cls;
+    double *din, *dout, *sin, *sout;
+};
+
+#ifndef VG_ALL_MINB
+#define VG_ALL_MINB 2
+#endif
+
+template <class S>
+VG_DEV void eval_all(const typename S::P &p, double x, double y, double z, double dx, double dy, double dz,
+                     double step_max, int &cls, double &din, double &dout, double &sdf)
+{
+    cls = S::inside(p, x, y, z);
+    sdf = S::safety(p, x, y, z);
+    const double a = S::dist_in(p, x, y, z, dx, dy, dz), b = S::dist_out(p, x, y, z, dx, dy, dz);
+    din = a <= step_max ? a : inf();
+    dout = b <= step_max ? b : inf();
+}
+
+template <class S, int TPT>
+__global__ void __launch_bounds__(kBlock, VG_ALL_MINB)
+    query_all_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, AllOut o)
+{
+    int64_t i = (int64_t(blockIdx.x) * kBlock + threadIdx.x) * TPT;
+    pdl_launch_dependents();
+    pdl_wait();
+    if (i >= n) return;
+    if (TPT == 2 && i + 1 < n) {
+        double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
+        double2 dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
+        int c0, c1;
+        double a0, a1, b0, b1, s0, s1;
+        eval_all<S>(p, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max, c0, a0, b0, s0);
+        eval_all<S>(p, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max, c1, a1, b1, s1);
+        stg2i(o.cls + i, c0, c1);
+        stg2(o.din + i, a0, a1);
+        stg2(o.dout + i, b0, b1);
+        stg2(o.sin + i, s0, s1);
+        stg2(o.sout + i, -s0, -s1);
+    } else {
+        double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+        double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+        int c0;
+        double a0, b0, s0;
+        eval_all<S>(p, x, y, z, dx, dy, dz, step_max, c0, a0, b0, s0);
+        stg1i(o.cls + i, c0);
+        stg1(o.din + i, a0);
+        stg1(o.dout + i, b0);
+        stg1(o.sin + i, s0);
+        stg1(o.sout + i, -s0);
+    }
+}
+
+template <class S>
+cudaError_t launch_all(const typename S::P &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec,
+                       cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    if (vec) {
+        int64_t threads = (n + 1) / 2;
+        unsigned grid = unsigned((threads + kBlock - 1) / kBlock);
+        return launch_kernel(query_all_kernel<S, 2>, grid, kBlock, 0, stream, p, t, step_max, n, o);
+    }
+    unsigned grid = unsigned((n + kBlock - 1) / kBlock);
+    return launch_kernel(query_all_kernel<S, 1>, grid, kBlock, 0, stream, p, t, step_max, n, o);
+}
+
 // ---- the pipelined form of the same kernel (the default for 16-byte aligned arrays and n >= g_pipe_min_n) ----
 //
 // Why: the plain kernel above keeps a thread's loads in flight only until its own arithmetic starts; with 60-90
@@ -467,6 +541,13 @@ cudaError_t launch_trd(int q, const TrdP &p, const Tracks &t, double step_max, i
                        cudaStream_t s);
 cudaError_t launch_polycone(int q, const PolyconeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
                             cudaStream_t s);
+
+// the fused five-query kernel of each solid (the polycone has none: its queries run as five launches)
+cudaError_t launch_box_all(const BoxP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
+cudaError_t launch_orb_all(const OrbP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
+cudaError_t launch_tube_all(const TubeP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
+cudaError_t launch_cone_all(const ConeP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
+cudaError_t launch_trd_all(const TrdP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
 
 // navigation (vg_nav.cu)
 cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,

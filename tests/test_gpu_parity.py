@@ -62,14 +62,24 @@ def check_all(vg, kind, params, t, queries=W.QUERIES5, step_max=W.STEP_MAX, what
     so, sg = O.Shape(kind, params), vg.Shape(kind, params)
     dt = dev(t)
     worst = 0.0
+    ref = {}
     for q in queries:
-        o = run_oracle(so, q, t, step_max)
+        o = ref[q] = run_oracle(so, q, t, step_max)
         g = run_gpu(sg, q, dt, step_max)
         tag = "%s %s n=%d" % (what, q, len(t[0]))
         if q == "inside":
             assert_int_equal(g, o, tag)
         else:
             worst = max(worst, assert_real_close(g, o, tag))
+    if tuple(queries) == tuple(W.QUERIES5) and len(t[0]) > 0:  # the fused five-query entry point against the same oracle values
+        fused = sg.query_all(*dt, step_max)
+        torch.cuda.synchronize()
+        for q, g in zip(W.QUERIES5, fused):
+            tag = "%s fused %s n=%d" % (what, q, len(t[0]))
+            if q == "inside":
+                assert_int_equal(g.cpu().numpy(), ref[q], tag)
+            else:
+                worst = max(worst, assert_real_close(g.cpu().numpy(), ref[q], tag))
     return worst
 
 
@@ -140,6 +150,42 @@ def test_tiny_sizes(vg, kernel_form, n):
         assert sg.inside(*e[:3]).numel() == 0 and sg.distance_to_in(*e).numel() == 0
         return
     check_all(vg, sc.kind, sc.params, t, what="tiny")
+
+
+def test_query_all_subsets_and_misaligned_outputs(vg):
+    """vg_query_all: NULL outputs are skipped (one kernel per requested answer), all five run fused; outputs that are
+    only 8-byte aligned take the 64-bit path; guard elements stay untouched."""
+    import ctypes as C
+    sc = W.shape_cases(1)[0]
+    so, sg = O.Shape(sc.kind, sc.params), vg.Shape(sc.kind, sc.params)
+    n = 4099
+    t = sc.tracks(n, band=oracle_band(so))
+    dt = dev(t)
+    ref = {q: run_oracle(so, q, t, W.STEP_MAX) for q in W.QUERIES5}
+    # misaligned outputs (offset 1) with guards
+    bufs = [torch.full((n + 3,), -7, dtype=torch.int32, device="cuda")] + \
+           [torch.full((n + 3,), -7.0, dtype=torch.float64, device="cuda") for _ in range(4)]
+    before = vg.vg_launch_count()
+    sg.query_all(*dt, W.STEP_MAX, out=[b[1:n + 1] for b in bufs])
+    torch.cuda.synchronize()
+    assert vg.vg_launch_count() - before == 1
+    for q, b in zip(W.QUERIES5, bufs):
+        assert b[0].item() == -7 and (b[n + 1:] == -7).all()
+        g = b[1:n + 1].cpu().numpy()
+        assert_int_equal(g, ref[q], "fused off=1 " + q) if q == "inside" else assert_real_close(g, ref[q], "fused off=1 " + q)
+    # a subset through the raw C ABI: NULL pointers skip that answer
+    din = torch.empty(n, dtype=torch.float64, device="cuda")
+    sout = torch.empty(n, dtype=torch.float64, device="cuda")
+    null = C.c_void_p(0)
+    p = [C.c_void_p(a.data_ptr()) for a in dt]
+    before = vg.vg_launch_count()
+    rc = vg._lib.vg_query_all(sg._h, *p, float(W.STEP_MAX), n, null, C.c_void_p(din.data_ptr()), null, null,
+                              C.c_void_p(sout.data_ptr()), C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    torch.cuda.synchronize()
+    assert rc == 0 and vg.vg_launch_count() - before == 2
+    assert_real_close(din.cpu().numpy(), ref["distance_to_in"], "subset din")
+    assert_real_close(sout.cpu().numpy(), ref["safety_to_out"], "subset sout")
+    assert vg._lib.vg_query_all(sg._h, *p, float(W.STEP_MAX), n, null, null, null, null, null, null) == vg.ERR_ARG
 
 
 def test_outputs_do_not_overrun(vg, kernel_form):
