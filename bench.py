@@ -32,7 +32,7 @@ METRIC = "tracks/sec per query per shape (1 B200) and fraction of HBM / FP64 roo
 UNIT = "track-queries/s"
 # algorithmic bytes per track: SoA inputs read once + one result written once
 BYTES = {"inside": 24 + 4, "safety_to_in": 24 + 8, "safety_to_out": 24 + 8, "distance_to_in": 48 + 8,
-         "distance_to_out": 48 + 8, "compute_step": 48 + 12}
+         "distance_to_out": 48 + 8, "compute_step": 48 + 12, "all": 48 + 4 + 4 * 8}
 L2_BYTES = 126e6
 HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
 
@@ -139,6 +139,7 @@ class Case:
         self.sets = [base] + [[a.clone() for a in base] for _ in range(self.nsets - 1)]
         self.outd = [torch.empty(self.n, dtype=torch.float64, device=dev) for _ in range(self.nsets)]
         self.outi = [torch.empty(self.n, dtype=torch.int32, device=dev) for _ in range(self.nsets)]
+        self.out4 = None  # four more result arrays per set, allocated on the first fused launch
         self.cursor = 0
 
     def _gpu3(self, fn, x, y, z):
@@ -151,7 +152,11 @@ class Case:
         k = self.cursor
         self.cursor = (k + 1) % self.nsets
         s = self.sets[k]
-        if q == "compute_step":
+        if q == "all":  # the fused five-query call (vg_query_all)
+            if self.out4 is None:
+                self.out4 = [[self.torch.empty_like(self.outd[0]) for _ in range(3)] for _ in range(self.nsets)]
+            self.handle.query_all(*s, W.STEP_MAX, out=[self.outi[k], self.outd[k]] + self.out4[k])
+        elif q == "compute_step":
             self.handle.compute_step(*s, step_max=W.STEP_MAX, step=self.outd[k], hit=self.outi[k])
         elif q == "inside":
             self.handle.inside(*s[:3], out=self.outi[k])
@@ -318,6 +323,12 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
             e = roofline_entry(case.kind, q, n, sec, hbm_peak, fma_rate)
             e.update({"config": k, "shape": sc.name, "query": q, "n": n, "cold_inputs": case.cold})
             rows.append(e)
+        if len(sc.queries) == 5 and sc.kind != W.POLYCONE:  # the fused five-query kernel on the same tracks
+            sec = time_query_alone(torch, case, "all")
+            e = roofline_entry(case.kind, "all", n, sec, hbm_peak, fma_rate)
+            e.update({"config": k, "shape": sc.name, "query": "all five (vg_query_all, one kernel)", "n": n, "cold_inputs": case.cold,
+                      "track_queries_per_s": 5 * n / sec})
+            rows.append(e)
         if case is not main_case:
             del case
             torch.cuda.empty_cache()
@@ -412,7 +423,8 @@ def run_ours(args, rank, world, local_rank):
 
     per_query = {q: roofline_entry(case.kind, q, case.n, per_q[q], hbm_peak, fma_rate) for q in case.queries}
     dom = max(case.queries, key=lambda q: per_q[q])
-    roof = {"bound": "hbm", "kernel": "query_kernel<Tube, %s>" % dom, "achieved": per_query[dom]["hbm_gbs"],
+    kname = ("query_stream_kernel<TubeT<hollow, wide phi>, %s>" if dom == "distance_to_in" else "query_kernel<TubeT<hollow, wide phi>, %s>") % dom
+    roof = {"bound": "hbm", "kernel": kname, "achieved": per_query[dom]["hbm_gbs"],
             "peak": hbm_peak, "unit": "GB/s", "frac": per_query[dom]["hbm_gbs"] / hbm_peak, "peak_source": hbm_src,
             "traffic": (ncu_traffic("Tube", dom, case.n) or {}).get("bytes"), "traffic_detail": ncu_traffic("Tube", dom, case.n),
             "algorithmic_bytes_per_launch": BYTES[dom] * case.n,
@@ -421,30 +433,49 @@ def run_ours(args, rank, world, local_rank):
             "kernel_timing": kernel_timing,
             "step_hbm_frac": sum(BYTES[q] for q in case.queries) * case.n / (ms * 1e-3 / args.steps) / 1e9 / hbm_peak}
 
-    # end to end: pinned host arrays -> C-ABI host entry points -> host results, copies inside the timed region
+    # the same step as ONE fused kernel (vg_query_all): 48 B read + 36 B written per track instead of 168 + 36
+    fused_s = time_query_alone(torch, case, "all")
+    fused = {"us_per_step": fused_s * 1e6, "value": nq * case.n / fused_s, "unit": UNIT, "api": "vg_query_all (one kernel, five results)",
+             "hbm_gbs": BYTES["all"] * case.n / fused_s / 1e9, "hbm_frac": BYTES["all"] * case.n / fused_s / 1e9 / hbm_peak,
+             "algorithmic_bytes_per_track": BYTES["all"], "speedup_vs_five_launches": sum(per_q.values()) / fused_s,
+             "note": "reported beside `value`, which stays the five per-query launches BASELINE.json's metric names"}
+
+    # end to end: pinned host arrays -> C-ABI host entry point -> pinned host results, copies inside the timed region.
+    # The call a user makes for one step over host tracks is vg_query_all_host (the tracks cross the host link once);
+    # the five single-query host calls are timed beside it.
     host = [torch.from_numpy(a).pin_memory() for a in case.host]
-    hout_d = torch.empty(case.n, dtype=torch.float64).pin_memory()
+    hout_d = [torch.empty(case.n, dtype=torch.float64).pin_memory() for _ in range(4)]
     hout_i = torch.empty(case.n, dtype=torch.int32).pin_memory()
 
     def e2e_step():
-        for q in case.queries:
-            case.handle.query_host(q, *host, step_max=W.STEP_MAX, out=hout_i if q == "inside" else hout_d)
+        case.handle.query_all_host(*host, step_max=W.STEP_MAX, out=[hout_i] + hout_d)
 
-    for _ in range(3):
-        e2e_step()
+    def e2e_step5():
+        for q in case.queries:
+            case.handle.query_host(q, *host, step_max=W.STEP_MAX, out=hout_i if q == "inside" else hout_d[0])
+
+    def time_e2e(fn):
+        for _ in range(3):
+            fn()
+        barrier()
+        w0 = time.perf_counter()
+        for _ in range(ke):
+            fn()
+        w1 = time.perf_counter()
+        barrier()
+        return max_over_ranks(w1 - w0, "cuda")
+
     ke = max(3, min(args.steps, 20))
-    barrier()
-    w0 = time.perf_counter()
-    for _ in range(ke):
-        e2e_step()
-    w1 = time.perf_counter()
-    barrier()
-    e2e_s = max_over_ranks(w1 - w0, "cuda")
-    h2d = sum((48 if q.startswith("distance") else 24) for q in case.queries) * case.n
+    e2e_s = time_e2e(e2e_step)
+    e2e5_s = time_e2e(e2e_step5)
+    h2d5 = sum((48 if q.startswith("distance") else 24) for q in case.queries) * case.n
     d2h = sum((4 if q == "inside" else 8) for q in case.queries) * case.n
-    e2e = {"value": tracks_all * nq * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+    e2e = {"value": tracks_all * nq * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 48 * case.n, "d2h_bytes_per_step": d2h,
            "steps": ke, "ms_per_step": e2e_s * 1e3 / ke,
-           "api": "vg_query_host x5 (pinned host SoA in, pinned host result out, chunked copy/compute overlap)"}
+           "api": "vg_query_all_host (pinned host SoA in, five pinned host results out, chunked copy/compute overlap)",
+           "host_link_gbs": (48 * case.n + d2h) / (e2e_s / ke) / 1e9,
+           "five_single_query_calls": {"value": tracks_all * nq * ke / e2e5_s, "ms_per_step": e2e5_s * 1e3 / ke,
+                                       "h2d_bytes_per_step": h2d5, "d2h_bytes_per_step": d2h, "api": "vg_query_host x5"}}
 
     launches_per_step = nq
     detail = None
@@ -467,7 +498,7 @@ def run_ours(args, rank, world, local_rank):
                            "pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N), "form": vg.vg_get_option(vg.OPT_FORM), "pdl": vg.vg_get_option(vg.OPT_PDL),
                            "parallelism": "tracks sharded over ranks, no collective" if world > 1 else "1 GPU"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-                "roofline": roof, "per_query": per_query,
+                "roofline": roof, "per_query": per_query, "fused": fused,
                 "fp64_peak": {"fma_per_s": fma_rate, "tflops": 2 * fma_rate / 1e12,
                               "how": "register-resident DFMA chains, vg_probe_fp64_fma_rate, same run"}}
         if world == 1:

@@ -168,6 +168,11 @@ int vg_query_host(const vg_shape *shape, int query, const double *x, const doubl
                   const double *dx, const double *dy, const double *dz, double step_max, int64_t n, void *out);
 int vg_compute_step_host(const vg_volume *volume, const double *x, const double *y, const double *z, const double *dx,
                          const double *dy, const double *dz, double step_max, int64_t n, double *step, int32_t *hit);
+/* vg_query_all over HOST arrays: the six track arrays cross the host link once for all five answers (48 B in,
+ * up to 36 B out per track).  Outputs are HOST pointers; any may be NULL (at least one must be given). */
+int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, const double *z, const double *dx,
+                      const double *dy, const double *dz, double step_max, int64_t n, int32_t *cls, double *dist_in,
+                      double *dist_out, double *safety_in, double *safety_out);
 
 /* ---- launch policy (process-wide; does not change any result) ----
  * VG_OPT_PIPE_MIN_N: queries over at least this many tracks whose arrays are all 16-byte aligned run as the

@@ -52,6 +52,7 @@ def _load():
     lib.vg_compute_step.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP, _VP]
     lib.vg_volume_safety.argtypes = [_VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
     lib.vg_query_host.argtypes = [_VP, C.c_int] + [_VP] * 6 + [C.c_double, C.c_int64, _VP]
+    lib.vg_query_all_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64] + [_VP] * 5
     lib.vg_compute_step_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP]
     lib.vg_probe_fp64_fma_rate.argtypes = [C.c_int, _PD, _VP]
     lib.vg_probe_empty_launch.argtypes = [C.c_int, _VP]
@@ -257,6 +258,22 @@ def vg_query_host(shape, query, x, y, z, dx=None, dy=None, dz=None, step_max=mat
     return out
 
 
+def vg_query_all_host(shape, x, y, z, dx, dy, dz, step_max=math.inf, out=None):
+    """All five answers over HOST track arrays (one pass of the tracks over the host link).  `out`: optional tuple of
+    CPU tensors (cls int32, dist_in, dist_out, safety_in, safety_out).  Returns that tuple when complete."""
+    n = _host_tracks((x, y, z, dx, dy, dz))
+    if out is None:
+        out = [torch.empty(n, dtype=torch.int32, pin_memory=True)] + \
+              [torch.empty(n, dtype=torch.float64, pin_memory=True) for _ in range(4)]
+    out = tuple(out)
+    for o, dt in zip(out, (torch.int32,) + (torch.float64,) * 4):
+        if o.is_cuda or o.dtype != dt or o.numel() != n or not o.is_contiguous():
+            raise TypeError("out: wrong dtype, length, device or layout")
+    _check(_lib.vg_query_all_host(_handle(shape), _p(x), _p(y), _p(z), _p(dx), _p(dy), _p(dz), float(step_max), n,
+                                  *[_p(o) for o in out]))
+    return out
+
+
 def vg_compute_step_host(volume, x, y, z, dx, dy, dz, step_max=math.inf, step=None, hit=None):
     n = _host_tracks((x, y, z, dx, dy, dz))
     if step is None:
@@ -325,6 +342,9 @@ class Shape:
 
     def query_all(self, x, y, z, dx, dy, dz, step_max=math.inf, **kw):
         return vg_query_all(self, x, y, z, dx, dy, dz, step_max, **kw)
+
+    def query_all_host(self, x, y, z, dx, dy, dz, step_max=math.inf, **kw):
+        return vg_query_all_host(self, x, y, z, dx, dy, dz, step_max, **kw)
 
     def query_host(self, name, x, y, z, dx=None, dy=None, dz=None, step_max=math.inf, out=None):
         return vg_query_host(self, name, x, y, z, dx, dy, dz, step_max, out)

@@ -22,7 +22,7 @@ struct HostPipe {
     bool ready = false;
     cudaStream_t st[kSlots];
     double *in[kSlots];   // 6 * kMaxChunk doubles
-    double *outd[kSlots]; // kMaxChunk doubles
+    double *outd[kSlots]; // 4 * kMaxChunk doubles (one result; four for the fused five-query call)
     int32_t *outi[kSlots]; // kMaxChunk int32
     std::mutex mu;
 };
@@ -47,7 +47,7 @@ static cudaError_t pipe_init(HostPipe &p)
         for (int s = 0; s < kSlots; ++s) {
             if ((e = cudaStreamCreateWithFlags(&p.st[s], cudaStreamNonBlocking)) != cudaSuccess) return e;
             if ((e = cudaMalloc(&p.in[s], 6 * kMaxChunk * sizeof(double))) != cudaSuccess) return e;
-            if ((e = cudaMalloc(&p.outd[s], kMaxChunk * sizeof(double))) != cudaSuccess) return e;
+            if ((e = cudaMalloc(&p.outd[s], 4 * kMaxChunk * sizeof(double))) != cudaSuccess) return e;
             if ((e = cudaMalloc(&p.outi[s], kMaxChunk * sizeof(int32_t))) != cudaSuccess) return e;
         }
         p.ready = true;
@@ -77,16 +77,21 @@ static int cuda_fail(cudaError_t e, const char *fn)
     return vg_set_error(VG_ERR_CUDA, buf);
 }
 
-// shape != NULL: query q of the shape; volume != NULL: ComputeStep
+constexpr int qAll = 5; // run_host: the five answers at once, `all` = {cls, dist_in, dist_out, safety_in, safety_out} (HOST, may be NULL)
+
+// shape != NULL: query q of the shape (or all five); volume != NULL: ComputeStep
 static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volume, int q, const double *const h[6],
-                    double step_max, int64_t n, void *out, int32_t *hit)
+                    double step_max, int64_t n, void *out, int32_t *hit, void *const *all = nullptr)
 {
-    bool dir = volume || q == qDistIn || q == qDistOut;
+    bool dir = volume || q == qDistIn || q == qDistOut || q == qAll;
     int na = dir ? 6 : 3;
     if (n < 0) return vg_set_error(VG_ERR_ARG, "host entry: n < 0");
     for (int a = 0; a < na; ++a)
         if (!h[a]) return vg_set_error(VG_ERR_ARG, "host entry: NULL track array");
-    if (!out || (volume && !hit)) return vg_set_error(VG_ERR_ARG, "host entry: NULL output array");
+    if (q == qAll) {
+        if (!all[0] && !all[1] && !all[2] && !all[3] && !all[4]) return vg_set_error(VG_ERR_ARG, "host entry: every output is NULL");
+    } else if (!out || (volume && !hit))
+        return vg_set_error(VG_ERR_ARG, "host entry: NULL output array");
     if (n == 0) return VG_OK;
     HostPipe *p = nullptr;
     cudaError_t e = pipe_slot(&p);
@@ -112,6 +117,17 @@ static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volu
             e = cudaMemcpyAsync(static_cast<double *>(out) + o, p->outd[s], m * sizeof(double), cudaMemcpyDeviceToHost, st);
             if (e == cudaSuccess)
                 e = cudaMemcpyAsync(hit + o, p->outi[s], m * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        } else if (q == qAll) {
+            double *od[4];
+            for (int a = 0; a < 4; ++a) od[a] = all[a + 1] ? p->outd[s] + a * kMaxChunk : nullptr;
+            rc = vg_query_all(shape, d[0], d[1], d[2], d[3], d[4], d[5], step_max, m, all[0] ? p->outi[s] : nullptr, od[0],
+                              od[1], od[2], od[3], st);
+            if (rc != VG_OK) break;
+            if (all[0])
+                e = cudaMemcpyAsync(static_cast<int32_t *>(all[0]) + o, p->outi[s], m * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+            for (int a = 0; a < 4 && e == cudaSuccess; ++a)
+                if (od[a])
+                    e = cudaMemcpyAsync(static_cast<double *>(all[a + 1]) + o, od[a], m * sizeof(double), cudaMemcpyDeviceToHost, st);
         } else if (q == qInside) {
             rc = vg_inside(shape, d[0], d[1], d[2], m, p->outi[s], st);
             if (rc != VG_OK) break;
@@ -152,4 +168,14 @@ extern "C" int vg_compute_step_host(const vg_volume *volume, const double *x, co
     if (!volume) return vg_set_error(VG_ERR_ARG, "vg_compute_step_host: volume is NULL");
     const double *h[6] = { x, y, z, dx, dy, dz };
     return run_host("vg_compute_step_host", nullptr, volume, -1, h, step_max, n, step, hit);
+}
+
+extern "C" int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, const double *z, const double *dx,
+                                 const double *dy, const double *dz, double step_max, int64_t n, int32_t *cls,
+                                 double *dist_in, double *dist_out, double *safety_in, double *safety_out)
+{
+    if (!shape) return vg_set_error(VG_ERR_ARG, "vg_query_all_host: shape is NULL");
+    const double *h[6] = { x, y, z, dx, dy, dz };
+    void *all[5] = { cls, dist_in, dist_out, safety_in, safety_out };
+    return run_host("vg_query_all_host", shape, nullptr, qAll, h, step_max, n, nullptr, nullptr, all);
 }

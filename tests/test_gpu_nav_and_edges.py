@@ -341,6 +341,15 @@ def test_host_entry_points_match_the_oracle(vg, n):
             assert_int_equal(g, so.inside(*t[:3]), "host inside")
         else:
             assert_real_close(g, getattr(so, q)(*t[:3]), "host %s" % q)
+    # the fused host call: one pass of the tracks over the host link for all five answers
+    fused = sg.query_all_host(*ht, step_max=W.STEP_MAX)
+    for q, g in zip(W.QUERIES5, fused):
+        if q.startswith("distance"):
+            assert_real_close(g.numpy(), getattr(so, q)(*t, W.STEP_MAX), "host fused %s" % q)
+        elif q == "inside":
+            assert_int_equal(g.numpy(), so.inside(*t[:3]), "host fused inside")
+        else:
+            assert_real_close(g.numpy(), getattr(so, q)(*t[:3]), "host fused %s" % q)
     # pageable memory works as well
     g = sg.query_host("distance_to_in", *[torch.from_numpy(a) for a in t], step_max=W.STEP_MAX,
                       out=torch.empty(n, dtype=torch.float64)).numpy()
