@@ -141,7 +141,7 @@ struct AllOut {
 };
 
 #ifndef VG_ALL_MINB
-#define VG_ALL_MINB 2
+#define VG_ALL_MINB 3
 #endif
 
 template <class S>
