@@ -36,6 +36,7 @@ static int fail_cuda(cudaError_t e, const char *what)
 }
 
 #include "vg_derive.h" // struct vg_shape, fill_shape (uses fail)
+#include "vg_pcon_grid.h"
 
 extern "C" const char *vg_last_error(void) { return g_err; }
 
@@ -78,6 +79,34 @@ extern "C" int64_t vg_get_option(int option)
     return fail(VG_ERR_ARG, "vg_get_option: unknown option %d", option);
 }
 
+// Builds the candidate grid and puts it on the current device.  Best effort: without a device (or memory) the shape
+// is still valid and its safeties run the ordered-walk kernel.
+static void upload_pcon_grid(vg_shape *s)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return;
+    }
+    std::vector<unsigned long long> masks;
+    std::vector<unsigned char> rows;
+    PconGridGeom geom;
+    pcon_grid_build(s->u.pcon, &geom, &masks, &rows);
+    const size_t mbytes = masks.size() * sizeof(unsigned long long);
+    unsigned char *blob = nullptr;
+    if (cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + rows.size()) != cudaSuccess ||
+        cudaMemcpy(blob, masks.data(), mbytes, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(blob + mbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        if (blob) cudaFree(blob);
+        return;
+    }
+    s->grid.masks = reinterpret_cast<const unsigned long long *>(blob);
+    s->grid.rows = blob + mbytes;
+    s->grid.g = geom;
+    s->grid_device = dev;
+}
+
 extern "C" int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **out)
 {
     if (!out) return fail(VG_ERR_ARG, "vg_shape_create: out is NULL");
@@ -92,11 +121,17 @@ extern "C" int vg_shape_create(vg_kind kind, const double *params, int nparams, 
         delete s;
         return rc;
     }
+    if (kind == VG_POLYCONE && s->u.pcon.w.full) upload_pcon_grid(s);
     *out = s;
     return VG_OK;
 }
 
-extern "C" void vg_shape_destroy(vg_shape *s) { delete s; }
+extern "C" void vg_shape_destroy(vg_shape *s)
+{
+    if (!s) return;
+    if (s->grid.masks) cudaFree(const_cast<unsigned long long *>(s->grid.masks)); // rows live in the same allocation
+    delete s;
+}
 
 extern "C" int vg_shape_kind(const vg_shape *s) { return s ? s->kind : fail(VG_ERR_ARG, "vg_shape_kind: NULL"); }
 
@@ -144,7 +179,13 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
     case VG_TUBE: e = launch_tube(q, s->u.tube, t, step_max, n, out, vec, st); break;
     case VG_CONE: e = launch_cone(q, s->u.cone, t, step_max, n, out, vec, st); break;
     case VG_TRD: e = launch_trd(q, s->u.trd, t, step_max, n, out, vec, st); break;
-    case VG_POLYCONE: e = launch_polycone(q, s->u.pcon, t, step_max, n, out, vec, st); break;
+    case VG_POLYCONE: {
+        PconGrid g = s->grid;
+        int dev = -1;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr;
+        e = launch_polycone(q, s->u.pcon, g, t, step_max, n, out, vec, st);
+        break;
+    }
     }
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;

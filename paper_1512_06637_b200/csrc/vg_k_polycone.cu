@@ -5,15 +5,21 @@
 
 namespace vg {
 
-cudaError_t launch_polycone(int q, const PolyconeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
-                            cudaStream_t s)
+cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n,
+                            void *out, bool vec, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     if (p.w.full) {
         if (vec && g_form.load(std::memory_order_relaxed) == 0) {
-            if (q == qDistIn) return launch_pcon_walk<qDistIn>(p, t, step_max, n, static_cast<double *>(out), s);
-            if (q == qSafeIn) return launch_pcon_walk<qSafeIn>(p, t, step_max, n, static_cast<double *>(out), s);
-            if (q == qSafeOut) return launch_pcon_walk<qSafeOut>(p, t, step_max, n, static_cast<double *>(out), s);
+            double *o = static_cast<double *>(out);
+            if (q == qDistIn) return launch_pcon_walk<qDistIn, false>(p, g, t, step_max, n, o, s);
+            // the safeties: candidate grid (built at vg_shape_create on the device it was created on), else the walk
+            if (q == qSafeIn)
+                return g.masks ? launch_pcon_walk<qSafeIn, true>(p, g, t, step_max, n, o, s)
+                               : launch_pcon_walk<qSafeIn, false>(p, g, t, step_max, n, o, s);
+            if (q == qSafeOut)
+                return g.masks ? launch_pcon_walk<qSafeOut, true>(p, g, t, step_max, n, o, s)
+                               : launch_pcon_walk<qSafeOut, false>(p, g, t, step_max, n, o, s);
         }
         return launch_any<Polycone, PolyconeT<solid_flags(false, kWmFull)>>(q, p, t, step_max, n, out, vec, s);
     }

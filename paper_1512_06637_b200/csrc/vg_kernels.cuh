@@ -539,8 +539,8 @@ cudaError_t launch_cone(int q, const ConeP &p, const Tracks &t, double step_max,
                         cudaStream_t s);
 cudaError_t launch_trd(int q, const TrdP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
                        cudaStream_t s);
-cudaError_t launch_polycone(int q, const PolyconeP &p, const Tracks &t, double step_max, int64_t n, void *out, bool vec,
-                            cudaStream_t s);
+cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n,
+                            void *out, bool vec, cudaStream_t s);
 
 // the fused five-query kernel of each solid (the polycone has none: its queries run as five launches)
 cudaError_t launch_box_all(const BoxP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);

@@ -75,6 +75,23 @@ struct PolyconeP {
     PconSec sec[kMaxSec];
 };
 
+// Candidate grid of a full-phi polycone (vg_pcon_grid.h): kPconGridZ x kPconGridR cells over
+// rho in [0, kPconGridR / inv_cr), z in [zg0, zg0 + kPconGridZ / inv_cz); one 64-bit mask of candidate segments per
+// cell (bit 2k = outer edge of section k, 2k + 1 = inner edge, 62 / 63 = lower / upper cap), one byte per z row with
+// the section index at the row's lower edge.  Device memory owned by the vg_shape.
+constexpr int kPconGridR = 64, kPconGridZ = 128;
+constexpr int kPconCapLoBit = 62, kPconCapHiBit = 63;
+
+struct PconGridGeom {
+    double inv_cr, inv_cz, zg0;
+};
+
+struct PconGrid {
+    const unsigned long long *masks; // [kPconGridZ][kPconGridR]; NULL: no grid, the ordered walk serves the safeties
+    const unsigned char *rows;       // [kPconGridZ]
+    PconGridGeom g;
+};
+
 // a solid that may be a mother or a daughter of a volume (every kind except the polycone)
 struct SolidU {
     int kind;

@@ -1,0 +1,130 @@
+// vg_pcon_grid.h -- host only: the candidate grid of a full-phi polycone, built once at vg_shape_create
+// (SURVEY.md sec. 8(a) A0 "shape set-up"; the safeties are the exact signed distance of sec. 8(c) c.3).
+//
+// The exact distance from (rho, z) to the (r, z) outline is the minimum over its segments (outer and inner edge of
+// every section, the two end caps).  For a CELL of a regular (rho, z) grid only a few segments can be that minimum
+// for any point of the cell: segment s is a candidate iff
+//     dmin_s(cell) <= min over s' of dmax_s'(cell)
+// (the nearest segment s* of a point p of the cell has d(p, s*) <= d(p, s') <= dmax_s' for every s', and
+// dmin_s* <= d(p, s*)).  dmax_s is the largest distance from a cell corner to s (the distance to a convex set is a
+// convex function, so its maximum over a rectangle sits at a corner); dmin_s is 0 if s meets the cell, else the
+// smaller of the corner-to-segment and endpoint-to-cell distances (two disjoint convex polygons in the plane are
+// closest at a vertex of one of them).  Both are evaluated for the cell inflated by `margin`, and the comparison
+// carries a slack, so a point that rounding bins into a neighbouring cell still finds its nearest segment.
+// The kernel (vg_pcon_walk.cuh, pcon_grid_sdf) evaluates the candidates of the point's cell only: same minimum,
+// same arithmetic per segment, a fraction of the work.  Points outside the grid take the ordered walk.
+#pragma once
+#include "vg_params.h"
+
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace vg {
+
+struct PconSegH {
+    double r0, z0, r1, z1;
+    int bit;
+};
+
+static inline double pg_dist_seg(double u, double v, const PconSegH &s)
+{
+    double er = s.r1 - s.r0, ez = s.z1 - s.z0;
+    double l2 = er * er + ez * ez;
+    double t = l2 > 0 ? ((u - s.r0) * er + (v - s.z0) * ez) / l2 : 0.0;
+    t = t < 0 ? 0 : (t > 1 ? 1 : t);
+    double du = u - s.r0 - t * er, dv = v - s.z0 - t * ez;
+    return std::sqrt(du * du + dv * dv);
+}
+
+static inline double pg_dist_rect(double u, double v, double u0, double u1, double v0, double v1)
+{
+    double qu = std::fmax(std::fmax(u0 - u, u - u1), 0.0), qv = std::fmax(std::fmax(v0 - v, v - v1), 0.0);
+    return std::sqrt(qu * qu + qv * qv);
+}
+
+// does the segment meet the closed rectangle?  (Liang-Barsky clip of t in [0, 1])
+static inline bool pg_seg_meets_rect(const PconSegH &s, double u0, double u1, double v0, double v1)
+{
+    double t0 = 0, t1 = 1;
+    const double p[4] = { -(s.r1 - s.r0), s.r1 - s.r0, -(s.z1 - s.z0), s.z1 - s.z0 };
+    const double q[4] = { s.r0 - u0, u1 - s.r0, s.z0 - v0, v1 - s.z0 };
+    for (int i = 0; i < 4; ++i) {
+        if (p[i] == 0) {
+            if (q[i] < 0) return false;
+        } else {
+            double r = q[i] / p[i];
+            if (p[i] < 0) t0 = std::fmax(t0, r);
+            else t1 = std::fmin(t1, r);
+        }
+    }
+    return t0 <= t1;
+}
+
+// segment numbering shared with the kernel: 2k = outer edge of section k, 2k + 1 = inner edge, 62 / 63 = the caps
+static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::vector<unsigned long long> *masks,
+                                   std::vector<unsigned char> *rows)
+{
+    std::vector<PconSegH> segs;
+    double rmax = 0;
+    for (int k = 0; k < c.nsec; ++k) {
+        const PconSec &s = c.sec[k];
+        segs.push_back(PconSegH{ s.out.r0, s.z0, s.out.r0 + s.out.er, s.z1, 2 * k });
+        if ((c.inner_mask >> k) & 1u) segs.push_back(PconSegH{ s.in.r0, s.z0, s.in.r0 + s.in.er, s.z1, 2 * k + 1 });
+        rmax = std::fmax(rmax, std::fmax(s.out.r0, s.out.r0 + s.out.er));
+    }
+    segs.push_back(PconSegH{ c.cap_lo_rmin, c.zlo, c.cap_lo_rmax, c.zlo, kPconCapLoBit });
+    segs.push_back(PconSegH{ c.cap_hi_rmin, c.zhi, c.cap_hi_rmax, c.zhi, kPconCapHiBit });
+
+    const double zl = c.zhi - c.zlo;
+    const double R = 2.25 * rmax, zg0 = c.zlo - 0.5 * zl, zg1 = c.zhi + 0.5 * zl;
+    const double cr = R / kPconGridR, cz = (zg1 - zg0) / kPconGridZ;
+    geom->inv_cr = 1.0 / cr;
+    geom->inv_cz = 1.0 / cz;
+    geom->zg0 = zg0;
+    const double margin = 1e-6 * std::fmax(cr, cz);
+    const size_t ns = segs.size();
+
+    // corner lattice of distances, one layer per segment
+    const int LR = kPconGridR + 1, LZ = kPconGridZ + 1;
+    std::vector<double> D(ns * size_t(LR) * LZ);
+    for (size_t s = 0; s < ns; ++s)
+        for (int j = 0; j < LZ; ++j)
+            for (int i = 0; i < LR; ++i) D[(s * LZ + j) * LR + i] = pg_dist_seg(i * cr, zg0 + j * cz, segs[s]);
+
+    masks->assign(size_t(kPconGridR) * kPconGridZ, 0ull);
+    std::vector<double> dmin(ns);
+    for (int j = 0; j < kPconGridZ; ++j)
+        for (int i = 0; i < kPconGridR; ++i) {
+            const double u0 = i * cr, u1 = u0 + cr, v0 = zg0 + j * cz, v1 = v0 + cz;
+            double thr = INFINITY;
+            for (size_t s = 0; s < ns; ++s) {
+                const double *L = &D[(s * LZ + j) * LR + i];
+                const double d00 = L[0], d10 = L[1], d01 = L[LR], d11 = L[LR + 1];
+                const double mx = std::fmax(std::fmax(d00, d10), std::fmax(d01, d11));
+                double mn = std::fmin(std::fmin(d00, d10), std::fmin(d01, d11));
+                mn = std::fmin(mn, pg_dist_rect(segs[s].r0, segs[s].z0, u0, u1, v0, v1));
+                mn = std::fmin(mn, pg_dist_rect(segs[s].r1, segs[s].z1, u0, u1, v0, v1));
+                if (pg_seg_meets_rect(segs[s], u0 - margin, u1 + margin, v0 - margin, v1 + margin)) mn = 0;
+                dmin[s] = mn;
+                thr = std::fmin(thr, mx);
+            }
+            // inflation by `margin` moves either bound by at most sqrt(2) margin; relative slack for the FMA rounding
+            thr = thr * (1 + 1e-9) + 4 * margin;
+            unsigned long long m = 0;
+            for (size_t s = 0; s < ns; ++s)
+                if (dmin[s] <= thr) m |= 1ull << segs[s].bit;
+            (*masks)[size_t(j) * kPconGridR + i] = m;
+        }
+
+    // section index at (slightly below) the lower edge of every z row: the kernel counts on from there
+    rows->assign(kPconGridZ, 0);
+    for (int j = 0; j < kPconGridZ; ++j) {
+        const double zr = zg0 + j * cz - margin;
+        int k = 0;
+        for (int q = 1; q < c.nsec; ++q) k += (c.sec[q].z0 <= zr) ? 1 : 0;
+        (*rows)[j] = (unsigned char)k;
+    }
+}
+
+} // namespace vg

@@ -178,11 +178,66 @@ VG_DEV double pcon_walk_sdf(const PolyconeP &p, const PconWalkSec *tab, double x
     return in2d ? -dist : dist;
 }
 
-template <int Q> VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z,
-                                              double dx, double dy, double dz, double step_max)
+// ---- candidate-grid form of the same signed distance (vg_pcon_grid.h) ----
+//
+// One record per segment of the (r, z) outline, numbered like the mask bits of the grid: (r0, z0), edge vector,
+// 1 / |edge|^2.  Five doubles per record: an odd stride, so lanes reading different records spread over the banks.
+constexpr int kPconSegStride = 5;
+
+VG_DEV void pcon_stage_segs(const PolyconeP &p, double *seg)
 {
-    if (Q == qSafeIn) return pcon_walk_sdf(p, tab, x, y, z);
-    if (Q == qSafeOut) return -pcon_walk_sdf(p, tab, x, y, z);
+    for (int s = threadIdx.x; s < 64; s += blockDim.x) {
+        double r0 = 0, z0 = 0, er = 0, ez = 0, il = 0;
+        const int k = s >> 1;
+        if (k < p.nsec) {
+            const PconSec &c = p.sec[k];
+            const Frustum &f = (s & 1) ? c.in : c.out;
+            r0 = f.r0, z0 = c.z0, er = f.er, ez = c.z1 - c.z0, il = f.inv_l2;
+        }
+        if (s == kPconCapLoBit) r0 = p.cap_lo_rmin, z0 = p.zlo, er = p.cap_lo_rmax - p.cap_lo_rmin, il = 1.0 / (er * er);
+        if (s == kPconCapHiBit) r0 = p.cap_hi_rmin, z0 = p.zhi, er = p.cap_hi_rmax - p.cap_hi_rmin, il = 1.0 / (er * er);
+        double *o = seg + kPconSegStride * s;
+        o[0] = r0, o[1] = z0, o[2] = er, o[3] = ez, o[4] = il;
+    }
+}
+
+// exact signed distance: minimum over the candidate segments of the point's cell (the cell's mask holds every segment
+// that can be nearest to any point of the cell), sign from the point's own section.  Off the grid: the ordered walk.
+VG_DEV double pcon_grid_sdf(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x,
+                            double y, double z)
+{
+    const double rho2 = fma(x, x, y * y);
+    const double rho = sqrt_nn(rho2);
+    const double fr = rho * g.g.inv_cr, fz = (z - g.g.zg0) * g.g.inv_cz;
+    if (!(fr < double(kPconGridR) && fz >= 0.0 && fz < double(kPconGridZ))) return pcon_walk_sdf(p, tab, x, y, z);
+    const int ir = int(fr), iz = int(fz);
+    unsigned long long m = __ldg(g.masks + iz * kPconGridR + ir);
+    int kz = __ldg(g.rows + iz);
+    while (kz + 1 < p.nsec && tab[kz + 1].z0 <= z) ++kz;
+    bool in2d;
+    {
+        const PconWalkSec &w = tab[kz];
+        in2d = z >= p.zlo && z <= p.zhi && rho <= fma(w.Bo, z, w.Ao) && rho >= fma(w.Bi, z, w.Ai);
+    }
+    double d2 = inf();
+    while (m) {
+        const int s = __ffsll((long long)m) - 1;
+        m &= m - 1;
+        const double *q = seg + kPconSegStride * s;
+        d2 = dmin(d2, seg_d2(rho, z, q[0], q[1], q[2], q[3], q[4]));
+    }
+    const double dist = sqrt_nn(d2);
+    return in2d ? -dist : dist;
+}
+
+template <int Q, bool GRID>
+VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x,
+                             double y, double z, double dx, double dy, double dz, double step_max)
+{
+    if (Q == qSafeIn || Q == qSafeOut) {
+        const double s = GRID ? pcon_grid_sdf(p, tab, seg, g, x, y, z) : pcon_walk_sdf(p, tab, x, y, z);
+        return Q == qSafeIn ? s : -s;
+    }
     const double t = pcon_walk_dist_in(p, tab, x, y, z, dx, dy, dz);
     return t <= step_max ? t : inf();
 }
@@ -192,13 +247,16 @@ template <int Q> VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalk
 #endif
 
 // persistent CTAs striding over tiles of 512 tracks, two tracks per thread (128-bit loads; arrays 16-byte aligned)
-template <int Q>
+template <int Q, bool GRID>
 __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
-    pcon_walk_kernel(const __grid_constant__ PolyconeP p, Tracks t, double step_max, int64_t n, double *out)
+    pcon_walk_kernel(const __grid_constant__ PolyconeP p, const __grid_constant__ PconGrid g, Tracks t, double step_max,
+                     int64_t n, double *out)
 {
     constexpr bool kDir = (Q == qDistIn);
     __shared__ __align__(16) PconWalkSec tab[kMaxSec];
+    __shared__ double seg[GRID ? 64 * kPconSegStride : 1];
     pcon_stage(p, tab);
+    if (GRID) pcon_stage_segs(p, seg);
     pdl_launch_dependents();
     __syncthreads();
     pdl_wait();
@@ -209,20 +267,21 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
             double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
             double2 dx = make_double2(0, 0), dy = dx, dz = dx;
             if (kDir) dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
-            const double r0 = pcon_walk_eval<Q>(p, tab, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max);
-            const double r1 = pcon_walk_eval<Q>(p, tab, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max);
+            const double r0 = pcon_walk_eval<Q, GRID>(p, tab, seg, g, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max);
+            const double r1 = pcon_walk_eval<Q, GRID>(p, tab, seg, g, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max);
             stg2(out + i, r0, r1);
         } else {
             double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
             double dx = 0, dy = 0, dz = 0;
             if (kDir) dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
-            stg1(out + i, pcon_walk_eval<Q>(p, tab, x, y, z, dx, dy, dz, step_max));
+            stg1(out + i, pcon_walk_eval<Q, GRID>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max));
         }
     }
 }
 
-template <int Q>
-cudaError_t launch_pcon_walk(const PolyconeP &p, const Tracks &t, double step_max, int64_t n, double *out, cudaStream_t s)
+template <int Q, bool GRID>
+cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, double *out,
+                             cudaStream_t s)
 {
     static std::atomic<int> cap_cache{ 0 };
     int cap = cap_cache.load(std::memory_order_acquire);
@@ -231,14 +290,14 @@ cudaError_t launch_pcon_walk(const PolyconeP &p, const Tracks &t, double step_ma
         cudaError_t e;
         if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
         if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_walk_kernel<Q>, kWalkBlock, 0)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_walk_kernel<Q, GRID>, kWalkBlock, 0)) != cudaSuccess) return e;
         cap = sms * (per_sm < 1 ? 1 : per_sm);
         cap_cache.store(cap, std::memory_order_release);
     }
     const int64_t npairs = (n + 1) >> 1;
     int64_t grid = (npairs + kWalkBlock - 1) / kWalkBlock;
     if (grid > cap) grid = cap;
-    return launch_kernel(pcon_walk_kernel<Q>, unsigned(grid), kWalkBlock, 0, s, p, t, step_max, n, out);
+    return launch_kernel(pcon_walk_kernel<Q, GRID>, unsigned(grid), kWalkBlock, 0, s, p, g, t, step_max, n, out);
 }
 
 } // namespace vg

@@ -373,3 +373,50 @@ def test_library_launch_counter_counts_kernels(vg):
     for _ in range(7):
         sg.safety_to_in(x, x, x)
     assert vg.vg_launch_count() - before == 7
+
+
+# ------------------------------------------------------------- candidate-grid safeties of the full-phi polycone
+
+def _random_polycone(seed, nz, rmin_hi=5.0):
+    rng = np.random.default_rng(seed)
+    z = np.sort(rng.uniform(-50.0, 50.0, nz))
+    z += np.arange(nz) * 1e-3  # strictly increasing even if two draws coincide
+    rmin = rng.uniform(0.0, rmin_hi, nz) if rmin_hi > 0 else np.zeros(nz)
+    rmax = rng.uniform(10.0, 30.0, nz)
+    out = [0.0, TWO_PI, float(nz)]
+    for i in range(nz):
+        out += [float(z[i]), float(rmin[i]), float(rmax[i])]
+    return out
+
+
+@pytest.mark.parametrize("seed,nz,rmin_hi", [(1, 2, 5.0), (2, 3, 0.0), (3, 10, 5.0), (4, 17, 9.0), (5, 32, 5.0), (6, 32, 0.0)])
+def test_polycone_grid_safeties_match_the_oracle(vg, seed, nz, rmin_hi):
+    """vg_pcon_grid.h: the per-cell candidate masks must hold the nearest segment of every point of the cell.  Points are
+    drawn in 3x the bounding box (so some fall off the grid and take the ordered walk inside the same kernel), plus
+    points on a lattice that lands exactly on cell corners and edges (rho = i / inv_cr, z = zg0 + j / inv_cz)."""
+    par = _random_polycone(seed, nz, rmin_hi)
+    so, sg = O.Shape(W.POLYCONE, par), vg.Shape(W.POLYCONE, par)
+    c, h = W.bounding_half(W.POLYCONE, par)
+    x, y, z = W.draw_tracks(100 + seed, 300001, c, tuple(3.0 * v for v in h))[:3]
+    # cell corners: the grid spans rho in [0, 2.25 rmax), z in [zlo - zl/2, zhi + zl/2) with 64 x 128 cells
+    rmax = h[0]
+    zl = 2.0 * h[2]
+    ii, jj = np.meshgrid(np.arange(65), np.arange(129))
+    rho_c = (ii * (2.25 * rmax / 64)).ravel()
+    z_c = (c[2] - h[2] - 0.5 * zl + jj * (2.0 * zl / 128)).ravel()
+    ang = np.random.default_rng(seed).uniform(0, TWO_PI, rho_c.size)
+    x = np.concatenate([x, rho_c * np.cos(ang)])
+    y = np.concatenate([y, rho_c * np.sin(ang)])
+    z = np.concatenate([z, z_c])
+    keep = np.abs(so.sdf(x, y, z)) >= W.SURFACE_BAND
+    t = tuple(np.ascontiguousarray(a[keep]) for a in (x, y, z))
+    dt = dev(t)
+    assert_real_close(sg.safety_to_in(*dt).cpu().numpy(), so.safety_to_in(*t), "grid safety_to_in nz=%d" % nz)
+    assert_real_close(sg.safety_to_out(*dt).cpu().numpy(), so.safety_to_out(*t), "grid safety_to_out nz=%d" % nz)
+    # the generic kernel (forced direct form) evaluates every segment: same answers
+    vg.vg_set_option(vg.OPT_FORM, vg.FORM_DIRECT)
+    try:
+        g2 = sg.safety_to_in(*dt).cpu().numpy()
+    finally:
+        vg.vg_set_option(vg.OPT_FORM, vg.FORM_AUTO)
+    assert_real_close(g2, so.safety_to_in(*t), "generic safety_to_in nz=%d" % nz)
