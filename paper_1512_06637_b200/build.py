@@ -41,6 +41,9 @@ def _compile(unit, force, extra):
 
 
 def build(force=False, verbose=False, extra=()):
+    # VG_NVCC_EXTRA="-DVG_IEEE_MATH ..." adds compile flags (tuning sweeps, bisecting a parity failure); the objects are
+    # keyed by time stamp only, so combine it with force / --force
+    extra = list(extra) + os.environ.get("VG_NVCC_EXTRA", "").split()
     os.makedirs(OBJ, exist_ok=True)
     with cf.ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as ex:
         results = list(ex.map(lambda u: _compile(u, force, extra), UNITS))

@@ -69,29 +69,48 @@ VG_DEV void eval_store(const typename S::P &p, double x, double y, double z, dou
 //             straight-line distance code takes ~100 registers if allowed to, which leaves 2 CTAs per SM and too
 //             few warps to cover the FP64 latencies; capped at 64 registers (4 CTAs) it runs 15-25 % faster.
 //   stream -- VG_FORM_AUTO runs the persistent streaming form (below) instead of the direct one.
+//   block  -- CTA size of the direct kernel.  128 threads serve the Tube safeties better at n = 2^20 (1024 tracks per
+//             SM-resident CTA pair instead of 512 per CTA: finer hand-out over the 148 SMs, shorter tail).
 template <class S, int Q> struct Tune {
     static constexpr int minb = (Q == qDistIn || Q == qDistOut) ? 4 : VG_MINB;
     static constexpr bool stream = false;
+    static constexpr int block = kBlock;
 };
 template <int F> struct Tune<TubeT<F>, qDistIn> {
     static constexpr int minb = 4;
     static constexpr bool stream = true;
+    static constexpr int block = kBlock;
+};
+#ifndef VG_TUBE_SAFE_BLOCK
+#define VG_TUBE_SAFE_BLOCK 128
+#endif
+template <int F> struct Tune<TubeT<F>, qSafeIn> {
+    static constexpr int minb = VG_MINB;
+    static constexpr bool stream = false;
+    static constexpr int block = VG_TUBE_SAFE_BLOCK;
+};
+template <int F> struct Tune<TubeT<F>, qSafeOut> {
+    static constexpr int minb = VG_MINB;
+    static constexpr bool stream = false;
+    static constexpr int block = VG_TUBE_SAFE_BLOCK;
 };
 template <> struct Tune<Trd, qSafeIn> {
     static constexpr int minb = VG_MINB;
     static constexpr bool stream = true;
+    static constexpr int block = kBlock;
 };
 template <> struct Tune<Trd, qSafeOut> {
     static constexpr int minb = VG_MINB;
     static constexpr bool stream = true;
+    static constexpr int block = kBlock;
 };
 
 template <class S, int Q, int TPT>
-__global__ void __launch_bounds__(kBlock, Tune<S, Q>::minb) query_kernel(const __grid_constant__ typename S::P p, Tracks t,
-                                                       double step_max, int64_t n, void *out)
+__global__ void __launch_bounds__(Tune<S, Q>::block, Tune<S, Q>::minb)
+    query_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, void *out)
 {
     constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
-    int64_t i = (int64_t(blockIdx.x) * kBlock + threadIdx.x) * TPT;
+    int64_t i = (int64_t(blockIdx.x) * Tune<S, Q>::block + threadIdx.x) * TPT;
     pdl_launch_dependents();
     pdl_wait();
     if (i >= n) return;
@@ -505,13 +524,14 @@ cudaError_t launch_query(const typename S::P &p, const Tracks &t, double step_ma
         grid = (npairs + per - 1) / per;
         return launch_kernel(query_stream_kernel<S, Q>, unsigned(grid), kSBlock, 0, stream, p, t, step_max, n, out, per);
     }
+    constexpr int kB = Tune<S, Q>::block;
     if (vec) {
         int64_t threads = (n + 1) / 2;
-        unsigned grid = unsigned((threads + kBlock - 1) / kBlock);
-        return launch_kernel(query_kernel<S, Q, 2>, grid, kBlock, 0, stream, p, t, step_max, n, out);
+        unsigned grid = unsigned((threads + kB - 1) / kB);
+        return launch_kernel(query_kernel<S, Q, 2>, grid, kB, 0, stream, p, t, step_max, n, out);
     }
-    unsigned grid = unsigned((n + kBlock - 1) / kBlock);
-    return launch_kernel(query_kernel<S, Q, 1>, grid, kBlock, 0, stream, p, t, step_max, n, out);
+    unsigned grid = unsigned((n + kB - 1) / kB);
+    return launch_kernel(query_kernel<S, Q, 1>, grid, kB, 0, stream, p, t, step_max, n, out);
 }
 
 template <class G, class S = G>

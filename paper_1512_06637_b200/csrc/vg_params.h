@@ -77,10 +77,16 @@ struct PolyconeP {
 
 // Candidate grid of a full-phi polycone (vg_pcon_grid.h): kPconGridZ x kPconGridR cells over
 // rho in [0, kPconGridR / inv_cr), z in [zg0, zg0 + kPconGridZ / inv_cz); one 64-bit mask of candidate segments per
-// cell (bit 2k = outer edge of section k, 2k + 1 = inner edge, 62 / 63 = lower / upper cap), one byte per z row with
-// the section index at the row's lower edge.  Device memory owned by the vg_shape.
-constexpr int kPconGridR = 64, kPconGridZ = 128;
-constexpr int kPconCapLoBit = 62, kPconCapHiBit = 63;
+// cell (bit 0 / 1 = lower / upper cap, bit 2 + 2k = outer edge of section k, 3 + 2k = inner edge: up to 15 sections fit
+// the low word), one byte per z row with the section index at the row's lower edge.  Device memory owned by the vg_shape.
+#ifndef VG_PCON_GRID_R
+#define VG_PCON_GRID_R 64
+#endif
+#ifndef VG_PCON_GRID_Z
+#define VG_PCON_GRID_Z 128
+#endif
+constexpr int kPconGridR = VG_PCON_GRID_R, kPconGridZ = VG_PCON_GRID_Z;
+constexpr int kPconCapLoBit = 0, kPconCapHiBit = 1, kPconSecBit0 = 2;
 
 struct PconGridGeom {
     double inv_cr, inv_cz, zg0;

@@ -27,20 +27,24 @@ struct PconSegH {
     int bit;
 };
 
-static inline double pg_dist_seg(double u, double v, const PconSegH &s)
+// plain selects (std::fmax / std::fmin are libm calls without fast-math; no NaN can reach these)
+static inline double pg_max(double a, double b) { return a > b ? a : b; }
+static inline double pg_min(double a, double b) { return a < b ? a : b; }
+
+// squared distances (the builder compares squares and takes one square root per cell)
+static inline double pg_dist2_seg(double u, double v, const PconSegH &s, double inv_l2)
 {
     double er = s.r1 - s.r0, ez = s.z1 - s.z0;
-    double l2 = er * er + ez * ez;
-    double t = l2 > 0 ? ((u - s.r0) * er + (v - s.z0) * ez) / l2 : 0.0;
+    double t = ((u - s.r0) * er + (v - s.z0) * ez) * inv_l2;
     t = t < 0 ? 0 : (t > 1 ? 1 : t);
     double du = u - s.r0 - t * er, dv = v - s.z0 - t * ez;
-    return std::sqrt(du * du + dv * dv);
+    return du * du + dv * dv;
 }
 
-static inline double pg_dist_rect(double u, double v, double u0, double u1, double v0, double v1)
+static inline double pg_dist2_rect(double u, double v, double u0, double u1, double v0, double v1)
 {
-    double qu = std::fmax(std::fmax(u0 - u, u - u1), 0.0), qv = std::fmax(std::fmax(v0 - v, v - v1), 0.0);
-    return std::sqrt(qu * qu + qv * qv);
+    double qu = pg_max(pg_max(u0 - u, u - u1), 0.0), qv = pg_max(pg_max(v0 - v, v - v1), 0.0);
+    return qu * qu + qv * qv;
 }
 
 // does the segment meet the closed rectangle?  (Liang-Barsky clip of t in [0, 1])
@@ -54,14 +58,14 @@ static inline bool pg_seg_meets_rect(const PconSegH &s, double u0, double u1, do
             if (q[i] < 0) return false;
         } else {
             double r = q[i] / p[i];
-            if (p[i] < 0) t0 = std::fmax(t0, r);
-            else t1 = std::fmin(t1, r);
+            if (p[i] < 0) t0 = pg_max(t0, r);
+            else t1 = pg_min(t1, r);
         }
     }
     return t0 <= t1;
 }
 
-// segment numbering shared with the kernel: 2k = outer edge of section k, 2k + 1 = inner edge, 62 / 63 = the caps
+// segment numbering shared with the kernel (vg_params.h): bits 0 / 1 = the caps, 2 + 2k / 3 + 2k = outer / inner edge of section k
 static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::vector<unsigned long long> *masks,
                                    std::vector<unsigned char> *rows)
 {
@@ -69,9 +73,9 @@ static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::
     double rmax = 0;
     for (int k = 0; k < c.nsec; ++k) {
         const PconSec &s = c.sec[k];
-        segs.push_back(PconSegH{ s.out.r0, s.z0, s.out.r0 + s.out.er, s.z1, 2 * k });
-        if ((c.inner_mask >> k) & 1u) segs.push_back(PconSegH{ s.in.r0, s.z0, s.in.r0 + s.in.er, s.z1, 2 * k + 1 });
-        rmax = std::fmax(rmax, std::fmax(s.out.r0, s.out.r0 + s.out.er));
+        segs.push_back(PconSegH{ s.out.r0, s.z0, s.out.r0 + s.out.er, s.z1, kPconSecBit0 + 2 * k });
+        if ((c.inner_mask >> k) & 1u) segs.push_back(PconSegH{ s.in.r0, s.z0, s.in.r0 + s.in.er, s.z1, kPconSecBit0 + 2 * k + 1 });
+        rmax = pg_max(rmax, pg_max(s.out.r0, s.out.r0 + s.out.er));
     }
     segs.push_back(PconSegH{ c.cap_lo_rmin, c.zlo, c.cap_lo_rmax, c.zlo, kPconCapLoBit });
     segs.push_back(PconSegH{ c.cap_hi_rmin, c.zhi, c.cap_hi_rmax, c.zhi, kPconCapHiBit });
@@ -82,15 +86,17 @@ static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::
     geom->inv_cr = 1.0 / cr;
     geom->inv_cz = 1.0 / cz;
     geom->zg0 = zg0;
-    const double margin = 1e-6 * std::fmax(cr, cz);
+    const double margin = 1e-6 * pg_max(cr, cz); // dmin, dmax, thr below are SQUARED distances
     const size_t ns = segs.size();
 
-    // corner lattice of distances, one layer per segment
+    // corner lattice of squared distances, one layer per segment
     const int LR = kPconGridR + 1, LZ = kPconGridZ + 1;
     std::vector<double> D(ns * size_t(LR) * LZ);
-    for (size_t s = 0; s < ns; ++s)
+    for (size_t s = 0; s < ns; ++s) {
+        const double er = segs[s].r1 - segs[s].r0, ez = segs[s].z1 - segs[s].z0, inv_l2 = 1.0 / (er * er + ez * ez);
         for (int j = 0; j < LZ; ++j)
-            for (int i = 0; i < LR; ++i) D[(s * LZ + j) * LR + i] = pg_dist_seg(i * cr, zg0 + j * cz, segs[s]);
+            for (int i = 0; i < LR; ++i) D[(s * LZ + j) * LR + i] = pg_dist2_seg(i * cr, zg0 + j * cz, segs[s], inv_l2);
+    }
 
     masks->assign(size_t(kPconGridR) * kPconGridZ, 0ull);
     std::vector<double> dmin(ns);
@@ -101,16 +107,19 @@ static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::
             for (size_t s = 0; s < ns; ++s) {
                 const double *L = &D[(s * LZ + j) * LR + i];
                 const double d00 = L[0], d10 = L[1], d01 = L[LR], d11 = L[LR + 1];
-                const double mx = std::fmax(std::fmax(d00, d10), std::fmax(d01, d11));
-                double mn = std::fmin(std::fmin(d00, d10), std::fmin(d01, d11));
-                mn = std::fmin(mn, pg_dist_rect(segs[s].r0, segs[s].z0, u0, u1, v0, v1));
-                mn = std::fmin(mn, pg_dist_rect(segs[s].r1, segs[s].z1, u0, u1, v0, v1));
-                if (pg_seg_meets_rect(segs[s], u0 - margin, u1 + margin, v0 - margin, v1 + margin)) mn = 0;
+                const double mx = pg_max(pg_max(d00, d10), pg_max(d01, d11));
+                double mn = pg_min(pg_min(d00, d10), pg_min(d01, d11));
+                mn = pg_min(mn, pg_dist2_rect(segs[s].r0, segs[s].z0, u0, u1, v0, v1));
+                mn = pg_min(mn, pg_dist2_rect(segs[s].r1, segs[s].z1, u0, u1, v0, v1));
+                const bool boxes_meet = pg_min(segs[s].r0, segs[s].r1) <= u1 + margin && pg_max(segs[s].r0, segs[s].r1) >= u0 - margin &&
+                                        segs[s].z0 <= v1 + margin && segs[s].z1 >= v0 - margin;
+                if (boxes_meet && pg_seg_meets_rect(segs[s], u0 - margin, u1 + margin, v0 - margin, v1 + margin)) mn = 0;
                 dmin[s] = mn;
-                thr = std::fmin(thr, mx);
+                thr = pg_min(thr, mx);
             }
             // inflation by `margin` moves either bound by at most sqrt(2) margin; relative slack for the FMA rounding
-            thr = thr * (1 + 1e-9) + 4 * margin;
+            thr = std::sqrt(thr) * (1 + 1e-9) + 4 * margin;
+            thr *= thr;
             unsigned long long m = 0;
             for (size_t s = 0; s < ns; ++s)
                 if (dmin[s] <= thr) m |= 1ull << segs[s].bit;

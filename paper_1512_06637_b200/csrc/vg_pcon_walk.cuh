@@ -180,16 +180,17 @@ VG_DEV double pcon_walk_sdf(const PolyconeP &p, const PconWalkSec *tab, double x
 
 // ---- candidate-grid form of the same signed distance (vg_pcon_grid.h) ----
 //
-// One record per segment of the (r, z) outline, numbered like the mask bits of the grid: (r0, z0), edge vector,
-// 1 / |edge|^2.  Five doubles per record: an odd stride, so lanes reading different records spread over the banks.
-constexpr int kPconSegStride = 5;
+// One record per segment of the (r, z) outline, numbered like the mask bits of the grid: (r0, z0), the edge vector
+// (er, ez) and the edge vector divided by |edge|^2, so that the foot parameter is t = w . e' (one FMA + one MUL).  Six
+// doubles, 16-byte aligned: three 128-bit shared loads per candidate.
+constexpr int kPconSegStride = 6;
 
 VG_DEV void pcon_stage_segs(const PolyconeP &p, double *seg)
 {
     for (int s = threadIdx.x; s < 64; s += blockDim.x) {
         double r0 = 0, z0 = 0, er = 0, ez = 0, il = 0;
-        const int k = s >> 1;
-        if (k < p.nsec) {
+        const int k = (s - kPconSecBit0) >> 1;
+        if (s >= kPconSecBit0 && k < p.nsec) {
             const PconSec &c = p.sec[k];
             const Frustum &f = (s & 1) ? c.in : c.out;
             r0 = f.r0, z0 = c.z0, er = f.er, ez = c.z1 - c.z0, il = f.inv_l2;
@@ -197,8 +198,20 @@ VG_DEV void pcon_stage_segs(const PolyconeP &p, double *seg)
         if (s == kPconCapLoBit) r0 = p.cap_lo_rmin, z0 = p.zlo, er = p.cap_lo_rmax - p.cap_lo_rmin, il = 1.0 / (er * er);
         if (s == kPconCapHiBit) r0 = p.cap_hi_rmin, z0 = p.zhi, er = p.cap_hi_rmax - p.cap_hi_rmin, il = 1.0 / (er * er);
         double *o = seg + kPconSegStride * s;
-        o[0] = r0, o[1] = z0, o[2] = er, o[3] = ez, o[4] = il;
+        o[0] = r0, o[1] = z0, o[2] = er, o[3] = ez, o[4] = er * il, o[5] = ez * il;
     }
+}
+
+// squared distance from (u, v) to the segment of record q (same value as seg_d2 up to the rounding of e' = e / |e|^2)
+VG_DEV double pcon_seg_d2(double u, double v, const double *q)
+{
+    const double2 a = *reinterpret_cast<const double2 *>(q), e = *reinterpret_cast<const double2 *>(q + 2),
+                  f = *reinterpret_cast<const double2 *>(q + 4);
+    const double wu = u - a.x, wv = v - a.y;
+    double t = fma(wu, f.x, wv * f.y);
+    t = dmin(dmax(t, 0.0), 1.0);
+    const double du = fma(-t, e.x, wu), dv = fma(-t, e.y, wv);
+    return fma(du, du, dv * dv);
 }
 
 // exact signed distance: minimum over the candidate segments of the point's cell (the cell's mask holds every segment
@@ -211,7 +224,7 @@ VG_DEV double pcon_grid_sdf(const PolyconeP &p, const PconWalkSec *tab, const do
     const double fr = rho * g.g.inv_cr, fz = (z - g.g.zg0) * g.g.inv_cz;
     if (!(fr < double(kPconGridR) && fz >= 0.0 && fz < double(kPconGridZ))) return pcon_walk_sdf(p, tab, x, y, z);
     const int ir = int(fr), iz = int(fz);
-    unsigned long long m = __ldg(g.masks + iz * kPconGridR + ir);
+    const uint2 m = __ldg(reinterpret_cast<const uint2 *>(g.masks) + iz * kPconGridR + ir);
     int kz = __ldg(g.rows + iz);
     while (kz + 1 < p.nsec && tab[kz + 1].z0 <= z) ++kz;
     bool in2d;
@@ -220,11 +233,17 @@ VG_DEV double pcon_grid_sdf(const PolyconeP &p, const PconWalkSec *tab, const do
         in2d = z >= p.zlo && z <= p.zhi && rho <= fma(w.Bo, z, w.Ao) && rho >= fma(w.Bi, z, w.Ai);
     }
     double d2 = inf();
-    while (m) {
-        const int s = __ffsll((long long)m) - 1;
-        m &= m - 1;
-        const double *q = seg + kPconSegStride * s;
-        d2 = dmin(d2, seg_d2(rho, z, q[0], q[1], q[2], q[3], q[4]));
+    unsigned w = m.x; // caps and sections 0..14
+    while (w) {
+        const int s = __ffs(int(w)) - 1;
+        w &= w - 1;
+        d2 = dmin(d2, pcon_seg_d2(rho, z, seg + kPconSegStride * s));
+    }
+    w = m.y; // sections 15..30
+    while (w) {
+        const int s = __ffs(int(w)) + 31;
+        w &= w - 1;
+        d2 = dmin(d2, pcon_seg_d2(rho, z, seg + kPconSegStride * s));
     }
     const double dist = sqrt_nn(d2);
     return in2d ? -dist : dist;
@@ -254,7 +273,7 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
 {
     constexpr bool kDir = (Q == qDistIn);
     __shared__ __align__(16) PconWalkSec tab[kMaxSec];
-    __shared__ double seg[GRID ? 64 * kPconSegStride : 1];
+    __shared__ __align__(16) double seg[GRID ? 64 * kPconSegStride : 2];
     pcon_stage(p, tab);
     if (GRID) pcon_stage_segs(p, seg);
     pdl_launch_dependents();
