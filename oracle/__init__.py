@@ -37,6 +37,12 @@ def _load(path):
     lib.orc_cross.argtypes = [C.c_void_p, _P, _P, _P, _P, _P, _P, C.c_int64, _P]
     lib.orc_compute_step.argtypes = [C.c_void_p, _P, _P, _P, _P, _P, _P, C.c_double, C.c_int64, _P, _PI]
     lib.orc_volume_safety.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _P]
+    lib.orc_world_create.restype = C.c_void_p
+    lib.orc_world_create.argtypes = [C.c_int, C.POINTER(C.c_void_p), _PI, _P]
+    lib.orc_world_destroy.argtypes = [C.c_void_p]
+    lib.orc_world_locate.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _PI]
+    lib.orc_world_step.argtypes = [C.c_void_p, _PI, _P, _P, _P, _P, _P, _P, C.c_double, C.c_int64, _P, _PI]
+    lib.orc_world_safety.argtypes = [C.c_void_p, _PI, _P, _P, _P, C.c_int64, _P]
     return lib
 
 
@@ -158,4 +164,47 @@ class Volume:
         x, y, z = map(_arr, (x, y, z))
         out = np.empty_like(x)
         self._l.orc_volume_safety(self._h, _ptr(x), _ptr(y), _ptr(z), x.size, _ptr(out))
+        return out
+
+
+class World:
+    """Tree of placed solids (readings R22-R25, vg_oracle.c): node 0 is the root, `parents[i] < i`,
+    `xforms` is (nn, 12) row-major [R | b] from the parent's local frame (the world frame for the root)."""
+
+    def __init__(self, shapes, parents, xforms):
+        self.shapes = list(shapes)
+        self._l = self.shapes[0]._l
+        nn = len(self.shapes)
+        self.parents = np.ascontiguousarray(np.asarray(parents, dtype=np.int32).reshape(nn))
+        self.xforms = np.ascontiguousarray(np.asarray(xforms, dtype=np.float64).reshape(nn, 12))
+        arr = (C.c_void_p * nn)(*[s._h for s in self.shapes])
+        self._h = self._l.orc_world_create(nn, arr, self.parents.ctypes.data_as(_PI), _ptr(self.xforms))
+        if not self._h:
+            raise ValueError("oracle: invalid world")
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._l.orc_world_destroy(self._h)
+            self._h = None
+
+    def locate(self, x, y, z):
+        x, y, z = map(_arr, (x, y, z))
+        node = np.empty(x.shape, dtype=np.int32)
+        self._l.orc_world_locate(self._h, _ptr(x), _ptr(y), _ptr(z), x.size, node.ctypes.data_as(_PI))
+        return node
+
+    def step(self, node, x, y, z, dx, dy, dz, step_max=np.inf):
+        x, y, z, dx, dy, dz = map(_arr, (x, y, z, dx, dy, dz))
+        node = np.ascontiguousarray(node, dtype=np.int32)
+        step = np.empty_like(x)
+        nxt = np.empty(x.shape, dtype=np.int32)
+        self._l.orc_world_step(self._h, node.ctypes.data_as(_PI), _ptr(x), _ptr(y), _ptr(z), _ptr(dx), _ptr(dy),
+                               _ptr(dz), float(step_max), x.size, _ptr(step), nxt.ctypes.data_as(_PI))
+        return step, nxt
+
+    def safety(self, node, x, y, z):
+        x, y, z = map(_arr, (x, y, z))
+        node = np.ascontiguousarray(node, dtype=np.int32)
+        out = np.empty_like(x)
+        self._l.orc_world_safety(self._h, node.ctypes.data_as(_PI), _ptr(x), _ptr(y), _ptr(z), x.size, _ptr(out))
         return out

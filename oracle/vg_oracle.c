@@ -6,10 +6,12 @@
  * "Is the particle inside or outside the solid?", "What is the minimal
  * distance between the particle and the border of the solid?", "What is the
  * maximal step length for a particle with a given velocity and direction?")
- * for box / orb / tube segment / cone segment / trd / polycone, and the
+ * for box / orb / tube segment / cone segment / trd / polycone, the
  * one-level navigation step (distance to the geometric
  * border against the physics step; "coordinate transformations and distance
- * calculations").
+ * calculations"), and the same step in a tree of placed volumes with the
+ * point location that goes with it ("hierarchical connections";
+ * readings R22-R25 at the end of this file).
  *
  * The paper gives no formula for any solid.  Every query here is the PLAIN
  * DEFINITION written out as brute force over the boundary patches of the
@@ -32,8 +34,10 @@
  * sampling for every sdf, the eikonal property, sphere tracing and ray
  * marching for every first crossing, special-case reductions between solids
  * (trd==box, cone==tube, polycone==cone==tube, inserted collinear z-plane),
- * rigid-motion and permutation invariance of the navigation step, and the
- * 80-bit long-double build of this same file (-DORC_LONG_DOUBLE).
+ * rigid-motion and permutation invariance of the navigation step, the world
+ * queries against per-node membership / one-level steps composed in numpy and
+ * against marching through orc_world_locate (tests/test_oracle_world.py), and
+ * the 80-bit long-double build of this same file (-DORC_LONG_DOUBLE).
  * Parity unpinned: nothing under readings R1-R21; behaviour INSIDE the
  * kTol surface band (R7) is outside the parity contract.
  */
@@ -652,6 +656,151 @@ void orc_volume_safety(const orc_volume *v, const double *x, const double *y, co
             real pl[3], dl[3];
             to_local(v->xf + 12 * k, p, d0, pl, dl);
             best = rmin2(best, sdf(v->daughter[k], pl[0], pl[1], pl[2]));
+        }
+        out[i] = (double)best;
+    }
+}
+
+/* ------------------------------------------------- hierarchy of volumes */
+/*
+ * Widening SURVEY.md 8(f) f3: "with hierarchical connections one can build
+ * the whole detector"; a particle whose geometric step wins
+ * "is transported to the border" and changes volume.  The paper
+ * gives no data structure or algorithm; readings R22-R25 of DESIGN.md:
+ *   R22  a world is a tree of placed solids ("nodes"): node 0 is the root,
+ *        parent[i] < i, xf[i] = row-major 3x4 [R | b] from the PARENT's local
+ *        frame to node i's local frame (for the root: from the world frame);
+ *        the children of a node are the nodes naming it as parent, in index
+ *        order; siblings do not overlap and lie inside their parent.
+ *   R23  Locate(p): -1 if p is not strictly inside the root (Inside != INSIDE);
+ *        else descend from the root: the first child (index order) that holds
+ *        p strictly inside becomes the current node; stop when no child does.
+ *   R24  Step(node, p, d): p, d given in the WORLD frame and mapped down the
+ *        chain root -> node one transform at a time; the one-level ComputeStep
+ *        of c.2 in that node (its solid as mother, its children as daughters,
+ *        R13 tie-break); `next` is the child entered, the parent (-1 above the
+ *        root) when the node's own exit wins, the node itself when step_max
+ *        wins (the physics step is shorter).
+ *   R25  Safety(node, p): min(SafetyToOut_node, SafetyToIn of every child),
+ *        i.e. orc_volume_safety in that node.
+ */
+
+typedef struct {
+    int nn;
+    const orc_shape **shape;
+    int32_t *parent;
+    real *xf; /* nn * 12 */
+} orc_world;
+
+orc_world *orc_world_create(int nn, const orc_shape *const *shapes, const int32_t *parent, const double *xf)
+{
+    if (nn < 1 || !shapes || !parent || !xf || parent[0] != -1) return NULL;
+    for (int i = 0; i < nn; ++i) {
+        if (!shapes[i]) return NULL;
+        if (i > 0 && (parent[i] < 0 || parent[i] >= i)) return NULL;
+    }
+    if (!finite_all(xf, 12 * nn)) return NULL;
+    orc_world *w = (orc_world *)calloc(1, sizeof *w);
+    if (!w) return NULL;
+    w->nn = nn;
+    w->shape = (const orc_shape **)calloc((size_t)nn, sizeof *w->shape);
+    w->parent = (int32_t *)calloc((size_t)nn, sizeof *w->parent);
+    w->xf = (real *)calloc((size_t)nn * 12, sizeof *w->xf);
+    for (int i = 0; i < nn; ++i) {
+        w->shape[i] = shapes[i];
+        w->parent[i] = parent[i];
+        for (int k = 0; k < 12; ++k) w->xf[12 * i + k] = xf[12 * i + k];
+    }
+    return w;
+}
+
+void orc_world_destroy(orc_world *w)
+{
+    if (!w) return;
+    free((void *)w->shape);
+    free(w->parent);
+    free(w->xf);
+    free(w);
+}
+
+/* world frame -> local frame of `node`, one transform at a time from the root down (R24) */
+static void world_to_node(const orc_world *w, int node, const real p[3], const real d[3], real pl[3], real dl[3])
+{
+    real pp[3], dp[3];
+    if (w->parent[node] >= 0) world_to_node(w, w->parent[node], p, d, pp, dp);
+    else { for (int k = 0; k < 3; ++k) { pp[k] = p[k]; dp[k] = d[k]; } }
+    to_local(w->xf + 12 * node, pp, dp, pl, dl);
+}
+
+/* R23 */
+void orc_world_locate(const orc_world *w, const double *x, const double *y, const double *z, int64_t n, int32_t *node)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d0[3] = { 0, 0, 0 }, pl[3], dl[3];
+        to_local(w->xf, p, d0, pl, dl);
+        if (inside(w->shape[0], pl[0], pl[1], pl[2]) != ORC_INSIDE) { node[i] = -1; continue; }
+        int cur = 0, moved = 1;
+        while (moved) {
+            moved = 0;
+            for (int c = cur + 1; c < w->nn; ++c) {
+                if (w->parent[c] != cur) continue;
+                real pc[3];
+                to_local(w->xf + 12 * c, pl, d0, pc, dl);
+                if (inside(w->shape[c], pc[0], pc[1], pc[2]) == ORC_INSIDE) {
+                    cur = c;
+                    pl[0] = pc[0]; pl[1] = pc[1]; pl[2] = pc[2];
+                    moved = 1;
+                    break;
+                }
+            }
+        }
+        node[i] = cur;
+    }
+}
+
+/* R24 */
+void orc_world_step(const orc_world *w, const int32_t *node, const double *x, const double *y, const double *z,
+                    const double *dx, const double *dy, const double *dz, double step_max, int64_t n, double *step,
+                    int32_t *next)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        int nd = node[i];
+        if (nd < 0 || nd >= w->nn) { step[i] = -1; next[i] = -1; continue; }
+        real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] }, pl[3], dl[3];
+        world_to_node(w, nd, p, d, pl, dl);
+        real best = distance_to_out(w->shape[nd], pl, dl, ORC_INF);
+        int32_t who = w->parent[nd];
+        for (int c = nd + 1; c < w->nn; ++c) {
+            if (w->parent[c] != nd) continue;
+            real pc[3], dc[3];
+            to_local(w->xf + 12 * c, pl, dl, pc, dc);
+            real t = distance_to_in(w->shape[c], pc, dc, ORC_INF);
+            if (t >= 0 && t < best) { best = t; who = c; }
+        }
+        if (best > step_max) { best = step_max; who = nd; }
+        step[i] = (double)best;
+        next[i] = who;
+    }
+}
+
+/* R25 */
+void orc_world_safety(const orc_world *w, const int32_t *node, const double *x, const double *y, const double *z,
+                      int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        int nd = node[i];
+        if (nd < 0 || nd >= w->nn) { out[i] = -1; continue; }
+        real p[3] = { x[i], y[i], z[i] }, d0[3] = { 0, 0, 0 }, pl[3], dl[3];
+        world_to_node(w, nd, p, d0, pl, dl);
+        real best = -sdf(w->shape[nd], pl[0], pl[1], pl[2]);
+        for (int c = nd + 1; c < w->nn; ++c) {
+            if (w->parent[c] != nd) continue;
+            real pc[3];
+            to_local(w->xf + 12 * c, pl, d0, pc, dl);
+            best = rmin2(best, sdf(w->shape[c], pc[0], pc[1], pc[2]));
         }
         out[i] = (double)best;
     }

@@ -207,3 +207,85 @@ class NavigatorCase:
 
 def navigator_case(**kw):
     return NavigatorCase(**kw)
+
+
+# ------------------------------------------------------------- hierarchy of volumes
+
+class WorldCase:
+    """A three-level tree of placed solids (readings R22-R25): the mother box and the 64 daughters of
+    configs[4] (nodes 1..64), and two grand-daughters with seeded random rotations inside every daughter
+    (nodes 65..192): an orb r = 3 and a trd inside each box, a hollow tube segment and a cone inside each tube.
+    Bounding spheres are disjoint and inside the parent, so siblings never overlap whatever the rotation.
+
+    Tracks: half of the points uniform in the mother box, half uniform in the local cube [-8, 8]^3 of a random
+    daughter (so that about a third of the tracks start below the root), isotropic directions.
+    """
+
+    def __init__(self, seed=None, n=4194304):
+        nav = NavigatorCase(seed=config_seed(4) if seed is None else seed, n=n)
+        self.cfg, self.seed, self.sizes = 5, nav.seed + 11, (n,)
+        self.center, self.half = nav.center, nav.half
+        rng = _rng(self.seed)
+        kinds, params, parents, xf = [nav.mother_kind], [nav.mother_params], [-1], [placement(np.eye(3), (0, 0, 0))]
+        for k in range(len(nav.daughter_kinds)):
+            kinds.append(nav.daughter_kinds[k])
+            params.append(nav.daughter_params[k])
+            parents.append(0)
+            xf.append(nav.xforms[k])
+        inner = {BOX: [(ORB, [3.0], (-3.5, 0.0, 0.0)), (TRD, [1.5, 2.5, 2.0, 1.0, 1.5], (4.0, 1.0, -1.0))],
+                 TUBE: [(TUBE, [1.0, 3.0, 3.0, 0.0, 4.0 * math.pi / 3.0], (0.0, 3.5, 2.0)),
+                        (CONE, [0.0, 1.0, 0.0, 2.5, 2.0, 0.0, TWO_PI], (0.0, -4.0, -3.0))]}
+        for k in range(len(nav.daughter_kinds)):
+            for kind, par, c in inner[nav.daughter_kinds[k]]:
+                u1, u2, u3 = rng.random(3)
+                q = (math.sqrt(1 - u1) * math.sin(TWO_PI * u2), math.sqrt(1 - u1) * math.cos(TWO_PI * u2),
+                     math.sqrt(u1) * math.sin(TWO_PI * u3), math.sqrt(u1) * math.cos(TWO_PI * u3))
+                kinds.append(kind)
+                params.append(par)
+                parents.append(1 + k)
+                xf.append(placement(quaternion_to_matrix(q), c))
+        self.kinds, self.params = kinds, params
+        self.parents = np.asarray(parents, dtype=np.int32)
+        self.xforms = np.ascontiguousarray(np.stack(xf))
+        self.level1 = np.arange(1, 1 + len(nav.daughter_kinds))
+
+    def tracks(self, n=None, band=None, max_rounds=64):
+        """`band(x, y, z)` -> True for points to redraw (surface band of any node, or outside the world)."""
+        n = int(self.sizes[-1] if n is None else n)
+        rng = _rng(self.seed + 1)
+
+        def points(m):
+            p = (2.0 * rng.random((m, 3)) - 1.0) * np.asarray(self.half)
+            low = rng.random(m) < 0.5
+            which = self.level1[rng.integers(0, len(self.level1), m)]
+            loc = (2.0 * rng.random((m, 3)) - 1.0) * 8.0
+            M = self.xforms[which].reshape(m, 3, 4)
+            # local -> mother: p = R^T (p_loc - b)
+            back = np.einsum("nji,nj->ni", M[:, :, :3], loc - M[:, :, 3])
+            p[low] = back[low]
+            return p
+
+        p = points(n)
+        v = rng.random((n, 2))
+        dz = 2.0 * v[:, 0] - 1.0
+        phi = TWO_PI * v[:, 1]
+        s = np.sqrt(np.maximum(0.0, 1.0 - dz * dz))
+        dx, dy = s * np.cos(phi), s * np.sin(phi)
+        norm = np.sqrt(dx * dx + dy * dy + dz * dz)
+        dx, dy, dz = dx / norm, dy / norm, dz / norm
+        x, y, z = (np.ascontiguousarray(p[:, i]) for i in range(3))
+        if band is not None and n > 0:
+            bad = np.flatnonzero(np.asarray(band(x, y, z), dtype=bool))
+            rounds = 0
+            while bad.size:
+                rounds += 1
+                if rounds > max_rounds:
+                    raise RuntimeError("WorldCase.tracks: rejection did not terminate")
+                q = points(bad.size)
+                x[bad], y[bad], z[bad] = q[:, 0], q[:, 1], q[:, 2]
+                bad = bad[np.asarray(band(x[bad], y[bad], z[bad]), dtype=bool)]
+        return x, y, z, np.ascontiguousarray(dx), np.ascontiguousarray(dy), np.ascontiguousarray(dz)
+
+
+def world_case(**kw):
+    return WorldCase(**kw)
