@@ -146,6 +146,46 @@ int vg_compute_step(const vg_volume *volume, const double *x, const double *y, c
 int vg_volume_safety(const vg_volume *volume, const double *x, const double *y, const double *z, int64_t n,
                      double *safety, void *stream);
 
+/* ---- hierarchy of volumes ("with hierarchical connections one can build the whole detector";
+ *      a particle whose geometric step wins "is transported to the border" and changes volume;
+ *      SURVEY.md sec. 8(f) f3; readings R22-R25 in DESIGN.md) ----
+ *
+ * A world is a tree of placed solids ("nodes").  Node 0 is the root; parent[i] < i for i > 0, parent[0] = -1.
+ * `xforms` (HOST): nnodes * 12 doubles, row-major 3x4 [R | b] per node, from the PARENT's local frame to the
+ * node's local frame (for the root: from the world frame), orthonormal R as for vg_volume_create.  The children of
+ * a node are the nodes that name it as parent, in index order; siblings must not overlap and must lie inside
+ * their parent (not checked).  Node kinds: box, orb, tube, cone, trd.  1 <= nnodes <= VG_MAX_NODES; a node has
+ * at most VG_MAX_DAUGHTERS children.  The shapes' constants are copied.  The node table lives in memory of the
+ * device that is current at create time.
+ */
+typedef struct vg_world vg_world;
+#define VG_MAX_NODES 65536
+int vg_world_create(int nnodes, const vg_shape *const *shapes, const int32_t *parent, const double *xforms,
+                    vg_world **out);
+void vg_world_destroy(vg_world *world); /* NULL is allowed */
+
+/* vg_world_locate -- the deepest node that holds each of n points given in the world frame (R23): -1 if the point
+ * is not strictly inside the root (Inside != VG_INSIDE); else descend from the root, the first child in index
+ * order that holds the point strictly inside becomes the current node, until no child does.
+ * node: DEVICE int32[n]. */
+int vg_world_locate(const vg_world *world, const double *x, const double *y, const double *z, int64_t n,
+                    int32_t *node, void *stream);
+
+/* vg_world_step -- navigation step of n tracks, each in its own node (R24).  x..dz are in the WORLD frame;
+ * node: DEVICE int32[n], the node each track is in (as vg_world_locate returns it).  The step is vg_compute_step
+ * in that node (its solid as mother, its children as daughters, same tie-break); next: DEVICE int32[n] = the child
+ * entered, the parent when the node's own exit wins (-1 above the root), the node itself when step_max wins.
+ * A track with node outside [0, nnodes) gets (-1, -1).  step: DEVICE double[n]. */
+int vg_world_step(const vg_world *world, const int32_t *node, const double *x, const double *y, const double *z,
+                  const double *dx, const double *dy, const double *dz, double step_max, int64_t n, double *step,
+                  int32_t *next, void *stream);
+
+/* vg_world_safety -- vg_volume_safety in the node of each point (R25): min(SafetyToOut of the node, SafetyToIn of
+ * every child); for a located point this is the distance to the nearest surface of ANY node of the world.
+ * -1 for a node outside [0, nnodes).  safety: DEVICE double[n]. */
+int vg_world_safety(const vg_world *world, const int32_t *node, const double *x, const double *y, const double *z,
+                    int64_t n, double *safety, void *stream);
+
 /* ---- host-buffer entry points (the scheduler hands baskets of tracks to the geometry every step;
  *      the GPU pays off once transfers are amortised) ----
  *

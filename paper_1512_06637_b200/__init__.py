@@ -51,6 +51,12 @@ def _load():
     lib.vg_volume_destroy.restype = None
     lib.vg_compute_step.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP, _VP]
     lib.vg_volume_safety.argtypes = [_VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
+    lib.vg_world_create.argtypes = [C.c_int, C.POINTER(_VP), C.POINTER(C.c_int32), _PD, C.POINTER(_VP)]
+    lib.vg_world_destroy.argtypes = [_VP]
+    lib.vg_world_destroy.restype = None
+    lib.vg_world_locate.argtypes = [_VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
+    lib.vg_world_step.argtypes = [_VP, _VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP, _VP]
+    lib.vg_world_safety.argtypes = [_VP, _VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
     lib.vg_query_host.argtypes = [_VP, C.c_int] + [_VP] * 6 + [C.c_double, C.c_int64, _VP]
     lib.vg_query_all_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64] + [_VP] * 5
     lib.vg_compute_step_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP]
@@ -134,7 +140,7 @@ def vg_shape_destroy(h):
 
 
 def _handle(s):
-    return s._h if isinstance(s, (Shape, Volume)) else s
+    return s._h if isinstance(s, (Shape, Volume, World)) else s
 
 
 def vg_inside(shape, x, y, z, out=None, stream=None):
@@ -222,6 +228,60 @@ def vg_volume_safety(volume, x, y, z, out=None, stream=None):
     out = _out(out, n, dev, torch.float64)
     with torch.cuda.device(dev):
         _check(_lib.vg_volume_safety(_handle(volume), _p(x), _p(y), _p(z), n, _p(out), _stream(stream)))
+    return out
+
+
+# ---- hierarchy of volumes (readings R22-R25) ----
+
+def vg_world_create(shapes, parents, xforms):
+    nn = len(shapes)
+    arr = (_VP * nn)(*[_handle(s) for s in shapes])
+    par = (C.c_int32 * nn)(*[int(v) for v in parents])
+    flat = [float(v) for row in xforms for v in row]
+    if len(flat) != 12 * nn:
+        raise ValueError("xforms must hold 12 doubles per node")
+    xf = (C.c_double * len(flat))(*flat)
+    h = _VP()
+    _check(_lib.vg_world_create(nn, arr, par, xf, C.byref(h)))
+    return h
+
+
+def vg_world_destroy(h):
+    _lib.vg_world_destroy(h)
+
+
+def _nodes(node, n, dev):
+    if not isinstance(node, torch.Tensor) or node.dtype != torch.int32 or node.numel() != n or node.device != dev or \
+            not node.is_contiguous():
+        raise TypeError("node: int32 CUDA tensor of the tracks' length expected")
+    return node
+
+
+def vg_world_locate(world, x, y, z, out=None, stream=None):
+    n, dev = _tracks((x, y, z))
+    out = _out(out, n, dev, torch.int32)
+    with torch.cuda.device(dev):
+        _check(_lib.vg_world_locate(_handle(world), _p(x), _p(y), _p(z), n, _p(out), _stream(stream)))
+    return out
+
+
+def vg_world_step(world, node, x, y, z, dx, dy, dz, step_max=math.inf, step=None, next=None, stream=None):
+    n, dev = _tracks((x, y, z, dx, dy, dz))
+    node = _nodes(node, n, dev)
+    step = _out(step, n, dev, torch.float64)
+    nxt = _out(next, n, dev, torch.int32)
+    with torch.cuda.device(dev):
+        _check(_lib.vg_world_step(_handle(world), _p(node), _p(x), _p(y), _p(z), _p(dx), _p(dy), _p(dz), float(step_max), n,
+                                  _p(step), _p(nxt), _stream(stream)))
+    return step, nxt
+
+
+def vg_world_safety(world, node, x, y, z, out=None, stream=None):
+    n, dev = _tracks((x, y, z))
+    node = _nodes(node, n, dev)
+    out = _out(out, n, dev, torch.float64)
+    with torch.cuda.device(dev):
+        _check(_lib.vg_world_safety(_handle(world), _p(node), _p(x), _p(y), _p(z), n, _p(out), _stream(stream)))
     return out
 
 
@@ -370,3 +430,26 @@ class Volume:
 
     def safety(self, x, y, z, **kw):
         return vg_volume_safety(self, x, y, z, **kw)
+
+
+class World:
+    """Tree of placed solids: node 0 is the root, `parents[i] < i`, `xforms` (nn, 12) row-major [R | b] from the
+    parent's local frame (the world frame for the root) to the node's (readings R22-R25)."""
+
+    def __init__(self, shapes, parents, xforms):
+        self.nn = len(shapes)
+        self._h = vg_world_create(shapes, parents, [list(map(float, r)) for r in xforms])
+
+    def __del__(self, _destroy=_lib.vg_world_destroy):
+        h, self._h = getattr(self, "_h", None), None
+        if h:
+            _destroy(h)
+
+    def locate(self, x, y, z, **kw):
+        return vg_world_locate(self, x, y, z, **kw)
+
+    def step(self, node, x, y, z, dx, dy, dz, step_max=math.inf, **kw):
+        return vg_world_step(self, node, x, y, z, dx, dy, dz, step_max, **kw)
+
+    def safety(self, node, x, y, z, **kw):
+        return vg_world_safety(self, node, x, y, z, **kw)

@@ -10,6 +10,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 using namespace vg;
 
@@ -428,6 +429,162 @@ extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const doubl
     if (n == 0) return VG_OK;
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
     cudaError_t e = launch_volume_safety(v->mother, v->table_dev, v->meta, t, n, safety, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+// ------------------------------------------------------------------------------------- hierarchy of volumes
+
+struct vg_world {
+    int nn;
+    WorldNode *nodes_dev; // one allocation: nn WorldNode records followed by the child lists (int32)
+    int32_t *kids_dev;
+    int device;
+};
+
+static bool rigid(const double *m)
+{
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) {
+            double dot = m[4 * r] * m[4 * c] + m[4 * r + 1] * m[4 * c + 1] + m[4 * r + 2] * m[4 * c + 2];
+            if (std::fabs(dot - (r == c ? 1.0 : 0.0)) > 1e-9) return false;
+        }
+    return true;
+}
+
+// C = A o B for row-major 3x4 [R | b]: first B, then A
+static void compose(const double *A, const double *B, double *C)
+{
+    for (int r = 0; r < 3; ++r) {
+        for (int c = 0; c < 3; ++c) C[4 * r + c] = A[4 * r] * B[c] + A[4 * r + 1] * B[4 + c] + A[4 * r + 2] * B[8 + c];
+        C[4 * r + 3] = A[4 * r] * B[3] + A[4 * r + 1] * B[7] + A[4 * r + 2] * B[11] + A[4 * r + 3];
+    }
+}
+
+extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int32_t *parent, const double *xforms,
+                               vg_world **out)
+{
+    const char *fn = "vg_world_create";
+    if (!out) return fail(VG_ERR_ARG, "%s: out is NULL", fn);
+    *out = nullptr;
+    if (nn < 1 || nn > VG_MAX_NODES) return fail(VG_ERR_PARAM, "%s: nnodes must be in [1, %d]", fn, VG_MAX_NODES);
+    if (!shapes || !parent || !xforms) return fail(VG_ERR_ARG, "%s: NULL shapes, parent or xforms", fn);
+    if (parent[0] != -1) return fail(VG_ERR_PARAM, "%s: node 0 is the root, parent[0] must be -1", fn);
+    std::vector<WorldNode> nodes(nn);
+    std::vector<int32_t> kids(nn > 1 ? nn - 1 : 1, 0);
+    std::vector<int> count(nn, 0), fill(nn, 0);
+    for (int i = 1; i < nn; ++i) {
+        if (parent[i] < 0 || parent[i] >= i) return fail(VG_ERR_PARAM, "%s: need 0 <= parent[%d] < %d", fn, i, i);
+        if (++count[parent[i]] > VG_MAX_DAUGHTERS)
+            return fail(VG_ERR_PARAM, "%s: node %d has more than %d children", fn, parent[i], VG_MAX_DAUGHTERS);
+    }
+    for (int i = 0, off = 0; i < nn; ++i) {
+        WorldNode &N = nodes[i];
+        std::memset(&N, 0, sizeof N);
+        if (!shapes[i]) return fail(VG_ERR_ARG, "%s: shape %d is NULL", fn, i);
+        const double *m = xforms + 12 * i;
+        if (!all_finite(m, 12)) return fail(VG_ERR_PARAM, "%s: non-finite transform of node %d", fn, i);
+        if (!rigid(m)) return fail(VG_ERR_PARAM, "%s: rotation of node %d is not orthonormal", fn, i);
+        int rc = to_solid(shapes[i], &N.s, "node");
+        if (rc != VG_OK) return rc;
+        std::memcpy(N.X, m, sizeof N.X);
+        if (i == 0) std::memcpy(N.G, m, sizeof N.G);
+        else compose(m, nodes[parent[i]].G, N.G);
+        N.parent = parent[i];
+        N.child0 = off;
+        N.nchild = count[i];
+        off += count[i];
+        if (i > 0) kids[nodes[parent[i]].child0 + fill[parent[i]]++] = i; // ascending i: lists come out sorted
+    }
+    for (int i = 0; i < nn; ++i) {
+        // bounding sphere in the parent's frame: centre c = -R^T b.  The tests evaluate |p - c|^2 (- (v.d)^2) in FP64 with
+        // |p - c| <= S = (parent's radius) + |c| + r: rounding error < 16 u S^2 (u = 2^-53); inflate well beyond it.
+        WorldNode &N = nodes[i];
+        const double *m = N.X;
+        double cx = -(m[0] * m[3] + m[4] * m[7] + m[8] * m[11]);
+        double cy = -(m[1] * m[3] + m[5] * m[7] + m[9] * m[11]);
+        double cz = -(m[2] * m[3] + m[6] * m[7] + m[10] * m[11]);
+        double r = bounding_radius(N.s);
+        double rp = i > 0 ? bounding_radius(nodes[parent[i]].s) : r;
+        double S = rp + std::sqrt(cx * cx + cy * cy + cz * cz) + r;
+        N.bs[0] = cx, N.bs[1] = cy, N.bs[2] = cz;
+        N.bs[3] = r * r * (1.0 + 1e-9) + 1e-12 * S * S;
+        N.br = std::sqrt(N.bs[3]);
+    }
+    vg_world *w = new (std::nothrow) vg_world;
+    if (!w) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
+    std::memset(w, 0, sizeof *w);
+    w->nn = nn;
+    const size_t nbytes = size_t(nn) * sizeof(WorldNode), kbytes = kids.size() * sizeof(int32_t);
+    unsigned char *blob = nullptr;
+    cudaError_t e = cudaGetDevice(&w->device);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + kbytes);
+    if (e == cudaSuccess) e = cudaMemcpy(blob, nodes.data(), nbytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes, kids.data(), kbytes, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        if (blob) cudaFree(blob);
+        delete w;
+        return fail_cuda(e, fn);
+    }
+    w->nodes_dev = reinterpret_cast<WorldNode *>(blob);
+    w->kids_dev = reinterpret_cast<int32_t *>(blob + nbytes);
+    *out = w;
+    return VG_OK;
+}
+
+extern "C" void vg_world_destroy(vg_world *w)
+{
+    if (!w) return;
+    if (w->nodes_dev) cudaFree(w->nodes_dev);
+    delete w;
+}
+
+extern "C" int vg_world_locate(const vg_world *w, const double *x, const double *y, const double *z, int64_t n,
+                               int32_t *node, void *stream)
+{
+    const char *fn = "vg_world_locate";
+    if (!w) return fail(VG_ERR_ARG, "%s: world is NULL", fn);
+    const void *ptrs[3] = { x, y, z };
+    bool vec = false;
+    int rc = check_arrays(fn, ptrs, 3, 4, node, n, &vec);
+    if (rc != VG_OK || n == 0) return rc;
+    Tracks t{ x, y, z, nullptr, nullptr, nullptr };
+    cudaError_t e = launch_world_locate(w->nodes_dev, w->kids_dev, t, n, node, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+extern "C" int vg_world_step(const vg_world *w, const int32_t *node, const double *x, const double *y, const double *z,
+                             const double *dx, const double *dy, const double *dz, double step_max, int64_t n,
+                             double *step, int32_t *next, void *stream)
+{
+    const char *fn = "vg_world_step";
+    if (!w) return fail(VG_ERR_ARG, "%s: world is NULL", fn);
+    const void *ptrs[6] = { x, y, z, dx, dy, dz };
+    bool vec = false;
+    int rc = check_arrays(fn, ptrs, 6, 8, step, n, &vec);
+    if (rc != VG_OK || n == 0) return rc;
+    if (!node || !aligned(node, 4) || !next || !aligned(next, 4)) return fail(VG_ERR_ARG, "%s: node / next array NULL or misaligned", fn);
+    if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
+    Tracks t{ x, y, z, dx, dy, dz };
+    cudaError_t e = launch_world_step(w->nodes_dev, w->kids_dev, w->nn, node, t, step_max, n, step, next,
+                                      static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const double *x, const double *y, const double *z,
+                               int64_t n, double *safety, void *stream)
+{
+    const char *fn = "vg_world_safety";
+    if (!w) return fail(VG_ERR_ARG, "%s: world is NULL", fn);
+    const void *ptrs[3] = { x, y, z };
+    bool vec = false;
+    int rc = check_arrays(fn, ptrs, 3, 8, safety, n, &vec);
+    if (rc != VG_OK || n == 0) return rc;
+    if (!node || !aligned(node, 4)) return fail(VG_ERR_ARG, "%s: node array NULL or misaligned", fn);
+    Tracks t{ x, y, z, nullptr, nullptr, nullptr };
+    cudaError_t e = launch_world_safety(w->nodes_dev, w->kids_dev, w->nn, node, t, n, safety, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }

@@ -15,6 +15,7 @@
 // The tie-break of R13 (lowest index, mother first) is kept by comparing (t, k) pairs explicitly, because
 // candidates are not visited in index order.
 #include "vg_kernels.cuh"
+#include "vg_solid.cuh"
 #include "vg_tma.cuh"
 
 namespace vg {
@@ -26,39 +27,6 @@ VG_DEV void tma_load_table(void *dst_smem, const void *src_gmem, uint32_t bytes,
 {
     mbar_expect_tx(bar, bytes);
     bulk_g2s(dst_smem, src_gmem, bytes, bar);
-}
-
-VG_DEV double solid_dist_in(const SolidU &s, double x, double y, double z, double dx, double dy, double dz)
-{
-    switch (s.kind) { // warp-uniform
-    case kBox: return Box::dist_in(s.u.box, x, y, z, dx, dy, dz);
-    case kOrb: return Orb::dist_in(s.u.orb, x, y, z, dx, dy, dz);
-    case kTube: return Tube::dist_in(s.u.tube, x, y, z, dx, dy, dz);
-    case kCone: return Cone::dist_in(s.u.cone, x, y, z, dx, dy, dz);
-    default: return Trd::dist_in(s.u.trd, x, y, z, dx, dy, dz);
-    }
-}
-
-VG_DEV double solid_dist_out(const SolidU &s, double x, double y, double z, double dx, double dy, double dz)
-{
-    switch (s.kind) {
-    case kBox: return Box::dist_out(s.u.box, x, y, z, dx, dy, dz);
-    case kOrb: return Orb::dist_out(s.u.orb, x, y, z, dx, dy, dz);
-    case kTube: return Tube::dist_out(s.u.tube, x, y, z, dx, dy, dz);
-    case kCone: return Cone::dist_out(s.u.cone, x, y, z, dx, dy, dz);
-    default: return Trd::dist_out(s.u.trd, x, y, z, dx, dy, dz);
-    }
-}
-
-VG_DEV double solid_sdf(const SolidU &s, double x, double y, double z)
-{
-    switch (s.kind) {
-    case kBox: return Box::safety(s.u.box, x, y, z);
-    case kOrb: return Orb::safety(s.u.orb, x, y, z);
-    case kTube: return Tube::safety(s.u.tube, x, y, z);
-    case kCone: return Cone::safety(s.u.cone, x, y, z);
-    default: return Trd::safety(s.u.trd, x, y, z);
-    }
 }
 
 template <class S> struct Pick;

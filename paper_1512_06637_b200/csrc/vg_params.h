@@ -135,4 +135,14 @@ struct NavMeta {
     unsigned long long kmask[kNavKinds][kNavChunks]; // bit j of kmask[kind][c]: daughter 64 c + j is of that kind
 };
 
+// hierarchy of volumes (vg_world.cu): one record per node, plus the child lists as one int32 array
+struct WorldNode {
+    double G[12];   // world frame -> local frame, composed at create from the chain of placements
+    double X[12];   // parent's local frame -> local frame (the placement itself)
+    double bs[4];   // bounding sphere in the PARENT's local frame: centre, squared radius inflated by the rounding bound
+    double br;      // its radius (inflated), for the safety cull
+    SolidU s;
+    int parent, child0, nchild, pad; // children: child_list[child0 .. child0 + nchild), ascending node index
+};
+
 } // namespace vg

@@ -1,0 +1,162 @@
+// vg_world.cu -- queries over a tree of placed solids ("with hierarchical connections one can build the
+// whole detector"; PAPER.md:98 the particle "is transported to the border" and changes volume; SURVEY.md sec. 8(f) f3;
+// readings R22-R25 in DESIGN.md): Locate, Step (one-level ComputeStep in each track's own node + the node entered)
+// and the per-node safety.
+//
+// Design: one thread per track; the node table (vg_params.h WorldNode, ~0.5 KiB per node) stays in global memory and
+// is read through L1 (tracks of a warp sit in different nodes, so there is no table to share per CTA as in
+// vg_nav.cu).  Every child is first tested against its bounding sphere in the parent's frame -- a point test for
+// Locate, a ray test for Step, a lower bound |p - c| - r for the safety -- and only the survivors pay for the 3x4
+// transform and the solid's own code.  The spheres are inflated by the rounding bound of the test, so the cull can
+// only keep too many children: a culled child's DistanceToIn is +inf, its Inside is OUTSIDE and its SafetyToIn exceeds
+// the running minimum, i.e. results are identical to visiting every child.  Children are visited in ascending node
+// index, so the strict `<` scan is the tie-break of R13.
+#include "vg_kernels.cuh"
+#include "vg_solid.cuh"
+
+namespace vg {
+
+constexpr int kWorldBlock = 128;
+
+VG_DEV void xf_point(const double *m, double x, double y, double z, double &lx, double &ly, double &lz)
+{
+    lx = fma(m[0], x, fma(m[1], y, fma(m[2], z, m[3])));
+    ly = fma(m[4], x, fma(m[5], y, fma(m[6], z, m[7])));
+    lz = fma(m[8], x, fma(m[9], y, fma(m[10], z, m[11])));
+}
+
+VG_DEV void xf_dir(const double *m, double dx, double dy, double dz, double &lx, double &ly, double &lz)
+{
+    lx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
+    ly = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
+    lz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
+}
+
+__global__ void __launch_bounds__(kWorldBlock)
+    world_locate_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids, Tracks t, int64_t n,
+                        int32_t *__restrict__ out)
+{
+    pdl_launch_dependents();
+    pdl_wait();
+    const int64_t i = int64_t(blockIdx.x) * kWorldBlock + threadIdx.x;
+    if (i >= n) return;
+    double x, y, z;
+    xf_point(nodes[0].X, ldg1(t.x + i), ldg1(t.y + i), ldg1(t.z + i), x, y, z);
+    int cur = -1;
+    if (solid_inside(nodes[0].s, x, y, z) == cInside) {
+        cur = 0;
+        bool moved = true;
+        while (moved) {
+            moved = false;
+            const int c0 = nodes[cur].child0, nc = nodes[cur].nchild;
+#pragma unroll 1
+            for (int j = 0; j < nc; ++j) {
+                const int c = kids[c0 + j];
+                const WorldNode &C = nodes[c];
+                const double vx = x - C.bs[0], vy = y - C.bs[1], vz = z - C.bs[2];
+                if (!(fma(vx, vx, fma(vy, vy, vz * vz)) <= C.bs[3])) continue; // outside the child's bounding sphere
+                double lx, ly, lz;
+                xf_point(C.X, x, y, z, lx, ly, lz);
+                if (solid_inside(C.s, lx, ly, lz) == cInside) {
+                    cur = c;
+                    x = lx, y = ly, z = lz;
+                    moved = true;
+                    break;
+                }
+            }
+        }
+    }
+    stg1i(out + i, cur);
+}
+
+// kStep: Step (R24); else the per-node safety (R25)
+template <bool kStep>
+__global__ void __launch_bounds__(kWorldBlock)
+    world_node_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids, int nnodes,
+                      const int32_t *__restrict__ node, Tracks t, double step_max, int64_t n, double *__restrict__ out,
+                      int32_t *__restrict__ next)
+{
+    pdl_launch_dependents();
+    pdl_wait();
+    const int64_t i = int64_t(blockIdx.x) * kWorldBlock + threadIdx.x;
+    if (i >= n) return;
+    const int nd = node[i];
+    if (nd < 0 || nd >= nnodes) {
+        stg1(out + i, -1.0);
+        if (kStep) stg1i(next + i, -1);
+        return;
+    }
+    const WorldNode &N = nodes[nd];
+    double x, y, z, dx = 0, dy = 0, dz = 0;
+    xf_point(N.G, ldg1(t.x + i), ldg1(t.y + i), ldg1(t.z + i), x, y, z);
+    if (kStep) xf_dir(N.G, ldg1(t.dx + i), ldg1(t.dy + i), ldg1(t.dz + i), dx, dy, dz);
+    const int c0 = N.child0, nc = N.nchild;
+    if (kStep) {
+        double best = solid_dist_out(N.s, x, y, z, dx, dy, dz);
+        int who = N.parent;
+#pragma unroll 1
+        for (int j = 0; j < nc; ++j) {
+            const int c = kids[c0 + j];
+            const WorldNode &C = nodes[c];
+            // ray against the bounding sphere: closest approach of the line, and the sphere not behind the start
+            const double vx = C.bs[0] - x, vy = C.bs[1] - y, vz = C.bs[2] - z;
+            const double vv = fma(vx, vx, fma(vy, vy, vz * vz));
+            const double tca = fma(vx, dx, fma(vy, dy, vz * dz));
+            const double d2 = fma(-tca, tca, vv);
+            if (!(d2 <= C.bs[3] && (tca >= 0.0 || vv <= C.bs[3]))) continue;
+            double lx, ly, lz, ldx, ldy, ldz;
+            xf_point(C.X, x, y, z, lx, ly, lz);
+            xf_dir(C.X, dx, dy, dz, ldx, ldy, ldz);
+            const double tk = solid_dist_in(C.s, lx, ly, lz, ldx, ldy, ldz);
+            const bool take = tk >= 0.0 && tk < best; // ascending child index: the strict < is R13's tie-break
+            best = take ? tk : best;
+            who = take ? c : who;
+        }
+        const bool phys = best > step_max; // the physics step is shorter than the geometric one
+        stg1(out + i, phys ? step_max : best);
+        stg1i(next + i, phys ? nd : who);
+    } else {
+        double best = -solid_sdf(N.s, x, y, z);
+#pragma unroll 1
+        for (int j = 0; j < nc; ++j) {
+            const int c = kids[c0 + j];
+            const WorldNode &C = nodes[c];
+            // SafetyToIn of the child >= |p - c| - r: skip it when that bound already exceeds the running minimum
+            const double vx = x - C.bs[0], vy = y - C.bs[1], vz = z - C.bs[2];
+            const double vv = fma(vx, vx, fma(vy, vy, vz * vz));
+            const double reach = best + C.br;
+            if (reach > 0.0 && vv > reach * reach * (1.0 + 1e-9)) continue;
+            double lx, ly, lz;
+            xf_point(C.X, x, y, z, lx, ly, lz);
+            best = dmin(best, solid_sdf(C.s, lx, ly, lz));
+        }
+        stg1(out + i, best);
+    }
+}
+
+cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const Tracks &t, int64_t n, int32_t *out,
+                                cudaStream_t s)
+{
+    if (n <= 0) return cudaSuccess;
+    const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
+    return launch_kernel(world_locate_kernel, grid, kWorldBlock, 0, s, nodes, kids, t, n, out);
+}
+
+cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, int nnodes, const int32_t *node, const Tracks &t,
+                              double step_max, int64_t n, double *step, int32_t *next, cudaStream_t s)
+{
+    if (n <= 0) return cudaSuccess;
+    const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
+    return launch_kernel(world_node_kernel<true>, grid, kWorldBlock, 0, s, nodes, kids, nnodes, node, t, step_max, n, step, next);
+}
+
+cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, int nnodes, const int32_t *node, const Tracks &t,
+                                int64_t n, double *safety, cudaStream_t s)
+{
+    if (n <= 0) return cudaSuccess;
+    const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
+    int32_t *none = nullptr;
+    return launch_kernel(world_node_kernel<false>, grid, kWorldBlock, 0, s, nodes, kids, nnodes, node, t, 0.0, n, safety, none);
+}
+
+} // namespace vg

@@ -1,0 +1,119 @@
+"""GPU parity of the world queries (tree of placed solids; include/vg.h vg_world_*; readings R22-R25) against the
+oracle on the same seeded inputs: node indices bit-exact, steps and safeties within max(1e-9, 1e-12 |oracle|)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as O
+import workloads as W
+from parity import assert_int_equal, assert_real_close
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def vg():
+    import paper_1512_06637_b200 as vg
+    return vg
+
+
+def dev(arrs):
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrs]
+
+
+@pytest.fixture(scope="module")
+def worlds(vg):
+    wc = W.world_case()
+    so = [O.Shape(k, p) for k, p in zip(wc.kinds, wc.params)]
+    sg = [vg.Shape(k, p) for k, p in zip(wc.kinds, wc.params)]
+    wo = O.World(so, wc.parents, wc.xforms)
+    wg = vg.World(sg, wc.parents, wc.xforms)
+
+    def band(x, y, z):
+        nd = wo.locate(x, y, z)
+        return (nd < 0) | (wo.safety(nd, x, y, z) < W.SURFACE_BAND)
+
+    return wc, wo, wg, band
+
+
+@pytest.mark.parametrize("n", [1, 129, 20001, 300007])
+def test_locate_step_safety_match_the_oracle(vg, worlds, n):
+    wc, wo, wg, band = worlds
+    t = wc.tracks(n, band)
+    dt = dev(t)
+    node_o = wo.locate(*t[:3])
+    node_g = wg.locate(*dt[:3])
+    assert_int_equal(node_g.cpu().numpy(), node_o, "world locate n=%d" % n)
+    for step_max in (W.STEP_MAX, 7.5):
+        so, no = wo.step(node_o, *t, step_max)
+        sg, ng = wg.step(node_g, *dt, step_max)
+        assert_int_equal(ng.cpu().numpy(), no, "world step next n=%d" % n)
+        assert_real_close(sg.cpu().numpy(), so, "world step n=%d" % n)
+    assert_real_close(wg.safety(node_g, *dt[:3]).cpu().numpy(), wo.safety(node_o, *t[:3]), "world safety n=%d" % n)
+    if n > 1000:
+        depth = np.where(node_o == 0, 0, np.where(node_o <= 64, 1, 2))
+        assert len(set(depth.tolist())) == 3
+
+
+def test_points_outside_the_world_and_bad_nodes(vg, worlds):
+    wc, wo, wg, band = worlds
+    x, y, z, dx, dy, dz = W.draw_tracks(77, 50000, (0, 0, 0), (130, 130, 130))
+    keep = np.abs(wo.shapes[0].sdf(x, y, z)) > 1e-6
+    t = [a[keep] for a in (x, y, z, dx, dy, dz)]
+    node_o = wo.locate(*t[:3])
+    # keep clear of every surface below the root as well
+    ok = (node_o < 0) | (wo.safety(np.maximum(node_o, 0), *t[:3]) >= W.SURFACE_BAND)
+    t = [np.ascontiguousarray(a[ok]) for a in t]
+    node_o = node_o[ok]
+    assert (node_o < 0).any() and (node_o >= 0).any()
+    dt = dev(t)
+    node_g = wg.locate(*dt[:3])
+    assert_int_equal(node_g.cpu().numpy(), node_o, "locate incl. outside")
+    so, no = wo.step(node_o, *t)
+    sg, ng = wg.step(node_g, *dt)
+    assert_int_equal(ng.cpu().numpy(), no, "step next incl. outside")
+    assert_real_close(sg.cpu().numpy(), so, "step incl. outside")
+    bad = torch.full_like(node_g, 100000)
+    sg, ng = wg.step(bad, *dt)
+    assert bool((sg == -1).all()) and bool((ng == -1).all())
+    assert bool((wg.safety(bad, *dt[:3]) == -1).all())
+
+
+def test_walk_through_the_world(vg, worlds):
+    """Propagate tracks step by step on the GPU alone (step, move a hair beyond the border, take `next` as the new node) and
+    check every state against the oracle's Locate: the relocation of PAPER.md:98 done by vg_world_step itself."""
+    wc, wo, wg, band = worlds
+    t = wc.tracks(40000, band)
+    x, y, z, dx, dy, dz = dev(t)
+    node = wg.locate(x, y, z)
+    eps = 1e-6
+    agree = []
+    for _ in range(6):
+        step, nxt = wg.step(node, x, y, z, dx, dy, dz)
+        alive = nxt >= 0
+        x = torch.where(alive, x + (step + eps) * dx, x)
+        y = torch.where(alive, y + (step + eps) * dy, y)
+        z = torch.where(alive, z + (step + eps) * dz, z)
+        node = torch.where(alive, nxt, node)
+        loc = wo.locate(x.cpu().numpy(), y.cpu().numpy(), z.cpu().numpy())
+        a = alive.cpu().numpy()
+        agree.append((loc[a] == node.cpu().numpy()[a]).mean())
+    # grazing crossings (within eps of an edge, or a border closer than eps behind the new point) are the only disagreements
+    assert min(agree) > 0.995, agree
+
+
+def test_world_create_rejects_bad_input(vg):
+    b = vg.Shape(W.BOX, [1, 1, 1])
+    ident = [1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]
+    with pytest.raises(vg.VgError):
+        vg.World([b, b], [0, 0], [ident, ident])
+    with pytest.raises(vg.VgError):
+        vg.World([b, b], [-1, 1], [ident, ident])
+    with pytest.raises(vg.VgError):
+        vg.World([b, b], [-1, 0], [ident, [2, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]])
+    pc = vg.Shape(W.POLYCONE, W.polycone_params(1))
+    with pytest.raises(vg.VgError):
+        vg.World([b, pc], [-1, 0], [ident, ident])
+    w = vg.World([b], [-1], [ident])
+    x = torch.zeros(5, dtype=torch.float64, device="cuda")
+    assert w.locate(x, x, x).tolist() == [0] * 5
