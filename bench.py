@@ -33,6 +33,7 @@ UNIT = "track-queries/s"
 # algorithmic bytes per track: SoA inputs read once + one result written once
 BYTES = {"inside": 24 + 4, "safety_to_in": 24 + 8, "safety_to_out": 24 + 8, "distance_to_in": 48 + 8,
          "distance_to_out": 48 + 8, "compute_step": 48 + 12, "all": 48 + 4 + 4 * 8}
+BYTES.update({"world_locate": 24 + 4, "world_step": 48 + 4 + 8 + 4, "world_safety": 24 + 4 + 8})
 L2_BYTES = 126e6
 HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
 
@@ -115,10 +116,21 @@ class ClockSampler:
 class Case:
     """One solid (or the navigation volume) with its seeded tracks resident in HBM as `nsets` rotating copies."""
 
-    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None):
+    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None, world=None):
         self.vg, self.torch, self.name, self.n, self.queries = vg, torch, name, int(n), tuple(queries)
         dev = torch.device("cuda", torch.cuda.current_device())
-        if nav is not None:
+        self.nodes = None
+        if world is not None:
+            self.kind = "world"
+            shapes = [vg.Shape(k, p) for k, p in zip(world.kinds, world.params)]
+            self.handle = vg.World(shapes, world.parents, world.xforms)
+
+            def band(x, y, z):  # outside the world, or in the surface band of any node (library's own queries)
+                d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (x, y, z)]
+                nd = self.handle.locate(*d)
+                s = self.handle.safety(torch.clamp(nd, min=0), *d)
+                return ((nd < 0) | (s < W.SURFACE_BAND)).cpu().numpy()
+        elif nav is not None:
             self.kind = "navigator"
             mother = vg.Shape(nav.mother_kind, nav.mother_params)
             daughters = [vg.Shape(k, p) for k, p in zip(nav.daughter_kinds, nav.daughter_params)]
@@ -131,7 +143,7 @@ class Case:
             self.handle = vg.Shape(shape.kind, shape.params)
             seed, center, half = shape.seed + seed_shift, shape.center, shape.half
             band = lambda x, y, z: np.abs(self._gpu3(self.handle.safety_to_in, x, y, z)) < W.SURFACE_BAND
-        self.host = W.draw_tracks(seed, self.n, center, half, band)
+        self.host = world.tracks(self.n, band) if world is not None else W.draw_tracks(seed, self.n, center, half, band)
         per_set = 48 * self.n
         self.nsets = int(min(16, max(2, -(-int(4 * L2_BYTES) // per_set))))
         self.cold = self.nsets * per_set >= 2 * L2_BYTES
@@ -141,6 +153,8 @@ class Case:
         self.outi = [torch.empty(self.n, dtype=torch.int32, device=dev) for _ in range(self.nsets)]
         self.out4 = None  # four more result arrays per set, allocated on the first fused launch
         self.cursor = 0
+        if world is not None:  # the node of every track, as vg_world_locate returns it
+            self.nodes = [self.handle.locate(*st[:3]) for st in self.sets]
 
     def _gpu3(self, fn, x, y, z):
         t = self.torch
@@ -156,6 +170,14 @@ class Case:
             if self.out4 is None:
                 self.out4 = [[self.torch.empty_like(self.outd[0]) for _ in range(3)] for _ in range(self.nsets)]
             self.handle.query_all(*s, W.STEP_MAX, out=[self.outi[k], self.outd[k]] + self.out4[k])
+        elif q == "world_locate":
+            self.handle.locate(*s[:3], out=self.outi[k])
+        elif q == "world_step":
+            if self.out4 is None:
+                self.out4 = [self.torch.empty_like(self.outi[0]) for _ in range(self.nsets)]
+            self.handle.step(self.nodes[k], *s, step_max=W.STEP_MAX, step=self.outd[k], next=self.out4[k])
+        elif q == "world_safety":
+            self.handle.safety(self.nodes[k], *s[:3], out=self.outd[k])
         elif q == "compute_step":
             self.handle.compute_step(*s, step_max=W.STEP_MAX, step=self.outd[k], hit=self.outi[k])
         elif q == "inside":
@@ -338,6 +360,17 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
     e = roofline_entry("navigator", "compute_step", case.n, sec, hbm_peak, fma_rate)
     e.update({"config": 4, "shape": "box(100)+64 daughters", "query": "compute_step", "n": case.n, "cold_inputs": case.cold})
     rows.append(e)
+    del case
+    torch.cuda.empty_cache()
+    # the three-level tree of placed solids (193 nodes), every track in its own node
+    wc = W.world_case()
+    case = Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc)
+    for q in case.queries:
+        sec = time_query_alone(torch, case, q)
+        e = roofline_entry("world", q, case.n, sec, hbm_peak, fma_rate)
+        e.update({"config": "8(f) f3", "shape": "box(100) > 64 daughters > 128 grand-daughters", "query": q, "n": case.n,
+                  "cold_inputs": case.cold, "bound": "alu"})
+        rows.append(e)
     return rows
 
 
@@ -359,6 +392,8 @@ def run_profile(args):
             cases.append(Case(vg, torch, sc.name, min(sc.sizes[-1], 4194304), sc.queries, shape=sc))
     nav = W.navigator_case()
     cases.append(Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step",), nav=nav))
+    wc = W.world_case()
+    cases.append(Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc))
     torch.cuda.synchronize()
     torch.cuda.profiler.start()  # ncu --profile-from-start off: the set-up launches (surface-band rejection) are skipped
     for _ in range(args.steps):

@@ -437,7 +437,8 @@ extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const doubl
 
 struct vg_world {
     int nn;
-    WorldNode *nodes_dev; // one allocation: nn WorldNode records followed by the child lists (int32)
+    WorldNode *nodes_dev; // one allocation: nn WorldNode records, the FP32 cull spheres and the child lists (int32)
+    float4 *cull_dev;     // one float4 {cx, cy, cz, r2} per child-list entry, same order as kids_dev
     int32_t *kids_dev;
     int device;
 };
@@ -511,23 +512,38 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         N.bs[3] = r * r * (1.0 + 1e-9) + 1e-12 * S * S;
         N.br = std::sqrt(N.bs[3]);
     }
+    // the same spheres for the FP32 culls of Locate and Step, in child-list order; error bound as in vg_volume_create:
+    // the FP32 evaluation is off by < 30 u S^2 (u = 2^-24), so r^2 is inflated by 64 u S^2 on top of a relative 1e-6
+    std::vector<float> cull(4 * kids.size(), 0.f);
+    for (int p = 0; p < nn; ++p)
+        for (int j = 0; j < nodes[p].nchild; ++j) {
+            const WorldNode &N = nodes[kids[nodes[p].child0 + j]];
+            const double r = bounding_radius(N.s);
+            const double S = bounding_radius(nodes[p].s) + std::sqrt(N.bs[0] * N.bs[0] + N.bs[1] * N.bs[1] + N.bs[2] * N.bs[2]) + r;
+            const double r2 = r * r * (1.0 + 1e-6) + 64.0 * std::ldexp(1.0, -24) * S * S;
+            float *e = &cull[4 * size_t(nodes[p].child0 + j)];
+            e[0] = float(N.bs[0]), e[1] = float(N.bs[1]), e[2] = float(N.bs[2]), e[3] = std::nextafterf(float(r2), INFINITY);
+        }
     vg_world *w = new (std::nothrow) vg_world;
     if (!w) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
     std::memset(w, 0, sizeof *w);
     w->nn = nn;
-    const size_t nbytes = size_t(nn) * sizeof(WorldNode), kbytes = kids.size() * sizeof(int32_t);
+    const size_t nbytes = size_t(nn) * sizeof(WorldNode), cbytes = cull.size() * sizeof(float), kbytes = kids.size() * sizeof(int32_t);
+    static_assert(sizeof(WorldNode) % 16 == 0, "the float4 array follows the node records");
     unsigned char *blob = nullptr;
     cudaError_t e = cudaGetDevice(&w->device);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + kbytes);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + cbytes + kbytes);
     if (e == cudaSuccess) e = cudaMemcpy(blob, nodes.data(), nbytes, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes, kids.data(), kbytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes, cull.data(), cbytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes + cbytes, kids.data(), kbytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         if (blob) cudaFree(blob);
         delete w;
         return fail_cuda(e, fn);
     }
     w->nodes_dev = reinterpret_cast<WorldNode *>(blob);
-    w->kids_dev = reinterpret_cast<int32_t *>(blob + nbytes);
+    w->cull_dev = reinterpret_cast<float4 *>(blob + nbytes);
+    w->kids_dev = reinterpret_cast<int32_t *>(blob + nbytes + cbytes);
     *out = w;
     return VG_OK;
 }
@@ -549,7 +565,7 @@ extern "C" int vg_world_locate(const vg_world *w, const double *x, const double 
     int rc = check_arrays(fn, ptrs, 3, 4, node, n, &vec);
     if (rc != VG_OK || n == 0) return rc;
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
-    cudaError_t e = launch_world_locate(w->nodes_dev, w->kids_dev, t, n, node, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_world_locate(w->nodes_dev, w->kids_dev, w->cull_dev, t, n, node, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }
@@ -567,7 +583,7 @@ extern "C" int vg_world_step(const vg_world *w, const int32_t *node, const doubl
     if (!node || !aligned(node, 4) || !next || !aligned(next, 4)) return fail(VG_ERR_ARG, "%s: node / next array NULL or misaligned", fn);
     if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
     Tracks t{ x, y, z, dx, dy, dz };
-    cudaError_t e = launch_world_step(w->nodes_dev, w->kids_dev, w->nn, node, t, step_max, n, step, next,
+    cudaError_t e = launch_world_step(w->nodes_dev, w->kids_dev, w->cull_dev, w->nn, node, t, step_max, n, step, next,
                                       static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
@@ -584,7 +600,7 @@ extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const dou
     if (rc != VG_OK || n == 0) return rc;
     if (!node || !aligned(node, 4)) return fail(VG_ERR_ARG, "%s: node array NULL or misaligned", fn);
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
-    cudaError_t e = launch_world_safety(w->nodes_dev, w->kids_dev, w->nn, node, t, n, safety, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_world_safety(w->nodes_dev, w->kids_dev, w->cull_dev, w->nn, node, t, n, safety, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }

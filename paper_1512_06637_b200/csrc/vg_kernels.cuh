@@ -576,11 +576,11 @@ cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *tabl
                                  double *safety, cudaStream_t s);
 
 // hierarchy of volumes (vg_world.cu)
-cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const Tracks &t, int64_t n, int32_t *out,
+cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const float4 *cull, const Tracks &t, int64_t n, int32_t *out,
                                 cudaStream_t s);
-cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, int nnodes, const int32_t *node, const Tracks &t,
+cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
                               double step_max, int64_t n, double *step, int32_t *next, cudaStream_t s);
-cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, int nnodes, const int32_t *node, const Tracks &t,
+cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
                                 int64_t n, double *safety, cudaStream_t s);
 
 // probes (vg_probe.cu)

@@ -136,7 +136,7 @@ struct NavMeta {
 };
 
 // hierarchy of volumes (vg_world.cu): one record per node, plus the child lists as one int32 array
-struct WorldNode {
+struct alignas(16) WorldNode {
     double G[12];   // world frame -> local frame, composed at create from the chain of placements
     double X[12];   // parent's local frame -> local frame (the placement itself)
     double bs[4];   // bounding sphere in the PARENT's local frame: centre, squared radius inflated by the rounding bound

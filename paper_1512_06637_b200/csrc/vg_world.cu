@@ -7,10 +7,12 @@
 // is read through L1 (tracks of a warp sit in different nodes, so there is no table to share per CTA as in
 // vg_nav.cu).  Every child is first tested against its bounding sphere in the parent's frame -- a point test for
 // Locate, a ray test for Step, a lower bound |p - c| - r for the safety -- and only the survivors pay for the 3x4
-// transform and the solid's own code.  The spheres are inflated by the rounding bound of the test, so the cull can
-// only keep too many children: a culled child's DistanceToIn is +inf, its Inside is OUTSIDE and its SafetyToIn exceeds
-// the running minimum, i.e. results are identical to visiting every child.  Children are visited in ascending node
-// index, so the strict `<` scan is the tie-break of R13.
+// transform and the solid's own code.  Locate and Step run the test as in vg_nav.cu: phase 1 on the FP32 pipe over a
+// compact float4 array laid out like the child lists (64 children per 64-bit mask), phase 2 walks the mask in FP64.
+// The spheres are inflated by the rounding bound of the test, so the cull can only keep too many children: a culled
+// child's DistanceToIn is +inf, its Inside is OUTSIDE and its SafetyToIn exceeds the running minimum, i.e. results
+// are identical to visiting every child.  Children are visited in ascending node index, so the strict `<` scan is
+// the tie-break of R13.
 #include "vg_kernels.cuh"
 #include "vg_solid.cuh"
 
@@ -33,8 +35,8 @@ VG_DEV void xf_dir(const double *m, double dx, double dy, double dz, double &lx,
 }
 
 __global__ void __launch_bounds__(kWorldBlock)
-    world_locate_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids, Tracks t, int64_t n,
-                        int32_t *__restrict__ out)
+    world_locate_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids,
+                        const float4 *__restrict__ cull, Tracks t, int64_t n, int32_t *__restrict__ out)
 {
     pdl_launch_dependents();
     pdl_wait();
@@ -49,19 +51,28 @@ __global__ void __launch_bounds__(kWorldBlock)
         while (moved) {
             moved = false;
             const int c0 = nodes[cur].child0, nc = nodes[cur].nchild;
-#pragma unroll 1
-            for (int j = 0; j < nc; ++j) {
-                const int c = kids[c0 + j];
-                const WorldNode &C = nodes[c];
-                const double vx = x - C.bs[0], vy = y - C.bs[1], vz = z - C.bs[2];
-                if (!(fma(vx, vx, fma(vy, vy, vz * vz)) <= C.bs[3])) continue; // outside the child's bounding sphere
-                double lx, ly, lz;
-                xf_point(C.X, x, y, z, lx, ly, lz);
-                if (solid_inside(C.s, lx, ly, lz) == cInside) {
-                    cur = c;
-                    x = lx, y = ly, z = lz;
-                    moved = true;
-                    break;
+            const float xf = float(x), yf = float(y), zf = float(z);
+            for (int base = 0; base < nc && !moved; base += 64) {
+                const int lim = min(64, nc - base);
+                unsigned long long m = 0;
+#pragma unroll 4
+                for (int j = 0; j < lim; ++j) { // phase 1, FP32: inside the child's bounding sphere?
+                    const float4 sp = __ldg(cull + c0 + base + j);
+                    const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                    m |= (unsigned long long)(fmaf(vx, vx, fmaf(vy, vy, vz * vz)) <= sp.w) << j;
+                }
+                while (m) { // phase 2, FP64, ascending child index
+                    const int c = kids[c0 + base + __ffsll((long long)m) - 1];
+                    m &= m - 1;
+                    const WorldNode &C = nodes[c];
+                    double lx, ly, lz;
+                    xf_point(C.X, x, y, z, lx, ly, lz);
+                    if (solid_inside(C.s, lx, ly, lz) == cInside) {
+                        cur = c;
+                        x = lx, y = ly, z = lz;
+                        moved = true;
+                        break;
+                    }
                 }
             }
         }
@@ -72,8 +83,8 @@ __global__ void __launch_bounds__(kWorldBlock)
 // kStep: Step (R24); else the per-node safety (R25)
 template <bool kStep>
 __global__ void __launch_bounds__(kWorldBlock)
-    world_node_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids, int nnodes,
-                      const int32_t *__restrict__ node, Tracks t, double step_max, int64_t n, double *__restrict__ out,
+    world_node_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids,
+                      const float4 *__restrict__ cull, int nnodes, const int32_t *__restrict__ node, Tracks t, double step_max, int64_t n, double *__restrict__ out,
                       int32_t *__restrict__ next)
 {
     pdl_launch_dependents();
@@ -94,69 +105,93 @@ __global__ void __launch_bounds__(kWorldBlock)
     if (kStep) {
         double best = solid_dist_out(N.s, x, y, z, dx, dy, dz);
         int who = N.parent;
-#pragma unroll 1
-        for (int j = 0; j < nc; ++j) {
-            const int c = kids[c0 + j];
-            const WorldNode &C = nodes[c];
-            // ray against the bounding sphere: closest approach of the line, and the sphere not behind the start
-            const double vx = C.bs[0] - x, vy = C.bs[1] - y, vz = C.bs[2] - z;
-            const double vv = fma(vx, vx, fma(vy, vy, vz * vz));
-            const double tca = fma(vx, dx, fma(vy, dy, vz * dz));
-            const double d2 = fma(-tca, tca, vv);
-            if (!(d2 <= C.bs[3] && (tca >= 0.0 || vv <= C.bs[3]))) continue;
-            double lx, ly, lz, ldx, ldy, ldz;
-            xf_point(C.X, x, y, z, lx, ly, lz);
-            xf_dir(C.X, dx, dy, dz, ldx, ldy, ldz);
-            const double tk = solid_dist_in(C.s, lx, ly, lz, ldx, ldy, ldz);
-            const bool take = tk >= 0.0 && tk < best; // ascending child index: the strict < is R13's tie-break
-            best = take ? tk : best;
-            who = take ? c : who;
+        const float xf = float(x), yf = float(y), zf = float(z), dxf = float(dx), dyf = float(dy), dzf = float(dz);
+        for (int base = 0; base < nc; base += 64) {
+            const int lim = min(64, nc - base);
+            unsigned long long m = 0;
+#pragma unroll 4
+            for (int j = 0; j < lim; ++j) {
+                // phase 1, FP32: ray against the bounding sphere (closest approach of the line; sphere not behind the start)
+                const float4 sp = __ldg(cull + c0 + base + j);
+                const float vx = sp.x - xf, vy = sp.y - yf, vz = sp.z - zf;
+                const float vv = fmaf(vx, vx, fmaf(vy, vy, vz * vz));
+                const float tca = fmaf(vx, dxf, fmaf(vy, dyf, vz * dzf));
+                const float d2 = fmaf(-tca, tca, vv);
+                m |= (unsigned long long)(d2 <= sp.w && (tca >= 0.f || vv <= sp.w)) << j;
+            }
+            while (m) { // phase 2, FP64, ascending child index: the strict < is R13's tie-break
+                const int c = kids[c0 + base + __ffsll((long long)m) - 1];
+                m &= m - 1;
+                const WorldNode &C = nodes[c];
+                double lx, ly, lz, ldx, ldy, ldz;
+                xf_point(C.X, x, y, z, lx, ly, lz);
+                xf_dir(C.X, dx, dy, dz, ldx, ldy, ldz);
+                const double tk = solid_dist_in(C.s, lx, ly, lz, ldx, ldy, ldz);
+                const bool take = tk >= 0.0 && tk < best;
+                best = take ? tk : best;
+                who = take ? c : who;
+            }
         }
         const bool phys = best > step_max; // the physics step is shorter than the geometric one
         stg1(out + i, phys ? step_max : best);
         stg1i(next + i, phys ? nd : who);
     } else {
         double best = -solid_sdf(N.s, x, y, z);
-#pragma unroll 1
-        for (int j = 0; j < nc; ++j) {
-            const int c = kids[c0 + j];
-            const WorldNode &C = nodes[c];
-            // SafetyToIn of the child >= |p - c| - r: skip it when that bound already exceeds the running minimum
-            const double vx = x - C.bs[0], vy = y - C.bs[1], vz = z - C.bs[2];
-            const double vv = fma(vx, vx, fma(vy, vy, vz * vz));
-            const double reach = best + C.br;
-            if (reach > 0.0 && vv > reach * reach * (1.0 + 1e-9)) continue;
-            double lx, ly, lz;
-            xf_point(C.X, x, y, z, lx, ly, lz);
-            best = dmin(best, solid_sdf(C.s, lx, ly, lz));
+        // SafetyToIn of a child >= |p - c| - r.  Phase 1, FP32: children whose bound can undercut the node's own
+        // SafetyToOut (the spheres carry the FP32 error bound, see vg_world_create); a point outside its node (best <= 0)
+        // is outside every child, whose SafetyToIn is then positive and never the minimum.  Phase 2, FP64: the same
+        // bound against the running minimum, then the child's exact distance.
+        const float xf = float(x), yf = float(y), zf = float(z), bf = float(best);
+        for (int base = 0; base < nc && best > 0.0; base += 64) {
+            const int lim = min(64, nc - base);
+            unsigned long long m = 0;
+#pragma unroll 4
+            for (int j = 0; j < lim; ++j) {
+                const float4 sp = __ldg(cull + c0 + base + j);
+                const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                const float reach = bf + sqrtf(sp.w);
+                m |= (unsigned long long)(fmaf(vx, vx, fmaf(vy, vy, vz * vz)) <= reach * reach) << j;
+            }
+            while (m) {
+                const int c = kids[c0 + base + __ffsll((long long)m) - 1];
+                m &= m - 1;
+                const WorldNode &C = nodes[c];
+                const double vx = x - C.bs[0], vy = y - C.bs[1], vz = z - C.bs[2];
+                const double vv = fma(vx, vx, fma(vy, vy, vz * vz));
+                const double reach = best + C.br;
+                if (vv > reach * reach * (1.0 + 1e-9)) continue;
+                double lx, ly, lz;
+                xf_point(C.X, x, y, z, lx, ly, lz);
+                best = dmin(best, solid_sdf(C.s, lx, ly, lz));
+            }
         }
         stg1(out + i, best);
     }
 }
 
-cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const Tracks &t, int64_t n, int32_t *out,
+cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const float4 *cull, const Tracks &t, int64_t n, int32_t *out,
                                 cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
-    return launch_kernel(world_locate_kernel, grid, kWorldBlock, 0, s, nodes, kids, t, n, out);
+    return launch_kernel(world_locate_kernel, grid, kWorldBlock, 0, s, nodes, kids, cull, t, n, out);
 }
 
-cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, int nnodes, const int32_t *node, const Tracks &t,
+cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
                               double step_max, int64_t n, double *step, int32_t *next, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
-    return launch_kernel(world_node_kernel<true>, grid, kWorldBlock, 0, s, nodes, kids, nnodes, node, t, step_max, n, step, next);
+    return launch_kernel(world_node_kernel<true>, grid, kWorldBlock, 0, s, nodes, kids, cull, nnodes, node, t, step_max, n, step, next);
 }
 
-cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, int nnodes, const int32_t *node, const Tracks &t,
+cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
                                 int64_t n, double *safety, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
     int32_t *none = nullptr;
-    return launch_kernel(world_node_kernel<false>, grid, kWorldBlock, 0, s, nodes, kids, nnodes, node, t, 0.0, n, safety, none);
+    return launch_kernel(world_node_kernel<false>, grid, kWorldBlock, 0, s, nodes, kids, cull, nnodes, node, t, 0.0, n, safety, none);
 }
 
 } // namespace vg

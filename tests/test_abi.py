@@ -134,6 +134,15 @@ def test_compute_calls_fail_loudly_without_a_gpu():
     m = vg.Shape(vg.BOX, [10, 10, 10])
     with pytest.raises(vg.VgError):
         vg.Volume(m, [s], [[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]])  # needs device memory for the table
+    with pytest.raises(vg.VgError) as e:
+        vg.World([m, s], [-1, 0], [[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]] * 2)  # the node table as well
+    assert e.value.code == vg.ERR_CUDA
+    with pytest.raises(vg.VgError) as e:
+        vg.World([m, s], [0, 0], [[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]] * 2)  # validation comes before the device
+    assert e.value.code == vg.ERR_PARAM
+    # a full-phi polycone is created without its candidate grid (no device to hold it) and stays a valid handle
+    pc = vg.Shape(vg.POLYCONE, [0.0, 7.0, 3.0, -1.0, 0.0, 2.0, 0.0, 1.0, 3.0, 2.0, 0.0, 1.0])
+    assert lib.vg_shape_kind(pc._h) == vg.POLYCONE
 
 
 # ------------------------------------------------------------------------------------------ sharding (gloo)
