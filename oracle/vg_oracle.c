@@ -197,7 +197,7 @@ orc_shape *orc_shape_create(int kind, const double *par, int np)
             ok = 1;
         }
         break;
-    case ORC_POLYCONE: { /* sphi dphi nz (z rmin rmax)*nz : 2n-gon, c.1; reading R18 */
+    case ORC_POLYCONE: { /* sphi dphi nz (z rmin rmax)*nz : 2n-gon, c.1; readings R18, R26 */
         if (np < 3) break;
         int nz = (int)par[2];
         if ((double)nz != par[2] || nz < 2 || nz > ORC_MAXZ || np != 3 + 3 * nz || !(par[1] > 0)) break;
@@ -205,7 +205,16 @@ orc_shape *orc_shape_create(int kind, const double *par, int np)
         for (int i = 0; i < nz; ++i) {
             double z = par[3 + 3 * i], rmin = par[4 + 3 * i], rmax = par[5 + 3 * i];
             if (rmin < 0 || rmax <= rmin) ok = 0;
-            if (i > 0 && !(z > par[3 + 3 * (i - 1)])) ok = 0;
+            if (i > 0 && !(z >= par[3 + 3 * (i - 1)])) ok = 0;
+            if (i > 0 && z == par[3 + 3 * (i - 1)]) {
+                /* reading R26: two planes at the same z are a STEP, the radii jump there and the
+                 * outline gets a horizontal edge (an annular face).  Not at either end, not three planes at one z, and
+                 * the radial ranges on both sides must overlap, so that the outline stays a simple polygon. */
+                double rmin_p = par[4 + 3 * (i - 1)], rmax_p = par[5 + 3 * (i - 1)];
+                if (i == 1 || i == nz - 1) ok = 0;
+                if (i >= 2 && z == par[3 + 3 * (i - 2)]) ok = 0;
+                if (!((rmin_p > rmin ? rmin_p : rmin) < (rmax_p < rmax ? rmax_p : rmax))) ok = 0;
+            }
             /* (rmin_0,z_0) ... (rmin_{n-1},z_{n-1}), (rmax_{n-1},z_{n-1}) ... (rmax_0,z_0) */
             s->pr[i] = rmin; s->pz[i] = z;
             s->pr[2 * nz - 1 - i] = rmax; s->pz[2 * nz - 1 - i] = z;

@@ -53,6 +53,8 @@ def member(kind, par, x, y, z):
     rho = np.sqrt(x * x + y * y)
     ok = np.zeros(x.shape, dtype=bool)
     for (z0, z1, a0, b0, a1, b1) in secs:
+        if z1 == z0:  # a z step of a polycone (R26): no volume of its own
+            continue
         rlo = _lin(a0, a1, z, z0, z1)
         rhi = _lin(b0, b1, z, z0, z1)
         ok |= (z >= z0) & (z <= z1) & (rho >= rlo) & (rho <= rhi)
@@ -120,10 +122,10 @@ def patches(kind, par):
         return f
 
     for (z0, z1, a0, b0, a1, b1) in secs:
-        out.append(frustum(z0, z1, b0, b1))
+        out.append(frustum(z0, z1, b0, b1))  # for a z step (z0 == z1) this is the annular face between the two radii
         if a0 > 0 or a1 > 0:
             out.append(frustum(z0, z1, a0, a1))
-        if dphi < TWO_PI:
+        if dphi < TWO_PI and z1 > z0:
             out.append(face(sphi, z0, z1, a0, b0, a1, b1))
             out.append(face(sphi + dphi, z0, z1, a0, b0, a1, b1))
     z0, _, a0, b0, _, _ = secs[0]

@@ -21,6 +21,10 @@ CONE_SEG_P = [2.0, 6.0, 4.0, 12.0, 20.0, 0.3, 1.9 * PI]
 TRD_P = [5.0, 10.0, 7.0, 3.0, 15.0]
 PCON_P = W.polycone_params(W.config_seed(3, 0))
 PCON_SEG_P = [0.4, 1.2 * PI] + PCON_P[2:]
+# polycones with z steps (reading R26): radii jump at z = -4 (outwards, and the bore opens) and at z = 6 (inwards)
+PCON_STEP_P = [0.0, 2 * PI, 7, -12.0, 0.0, 6.0, -4.0, 1.0, 8.0, -4.0, 3.0, 12.0, 2.0, 2.0, 10.0, 6.0, 2.0, 11.0, 6.0, 0.0, 5.0,
+               14.0, 1.5, 4.0]
+PCON_STEP_SEG_P = [-0.7, 1.3 * PI] + PCON_STEP_P[2:]
 
 SHAPES = {
     "box": (O.BOX, [5.0, 5.0, 5.0]),
@@ -33,6 +37,8 @@ SHAPES = {
     "trd": (O.TRD, TRD_P),
     "polycone": (O.POLYCONE, PCON_P),
     "polycone_seg": (O.POLYCONE, PCON_SEG_P),
+    "polycone_step": (O.POLYCONE, PCON_STEP_P),
+    "polycone_step_seg": (O.POLYCONE, PCON_STEP_SEG_P),
 }
 
 
@@ -195,6 +201,36 @@ def test_three_plane_polycone_with_equal_radii_is_tube():
     pc = O.Shape(O.POLYCONE, [0, 4 * PI / 3, 3, -15, 5, 10, 2, 5, 10, 15, 5, 10])
     _, t = tracks_for("tube", 20000)
     _same(_five(pc, t), _five(tube, t))
+
+
+def test_stepped_polycone_of_two_cylinders_is_the_union_of_two_tubes():
+    """R26: a polycone whose radii jump at z = 0 is the union of two tubes that share the plane z = 0.  Outside the union
+    the distance to it is the smaller of the two tube distances (distance to a union of sets), DistanceToIn the smaller of
+    the two DistanceToIn (the first entry into either part), Inside the OR of the memberships."""
+    pc = O.Shape(O.POLYCONE, [0, 2 * PI, 4, -10, 2, 5, 0, 2, 5, 0, 3, 9, 6, 3, 9])
+    lo = O.Shape(O.TUBE, [2, 5, 5, 0, 2 * PI])   # z in [-10, 0] about z = -5
+    hi = O.Shape(O.TUBE, [3, 9, 3, 0, 2 * PI])   # z in [0, 6] about z = 3
+    x, y, z, dx, dy, dz = W.draw_tracks(21, 40000, (0, 0, -2), (13.5, 13.5, 12),
+                                        lambda x, y, z: np.abs(pc.sdf(x, y, z)) < W.SURFACE_BAND)
+    s_lo, s_hi = lo.sdf(x, y, z + 5), hi.sdf(x, y, z - 3)
+    out = (s_lo > 0) & (s_hi > 0)
+    assert 0.5 < out.mean() < 0.95
+    assert np.array_equal(pc.inside(x, y, z) == O.OUTSIDE, out)
+    assert np.max(np.abs(pc.sdf(x, y, z)[out] - np.minimum(s_lo, s_hi)[out])) < 1e-12
+    want = np.minimum(lo.distance_to_in(x, y, z + 5, dx, dy, dz), hi.distance_to_in(x, y, z - 3, dx, dy, dz))
+    got = pc.distance_to_in(x, y, z, dx, dy, dz)
+    fin = np.isfinite(want[out])
+    assert np.array_equal(np.isfinite(got[out]), fin) and 0.05 < fin.mean() < 0.9
+    assert np.max(np.abs(got[out][fin] - want[out][fin])) < 1e-11
+    # inside the union the way out passes through both parts: DistanceToOut >= the exit of the part the point is in
+    ins = ~out
+    t_part = np.where(s_lo < 0, lo.distance_to_out(x, y, z + 5, dx, dy, dz), hi.distance_to_out(x, y, z - 3, dx, dy, dz))
+    assert np.all(pc.distance_to_out(x, y, z, dx, dy, dz)[ins] >= t_part[ins] - 1e-11)
+    # a hand-worked point: (7, 0, -1) lies 1 below the step annulus 5 <= rho <= 9 at z = 0 and 2 outside the lower tube
+    assert abs(pc.sdf(7.0, 0.0, -1.0)[0] - 1.0) < 1e-15
+    assert pc.distance_to_in(7.0, 0.0, -1.0, 0.0, 0.0, 1.0)[0] == 1.0
+    assert pc.distance_to_in(7.0, 0.0, -1.0, -1.0, 0.0, 0.0)[0] == 2.0
+    assert pc.distance_to_out(4.0, 0.0, -1.0, 0.0, 0.0, 1.0)[0] == 7.0   # through the plane z = 0 into the upper part
 
 
 def test_orb_rotation_invariance():
@@ -410,7 +446,11 @@ def test_zero_direction_components_and_tangents():
 def test_invalid_parameters_are_rejected():
     bad = [(O.BOX, [5, 0, 5]), (O.BOX, [5, 5]), (O.ORB, [-1]), (O.TUBE, [10, 5, 15, 0, 1]), (O.TUBE, [5, 10, 15, 0, 0]),
            (O.CONE, [2, 6, 12, 4, 20, 0, 1]), (O.TRD, [5, 10, 7, 3, -1]), (O.POLYCONE, [0, 1, 1, 0, 1, 2]),
-           (O.POLYCONE, [0, 1, 2, 0, 1, 2, 0, 1, 2]), (O.BOX, [float("nan"), 1, 1])]
+           (O.POLYCONE, [0, 1, 2, 0, 1, 2, 0, 1, 2]), (O.BOX, [float("nan"), 1, 1]),
+           # z steps (R26): not at an end, not three planes at one z, radial ranges must overlap, z never decreases
+           (O.POLYCONE, [0, 7, 3, 0, 1, 2, 0, 1, 3, 5, 1, 3]), (O.POLYCONE, [0, 7, 3, 0, 1, 2, 5, 1, 3, 5, 1, 2]),
+           (O.POLYCONE, [0, 7, 5, 0, 1, 2, 3, 1, 2, 3, 1, 3, 3, 1, 4, 6, 1, 4]),
+           (O.POLYCONE, [0, 7, 4, 0, 1, 2, 3, 1, 2, 3, 2, 4, 6, 2, 4]), (O.POLYCONE, [0, 7, 3, 0, 1, 2, 3, 1, 2, 2, 1, 2])]
     for kind, par in bad:
         with pytest.raises(ValueError):
             O.Shape(kind, par)
