@@ -77,11 +77,16 @@ typedef enum {
  *   VG_CONE     [rmin1, rmax1, rmin2, rmax2, dz, sphi, dphi]  radii linear in z, index 1 at z=-dz, 2 at z=+dz
  *   VG_TRD      [dx1, dx2, dy1, dy2, dz]                   half-lengths, index 1 at z=-dz, 2 at z=+dz
  *   VG_POLYCONE [sphi, dphi, nz, z_0, rmin_0, rmax_0, ..., z_{nz-1}, rmin_{nz-1}, rmax_{nz-1}]
- *               radii linear between consecutive z-planes, z strictly increasing, 2 <= nz <= VG_MAX_ZPLANES
+ *               radii linear between consecutive z-planes, z non-decreasing, 2 <= nz <= VG_MAX_ZPLANES.  Two planes
+ *               at the same z are a STEP (reading R26): the radii jump there and the solid gets an
+ *               annular face at that z.  A step may not sit at the first or last plane, at most two planes share a z,
+ *               and the radial ranges on the two sides of a step must overlap.
  *   dphi >= 2 pi (as FP64) means the full revolution.
  * Validation (VG_ERR_PARAM): wrong nparams, non-finite values, lengths <= 0, rmin < 0, rmin >= rmax at any
- * plane, dphi <= 0, nz out of range or not an integer, z not strictly increasing.
- * On success *out receives a handle; derived constants are computed once here on the host.
+ * plane, dphi <= 0, nz out of range or not an integer, z decreasing, a z step that breaks the rules above.
+ * On success *out receives a handle; derived constants are computed once here on the host.  For a full-phi polycone
+ * the candidate grid of its safeties (DESIGN.md sec. 6.2, 65 KiB) is built here and placed on the CURRENT device if
+ * there is one; on another device, or without one at create time, the safeties run the ordered-walk kernel instead.
  */
 int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **out);
 void vg_shape_destroy(vg_shape *shape); /* NULL is allowed */

@@ -148,12 +148,17 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         for (int i = 0; i < nz; ++i) {
             if (!(zp[3 * i + 1] >= 0 && zp[3 * i + 2] > zp[3 * i + 1]))
                 return fail(VG_ERR_PARAM, "polycone: need 0 <= rmin < rmax at plane %d", i);
-            if (i > 0 && !(zp[3 * i] > zp[3 * (i - 1)]))
-                return fail(VG_ERR_PARAM, "polycone: z must be strictly increasing (plane %d)", i);
+            if (i > 0 && !(zp[3 * i] >= zp[3 * (i - 1)]))
+                return fail(VG_ERR_PARAM, "polycone: z must not decrease (plane %d)", i);
+            if (i > 0 && zp[3 * i] == zp[3 * (i - 1)]) { // a z step (reading R26)
+                if (i == 1 || i == nz - 1) return fail(VG_ERR_PARAM, "polycone: a z step at an end plane (plane %d)", i);
+                if (zp[3 * i] == zp[3 * (i - 2)]) return fail(VG_ERR_PARAM, "polycone: three planes at one z (plane %d)", i);
+                if (!(std::fmax(zp[3 * i + 1], zp[3 * i - 2]) < std::fmin(zp[3 * i + 2], zp[3 * i - 1])))
+                    return fail(VG_ERR_PARAM, "polycone: radial ranges on the two sides of the z step at plane %d do not overlap", i);
+            }
         }
         PolyconeP &c = s->u.pcon;
         std::memset(&c, 0, sizeof c);
-        c.nsec = nz - 1;
         c.w = make_wedge(p[0], p[1]);
         c.zlo = zp[0];
         c.zhi = zp[3 * (nz - 1)];
@@ -166,14 +171,30 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
             for (int i = 0; i < nz; ++i) rb = std::fmax(rb, zp[3 * i + 2]);
             c.rb2 = rb * rb * (1 + 2e-9);
         }
+        int ns = 0;
         for (int k = 0; k < nz - 1; ++k) {
             const double *a = zp + 3 * k, *b = zp + 3 * (k + 1);
-            c.sec[k].z0 = a[0];
-            c.sec[k].z1 = b[0];
-            c.sec[k].out = make_frustum(a[0], a[2], b[0], b[2]);
-            c.sec[k].in = make_frustum(a[0], a[1], b[0], b[1]);
-            if (a[1] > 0 || b[1] > 0) c.inner_mask |= 1u << k;
+            if (b[0] == a[0]) { // the step between the section just stored and the next one
+                PconStep &t = c.step[ns - 1];
+                t.z = a[0];
+                t.olo = std::fmin(a[2], b[2]), t.ohi = std::fmax(a[2], b[2]);
+                t.ilo = std::fmin(a[1], b[1]), t.ihi = std::fmax(a[1], b[1]);
+                t.oup = a[2] > b[2];
+                t.iup = a[1] < b[1];
+                if (!(t.ohi > t.olo)) t.olo = 1.0, t.ohi = -1.0; // no jump: an empty range no radius falls into
+                if (!(t.ihi > t.ilo)) t.ilo = 1.0, t.ihi = -1.0;
+                c.step_mask |= 1u << (ns - 1);
+                ++c.nstep;
+                continue;
+            }
+            c.sec[ns].z0 = a[0];
+            c.sec[ns].z1 = b[0];
+            c.sec[ns].out = make_frustum(a[0], a[2], b[0], b[2]);
+            c.sec[ns].in = make_frustum(a[0], a[1], b[0], b[1]);
+            if (a[1] > 0 || b[1] > 0) c.inner_mask |= 1u << ns;
+            ++ns;
         }
+        c.nsec = ns;
         return VG_OK;
     }
     }

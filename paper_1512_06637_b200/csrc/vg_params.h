@@ -65,20 +65,35 @@ struct PconSec {
     Frustum out, in;
 };
 
+// A z step (reading R26: two planes at one z): the radii jump between section k and section k + 1 and the outline has
+// a horizontal edge there, i.e. up to two annular faces at z: [olo, ohi] where the outer radius jumps and [ilo, ihi]
+// where the inner one does (an empty range, lo > hi, if that radius does not jump).  `oup` / `iup`: the material lies
+// BELOW the face (its outward normal is +z): rmax falls across the step / rmin rises across it.
+struct PconStep {
+    double z;
+    double olo, ohi, ilo, ihi;
+    int oup, iup;
+};
+
 struct PolyconeP {
-    int nsec;
+    int nsec;            // sections of non-zero length, in z order; consecutive sections share their boundary plane
     unsigned inner_mask; // bit k: section k has an inner surface (rmin_k > 0 || rmin_{k+1} > 0)
+    unsigned step_mask;  // bit k: the radii jump at the plane between section k and section k + 1 (step[k] is valid)
+    int nstep;
     Wedge w;
     double zlo, zhi;
     double cap_lo_rmin, cap_lo_rmax, cap_hi_rmin, cap_hi_rmax;
     double rb2; // square of the largest rmax, inflated by 1e-9 relative: bounding cylinder of the ordered walk
     PconSec sec[kMaxSec];
+    PconStep step[kMaxSec - 1];
 };
 
 // Candidate grid of a full-phi polycone (vg_pcon_grid.h): kPconGridZ x kPconGridR cells over
 // rho in [0, kPconGridR / inv_cr), z in [zg0, zg0 + kPconGridZ / inv_cz); one 64-bit mask of candidate segments per
 // cell (bit 0 / 1 = lower / upper cap, bit 2 + 2k = outer edge of section k, 3 + 2k = inner edge: up to 15 sections fit
-// the low word), one byte per z row with the section index at the row's lower edge.  Device memory owned by the vg_shape.
+// the low word; the faces of the j-th z step follow the sections at bits 2 + 2 nsec + 2j (outer) and + 1 (inner);
+// sections + steps <= 31, so 64 bits suffice), one byte per z row with the section index at the row's lower edge.
+// Device memory owned by the vg_shape.
 #ifndef VG_PCON_GRID_R
 #define VG_PCON_GRID_R 64
 #endif

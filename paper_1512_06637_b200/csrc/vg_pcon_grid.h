@@ -2,7 +2,7 @@
 // (SURVEY.md sec. 8(a) A0 "shape set-up"; the safeties are the exact signed distance of sec. 8(c) c.3).
 //
 // The exact distance from (rho, z) to the (r, z) outline is the minimum over its segments (outer and inner edge of
-// every section, the two end caps).  For a CELL of a regular (rho, z) grid only a few segments can be that minimum
+// every section, the two end caps, the annular faces of z steps).  For a CELL of a regular (rho, z) grid only a few segments can be that minimum
 // for any point of the cell: segment s is a candidate iff
 //     dmin_s(cell) <= min over s' of dmax_s'(cell)
 // (the nearest segment s* of a point p of the cell has d(p, s*) <= d(p, s') <= dmax_s' for every s', and
@@ -65,7 +65,8 @@ static inline bool pg_seg_meets_rect(const PconSegH &s, double u0, double u1, do
     return t0 <= t1;
 }
 
-// segment numbering shared with the kernel (vg_params.h): bits 0 / 1 = the caps, 2 + 2k / 3 + 2k = outer / inner edge of section k
+// segment numbering shared with the kernel (vg_params.h): bits 0 / 1 = the caps, 2 + 2k / 3 + 2k = outer / inner edge of
+// section k, then two bits per z step
 static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::vector<unsigned long long> *masks,
                                    std::vector<unsigned char> *rows)
 {
@@ -76,6 +77,13 @@ static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::
         segs.push_back(PconSegH{ s.out.r0, s.z0, s.out.r0 + s.out.er, s.z1, kPconSecBit0 + 2 * k });
         if ((c.inner_mask >> k) & 1u) segs.push_back(PconSegH{ s.in.r0, s.z0, s.in.r0 + s.in.er, s.z1, kPconSecBit0 + 2 * k + 1 });
         rmax = pg_max(rmax, pg_max(s.out.r0, s.out.r0 + s.out.er));
+    }
+    for (int k = 0, j = 0; k + 1 < c.nsec; ++k) { // the annular faces of the z steps (R26), bits after the sections
+        if (!((c.step_mask >> k) & 1u)) continue;
+        const PconStep &t = c.step[k];
+        const int bit = kPconSecBit0 + 2 * c.nsec + 2 * j++;
+        if (t.ohi > t.olo) segs.push_back(PconSegH{ t.olo, t.z, t.ohi, t.z, bit });
+        if (t.ihi > t.ilo) segs.push_back(PconSegH{ t.ilo, t.z, t.ihi, t.z, bit + 1 });
     }
     segs.push_back(PconSegH{ c.cap_lo_rmin, c.zlo, c.cap_lo_rmax, c.zlo, kPconCapLoBit });
     segs.push_back(PconSegH{ c.cap_hi_rmin, c.zhi, c.cap_hi_rmax, c.zhi, kPconCapHiBit });

@@ -63,6 +63,43 @@ VG_DEV void pcon_sections_of(const PolyconeP &p, double za, double zb, double zc
     }
 }
 
+// ---- z steps (reading R26).  Step k sits on the plane between section k and section k + 1; its constants are read from
+// the constant bank with a lane-dependent index, but only by the lanes whose walk reaches a step (step_mask is uniform).
+
+// is (rho^2, z) within kTol of an annular face of step k?  (such a point is on the surface, not inside)
+VG_DEV bool pcon_near_step(const PolyconeP &p, int k, double rho2, double z)
+{
+    if (k < 0 || k + 1 >= p.nsec || !((p.step_mask >> k) & 1u)) return false;
+    const PconStep &t = p.step[k];
+    const double rho = sqrt_nn(rho2);
+    return fabs(z - t.z) <= kTol && ((rho >= t.olo - kTol && rho <= t.ohi + kTol) || (rho >= t.ilo - kTol && rho <= t.ihi + kTol));
+}
+
+// entering crossing of the faces of step k by the ray, +inf if none; same tests as PolyconeT::cross(leaving = false)
+VG_DEV double pcon_step_enter(const PolyconeP &p, int k, const RayRZ &r, double z, double dz, double idz)
+{
+    if (k < 0 || k + 1 >= p.nsec || !((p.step_mask >> k) & 1u)) return inf();
+    const PconStep &st = p.step[k];
+    const double t = (st.z - z) * idz;
+    const double rh2 = fma(t, fma(t, r.a_xy, r.b_xy + r.b_xy), r.rho2);
+    const bool up = dz > 0.0;
+    const bool on_o = rh2 >= st.olo * st.olo && rh2 <= st.ohi * st.ohi && st.ohi > st.olo && (st.oup != 0) != up;
+    const bool on_i = rh2 >= st.ilo * st.ilo && rh2 <= st.ihi * st.ihi && st.ihi > st.ilo && (st.iup != 0) != up;
+    return (t > 0.0 && (on_o || on_i)) ? t : inf();
+}
+
+// squared distance from (u, v) to the horizontal edges of step k (the running minimum d2 goes in and comes out)
+VG_DEV double pcon_step_d2(const PolyconeP &p, int k, double u, double v, double d2)
+{
+    if (k < 0 || k + 1 >= p.nsec || !((p.step_mask >> k) & 1u)) return d2;
+    const PconStep &t = p.step[k];
+    const double vz = v - t.z, vz2 = vz * vz;
+    const double bo = dmax(dmax(t.olo - u, u - t.ohi), 0.0), bi = dmax(dmax(t.ilo - u, u - t.ihi), 0.0);
+    d2 = t.ohi > t.olo ? dmin(d2, fma(bo, bo, vz2)) : d2;
+    d2 = t.ihi > t.ilo ? dmin(d2, fma(bi, bi, vz2)) : d2;
+    return d2;
+}
+
 // DistanceToIn of the full-phi polycone; same candidates and validity tests as PolyconeT::dist_in
 VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z, double dx,
                                 double dy, double dz)
@@ -105,6 +142,7 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
         const double ri = fma(w.Bi, z, w.Ai) + kTol * w.seci;
         const bool inner = (p.inner_mask >> kz) & 1u;
         in = z > p.zlo + kTol && z < p.zhi - kTol && ro > 0.0 && r.rho2 < ro * ro && (!inner || ri < 0.0 || r.rho2 > ri * ri);
+        if (p.step_mask) in = in && !pcon_near_step(p, kz, r.rho2, z) && !pcon_near_step(p, kz - 1, r.rho2, z);
     }
 
     // a ray that starts beyond an end plane meets that cap before anything else
@@ -137,6 +175,10 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
         ok = ok && ((p.inner_mask >> k) & 1u) && zh >= w.z0 && zh <= w.z1;
         best = (ok && t < best) ? t : best;
         go = !(best < inf()) && k != kend;
+        if (go && p.step_mask) { // the step face on the plane the ray crosses next comes before anything of the next section
+            best = pcon_step_enter(p, up ? k : k - 1, r, z, dz, idz);
+            go = !(best < inf());
+        }
         k += step;
     }
     return in ? -1.0 : best;
@@ -164,6 +206,7 @@ VG_DEV double pcon_walk_sdf(const PolyconeP &p, const PconWalkSec *tab, double x
         d2 = dmin(d2, seg_d2(rho, z, w.ro0, w.z0, w.ero, ez, w.ilo));
         const double di = seg_d2(rho, z, w.ri0, w.z0, w.eri, ez, w.ili);
         d2 = ((p.inner_mask >> k) & 1u) ? dmin(d2, di) : d2;
+        if (p.step_mask) d2 = pcon_step_d2(p, k, rho, z, d2); // the step on top of section k (never nearer than the section's slab)
     }
     for (int k = kz - 1; k >= 0; --k) { // downwards
         const PconWalkSec w = tab[k];
@@ -173,6 +216,7 @@ VG_DEV double pcon_walk_sdf(const PolyconeP &p, const PconWalkSec *tab, double x
         d2 = dmin(d2, seg_d2(rho, z, w.ro0, w.z0, w.ero, ez, w.ilo));
         const double di = seg_d2(rho, z, w.ri0, w.z0, w.eri, ez, w.ili);
         d2 = ((p.inner_mask >> k) & 1u) ? dmin(d2, di) : d2;
+        if (p.step_mask) d2 = pcon_step_d2(p, k, rho, z, d2);
     }
     const double dist = sqrt_nn(d2);
     return in2d ? -dist : dist;
@@ -194,6 +238,17 @@ VG_DEV void pcon_stage_segs(const PolyconeP &p, double *seg)
             const PconSec &c = p.sec[k];
             const Frustum &f = (s & 1) ? c.in : c.out;
             r0 = f.r0, z0 = c.z0, er = f.er, ez = c.z1 - c.z0, il = f.inv_l2;
+        }
+        const int js = s - kPconSecBit0 - 2 * p.nsec; // >= 0: face (js & 1 ? inner : outer) of the (js >> 1)-th z step
+        if (js >= 0 && (js >> 1) < p.nstep) {
+            int kk = -1;
+            for (int q = 0, seen = 0; q + 1 < p.nsec; ++q)
+                if ((p.step_mask >> q) & 1u) {
+                    if (seen++ == (js >> 1)) kk = q;
+                }
+            const PconStep &t = p.step[kk];
+            const double lo = (js & 1) ? t.ilo : t.olo, hi = (js & 1) ? t.ihi : t.ohi;
+            if (hi > lo) r0 = lo, z0 = t.z, er = hi - lo, ez = 0.0, il = 1.0 / (er * er);
         }
         if (s == kPconCapLoBit) r0 = p.cap_lo_rmin, z0 = p.zlo, er = p.cap_lo_rmax - p.cap_lo_rmin, il = 1.0 / (er * er);
         if (s == kPconCapHiBit) r0 = p.cap_hi_rmin, z0 = p.zhi, er = p.cap_hi_rmax - p.cap_hi_rmin, il = 1.0 / (er * er);

@@ -91,7 +91,8 @@ VG_DEV double seg_d2(double u, double v, double r0, double z0, double er, double
 // Returns NaN/inf garbage when D <= 0; the caller tests D > 0.
 VG_DEV double quad_root(double a, double b, double c, double s, bool leaving)
 {
-    bool bpos = b >= 0.0;
+    bool bpos = not_neg(b); // the SIGN BIT, as copysign_bits reads it: b = -0.0 (a point on the axis of a cylinder) must
+                            // take the same branch here and there, or the two roots swap and the hit is lost
     double q = -(b + copysign_bits(s, b));
     // bpos: q = -(b+s): (-b - s)/a = q/a, (-b + s)/a = c/q.   !bpos: q = -b + s: (-b + s)/a = q/a, (-b - s)/a = c/q
     bool use_qa = (bpos != leaving);
@@ -675,6 +676,14 @@ template <int F> struct PolyconeT {
         }
         in = any_in && z > p.zlo + kTol && z < p.zhi - kTol;
         out = !any_near;
+        // z steps (R26): within kTol of an annular step face the point is on the surface, whatever the sections say
+#pragma unroll 1
+        for (int k = 0; k + 1 < p.nsec; ++k) {
+            if (!((p.step_mask >> k) & 1u)) continue;
+            const PconStep &t = p.step[k];
+            bool near_face = (rho >= t.olo - kTol && rho <= t.ohi + kTol) || (rho >= t.ilo - kTol && rho <= t.ihi + kTol);
+            in = in && !(fabs(z - t.z) <= kTol && near_face);
+        }
         if (!full(p)) wedge_classify<WM>(p.w, wedge_eval(p.w, x, y), rho2, in, out);
     }
     VG_DEV static int inside(const P &p, double x, double y, double z)
@@ -695,6 +704,13 @@ template <int F> struct PolyconeT {
             d2 = dmin(d2, seg_d2(u, v, s.out.r0, s.z0, s.out.er, ez, s.out.inv_l2));
             double di = seg_d2(u, v, s.in.r0, s.z0, s.in.er, ez, s.in.inv_l2);
             d2 = (has_inner(p, k) || axis) ? dmin(d2, di) : d2;
+            if ((p.step_mask >> k) & 1u) { // the horizontal edges of the z step above this section (empty ranges: lo > hi)
+                const PconStep &t = p.step[k];
+                double vz = v - t.z, vz2 = vz * vz;
+                double bo = dmax(dmax(t.olo - u, u - t.ohi), 0.0), bi = dmax(dmax(t.ilo - u, u - t.ihi), 0.0);
+                d2 = t.ohi > t.olo ? dmin(d2, fma(bo, bo, vz2)) : d2;
+                d2 = t.ihi > t.ilo ? dmin(d2, fma(bi, bi, vz2)) : d2;
+            }
         }
         return d2;
     }
@@ -749,8 +765,23 @@ template <int F> struct PolyconeT {
                 best = (ok && t < best) ? t : best;
             }
         }
+        double idz = rcp(dz); // NaN for dz = 0: caps and step faces rejected
+        // z steps (R26): annular faces at internal planes; a face whose material lies below (normal +z) is entered going
+        // down and left going up, and the other way round
+#pragma unroll 1
+        for (int k = 0; k + 1 < p.nsec; ++k) {
+            if (!((p.step_mask >> k) & 1u)) continue;
+            const PconStep &st = p.step[k];
+            double t = (st.z - z) * idz;
+            double rh2 = fma(t, fma(t, r.a_xy, r.b_xy + r.b_xy), r.rho2);
+            bool up = dz > 0.0;
+            bool on_o = rh2 >= st.olo * st.olo && rh2 <= st.ohi * st.ohi && st.ohi > st.olo && (leaving ? (st.oup != 0) == up : (st.oup != 0) != up);
+            bool on_i = rh2 >= st.ilo * st.ilo && rh2 <= st.ihi * st.ihi && st.ihi > st.ilo && (leaving ? (st.iup != 0) == up : (st.iup != 0) != up);
+            bool ok = t > 0.0 && (on_o || on_i);
+            if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
+            best = (ok && t < best) ? t : best;
+        }
         // end caps: entering from beyond, leaving from within
-        double idz = rcp(dz); // NaN for dz = 0: both caps rejected
         {
             double t = (p.zlo - z) * idz;
             double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);

@@ -80,6 +80,10 @@ SHAPES = {
     "cone": (W.CONE, [2.0, 6.0, 4.0, 12.0, 20.0, 0.0, TWO_PI]),
     "trd": (W.TRD, [5.0, 10.0, 7.0, 3.0, 15.0]),
     "polycone": (W.POLYCONE, W.polycone_params(W.config_seed(3, 0))),
+    # cylindrical patches (B = 0) seen from the axis: b = -0.0 in the quadratic (the root selection reads the sign bit)
+    "cone_cylinder": (W.CONE, [3.0, 8.0, 3.0, 8.0, 10.0, 0.0, TWO_PI]),
+    "polycone_step": (W.POLYCONE, [0.0, TWO_PI, 7.0, -12.0, 0.0, 6.0, -4.0, 1.0, 8.0, -4.0, 3.0, 12.0, 2.0, 2.0, 10.0, 6.0, 2.0, 11.0,
+                                   6.0, 0.0, 5.0, 14.0, 1.5, 4.0]),
 }
 
 

@@ -223,6 +223,13 @@ VARIANTS = [
     ("polycone_wedge", W.POLYCONE, [0.5, 4.0, 4.0, -10.0, 1.0, 5.0, -2.0, 2.0, 9.0, 3.0, 0.0, 6.0, 12.0, 3.0, 4.0]),
     ("polycone_solid", W.POLYCONE, [0.0, TWO_PI, 3.0, -10.0, 0.0, 5.0, 0.0, 0.0, 9.0, 8.0, 0.0, 2.0]),
     ("polycone_narrow", W.POLYCONE, [-1.0, 1.2, 3.0, -10.0, 0.0, 5.0, 0.0, 0.0, 9.0, 8.0, 3.0, 4.0]),
+    # z steps (reading R26): radii jump at z = -4 (outwards, the bore opens) and at z = 6 (inwards, the bore closes)
+    ("polycone_step", W.POLYCONE, [0.0, TWO_PI, 7.0, -12.0, 0.0, 6.0, -4.0, 1.0, 8.0, -4.0, 3.0, 12.0, 2.0, 2.0, 10.0, 6.0, 2.0, 11.0,
+                                   6.0, 0.0, 5.0, 14.0, 1.5, 4.0]),
+    ("polycone_step_wedge", W.POLYCONE, [-0.7, 4.1, 7.0, -12.0, 0.0, 6.0, -4.0, 1.0, 8.0, -4.0, 3.0, 12.0, 2.0, 2.0, 10.0, 6.0, 2.0,
+                                         11.0, 6.0, 0.0, 5.0, 14.0, 1.5, 4.0]),
+    ("polycone_two_tubes", W.POLYCONE, [0.0, TWO_PI, 4.0, -10.0, 2.0, 5.0, 0.0, 2.0, 5.0, 0.0, 3.0, 9.0, 6.0, 3.0, 9.0]),
+    ("polycone_step_outer_only", W.POLYCONE, [0.0, TWO_PI, 4.0, -10.0, 0.0, 9.0, 0.0, 0.0, 9.0, 0.0, 0.0, 4.0, 6.0, 0.0, 4.0]),
 ]
 
 
@@ -257,6 +264,15 @@ def _random_params(kind, rng):
     for i in range(nz):
         a = float(rng.choice([0.0, rng.uniform(0.0, 5.0)]))
         out += [float(z[i]), a, a + float(rng.uniform(0.5, 20.0))]
+    # every other polycone gets z steps (R26): an interior plane is duplicated with new radii that overlap the old range
+    if nz >= 3 and rng.random() < 0.5:
+        for i in sorted(rng.choice(np.arange(1, nz - 1), size=min(2, nz - 2), replace=False), reverse=True):
+            zi, a, b = out[3 + 3 * i: 6 + 3 * i]
+            mid = 0.5 * (a + b)
+            a2 = float(rng.choice([0.0, rng.uniform(0.0, mid)]))
+            b2 = mid + float(rng.uniform(0.2, 15.0))
+            out[6 + 3 * i: 6 + 3 * i] = [zi, a2 if a2 < mid else 0.0, b2]
+            out[2] += 1.0
     return out
 
 
