@@ -275,6 +275,92 @@ def cpu_baseline(seconds=10.0):
                       "gcc -O2 -ffp-contract=off, OpenMP static)" % (reps, len(t[0]), el)}
 
 
+# ---- the paper's own measurement (Fig. 4): DistanceToOut on a Box and a Tube, particles placed at
+# random INSIDE the body "escaping" from it, N = 10^3, 10^4, 10^5 on the x axis, every point repeated many times, speed
+# relative to a serial CPU code.  The figure's values did not survive the text extraction, so this is the
+# same protocol measured here, not a comparison with the paper's curve.
+
+FIG4_N = (1000, 10000, 100000)
+
+
+def fig4_cases():
+    box, tube = W.shape_cases(0)[0], W.shape_cases(1)[0]
+    return [("box", box.kind, box.params, (0, 0, 0), tuple(box.params)),
+            ("tube", tube.kind, tube.params, (0, 0, 0), (tube.params[1], tube.params[1], tube.params[2]))]
+
+
+def fig4_cpu(seconds_per_point=0.25):
+    """Serial-CPU leg of the Fig. 4 protocol: the oracle on ONE thread (part of the cpu_baseline object)."""
+    import oracle as O
+    nthreads = O.num_threads()
+    O.set_num_threads(1)
+    rows = []
+    try:
+        for name, kind, par, c, h in fig4_cases():
+            s = O.Shape(kind, par)
+            for n in FIG4_N:
+                t = W.draw_tracks(W.config_seed(9) + n, n, c, h, lambda x, y, z: s.sdf(x, y, z) > -W.SURFACE_BAND)
+                s.distance_to_out(*t, W.STEP_MAX)
+                reps, t0 = 0, time.perf_counter()
+                while True:
+                    s.distance_to_out(*t, W.STEP_MAX)
+                    reps += 1
+                    el = time.perf_counter() - t0
+                    if el >= seconds_per_point:
+                        break
+                rows.append({"shape": name, "n": n, "us_per_call": el * 1e6 / reps, "threads": 1})
+    finally:
+        O.set_num_threads(nthreads)
+    return rows
+
+
+def fig4_gpu(vg, torch, reps=5000):
+    """GPU legs: device-resident tracks, `reps` back-to-back launches as one CUDA graph (the paper repeated every point
+    5000 times on the same particles: a hot-cache number by construction); and the host-fed call (pinned host arrays in,
+    pinned result out) that includes both transfers, which is what the paper's GPU curve paid at small N."""
+    rows = []
+    for name, kind, par, c, h in fig4_cases():
+        sg = vg.Shape(kind, par)
+
+        def outside(x, y, z):
+            d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (x, y, z)]
+            return (sg.safety_to_in(*d) > -W.SURFACE_BAND).cpu().numpy()
+
+        for n in FIG4_N:
+            host = W.draw_tracks(W.config_seed(9) + n, n, c, h, outside)
+            dev = [torch.from_numpy(a).cuda() for a in host]
+            out = torch.empty(n, dtype=torch.float64, device="cuda")
+            sg.distance_to_out(*dev, W.STEP_MAX, out=out)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            per_graph = 100
+            with torch.cuda.graph(g):
+                for _ in range(per_graph):
+                    sg.distance_to_out(*dev, W.STEP_MAX, out=out)
+            g.replay()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(reps // per_graph):
+                g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            us_dev = e0.elapsed_time(e1) * 1e3 / (reps // per_graph * per_graph)
+            assert bool((out > 0).all()), "Fig. 4 protocol: every particle starts inside and escapes"
+            hp = [torch.from_numpy(a).pin_memory() for a in host]
+            hout = torch.empty(n, dtype=torch.float64).pin_memory()
+            for _ in range(5):
+                sg.query_host("distance_to_out", *hp, step_max=W.STEP_MAX, out=hout)
+            k, w0 = 200, time.perf_counter()
+            for _ in range(k):
+                sg.query_host("distance_to_out", *hp, step_max=W.STEP_MAX, out=hout)
+            us_host = (time.perf_counter() - w0) * 1e6 / k
+            rows.append({"shape": name, "query": "distance_to_out", "n": n, "repetitions": reps // per_graph * per_graph,
+                         "device_resident_us_per_launch": us_dev, "device_resident_tracks_per_s": n / us_dev * 1e6,
+                         "host_fed_us_per_call": us_host, "host_fed_tracks_per_s": n / us_host * 1e6})
+    return rows
+
+
 def run_reference(args, rank):
     """--impl reference: the oracle on the host cores, same config / metric / unit (rank 0 only)."""
     if rank != 0:
@@ -515,9 +601,10 @@ def run_ours(args, rank, world, local_rank):
                                        "h2d_bytes_per_step": h2d5, "d2h_bytes_per_step": d2h, "api": "vg_query_host x5"}}
 
     launches_per_step = nq
-    detail = None
+    detail, fig4 = None, None
     if world == 1 and not args.no_detail:
         detail = detail_sweep(vg, torch, hbm_peak, fma_rate, case)
+        fig4 = fig4_gpu(vg, torch)
     load1 = time.time()
     sampler.stop()
     clocks = sampler.summary(t0, t1, load0, load1)
@@ -540,6 +627,17 @@ def run_ours(args, rank, world, local_rank):
                               "how": "register-resident DFMA chains, vg_probe_fp64_fma_rate, same run"}}
         if world == 1:
             line["cpu_baseline"] = cpu_baseline()
+            if fig4 is not None:  # the serial-CPU leg of the Fig. 4 protocol and the speed relative to it
+                cpu4 = fig4_cpu()
+                line["cpu_baseline"]["fig4_serial"] = cpu4
+                ref = {(r["shape"], r["n"]): r["us_per_call"] for r in cpu4}
+                for r in fig4:
+                    r["serial_oracle_us_per_call"] = ref[(r["shape"], r["n"])]
+                    r["speedup_device_resident"] = r["serial_oracle_us_per_call"] / r["device_resident_us_per_launch"]
+                    r["speedup_host_fed"] = r["serial_oracle_us_per_call"] / r["host_fed_us_per_call"]
+                line["fig4_protocol"] = {"what": "PAPER.md:120-136 (Fig. 4): DistanceToOut, Box and Tube, particles inside the body, "
+                                                 "speed relative to a serial CPU code (here: the oracle on one thread; the paper's "
+                                                 "own curve is not in the text, BASELINE.md)", "rows": fig4}
         if detail is not None:
             line["detail"] = detail
         print(json.dumps(line), flush=True)
