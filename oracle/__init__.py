@@ -37,6 +37,14 @@ def _load(path):
     lib.orc_cross.argtypes = [C.c_void_p, _P, _P, _P, _P, _P, _P, C.c_int64, _P]
     lib.orc_compute_step.argtypes = [C.c_void_p, _P, _P, _P, _P, _P, _P, C.c_double, C.c_int64, _P, _PI]
     lib.orc_volume_safety.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _P]
+    lib.orc_boolean_create.restype = C.c_void_p
+    lib.orc_boolean_create.argtypes = [C.c_int, C.c_void_p, C.c_void_p, _P]
+    lib.orc_boolean_destroy.argtypes = [C.c_void_p]
+    lib.orc_boolean_inside.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _PI]
+    lib.orc_boolean_sdf.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _P]
+    lib.orc_boolean_distance.argtypes = [C.c_void_p, C.c_int, _P, _P, _P, _P, _P, _P, C.c_double, C.c_int64, _P]
+    lib.orc_all_crossings.restype = C.c_int
+    lib.orc_all_crossings.argtypes = [C.c_void_p] + [C.c_double] * 6 + [_P, C.c_int]
     lib.orc_world_create.restype = C.c_void_p
     lib.orc_world_create.argtypes = [C.c_int, C.POINTER(C.c_void_p), _PI, _P]
     lib.orc_world_destroy.argtypes = [C.c_void_p]
@@ -133,6 +141,12 @@ class Shape:
     def cross(self, x, y, z, dx, dy, dz):
         return self._f6(self._l.orc_cross, x, y, z, dx, dy, dz)
 
+    def all_crossings(self, p, d):
+        """Every crossing t > 0 of the boundary by the ray p + t d, ascending (one track)."""
+        out = np.empty(512, dtype=np.float64)
+        n = self._l.orc_all_crossings(self._h, *[float(v) for v in p], *[float(v) for v in d], _ptr(out), out.size)
+        return out[:n].copy()
+
 
 class Volume:
     """Mother solid + placed daughters; `xforms` is (nd, 12) row-major [R | b], mother -> local."""
@@ -165,6 +179,58 @@ class Volume:
         out = np.empty_like(x)
         self._l.orc_volume_safety(self._h, _ptr(x), _ptr(y), _ptr(z), x.size, _ptr(out))
         return out
+
+
+UNION, INTERSECTION, SUBTRACTION = 0, 1, 2
+
+
+class Boolean:
+    """C = A op B (readings R27-R29, vg_oracle.c): `xform` is the row-major 3x4 [R | b] from the frame of C (= of A)
+    to the frame of B.  Same query names as Shape; the safeties are the composed bound of R29."""
+
+    def __init__(self, op, a, b, xform):
+        self._l = a._l
+        self.op, self.a, self.b = int(op), a, b
+        self.xform = np.ascontiguousarray(np.asarray(xform, dtype=np.float64).reshape(12))
+        self._h = self._l.orc_boolean_create(self.op, a._h, b._h, _ptr(self.xform))
+        if not self._h:
+            raise ValueError("oracle: invalid boolean")
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            self._l.orc_boolean_destroy(self._h)
+            self._h = None
+
+    def inside(self, x, y, z):
+        x, y, z = map(_arr, (x, y, z))
+        out = np.empty(x.shape, dtype=np.int32)
+        self._l.orc_boolean_inside(self._h, _ptr(x), _ptr(y), _ptr(z), x.size, out.ctypes.data_as(_PI))
+        return out
+
+    def sdf(self, x, y, z):
+        x, y, z = map(_arr, (x, y, z))
+        out = np.empty_like(x)
+        self._l.orc_boolean_sdf(self._h, _ptr(x), _ptr(y), _ptr(z), x.size, _ptr(out))
+        return out
+
+    def safety_to_in(self, x, y, z):
+        return self.sdf(x, y, z)
+
+    def safety_to_out(self, x, y, z):
+        return -self.sdf(x, y, z)
+
+    def _dist(self, which, x, y, z, dx, dy, dz, step_max):
+        x, y, z, dx, dy, dz = map(_arr, (x, y, z, dx, dy, dz))
+        out = np.empty_like(x)
+        self._l.orc_boolean_distance(self._h, which, _ptr(x), _ptr(y), _ptr(z), _ptr(dx), _ptr(dy), _ptr(dz),
+                                     float(step_max), x.size, _ptr(out))
+        return out
+
+    def distance_to_in(self, x, y, z, dx, dy, dz, step_max=np.inf):
+        return self._dist(0, x, y, z, dx, dy, dz, step_max)
+
+    def distance_to_out(self, x, y, z, dx, dy, dz, step_max=np.inf):
+        return self._dist(1, x, y, z, dx, dy, dz, step_max)
 
 
 class World:

@@ -11,7 +11,8 @@
  * border against the physics step; "coordinate transformations and distance
  * calculations"), and the same step in a tree of placed volumes with the
  * point location that goes with it ("hierarchical connections";
- * readings R22-R25 at the end of this file).
+ * readings R22-R25 at the end of this file), and boolean solids of two
+ * primitives (readings R27-R29 at the end of this file).
  *
  * The paper gives no formula for any solid.  Every query here is the PLAIN
  * DEFINITION written out as brute force over the boundary patches of the
@@ -36,7 +37,10 @@
  * (trd==box, cone==tube, polycone==cone==tube, inserted collinear z-plane),
  * rigid-motion and permutation invariance of the navigation step, the world
  * queries against per-node membership / one-level steps composed in numpy and
- * against marching through orc_world_locate (tests/test_oracle_world.py), and
+ * against marching through orc_world_locate (tests/test_oracle_world.py), the
+ * boolean solids against set-definition membership, ray marching, reductions
+ * to one primitive and the never-over-estimating property of their composed
+ * safety (tests/test_oracle_boolean.py), and
  * the 80-bit long-double build of this same file (-DORC_LONG_DOUBLE).
  * Parity unpinned: nothing under readings R1-R21; behaviour INSIDE the
  * kTol surface band (R7) is outside the parity contract.
@@ -813,4 +817,225 @@ void orc_world_safety(const orc_world *w, const int32_t *node, const double *x, 
         }
         out[i] = (double)best;
     }
+}
+
+/* ------------------------------------------------------- boolean solids */
+/*
+ * Widening SURVEY.md 8(f) f2: the paper's geometry holds "rotations, translations, logical operations, and distance
+ * calculations" and builds solids by "boolean operations"; it defines none of them.
+ * Readings R27-R29 of DESIGN.md:
+ *   R27  C = A op B, op in {union, intersection, subtraction (A minus B)}; A, B primitive solids, A in the frame of
+ *        C, B placed by a row-major 3x4 [R | b] from the frame of C to the frame of B.  Membership is the set
+ *        operation on the closed sets.  Inside(p) combines the two classes: union: INSIDE if either is INSIDE,
+ *        OUTSIDE if both are OUTSIDE; intersection: INSIDE if both, OUTSIDE if either is OUTSIDE; subtraction:
+ *        INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A OUTSIDE or B INSIDE; SURFACE otherwise.
+ *   R28  Distances: along the ray each solid is a union of intervals bounded by its crossings (ALL crossings of
+ *        c.4, not only the first); C's membership along the ray is the set operation on the two interval sets;
+ *        DistanceToIn / DistanceToOut is the first t > 0 at which C's membership differs from its value at the
+ *        start point (strict membership of A and B at p, R6), +inf if it never does; -1 on the wrong side as R4.
+ *   R29  Safeties: the usual composition sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB).  This is
+ *        NOT the exact distance of R2: it never over-estimates the distance to the surface of C, is exact where
+ *        only one operand matters, and has the sign of the membership (pinned as such).
+ */
+
+enum { ORC_UNION = 0, ORC_INTERSECTION = 1, ORC_SUBTRACTION = 2 };
+
+typedef struct {
+    int op;
+    const orc_shape *a, *b;
+    real xf[12];
+} orc_boolean;
+
+orc_boolean *orc_boolean_create(int op, const orc_shape *a, const orc_shape *b, const double *xf)
+{
+    if (op < 0 || op > 2 || !a || !b || !xf || !finite_all(xf, 12)) return NULL;
+    orc_boolean *c = (orc_boolean *)calloc(1, sizeof *c);
+    if (!c) return NULL;
+    c->op = op;
+    c->a = a;
+    c->b = b;
+    for (int k = 0; k < 12; ++k) c->xf[k] = xf[k];
+    return c;
+}
+
+void orc_boolean_destroy(orc_boolean *c) { free(c); }
+
+#define ORC_MAXX (4 * ORC_MAXV + 8)
+
+/* every crossing t > 0 of the boundary of one solid by the ray, ascending (c.4 with "collect" in place of "min") */
+static int all_crossings(const orc_shape *s, const real p[3], const real d[3], real *out)
+{
+    int n = 0;
+    if (s->kind == ORC_BOX || s->kind == ORC_TRD) { /* convex: the interval [tin, tout] of the clip */
+        real tin = -ORC_INF, tout = ORC_INF;
+        if (s->kind == ORC_BOX) {
+            for (int i = 0; i < 3; ++i) {
+                real h = s->h[i];
+                if (d[i] != 0) {
+                    real sg = d[i] > 0 ? 1 : -1;
+                    tin = rmax2(tin, (-sg * h - p[i]) / d[i]);
+                    tout = rmin2(tout, (sg * h - p[i]) / d[i]);
+                } else if (R_FABS(p[i]) >= h) {
+                    return 0;
+                }
+            }
+        } else {
+            for (int j = 0; j < 6; ++j) {
+                real num = s->ph[j] - (s->pn[j][0] * p[0] + s->pn[j][1] * p[1] + s->pn[j][2] * p[2]);
+                real den = s->pn[j][0] * d[0] + s->pn[j][1] * d[1] + s->pn[j][2] * d[2];
+                if (den > 0) tout = rmin2(tout, num / den);
+                else if (den < 0) tin = rmax2(tin, num / den);
+                else if (num < 0) return 0;
+            }
+        }
+        if (!(tin < tout)) return 0;
+        if (tin > 0) out[n++] = tin;
+        if (tout > 0) out[n++] = tout;
+        return n;
+    }
+    if (s->kind == ORC_ORB) {
+        real t[2];
+        real b = p[0] * d[0] + p[1] * d[1] + p[2] * d[2];
+        real c = p[0] * p[0] + p[1] * p[1] + p[2] * p[2] - s->r * s->r;
+        int m = quad_roots(1, b, c, t);
+        for (int i = 0; i < m; ++i)
+            if (t[i] > 0) out[n++] = t[i];
+    } else { /* RZ polygon + phi wedge: the candidate loops of cross_rz */
+        real x = p[0], y = p[1], z = p[2], dx = d[0], dy = d[1], dz = d[2];
+        for (int i = 0; i < s->nv; ++i) {
+            if (edge_on_axis(s, i)) continue;
+            int j = (i + 1) % s->nv;
+            real r0 = s->pr[i], z0 = s->pz[i], r1 = s->pr[j], z1 = s->pz[j];
+            if (z0 != z1) {
+                real B = (r1 - r0) / (z1 - z0), A = r0 - B * z0, k = A + B * z;
+                real t[2];
+                int m = quad_roots(dx * dx + dy * dy - B * B * dz * dz, x * dx + y * dy - B * dz * k, x * x + y * y - k * k, t);
+                for (int q = 0; q < m; ++q) {
+                    if (!(t[q] > 0)) continue;
+                    real zh = z + t[q] * dz;
+                    if (zh < rmin2(z0, z1) || zh > rmax2(z0, z1)) continue;
+                    if (!in_phi(s, x + t[q] * dx, y + t[q] * dy)) continue;
+                    out[n++] = t[q];
+                }
+            } else if (dz != 0) {
+                real t = (z0 - z) / dz;
+                if (!(t > 0)) continue;
+                real hx = x + t * dx, hy = y + t * dy, rh2 = hx * hx + hy * hy;
+                real rlo = rmin2(r0, r1), rhi = rmax2(r0, r1);
+                if (rh2 < rlo * rlo || rh2 > rhi * rhi) continue;
+                if (!in_phi(s, hx, hy)) continue;
+                out[n++] = t;
+            }
+        }
+        if (!s->full) {
+            for (int k = 0; k < 2; ++k) {
+                real ex = s->e[k][0], ey = s->e[k][1], nx = -ey, ny = ex;
+                real nd = nx * dx + ny * dy;
+                if (nd == 0) continue;
+                real t = -(nx * x + ny * y) / nd;
+                if (!(t > 0)) continue;
+                real hx = x + t * dx, hy = y + t * dy;
+                if (!in_poly(s, ex * hx + ey * hy, z + t * dz)) continue;
+                out[n++] = t;
+            }
+        }
+    }
+    for (int i = 1; i < n; ++i) { /* insertion sort */
+        real v = out[i];
+        int j = i - 1;
+        while (j >= 0 && out[j] > v) { out[j + 1] = out[j]; --j; }
+        out[j + 1] = v;
+    }
+    return n;
+}
+
+static int bool_member(int op, int ina, int inb)
+{
+    if (op == ORC_UNION) return ina || inb;
+    if (op == ORC_INTERSECTION) return ina && inb;
+    return ina && !inb;
+}
+
+/* R27 */
+static int bool_inside(const orc_boolean *c, const real p[3])
+{
+    real d0[3] = { 0, 0, 0 }, pb[3], db[3];
+    to_local(c->xf, p, d0, pb, db);
+    int ca = inside(c->a, p[0], p[1], p[2]), cb = inside(c->b, pb[0], pb[1], pb[2]);
+    int ain = ca == ORC_INSIDE, aout = ca == ORC_OUTSIDE, bin = cb == ORC_INSIDE, bout = cb == ORC_OUTSIDE;
+    int in, out;
+    if (c->op == ORC_UNION) { in = ain || bin; out = aout && bout; }
+    else if (c->op == ORC_INTERSECTION) { in = ain && bin; out = aout || bout; }
+    else { in = ain && bout; out = aout || bin; }
+    return in ? ORC_INSIDE : (out ? ORC_OUTSIDE : ORC_SURFACE);
+}
+
+/* R29 */
+static real bool_sdf(const orc_boolean *c, const real p[3])
+{
+    real d0[3] = { 0, 0, 0 }, pb[3], db[3];
+    to_local(c->xf, p, d0, pb, db);
+    real sa = sdf(c->a, p[0], p[1], p[2]), sb = sdf(c->b, pb[0], pb[1], pb[2]);
+    if (c->op == ORC_UNION) return rmin2(sa, sb);
+    if (c->op == ORC_INTERSECTION) return rmax2(sa, sb);
+    return rmax2(sa, -sb);
+}
+
+/* R28: first t > 0 at which the membership of C along the ray differs from its value at p */
+static real bool_cross(const orc_boolean *c, const real p[3], const real d[3])
+{
+    real pb[3], db[3], ta[ORC_MAXX], tb[ORC_MAXX];
+    to_local(c->xf, p, d, pb, db);
+    int na = all_crossings(c->a, p, d, ta), nb = all_crossings(c->b, pb, db, tb);
+    int ina = inside(c->a, p[0], p[1], p[2]) == ORC_INSIDE, inb = inside(c->b, pb[0], pb[1], pb[2]) == ORC_INSIDE;
+    int start = bool_member(c->op, ina, inb);
+    int i = 0, j = 0;
+    while (i < na || j < nb) {
+        real t;
+        if (j >= nb || (i < na && ta[i] <= tb[j])) { t = ta[i++]; ina = !ina; }
+        else { t = tb[j++]; inb = !inb; }
+        if (bool_member(c->op, ina, inb) != start) return t;
+    }
+    return ORC_INF;
+}
+
+void orc_boolean_inside(const orc_boolean *c, const double *x, const double *y, const double *z, int64_t n, int32_t *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] };
+        out[i] = bool_inside(c, p);
+    }
+}
+
+void orc_boolean_sdf(const orc_boolean *c, const double *x, const double *y, const double *z, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] };
+        out[i] = (double)bool_sdf(c, p);
+    }
+}
+
+/* which = 0: DistanceToIn, 1: DistanceToOut (R4, R5 as for the primitives) */
+void orc_boolean_distance(const orc_boolean *c, int which, const double *x, const double *y, const double *z,
+                          const double *dx, const double *dy, const double *dz, double step_max, int64_t n, double *out)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] };
+        int cls = bool_inside(c, p);
+        if ((which == 0 && cls == ORC_INSIDE) || (which == 1 && cls == ORC_OUTSIDE)) { out[i] = -1; continue; }
+        real t = bool_cross(c, p, d);
+        out[i] = (double)(t <= step_max ? t : ORC_INF);
+    }
+}
+
+/* the crossings of one primitive, exposed for the pins: writes up to `max` ascending values, returns the count */
+int orc_all_crossings(const orc_shape *s, double x, double y, double z, double dx, double dy, double dz, double *out, int max)
+{
+    real p[3] = { x, y, z }, d[3] = { dx, dy, dz }, t[ORC_MAXX];
+    int n = all_crossings(s, p, d, t);
+    for (int i = 0; i < n && i < max; ++i) out[i] = (double)t[i];
+    return n;
 }

@@ -289,3 +289,47 @@ class WorldCase:
 
 def world_case(**kw):
     return WorldCase(**kw)
+
+
+# ------------------------------------------------------------------ boolean solids
+
+UNION, INTERSECTION, SUBTRACTION = 0, 1, 2
+OP_NAME = {UNION: "union", INTERSECTION: "intersection", SUBTRACTION: "subtraction"}
+
+
+class BooleanCase:
+    """C = A op B (readings R27-R29): B placed in the frame of A by a seeded rotation and an offset; tracks
+    from points uniform in 1.2 x the box that bounds A and the bounding sphere of B, isotropic directions."""
+
+    def __init__(self, name, op, kind_a, par_a, kind_b, par_b, offset, quat, seed):
+        self.name, self.op = name, op
+        self.kind_a, self.par_a = kind_a, [float(v) for v in par_a]
+        self.kind_b, self.par_b = kind_b, [float(v) for v in par_b]
+        self.xform = placement(quaternion_to_matrix(quat), offset)
+        self.seed = seed
+        ca, ha = bounding_half(kind_a, par_a)
+        cb, hb = bounding_half(kind_b, par_b)
+        rb = math.sqrt(sum(v * v for v in hb)) + math.sqrt(sum(v * v for v in cb))
+        lo = [min(ca[i] - ha[i], offset[i] - rb) for i in range(3)]
+        hi = [max(ca[i] + ha[i], offset[i] + rb) for i in range(3)]
+        self.center = tuple(0.5 * (lo[i] + hi[i]) for i in range(3))
+        self.half = tuple(0.6 * (hi[i] - lo[i]) for i in range(3))
+
+    def tracks(self, n, band=None):
+        return draw_tracks(self.seed, n, self.center, self.half, band)
+
+
+def boolean_cases():
+    s2 = math.sqrt(0.5)
+    q = [(0.0, 0.0, 0.0, 1.0), (s2, 0.0, 0.0, s2), (0.18257418583505536, 0.3651483716701107, 0.5477225575051661, 0.7302967433402214),
+         (0.5, -0.5, 0.5, 0.5)]
+    seed = BASE_SEED + 600
+    return [
+        BooleanCase("tube_union_box", UNION, TUBE, [5.0, 10.0, 15.0, 0.0, 4.0 * math.pi / 3.0], BOX, [4.0, 4.0, 20.0], (6.0, -2.0, 1.0), q[2], seed),
+        BooleanCase("box_union_orb", UNION, BOX, [5.0, 5.0, 5.0], ORB, [6.0], (3.0, 2.0, -1.0), q[0], seed + 1),
+        BooleanCase("cone_intersection_orb", INTERSECTION, CONE, [2.0, 6.0, 4.0, 12.0, 20.0, 0.0, TWO_PI], ORB, [14.0], (2.0, 1.0, 6.0), q[0], seed + 2),
+        BooleanCase("trd_intersection_tube", INTERSECTION, TRD, [5.0, 10.0, 7.0, 3.0, 15.0], TUBE, [2.0, 8.0, 12.0, 0.0, TWO_PI], (1.0, 0.5, -2.0), q[1], seed + 3),
+        BooleanCase("box_minus_tube", SUBTRACTION, BOX, [10.0, 10.0, 10.0], TUBE, [0.0, 4.0, 12.0, 0.0, TWO_PI], (1.0, -2.0, 0.0), q[2], seed + 4),
+        BooleanCase("orb_minus_box", SUBTRACTION, ORB, [12.0], BOX, [9.0, 3.0, 20.0], (0.0, 2.0, 0.0), q[3], seed + 5),
+        BooleanCase("tube_minus_cone", SUBTRACTION, TUBE, [0.0, 10.0, 10.0, 0.0, TWO_PI], CONE, [0.0, 2.0, 0.0, 9.0, 8.0, 0.5, 5.0], (0.0, 0.0, 3.0), q[0], seed + 6),
+    ]
