@@ -49,7 +49,8 @@ extern "C" {
 typedef struct vg_shape vg_shape;   /* opaque solid; owned by the library until vg_shape_destroy          */
 typedef struct vg_volume vg_volume; /* opaque mother + placed daughters; does NOT own the vg_shape objects */
 
-typedef enum { VG_BOX = 0, VG_ORB = 1, VG_TUBE = 2, VG_CONE = 3, VG_TRD = 4, VG_POLYCONE = 5 } vg_kind;
+typedef enum { VG_BOX = 0, VG_ORB = 1, VG_TUBE = 2, VG_CONE = 3, VG_TRD = 4, VG_POLYCONE = 5,
+               VG_BOOLEAN = 6 /* made by vg_boolean_create only */ } vg_kind;
 
 enum { VG_OUTSIDE = 0, VG_SURFACE = 1, VG_INSIDE = 2 }; /* values written by vg_inside */
 
@@ -89,6 +90,25 @@ typedef enum {
  * there is one; on another device, or without one at create time, the safeties run the ordered-walk kernel instead.
  */
 int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **out);
+
+/*
+ * vg_boolean_create -- the boolean solid C = A op B of two primitives ("boolean operations", PAPER.md:110
+ * "logical operations"; readings R27-R29 in DESIGN.md).  A sits in the frame of C; `xform_b` (HOST,
+ * 12 doubles, row-major 3x4 [R | b], orthonormal R) maps the frame of C to the frame of B.  A and B: box, orb, tube,
+ * cone or trd (VG_ERR_ARG otherwise); their constants are copied.  The result is a vg_shape of kind VG_BOOLEAN that
+ * every query below accepts:
+ *   Inside       combines the operands' classes: union INSIDE if either is, OUTSIDE if both are; intersection INSIDE if
+ *                both are, OUTSIDE if either is; subtraction (A minus B) INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A
+ *                OUTSIDE or B INSIDE; SURFACE otherwise (R27);
+ *   distances    the first t > 0 at which the membership of C along the ray differs from its value at the start point,
+ *                +inf if none, -1 on the wrong side (R28);
+ *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
+ *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
+ *                safeties it is not the exact distance everywhere (R29).
+ * A boolean cannot be an operand, a daughter of a volume or a node of a world in this build.
+ */
+typedef enum { VG_UNION = 0, VG_INTERSECTION = 1, VG_SUBTRACTION = 2 } vg_bool_op;
+int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out);
 void vg_shape_destroy(vg_shape *shape); /* NULL is allowed */
 int vg_shape_kind(const vg_shape *shape); /* the vg_kind, or VG_ERR_ARG for NULL */
 
@@ -114,7 +134,7 @@ int vg_safety_to_out(const vg_shape *shape, const double *x, const double *y, co
  * vg_query_all -- the five answers of n tracks in one call (a basket of particles in one volume asks all three
  * questions of PAPER.md:110-114 every step).  Same results, element by element, as the five
  * calls above.  Any output pointer may be NULL (that answer is skipped; at least one must be given).  When all five
- * are given and the solid is not a polycone, ONE fused kernel reads the six track arrays once (48 B per track
+ * are given and the solid is neither a polycone nor a boolean, ONE fused kernel reads the six track arrays once (48 B per track
  * instead of 168 B) and writes the five results; otherwise the call enqueues one kernel per requested answer.
  * cls: DEVICE int32[n]; the other four: DEVICE double[n]; dx, dy, dz and step_max as for vg_distance_to_in.
  */

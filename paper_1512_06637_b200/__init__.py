@@ -17,6 +17,8 @@ import torch
 from . import build as _build
 
 BOX, ORB, TUBE, CONE, TRD, POLYCONE = range(6)
+BOOLEAN = 6
+UNION, INTERSECTION, SUBTRACTION = 0, 1, 2
 OUTSIDE, SURFACE, INSIDE = 0, 1, 2
 HIT_MOTHER, HIT_STEPMAX = -1, -2
 KTOLERANCE = 1e-9
@@ -51,6 +53,7 @@ def _load():
     lib.vg_volume_destroy.restype = None
     lib.vg_compute_step.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP, _VP]
     lib.vg_volume_safety.argtypes = [_VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
+    lib.vg_boolean_create.argtypes = [C.c_int, _VP, _VP, _PD, C.POINTER(_VP)]
     lib.vg_world_create.argtypes = [C.c_int, C.POINTER(_VP), C.POINTER(C.c_int32), _PD, C.POINTER(_VP)]
     lib.vg_world_destroy.argtypes = [_VP]
     lib.vg_world_destroy.restype = None
@@ -137,6 +140,15 @@ def vg_shape_create(kind, params):
 
 def vg_shape_destroy(h):
     _lib.vg_shape_destroy(h)
+
+
+def vg_boolean_create(op, a, b, xform_b):
+    flat = [float(v) for v in xform_b]
+    if len(flat) != 12:
+        raise ValueError("xform_b must hold 12 doubles")
+    h = _VP()
+    _check(_lib.vg_boolean_create(int(op), _handle(a), _handle(b), (C.c_double * 12)(*flat), C.byref(h)))
+    return h
 
 
 def _handle(s):
@@ -408,6 +420,15 @@ class Shape:
 
     def query_host(self, name, x, y, z, dx=None, dy=None, dz=None, step_max=math.inf, out=None):
         return vg_query_host(self, name, x, y, z, dx, dy, dz, step_max, out)
+
+
+class Boolean(Shape):
+    """C = A op B of two primitives (readings R27-R29): `xform_b` is the row-major 3x4 [R | b] from the frame of C (= of A)
+    to the frame of B.  Every query of Shape applies."""
+
+    def __init__(self, op, a, b, xform_b):
+        self.kind, self.op = BOOLEAN, int(op)
+        self._h = vg_boolean_create(op, a, b, xform_b)
 
 
 class Volume:

@@ -187,6 +187,7 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
         e = launch_polycone(q, s->u.pcon, g, t, step_max, n, out, vec, st);
         break;
     }
+    case VG_BOOLEAN: e = launch_boolean(q, s->u.boolean, t, step_max, n, out, st); break;
     }
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
@@ -231,7 +232,7 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
     const char *fn = "vg_query_all";
     if (!s) return fail(VG_ERR_ARG, "%s: shape is NULL", fn);
     const bool all = cls && dist_in && dist_out && safety_in && safety_out;
-    if (!all || s->kind == VG_POLYCONE) { // a subset, or no fused kernel for this solid: one launch per requested answer
+    if (!all || s->kind == VG_POLYCONE || s->kind == VG_BOOLEAN) { // a subset, or no fused kernel for this solid: one launch per requested answer
         if (!cls && !dist_in && !dist_out && !safety_in && !safety_out) return fail(VG_ERR_ARG, "%s: every output is NULL", fn);
         int rc = VG_OK;
         if (cls && rc == VG_OK) rc = vg_inside(s, x, y, z, n, cls, stream);
@@ -298,7 +299,7 @@ static int to_solid(const vg_shape *s, SolidU *o, const char *what)
     case VG_TUBE: o->u.tube = s->u.tube; return VG_OK;
     case VG_CONE: o->u.cone = s->u.cone; return VG_OK;
     case VG_TRD: o->u.trd = s->u.trd; return VG_OK;
-    default: return fail(VG_ERR_ARG, "vg_volume_create: a polycone %s is not supported in this build", what);
+    default: return fail(VG_ERR_ARG, "a polycone or boolean %s is not supported in this build", what);
     }
 }
 
@@ -460,6 +461,34 @@ static void compose(const double *A, const double *B, double *C)
         for (int c = 0; c < 3; ++c) C[4 * r + c] = A[4 * r] * B[c] + A[4 * r + 1] * B[4 + c] + A[4 * r + 2] * B[8 + c];
         C[4 * r + 3] = A[4 * r] * B[3] + A[4 * r + 1] * B[7] + A[4 * r + 2] * B[11] + A[4 * r + 3];
     }
+}
+
+// --------------------------------------------------------------------------------------------- boolean solids
+
+extern "C" int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out)
+{
+    const char *fn = "vg_boolean_create";
+    if (!out) return fail(VG_ERR_ARG, "%s: out is NULL", fn);
+    *out = nullptr;
+    if (op < VG_UNION || op > VG_SUBTRACTION) return fail(VG_ERR_PARAM, "%s: op must be VG_UNION, VG_INTERSECTION or VG_SUBTRACTION", fn);
+    if (!a || !b || !xform_b) return fail(VG_ERR_ARG, "%s: NULL operand or transform", fn);
+    if (!all_finite(xform_b, 12)) return fail(VG_ERR_PARAM, "%s: non-finite transform", fn);
+    if (!rigid(xform_b)) return fail(VG_ERR_PARAM, "%s: the rotation of B is not orthonormal", fn);
+    vg_shape *s = new (std::nothrow) vg_shape;
+    if (!s) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
+    std::memset(s, 0, sizeof *s);
+    s->kind = VG_BOOLEAN;
+    BoolP &c = s->u.boolean;
+    c.op = op;
+    std::memcpy(c.X, xform_b, sizeof c.X);
+    int rc = to_solid(a, &c.a, "operand");
+    if (rc == VG_OK) rc = to_solid(b, &c.b, "operand");
+    if (rc != VG_OK) {
+        delete s;
+        return rc;
+    }
+    *out = s;
+    return VG_OK;
 }
 
 extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int32_t *parent, const double *xforms,

@@ -19,6 +19,7 @@ struct vg_shape {
         ConeP cone;
         TrdP trd;
         PolyconeP pcon;
+        BoolP boolean;
     } u;
     // full-phi polycone only: the candidate grid of vg_pcon_grid.h in device memory of `grid_device` (masks == NULL if
     // no device was available at create; the safeties then run the ordered walk)
@@ -198,6 +199,7 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         return VG_OK;
     }
     }
+    if (kind == VG_BOOLEAN) return fail(VG_ERR_ARG, "a boolean solid is made by vg_boolean_create");
     return fail(VG_ERR_PARAM, "unknown shape kind %d", int(kind));
 }
 

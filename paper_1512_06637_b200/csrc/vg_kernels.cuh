@@ -575,6 +575,9 @@ cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table
 cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t, int64_t n,
                                  double *safety, cudaStream_t s);
 
+// boolean solids (vg_bool.cu)
+cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
+
 // hierarchy of volumes (vg_world.cu)
 cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const float4 *cull, const Tracks &t, int64_t n, int32_t *out,
                                 cudaStream_t s);

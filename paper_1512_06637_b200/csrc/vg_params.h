@@ -9,7 +9,7 @@ namespace vg {
 constexpr int kMaxZ = 32;       // polycone z-planes
 constexpr int kMaxSec = kMaxZ - 1;
 
-enum Kind : int { kBox = 0, kOrb = 1, kTube = 2, kCone = 3, kTrd = 4, kPolycone = 5 };
+enum Kind : int { kBox = 0, kOrb = 1, kTube = 2, kCone = 3, kTrd = 4, kPolycone = 5, kBoolean = 6 };
 enum Query : int { qInside = 0, qDistIn = 1, qDistOut = 2, qSafeIn = 3, qSafeOut = 4 };
 
 // phi segment [sphi, sphi + dphi]; e0, e1 = unit vectors of the two bounding half-planes (reading R11)
@@ -124,6 +124,15 @@ struct SolidU {
         ConeP cone;
         TrdP trd;
     } u;
+};
+
+// boolean solid C = A op B of two primitives (readings R27-R29): A in the frame of C, B placed by X (frame of C -> frame of B)
+enum BoolOp : int { kUnion = 0, kIntersection = 1, kSubtraction = 2 };
+struct BoolP {
+    int op;
+    int pad;
+    double X[12];
+    SolidU a, b;
 };
 
 // navigation: one placed daughter
