@@ -116,7 +116,7 @@ class ClockSampler:
 class Case:
     """One solid (or the navigation volume) with its seeded tracks resident in HBM as `nsets` rotating copies."""
 
-    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None, world=None):
+    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None, world=None, boolean=None):
         self.vg, self.torch, self.name, self.n, self.queries = vg, torch, name, int(n), tuple(queries)
         dev = torch.device("cuda", torch.cuda.current_device())
         self.nodes = None
@@ -130,6 +130,17 @@ class Case:
                 nd = self.handle.locate(*d)
                 s = self.handle.safety(torch.clamp(nd, min=0), *d)
                 return ((nd < 0) | (s < W.SURFACE_BAND)).cpu().numpy()
+        elif boolean is not None:
+            self.kind = "boolean"
+            a, b = vg.Shape(boolean.kind_a, boolean.par_a), vg.Shape(boolean.kind_b, boolean.par_b)
+            self.handle = vg.Boolean(boolean.op, a, b, boolean.xform)
+            seed, center, half = boolean.seed + seed_shift, boolean.center, boolean.half
+            M = np.asarray(boolean.xform).reshape(3, 4)
+
+            def band(x, y, z):  # clear of both operands' surfaces (library's own safeties)
+                L = M[:, :3] @ np.stack([x, y, z]) + M[:, 3:4]
+                return (np.abs(self._gpu3(a.safety_to_in, x, y, z)) < W.SURFACE_BAND) | \
+                       (np.abs(self._gpu3(b.safety_to_in, L[0], L[1], L[2])) < W.SURFACE_BAND)
         elif nav is not None:
             self.kind = "navigator"
             mother = vg.Shape(nav.mother_kind, nav.mother_params)
@@ -448,6 +459,18 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
     rows.append(e)
     del case
     torch.cuda.empty_cache()
+    # boolean solids of two primitives (one of each operation)
+    for bc in [b for b in W.boolean_cases() if b.name in ("tube_union_box", "cone_intersection_orb", "box_minus_tube")]:
+        case = Case(vg, torch, bc.name, 4194304, W.QUERIES5, boolean=bc)
+        for q in case.queries:
+            sec = time_query_alone(torch, case, q)
+            e = roofline_entry("boolean", q, case.n, sec, hbm_peak, fma_rate)
+            e.update({"config": "8(f) f2", "shape": bc.name, "query": q, "n": case.n, "cold_inputs": case.cold})
+            if q.startswith("distance"):
+                e["bound"] = "alu"
+            rows.append(e)
+        del case
+        torch.cuda.empty_cache()
     # the three-level tree of placed solids (193 nodes), every track in its own node
     wc = W.world_case()
     case = Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc)
@@ -480,12 +503,17 @@ def run_profile(args):
     cases.append(Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step",), nav=nav))
     wc = W.world_case()
     cases.append(Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc))
+    bc = [b for b in W.boolean_cases() if b.name == "box_minus_tube"][0]
+    cases.append(Case(vg, torch, bc.name, 4194304, W.QUERIES5, boolean=bc))
+    stepped = W.ShapeCase(3, "polycone_step", W.POLYCONE, W.STEPPED_POLYCONE, *W._scaled(W.POLYCONE, W.STEPPED_POLYCONE),
+                          W.config_seed(3, 2), [4194304], ("distance_to_in", "safety_to_in"))
+    cases.append(Case(vg, torch, stepped.name, 4194304, stepped.queries, shape=stepped))
     torch.cuda.synchronize()
     torch.cuda.profiler.start()  # ncu --profile-from-start off: the set-up launches (surface-band rejection) are skipped
     for _ in range(args.steps):
         for c in cases:
             c.step()
-            if len(c.queries) == 5 and c.kind != "polycone":
+            if len(c.queries) == 5 and c.kind not in ("polycone", "boolean"):
                 c.launch("all")  # the fused five-query kernel
     torch.cuda.synchronize()
     torch.cuda.profiler.stop()

@@ -1,0 +1,161 @@
+// vg_bool.cuh -- device code of the boolean solids; see vg_bool.cu for the design.  Included by vg_bool.cu (Inside, the
+// safeties, the dispatch) and by vg_bool_k<A>.cu (the distance kernels of operand kind A against every kind B: one
+// translation unit per A so that the 50 instantiations compile in parallel).
+#pragma once
+#include "vg_kernels.cuh"
+#include "vg_solid.cuh"
+
+namespace vg {
+
+constexpr int kBoolBlock = 128;
+constexpr int kBoolMaxEvents = 64; // an operand has at most ~10 crossings with a line; the loop ends long before
+
+// next crossing of the operand's boundary at t > 0 in the given sense (leaving: the track is inside it), +inf if none.
+// K = the operand's kind at compile time (the distance kernels are instantiated per pair of kinds: straight-line code,
+// no divergence between lanes over the kind), or -1 to read it from the record.
+template <int K>
+VG_DEV double solid_next(const SolidU &s, bool inside, double x, double y, double z, double dx, double dy, double dz)
+{
+    double t;
+    switch (K < 0 ? s.kind : K) {
+    case kBox: {
+        double tin, tout;
+        Box::slabs(s.u.box, x, y, z, dx, dy, dz, tin, tout);
+        t = inside ? tout : ((tin < tout) ? tin : inf());
+        break;
+    }
+    case kTrd: {
+        double tin, tout;
+        Trd::clip_all(s.u.trd, x, y, z, dx, dy, dz, tin, tout);
+        t = inside ? tout : ((tin < tout) ? tin : inf());
+        break;
+    }
+    case kOrb: { // a = 1: the entering root is the smaller one, the leaving root the larger
+        const double pp = fma(x, x, fma(y, y, z * z)), b = fma(x, dx, fma(y, dy, z * dz));
+        const double c = pp - s.u.orb.r2, D = fma(b, b, -c);
+        const double sq = sqrt_pos(D);
+        const double q = -(b + copysign_bits(sq, b));
+        const double t1 = q, t2 = c * rcp(q);
+        t = D > 0.0 ? (inside ? dmax(t1, t2) : dmin(t1, t2)) : inf();
+        break;
+    }
+    case kTube: t = inside ? Tube::dist_out(s.u.tube, x, y, z, dx, dy, dz) : Tube::dist_in(s.u.tube, x, y, z, dx, dy, dz); break;
+    default: t = inside ? Cone::dist_out(s.u.cone, x, y, z, dx, dy, dz) : Cone::dist_in(s.u.cone, x, y, z, dx, dy, dz); break;
+    }
+    return t > 0.0 ? t : inf(); // a crossing behind the point, a wrong-side -1 or a NaN is "no crossing"
+}
+
+VG_DEV bool bool_member(int op, bool ina, bool inb)
+{
+    return op == kUnion ? (ina || inb) : (op == kIntersection ? (ina && inb) : (ina && !inb));
+}
+
+VG_DEV int bool_classify(int op, int ca, int cb)
+{
+    const bool ain = ca == cInside, aout = ca == cOutside, bin = cb == cInside, bout = cb == cOutside;
+    bool in, out;
+    if (op == kUnion) in = ain || bin, out = aout && bout;
+    else if (op == kIntersection) in = ain && bin, out = aout || bout;
+    else in = ain && bout, out = aout || bin;
+    return classify(in, out);
+}
+
+#ifndef VG_BOOL_MINB
+#define VG_BOOL_MINB 3
+#endif
+
+template <int Q, int KA, int KB>
+__global__ void __launch_bounds__(kBoolBlock, (Q == qDistIn || Q == qDistOut) ? VG_BOOL_MINB : 1)
+    bool_kernel(const __grid_constant__ BoolP p, Tracks t, double step_max, int64_t n, void *out)
+{
+    constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
+    pdl_launch_dependents();
+    pdl_wait();
+    const int64_t i = int64_t(blockIdx.x) * kBoolBlock + threadIdx.x;
+    if (i >= n) return;
+    const double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+    const double *m = p.X;
+    const double bx = fma(m[0], x, fma(m[1], y, fma(m[2], z, m[3])));
+    const double by = fma(m[4], x, fma(m[5], y, fma(m[6], z, m[7])));
+    const double bz = fma(m[8], x, fma(m[9], y, fma(m[10], z, m[11])));
+    if (Q == qSafeIn || Q == qSafeOut) { // R29
+        const double sa = solid_sdf(p.a, x, y, z), sb = solid_sdf(p.b, bx, by, bz);
+        const double s = p.op == kUnion ? dmin(sa, sb) : (p.op == kIntersection ? dmax(sa, sb) : dmax(sa, -sb));
+        stg1(static_cast<double *>(out) + i, Q == qSafeIn ? s : -s);
+        return;
+    }
+    const int ca = solid_inside(p.a, x, y, z), cb = solid_inside(p.b, bx, by, bz);
+    const int cls = bool_classify(p.op, ca, cb); // R27
+    if (Q == qInside) {
+        stg1i(static_cast<int32_t *>(out) + i, cls);
+        return;
+    }
+    if (kDir) { // R28
+        const double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+        const double bdx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
+        const double bdy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
+        const double bdz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
+        double res;
+        if ((Q == qDistIn && cls == cInside) || (Q == qDistOut && cls == cOutside)) {
+            res = -1.0;
+        } else {
+            bool ina = ca == cInside, inb = cb == cInside;
+            const bool start = bool_member(p.op, ina, inb);
+            double tt = 0.0;
+            res = inf();
+#pragma unroll 1
+            for (int it = 0; it < kBoolMaxEvents; ++it) {
+                const double ea = solid_next<KA>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
+                const double eb = solid_next<KB>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
+                const bool a_first = ea <= eb; // a tie goes to A, as in the oracle's merge
+                const double e = a_first ? ea : eb;
+                if (!(e < inf())) break;
+                tt += e;
+                ina = a_first ? !ina : ina;
+                inb = a_first ? inb : !inb;
+                if (bool_member(p.op, ina, inb) != start) {
+                    res = tt;
+                    break;
+                }
+            }
+            res = res <= step_max ? res : inf();
+        }
+        stg1(static_cast<double *>(out) + i, res);
+    }
+}
+
+
+// the two distance kernels for operand kinds (A, kb), kb at run time: one plain function per kind of A, each defined in
+// its own translation unit vg_bool_k<A>.cu
+#define VG_BOOL_DECLARE_DIST(NAME)                                                                                     \
+    cudaError_t launch_boolean_dist_##NAME(int q, int kb, const BoolP &p, const Tracks &t, double step_max, int64_t n, \
+                                           void *out, unsigned grid, cudaStream_t s);
+VG_BOOL_DECLARE_DIST(kBox)
+VG_BOOL_DECLARE_DIST(kOrb)
+VG_BOOL_DECLARE_DIST(kTube)
+VG_BOOL_DECLARE_DIST(kCone)
+VG_BOOL_DECLARE_DIST(kTrd)
+
+template <int Q, int KA>
+cudaError_t launch_boolean_dist_b(int kb, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, unsigned grid,
+                                  cudaStream_t s)
+{
+    switch (kb) {
+    case kBox: return launch_kernel(bool_kernel<Q, KA, kBox>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);
+    case kOrb: return launch_kernel(bool_kernel<Q, KA, kOrb>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);
+    case kTube: return launch_kernel(bool_kernel<Q, KA, kTube>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);
+    case kCone: return launch_kernel(bool_kernel<Q, KA, kCone>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);
+    case kTrd: return launch_kernel(bool_kernel<Q, KA, kTrd>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);
+    }
+    return cudaErrorInvalidValue;
+}
+
+#define VG_BOOL_DEFINE_DIST(NAME)                                                                                      \
+    cudaError_t launch_boolean_dist_##NAME(int q, int kb, const BoolP &p, const Tracks &t, double step_max, int64_t n, \
+                                           void *out, unsigned grid, cudaStream_t s)                                   \
+    {                                                                                                                  \
+        return q == qDistIn ? launch_boolean_dist_b<qDistIn, NAME>(kb, p, t, step_max, n, out, grid, s)                \
+                            : launch_boolean_dist_b<qDistOut, NAME>(kb, p, t, step_max, n, out, grid, s);              \
+    }
+
+} // namespace vg

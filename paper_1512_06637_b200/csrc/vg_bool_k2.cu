@@ -1,0 +1,6 @@
+// vg_bool_k2.cu -- boolean distance kernels with operand A of kind kTube against every kind of B (see vg_bool.cuh)
+#include "vg_bool.cuh"
+
+namespace vg {
+VG_BOOL_DEFINE_DIST(kTube)
+}

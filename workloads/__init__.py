@@ -106,6 +106,11 @@ def polycone_params(seed, nz=10):
     return out
 
 
+# a polycone with two z steps (reading R26): the radii jump outwards at z = -4 (the bore opens) and inwards at z = 6
+STEPPED_POLYCONE = [0.0, TWO_PI, 7.0, -12.0, 0.0, 6.0, -4.0, 1.0, 8.0, -4.0, 3.0, 12.0, 2.0, 2.0, 10.0, 6.0, 2.0, 11.0,
+                    6.0, 0.0, 5.0, 14.0, 1.5, 4.0]
+
+
 class ShapeCase:
     """One (shape, sampling box, seed) of a config."""
 
