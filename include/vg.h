@@ -251,8 +251,10 @@ int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, c
  * results).  DIRECT: one CTA per 512 tracks.  PIPELINED: the TMA ring above (subject to VG_OPT_PIPE_MIN_N and the
  * alignment rule).  STREAMING: one resident wave of CTAs, each owning one contiguous range of tracks and loading its
  * next pair of tracks while it evaluates the current one (16-byte aligned arrays only).  AUTO takes, per (solid,
- * query), the form that measured fastest (profiles/). */
-typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2 } vg_option;
+ * query), the form that measured fastest (profiles/).
+ * VG_OPT_HOST_CHUNK (default 0 = chosen from n): tracks per chunk of the host-buffer entry points' copy / compute
+ * pipeline (clamped to 2^20). */
+typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2, VG_OPT_HOST_CHUNK = 3 } vg_option;
 enum { VG_FORM_AUTO = 0, VG_FORM_DIRECT = 1, VG_FORM_PIPELINED = 2, VG_FORM_STREAMING = 3 };
 int vg_set_option(int option, int64_t value);
 int64_t vg_get_option(int option); /* the value, or VG_ERR_ARG for an unknown option */

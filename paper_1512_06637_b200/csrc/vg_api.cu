@@ -49,6 +49,7 @@ std::atomic<int64_t> g_launches{ 0 };
 std::atomic<int64_t> g_pipe_min_n{ int64_t(1) << 17 };
 std::atomic<int64_t> g_pdl{ 1 };
 std::atomic<int64_t> g_form{ VG_FORM_AUTO };
+std::atomic<int64_t> g_host_chunk{ 0 };
 }
 extern "C" int64_t vg_launch_count(void) { return vg::g_launches.load(); }
 
@@ -61,6 +62,10 @@ extern "C" int vg_set_option(int option, int64_t value)
         return VG_OK;
     case VG_OPT_PDL:
         vg::g_pdl.store(value != 0);
+        return VG_OK;
+    case VG_OPT_HOST_CHUNK:
+        if (value < 0) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_HOST_CHUNK must be >= 0");
+        vg::g_host_chunk.store(value);
         return VG_OK;
     case VG_OPT_FORM:
         if (value < VG_FORM_AUTO || value > VG_FORM_STREAMING) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_FORM must be 0..3");
@@ -76,6 +81,7 @@ extern "C" int64_t vg_get_option(int option)
     case VG_OPT_PIPE_MIN_N: return vg::g_pipe_min_n.load();
     case VG_OPT_PDL: return vg::g_pdl.load();
     case VG_OPT_FORM: return vg::g_form.load();
+    case VG_OPT_HOST_CHUNK: return vg::g_host_chunk.load();
     }
     return fail(VG_ERR_ARG, "vg_get_option: unknown option %d", option);
 }

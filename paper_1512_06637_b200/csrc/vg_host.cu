@@ -16,6 +16,7 @@ namespace vg {
 constexpr int kSlots = 4;
 constexpr int64_t kMaxChunk = int64_t(1) << 20; // tracks per chunk: 8 MiB per coordinate array
 constexpr int64_t kMinChunk = int64_t(1) << 16;
+constexpr int64_t kBigChunk = int64_t(1) << 19; // the automatic choice stays at or below this
 constexpr int kMaxDev = 16;
 
 struct HostPipe {
@@ -57,10 +58,15 @@ static cudaError_t pipe_init(HostPipe &p)
 
 static int64_t pick_chunk(int64_t n)
 {
-    int64_t c = (n + 2 * kSlots - 1) / (2 * kSlots); // about two rounds over the slots
+    const int64_t forced = g_host_chunk.load(std::memory_order_relaxed); // vg_set_option(VG_OPT_HOST_CHUNK)
+    if (forced > 0) return forced < kMaxChunk ? (forced + 1) / 2 * 2 : kMaxChunk;
+    // One chunk per slot, between 64 Ki and 512 Ki tracks: every cudaMemcpyAsync costs ~5 us of engine set-up, so copies
+    // under ~2 MB per array leave the link idle (measured, profiles/r1g_host_chunk.md: 1 Mi tracks 1.70 ms with 128 Ki
+    // chunks, 1.41 ms with 256-512 Ki), while fewer than three chunks cannot overlap H2D with D2H.
+    int64_t c = (n + kSlots - 1) / kSlots;
     c = (c + 4095) / 4096 * 4096;
     if (c < kMinChunk) c = kMinChunk;
-    if (c > kMaxChunk) c = kMaxChunk;
+    if (c > kBigChunk) c = kBigChunk;
     return c;
 }
 
