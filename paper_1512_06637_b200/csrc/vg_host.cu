@@ -83,6 +83,17 @@ static int cuda_fail(cudaError_t e, const char *fn)
     return vg_set_error(VG_ERR_CUDA, buf);
 }
 
+// distance in doubles between consecutive arrays if it is the same for all of them and at least n (no overlap), else 0
+static int64_t equal_pitch(const double *const *h, int count, int64_t n)
+{
+    if (count < 2) return 0;
+    const int64_t pitch = h[1] - h[0];
+    if (pitch < n) return 0;
+    for (int a = 2; a < count; ++a)
+        if (h[a] - h[a - 1] != pitch) return 0;
+    return pitch;
+}
+
 constexpr int qAll = 5; // run_host: the five answers at once, `all` = {cls, dist_in, dist_out, safety_in, safety_out} (HOST, may be NULL)
 
 // shape != NULL: query q of the shape (or all five); volume != NULL: ComputeStep
@@ -105,6 +116,15 @@ static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volu
     std::lock_guard<std::mutex> lock(p->mu);
     if ((e = pipe_init(*p)) != cudaSuccess) return cuda_fail(e, fn);
     int64_t chunk = pick_chunk(n);
+    // Host arrays that sit at one constant distance from each other (rows of one allocation) travel as one 2-D copy per
+    // chunk: every copy costs a few microseconds of set-up, which is most of the time of a small call.
+    int64_t in_pitch = equal_pitch(h, na, n);
+    int64_t out_pitch = 0;
+    if (q == qAll && all[1] && all[2] && all[3] && all[4]) {
+        const double *od4[4] = { static_cast<double *>(all[1]), static_cast<double *>(all[2]), static_cast<double *>(all[3]),
+                                 static_cast<double *>(all[4]) };
+        out_pitch = equal_pitch(od4, 4, n);
+    }
     int rc = VG_OK;
     int c = 0;
     for (int64_t o = 0; o < n && rc == VG_OK; o += chunk, ++c) {
@@ -112,10 +132,22 @@ static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volu
         int64_t m = n - o < chunk ? n - o : chunk;
         cudaStream_t st = p->st[s];
         double *d[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
-        for (int a = 0; a < na; ++a) {
-            d[a] = p->in[s] + a * kMaxChunk;
-            e = cudaMemcpyAsync(d[a], h[a] + o, m * sizeof(double), cudaMemcpyHostToDevice, st);
-            if (e != cudaSuccess) return cuda_fail(e, fn);
+        for (int a = 0; a < na; ++a) d[a] = p->in[s] + a * kMaxChunk;
+        if (in_pitch > 0) { // equally spaced host arrays (one [6][N] basket): ONE strided copy instead of six
+            e = cudaMemcpy2DAsync(d[0], kMaxChunk * sizeof(double), h[0] + o, size_t(in_pitch) * sizeof(double), m * sizeof(double), na,
+                                  cudaMemcpyHostToDevice, st);
+            if (e == cudaErrorInvalidValue) { // equally spaced but not ONE allocation (the driver refuses the span): six copies
+                cudaGetLastError();
+                in_pitch = 0;
+            } else if (e != cudaSuccess) {
+                return cuda_fail(e, fn);
+            }
+        }
+        if (in_pitch == 0) {
+            for (int a = 0; a < na; ++a) {
+                e = cudaMemcpyAsync(d[a], h[a] + o, m * sizeof(double), cudaMemcpyHostToDevice, st);
+                if (e != cudaSuccess) return cuda_fail(e, fn);
+            }
         }
         if (volume) {
             rc = vg_compute_step(volume, d[0], d[1], d[2], d[3], d[4], d[5], step_max, m, p->outd[s], p->outi[s], st);
@@ -131,9 +163,20 @@ static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volu
             if (rc != VG_OK) break;
             if (all[0])
                 e = cudaMemcpyAsync(static_cast<int32_t *>(all[0]) + o, p->outi[s], m * sizeof(int32_t), cudaMemcpyDeviceToHost, st);
-            for (int a = 0; a < 4 && e == cudaSuccess; ++a)
-                if (od[a])
-                    e = cudaMemcpyAsync(static_cast<double *>(all[a + 1]) + o, od[a], m * sizeof(double), cudaMemcpyDeviceToHost, st);
+            if (out_pitch > 0 && e == cudaSuccess) {
+                e = cudaMemcpy2DAsync(static_cast<double *>(all[1]) + o, size_t(out_pitch) * sizeof(double), od[0], kMaxChunk * sizeof(double),
+                                      m * sizeof(double), 4, cudaMemcpyDeviceToHost, st);
+                if (e == cudaErrorInvalidValue) {
+                    cudaGetLastError();
+                    out_pitch = 0;
+                    e = cudaSuccess;
+                }
+            }
+            if (out_pitch == 0) {
+                for (int a = 0; a < 4 && e == cudaSuccess; ++a)
+                    if (od[a])
+                        e = cudaMemcpyAsync(static_cast<double *>(all[a + 1]) + o, od[a], m * sizeof(double), cudaMemcpyDeviceToHost, st);
+            }
         } else if (q == qInside) {
             rc = vg_inside(shape, d[0], d[1], d[2], m, p->outi[s], st);
             if (rc != VG_OK) break;
@@ -151,7 +194,7 @@ static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volu
         }
         if (e != cudaSuccess) return cuda_fail(e, fn);
     }
-    for (int s = 0; s < kSlots; ++s) {
+    for (int s = 0; s < kSlots && s < c; ++s) { // only the slots this call used
         e = cudaStreamSynchronize(p->st[s]);
         if (e != cudaSuccess && rc == VG_OK) rc = cuda_fail(e, fn);
     }

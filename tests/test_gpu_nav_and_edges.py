@@ -360,6 +360,34 @@ def test_host_entry_points_match_the_oracle(vg, n):
     assert_real_close(g, so.distance_to_in(*t, W.STEP_MAX), "host pageable")
 
 
+def test_host_entry_points_with_one_block_baskets(vg):
+    """Equally spaced host arrays (rows of one [6][n] allocation, results in one [4][n]) travel as strided 2-D copies: same
+    answers as separately allocated arrays; rows of a block with a larger pitch and pageable blocks work as well."""
+    sc = W.shape_cases(1)[0]
+    so, sg = O.Shape(sc.kind, sc.params), vg.Shape(sc.kind, sc.params)
+    for n in (1, 1000, 70001, 1048576 + 3):
+        t = sc.tracks(n, band=oracle_band(so))
+        for pitch, pin in ((n, True), (n + 13, True), (n, False)):
+            blk = torch.empty((6, pitch), dtype=torch.float64)
+            blk = blk.pin_memory() if pin else blk
+            for i in range(6):
+                blk[i, :n].copy_(torch.from_numpy(t[i]))
+            rows = [blk[i, :n] for i in range(6)]
+            oblk = torch.empty((4, pitch), dtype=torch.float64)
+            oblk = oblk.pin_memory() if pin else oblk
+            out = [torch.empty(n, dtype=torch.int32)] + [oblk[i, :n] for i in range(4)]
+            fused = sg.query_all_host(*rows, step_max=W.STEP_MAX, out=out)
+            for q, g in zip(W.QUERIES5, fused):
+                if q.startswith("distance"):
+                    assert_real_close(g.numpy(), getattr(so, q)(*t, W.STEP_MAX), "block host fused %s" % q)
+                elif q == "inside":
+                    assert_int_equal(g.numpy(), so.inside(*t[:3]), "block host fused inside")
+                else:
+                    assert_real_close(g.numpy(), getattr(so, q)(*t[:3]), "block host fused %s" % q)
+            g = sg.query_host("safety_to_in", *rows[:3]).numpy()
+            assert_real_close(g, so.safety_to_in(*t[:3]), "block host safety")
+
+
 def test_host_compute_step(vg):
     nav = W.navigator_case()
     vo, vgv = build_volumes(vg, nav)
