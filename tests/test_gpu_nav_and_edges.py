@@ -452,3 +452,10 @@ def test_polycone_grid_safeties_match_the_oracle(vg, seed, nz, rmin_hi):
     finally:
         vg.vg_set_option(vg.OPT_FORM, vg.FORM_AUTO)
     assert_real_close(g2, so.safety_to_in(*t), "generic safety_to_in nz=%d" % nz)
+
+
+def test_exercise_all_kernels_script(vg):
+    """tests/exercise_all_kernels.py: every kernel once on odd sizes with guard words around the results (the pool has
+    no compute-sanitizer), each compared with the oracle."""
+    import exercise_all_kernels
+    exercise_all_kernels.main()
