@@ -481,7 +481,18 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
         sec = time_query_alone(torch, case, q)
         e = roofline_entry("world", q, case.n, sec, hbm_peak, fma_rate)
         e.update({"config": "8(f) f3", "shape": "box(100) > 64 daughters > 128 grand-daughters", "query": q, "n": case.n,
-                  "cold_inputs": case.cold, "bound": "alu"})
+                  "cold_inputs": case.cold, "bound": "alu", "track_order": "as drawn (nodes mixed within a warp)"})
+        rows.append(e)
+    # the same tracks in basket order (sorted by node, what the paper's scheduler hands to the geometry)
+    for k in range(case.nsets):
+        order = torch.argsort(case.nodes[k].to(torch.int64), stable=True)
+        case.sets[k] = [a[order].contiguous() for a in case.sets[k]]
+        case.nodes[k] = case.nodes[k][order].contiguous()
+    for q in case.queries:
+        sec = time_query_alone(torch, case, q)
+        e = roofline_entry("world", q, case.n, sec, hbm_peak, fma_rate)
+        e.update({"config": "8(f) f3", "shape": "box(100) > 64 daughters > 128 grand-daughters", "query": q, "n": case.n,
+                  "cold_inputs": case.cold, "bound": "alu", "track_order": "sorted by node (baskets)"})
         rows.append(e)
     return rows
 
