@@ -107,3 +107,25 @@ def test_boolean_create_rejects_bad_input(vg):
         vg.Boolean(vg.UNION, a, c, ident)  # no nested booleans in this build
     with pytest.raises(vg.VgError):
         vg.Volume(vg.Shape(W.BOX, [10, 10, 10]), [c], [ident])
+
+
+@pytest.mark.parametrize("name", ["tube_union_box", "cone_intersection_orb", "box_minus_tube"])
+def test_full_size_as_benchmarked_on_sampled_tracks(vg, name):
+    """4,194,304 tracks (the size bench.py times); the oracle checks every 16th track, a property checks them all."""
+    bc = CASES[name]
+    co, cg = build(vg, bc)
+    t = bc.tracks(4194304, clear_of_both(co, bc))
+    dt = dev(t)
+    cls = cg.inside(*dt[:3])
+    din, dout = cg.distance_to_in(*dt, W.STEP_MAX), cg.distance_to_out(*dt, W.STEP_MAX)
+    sin = cg.safety_to_in(*dt[:3])
+    sel = np.arange(3, 4194304, 16)
+    ts = [np.ascontiguousarray(a[sel]) for a in t]
+    assert_int_equal(cls.cpu().numpy()[sel], co.inside(*ts[:3]), name + " full-size inside")
+    assert_real_close(din.cpu().numpy()[sel], co.distance_to_in(*ts, W.STEP_MAX), name + " full-size din")
+    assert_real_close(dout.cpu().numpy()[sel], co.distance_to_out(*ts, W.STEP_MAX), name + " full-size dout")
+    assert_real_close(sin.cpu().numpy()[sel], co.safety_to_in(*ts[:3]), name + " full-size safety")
+    # every track: wrong-side sentinels follow the class, and the composed safety never exceeds the distance
+    assert bool(((din == -1.0) == (cls == vg.INSIDE)).all()) and bool(((dout == -1.0) == (cls == vg.OUTSIDE)).all())
+    outside = cls == vg.OUTSIDE
+    assert bool((sin[outside] <= din[outside] * (1 + 1e-12)).all())

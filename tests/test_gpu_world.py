@@ -117,3 +117,23 @@ def test_world_create_rejects_bad_input(vg):
     w = vg.World([b], [-1], [ident])
     x = torch.zeros(5, dtype=torch.float64, device="cuda")
     assert w.locate(x, x, x).tolist() == [0] * 5
+
+
+def test_full_size_as_benchmarked_on_sampled_tracks(vg, worlds):
+    """4,194,304 tracks (the size and launch configuration bench.py times); the oracle checks every 16th track."""
+    wc, wo, wg, band = worlds
+    t = wc.tracks(4194304, band)
+    dt = dev(t)
+    node_g = wg.locate(*dt[:3])
+    step_g, next_g = wg.step(node_g, *dt, W.STEP_MAX)
+    safe_g = wg.safety(node_g, *dt[:3])
+    sel = np.arange(5, 4194304, 16)
+    ts = [np.ascontiguousarray(a[sel]) for a in t]
+    node_o = wo.locate(*ts[:3])
+    assert_int_equal(node_g.cpu().numpy()[sel], node_o, "full-size locate")
+    so, no = wo.step(node_o, *ts, W.STEP_MAX)
+    assert_int_equal(next_g.cpu().numpy()[sel], no, "full-size next")
+    assert_real_close(step_g.cpu().numpy()[sel], so, "full-size step")
+    assert_real_close(safe_g.cpu().numpy()[sel], wo.safety(node_o, *ts[:3]), "full-size safety")
+    # a property that holds for every track: the safety never exceeds the step
+    assert bool((safe_g <= step_g * (1 + 1e-12)).all())
