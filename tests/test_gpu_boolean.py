@@ -129,3 +129,45 @@ def test_full_size_as_benchmarked_on_sampled_tracks(vg, name):
     assert bool(((din == -1.0) == (cls == vg.INSIDE)).all()) and bool(((dout == -1.0) == (cls == vg.OUTSIDE)).all())
     outside = cls == vg.OUTSIDE
     assert bool((sin[outside] <= din[outside] * (1 + 1e-12)).all())
+
+
+def _random_primitive(rng):
+    kind = int(rng.integers(0, 5))
+    two_pi = 2 * np.pi
+    if kind == W.BOX:
+        return kind, [float(v) for v in rng.uniform(1.0, 10.0, 3)]
+    if kind == W.ORB:
+        return kind, [float(rng.uniform(2.0, 10.0))]
+    if kind == W.TUBE:
+        rmin = float(rng.choice([0.0, rng.uniform(0.5, 4.0)]))
+        return kind, [rmin, rmin + float(rng.uniform(1.0, 6.0)), float(rng.uniform(1.0, 10.0)), float(rng.uniform(-3, 3)),
+                      float(rng.choice([two_pi, rng.uniform(0.5, 6.0)]))]
+    if kind == W.CONE:
+        a, b = float(rng.choice([0.0, rng.uniform(0.5, 3.0)])), float(rng.choice([0.0, rng.uniform(0.5, 3.0)]))
+        return kind, [a, a + float(rng.uniform(1.0, 6.0)), b, b + float(rng.uniform(1.0, 6.0)), float(rng.uniform(1.0, 10.0)),
+                      float(rng.uniform(-3, 3)), float(rng.choice([two_pi, rng.uniform(0.5, 6.0)]))]
+    return kind, [float(v) for v in rng.uniform(1.0, 8.0, 5)]
+
+
+def test_random_booleans(vg):
+    """Random operand kinds, parameters, operations and placements (all 25 kind pairs are specialised kernels)."""
+    rng = np.random.default_rng(4711)
+    pairs = set()
+    for rep in range(60):
+        ka, pa = _random_primitive(rng)
+        kb, pb = _random_primitive(rng)
+        op = int(rng.integers(0, 3))
+        q = rng.normal(size=4)
+        q /= np.linalg.norm(q)
+        off = tuple(float(v) for v in rng.uniform(-5, 5, 3))
+        bc = W.BooleanCase("random%d" % rep, op, ka, pa, kb, pb, off, tuple(q), 9100 + rep)
+        co, cg = build(vg, bc)
+        t = bc.tracks(20011, clear_of_both(co, bc))
+        dt = dev(t)
+        what = "%s %s%r %s%r @%r" % (W.OP_NAME[op], W.KIND_NAME[ka], pa, W.KIND_NAME[kb], pb, off)
+        assert_int_equal(cg.inside(*dt[:3]).cpu().numpy(), co.inside(*t[:3]), what)
+        assert_real_close(cg.distance_to_in(*dt, W.STEP_MAX).cpu().numpy(), co.distance_to_in(*t, W.STEP_MAX), what + " din")
+        assert_real_close(cg.distance_to_out(*dt, W.STEP_MAX).cpu().numpy(), co.distance_to_out(*t, W.STEP_MAX), what + " dout")
+        assert_real_close(cg.safety_to_in(*dt[:3]).cpu().numpy(), co.safety_to_in(*t[:3]), what + " safety")
+        pairs.add((ka, kb))
+    assert len(pairs) >= 20
