@@ -47,6 +47,8 @@ def _load(path):
     lib.orc_all_crossings.argtypes = [C.c_void_p] + [C.c_double] * 6 + [_P, C.c_int]
     lib.orc_world_create.restype = C.c_void_p
     lib.orc_world_create.argtypes = [C.c_int, C.POINTER(C.c_void_p), _PI, _P]
+    lib.orc_world_create_mixed.restype = C.c_void_p
+    lib.orc_world_create_mixed.argtypes = [C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), _PI, _P]
     lib.orc_world_destroy.argtypes = [C.c_void_p]
     lib.orc_world_locate.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _PI]
     lib.orc_world_step.argtypes = [C.c_void_p, _PI, _P, _P, _P, _P, _P, _P, C.c_double, C.c_int64, _P, _PI]
@@ -234,7 +236,7 @@ class Boolean:
 
 
 class World:
-    """Tree of placed solids (readings R22-R25, vg_oracle.c): node 0 is the root, `parents[i] < i`,
+    """Tree of placed solids (readings R22-R25, R30, vg_oracle.c; a node is a Shape or a Boolean): node 0 is the root, `parents[i] < i`,
     `xforms` is (nn, 12) row-major [R | b] from the parent's local frame (the world frame for the root)."""
 
     def __init__(self, shapes, parents, xforms):
@@ -243,8 +245,9 @@ class World:
         nn = len(self.shapes)
         self.parents = np.ascontiguousarray(np.asarray(parents, dtype=np.int32).reshape(nn))
         self.xforms = np.ascontiguousarray(np.asarray(xforms, dtype=np.float64).reshape(nn, 12))
-        arr = (C.c_void_p * nn)(*[s._h for s in self.shapes])
-        self._h = self._l.orc_world_create(nn, arr, self.parents.ctypes.data_as(_PI), _ptr(self.xforms))
+        arr = (C.c_void_p * nn)(*[None if isinstance(s, Boolean) else s._h for s in self.shapes])
+        barr = (C.c_void_p * nn)(*[s._h if isinstance(s, Boolean) else None for s in self.shapes])
+        self._h = self._l.orc_world_create_mixed(nn, arr, barr, self.parents.ctypes.data_as(_PI), _ptr(self.xforms))
         if not self._h:
             raise ValueError("oracle: invalid world")
 

@@ -698,18 +698,52 @@ void orc_volume_safety(const orc_volume *v, const double *x, const double *y, co
  *        i.e. orc_volume_safety in that node.
  */
 
+/* boolean solids are defined further down (R27-R29); a node may be one (R30: a node is any solid of this file, a
+ * primitive, a polycone or a boolean; with a boolean among a node and its children the node's safety inherits R29's
+ * "never over-estimates" in place of "exact") */
+typedef struct orc_boolean_s orc_boolean;
+static int bool_inside(const orc_boolean *c, const real p[3]);
+static real bool_sdf(const orc_boolean *c, const real p[3]);
+static real bool_cross(const orc_boolean *c, const real p[3], const real d[3]);
+
 typedef struct {
     int nn;
-    const orc_shape **shape;
+    const orc_shape **shape;     /* NULL where the node is a boolean */
+    const orc_boolean **boolean; /* NULL where the node is a plain solid */
     int32_t *parent;
     real *xf; /* nn * 12 */
 } orc_world;
 
-orc_world *orc_world_create(int nn, const orc_shape *const *shapes, const int32_t *parent, const double *xf)
+static int node_inside(const orc_world *w, int i, const real p[3])
+{
+    return w->boolean[i] ? bool_inside(w->boolean[i], p) : inside(w->shape[i], p[0], p[1], p[2]);
+}
+
+static real node_sdf(const orc_world *w, int i, const real p[3])
+{
+    return w->boolean[i] ? bool_sdf(w->boolean[i], p) : sdf(w->shape[i], p[0], p[1], p[2]);
+}
+
+static real node_distance_to_in(const orc_world *w, int i, const real p[3], const real d[3])
+{
+    if (!w->boolean[i]) return distance_to_in(w->shape[i], p, d, ORC_INF);
+    return bool_inside(w->boolean[i], p) == ORC_INSIDE ? (real)-1 : bool_cross(w->boolean[i], p, d);
+}
+
+static real node_distance_to_out(const orc_world *w, int i, const real p[3], const real d[3])
+{
+    if (!w->boolean[i]) return distance_to_out(w->shape[i], p, d, ORC_INF);
+    return bool_inside(w->boolean[i], p) == ORC_OUTSIDE ? (real)-1 : bool_cross(w->boolean[i], p, d);
+}
+
+/* exactly one of shapes[i], booleans[i] is given per node (booleans may be NULL: no boolean nodes) */
+orc_world *orc_world_create_mixed(int nn, const orc_shape *const *shapes, const orc_boolean *const *booleans,
+                                  const int32_t *parent, const double *xf)
 {
     if (nn < 1 || !shapes || !parent || !xf || parent[0] != -1) return NULL;
     for (int i = 0; i < nn; ++i) {
-        if (!shapes[i]) return NULL;
+        int nb = booleans && booleans[i];
+        if ((shapes[i] != NULL) == nb) return NULL;
         if (i > 0 && (parent[i] < 0 || parent[i] >= i)) return NULL;
     }
     if (!finite_all(xf, 12 * nn)) return NULL;
@@ -717,20 +751,28 @@ orc_world *orc_world_create(int nn, const orc_shape *const *shapes, const int32_
     if (!w) return NULL;
     w->nn = nn;
     w->shape = (const orc_shape **)calloc((size_t)nn, sizeof *w->shape);
+    w->boolean = (const orc_boolean **)calloc((size_t)nn, sizeof *w->boolean);
     w->parent = (int32_t *)calloc((size_t)nn, sizeof *w->parent);
     w->xf = (real *)calloc((size_t)nn * 12, sizeof *w->xf);
     for (int i = 0; i < nn; ++i) {
         w->shape[i] = shapes[i];
+        w->boolean[i] = booleans ? booleans[i] : NULL;
         w->parent[i] = parent[i];
         for (int k = 0; k < 12; ++k) w->xf[12 * i + k] = xf[12 * i + k];
     }
     return w;
 }
 
+orc_world *orc_world_create(int nn, const orc_shape *const *shapes, const int32_t *parent, const double *xf)
+{
+    return orc_world_create_mixed(nn, shapes, NULL, parent, xf);
+}
+
 void orc_world_destroy(orc_world *w)
 {
     if (!w) return;
     free((void *)w->shape);
+    free((void *)w->boolean);
     free(w->parent);
     free(w->xf);
     free(w);
@@ -752,7 +794,7 @@ void orc_world_locate(const orc_world *w, const double *x, const double *y, cons
     for (int64_t i = 0; i < n; ++i) {
         real p[3] = { x[i], y[i], z[i] }, d0[3] = { 0, 0, 0 }, pl[3], dl[3];
         to_local(w->xf, p, d0, pl, dl);
-        if (inside(w->shape[0], pl[0], pl[1], pl[2]) != ORC_INSIDE) { node[i] = -1; continue; }
+        if (node_inside(w, 0, pl) != ORC_INSIDE) { node[i] = -1; continue; }
         int cur = 0, moved = 1;
         while (moved) {
             moved = 0;
@@ -760,7 +802,7 @@ void orc_world_locate(const orc_world *w, const double *x, const double *y, cons
                 if (w->parent[c] != cur) continue;
                 real pc[3];
                 to_local(w->xf + 12 * c, pl, d0, pc, dl);
-                if (inside(w->shape[c], pc[0], pc[1], pc[2]) == ORC_INSIDE) {
+                if (node_inside(w, c, pc) == ORC_INSIDE) {
                     cur = c;
                     pl[0] = pc[0]; pl[1] = pc[1]; pl[2] = pc[2];
                     moved = 1;
@@ -783,13 +825,13 @@ void orc_world_step(const orc_world *w, const int32_t *node, const double *x, co
         if (nd < 0 || nd >= w->nn) { step[i] = -1; next[i] = -1; continue; }
         real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] }, pl[3], dl[3];
         world_to_node(w, nd, p, d, pl, dl);
-        real best = distance_to_out(w->shape[nd], pl, dl, ORC_INF);
+        real best = node_distance_to_out(w, nd, pl, dl);
         int32_t who = w->parent[nd];
         for (int c = nd + 1; c < w->nn; ++c) {
             if (w->parent[c] != nd) continue;
             real pc[3], dc[3];
             to_local(w->xf + 12 * c, pl, dl, pc, dc);
-            real t = distance_to_in(w->shape[c], pc, dc, ORC_INF);
+            real t = node_distance_to_in(w, c, pc, dc);
             if (t >= 0 && t < best) { best = t; who = c; }
         }
         if (best > step_max) { best = step_max; who = nd; }
@@ -808,12 +850,12 @@ void orc_world_safety(const orc_world *w, const int32_t *node, const double *x, 
         if (nd < 0 || nd >= w->nn) { out[i] = -1; continue; }
         real p[3] = { x[i], y[i], z[i] }, d0[3] = { 0, 0, 0 }, pl[3], dl[3];
         world_to_node(w, nd, p, d0, pl, dl);
-        real best = -sdf(w->shape[nd], pl[0], pl[1], pl[2]);
+        real best = -node_sdf(w, nd, pl);
         for (int c = nd + 1; c < w->nn; ++c) {
             if (w->parent[c] != nd) continue;
             real pc[3];
             to_local(w->xf + 12 * c, pl, d0, pc, dl);
-            best = rmin2(best, sdf(w->shape[c], pc[0], pc[1], pc[2]));
+            best = rmin2(best, node_sdf(w, c, pc));
         }
         out[i] = (double)best;
     }
@@ -840,11 +882,11 @@ void orc_world_safety(const orc_world *w, const int32_t *node, const double *x, 
 
 enum { ORC_UNION = 0, ORC_INTERSECTION = 1, ORC_SUBTRACTION = 2 };
 
-typedef struct {
+struct orc_boolean_s {
     int op;
     const orc_shape *a, *b;
     real xf[12];
-} orc_boolean;
+};
 
 orc_boolean *orc_boolean_create(int op, const orc_shape *a, const orc_shape *b, const double *xf)
 {

@@ -189,3 +189,85 @@ def test_world_create_rejects_bad_trees():
         O.World([b, b], [0, 0], [ident, ident])  # root must have parent -1
     with pytest.raises(ValueError):
         O.World([b, b], [-1, 1], [ident, ident])  # parent must come first
+
+
+# ------------------------------------------------- nodes that are polycones and booleans (reading R30)
+
+def build_mixed(mc, mod=O):
+    def mk(nd):
+        if nd[0] == "shape":
+            return mod.Shape(nd[1], nd[2])
+        b = nd[1]
+        return mod.Boolean(b.op, mod.Shape(b.kind_a, b.par_a), mod.Shape(b.kind_b, b.par_b), b.xform)
+    objs = [mk(nd) for nd in mc.nodes]
+    return objs, mod.World(objs, mc.parents, mc.xforms)
+
+
+@pytest.fixture(scope="module")
+def mixed():
+    mc = W.mixed_world_case()
+    objs, w = build_mixed(mc)
+
+    def band(x, y, z):
+        nd = w.locate(x, y, z)
+        return (nd < 0) | (w.safety(nd, x, y, z) < W.SURFACE_BAND)
+
+    return mc, objs, w, mc.tracks(60000, band)
+
+
+def test_mixed_world_locate_is_the_deepest_holder(mixed):
+    mc, objs, w, t = mixed
+    x, y, z = t[:3]
+    nn = len(objs)
+    G = np.zeros((nn, 4, 4))
+    for i in range(nn):
+        X = np.eye(4)
+        X[:3, :] = mc.xforms[i].reshape(3, 4)
+        G[i] = X if mc.parents[i] < 0 else X @ G[mc.parents[i]]
+    held = np.zeros((nn, x.size), dtype=bool)
+    for i in range(nn):
+        held[i] = objs[i].inside(*to_node(G, i, x, y, z)) == O.INSIDE
+        if i > 0:
+            held[i] &= held[mc.parents[i]]
+    expect = np.array([np.flatnonzero(held[:, j])[-1] for j in range(x.size)])
+    got = w.locate(x, y, z)
+    assert np.array_equal(got, expect)
+    counts = np.bincount(got, minlength=nn)
+    assert np.all(counts[1:9] > 100) and counts[9:].sum() > 5
+
+
+def test_mixed_world_step_and_safety_properties(mixed):
+    mc, objs, w, t = mixed
+    x, y, z, dx, dy, dz = t
+    node = w.locate(x, y, z)
+    step, nxt = w.step(node, x, y, z, dx, dy, dz)
+    assert np.all(step > 0) and np.all(np.isfinite(step))
+    eps = 1e-6
+    ok = step > 2 * eps
+    before = w.locate(x + (step - eps) * dx, y + (step - eps) * dy, z + (step - eps) * dz)
+    after = w.locate(x + (step + eps) * dx, y + (step + eps) * dy, z + (step + eps) * dz)
+    assert (before[ok] != node[ok]).mean() < 2e-3 and (after[ok] != nxt[ok]).mean() < 2e-3
+    for frac in (0.1, 0.5, 0.9):
+        mid = w.locate(x + frac * step * dx, y + frac * step * dy, z + frac * step * dz)
+        assert (mid != node).mean() < 1e-3
+    # safety: never beyond the step, and the ball of that radius stays in the node (probe 60 directions per point)
+    s = w.safety(node, x, y, z)
+    assert np.all(s >= W.SURFACE_BAND) and np.all(s <= step * (1 + 1e-12))
+    rng = np.random.default_rng(8)
+    sel = rng.choice(x.size, 3000, replace=False)
+    for _ in range(60):
+        v = rng.normal(size=3)
+        v /= np.linalg.norm(v)
+        r = s[sel] * (1 - 1e-9)
+        assert np.array_equal(w.locate(x[sel] + r * v[0], y[sel] + r * v[1], z[sel] + r * v[2]), node[sel])
+    # and no direction reaches a border sooner than the safety; in nodes without booleans (polycones, the orbs inside
+    # them) the safety is exact, so the nearest border over 4000 directions comes close to it for most points
+    idx = np.flatnonzero(np.isin(node, [1, 3, 5, 7, 9, 11]))[:200]
+    v = rng.normal(size=(3, 4000))
+    v /= np.linalg.norm(v, axis=0)
+    ratio = []
+    for j in idx:
+        tt, _ = w.step(np.full(4000, node[j], dtype=np.int32), np.full(4000, x[j]), np.full(4000, y[j]), np.full(4000, z[j]), v[0], v[1], v[2])
+        assert s[j] <= tt.min() * (1 + 1e-12)
+        ratio.append(tt.min() / s[j])
+    assert np.median(ratio) < 1.02

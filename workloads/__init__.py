@@ -263,7 +263,7 @@ class WorldCase:
             p = (2.0 * rng.random((m, 3)) - 1.0) * np.asarray(self.half)
             low = rng.random(m) < 0.5
             which = self.level1[rng.integers(0, len(self.level1), m)]
-            loc = (2.0 * rng.random((m, 3)) - 1.0) * 8.0
+            loc = (2.0 * rng.random((m, 3)) - 1.0) * getattr(self, "local_cube", 8.0)
             M = self.xforms[which].reshape(m, 3, 4)
             # local -> mother: p = R^T (p_loc - b)
             back = np.einsum("nji,nj->ni", M[:, :, :3], loc - M[:, :, 3])
@@ -338,3 +338,64 @@ def boolean_cases():
         BooleanCase("orb_minus_box", SUBTRACTION, ORB, [12.0], BOX, [9.0, 3.0, 20.0], (0.0, 2.0, 0.0), q[3], seed + 5),
         BooleanCase("tube_minus_cone", SUBTRACTION, TUBE, [0.0, 10.0, 10.0, 0.0, TWO_PI], CONE, [0.0, 2.0, 0.0, 9.0, 8.0, 0.5, 5.0], (0.0, 0.0, 3.0), q[0], seed + 6),
     ]
+
+
+class MixedWorldCase:
+    """A tree whose nodes are not only primitives (reading R30): the mother box (100) holds eight daughters at
+    (+-50, +-50, +-50) with seeded rotations -- two stepped polycones, two booleans box-minus-tube, two configs[3]
+    polycones, two booleans tube-union-box -- and a grand-daughter inside the material of each stepped polycone (an orb)
+    and of each box-minus-tube (a small box in a corner clear of the bore).  13 nodes.
+
+    `nodes[i]` is ("shape", kind, params) or ("boolean", BooleanCase); tracks as in WorldCase (half in the mother box,
+    half in the local cube [-14, 14]^3 of a random daughter)."""
+
+    def __init__(self, seed=None, n=1048576):
+        self.seed = (config_seed(4) + 23) if seed is None else seed
+        self.sizes = (n,)
+        self.center, self.half = (0.0, 0.0, 0.0), (100.0, 100.0, 100.0)
+        rng = _rng(self.seed)
+        bools = {b.name: b for b in boolean_cases()}
+        kinds4 = [("shape", POLYCONE, STEPPED_POLYCONE), ("boolean", bools["box_minus_tube"]),
+                  ("shape", POLYCONE, polycone_params(config_seed(3, 0))), ("boolean", bools["tube_union_box"])]
+        nodes, parents, xf = [("shape", BOX, [100.0, 100.0, 100.0])], [-1], [placement(np.eye(3), (0, 0, 0))]
+
+        def rot():
+            u1, u2, u3 = rng.random(3)
+            return quaternion_to_matrix((math.sqrt(1 - u1) * math.sin(TWO_PI * u2), math.sqrt(1 - u1) * math.cos(TWO_PI * u2),
+                                         math.sqrt(u1) * math.sin(TWO_PI * u3), math.sqrt(u1) * math.cos(TWO_PI * u3)))
+        k = 0
+        for sz in (-50.0, 50.0):
+            for sy in (-50.0, 50.0):
+                for sx in (-50.0, 50.0):
+                    nodes.append(kinds4[k % 4])
+                    parents.append(0)
+                    xf.append(placement(rot(), (sx, sy, sz)))
+                    k += 1
+        # the corner of box-minus-tube farthest from the bore: distance from the tube's axis (a line through the placement
+        # centre along R^T e_z in the boolean's frame)
+        M = np.asarray(bools["box_minus_tube"].xform).reshape(3, 4)
+        axis, centre = M[2, :3], -M[:, :3].T @ M[:, 3]
+        corners = [np.array([a, b, c]) for a in (-7.0, 7.0) for b in (-7.0, 7.0) for c in (-7.0, 7.0)]
+        corner = max(corners, key=lambda p: np.linalg.norm(np.cross(p - centre, axis)))
+        assert np.linalg.norm(np.cross(corner - centre, axis)) > 4.0 + 2.6 + 0.2
+        for i in range(1, 9):
+            kind = nodes[i]
+            if kind[0] == "shape" and kind[2] is STEPPED_POLYCONE:
+                nodes.append(("shape", ORB, [2.5]))
+                parents.append(i)
+                xf.append(placement(rot(), (7.0, 0.0, -1.0)))
+            elif kind[0] == "boolean" and kind[1].name == "box_minus_tube":
+                nodes.append(("shape", BOX, [1.5, 1.5, 1.5]))
+                parents.append(i)
+                xf.append(placement(rot(), tuple(corner)))
+        self.nodes = nodes
+        self.parents = np.asarray(parents, dtype=np.int32)
+        self.xforms = np.ascontiguousarray(np.stack(xf))
+        self.level1 = np.arange(1, 9)
+
+    tracks = WorldCase.tracks
+    local_cube = 14.0
+
+
+def mixed_world_case(**kw):
+    return MixedWorldCase(**kw)
