@@ -105,7 +105,7 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
  *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
  *                safeties it is not the exact distance everywhere (R29).
- * A boolean cannot be an operand, a daughter of a volume or a node of a world in this build.
+ * A boolean can be a node of a world (vg_world_create); it cannot be an operand or a daughter of a vg_volume in this build.
  */
 typedef enum { VG_UNION = 0, VG_INTERSECTION = 1, VG_SUBTRACTION = 2 } vg_bool_op;
 int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out);
@@ -179,7 +179,9 @@ int vg_volume_safety(const vg_volume *volume, const double *x, const double *y, 
  * `xforms` (HOST): nnodes * 12 doubles, row-major 3x4 [R | b] per node, from the PARENT's local frame to the
  * node's local frame (for the root: from the world frame), orthonormal R as for vg_volume_create.  The children of
  * a node are the nodes that name it as parent, in index order; siblings must not overlap and must lie inside
- * their parent (not checked).  Node kinds: box, orb, tube, cone, trd.  1 <= nnodes <= VG_MAX_NODES; a node has
+ * their parent (not checked).  A node may be any vg_shape: the five primitives, a polycone or a boolean (reading R30;
+ * worlds without polycone / boolean nodes run leaner kernels; with a boolean among a node and its children
+ * vg_world_safety inherits the boolean's "never over-estimates" in place of "exact").  1 <= nnodes <= VG_MAX_NODES; a node has
  * at most VG_MAX_DAUGHTERS children.  The shapes' constants are copied.  The node table lives in memory of the
  * device that is current at create time.
  */

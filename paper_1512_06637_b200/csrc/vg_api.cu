@@ -295,6 +295,36 @@ static double bounding_radius(const SolidU &s)
     }
 }
 
+// the same for any vg_shape, polycones and booleans included (world nodes, reading R30)
+static double shape_radius(const vg_shape *s)
+{
+    if (s->kind == VG_POLYCONE) {
+        const PolyconeP &c = s->u.pcon;
+        double zm = std::fmax(std::fabs(c.zlo), std::fabs(c.zhi));
+        return std::sqrt(c.rb2 + zm * zm);
+    }
+    if (s->kind == VG_BOOLEAN) {
+        const BoolP &c = s->u.boolean;
+        double ra = bounding_radius(c.a);
+        if (c.op != kUnion) return ra; // an intersection and a subtraction lie inside A
+        const double *m = c.X;         // centre of B in the frame of C: -R^T b
+        double cx = -(m[0] * m[3] + m[4] * m[7] + m[8] * m[11]), cy = -(m[1] * m[3] + m[5] * m[7] + m[9] * m[11]),
+               cz = -(m[2] * m[3] + m[6] * m[7] + m[10] * m[11]);
+        return std::fmax(ra, std::sqrt(cx * cx + cy * cy + cz * cz) + bounding_radius(c.b));
+    }
+    SolidU u;
+    std::memset(&u, 0, sizeof u);
+    u.kind = s->kind;
+    switch (s->kind) {
+    case VG_BOX: u.u.box = s->u.box; break;
+    case VG_ORB: u.u.orb = s->u.orb; break;
+    case VG_TUBE: u.u.tube = s->u.tube; break;
+    case VG_CONE: u.u.cone = s->u.cone; break;
+    default: u.u.trd = s->u.trd; break;
+    }
+    return bounding_radius(u);
+}
+
 static int to_solid(const vg_shape *s, SolidU *o, const char *what)
 {
     std::memset(o, 0, sizeof *o);
@@ -444,9 +474,8 @@ extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const doubl
 
 struct vg_world {
     int nn;
-    WorldNode *nodes_dev; // one allocation: nn WorldNode records, the FP32 cull spheres and the child lists (int32)
-    float4 *cull_dev;     // one float4 {cx, cy, cz, r2} per child-list entry, same order as kids_dev
-    int32_t *kids_dev;
+    WorldTab tab;          // device pointers into ONE allocation: node records, FP32 cull spheres, child lists, then the
+    unsigned char *blob;   // polycone and boolean constants of the nodes that are not primitives (reading R30)
     int device;
 };
 
@@ -509,6 +538,9 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     std::vector<WorldNode> nodes(nn);
     std::vector<int32_t> kids(nn > 1 ? nn - 1 : 1, 0);
     std::vector<int> count(nn, 0), fill(nn, 0);
+    std::vector<PolyconeP> pcons;
+    std::vector<BoolP> bools;
+    std::vector<double> radius(nn, 0.0);
     for (int i = 1; i < nn; ++i) {
         if (parent[i] < 0 || parent[i] >= i) return fail(VG_ERR_PARAM, "%s: need 0 <= parent[%d] < %d", fn, i, i);
         if (++count[parent[i]] > VG_MAX_DAUGHTERS)
@@ -521,8 +553,19 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         const double *m = xforms + 12 * i;
         if (!all_finite(m, 12)) return fail(VG_ERR_PARAM, "%s: non-finite transform of node %d", fn, i);
         if (!rigid(m)) return fail(VG_ERR_PARAM, "%s: rotation of node %d is not orthonormal", fn, i);
-        int rc = to_solid(shapes[i], &N.s, "node");
-        if (rc != VG_OK) return rc;
+        if (shapes[i]->kind == VG_POLYCONE) { // R30: constants in a side array, the record keeps kind + index
+            N.s.kind = kPolycone;
+            N.ext = int(pcons.size());
+            pcons.push_back(shapes[i]->u.pcon);
+        } else if (shapes[i]->kind == VG_BOOLEAN) {
+            N.s.kind = kBoolean;
+            N.ext = int(bools.size());
+            bools.push_back(shapes[i]->u.boolean);
+        } else {
+            int rc = to_solid(shapes[i], &N.s, "node");
+            if (rc != VG_OK) return rc;
+        }
+        radius[i] = shape_radius(shapes[i]);
         std::memcpy(N.X, m, sizeof N.X);
         if (i == 0) std::memcpy(N.G, m, sizeof N.G);
         else compose(m, nodes[parent[i]].G, N.G);
@@ -540,8 +583,8 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         double cx = -(m[0] * m[3] + m[4] * m[7] + m[8] * m[11]);
         double cy = -(m[1] * m[3] + m[5] * m[7] + m[9] * m[11]);
         double cz = -(m[2] * m[3] + m[6] * m[7] + m[10] * m[11]);
-        double r = bounding_radius(N.s);
-        double rp = i > 0 ? bounding_radius(nodes[parent[i]].s) : r;
+        double r = radius[i];
+        double rp = i > 0 ? radius[parent[i]] : r;
         double S = rp + std::sqrt(cx * cx + cy * cy + cz * cz) + r;
         N.bs[0] = cx, N.bs[1] = cy, N.bs[2] = cz;
         N.bs[3] = r * r * (1.0 + 1e-9) + 1e-12 * S * S;
@@ -553,8 +596,8 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     for (int p = 0; p < nn; ++p)
         for (int j = 0; j < nodes[p].nchild; ++j) {
             const WorldNode &N = nodes[kids[nodes[p].child0 + j]];
-            const double r = bounding_radius(N.s);
-            const double S = bounding_radius(nodes[p].s) + std::sqrt(N.bs[0] * N.bs[0] + N.bs[1] * N.bs[1] + N.bs[2] * N.bs[2]) + r;
+            const double r = radius[kids[nodes[p].child0 + j]];
+            const double S = radius[p] + std::sqrt(N.bs[0] * N.bs[0] + N.bs[1] * N.bs[1] + N.bs[2] * N.bs[2]) + r;
             const double r2 = r * r * (1.0 + 1e-6) + 64.0 * std::ldexp(1.0, -24) * S * S;
             float *e = &cull[4 * size_t(nodes[p].child0 + j)];
             e[0] = float(N.bs[0]), e[1] = float(N.bs[1]), e[2] = float(N.bs[2]), e[3] = std::nextafterf(float(r2), INFINITY);
@@ -563,22 +606,33 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     if (!w) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
     std::memset(w, 0, sizeof *w);
     w->nn = nn;
-    const size_t nbytes = size_t(nn) * sizeof(WorldNode), cbytes = cull.size() * sizeof(float), kbytes = kids.size() * sizeof(int32_t);
+    auto up16 = [](size_t v) { return (v + 15) / 16 * 16; };
+    const size_t nbytes = size_t(nn) * sizeof(WorldNode), cbytes = cull.size() * sizeof(float), kbytes = up16(kids.size() * sizeof(int32_t));
+    const size_t pbytes = up16(pcons.size() * sizeof(PolyconeP)), bbytes = bools.size() * sizeof(BoolP);
     static_assert(sizeof(WorldNode) % 16 == 0, "the float4 array follows the node records");
     unsigned char *blob = nullptr;
     cudaError_t e = cudaGetDevice(&w->device);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + cbytes + kbytes);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + cbytes + kbytes + pbytes + bbytes + 16);
     if (e == cudaSuccess) e = cudaMemcpy(blob, nodes.data(), nbytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes, cull.data(), cbytes, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes + cbytes, kids.data(), kbytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes + cbytes, kids.data(), kids.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !pcons.empty())
+        e = cudaMemcpy(blob + nbytes + cbytes + kbytes, pcons.data(), pcons.size() * sizeof(PolyconeP), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !bools.empty())
+        e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes, bools.data(), bbytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         if (blob) cudaFree(blob);
         delete w;
         return fail_cuda(e, fn);
     }
-    w->nodes_dev = reinterpret_cast<WorldNode *>(blob);
-    w->cull_dev = reinterpret_cast<float4 *>(blob + nbytes);
-    w->kids_dev = reinterpret_cast<int32_t *>(blob + nbytes + cbytes);
+    w->blob = blob;
+    w->tab.nodes = reinterpret_cast<WorldNode *>(blob);
+    w->tab.cull = reinterpret_cast<float4 *>(blob + nbytes);
+    w->tab.kids = reinterpret_cast<int32_t *>(blob + nbytes + cbytes);
+    w->tab.pcons = reinterpret_cast<PolyconeP *>(blob + nbytes + cbytes + kbytes);
+    w->tab.bools = reinterpret_cast<BoolP *>(blob + nbytes + cbytes + kbytes + pbytes);
+    w->tab.nnodes = nn;
+    w->tab.has_ext = !(pcons.empty() && bools.empty());
     *out = w;
     return VG_OK;
 }
@@ -586,7 +640,7 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
 extern "C" void vg_world_destroy(vg_world *w)
 {
     if (!w) return;
-    if (w->nodes_dev) cudaFree(w->nodes_dev);
+    if (w->blob) cudaFree(w->blob);
     delete w;
 }
 
@@ -600,7 +654,7 @@ extern "C" int vg_world_locate(const vg_world *w, const double *x, const double 
     int rc = check_arrays(fn, ptrs, 3, 4, node, n, &vec);
     if (rc != VG_OK || n == 0) return rc;
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
-    cudaError_t e = launch_world_locate(w->nodes_dev, w->kids_dev, w->cull_dev, t, n, node, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_world_locate(w->tab, t, n, node, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }
@@ -618,7 +672,7 @@ extern "C" int vg_world_step(const vg_world *w, const int32_t *node, const doubl
     if (!node || !aligned(node, 4) || !next || !aligned(next, 4)) return fail(VG_ERR_ARG, "%s: node / next array NULL or misaligned", fn);
     if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
     Tracks t{ x, y, z, dx, dy, dz };
-    cudaError_t e = launch_world_step(w->nodes_dev, w->kids_dev, w->cull_dev, w->nn, node, t, step_max, n, step, next,
+    cudaError_t e = launch_world_step(w->tab, node, t, step_max, n, step, next,
                                       static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
@@ -635,7 +689,7 @@ extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const dou
     if (rc != VG_OK || n == 0) return rc;
     if (!node || !aligned(node, 4)) return fail(VG_ERR_ARG, "%s: node array NULL or misaligned", fn);
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
-    cudaError_t e = launch_world_safety(w->nodes_dev, w->kids_dev, w->cull_dev, w->nn, node, t, n, safety, static_cast<cudaStream_t>(stream));
+    cudaError_t e = launch_world_safety(w->tab, node, t, n, safety, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }

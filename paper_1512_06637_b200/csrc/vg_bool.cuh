@@ -60,6 +60,62 @@ VG_DEV int bool_classify(int op, int ca, int cb)
     return classify(in, out);
 }
 
+// ---- the three answers as device functions (the kernel below and the world kernels of vg_world.cu call them) ----
+
+VG_DEV void bool_to_b(const BoolP &p, double x, double y, double z, double &bx, double &by, double &bz)
+{
+    const double *m = p.X;
+    bx = fma(m[0], x, fma(m[1], y, fma(m[2], z, m[3])));
+    by = fma(m[4], x, fma(m[5], y, fma(m[6], z, m[7])));
+    bz = fma(m[8], x, fma(m[9], y, fma(m[10], z, m[11])));
+}
+
+VG_DEV int bool_inside_pt(const BoolP &p, double x, double y, double z) // R27
+{
+    double bx, by, bz;
+    bool_to_b(p, x, y, z, bx, by, bz);
+    return bool_classify(p.op, solid_inside(p.a, x, y, z), solid_inside(p.b, bx, by, bz));
+}
+
+VG_DEV double bool_sdf_pt(const BoolP &p, double x, double y, double z) // R29
+{
+    double bx, by, bz;
+    bool_to_b(p, x, y, z, bx, by, bz);
+    const double sa = solid_sdf(p.a, x, y, z), sb = solid_sdf(p.b, bx, by, bz);
+    return p.op == kUnion ? dmin(sa, sb) : (p.op == kIntersection ? dmax(sa, sb) : dmax(sa, -sb));
+}
+
+// R28: DistanceToIn (to_out = false) or DistanceToOut (true): -1 on the wrong side, +inf if the membership never changes
+template <int KA, int KB>
+VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, double z, double dx, double dy, double dz)
+{
+    const double *m = p.X;
+    double bx, by, bz;
+    bool_to_b(p, x, y, z, bx, by, bz);
+    const int ca = solid_inside(p.a, x, y, z), cb = solid_inside(p.b, bx, by, bz);
+    const int cls = bool_classify(p.op, ca, cb);
+    if ((!to_out && cls == cInside) || (to_out && cls == cOutside)) return -1.0;
+    const double bdx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
+    const double bdy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
+    const double bdz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
+    bool ina = ca == cInside, inb = cb == cInside;
+    const bool start = bool_member(p.op, ina, inb);
+    double tt = 0.0;
+#pragma unroll 1
+    for (int it = 0; it < kBoolMaxEvents; ++it) {
+        const double ea = solid_next<KA>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
+        const double eb = solid_next<KB>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
+        const bool a_first = ea <= eb; // a tie goes to A, as in the oracle's merge
+        const double e = a_first ? ea : eb;
+        if (!(e < inf())) break;
+        tt += e;
+        ina = a_first ? !ina : ina;
+        inb = a_first ? inb : !inb;
+        if (bool_member(p.op, ina, inb) != start) return tt;
+    }
+    return inf();
+}
+
 #ifndef VG_BOOL_MINB
 #define VG_BOOL_MINB 3
 #endif
@@ -68,59 +124,20 @@ template <int Q, int KA, int KB>
 __global__ void __launch_bounds__(kBoolBlock, (Q == qDistIn || Q == qDistOut) ? VG_BOOL_MINB : 1)
     bool_kernel(const __grid_constant__ BoolP p, Tracks t, double step_max, int64_t n, void *out)
 {
-    constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
     pdl_launch_dependents();
     pdl_wait();
     const int64_t i = int64_t(blockIdx.x) * kBoolBlock + threadIdx.x;
     if (i >= n) return;
     const double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
-    const double *m = p.X;
-    const double bx = fma(m[0], x, fma(m[1], y, fma(m[2], z, m[3])));
-    const double by = fma(m[4], x, fma(m[5], y, fma(m[6], z, m[7])));
-    const double bz = fma(m[8], x, fma(m[9], y, fma(m[10], z, m[11])));
-    if (Q == qSafeIn || Q == qSafeOut) { // R29
-        const double sa = solid_sdf(p.a, x, y, z), sb = solid_sdf(p.b, bx, by, bz);
-        const double s = p.op == kUnion ? dmin(sa, sb) : (p.op == kIntersection ? dmax(sa, sb) : dmax(sa, -sb));
+    if (Q == qSafeIn || Q == qSafeOut) {
+        const double s = bool_sdf_pt(p, x, y, z);
         stg1(static_cast<double *>(out) + i, Q == qSafeIn ? s : -s);
-        return;
-    }
-    const int ca = solid_inside(p.a, x, y, z), cb = solid_inside(p.b, bx, by, bz);
-    const int cls = bool_classify(p.op, ca, cb); // R27
-    if (Q == qInside) {
-        stg1i(static_cast<int32_t *>(out) + i, cls);
-        return;
-    }
-    if (kDir) { // R28
+    } else if (Q == qInside) {
+        stg1i(static_cast<int32_t *>(out) + i, bool_inside_pt(p, x, y, z));
+    } else {
         const double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
-        const double bdx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
-        const double bdy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
-        const double bdz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
-        double res;
-        if ((Q == qDistIn && cls == cInside) || (Q == qDistOut && cls == cOutside)) {
-            res = -1.0;
-        } else {
-            bool ina = ca == cInside, inb = cb == cInside;
-            const bool start = bool_member(p.op, ina, inb);
-            double tt = 0.0;
-            res = inf();
-#pragma unroll 1
-            for (int it = 0; it < kBoolMaxEvents; ++it) {
-                const double ea = solid_next<KA>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
-                const double eb = solid_next<KB>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
-                const bool a_first = ea <= eb; // a tie goes to A, as in the oracle's merge
-                const double e = a_first ? ea : eb;
-                if (!(e < inf())) break;
-                tt += e;
-                ina = a_first ? !ina : ina;
-                inb = a_first ? inb : !inb;
-                if (bool_member(p.op, ina, inb) != start) {
-                    res = tt;
-                    break;
-                }
-            }
-            res = res <= step_max ? res : inf();
-        }
-        stg1(static_cast<double *>(out) + i, res);
+        const double r = bool_distance<KA, KB>(p, Q == qDistOut, x, y, z, dx, dy, dz);
+        stg1(static_cast<double *>(out) + i, r <= step_max ? r : inf());
     }
 }
 

@@ -580,12 +580,10 @@ cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *tabl
 cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
 
 // hierarchy of volumes (vg_world.cu)
-cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const float4 *cull, const Tracks &t, int64_t n, int32_t *out,
-                                cudaStream_t s);
-cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
-                              double step_max, int64_t n, double *step, int32_t *next, cudaStream_t s);
-cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
-                                int64_t n, double *safety, cudaStream_t s);
+cudaError_t launch_world_locate(const WorldTab &w, const Tracks &t, int64_t n, int32_t *out, cudaStream_t s);
+cudaError_t launch_world_step(const WorldTab &w, const int32_t *node, const Tracks &t, double step_max, int64_t n, double *step,
+                              int32_t *next, cudaStream_t s);
+cudaError_t launch_world_safety(const WorldTab &w, const int32_t *node, const Tracks &t, int64_t n, double *safety, cudaStream_t s);
 
 // probes (vg_probe.cu)
 cudaError_t probe_fp64_fma_rate(int launches, double *fma_per_s, cudaStream_t s);

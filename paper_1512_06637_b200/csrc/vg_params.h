@@ -3,6 +3,7 @@
 // warp-uniform operands cost no instruction and no register).
 #pragma once
 #include <stdint.h>
+#include <vector_types.h> // float4
 
 namespace vg {
 
@@ -166,7 +167,19 @@ struct alignas(16) WorldNode {
     double bs[4];   // bounding sphere in the PARENT's local frame: centre, squared radius inflated by the rounding bound
     double br;      // its radius (inflated), for the safety cull
     SolidU s;
-    int parent, child0, nchild, pad; // children: child_list[child0 .. child0 + nchild), ascending node index
+    int parent, child0, nchild; // children: child_list[child0 .. child0 + nchild), ascending node index
+    int ext;                    // s.kind == kPolycone / kBoolean: index into the world's polycone / boolean array
+};
+
+// everything a world kernel needs, by value in kernel-parameter space
+struct WorldTab {
+    const WorldNode *nodes;
+    const int32_t *kids;          // the child lists
+    const float4 *cull;           // FP32 bounding spheres in child-list order
+    const struct PolyconeP *pcons; // nodes that are polycones (reading R30)
+    const struct BoolP *bools;     // nodes that are booleans
+    int nnodes;
+    int has_ext;                   // any polycone / boolean node: the kernels with their code are launched
 };
 
 } // namespace vg

@@ -1,6 +1,6 @@
 // vg_world.cu -- queries over a tree of placed solids ("with hierarchical connections one can build the
 // whole detector"; PAPER.md:98 the particle "is transported to the border" and changes volume; SURVEY.md sec. 8(f) f3;
-// readings R22-R25 in DESIGN.md): Locate, Step (one-level ComputeStep in each track's own node + the node entered)
+// readings R22-R25, R30 in DESIGN.md): Locate, Step (one-level ComputeStep in each track's own node + the node entered)
 // and the per-node safety.
 //
 // Design: one thread per track; the node table (vg_params.h WorldNode, ~0.5 KiB per node) stays in global memory and
@@ -13,8 +13,7 @@
 // child's DistanceToIn is +inf, its Inside is OUTSIDE and its SafetyToIn exceeds the running minimum, i.e. results
 // are identical to visiting every child.  Children are visited in ascending node index, so the strict `<` scan is
 // the tie-break of R13.
-#include "vg_kernels.cuh"
-#include "vg_solid.cuh"
+#include "vg_bool.cuh"
 
 namespace vg {
 
@@ -34,10 +33,55 @@ VG_DEV void xf_dir(const double *m, double dx, double dy, double dz, double &lx,
     lz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
 }
 
-__global__ void __launch_bounds__(kWorldBlock)
-    world_locate_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids,
-                        const float4 *__restrict__ cull, Tracks t, int64_t n, int32_t *__restrict__ out)
+// ---- a node's solid: the five placeable primitives inline; polycones and booleans (reading R30) live in side arrays and
+// are reached through calls that are NOT inlined, so that the common path keeps its registers ----
+
+__device__ __noinline__ int ext_inside(const WorldTab &w, const WorldNode &N, double x, double y, double z)
 {
+    return N.s.kind == kPolycone ? Polycone::inside(w.pcons[N.ext], x, y, z) : bool_inside_pt(w.bools[N.ext], x, y, z);
+}
+
+__device__ __noinline__ double ext_sdf(const WorldTab &w, const WorldNode &N, double x, double y, double z)
+{
+    return N.s.kind == kPolycone ? Polycone::safety(w.pcons[N.ext], x, y, z) : bool_sdf_pt(w.bools[N.ext], x, y, z);
+}
+
+__device__ __noinline__ double ext_distance(const WorldTab &w, const WorldNode &N, bool to_out, double x, double y, double z,
+                                            double dx, double dy, double dz)
+{
+    if (N.s.kind == kPolycone)
+        return to_out ? Polycone::dist_out(w.pcons[N.ext], x, y, z, dx, dy, dz) : Polycone::dist_in(w.pcons[N.ext], x, y, z, dx, dy, dz);
+    return bool_distance<-1, -1>(w.bools[N.ext], to_out, x, y, z, dx, dy, dz);
+}
+
+template <bool EXT> VG_DEV int node_inside(const WorldTab &w, const WorldNode &N, double x, double y, double z)
+{
+    return (!EXT || N.s.kind < kPolycone) ? solid_inside(N.s, x, y, z) : ext_inside(w, N, x, y, z);
+}
+
+template <bool EXT> VG_DEV double node_sdf(const WorldTab &w, const WorldNode &N, double x, double y, double z)
+{
+    return (!EXT || N.s.kind < kPolycone) ? solid_sdf(N.s, x, y, z) : ext_sdf(w, N, x, y, z);
+}
+
+template <bool EXT> VG_DEV double node_dist_in(const WorldTab &w, const WorldNode &N, double x, double y, double z, double dx, double dy, double dz)
+{
+    return (!EXT || N.s.kind < kPolycone) ? solid_dist_in(N.s, x, y, z, dx, dy, dz) : ext_distance(w, N, false, x, y, z, dx, dy, dz);
+}
+
+template <bool EXT> VG_DEV double node_dist_out(const WorldTab &w, const WorldNode &N, double x, double y, double z, double dx, double dy, double dz)
+{
+    return (!EXT || N.s.kind < kPolycone) ? solid_dist_out(N.s, x, y, z, dx, dy, dz) : ext_distance(w, N, true, x, y, z, dx, dy, dz);
+}
+
+// EXT: the world holds polycone / boolean nodes (their code costs registers: primitive-only worlds run the lean instantiation)
+template <bool EXT>
+__global__ void __launch_bounds__(kWorldBlock)
+    world_locate_kernel(const __grid_constant__ WorldTab w, Tracks t, int64_t n, int32_t *__restrict__ out)
+{
+    const WorldNode *__restrict__ nodes = w.nodes;
+    const int32_t *__restrict__ kids = w.kids;
+    const float4 *__restrict__ cull = w.cull;
     pdl_launch_dependents();
     pdl_wait();
     const int64_t i = int64_t(blockIdx.x) * kWorldBlock + threadIdx.x;
@@ -45,7 +89,7 @@ __global__ void __launch_bounds__(kWorldBlock)
     double x, y, z;
     xf_point(nodes[0].X, ldg1(t.x + i), ldg1(t.y + i), ldg1(t.z + i), x, y, z);
     int cur = -1;
-    if (solid_inside(nodes[0].s, x, y, z) == cInside) {
+    if (node_inside<EXT>(w, nodes[0], x, y, z) == cInside) {
         cur = 0;
         bool moved = true;
         while (moved) {
@@ -67,7 +111,7 @@ __global__ void __launch_bounds__(kWorldBlock)
                     const WorldNode &C = nodes[c];
                     double lx, ly, lz;
                     xf_point(C.X, x, y, z, lx, ly, lz);
-                    if (solid_inside(C.s, lx, ly, lz) == cInside) {
+                    if (node_inside<EXT>(w, C, lx, ly, lz) == cInside) {
                         cur = c;
                         x = lx, y = ly, z = lz;
                         moved = true;
@@ -81,12 +125,15 @@ __global__ void __launch_bounds__(kWorldBlock)
 }
 
 // kStep: Step (R24); else the per-node safety (R25)
-template <bool kStep>
+template <bool kStep, bool EXT>
 __global__ void __launch_bounds__(kWorldBlock)
-    world_node_kernel(const WorldNode *__restrict__ nodes, const int32_t *__restrict__ kids,
-                      const float4 *__restrict__ cull, int nnodes, const int32_t *__restrict__ node, Tracks t, double step_max, int64_t n, double *__restrict__ out,
-                      int32_t *__restrict__ next)
+    world_node_kernel(const __grid_constant__ WorldTab w, const int32_t *__restrict__ node, Tracks t, double step_max,
+                      int64_t n, double *__restrict__ out, int32_t *__restrict__ next)
 {
+    const WorldNode *__restrict__ nodes = w.nodes;
+    const int32_t *__restrict__ kids = w.kids;
+    const float4 *__restrict__ cull = w.cull;
+    const int nnodes = w.nnodes;
     pdl_launch_dependents();
     pdl_wait();
     const int64_t i = int64_t(blockIdx.x) * kWorldBlock + threadIdx.x;
@@ -103,7 +150,7 @@ __global__ void __launch_bounds__(kWorldBlock)
     if (kStep) xf_dir(N.G, ldg1(t.dx + i), ldg1(t.dy + i), ldg1(t.dz + i), dx, dy, dz);
     const int c0 = N.child0, nc = N.nchild;
     if (kStep) {
-        double best = solid_dist_out(N.s, x, y, z, dx, dy, dz);
+        double best = node_dist_out<EXT>(w, N, x, y, z, dx, dy, dz);
         int who = N.parent;
         const float xf = float(x), yf = float(y), zf = float(z), dxf = float(dx), dyf = float(dy), dzf = float(dz);
         for (int base = 0; base < nc; base += 64) {
@@ -126,7 +173,7 @@ __global__ void __launch_bounds__(kWorldBlock)
                 double lx, ly, lz, ldx, ldy, ldz;
                 xf_point(C.X, x, y, z, lx, ly, lz);
                 xf_dir(C.X, dx, dy, dz, ldx, ldy, ldz);
-                const double tk = solid_dist_in(C.s, lx, ly, lz, ldx, ldy, ldz);
+                const double tk = node_dist_in<EXT>(w, C, lx, ly, lz, ldx, ldy, ldz);
                 const bool take = tk >= 0.0 && tk < best;
                 best = take ? tk : best;
                 who = take ? c : who;
@@ -136,7 +183,7 @@ __global__ void __launch_bounds__(kWorldBlock)
         stg1(out + i, phys ? step_max : best);
         stg1i(next + i, phys ? nd : who);
     } else {
-        double best = -solid_sdf(N.s, x, y, z);
+        double best = -node_sdf<EXT>(w, N, x, y, z);
         // SafetyToIn of a child >= |p - c| - r.  Phase 1, FP32: children whose bound can undercut the node's own
         // SafetyToOut (the spheres carry the FP32 error bound, see vg_world_create); a point outside its node (best <= 0)
         // is outside every child, whose SafetyToIn is then positive and never the minimum.  Phase 2, FP64: the same
@@ -162,36 +209,37 @@ __global__ void __launch_bounds__(kWorldBlock)
                 if (vv > reach * reach * (1.0 + 1e-9)) continue;
                 double lx, ly, lz;
                 xf_point(C.X, x, y, z, lx, ly, lz);
-                best = dmin(best, solid_sdf(C.s, lx, ly, lz));
+                best = dmin(best, node_sdf<EXT>(w, C, lx, ly, lz));
             }
         }
         stg1(out + i, best);
     }
 }
 
-cudaError_t launch_world_locate(const WorldNode *nodes, const int32_t *kids, const float4 *cull, const Tracks &t, int64_t n, int32_t *out,
-                                cudaStream_t s)
+cudaError_t launch_world_locate(const WorldTab &w, const Tracks &t, int64_t n, int32_t *out, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
-    return launch_kernel(world_locate_kernel, grid, kWorldBlock, 0, s, nodes, kids, cull, t, n, out);
+    return w.has_ext ? launch_kernel(world_locate_kernel<true>, grid, kWorldBlock, 0, s, w, t, n, out)
+                     : launch_kernel(world_locate_kernel<false>, grid, kWorldBlock, 0, s, w, t, n, out);
 }
 
-cudaError_t launch_world_step(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
-                              double step_max, int64_t n, double *step, int32_t *next, cudaStream_t s)
+cudaError_t launch_world_step(const WorldTab &w, const int32_t *node, const Tracks &t, double step_max, int64_t n, double *step,
+                              int32_t *next, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
-    return launch_kernel(world_node_kernel<true>, grid, kWorldBlock, 0, s, nodes, kids, cull, nnodes, node, t, step_max, n, step, next);
+    return w.has_ext ? launch_kernel(world_node_kernel<true, true>, grid, kWorldBlock, 0, s, w, node, t, step_max, n, step, next)
+                     : launch_kernel(world_node_kernel<true, false>, grid, kWorldBlock, 0, s, w, node, t, step_max, n, step, next);
 }
 
-cudaError_t launch_world_safety(const WorldNode *nodes, const int32_t *kids, const float4 *cull, int nnodes, const int32_t *node, const Tracks &t,
-                                int64_t n, double *safety, cudaStream_t s)
+cudaError_t launch_world_safety(const WorldTab &w, const int32_t *node, const Tracks &t, int64_t n, double *safety, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kWorldBlock - 1) / kWorldBlock);
     int32_t *none = nullptr;
-    return launch_kernel(world_node_kernel<false>, grid, kWorldBlock, 0, s, nodes, kids, cull, nnodes, node, t, 0.0, n, safety, none);
+    return w.has_ext ? launch_kernel(world_node_kernel<false, true>, grid, kWorldBlock, 0, s, w, node, t, 0.0, n, safety, none)
+                     : launch_kernel(world_node_kernel<false, false>, grid, kWorldBlock, 0, s, w, node, t, 0.0, n, safety, none);
 }
 
 } // namespace vg

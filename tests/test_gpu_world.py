@@ -111,9 +111,6 @@ def test_world_create_rejects_bad_input(vg):
         vg.World([b, b], [-1, 1], [ident, ident])
     with pytest.raises(vg.VgError):
         vg.World([b, b], [-1, 0], [ident, [2, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]])
-    pc = vg.Shape(W.POLYCONE, W.polycone_params(1))
-    with pytest.raises(vg.VgError):
-        vg.World([b, pc], [-1, 0], [ident, ident])
     w = vg.World([b], [-1], [ident])
     x = torch.zeros(5, dtype=torch.float64, device="cuda")
     assert w.locate(x, x, x).tolist() == [0] * 5
@@ -137,3 +134,61 @@ def test_full_size_as_benchmarked_on_sampled_tracks(vg, worlds):
     assert_real_close(safe_g.cpu().numpy()[sel], wo.safety(node_o, *ts[:3]), "full-size safety")
     # a property that holds for every track: the safety never exceeds the step
     assert bool((safe_g <= step_g * (1 + 1e-12)).all())
+
+
+# ------------------------------------------------- nodes that are polycones and booleans (reading R30)
+
+def _build_mixed(mod, mc):
+    def mk(nd):
+        if nd[0] == "shape":
+            return mod.Shape(nd[1], nd[2])
+        b = nd[1]
+        return mod.Boolean(b.op, mod.Shape(b.kind_a, b.par_a), mod.Shape(b.kind_b, b.par_b), b.xform)
+    objs = [mk(nd) for nd in mc.nodes]
+    return objs, mod.World(objs, mc.parents, mc.xforms)
+
+
+@pytest.fixture(scope="module")
+def mixed_worlds(vg):
+    mc = W.mixed_world_case()
+    objs_o, wo = _build_mixed(O, mc)
+    objs_g, wg = _build_mixed(vg, mc)
+    # clear of every surface of every node AND of every boolean operand (the state machine's contract, R7)
+    G = np.zeros((len(mc.nodes), 4, 4))
+    for i in range(len(mc.nodes)):
+        X = np.eye(4)
+        X[:3, :] = mc.xforms[i].reshape(3, 4)
+        G[i] = X if mc.parents[i] < 0 else X @ G[mc.parents[i]]
+
+    def band(x, y, z):
+        nd = wo.locate(x, y, z)
+        bad = (nd < 0) | (wo.safety(np.maximum(nd, 0), x, y, z) < W.SURFACE_BAND)
+        P = np.stack([x, y, z, np.ones_like(x)])
+        for i, o in enumerate(objs_o):
+            if isinstance(o, O.Boolean):
+                L = G[i] @ P
+                B = np.asarray(o.xform).reshape(3, 4)
+                LB = B[:, :3] @ L[:3] + B[:, 3:4]
+                bad |= (np.abs(o.a.sdf(L[0], L[1], L[2])) < W.SURFACE_BAND) | (np.abs(o.b.sdf(LB[0], LB[1], LB[2])) < W.SURFACE_BAND)
+        return bad
+
+    return mc, wo, wg, band
+
+
+@pytest.mark.parametrize("n", [1, 4099, 400003])
+def test_mixed_world_matches_the_oracle(vg, mixed_worlds, n):
+    mc, wo, wg, band = mixed_worlds
+    t = mc.tracks(n, band)
+    dt = dev(t)
+    node_o = wo.locate(*t[:3])
+    node_g = wg.locate(*dt[:3])
+    assert_int_equal(node_g.cpu().numpy(), node_o, "mixed world locate n=%d" % n)
+    for step_max in (W.STEP_MAX, 9.0):
+        so, no = wo.step(node_o, *t, step_max)
+        sg, ng = wg.step(node_g, *dt, step_max)
+        assert_int_equal(ng.cpu().numpy(), no, "mixed world next n=%d" % n)
+        assert_real_close(sg.cpu().numpy(), so, "mixed world step n=%d" % n)
+    assert_real_close(wg.safety(node_g, *dt[:3]).cpu().numpy(), wo.safety(node_o, *t[:3]), "mixed world safety n=%d" % n)
+    if n > 100000:
+        counts = np.bincount(node_o, minlength=13)
+        assert np.all(counts[:9] > 1000) and counts[9:].sum() > 50
