@@ -105,7 +105,7 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
  *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
  *                safeties it is not the exact distance everywhere (R29).
- * A boolean can be a node of a world (vg_world_create); it cannot be an operand or a daughter of a vg_volume in this build.
+ * A boolean can be a node of a world and the mother or a daughter of a volume; it cannot be an operand of another boolean.
  */
 typedef enum { VG_UNION = 0, VG_INTERSECTION = 1, VG_SUBTRACTION = 2 } vg_bool_op;
 int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out);
@@ -147,7 +147,9 @@ int vg_query_all(const vg_shape *shape, const double *x, const double *y, const 
  * transformations"; BASELINE.json configs[4]).  `xforms` (HOST): ndaughters * 12 doubles, row-major 3x4
  * [R | b] per daughter, mother -> daughter-local: p_loc = R p + b, d_loc = R d (reading R12).  R is
  * expected to be orthonormal (checked to 1e-9: VG_ERR_PARAM otherwise).  0 <= ndaughters <= VG_MAX_DAUGHTERS.
- * Daughter kinds: box, orb, tube, cone, trd (a polycone daughter gives VG_ERR_ARG in this build).
+ * Mother and daughters may be any vg_shape.  With the five primitives only, ComputeStep runs the dedicated kernel (the
+ * daughter table staged in shared memory by TMA); a polycone or boolean among them (reading R30) makes the volume a
+ * one-level world served by the world kernels, with the same results and conventions.
  * The shapes' constants are copied; the vg_shape handles may be destroyed afterwards.
  */
 int vg_volume_create(const vg_shape *mother, int ndaughters, const vg_shape *const *daughters, const double *xforms,

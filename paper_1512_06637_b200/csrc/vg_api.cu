@@ -14,10 +14,12 @@
 
 using namespace vg;
 
+struct vg_world;
 struct vg_volume {
     SolidU mother;
     NavMeta meta;
     unsigned char *table_dev; // the blob described in vg_params.h
+    vg_world *general;        // mother or a daughter is a polycone / boolean: the volume is held as a one-level world instead
 };
 
 static thread_local char g_err[512] = "";
@@ -277,6 +279,8 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
 
 // ---------------------------------------------------------------------------------------------- navigation
 
+static const WorldTab &world_tab(const vg_world *w); // defined with struct vg_world below
+
 // radius of a sphere about the local origin that contains the solid (phi cuts ignored)
 static double bounding_radius(const SolidU &s)
 {
@@ -351,6 +355,26 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
     vg_volume *v = new (std::nothrow) vg_volume;
     if (!v) return fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
     std::memset(v, 0, sizeof *v);
+    bool general = mother->kind >= VG_POLYCONE;
+    for (int i = 0; i < nd && !general; ++i) general = daughters[i] && daughters[i]->kind >= VG_POLYCONE;
+    if (general) { // polycones / booleans do not fit the fixed-size daughter records: a one-level world serves the volume
+        std::vector<const vg_shape *> shapes(1, mother);
+        std::vector<int32_t> parent(1, -1);
+        std::vector<double> xf = { 1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0 };
+        for (int i = 0; i < nd; ++i) {
+            shapes.push_back(daughters[i]);
+            parent.push_back(0);
+            xf.insert(xf.end(), xforms + 12 * i, xforms + 12 * i + 12);
+        }
+        int rcw = vg_world_create(nd + 1, shapes.data(), parent.data(), xf.data(), &v->general);
+        if (rcw != VG_OK) {
+            delete v;
+            return rcw;
+        }
+        v->meta.nd = nd;
+        *out = v;
+        return VG_OK;
+    }
     int rc = to_solid(mother, &v->mother, "mother");
     NavMeta &mt = v->meta;
     mt.nd = nd;
@@ -430,6 +454,7 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
 extern "C" void vg_volume_destroy(vg_volume *v)
 {
     if (!v) return;
+    if (v->general) vg_world_destroy(v->general);
     if (v->table_dev) cudaFree(v->table_dev);
     delete v;
 }
@@ -448,8 +473,9 @@ extern "C" int vg_compute_step(const vg_volume *v, const double *x, const double
     if (!hit || !aligned(hit, 4)) return fail(VG_ERR_ARG, "%s: hit array NULL or misaligned", fn);
     if (!(step_max >= 0)) return fail(VG_ERR_ARG, "%s: step_max must be >= 0 (may be +inf)", fn);
     Tracks t{ x, y, z, dx, dy, dz };
-    cudaError_t e = launch_compute_step(v->mother, v->table_dev, v->meta, t, step_max, n, step, hit,
-                                        static_cast<cudaStream_t>(stream));
+    cudaError_t e = v->general ? launch_world_step(world_tab(v->general), nullptr, t, step_max, n, step, hit, static_cast<cudaStream_t>(stream))
+                               : launch_compute_step(v->mother, v->table_dev, v->meta, t, step_max, n, step, hit,
+                                                     static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }
@@ -465,7 +491,8 @@ extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const doubl
     if (rc != VG_OK) return rc;
     if (n == 0) return VG_OK;
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
-    cudaError_t e = launch_volume_safety(v->mother, v->table_dev, v->meta, t, n, safety, static_cast<cudaStream_t>(stream));
+    cudaError_t e = v->general ? launch_world_safety(world_tab(v->general), nullptr, t, n, safety, static_cast<cudaStream_t>(stream))
+                               : launch_volume_safety(v->mother, v->table_dev, v->meta, t, n, safety, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
 }
@@ -478,6 +505,8 @@ struct vg_world {
     unsigned char *blob;   // polycone and boolean constants of the nodes that are not primitives (reading R30)
     int device;
 };
+
+static const WorldTab &world_tab(const vg_world *w) { return w->tab; }
 
 static bool rigid(const double *m)
 {

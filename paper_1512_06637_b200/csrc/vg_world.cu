@@ -138,7 +138,10 @@ __global__ void __launch_bounds__(kWorldBlock)
     pdl_wait();
     const int64_t i = int64_t(blockIdx.x) * kWorldBlock + threadIdx.x;
     if (i >= n) return;
-    const int nd = node[i];
+    // node == NULL: a one-level volume held as a world (vg_volume with polycone / boolean solids): every track is in node 0
+    // and the result follows vg_compute_step's convention (hit = daughter index, -1 mother exit, -2 physics step)
+    const bool vol = node == nullptr;
+    const int nd = vol ? 0 : node[i];
     if (nd < 0 || nd >= nnodes) {
         stg1(out + i, -1.0);
         if (kStep) stg1i(next + i, -1);
@@ -181,7 +184,7 @@ __global__ void __launch_bounds__(kWorldBlock)
         }
         const bool phys = best > step_max; // the physics step is shorter than the geometric one
         stg1(out + i, phys ? step_max : best);
-        stg1i(next + i, phys ? nd : who);
+        stg1i(next + i, vol ? (phys ? -2 : (who < 0 ? -1 : who - 1)) : (phys ? nd : who));
     } else {
         double best = -node_sdf<EXT>(w, N, x, y, z);
         // SafetyToIn of a child >= |p - c| - r.  Phase 1, FP32: children whose bound can undercut the node's own

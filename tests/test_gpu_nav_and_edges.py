@@ -324,9 +324,47 @@ def test_volume_create_rejects_bad_input(vg):
     bad = [[2, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]]
     with pytest.raises(vg.VgError):
         vg.Volume(m, [d], bad)
-    pc = vg.Shape(W.POLYCONE, W.polycone_params(1))
-    with pytest.raises(vg.VgError):
-        vg.Volume(m, [pc], [[1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]])
+
+
+def test_volume_with_polycone_and_boolean_solids(vg):
+    """A one-level volume whose solids are not all primitives (reading R30) is served by the world kernels behind
+    vg_compute_step / vg_volume_safety: same conventions (hit = daughter index, -1 mother exit, -2 physics step)."""
+    bools = {b.name: b for b in W.boolean_cases()}
+    b1 = bools["box_minus_tube"]
+    specs = [("shape", W.POLYCONE, W.STEPPED_POLYCONE, (-40.0, -40.0, 0.0)), ("boolean", b1, None, (40.0, -40.0, 5.0)),
+             ("shape", W.TUBE, [5.0, 10.0, 15.0, 0.0, 4 * PI / 3], (-40.0, 40.0, -5.0)),
+             ("shape", W.POLYCONE, [0.5, 4.0] + W.STEPPED_POLYCONE[2:], (40.0, 40.0, 0.0))]
+    rng = np.random.default_rng(12)
+
+    def mk(mod, sp):
+        if sp[0] == "shape":
+            return mod.Shape(sp[1], sp[2])
+        b = sp[1]
+        return mod.Boolean(b.op, mod.Shape(b.kind_a, b.par_a), mod.Shape(b.kind_b, b.par_b), b.xform)
+    xf = []
+    for sp in specs:
+        q = rng.normal(size=4)
+        xf.append(W.placement(W.quaternion_to_matrix(tuple(q / np.linalg.norm(q))), sp[3]))
+    ident = W.placement(np.eye(3), (0, 0, 0))
+    for mother in (("shape", W.BOX, [80.0, 80.0, 40.0]), ("boolean", bools["box_union_orb"].__class__(
+            "m", W.SUBTRACTION, W.BOX, [80.0, 80.0, 40.0], W.ORB, [6.0], (0.0, 0.0, 0.0), (0.0, 0.0, 0.0, 1.0), 1), None)):
+        wo = O.World([mk(O, mother)] + [mk(O, sp) for sp in specs], [-1, 0, 0, 0, 0], [ident] + xf)
+        vgv = vg.Volume(mk(vg, mother), [mk(vg, sp) for sp in specs], xf)
+
+        def band(x, y, z):
+            nd = wo.locate(x, y, z)
+            zero = np.zeros(x.size, dtype=np.int32)
+            return (nd != 0) | (wo.safety(zero, x, y, z) < 1e-4)  # in the mother, outside every daughter, clear of operands too
+        t = W.draw_tracks(91, 150001, (0, 0, 0), (80, 80, 40), band)
+        zero = np.zeros(t[0].size, dtype=np.int32)
+        for step_max in (W.STEP_MAX, 20.0):
+            so, no = wo.step(zero, *t, step_max)
+            sg, hg = vgv.compute_step(*dev(t), step_max)
+            want_hit = np.where(no == 0, -2, np.where(no < 0, -1, no - 1))
+            assert_int_equal(hg.cpu().numpy(), want_hit, "general volume hit")
+            assert_real_close(sg.cpu().numpy(), so, "general volume step")
+        assert set(np.unique(want_hit)) >= {-2, -1, 0, 1, 2, 3}
+        assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), wo.safety(zero, *t[:3]), "general volume safety")
 
 
 # ------------------------------------------------------------------------------- host-buffer entry points
