@@ -462,6 +462,20 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
     rows.append(e)
     del case
     torch.cuda.empty_cache()
+    # polycone variants -- the configs[3] polycone cut to phi in [0, 4 pi / 3], and one with two z steps
+    pc = W.polycone_params(W.config_seed(3, 0))
+    variants = [("polycone_phi_segment", [0.0, 4.0 * np.pi / 3.0] + pc[2:]), ("polycone_z_steps", W.STEPPED_POLYCONE)]
+    for vname, vpar in variants:
+        sc = W.ShapeCase(3, vname, W.POLYCONE, vpar, *W._scaled(W.POLYCONE, vpar), W.config_seed(3, 3), [4194304],
+                         ("distance_to_in", "safety_to_in"))
+        case = Case(vg, torch, sc.name, 4194304, sc.queries, shape=sc)
+        for q in sc.queries:
+            sec = time_query_alone(torch, case, q)
+            e = roofline_entry("polycone_variant", q, case.n, sec, hbm_peak, fma_rate)
+            e.update({"config": "8(f) f2", "shape": vname, "query": q, "n": case.n, "cold_inputs": case.cold, "bound": "alu"})
+            rows.append(e)
+        del case
+        torch.cuda.empty_cache()
     # boolean solids of two primitives (one of each operation)
     for bc in [b for b in W.boolean_cases() if b.name in ("tube_union_box", "cone_intersection_orb", "box_minus_tube")]:
         case = Case(vg, torch, bc.name, 4194304, W.QUERIES5, boolean=bc)
