@@ -39,6 +39,8 @@ def _load(path):
     lib.orc_volume_safety.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _P]
     lib.orc_boolean_create.restype = C.c_void_p
     lib.orc_boolean_create.argtypes = [C.c_int, C.c_void_p, C.c_void_p, _P]
+    lib.orc_boolean_create_nested.restype = C.c_void_p
+    lib.orc_boolean_create_nested.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, _P]
     lib.orc_boolean_destroy.argtypes = [C.c_void_p]
     lib.orc_boolean_inside.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _PI]
     lib.orc_boolean_sdf.argtypes = [C.c_void_p, _P, _P, _P, C.c_int64, _P]
@@ -188,13 +190,24 @@ UNION, INTERSECTION, SUBTRACTION = 0, 1, 2
 
 class Boolean:
     """C = A op B (readings R27-R29, vg_oracle.c): `xform` is the row-major 3x4 [R | b] from the frame of C (= of A)
-    to the frame of B.  Same query names as Shape; the safeties are the composed bound of R29."""
+    to the frame of B; A and B are Shapes or Booleans (R31, at most 8 primitives per tree).  Same query names as Shape;
+    the safeties are the composed bound of R29."""
+
+    def leaves(self, pre=None):
+        """[(primitive Shape, 3x4 matrix frame of this boolean -> frame of the primitive)] in tree order."""
+        pre = np.eye(4) if pre is None else pre
+        out = []
+        for operand, M in ((self.a, pre), (self.b, np.vstack([self.xform.reshape(3, 4), [0, 0, 0, 1]]) @ pre)):
+            out += operand.leaves(M) if isinstance(operand, Boolean) else [(operand, M[:3])]
+        return out
 
     def __init__(self, op, a, b, xform):
         self._l = a._l
         self.op, self.a, self.b = int(op), a, b
         self.xform = np.ascontiguousarray(np.asarray(xform, dtype=np.float64).reshape(12))
-        self._h = self._l.orc_boolean_create(self.op, a._h, b._h, _ptr(self.xform))
+        na, nb = isinstance(a, Boolean), isinstance(b, Boolean)  # R31: an operand may be a boolean itself
+        self._h = self._l.orc_boolean_create_nested(self.op, None if na else a._h, a._h if na else None,
+                                                    None if nb else b._h, b._h if nb else None, _ptr(self.xform))
         if not self._h:
             raise ValueError("oracle: invalid boolean")
 

@@ -882,22 +882,40 @@ void orc_world_safety(const orc_world *w, const int32_t *node, const double *x, 
 
 enum { ORC_UNION = 0, ORC_INTERSECTION = 1, ORC_SUBTRACTION = 2 };
 
+/* R31: an operand may itself be a boolean (a CSG tree); R27-R29 apply unchanged with "operand" read recursively: the
+ * class, the composed sdf and the membership intervals of an operand that is a boolean are those of that boolean.
+ * At most ORC_MAXLEAF primitives per tree. */
+#define ORC_MAXLEAF 8
+
 struct orc_boolean_s {
     int op;
-    const orc_shape *a, *b;
+    const orc_shape *a, *b;    /* operand is a primitive ... */
+    const orc_boolean *ca, *cb; /* ... or a boolean: exactly one of (a, ca) and one of (b, cb) is given */
+    int nleaf;
     real xf[12];
 };
 
-orc_boolean *orc_boolean_create(int op, const orc_shape *a, const orc_shape *b, const double *xf)
+orc_boolean *orc_boolean_create_nested(int op, const orc_shape *a, const orc_boolean *ca, const orc_shape *b,
+                                       const orc_boolean *cb, const double *xf)
 {
-    if (op < 0 || op > 2 || !a || !b || !xf || !finite_all(xf, 12)) return NULL;
+    if (op < 0 || op > 2 || ((a != NULL) == (ca != NULL)) || ((b != NULL) == (cb != NULL)) || !xf || !finite_all(xf, 12)) return NULL;
+    int nleaf = (a ? 1 : ca->nleaf) + (b ? 1 : cb->nleaf);
+    if (nleaf > ORC_MAXLEAF) return NULL;
     orc_boolean *c = (orc_boolean *)calloc(1, sizeof *c);
     if (!c) return NULL;
     c->op = op;
     c->a = a;
     c->b = b;
+    c->ca = ca;
+    c->cb = cb;
+    c->nleaf = nleaf;
     for (int k = 0; k < 12; ++k) c->xf[k] = xf[k];
     return c;
+}
+
+orc_boolean *orc_boolean_create(int op, const orc_shape *a, const orc_shape *b, const double *xf)
+{
+    return orc_boolean_create_nested(op, a, NULL, b, NULL, xf);
 }
 
 void orc_boolean_destroy(orc_boolean *c) { free(c); }
@@ -998,12 +1016,31 @@ static int bool_member(int op, int ina, int inb)
     return ina && !inb;
 }
 
+/* an operand's answers: the primitive's, or (R31) the nested boolean's */
+static int operand_inside(const orc_shape *s, const orc_boolean *c, const real p[3])
+{
+    return s ? inside(s, p[0], p[1], p[2]) : bool_inside(c, p);
+}
+
+static real operand_sdf(const orc_shape *s, const orc_boolean *c, const real p[3])
+{
+    return s ? sdf(s, p[0], p[1], p[2]) : bool_sdf(c, p);
+}
+
+static int bool_events(const orc_boolean *c, const real p[3], const real d[3], real *out);
+
+/* every t > 0 at which the operand's membership flips along the ray, ascending */
+static int operand_events(const orc_shape *s, const orc_boolean *c, const real p[3], const real d[3], real *out)
+{
+    return s ? all_crossings(s, p, d, out) : bool_events(c, p, d, out);
+}
+
 /* R27 */
 static int bool_inside(const orc_boolean *c, const real p[3])
 {
     real d0[3] = { 0, 0, 0 }, pb[3], db[3];
     to_local(c->xf, p, d0, pb, db);
-    int ca = inside(c->a, p[0], p[1], p[2]), cb = inside(c->b, pb[0], pb[1], pb[2]);
+    int ca = operand_inside(c->a, c->ca, p), cb = operand_inside(c->b, c->cb, pb);
     int ain = ca == ORC_INSIDE, aout = ca == ORC_OUTSIDE, bin = cb == ORC_INSIDE, bout = cb == ORC_OUTSIDE;
     int in, out;
     if (c->op == ORC_UNION) { in = ain || bin; out = aout && bout; }
@@ -1017,28 +1054,41 @@ static real bool_sdf(const orc_boolean *c, const real p[3])
 {
     real d0[3] = { 0, 0, 0 }, pb[3], db[3];
     to_local(c->xf, p, d0, pb, db);
-    real sa = sdf(c->a, p[0], p[1], p[2]), sb = sdf(c->b, pb[0], pb[1], pb[2]);
+    real sa = operand_sdf(c->a, c->ca, p), sb = operand_sdf(c->b, c->cb, pb);
     if (c->op == ORC_UNION) return rmin2(sa, sb);
     if (c->op == ORC_INTERSECTION) return rmax2(sa, sb);
     return rmax2(sa, -sb);
 }
 
-/* R28: first t > 0 at which the membership of C along the ray differs from its value at p */
-static real bool_cross(const orc_boolean *c, const real p[3], const real d[3])
+/* R28: every t > 0 at which the membership of C along the ray flips (merge of the operands' flips, a tie goes to A) */
+static int bool_events(const orc_boolean *c, const real p[3], const real d[3], real *out)
 {
-    real pb[3], db[3], ta[ORC_MAXX], tb[ORC_MAXX];
+    real pb[3], db[3];
+    real *ta = (real *)malloc(sizeof(real) * 2 * ORC_MAXLEAF * ORC_MAXX), *tb = ta + ORC_MAXLEAF * ORC_MAXX;
     to_local(c->xf, p, d, pb, db);
-    int na = all_crossings(c->a, p, d, ta), nb = all_crossings(c->b, pb, db, tb);
-    int ina = inside(c->a, p[0], p[1], p[2]) == ORC_INSIDE, inb = inside(c->b, pb[0], pb[1], pb[2]) == ORC_INSIDE;
-    int start = bool_member(c->op, ina, inb);
-    int i = 0, j = 0;
+    int na = operand_events(c->a, c->ca, p, d, ta), nb = operand_events(c->b, c->cb, pb, db, tb);
+    int ina = operand_inside(c->a, c->ca, p) == ORC_INSIDE, inb = operand_inside(c->b, c->cb, pb) == ORC_INSIDE;
+    int cur = bool_member(c->op, ina, inb);
+    int i = 0, j = 0, n = 0;
     while (i < na || j < nb) {
         real t;
         if (j >= nb || (i < na && ta[i] <= tb[j])) { t = ta[i++]; ina = !ina; }
         else { t = tb[j++]; inb = !inb; }
-        if (bool_member(c->op, ina, inb) != start) return t;
+        int now = bool_member(c->op, ina, inb);
+        if (now != cur) { out[n++] = t; cur = now; }
     }
-    return ORC_INF;
+    free(ta);
+    return n;
+}
+
+/* R28: the first of them */
+static real bool_cross(const orc_boolean *c, const real p[3], const real d[3])
+{
+    real *t = (real *)malloc(sizeof(real) * ORC_MAXLEAF * ORC_MAXX);
+    int n = bool_events(c, p, d, t);
+    real first = n > 0 ? t[0] : ORC_INF;
+    free(t);
+    return first;
 }
 
 void orc_boolean_inside(const orc_boolean *c, const double *x, const double *y, const double *z, int64_t n, int32_t *out)

@@ -231,3 +231,90 @@ def test_invalid_booleans_are_rejected():
         O.Boolean(3, a, a, IDENT)
     with pytest.raises(ValueError):
         O.Boolean(O.UNION, a, a, [float("nan")] * 12)
+
+
+# ------------------------------------------------------------------ nested booleans (reading R31)
+
+CSG = {c.name: c for c in W.csg_cases()}
+
+
+def csg_member(tree, x, y, z):
+    """Set definition of a CSG tree on the closed sets, composed in numpy (independent of the oracle)."""
+    if tree[0] == "leaf":
+        return G.member(tree[1], tree[2], x, y, z)
+    ma = csg_member(tree[2], x, y, z)
+    mb = csg_member(tree[3], *to_b(tree[4], x, y, z))
+    return {W.UNION: ma | mb, W.INTERSECTION: ma & mb, W.SUBTRACTION: ma & ~mb}[tree[1]]
+
+
+def csg_band(c):
+    """Clear of the surface of EVERY primitive of the tree (the contract of the distances, R7)."""
+    leaves = c.leaves()
+
+    def band(x, y, z):
+        bad = np.zeros(np.shape(x), dtype=bool)
+        for shape, M in leaves:
+            L = M[:, :3] @ np.stack([x, y, z]) + M[:, 3:4]
+            bad |= np.abs(shape.sdf(L[0], L[1], L[2])) < W.SURFACE_BAND
+        return bad
+    return band
+
+
+@pytest.mark.parametrize("name", list(CSG))
+def test_nested_boolean_membership_distances_and_safety(name):
+    cc = CSG[name]
+    c = cc.build(O)
+    x, y, z, dx, dy, dz = cc.tracks(30000, csg_band(c))
+    mem = csg_member(cc.tree, x, y, z)
+    cls = c.inside(x, y, z)
+    assert np.array_equal(cls == O.INSIDE, mem) and np.array_equal(cls == O.OUTSIDE, ~mem)
+    assert 0.03 < mem.mean() < 0.7
+    s = c.sdf(x, y, z)
+    assert np.array_equal(s < 0, mem)
+    din, dout = c.distance_to_in(x, y, z, dx, dy, dz), c.distance_to_out(x, y, z, dx, dy, dz)
+    assert np.array_equal(din == -1.0, mem) and np.array_equal(dout == -1.0, ~mem)
+    t = np.where(mem, dout, din)
+    hit = np.isfinite(t)
+    assert np.all(hit[mem]) and 0.05 < hit.mean() < 0.95
+    tt = t[hit]
+    hx, hy, hz = x[hit] + tt * dx[hit], y[hit] + tt * dy[hit], z[hit] + tt * dz[hit]
+    assert np.max(np.abs(c.sdf(hx, hy, hz))) <= 1e-9
+    e = 1e-6
+    before = csg_member(cc.tree, hx - e * dx[hit], hy - e * dy[hit], hz - e * dz[hit])
+    after = csg_member(cc.tree, hx + e * dx[hit], hy + e * dy[hit], hz + e * dz[hit])
+    assert np.mean(before != after) > 0.997
+    for frac in (0.03, 0.3, 0.6, 0.97):
+        mid = csg_member(cc.tree, x[hit] + frac * tt * dx[hit], y[hit] + frac * tt * dy[hit], z[hit] + frac * tt * dz[hit])
+        assert np.array_equal(mid, mem[hit])
+    for far in (0.5, 3.0, 12.0, 60.0):
+        assert not csg_member(cc.tree, x[~hit] + far * dx[~hit], y[~hit] + far * dy[~hit], z[~hit] + far * dz[~hit]).any()
+    assert np.all(np.abs(s)[hit] <= tt * (1 + 1e-12))  # the composed safety never exceeds a distance
+
+
+def test_nested_boolean_reductions():
+    """(A u small-inside-A) - C == A - C; regrouping a union changes nothing; A n (B n C) == (A n B) n C."""
+    a = O.Shape(O.BOX, [8, 8, 8])
+    small = O.Shape(O.ORB, [1.0])
+    tube = O.Shape(O.TUBE, [0, 3, 12, 0, 2 * math.pi])
+    orb = O.Shape(O.ORB, [9.5])
+    q = W.quaternion_to_matrix((0.5, 0.5, 0.5, 0.5))
+    p_small, p_tube, p_orb = W.placement(np.eye(3), (4.0, 4.0, 4.0)), W.placement(q, (1.0, 0.0, -1.0)), W.placement(np.eye(3), (1.0, 1.0, 0.0))
+    flat = O.Boolean(O.SUBTRACTION, a, tube, p_tube)
+    nested = O.Boolean(O.SUBTRACTION, O.Boolean(O.UNION, a, small, p_small), tube, p_tube)
+    t = W.draw_tracks(51, 30000, (0, 0, 0), (12, 12, 12), csg_band(nested))
+    _same(_five(nested, t), _five(flat, t))
+    # ((a n orb) n tube) == (a n (orb n tube')) with tube' placed relative to the orb's frame
+    left = O.Boolean(O.INTERSECTION, O.Boolean(O.INTERSECTION, a, orb, p_orb), tube, p_tube)
+    Mo = np.vstack([np.asarray(p_orb).reshape(3, 4), [0, 0, 0, 1]])
+    Mt = np.vstack([np.asarray(p_tube).reshape(3, 4), [0, 0, 0, 1]])
+    rel = (Mt @ np.linalg.inv(Mo))[:3].reshape(12)  # frame of the orb -> frame of the tube
+    right = O.Boolean(O.INTERSECTION, a, O.Boolean(O.INTERSECTION, orb, tube, rel), p_orb)
+    t = W.draw_tracks(52, 30000, (0, 0, 0), (12, 12, 12), csg_band(left))
+    _same(_five(left, t), _five(right, t), tol=1e-11)
+    lu = O.Boolean(O.UNION, O.Boolean(O.UNION, a, orb, p_orb), tube, p_tube)
+    ru = O.Boolean(O.UNION, a, O.Boolean(O.UNION, orb, tube, rel), p_orb)
+    _same(_five(lu, t), _five(ru, t), tol=1e-11)
+    with pytest.raises(ValueError):  # more than eight primitives
+        big = a
+        for _ in range(8):
+            big = O.Boolean(O.UNION, big, small, p_small)

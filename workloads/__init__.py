@@ -399,3 +399,52 @@ class MixedWorldCase:
 
 def mixed_world_case(**kw):
     return MixedWorldCase(**kw)
+
+
+# ------------------------------------------------------------------ nested booleans (reading R31)
+
+class CsgCase:
+    """A CSG tree: `tree` is ("leaf", kind, params) or ("op", op, left, right, xform) with `xform` the row-major 3x4
+    [R | b] from the frame of the node (= of its left operand) to the frame of its right operand."""
+
+    def __init__(self, name, tree, center, half, seed):
+        self.name, self.tree, self.center, self.half, self.seed = name, tree, tuple(center), tuple(half), seed
+
+    def tracks(self, n, band=None):
+        return draw_tracks(self.seed, n, self.center, self.half, band)
+
+    def build(self, mod):
+        """The tree as objects of `mod` (the oracle package or the CUDA binding: both have Shape and Boolean)."""
+        def mk(t):
+            if t[0] == "leaf":
+                return mod.Shape(t[1], t[2])
+            return mod.Boolean(t[1], mk(t[2]), mk(t[3]), t[4])
+        return mk(self.tree)
+
+
+def csg_cases():
+    s2 = math.sqrt(0.5)
+    ident = placement(np.eye(3), (0, 0, 0))
+    rx = quaternion_to_matrix((s2, 0.0, 0.0, s2))
+    rq = quaternion_to_matrix((0.18257418583505536, 0.3651483716701107, 0.5477225575051661, 0.7302967433402214))
+    leaf = lambda k, p: ("leaf", k, [float(v) for v in p])
+    seed = BASE_SEED + 700
+    rounded = ("op", INTERSECTION, leaf(BOX, [5, 5, 5]), leaf(ORB, [6.5]), ident)
+    return [
+        CsgCase("rounded_cube_with_bore", ("op", SUBTRACTION, rounded, leaf(TUBE, [0, 2, 10, 0, TWO_PI]), placement(rq, (0.5, -0.5, 0.0))),
+                (0, 0, 0), (8, 8, 8), seed),
+        CsgCase("three_way_union", ("op", UNION, ("op", UNION, leaf(TUBE, [5, 10, 15, 0, 4 * math.pi / 3]), leaf(BOX, [4, 4, 20]),
+                                                   placement(rq, (6.0, -2.0, 1.0))),
+                                    leaf(CONE, [0, 3, 0, 8, 10, 0, TWO_PI]), placement(rx, (-9.0, 4.0, 0.0))),
+                (0, 0, 0), (22, 22, 26), seed + 1),
+        CsgCase("box_minus_union", ("op", SUBTRACTION, leaf(BOX, [10, 10, 10]),
+                                    ("op", UNION, leaf(ORB, [5]), leaf(TUBE, [0, 3, 14, 0, TWO_PI]), placement(rx, (0.0, 0.0, 2.0))),
+                                    placement(rq, (1.0, -1.0, 0.5))),
+                (0, 0, 0), (14, 14, 14), seed + 2),
+        CsgCase("twice_drilled_block_in_a_sphere",
+                ("op", INTERSECTION,
+                 ("op", SUBTRACTION, ("op", SUBTRACTION, leaf(BOX, [9, 9, 9]), leaf(TUBE, [0, 3, 12, 0, TWO_PI]), ident),
+                  leaf(TUBE, [0, 2.5, 12, 0, TWO_PI]), placement(rx, (0.0, 1.0, 0.0))),
+                 leaf(ORB, [11]), placement(np.eye(3), (1.0, 0.0, -1.0))),
+                (0, 0, 0), (13, 13, 13), seed + 3),
+    ]
