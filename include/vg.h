@@ -95,8 +95,10 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  * vg_boolean_create -- the boolean solid C = A op B of two primitives ("boolean operations", PAPER.md:110
  * "logical operations"; readings R27-R29 in DESIGN.md).  A sits in the frame of C; `xform_b` (HOST,
  * 12 doubles, row-major 3x4 [R | b], orthonormal R) maps the frame of C to the frame of B.  A and B: box, orb, tube,
- * cone or trd (VG_ERR_ARG otherwise); their constants are copied.  The result is a vg_shape of kind VG_BOOLEAN that
- * every query below accepts:
+ * cone, trd, or a boolean made by this call (reading R31: a CSG tree; at most 8 primitives per tree, VG_ERR_PARAM
+ * beyond; a polycone operand gives VG_ERR_ARG); their constants are copied.  Two primitives run kernels specialised
+ * per pair of kinds, a tree is flattened into a program over its primitives and runs the general kernel (vg_csg.cu).
+ * The result is a vg_shape of kind VG_BOOLEAN that every query below accepts ("operand" read recursively for a tree):
  *   Inside       combines the operands' classes: union INSIDE if either is, OUTSIDE if both are; intersection INSIDE if
  *                both are, OUTSIDE if either is; subtraction (A minus B) INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A
  *                OUTSIDE or B INSIDE; SURFACE otherwise (R27);
@@ -105,7 +107,7 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
  *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
  *                safeties it is not the exact distance everywhere (R29).
- * A boolean can be a node of a world and the mother or a daughter of a volume; it cannot be an operand of another boolean.
+ * A boolean of two primitives can be a node of a world and the mother or a daughter of a volume; a tree cannot (VG_ERR_ARG).
  */
 typedef enum { VG_UNION = 0, VG_INTERSECTION = 1, VG_SUBTRACTION = 2 } vg_bool_op;
 int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out);

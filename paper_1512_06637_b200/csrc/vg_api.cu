@@ -142,7 +142,11 @@ extern "C" void vg_shape_destroy(vg_shape *s)
     delete s;
 }
 
-extern "C" int vg_shape_kind(const vg_shape *s) { return s ? s->kind : fail(VG_ERR_ARG, "vg_shape_kind: NULL"); }
+extern "C" int vg_shape_kind(const vg_shape *s)
+{
+    if (!s) return fail(VG_ERR_ARG, "vg_shape_kind: NULL");
+    return s->kind == kCsg ? int(VG_BOOLEAN) : s->kind; // a nested boolean is a boolean to the caller
+}
 
 // ------------------------------------------------------------------------------------------------- queries
 
@@ -196,6 +200,7 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
         break;
     }
     case VG_BOOLEAN: e = launch_boolean(q, s->u.boolean, t, step_max, n, out, st); break;
+    case kCsg: e = launch_csg(q, s->u.csg, t, step_max, n, out, st); break;
     }
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
@@ -240,7 +245,7 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
     const char *fn = "vg_query_all";
     if (!s) return fail(VG_ERR_ARG, "%s: shape is NULL", fn);
     const bool all = cls && dist_in && dist_out && safety_in && safety_out;
-    if (!all || s->kind == VG_POLYCONE || s->kind == VG_BOOLEAN) { // a subset, or no fused kernel for this solid: one launch per requested answer
+    if (!all || s->kind >= VG_POLYCONE) { // a subset, or no fused kernel for this solid: one launch per requested answer
         if (!cls && !dist_in && !dist_out && !safety_in && !safety_out) return fail(VG_ERR_ARG, "%s: every output is NULL", fn);
         int rc = VG_OK;
         if (cls && rc == VG_OK) rc = vg_inside(s, x, y, z, n, cls, stream);
@@ -529,6 +534,42 @@ static void compose(const double *A, const double *B, double *C)
 
 // --------------------------------------------------------------------------------------------- boolean solids
 
+// an operand as a list of primitives with their transforms (frame of the operand -> frame of the primitive) and a postfix
+// program over them (vg_params.h CsgP)
+struct CsgOperand {
+    int nleaf = 0, nprog = 0;
+    SolidU leaf[kCsgMaxLeaf];
+    double X[kCsgMaxLeaf][12];
+    unsigned char prog[kCsgMaxProg];
+};
+
+static const double kIdentity12[12] = { 1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0 };
+
+static int csg_operand(const vg_shape *s, CsgOperand *o)
+{
+    if (s->kind == kCsg) {
+        const CsgP &c = s->u.csg;
+        o->nleaf = c.nleaf, o->nprog = c.nprog;
+        std::memcpy(o->leaf, c.leaf, sizeof o->leaf);
+        std::memcpy(o->X, c.X, sizeof o->X);
+        std::memcpy(o->prog, c.prog, sizeof o->prog);
+        return VG_OK;
+    }
+    if (s->kind == VG_BOOLEAN) {
+        const BoolP &c = s->u.boolean;
+        o->nleaf = 2, o->nprog = 3;
+        o->leaf[0] = c.a, o->leaf[1] = c.b;
+        std::memcpy(o->X[0], kIdentity12, sizeof kIdentity12);
+        std::memcpy(o->X[1], c.X, sizeof c.X);
+        o->prog[0] = 0, o->prog[1] = 1, o->prog[2] = (unsigned char)(0x80 | c.op);
+        return VG_OK;
+    }
+    o->nleaf = 1, o->nprog = 1;
+    std::memcpy(o->X[0], kIdentity12, sizeof kIdentity12);
+    o->prog[0] = 0;
+    return to_solid(s, &o->leaf[0], "operand");
+}
+
 extern "C" int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out)
 {
     const char *fn = "vg_boolean_create";
@@ -541,12 +582,39 @@ extern "C" int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, c
     vg_shape *s = new (std::nothrow) vg_shape;
     if (!s) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
     std::memset(s, 0, sizeof *s);
-    s->kind = VG_BOOLEAN;
-    BoolP &c = s->u.boolean;
-    c.op = op;
-    std::memcpy(c.X, xform_b, sizeof c.X);
-    int rc = to_solid(a, &c.a, "operand");
-    if (rc == VG_OK) rc = to_solid(b, &c.b, "operand");
+    int rc = VG_OK;
+    if (a->kind < VG_POLYCONE && b->kind < VG_POLYCONE) { // two primitives: the specialised kernels of vg_bool.cu
+        s->kind = VG_BOOLEAN;
+        BoolP &c = s->u.boolean;
+        c.op = op;
+        std::memcpy(c.X, xform_b, sizeof c.X);
+        rc = to_solid(a, &c.a, "operand");
+        if (rc == VG_OK) rc = to_solid(b, &c.b, "operand");
+    } else { // an operand is a boolean (reading R31): flatten the tree
+        CsgOperand oa, ob;
+        rc = csg_operand(a, &oa);
+        if (rc == VG_OK) rc = csg_operand(b, &ob);
+        if (rc == VG_OK && oa.nleaf + ob.nleaf > kCsgMaxLeaf)
+            rc = fail(VG_ERR_PARAM, "%s: more than %d primitives in the tree", fn, kCsgMaxLeaf);
+        if (rc == VG_OK) {
+            s->kind = kCsg;
+            CsgP &c = s->u.csg;
+            c.nleaf = oa.nleaf + ob.nleaf;
+            for (int i = 0; i < oa.nleaf; ++i) {
+                c.leaf[i] = oa.leaf[i];
+                std::memcpy(c.X[i], oa.X[i], sizeof c.X[i]);
+            }
+            for (int i = 0; i < ob.nleaf; ++i) { // frame of the tree -> frame of B -> frame of the primitive
+                c.leaf[oa.nleaf + i] = ob.leaf[i];
+                compose(ob.X[i], xform_b, c.X[oa.nleaf + i]);
+            }
+            int k = 0;
+            for (int i = 0; i < oa.nprog; ++i) c.prog[k++] = oa.prog[i];
+            for (int i = 0; i < ob.nprog; ++i) c.prog[k++] = ob.prog[i] < 0x80 ? (unsigned char)(ob.prog[i] + oa.nleaf) : ob.prog[i];
+            c.prog[k++] = (unsigned char)(0x80 | op);
+            c.nprog = k;
+        }
+    }
     if (rc != VG_OK) {
         delete s;
         return rc;

@@ -20,6 +20,7 @@ struct vg_shape {
         TrdP trd;
         PolyconeP pcon;
         BoolP boolean;
+        CsgP csg;
     } u;
     // full-phi polycone only: the candidate grid of vg_pcon_grid.h in device memory of `grid_device` (masks == NULL if
     // no device was available at create; the safeties then run the ordered walk)

@@ -579,6 +579,9 @@ cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *tabl
 // boolean solids (vg_bool.cu)
 cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
 
+// nested booleans (vg_csg.cu)
+cudaError_t launch_csg(int q, const CsgP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
+
 // hierarchy of volumes (vg_world.cu)
 cudaError_t launch_world_locate(const WorldTab &w, const Tracks &t, int64_t n, int32_t *out, cudaStream_t s);
 cudaError_t launch_world_step(const WorldTab &w, const int32_t *node, const Tracks &t, double step_max, int64_t n, double *step,

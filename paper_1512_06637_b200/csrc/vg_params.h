@@ -10,7 +10,8 @@ namespace vg {
 constexpr int kMaxZ = 32;       // polycone z-planes
 constexpr int kMaxSec = kMaxZ - 1;
 
-enum Kind : int { kBox = 0, kOrb = 1, kTube = 2, kCone = 3, kTrd = 4, kPolycone = 5, kBoolean = 6 };
+enum Kind : int { kBox = 0, kOrb = 1, kTube = 2, kCone = 3, kTrd = 4, kPolycone = 5, kBoolean = 6,
+                  kCsg = 7 /* internal: a boolean whose operands include booleans (reading R31); reported as VG_BOOLEAN */ };
 enum Query : int { qInside = 0, qDistIn = 1, qDistOut = 2, qSafeIn = 3, qSafeOut = 4 };
 
 // phi segment [sphi, sphi + dphi]; e0, e1 = unit vectors of the two bounding half-planes (reading R11)
@@ -134,6 +135,18 @@ struct BoolP {
     int pad;
     double X[12];
     SolidU a, b;
+};
+
+// A CSG tree flattened at vg_boolean_create (reading R31): up to kCsgMaxLeaf primitives, each with the transform from the
+// frame of the tree to its own frame, and the tree as a postfix program over them (token < 0x80: push that leaf,
+// 0x80 | op: combine the two on top, left operand below).  Leaves appear in tree order, so "lowest leaf first" is the
+// oracle's "a tie goes to the left operand".
+constexpr int kCsgMaxLeaf = 8, kCsgMaxProg = 2 * kCsgMaxLeaf;
+struct CsgP {
+    int nleaf, nprog;
+    unsigned char prog[kCsgMaxProg];
+    double X[kCsgMaxLeaf][12];
+    SolidU leaf[kCsgMaxLeaf];
 };
 
 // navigation: one placed daughter

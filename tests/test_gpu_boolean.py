@@ -103,8 +103,7 @@ def test_boolean_create_rejects_bad_input(vg):
     with pytest.raises(vg.VgError):
         vg.Boolean(vg.UNION, a, pc, ident)
     c = vg.Boolean(vg.UNION, a, a, ident)
-    with pytest.raises(vg.VgError):
-        vg.Boolean(vg.UNION, a, c, ident)  # no nested booleans in this build
+    assert vg.Boolean(vg.UNION, a, c, ident).kind == vg.BOOLEAN  # a boolean operand makes a nested boolean (R31)
     vg.Volume(vg.Shape(W.BOX, [10, 10, 10]), [c], [ident])  # a boolean daughter is served by the world kernels (R30)
 
 
@@ -170,3 +169,80 @@ def test_random_booleans(vg):
         assert_real_close(cg.safety_to_in(*dt[:3]).cpu().numpy(), co.safety_to_in(*t[:3]), what + " safety")
         pairs.add((ka, kb))
     assert len(pairs) >= 20
+
+
+# ------------------------------------------------------------------ nested booleans (reading R31)
+
+CSG = {c.name: c for c in W.csg_cases()}
+
+
+def csg_band(co):
+    leaves = co.leaves()
+
+    def band(x, y, z):
+        bad = np.zeros(np.shape(x), dtype=bool)
+        for shape, M in leaves:
+            L = M[:, :3] @ np.stack([x, y, z]) + M[:, 3:4]
+            bad |= np.abs(shape.sdf(L[0], L[1], L[2])) < W.SURFACE_BAND
+        return bad
+    return band
+
+
+@pytest.mark.parametrize("name", list(CSG))
+@pytest.mark.parametrize("n", [1, 30011, 300007])
+def test_nested_booleans_match_the_oracle(vg, name, n):
+    cc = CSG[name]
+    co, cg = cc.build(O), cc.build(vg)
+    t = cc.tracks(n, csg_band(co))
+    dt = dev(t)
+    assert_int_equal(cg.inside(*dt[:3]).cpu().numpy(), co.inside(*t[:3]), name + " inside")
+    for q in ("distance_to_in", "distance_to_out"):
+        for step_max in (W.STEP_MAX, 4.0):
+            assert_real_close(getattr(cg, q)(*dt, step_max).cpu().numpy(), getattr(co, q)(*t, step_max), "%s %s" % (name, q))
+    for q in ("safety_to_in", "safety_to_out"):
+        assert_real_close(getattr(cg, q)(*dt[:3]).cpu().numpy(), getattr(co, q)(*t[:3]), "%s %s" % (name, q))
+    if n > 1000:
+        cls = co.inside(*t[:3])
+        assert (cls == O.INSIDE).mean() > 0.03 and (cls == O.OUTSIDE).mean() > 0.03
+    assert cg.kind == vg.BOOLEAN
+
+
+def test_random_nested_booleans(vg):
+    """Random trees of 3 to 8 primitives: random grouping (left-deep, right-deep, balanced), operations and placements."""
+    rng = np.random.default_rng(815)
+
+    def tree(nleaf):
+        if nleaf == 1:
+            k, p = _random_primitive(rng)
+            return ("leaf", k, p)
+        nl = int(rng.integers(1, nleaf))
+        q = rng.normal(size=4)
+        q /= np.linalg.norm(q)
+        xf = W.placement(W.quaternion_to_matrix(tuple(q)), tuple(float(v) for v in rng.uniform(-4, 4, 3)))
+        return ("op", int(rng.integers(0, 3)), tree(nl), tree(nleaf - nl), xf)
+    done = 0
+    for rep in range(40):
+        cc = W.CsgCase("random%d" % rep, tree(int(rng.integers(3, 9))), (0, 0, 0), (14, 14, 14), 9300 + rep)
+        co, cg = cc.build(O), cc.build(vg)
+        t = cc.tracks(12007, csg_band(co))
+        cls = co.inside(*t[:3])
+        dt = dev(t)
+        what = repr(cc.tree)[:200]
+        assert_int_equal(cg.inside(*dt[:3]).cpu().numpy(), cls, what)
+        assert_real_close(cg.distance_to_in(*dt, W.STEP_MAX).cpu().numpy(), co.distance_to_in(*t, W.STEP_MAX), what + " din")
+        assert_real_close(cg.distance_to_out(*dt, W.STEP_MAX).cpu().numpy(), co.distance_to_out(*t, W.STEP_MAX), what + " dout")
+        assert_real_close(cg.safety_to_in(*dt[:3]).cpu().numpy(), co.safety_to_in(*t[:3]), what + " safety")
+        done += int((cls == O.INSIDE).any())
+    assert done >= 20  # most random trees are not empty
+
+
+def test_nested_boolean_limits(vg):
+    a = vg.Shape(W.BOX, [1, 1, 1])
+    ident = [1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0]
+    c = a
+    for _ in range(7):
+        c = vg.Boolean(vg.UNION, c, a, ident)  # 8 primitives: the limit
+    with pytest.raises(vg.VgError):
+        vg.Boolean(vg.UNION, c, a, ident)
+    with pytest.raises(vg.VgError):
+        vg.World([vg.Shape(W.BOX, [10, 10, 10]), c], [-1, 0], [ident, ident])  # a nested boolean is not a node in this build
