@@ -107,7 +107,7 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
  *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
  *                safeties it is not the exact distance everywhere (R29).
- * A boolean of two primitives can be a node of a world and the mother or a daughter of a volume; a tree cannot (VG_ERR_ARG).
+ * A boolean (of two primitives or a tree) can be a node of a world and the mother or a daughter of a volume.
  */
 typedef enum { VG_UNION = 0, VG_INTERSECTION = 1, VG_SUBTRACTION = 2 } vg_bool_op;
 int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, const double *xform_b, vg_shape **out);

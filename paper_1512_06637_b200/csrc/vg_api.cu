@@ -312,6 +312,17 @@ static double shape_radius(const vg_shape *s)
         double zm = std::fmax(std::fabs(c.zlo), std::fabs(c.zhi));
         return std::sqrt(c.rb2 + zm * zm);
     }
+    if (s->kind == kCsg) { // any tree lies inside the union of its primitives
+        const CsgP &c = s->u.csg;
+        double r = 0;
+        for (int i = 0; i < c.nleaf; ++i) {
+            const double *m = c.X[i];
+            double cx = -(m[0] * m[3] + m[4] * m[7] + m[8] * m[11]), cy = -(m[1] * m[3] + m[5] * m[7] + m[9] * m[11]),
+                   cz = -(m[2] * m[3] + m[6] * m[7] + m[10] * m[11]);
+            r = std::fmax(r, std::sqrt(cx * cx + cy * cy + cz * cz) + bounding_radius(c.leaf[i]));
+        }
+        return r;
+    }
     if (s->kind == VG_BOOLEAN) {
         const BoolP &c = s->u.boolean;
         double ra = bounding_radius(c.a);
@@ -637,6 +648,7 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     std::vector<int> count(nn, 0), fill(nn, 0);
     std::vector<PolyconeP> pcons;
     std::vector<BoolP> bools;
+    std::vector<CsgP> csgs;
     std::vector<double> radius(nn, 0.0);
     for (int i = 1; i < nn; ++i) {
         if (parent[i] < 0 || parent[i] >= i) return fail(VG_ERR_PARAM, "%s: need 0 <= parent[%d] < %d", fn, i, i);
@@ -658,6 +670,10 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
             N.s.kind = kBoolean;
             N.ext = int(bools.size());
             bools.push_back(shapes[i]->u.boolean);
+        } else if (shapes[i]->kind == kCsg) {
+            N.s.kind = kCsg;
+            N.ext = int(csgs.size());
+            csgs.push_back(shapes[i]->u.csg);
         } else {
             int rc = to_solid(shapes[i], &N.s, "node");
             if (rc != VG_OK) return rc;
@@ -705,18 +721,20 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     w->nn = nn;
     auto up16 = [](size_t v) { return (v + 15) / 16 * 16; };
     const size_t nbytes = size_t(nn) * sizeof(WorldNode), cbytes = cull.size() * sizeof(float), kbytes = up16(kids.size() * sizeof(int32_t));
-    const size_t pbytes = up16(pcons.size() * sizeof(PolyconeP)), bbytes = bools.size() * sizeof(BoolP);
+    const size_t pbytes = up16(pcons.size() * sizeof(PolyconeP)), bbytes = up16(bools.size() * sizeof(BoolP)), gbytes = csgs.size() * sizeof(CsgP);
     static_assert(sizeof(WorldNode) % 16 == 0, "the float4 array follows the node records");
     unsigned char *blob = nullptr;
     cudaError_t e = cudaGetDevice(&w->device);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + cbytes + kbytes + pbytes + bbytes + 16);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + cbytes + kbytes + pbytes + bbytes + gbytes + 16);
     if (e == cudaSuccess) e = cudaMemcpy(blob, nodes.data(), nbytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes, cull.data(), cbytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes + cbytes, kids.data(), kids.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e == cudaSuccess && !pcons.empty())
         e = cudaMemcpy(blob + nbytes + cbytes + kbytes, pcons.data(), pcons.size() * sizeof(PolyconeP), cudaMemcpyHostToDevice);
     if (e == cudaSuccess && !bools.empty())
-        e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes, bools.data(), bbytes, cudaMemcpyHostToDevice);
+        e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes, bools.data(), bools.size() * sizeof(BoolP), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !csgs.empty())
+        e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes + bbytes, csgs.data(), gbytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
         if (blob) cudaFree(blob);
         delete w;
@@ -728,8 +746,9 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     w->tab.kids = reinterpret_cast<int32_t *>(blob + nbytes + cbytes);
     w->tab.pcons = reinterpret_cast<PolyconeP *>(blob + nbytes + cbytes + kbytes);
     w->tab.bools = reinterpret_cast<BoolP *>(blob + nbytes + cbytes + kbytes + pbytes);
+    w->tab.csgs = reinterpret_cast<CsgP *>(blob + nbytes + cbytes + kbytes + pbytes + bbytes);
     w->tab.nnodes = nn;
-    w->tab.has_ext = !(pcons.empty() && bools.empty());
+    w->tab.has_ext = !(pcons.empty() && bools.empty() && csgs.empty());
     *out = w;
     return VG_OK;
 }

@@ -1,0 +1,135 @@
+// vg_csg.cuh -- device code of the nested booleans (reading R31); see vg_csg.cu for the design.
+#pragma once
+#include "vg_bool.cuh"
+
+namespace vg {
+
+constexpr int kCsgMaxEvents = 16 * kCsgMaxLeaf;
+
+// the tree's membership from one bit per primitive; the stack lives in the bits of `st`
+VG_DEV bool csg_member(const CsgP &p, unsigned bits)
+{
+    unsigned st = 0;
+    int sp = 0;
+#pragma unroll 1
+    for (int k = 0; k < p.nprog; ++k) {
+        const unsigned tok = p.prog[k];
+        if (tok < 0x80u) {
+            st = (st & ~(1u << sp)) | (((bits >> tok) & 1u) << sp);
+            ++sp;
+        } else {
+            const bool b = (st >> (sp - 1)) & 1u, a = (st >> (sp - 2)) & 1u;
+            const bool r = bool_member(int(tok & 0x7fu), a, b);
+            sp -= 1;
+            st = (st & ~(1u << (sp - 1))) | (unsigned(r) << (sp - 1));
+        }
+    }
+    return st & 1u;
+}
+
+VG_DEV void csg_to_leaf(const double *m, double x, double y, double z, double &lx, double &ly, double &lz)
+{
+    lx = fma(m[0], x, fma(m[1], y, fma(m[2], z, m[3])));
+    ly = fma(m[4], x, fma(m[5], y, fma(m[6], z, m[7])));
+    lz = fma(m[8], x, fma(m[9], y, fma(m[10], z, m[11])));
+}
+
+// classes of all primitives as two bit sets (strictly inside / strictly outside)
+VG_DEV void csg_classes(const CsgP &p, double x, double y, double z, unsigned &in, unsigned &out)
+{
+    in = out = 0;
+#pragma unroll 1
+    for (int i = 0; i < p.nleaf; ++i) {
+        double lx, ly, lz;
+        csg_to_leaf(p.X[i], x, y, z, lx, ly, lz);
+        const int c = solid_inside(p.leaf[i], lx, ly, lz);
+        in |= unsigned(c == cInside) << i;
+        out |= unsigned(c == cOutside) << i;
+    }
+}
+
+// R27 read recursively: the program on (in, out) pairs
+VG_DEV int csg_classify(const CsgP &p, unsigned in, unsigned out)
+{
+    unsigned sin = 0, sout = 0;
+    int sp = 0;
+#pragma unroll 1
+    for (int k = 0; k < p.nprog; ++k) {
+        const unsigned tok = p.prog[k];
+        if (tok < 0x80u) {
+            sin = (sin & ~(1u << sp)) | (((in >> tok) & 1u) << sp);
+            sout = (sout & ~(1u << sp)) | (((out >> tok) & 1u) << sp);
+            ++sp;
+        } else {
+            const bool bin = (sin >> (sp - 1)) & 1u, bout = (sout >> (sp - 1)) & 1u;
+            const bool ain = (sin >> (sp - 2)) & 1u, aout = (sout >> (sp - 2)) & 1u;
+            const int op = int(tok & 0x7fu);
+            bool rin, rout;
+            if (op == kUnion) rin = ain || bin, rout = aout && bout;
+            else if (op == kIntersection) rin = ain && bin, rout = aout || bout;
+            else rin = ain && bout, rout = aout || bin;
+            sp -= 1;
+            sin = (sin & ~(1u << (sp - 1))) | (unsigned(rin) << (sp - 1));
+            sout = (sout & ~(1u << (sp - 1))) | (unsigned(rout) << (sp - 1));
+        }
+    }
+    return classify(sin & 1u, sout & 1u);
+}
+
+// R29 read recursively: the program on signed distances
+VG_DEV double csg_sdf(const CsgP &p, double x, double y, double z)
+{
+    double st[kCsgMaxLeaf];
+    int sp = 0;
+#pragma unroll 1
+    for (int k = 0; k < p.nprog; ++k) {
+        const unsigned tok = p.prog[k];
+        if (tok < 0x80u) {
+            double lx, ly, lz;
+            csg_to_leaf(p.X[tok], x, y, z, lx, ly, lz);
+            st[sp++] = solid_sdf(p.leaf[tok], lx, ly, lz);
+        } else {
+            const double b = st[sp - 1], a = st[sp - 2];
+            const int op = int(tok & 0x7fu);
+            sp -= 1;
+            st[sp - 1] = op == kUnion ? dmin(a, b) : (op == kIntersection ? dmax(a, b) : dmax(a, -b));
+        }
+    }
+    return st[0];
+}
+
+// R28 read recursively
+VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, double z, double dx, double dy, double dz)
+{
+    unsigned in, out;
+    csg_classes(p, x, y, z, in, out);
+    const int cls = csg_classify(p, in, out);
+    if ((!to_out && cls == cInside) || (to_out && cls == cOutside)) return -1.0;
+    unsigned bits = in;
+    const bool start = csg_member(p, bits);
+    double tt = 0.0;
+#pragma unroll 1
+    for (int it = 0; it < kCsgMaxEvents; ++it) {
+        double emin = inf();
+        int imin = -1;
+        const double px = fma(tt, dx, x), py = fma(tt, dy, y), pz = fma(tt, dz, z);
+#pragma unroll 1
+        for (int i = 0; i < p.nleaf; ++i) {
+            const double *m = p.X[i];
+            double lx, ly, lz;
+            csg_to_leaf(m, px, py, pz, lx, ly, lz);
+            const double ldx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
+            const double ldy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
+            const double ldz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
+            const double e = solid_next<-1>(p.leaf[i], (bits >> i) & 1u, lx, ly, lz, ldx, ldy, ldz);
+            if (e < emin) emin = e, imin = i; // strict: the lowest leaf wins a tie
+        }
+        if (imin < 0) break;
+        tt += emin;
+        bits ^= 1u << imin;
+        if (csg_member(p, bits) != start) return tt;
+    }
+    return inf();
+}
+
+} // namespace vg

@@ -190,7 +190,8 @@ struct WorldTab {
     const int32_t *kids;          // the child lists
     const float4 *cull;           // FP32 bounding spheres in child-list order
     const struct PolyconeP *pcons; // nodes that are polycones (reading R30)
-    const struct BoolP *bools;     // nodes that are booleans
+    const struct BoolP *bools;     // nodes that are booleans of two primitives
+    const struct CsgP *csgs;       // nodes that are nested booleans (reading R31)
     int nnodes;
     int has_ext;                   // any polycone / boolean node: the kernels with their code are launched
 };

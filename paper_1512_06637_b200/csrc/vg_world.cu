@@ -13,7 +13,7 @@
 // child's DistanceToIn is +inf, its Inside is OUTSIDE and its SafetyToIn exceeds the running minimum, i.e. results
 // are identical to visiting every child.  Children are visited in ascending node index, so the strict `<` scan is
 // the tie-break of R13.
-#include "vg_bool.cuh"
+#include "vg_csg.cuh"
 
 namespace vg {
 
@@ -38,11 +38,17 @@ VG_DEV void xf_dir(const double *m, double dx, double dy, double dz, double &lx,
 
 __device__ __noinline__ int ext_inside(const WorldTab &w, const WorldNode &N, double x, double y, double z)
 {
+    if (N.s.kind == kCsg) {
+        unsigned in, out;
+        csg_classes(w.csgs[N.ext], x, y, z, in, out);
+        return csg_classify(w.csgs[N.ext], in, out);
+    }
     return N.s.kind == kPolycone ? Polycone::inside(w.pcons[N.ext], x, y, z) : bool_inside_pt(w.bools[N.ext], x, y, z);
 }
 
 __device__ __noinline__ double ext_sdf(const WorldTab &w, const WorldNode &N, double x, double y, double z)
 {
+    if (N.s.kind == kCsg) return csg_sdf(w.csgs[N.ext], x, y, z);
     return N.s.kind == kPolycone ? Polycone::safety(w.pcons[N.ext], x, y, z) : bool_sdf_pt(w.bools[N.ext], x, y, z);
 }
 
@@ -51,6 +57,7 @@ __device__ __noinline__ double ext_distance(const WorldTab &w, const WorldNode &
 {
     if (N.s.kind == kPolycone)
         return to_out ? Polycone::dist_out(w.pcons[N.ext], x, y, z, dx, dy, dz) : Polycone::dist_in(w.pcons[N.ext], x, y, z, dx, dy, dz);
+    if (N.s.kind == kCsg) return csg_distance(w.csgs[N.ext], to_out, x, y, z, dx, dy, dz);
     return bool_distance<-1, -1>(w.bools[N.ext], to_out, x, y, z, dx, dy, dz);
 }
 

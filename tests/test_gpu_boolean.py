@@ -244,5 +244,38 @@ def test_nested_boolean_limits(vg):
         c = vg.Boolean(vg.UNION, c, a, ident)  # 8 primitives: the limit
     with pytest.raises(vg.VgError):
         vg.Boolean(vg.UNION, c, a, ident)
-    with pytest.raises(vg.VgError):
-        vg.World([vg.Shape(W.BOX, [10, 10, 10]), c], [-1, 0], [ident, ident])  # a nested boolean is not a node in this build
+
+
+def test_nested_boolean_as_a_world_node_and_a_daughter(vg):
+    """A tree placed in a box: node of a world (R30 + R31) and daughter of a volume, against the oracle's world."""
+    cc = CSG["twice_drilled_block_in_a_sphere"]
+    q = np.array([0.3, -0.4, 0.5, 0.7])
+    xf = [W.placement(np.eye(3), (0, 0, 0)), W.placement(W.quaternion_to_matrix(tuple(q / np.linalg.norm(q))), (3.0, -2.0, 4.0))]
+    wo = O.World([O.Shape(W.BOX, [30, 30, 30]), cc.build(O)], [-1, 0], xf)
+    wg = vg.World([vg.Shape(W.BOX, [30, 30, 30]), cc.build(vg)], [-1, 0], xf)
+    leaves = wo.shapes[1].leaves()
+    M1 = np.asarray(xf[1]).reshape(3, 4)
+
+    def band(x, y, z):
+        L1 = M1[:, :3] @ np.stack([x, y, z]) + M1[:, 3:4]
+        bad = np.abs(wo.shapes[0].sdf(x, y, z)) < W.SURFACE_BAND
+        for shape, M in leaves:
+            L = M[:, :3] @ L1 + M[:, 3:4]
+            bad |= np.abs(shape.sdf(L[0], L[1], L[2])) < W.SURFACE_BAND
+        return bad
+    t = W.draw_tracks(61, 200003, (3, -2, 4), (16, 16, 16), band)
+    dt = dev(t)
+    node_o, node_g = wo.locate(*t[:3]), wg.locate(*dt[:3])
+    assert_int_equal(node_g.cpu().numpy(), node_o, "tree node locate")
+    assert (node_o == 1).mean() > 0.05
+    so, no = wo.step(node_o, *t, W.STEP_MAX)
+    sg, ng = wg.step(node_g, *dt, W.STEP_MAX)
+    assert_int_equal(ng.cpu().numpy(), no, "tree node next")
+    assert_real_close(sg.cpu().numpy(), so, "tree node step")
+    assert_real_close(wg.safety(node_g, *dt[:3]).cpu().numpy(), wo.safety(node_o, *t[:3]), "tree node safety")
+    vol = vg.Volume(vg.Shape(W.BOX, [30, 30, 30]), [cc.build(vg)], [xf[1]])
+    root = node_o == 0
+    tr = [np.ascontiguousarray(a[root]) for a in t]
+    sv, hv = vol.compute_step(*dev(tr), W.STEP_MAX)
+    assert_real_close(sv.cpu().numpy(), so[root], "tree daughter step")
+    assert_int_equal(hv.cpu().numpy(), np.where(no[root] < 0, -1, no[root] - 1), "tree daughter hit")
