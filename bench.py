@@ -116,7 +116,7 @@ class ClockSampler:
 class Case:
     """One solid (or the navigation volume) with its seeded tracks resident in HBM as `nsets` rotating copies."""
 
-    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None, world=None, boolean=None):
+    def __init__(self, vg, torch, name, n, queries, seed_shift=0, shape=None, nav=None, world=None, boolean=None, csg=None):
         self.vg, self.torch, self.name, self.n, self.queries = vg, torch, name, int(n), tuple(queries)
         dev = torch.device("cuda", torch.cuda.current_device())
         self.nodes = None
@@ -130,6 +130,26 @@ class Case:
                 nd = self.handle.locate(*d)
                 s = self.handle.safety(torch.clamp(nd, min=0), *d)
                 return ((nd < 0) | (s < W.SURFACE_BAND)).cpu().numpy()
+        elif csg is not None:  # a nested boolean (reading R31)
+            self.kind = "boolean"
+            self.handle = csg.build(vg)
+            seed, center, half = csg.seed + seed_shift, csg.center, csg.half
+            leaves = []  # (primitive handle, 4x4 frame of the tree -> frame of the primitive), composed here for the band only
+
+            def walk(t, pre):
+                if t[0] == "leaf":
+                    leaves.append((vg.Shape(t[1], t[2]), pre))
+                    return
+                walk(t[2], pre)
+                walk(t[3], np.vstack([np.asarray(t[4]).reshape(3, 4), [0, 0, 0, 1]]) @ pre)
+            walk(csg.tree, np.eye(4))
+
+            def band(x, y, z):  # clear of the surface of every primitive of the tree (library's own safeties)
+                bad = np.zeros(len(x), dtype=bool)
+                for h, M in leaves:
+                    L = M[:3, :3] @ np.stack([x, y, z]) + M[:3, 3:4]
+                    bad |= np.abs(self._gpu3(h.safety_to_in, L[0], L[1], L[2])) < W.SURFACE_BAND
+                return bad
         elif boolean is not None:
             self.kind = "boolean"
             a, b = vg.Shape(boolean.kind_a, boolean.par_a), vg.Shape(boolean.kind_b, boolean.par_b)
@@ -488,6 +508,15 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
             rows.append(e)
         del case
         torch.cuda.empty_cache()
+    cc = [c for c in W.csg_cases() if c.name == "twice_drilled_block_in_a_sphere"][0]  # a tree of four primitives (R31)
+    case = Case(vg, torch, cc.name, 4194304, W.QUERIES5, csg=cc)
+    for q in case.queries:
+        sec = time_query_alone(torch, case, q)
+        e = roofline_entry("boolean", q, case.n, sec, hbm_peak, fma_rate)
+        e.update({"config": "8(f) f2", "shape": "csg tree: " + cc.name, "query": q, "n": case.n, "cold_inputs": case.cold, "bound": "alu"})
+        rows.append(e)
+    del case
+    torch.cuda.empty_cache()
     # the three-level tree of placed solids (193 nodes), every track in its own node
     wc = W.world_case()
     case = Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc)

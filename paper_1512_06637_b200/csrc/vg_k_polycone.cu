@@ -23,6 +23,9 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
         }
         return launch_any<Polycone, PolyconeT<solid_flags(false, kWmFull)>>(q, p, t, step_max, n, out, vec, s);
     }
+    // a phi cut: the ordered walk serves DistanceToIn (every candidate also tested against the segment, the phi faces added)
+    if (vec && q == qDistIn && g_form.load(std::memory_order_relaxed) == 0)
+        return launch_pcon_walk<qDistIn, false, true>(p, g, t, step_max, n, static_cast<double *>(out), s);
     return launch_any<Polycone>(q, p, t, step_max, n, out, vec, s);
 }
 

@@ -100,11 +100,30 @@ VG_DEV double pcon_step_d2(const PolyconeP &p, int k, double u, double v, double
     return d2;
 }
 
-// DistanceToIn of the full-phi polycone; same candidates and validity tests as PolyconeT::dist_in
+// (u, v) in the closed (r, z) outline?  Same set as PolyconeT::in_outline (the union of the closed sections), from the
+// section that holds v and, on a shared plane, the one below it
+VG_DEV bool pcon_in_outline(const PolyconeP &p, const PconWalkSec *tab, double u, double v)
+{
+    const int k = pcon_section_of(p, v);
+    const PconWalkSec &w = tab[k];
+    bool in = v >= w.z0 && v <= w.z1 && u <= fma(w.Bo, v, w.Ao) && u >= fma(w.Bi, v, w.Ai);
+    if (k > 0 && v <= tab[k - 1].z1) {
+        const PconWalkSec &b = tab[k - 1];
+        in = in || (v >= b.z0 && u <= fma(b.Bo, v, b.Ao) && u >= fma(b.Bi, v, b.Ai));
+    }
+    return in;
+}
+
+// DistanceToIn of the polycone; same candidates and validity tests as PolyconeT::dist_in.  WEDGE: the polycone has a phi
+// cut: every crossing must also lie in the segment (linear test along the ray), the two phi faces are two more candidates
+// (entering sense, hit point inside the (r, z) outline) taken after the walk, and Inside includes the wedge.
+template <bool WEDGE>
 VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z, double dx,
                                 double dy, double dz)
 {
     RayRZ r;
+    WedgeEval ep = {}, ed = {};
+    if (WEDGE) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
     r.rho2 = fma(x, x, y * y);
     r.a_xy = fma(dx, dx, dy * dy);
     r.b_xy = fma(x, dx, y * dy);
@@ -143,6 +162,10 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
         const bool inner = (p.inner_mask >> kz) & 1u;
         in = z > p.zlo + kTol && z < p.zhi - kTol && ro > 0.0 && r.rho2 < ro * ro && (!inner || ri < 0.0 || r.rho2 > ri * ri);
         if (p.step_mask) in = in && !pcon_near_step(p, kz, r.rho2, z) && !pcon_near_step(p, kz - 1, r.rho2, z);
+        if (WEDGE) {
+            bool out_unused = false;
+            wedge_classify<kWmRuntime>(p.w, ep, r.rho2, in, out_unused);
+        }
     }
 
     // a ray that starts beyond an end plane meets that cap before anything else
@@ -150,7 +173,8 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
     const double rc2 = fma(tc, fma(tc, a, b + b), r.rho2);
     const double clo = up ? p.cap_lo_rmin : p.cap_hi_rmin, chi = up ? p.cap_lo_rmax : p.cap_hi_rmax;
     const bool beyond = up ? z < p.zlo : z > p.zhi;
-    const bool cap_hit = beyond && !horizontal && rc2 >= clo * clo && rc2 <= chi * chi;
+    bool cap_hit = beyond && !horizontal && rc2 >= clo * clo && rc2 <= chi * chi;
+    if (WEDGE) cap_hit = cap_hit && wedge_member_at<kWmRuntime>(p.w, ep, ed, tc);
 
     double best = cap_hit ? tc : inf();
     bool go = rad_ok && z_ok && t0 <= t1 && !in && !cap_hit;
@@ -168,18 +192,36 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
         double t = frustum_root(f, r, z, dz, false, ok); // outer patch, entering root
         double zh = fma(t, dz, z);
         ok = ok && zh >= w.z0 && zh <= w.z1;
+        if (WEDGE) ok = ok && wedge_member_at<kWmRuntime>(p.w, ep, ed, t);
         best = (ok && t < best) ? t : best;
         f.A = w.Ai, f.B = w.Bi;
         t = frustum_root(f, r, z, dz, true, ok); // inner patch: the ray enters where it leaves the bore
         zh = fma(t, dz, z);
         ok = ok && ((p.inner_mask >> k) & 1u) && zh >= w.z0 && zh <= w.z1;
+        if (WEDGE) ok = ok && wedge_member_at<kWmRuntime>(p.w, ep, ed, t);
         best = (ok && t < best) ? t : best;
         go = !(best < inf()) && k != kend;
         if (go && p.step_mask) { // the step face on the plane the ray crosses next comes before anything of the next section
-            best = pcon_step_enter(p, up ? k : k - 1, r, z, dz, idz);
-            go = !(best < inf());
+            const double ts = pcon_step_enter(p, up ? k : k - 1, r, z, dz, idz);
+            const bool ok_s = ts < inf() && (!WEDGE || wedge_member_at<kWmRuntime>(p.w, ep, ed, ts));
+            best = ok_s ? ts : best;
+            go = !ok_s;
         }
         k += step;
+    }
+    if (WEDGE) { // the two phi faces, entering sense; the hit point must lie in the (r, z) outline (R1: closed)
+        {
+            const double t = -ep.c0 * rcp(ed.c0);
+            const bool ok = ed.c0 > 0.0 && t > 0.0 && t < best &&
+                            pcon_in_outline(p, tab, fma(t, ed.u0, ep.u0), fma(t, dz, z));
+            best = ok ? t : best;
+        }
+        {
+            const double t = -ep.c1 * rcp(ed.c1);
+            const bool ok = ed.c1 > 0.0 && t > 0.0 && t < best &&
+                            pcon_in_outline(p, tab, fma(t, ed.u1, ep.u1), fma(t, dz, z));
+            best = ok ? t : best;
+        }
     }
     return in ? -1.0 : best;
 }
@@ -304,7 +346,7 @@ VG_DEV double pcon_grid_sdf(const PolyconeP &p, const PconWalkSec *tab, const do
     return in2d ? -dist : dist;
 }
 
-template <int Q, bool GRID>
+template <int Q, bool GRID, bool WEDGE>
 VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x,
                              double y, double z, double dx, double dy, double dz, double step_max)
 {
@@ -312,7 +354,7 @@ VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const d
         const double s = GRID ? pcon_grid_sdf(p, tab, seg, g, x, y, z) : pcon_walk_sdf(p, tab, x, y, z);
         return Q == qSafeIn ? s : -s;
     }
-    const double t = pcon_walk_dist_in(p, tab, x, y, z, dx, dy, dz);
+    const double t = pcon_walk_dist_in<WEDGE>(p, tab, x, y, z, dx, dy, dz);
     return t <= step_max ? t : inf();
 }
 
@@ -321,7 +363,7 @@ VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const d
 #endif
 
 // persistent CTAs striding over tiles of 512 tracks, two tracks per thread (128-bit loads; arrays 16-byte aligned)
-template <int Q, bool GRID>
+template <int Q, bool GRID, bool WEDGE>
 __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
     pcon_walk_kernel(const __grid_constant__ PolyconeP p, const __grid_constant__ PconGrid g, Tracks t, double step_max,
                      int64_t n, double *out)
@@ -341,19 +383,19 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
             double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
             double2 dx = make_double2(0, 0), dy = dx, dz = dx;
             if (kDir) dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
-            const double r0 = pcon_walk_eval<Q, GRID>(p, tab, seg, g, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max);
-            const double r1 = pcon_walk_eval<Q, GRID>(p, tab, seg, g, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max);
+            const double r0 = pcon_walk_eval<Q, GRID, WEDGE>(p, tab, seg, g, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max);
+            const double r1 = pcon_walk_eval<Q, GRID, WEDGE>(p, tab, seg, g, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max);
             stg2(out + i, r0, r1);
         } else {
             double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
             double dx = 0, dy = 0, dz = 0;
             if (kDir) dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
-            stg1(out + i, pcon_walk_eval<Q, GRID>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max));
+            stg1(out + i, pcon_walk_eval<Q, GRID, WEDGE>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max));
         }
     }
 }
 
-template <int Q, bool GRID>
+template <int Q, bool GRID, bool WEDGE = false>
 cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, double *out,
                              cudaStream_t s)
 {
@@ -364,14 +406,14 @@ cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks
         cudaError_t e;
         if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
         if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_walk_kernel<Q, GRID>, kWalkBlock, 0)) != cudaSuccess) return e;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_walk_kernel<Q, GRID, WEDGE>, kWalkBlock, 0)) != cudaSuccess) return e;
         cap = sms * (per_sm < 1 ? 1 : per_sm);
         cap_cache.store(cap, std::memory_order_release);
     }
     const int64_t npairs = (n + 1) >> 1;
     int64_t grid = (npairs + kWalkBlock - 1) / kWalkBlock;
     if (grid > cap) grid = cap;
-    return launch_kernel(pcon_walk_kernel<Q, GRID>, unsigned(grid), kWalkBlock, 0, s, p, g, t, step_max, n, out);
+    return launch_kernel(pcon_walk_kernel<Q, GRID, WEDGE>, unsigned(grid), kWalkBlock, 0, s, p, g, t, step_max, n, out);
 }
 
 } // namespace vg
