@@ -85,8 +85,8 @@ typedef enum {
  *   dphi >= 2 pi (as FP64) means the full revolution.
  * Validation (VG_ERR_PARAM): wrong nparams, non-finite values, lengths <= 0, rmin < 0, rmin >= rmax at any
  * plane, dphi <= 0, nz out of range or not an integer, z decreasing, a z step that breaks the rules above.
- * On success *out receives a handle; derived constants are computed once here on the host.  For a full-phi polycone
- * the candidate grid of its safeties (DESIGN.md sec. 6.2, 65 KiB) is built here and placed on the CURRENT device if
+ * On success *out receives a handle; derived constants are computed once here on the host.  For a polycone
+ * the candidate grid of its safeties (DESIGN.md sec. 6.2, 65 KiB; 193 KiB with a phi cut) is built here and placed on the CURRENT device if
  * there is one; on another device, or without one at create time, the safeties run the ordered-walk kernel instead.
  */
 int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **out);

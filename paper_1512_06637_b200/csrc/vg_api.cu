@@ -97,21 +97,25 @@ static void upload_pcon_grid(vg_shape *s)
         cudaGetLastError();
         return;
     }
-    std::vector<unsigned long long> masks;
-    std::vector<unsigned char> rows;
-    PconGridGeom geom;
-    pcon_grid_build(s->u.pcon, &geom, &masks, &rows);
-    const size_t mbytes = masks.size() * sizeof(unsigned long long);
+    std::vector<unsigned long long> masks, fmasks;
+    std::vector<unsigned char> rows, rows2;
+    PconGridGeom geom, geom2;
+    pcon_grid_build(s->u.pcon, false, &geom, &masks, &rows);
+    if (!s->u.pcon.w.full) pcon_grid_build(s->u.pcon, true, &geom2, &fmasks, &rows2); // same geometry, twice the columns
+    const size_t mbytes = masks.size() * sizeof(unsigned long long), fbytes = fmasks.size() * sizeof(unsigned long long);
     unsigned char *blob = nullptr;
-    if (cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + rows.size()) != cudaSuccess ||
-        cudaMemcpy(blob, masks.data(), mbytes, cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(blob + mbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + rows.size()) == cudaSuccess &&
+              cudaMemcpy(blob, masks.data(), mbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
+              (fbytes == 0 || cudaMemcpy(blob + mbytes, fmasks.data(), fbytes, cudaMemcpyHostToDevice) == cudaSuccess) &&
+              cudaMemcpy(blob + mbytes + fbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) {
         cudaGetLastError();
         if (blob) cudaFree(blob);
         return;
     }
     s->grid.masks = reinterpret_cast<const unsigned long long *>(blob);
-    s->grid.rows = blob + mbytes;
+    s->grid.face_masks = fbytes ? reinterpret_cast<const unsigned long long *>(blob + mbytes) : nullptr;
+    s->grid.rows = blob + mbytes + fbytes;
     s->grid.g = geom;
     s->grid_device = dev;
 }
@@ -130,7 +134,7 @@ extern "C" int vg_shape_create(vg_kind kind, const double *params, int nparams, 
         delete s;
         return rc;
     }
-    if (kind == VG_POLYCONE && s->u.pcon.w.full) upload_pcon_grid(s);
+    if (kind == VG_POLYCONE) upload_pcon_grid(s);
     *out = s;
     return VG_OK;
 }

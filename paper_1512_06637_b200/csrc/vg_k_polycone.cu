@@ -26,6 +26,11 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
     // a phi cut: the ordered walk serves DistanceToIn (every candidate also tested against the segment, the phi faces added)
     if (vec && q == qDistIn && g_form.load(std::memory_order_relaxed) == 0)
         return launch_pcon_walk<qDistIn, false, true>(p, g, t, step_max, n, static_cast<double *>(out), s);
+    // ... and the two candidate grids (surface of revolution, phi face) the safeties
+    if (vec && g.masks && g.face_masks && g_form.load(std::memory_order_relaxed) == 0) {
+        if (q == qSafeIn) return launch_pcon_walk<qSafeIn, true, true>(p, g, t, step_max, n, static_cast<double *>(out), s);
+        if (q == qSafeOut) return launch_pcon_walk<qSafeOut, true, true>(p, g, t, step_max, n, static_cast<double *>(out), s);
+    }
     return launch_any<Polycone>(q, p, t, step_max, n, out, vec, s);
 }
 

@@ -111,6 +111,7 @@ struct PconGridGeom {
 
 struct PconGrid {
     const unsigned long long *masks; // [kPconGridZ][kPconGridR]; NULL: no grid, the ordered walk serves the safeties
+    const unsigned long long *face_masks; // phi cut only: [kPconGridZ][2 kPconGridR] over u in [-R, R), every outline edge
     const unsigned char *rows;       // [kPconGridZ]
     PconGridGeom g;
 };

@@ -67,15 +67,19 @@ static inline bool pg_seg_meets_rect(const PconSegH &s, double u0, double u1, do
 
 // segment numbering shared with the kernel (vg_params.h): bits 0 / 1 = the caps, 2 + 2k / 3 + 2k = outer / inner edge of
 // section k, then two bits per z step
-static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::vector<unsigned long long> *masks,
+// `face` = false: the grid of the surface of revolution (rho in [0, R): kPconGridR columns, edges on the axis left out).
+// `face` = true: the grid of a phi FACE (u in [-R, R): 2 kPconGridR columns, EVERY edge of the outline: on a face the
+// edges on the axis bound the filled outline too, c.3), used for points outside the outline.
+static inline void pcon_grid_build(const PolyconeP &c, bool face, PconGridGeom *geom, std::vector<unsigned long long> *masks,
                                    std::vector<unsigned char> *rows)
 {
     std::vector<PconSegH> segs;
     double rmax = 0;
+    const int ncol = face ? 2 * kPconGridR : kPconGridR;
     for (int k = 0; k < c.nsec; ++k) {
         const PconSec &s = c.sec[k];
         segs.push_back(PconSegH{ s.out.r0, s.z0, s.out.r0 + s.out.er, s.z1, kPconSecBit0 + 2 * k });
-        if ((c.inner_mask >> k) & 1u) segs.push_back(PconSegH{ s.in.r0, s.z0, s.in.r0 + s.in.er, s.z1, kPconSecBit0 + 2 * k + 1 });
+        if (face || ((c.inner_mask >> k) & 1u)) segs.push_back(PconSegH{ s.in.r0, s.z0, s.in.r0 + s.in.er, s.z1, kPconSecBit0 + 2 * k + 1 });
         rmax = pg_max(rmax, pg_max(s.out.r0, s.out.r0 + s.out.er));
     }
     for (int k = 0, j = 0; k + 1 < c.nsec; ++k) { // the annular faces of the z steps (R26), bits after the sections
@@ -98,19 +102,20 @@ static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::
     const size_t ns = segs.size();
 
     // corner lattice of squared distances, one layer per segment
-    const int LR = kPconGridR + 1, LZ = kPconGridZ + 1;
+    const int LR = ncol + 1, LZ = kPconGridZ + 1;
+    const double umin = face ? -R : 0.0;
     std::vector<double> D(ns * size_t(LR) * LZ);
     for (size_t s = 0; s < ns; ++s) {
         const double er = segs[s].r1 - segs[s].r0, ez = segs[s].z1 - segs[s].z0, inv_l2 = 1.0 / (er * er + ez * ez);
         for (int j = 0; j < LZ; ++j)
-            for (int i = 0; i < LR; ++i) D[(s * LZ + j) * LR + i] = pg_dist2_seg(i * cr, zg0 + j * cz, segs[s], inv_l2);
+            for (int i = 0; i < LR; ++i) D[(s * LZ + j) * LR + i] = pg_dist2_seg(umin + i * cr, zg0 + j * cz, segs[s], inv_l2);
     }
 
-    masks->assign(size_t(kPconGridR) * kPconGridZ, 0ull);
+    masks->assign(size_t(ncol) * kPconGridZ, 0ull);
     std::vector<double> dmin(ns);
     for (int j = 0; j < kPconGridZ; ++j)
-        for (int i = 0; i < kPconGridR; ++i) {
-            const double u0 = i * cr, u1 = u0 + cr, v0 = zg0 + j * cz, v1 = v0 + cz;
+        for (int i = 0; i < ncol; ++i) {
+            const double u0 = umin + i * cr, u1 = u0 + cr, v0 = zg0 + j * cz, v1 = v0 + cz;
             double thr = INFINITY;
             for (size_t s = 0; s < ns; ++s) {
                 const double *L = &D[(s * LZ + j) * LR + i];
@@ -131,7 +136,7 @@ static inline void pcon_grid_build(const PolyconeP &c, PconGridGeom *geom, std::
             unsigned long long m = 0;
             for (size_t s = 0; s < ns; ++s)
                 if (dmin[s] <= thr) m |= 1ull << segs[s].bit;
-            (*masks)[size_t(j) * kPconGridR + i] = m;
+            (*masks)[size_t(j) * ncol + i] = m;
         }
 
     // section index at (slightly below) the lower edge of every z row: the kernel counts on from there

@@ -346,12 +346,62 @@ VG_DEV double pcon_grid_sdf(const PolyconeP &p, const PconWalkSec *tab, const do
     return in2d ? -dist : dist;
 }
 
+// minimum squared distance from (u, v) to the candidate segments of its cell; `col0` / `ncol`: the surface grid starts at
+// u = 0 with kPconGridR columns, the face grid at u = -R with twice as many.  Off the grid: NaN.
+VG_DEV double pcon_grid_d2(const unsigned long long *masks, int ncol, double u_shift, const double *seg, const PconGrid &g,
+                           double u, double v)
+{
+    const double fr = (u + u_shift) * g.g.inv_cr, fz = (v - g.g.zg0) * g.g.inv_cz;
+    if (!(fr >= 0.0 && fr < double(ncol) && fz >= 0.0 && fz < double(kPconGridZ))) return __longlong_as_double(0x7ff8000000000000LL);
+    const uint2 m = __ldg(reinterpret_cast<const uint2 *>(masks) + int(fz) * ncol + int(fr));
+    double d2 = inf();
+    unsigned w = m.x;
+    while (w) {
+        const int s = __ffs(int(w)) - 1;
+        w &= w - 1;
+        d2 = dmin(d2, pcon_seg_d2(u, v, seg + kPconSegStride * s));
+    }
+    w = m.y;
+    while (w) {
+        const int s = __ffs(int(w)) + 31;
+        w &= w - 1;
+        d2 = dmin(d2, pcon_seg_d2(u, v, seg + kPconSegStride * s));
+    }
+    return d2;
+}
+
+// signed distance of a polycone WITH a phi cut from the two grids (c.3): the surface of revolution where the point is
+// in the segment, and per phi face the in-plane distance to the filled outline (0 inside it, else the face grid: every
+// edge incl. those on the axis) combined with the distance to the face's plane.  Any look-up off its grid: the generic
+// code (all segments).
+VG_DEV double pcon_grid_sdf_wedge(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x,
+                                  double y, double z)
+{
+    const double rho2 = fma(x, x, y * y);
+    const double rho = sqrt_nn(rho2);
+    const WedgeEval e = wedge_eval(p.w, x, y);
+    const bool mem = wedge_member<kWmRuntime>(p.w, e.c0, e.c1);
+    const double R = double(kPconGridR) / g.g.inv_cr;
+    const double dB = pcon_grid_d2(g.masks, kPconGridR, 0.0, seg, g, rho, z);
+    const bool in0 = pcon_in_outline(p, tab, e.u0, z), in1 = pcon_in_outline(p, tab, e.u1, z);
+    const double f0 = in0 ? 0.0 : pcon_grid_d2(g.face_masks, 2 * kPconGridR, R, seg, g, e.u0, z);
+    const double f1 = in1 ? 0.0 : pcon_grid_d2(g.face_masks, 2 * kPconGridR, R, seg, g, e.u1, z);
+    if (!(dB == dB && f0 == f0 && f1 == f1)) return PolyconeT<kFlagsRuntime>::safety(p, x, y, z); // a NaN: off a grid
+    const bool in2d = pcon_in_outline(p, tab, rho, z);
+    double D2 = mem ? dB : inf();
+    D2 = dmin(D2, fma(e.c0, e.c0, f0));
+    D2 = dmin(D2, fma(e.c1, e.c1, f1));
+    const double D = sqrt_nn(D2);
+    return (mem && in2d) ? -D : D;
+}
+
 template <int Q, bool GRID, bool WEDGE>
 VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x,
                              double y, double z, double dx, double dy, double dz, double step_max)
 {
     if (Q == qSafeIn || Q == qSafeOut) {
-        const double s = GRID ? pcon_grid_sdf(p, tab, seg, g, x, y, z) : pcon_walk_sdf(p, tab, x, y, z);
+        const double s = WEDGE ? pcon_grid_sdf_wedge(p, tab, seg, g, x, y, z)
+                               : (GRID ? pcon_grid_sdf(p, tab, seg, g, x, y, z) : pcon_walk_sdf(p, tab, x, y, z));
         return Q == qSafeIn ? s : -s;
     }
     const double t = pcon_walk_dist_in<WEDGE>(p, tab, x, y, z, dx, dy, dz);

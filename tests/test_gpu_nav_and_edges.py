@@ -459,12 +459,15 @@ def _random_polycone(seed, nz, rmin_hi=5.0):
     return out
 
 
+@pytest.mark.parametrize("wedge", [None, (0.3, 4.0), (-2.0, 1.1), (1.0, math.pi)], ids=["full", "wide", "narrow", "half"])
 @pytest.mark.parametrize("seed,nz,rmin_hi", [(1, 2, 5.0), (2, 3, 0.0), (3, 10, 5.0), (4, 17, 9.0), (5, 32, 5.0), (6, 32, 0.0)])
-def test_polycone_grid_safeties_match_the_oracle(vg, seed, nz, rmin_hi):
+def test_polycone_grid_safeties_match_the_oracle(vg, seed, nz, rmin_hi, wedge):
     """vg_pcon_grid.h: the per-cell candidate masks must hold the nearest segment of every point of the cell.  Points are
     drawn in 3x the bounding box (so some fall off the grid and take the ordered walk inside the same kernel), plus
     points on a lattice that lands exactly on cell corners and edges (rho = i / inv_cr, z = zg0 + j / inv_cz)."""
     par = _random_polycone(seed, nz, rmin_hi)
+    if wedge is not None:  # a phi cut: the surface grid plus the face grid (u in [-R, R), every outline edge)
+        par[0], par[1] = wedge
     so, sg = O.Shape(W.POLYCONE, par), vg.Shape(W.POLYCONE, par)
     c, h = W.bounding_half(W.POLYCONE, par)
     x, y, z = W.draw_tracks(100 + seed, 300001, c, tuple(3.0 * v for v in h))[:3]
