@@ -152,13 +152,21 @@ static cudaError_t launch_nav(const SolidU &mother, const unsigned char *table_d
 {
     if (n <= 0) return cudaSuccess;
     size_t smem = meta.bytes;
-    // per-thread caches of the device queries: the launch path makes no CUDA call but the launch itself
-    static thread_local int sm_count = 0, per_sm = 0;
-    static thread_local size_t smem_granted = 48 * 1024, smem_occ = size_t(-1);
+    // caches of the device queries, per host thread AND per device (the shared-memory opt-in is a per-device attribute of
+    // the kernel): after the first launch on a device the path makes no CUDA call but cudaGetDevice and the launch
+    constexpr int kMaxDev = 64;
+    struct DevCache {
+        int sm_count = 0, per_sm = 0;
+        size_t smem_granted = 48 * 1024, smem_occ = size_t(-1);
+    };
+    static thread_local DevCache cache[kMaxDev];
     cudaError_t err;
+    int dev = 0;
+    if ((err = cudaGetDevice(&dev)) != cudaSuccess) return err;
+    if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+    int &sm_count = cache[dev].sm_count, &per_sm = cache[dev].per_sm;
+    size_t &smem_granted = cache[dev].smem_granted, &smem_occ = cache[dev].smem_occ;
     if (sm_count == 0) {
-        int dev = 0;
-        if ((err = cudaGetDevice(&dev)) != cudaSuccess) return err;
         if ((err = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return err;
     }
     if (smem > smem_granted) {

@@ -449,16 +449,18 @@ template <int Q, bool GRID, bool WEDGE = false>
 cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, double *out,
                              cudaStream_t s)
 {
-    static std::atomic<int> cap_cache{ 0 };
-    int cap = cap_cache.load(std::memory_order_acquire);
+    constexpr int kMaxDev = 64; // resident CTAs of this instantiation, queried once per device
+    static std::atomic<int> cap_cache[kMaxDev];
+    int dev = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    int cap = (dev >= 0 && dev < kMaxDev) ? cap_cache[dev].load(std::memory_order_acquire) : 0;
     if (cap <= 0) {
-        int dev = 0, sms = 0, per_sm = 0;
-        cudaError_t e;
-        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        int sms = 0, per_sm = 0;
         if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_walk_kernel<Q, GRID, WEDGE>, kWalkBlock, 0)) != cudaSuccess) return e;
         cap = sms * (per_sm < 1 ? 1 : per_sm);
-        cap_cache.store(cap, std::memory_order_release);
+        if (dev >= 0 && dev < kMaxDev) cap_cache[dev].store(cap, std::memory_order_release);
     }
     const int64_t npairs = (n + 1) >> 1;
     int64_t grid = (npairs + kWalkBlock - 1) / kWalkBlock;
