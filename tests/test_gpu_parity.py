@@ -2,6 +2,7 @@
 same seeded inputs (BASELINE.json configs[0..3]).  Inputs come from workloads/ with
 the oracle's sdf deciding the 1e-6 surface-band rejection; nothing here comes from the CUDA path."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -279,7 +280,7 @@ def _random_params(kind, rng):
 @pytest.mark.parametrize("kind", range(6), ids=[W.KIND_NAME[k] for k in range(6)])
 def test_random_parameters(vg, kind):
     rng = np.random.default_rng(9000 + kind)
-    for rep in range(12):
+    for rep in range(int(os.environ.get("VG_STRESS_REPS", "12"))):  # VG_STRESS_REPS=200 for a long soak
         params = _random_params(kind, rng)
         c, h = W.bounding_half(kind, params)
         so = O.Shape(kind, params)
