@@ -450,9 +450,29 @@ def roofline_entry(shape_kind, q, n, seconds, hbm_peak, fp64_fma_per_s):
     return e
 
 
+def launch_floor(vg, torch, per_graph=64, reps=50):
+    """Duration of one EMPTY kernel launch in a graph of back-to-back launches (vg_probe_empty_launch): the floor under
+    any single launch, whatever it computes (the latency-adjusted bound of the small-N rows)."""
+    vg.vg_probe_empty_launch(4)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        vg.vg_probe_empty_launch(per_graph)
+    g.replay()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        g.replay()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3 / (reps * per_graph)
+
+
 def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
     """Every (config, shape, query) of BASELINE.json configs[0..4], each launch timed alone on cold inputs."""
     rows = []
+    floor_s = launch_floor(vg, torch)
     plan = []
     for k in (0, 1, 2, 3):
         for i, sc in enumerate(W.shape_cases(k)):
@@ -464,6 +484,10 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
             sec = time_query_alone(torch, case, q)
             e = roofline_entry(case.kind, q, n, sec, hbm_peak, fma_rate)
             e.update({"config": k, "shape": sc.name, "query": q, "n": n, "cold_inputs": case.cold})
+            if n <= 262144:  # launch-bound sizes: the bound a single launch can reach is max(bytes / BW, empty launch)
+                ideal = max(BYTES[q] * n / (hbm_peak * 1e9), floor_s)
+                e.update({"empty_launch_us": floor_s * 1e6, "latency_adjusted_bound_us": ideal * 1e6,
+                          "latency_adjusted_frac": ideal / sec})
             rows.append(e)
         if len(sc.queries) == 5 and sc.kind != W.POLYCONE:  # the fused five-query kernel on the same tracks
             sec = time_query_alone(torch, case, "all")
