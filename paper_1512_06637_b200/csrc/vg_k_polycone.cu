@@ -13,6 +13,8 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
         if (vec && g_form.load(std::memory_order_relaxed) == 0) {
             double *o = static_cast<double *>(out);
             if (q == qDistIn) return launch_pcon_walk<qDistIn, false>(p, g, t, step_max, n, o, s);
+            if (q == qDistOut) return launch_pcon_walk<qDistOut, false>(p, g, t, step_max, n, o, s);
+            if (q == qInside) return launch_pcon_walk<qInside, false>(p, g, t, step_max, n, out, s);
             // the safeties: candidate grid (built at vg_shape_create on the device it was created on), else the walk
             if (q == qSafeIn)
                 return g.masks ? launch_pcon_walk<qSafeIn, true>(p, g, t, step_max, n, o, s)
@@ -24,8 +26,11 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
         return launch_any<Polycone, PolyconeT<solid_flags(false, kWmFull)>>(q, p, t, step_max, n, out, vec, s);
     }
     // a phi cut: the ordered walk serves DistanceToIn (every candidate also tested against the segment, the phi faces added)
-    if (vec && q == qDistIn && g_form.load(std::memory_order_relaxed) == 0)
-        return launch_pcon_walk<qDistIn, false, true>(p, g, t, step_max, n, static_cast<double *>(out), s);
+    if (vec && g_form.load(std::memory_order_relaxed) == 0) {
+        if (q == qDistIn) return launch_pcon_walk<qDistIn, false, true>(p, g, t, step_max, n, out, s);
+        if (q == qDistOut) return launch_pcon_walk<qDistOut, false, true>(p, g, t, step_max, n, out, s);
+        if (q == qInside) return launch_pcon_walk<qInside, false, true>(p, g, t, step_max, n, out, s);
+    }
     // ... and the two candidate grids (surface of revolution, phi face) the safeties
     if (vec && g.masks && g.face_masks && g_form.load(std::memory_order_relaxed) == 0) {
         if (q == qSafeIn) return launch_pcon_walk<qSafeIn, true, true>(p, g, t, step_max, n, static_cast<double *>(out), s);

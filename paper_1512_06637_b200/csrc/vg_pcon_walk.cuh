@@ -395,6 +395,116 @@ VG_DEV double pcon_grid_sdf_wedge(const PolyconeP &p, const PconWalkSec *tab, co
     return (mem && in2d) ? -D : D;
 }
 
+// Inside flags from the point's own section and its two neighbours (a tolerance band reaches at most the next section):
+// the same tests as PolyconeT::classify_pt, which loops over every section
+template <bool WEDGE>
+VG_DEV void pcon_walk_classify(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z, bool &in, bool &out)
+{
+    const double rho2 = fma(x, x, y * y);
+    const double rho = sqrt_nn(rho2);
+    const int kz = pcon_section_of(p, z);
+    bool any_in = false, any_near = false;
+#pragma unroll
+    for (int j = -1; j <= 1; ++j) {
+        const int k = kz + j;
+        if (k < 0 || k >= p.nsec) continue;
+        const PconWalkSec &w = tab[k];
+        const double ro = fma(w.Bo, z, w.Ao), ri = fma(w.Bi, z, w.Ai);
+        const double to = kTol * w.seco, ti = kTol * w.seci;
+        const bool zin = z >= w.z0 && z <= w.z1;
+        const bool znear = z >= w.z0 - kTol && z <= w.z1 + kTol;
+        const bool inner = (p.inner_mask >> k) & 1u;
+        any_in = any_in || (zin && rho < ro - to && (!inner || rho > ri + ti));
+        any_near = any_near || (znear && rho <= ro + to && (!inner || rho >= ri - ti));
+    }
+    in = any_in && z > p.zlo + kTol && z < p.zhi - kTol;
+    out = !any_near;
+    if (p.step_mask) in = in && !pcon_near_step(p, kz, rho2, z) && !pcon_near_step(p, kz - 1, rho2, z);
+    if (WEDGE) wedge_classify<kWmRuntime>(p.w, wedge_eval(p.w, x, y), rho2, in, out);
+}
+
+// leaving crossing of the faces of step k, +inf if none (PolyconeT::cross with leaving = true)
+VG_DEV double pcon_step_leave(const PolyconeP &p, int k, const RayRZ &r, double z, double dz, double idz)
+{
+    if (k < 0 || k + 1 >= p.nsec || !((p.step_mask >> k) & 1u)) return inf();
+    const PconStep &st = p.step[k];
+    const double t = (st.z - z) * idz;
+    const double rh2 = fma(t, fma(t, r.a_xy, r.b_xy + r.b_xy), r.rho2);
+    const bool up = dz > 0.0;
+    const bool on_o = rh2 >= st.olo * st.olo && rh2 <= st.ohi * st.ohi && st.ohi > st.olo && (st.oup != 0) == up;
+    const bool on_i = rh2 >= st.ilo * st.ilo && rh2 <= st.ihi * st.ihi && st.ihi > st.ilo && (st.iup != 0) == up;
+    return (t > 0.0 && (on_o || on_i)) ? t : inf();
+}
+
+// DistanceToOut: from the point's own section the ray stays in the material until it leaves through a patch of the
+// section it is in (outer: leaving root, inner: entering root), through a step face on the plane it crosses next, or
+// through an end cap; sections are visited in the order the ray meets them.  Same candidates and tests as
+// PolyconeT::dist_out, which evaluates every section.
+template <bool WEDGE>
+VG_DEV double pcon_walk_dist_out(const PolyconeP &p, const PconWalkSec *tab, double x, double y, double z, double dx,
+                                 double dy, double dz)
+{
+    bool in, out;
+    pcon_walk_classify<WEDGE>(p, tab, x, y, z, in, out);
+    RayRZ r;
+    r.rho2 = fma(x, x, y * y);
+    r.a_xy = fma(dx, dx, dy * dy);
+    r.b_xy = fma(x, dx, y * dy);
+    WedgeEval ep = {}, ed = {};
+    if (WEDGE) ep = wedge_eval(p.w, x, y), ed = wedge_eval(p.w, dx, dy);
+    const double idz = rcp(dz); // NaN for dz = 0: a horizontal ray never reaches a plane and ends in its own section
+    const bool up = not_neg(dz);
+    const int step = up ? 1 : -1;
+    int k = pcon_section_of(p, z);
+    double best = inf();
+    bool go = !out;
+    while (go) {
+        const PconWalkSec w = tab[k];
+        Frustum f;
+        bool ok;
+        f.A = w.Ao, f.B = w.Bo;
+        double t = frustum_root(f, r, z, dz, true, ok);
+        double zh = fma(t, dz, z);
+        ok = ok && zh >= w.z0 && zh <= w.z1;
+        if (WEDGE) ok = ok && wedge_member_at<kWmRuntime>(p.w, ep, ed, t);
+        best = (ok && t < best) ? t : best;
+        f.A = w.Ai, f.B = w.Bi;
+        t = frustum_root(f, r, z, dz, false, ok);
+        zh = fma(t, dz, z);
+        ok = ok && ((p.inner_mask >> k) & 1u) && zh >= w.z0 && zh <= w.z1;
+        if (WEDGE) ok = ok && wedge_member_at<kWmRuntime>(p.w, ep, ed, t);
+        best = (ok && t < best) ? t : best;
+        if (best < inf() || !(fabs(dz) >= kTiny)) break;
+        const int kn = k + step;
+        if (kn < 0 || kn >= p.nsec) { // the end cap
+            const double tc = ((up ? p.zhi : p.zlo) - z) * idz;
+            const bool okc = tc > 0.0 && (!WEDGE || wedge_member_at<kWmRuntime>(p.w, ep, ed, tc));
+            best = okc ? tc : best;
+            break;
+        }
+        if (p.step_mask) {
+            const double ts = pcon_step_leave(p, up ? k : kn, r, z, dz, idz);
+            const bool oks = ts < inf() && (!WEDGE || wedge_member_at<kWmRuntime>(p.w, ep, ed, ts));
+            best = oks ? ts : best;
+            if (oks) break;
+        }
+        k = kn;
+    }
+    if (WEDGE && !out) { // the phi faces in the leaving sense
+        {
+            const double t = -ep.c0 * rcp(ed.c0);
+            const bool ok = ed.c0 < 0.0 && t > 0.0 && t < best && pcon_in_outline(p, tab, fma(t, ed.u0, ep.u0), fma(t, dz, z));
+            best = ok ? t : best;
+        }
+        {
+            const double t = -ep.c1 * rcp(ed.c1);
+            const bool ok = ed.c1 < 0.0 && t > 0.0 && t < best && pcon_in_outline(p, tab, fma(t, ed.u1, ep.u1), fma(t, dz, z));
+            best = ok ? t : best;
+        }
+    }
+    return out ? -1.0 : best;
+}
+
 template <int Q, bool GRID, bool WEDGE>
 VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x,
                              double y, double z, double dx, double dy, double dz, double step_max)
@@ -404,7 +514,8 @@ VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const d
                                : (GRID ? pcon_grid_sdf(p, tab, seg, g, x, y, z) : pcon_walk_sdf(p, tab, x, y, z));
         return Q == qSafeIn ? s : -s;
     }
-    const double t = pcon_walk_dist_in<WEDGE>(p, tab, x, y, z, dx, dy, dz);
+    const double t = Q == qDistOut ? pcon_walk_dist_out<WEDGE>(p, tab, x, y, z, dx, dy, dz)
+                                   : pcon_walk_dist_in<WEDGE>(p, tab, x, y, z, dx, dy, dz);
     return t <= step_max ? t : inf();
 }
 
@@ -416,9 +527,11 @@ VG_DEV double pcon_walk_eval(const PolyconeP &p, const PconWalkSec *tab, const d
 template <int Q, bool GRID, bool WEDGE>
 __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
     pcon_walk_kernel(const __grid_constant__ PolyconeP p, const __grid_constant__ PconGrid g, Tracks t, double step_max,
-                     int64_t n, double *out)
+                     int64_t n, void *out_any)
 {
-    constexpr bool kDir = (Q == qDistIn);
+    constexpr bool kDir = (Q == qDistIn || Q == qDistOut);
+    double *out = static_cast<double *>(out_any);
+    int32_t *outi = static_cast<int32_t *>(out_any);
     __shared__ __align__(16) PconWalkSec tab[kMaxSec];
     __shared__ __align__(16) double seg[GRID ? 64 * kPconSegStride : 2];
     pcon_stage(p, tab);
@@ -433,6 +546,13 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
             double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
             double2 dx = make_double2(0, 0), dy = dx, dz = dx;
             if (kDir) dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
+            if (Q == qInside) {
+                bool in0, out0, in1, out1;
+                pcon_walk_classify<WEDGE>(p, tab, x.x, y.x, z.x, in0, out0);
+                pcon_walk_classify<WEDGE>(p, tab, x.y, y.y, z.y, in1, out1);
+                stg2i(outi + i, classify(in0, out0), classify(in1, out1));
+                continue;
+            }
             const double r0 = pcon_walk_eval<Q, GRID, WEDGE>(p, tab, seg, g, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max);
             const double r1 = pcon_walk_eval<Q, GRID, WEDGE>(p, tab, seg, g, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max);
             stg2(out + i, r0, r1);
@@ -440,13 +560,19 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
             double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
             double dx = 0, dy = 0, dz = 0;
             if (kDir) dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+            if (Q == qInside) {
+                bool in0, out0;
+                pcon_walk_classify<WEDGE>(p, tab, x, y, z, in0, out0);
+                stg1i(outi + i, classify(in0, out0));
+                continue;
+            }
             stg1(out + i, pcon_walk_eval<Q, GRID, WEDGE>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max));
         }
     }
 }
 
 template <int Q, bool GRID, bool WEDGE = false>
-cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, double *out,
+cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, void *out,
                              cudaStream_t s)
 {
     constexpr int kMaxDev = 64; // resident CTAs of this instantiation, queried once per device
