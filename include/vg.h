@@ -136,7 +136,7 @@ int vg_safety_to_out(const vg_shape *shape, const double *x, const double *y, co
  * vg_query_all -- the five answers of n tracks in one call (a basket of particles in one volume asks all three
  * questions of PAPER.md:110-114 every step).  Same results, element by element, as the five
  * calls above.  Any output pointer may be NULL (that answer is skipped; at least one must be given).  When all five
- * are given and the solid is neither a polycone nor a boolean, ONE fused kernel reads the six track arrays once (48 B per track
+ * are given and the solid is not a boolean (for a polycone: and every array is 16-byte aligned), ONE fused kernel reads the six track arrays once (48 B per track
  * instead of 168 B) and writes the five results; otherwise the call enqueues one kernel per requested answer.
  * cls: DEVICE int32[n]; the other four: DEVICE double[n]; dx, dy, dz and step_max as for vg_distance_to_in.
  */

@@ -249,6 +249,25 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
     const char *fn = "vg_query_all";
     if (!s) return fail(VG_ERR_ARG, "%s: shape is NULL", fn);
     const bool all = cls && dist_in && dist_out && safety_in && safety_out;
+    if (all && s->kind == VG_POLYCONE && n > 0 && step_max >= 0) { // the polycone's fused kernel, when its conditions hold
+        const void *ptrs6[6] = { x, y, z, dx, dy, dz };
+        bool vec = false, v2 = false;
+        int rcp = check_arrays(fn, ptrs6, 6, 4, cls, n, &vec);
+        double *outs4[4] = { dist_in, dist_out, safety_in, safety_out };
+        for (int i = 0; i < 4 && rcp == VG_OK; ++i) {
+            rcp = check_arrays(fn, ptrs6, 6, 8, outs4[i], n, &v2);
+            vec = vec && v2;
+        }
+        if (rcp != VG_OK) return rcp;
+        PconGrid g = s->grid;
+        int dev = -1;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr;
+        Tracks t{ x, y, z, dx, dy, dz };
+        AllOut o{ cls, dist_in, dist_out, safety_in, safety_out };
+        cudaError_t e = launch_polycone_all(s->u.pcon, g, t, step_max, n, o, vec, static_cast<cudaStream_t>(stream));
+        if (e == cudaSuccess) return VG_OK;
+        if (e != cudaErrorNotSupported) return fail_cuda(e, fn);
+    }
     if (!all || s->kind >= VG_POLYCONE) { // a subset, or no fused kernel for this solid: one launch per requested answer
         if (!cls && !dist_in && !dist_out && !safety_in && !safety_out) return fail(VG_ERR_ARG, "%s: every output is NULL", fn);
         int rc = VG_OK;

@@ -39,4 +39,17 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
     return launch_any<Polycone>(q, p, t, step_max, n, out, vec, s);
 }
 
+// the fused five-query kernel of a polycone: needs 16-byte aligned arrays and, for the safeties of a polycone with a phi
+// cut, its candidate grids; cudaErrorNotSupported tells the caller to run the five queries as separate launches
+cudaError_t launch_polycone_all(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, const AllOut &o,
+                                bool vec, cudaStream_t s)
+{
+    if (n <= 0) return cudaSuccess;
+    if (!vec || g_form.load(std::memory_order_relaxed) != 0) return cudaErrorNotSupported;
+    if (p.w.full)
+        return g.masks ? launch_pcon_all<true, false>(p, g, t, step_max, n, o, s) : launch_pcon_all<false, false>(p, g, t, step_max, n, o, s);
+    if (g.masks && g.face_masks) return launch_pcon_all<true, true>(p, g, t, step_max, n, o, s);
+    return cudaErrorNotSupported;
+}
+
 } // namespace vg

@@ -570,6 +570,9 @@ cudaError_t launch_tube_all(const TubeP &p, const Tracks &t, double step_max, in
 cudaError_t launch_cone_all(const ConeP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
 cudaError_t launch_trd_all(const TrdP &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec, cudaStream_t s);
 
+cudaError_t launch_polycone_all(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, const AllOut &o,
+                                bool vec, cudaStream_t s); // cudaErrorNotSupported: run the five queries separately
+
 // navigation (vg_nav.cu)
 cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                 double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s);

@@ -571,6 +571,76 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
     }
 }
 
+// ---- the fused five-query call for a polycone (vg_query_all): one pass over the six coordinates ----
+template <bool GRID, bool WEDGE>
+VG_DEV void pcon_all_eval(const PolyconeP &p, const PconWalkSec *tab, const double *seg, const PconGrid &g, double x, double y,
+                          double z, double dx, double dy, double dz, double step_max, int &cls, double &din, double &dout,
+                          double &sdf)
+{
+    bool in, out;
+    pcon_walk_classify<WEDGE>(p, tab, x, y, z, in, out);
+    cls = classify(in, out);
+    sdf = pcon_walk_eval<qSafeIn, GRID, WEDGE>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max);
+    din = pcon_walk_eval<qDistIn, GRID, WEDGE>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max);
+    dout = pcon_walk_eval<qDistOut, GRID, WEDGE>(p, tab, seg, g, x, y, z, dx, dy, dz, step_max);
+}
+
+template <bool GRID, bool WEDGE>
+__global__ void __launch_bounds__(kWalkBlock, 2)
+    pcon_all_kernel(const __grid_constant__ PolyconeP p, const __grid_constant__ PconGrid g, Tracks t, double step_max, int64_t n,
+                    AllOut o)
+{
+    __shared__ __align__(16) PconWalkSec tab[kMaxSec];
+    __shared__ __align__(16) double seg[GRID ? 64 * kPconSegStride : 2];
+    pcon_stage(p, tab);
+    if (GRID) pcon_stage_segs(p, seg);
+    pdl_launch_dependents();
+    __syncthreads();
+    pdl_wait();
+    const int64_t npairs = (n + 1) >> 1;
+    for (int64_t j = int64_t(blockIdx.x) * kWalkBlock + threadIdx.x; j < npairs; j += int64_t(gridDim.x) * kWalkBlock) {
+        const int64_t i = 2 * j;
+        if (i + 1 < n) {
+            const double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
+            const double2 dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
+            int c0, c1;
+            double a0, a1, b0, b1, s0, s1;
+            pcon_all_eval<GRID, WEDGE>(p, tab, seg, g, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max, c0, a0, b0, s0);
+            pcon_all_eval<GRID, WEDGE>(p, tab, seg, g, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max, c1, a1, b1, s1);
+            stg2i(o.cls + i, c0, c1);
+            stg2(o.din + i, a0, a1);
+            stg2(o.dout + i, b0, b1);
+            stg2(o.sin + i, s0, s1);
+            stg2(o.sout + i, -s0, -s1);
+        } else {
+            int c0;
+            double a0, b0, s0;
+            pcon_all_eval<GRID, WEDGE>(p, tab, seg, g, ldg1(t.x + i), ldg1(t.y + i), ldg1(t.z + i), ldg1(t.dx + i), ldg1(t.dy + i),
+                                       ldg1(t.dz + i), step_max, c0, a0, b0, s0);
+            stg1i(o.cls + i, c0);
+            stg1(o.din + i, a0);
+            stg1(o.dout + i, b0);
+            stg1(o.sin + i, s0);
+            stg1(o.sout + i, -s0);
+        }
+    }
+}
+
+template <bool GRID, bool WEDGE>
+cudaError_t launch_pcon_all(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, const AllOut &o,
+                            cudaStream_t s)
+{
+    int dev = 0, sms = 0, per_sm = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pcon_all_kernel<GRID, WEDGE>, kWalkBlock, 0)) != cudaSuccess) return e;
+    const int64_t cap = int64_t(sms) * (per_sm < 1 ? 1 : per_sm), npairs = (n + 1) >> 1;
+    int64_t grid = (npairs + kWalkBlock - 1) / kWalkBlock;
+    if (grid > cap) grid = cap;
+    return launch_kernel(pcon_all_kernel<GRID, WEDGE>, unsigned(grid), kWalkBlock, 0, s, p, g, t, step_max, n, o);
+}
+
 template <int Q, bool GRID, bool WEDGE = false>
 cudaError_t launch_pcon_walk(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, void *out,
                              cudaStream_t s)
