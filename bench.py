@@ -248,9 +248,11 @@ def capture_steps(torch, case, with_events):
     return graphs, events
 
 
-def time_query_alone(torch, case, q, min_ms=30.0):
+def time_query_alone(torch, case, q, min_ms=30.0, hot=False):
     """Average duration of one launch of `q` (cold inputs): a graph of nsets launches over the rotating sets,
-    replayed between two CUDA events on the launching stream until >= min_ms have been timed."""
+    replayed between two CUDA events on the launching stream until >= min_ms have been timed.  hot = True: every
+    launch reads the SAME buffer set (what the paper's 5000 repetitions on fixed particles did): the
+    batch stays in the 126 MB L2 if it fits."""
     case.cursor = 0
     case.launch(q)
     torch.cuda.synchronize()
@@ -258,6 +260,8 @@ def time_query_alone(torch, case, q, min_ms=30.0):
     g = torch.cuda.CUDAGraph()
     with torch.cuda.graph(g):
         for _ in range(case.nsets):
+            if hot:
+                case.cursor = 0
             case.launch(q)
     for _ in range(3):
         g.replay()
@@ -654,6 +658,10 @@ def run_ours(args, rank, world, local_rank):
     per_q = {q: time_query_alone(torch, case, q) for q in case.queries}
 
     per_query = {q: roofline_entry(case.kind, q, case.n, per_q[q], hbm_peak, fma_rate) for q in case.queries}
+    for q in case.queries:  # the hot variant: same buffers every launch, the 48 MB batch stays in L2
+        hot_s = time_query_alone(torch, case, q, hot=True)
+        per_query[q]["hot_us_per_launch"] = hot_s * 1e6
+        per_query[q]["hot_tracks_per_s"] = case.n / hot_s
     dom = max(case.queries, key=lambda q: per_q[q])
     kname = ("query_stream_kernel<TubeT<hollow, wide phi>, %s>" if dom == "distance_to_in" else "query_kernel<TubeT<hollow, wide phi>, %s>") % dom
     roof = {"bound": "hbm", "kernel": kname, "achieved": per_query[dom]["hbm_gbs"],
