@@ -224,7 +224,9 @@ int vg_world_safety(const vg_world *world, const int32_t *node, const double *x,
  * pinned; pinned memory makes the copies asynchronous).  The library cuts the arrays into chunks and pipelines
  * host->device copy, the same kernels, device->host copy over several internal streams and per-device staging
  * memory allocated once on first use.  The call returns when the outputs are complete (it synchronises its own
- * streams only).  Calls on one device are serialised by a lock.
+ * streams only).  Calls on one device are serialised by a lock.  Equally spaced arrays (rows of one allocation) cross
+ * the link as one strided copy per chunk; calls of up to 2^14 tracks whose arrays are all pinned run without copies
+ * (the kernel addresses the pinned host memory directly).
  *
  * vg_query_host: `query` is a vg_query; out is int32[n] for VG_Q_INSIDE, double[n] otherwise; dx, dy, dz are
  * read only by the two distance queries (may be NULL otherwise), step_max likewise. */

@@ -18,6 +18,7 @@ constexpr int64_t kMaxChunk = int64_t(1) << 20; // tracks per chunk: 8 MiB per c
 constexpr int64_t kMinChunk = int64_t(1) << 16;
 constexpr int64_t kBigChunk = int64_t(1) << 19; // the automatic choice stays at or below this
 constexpr int kMaxDev = 16;
+constexpr int64_t kZeroCopyMax = int64_t(1) << 14; // tracks: up to here a call on pinned memory runs without copies
 
 struct HostPipe {
     bool ready = false;
@@ -115,6 +116,43 @@ static int run_host(const char *fn, const vg_shape *shape, const vg_volume *volu
     if (e != cudaSuccess) return cuda_fail(e, fn);
     std::lock_guard<std::mutex> lock(p->mu);
     if ((e = pipe_init(*p)) != cudaSuccess) return cuda_fail(e, fn);
+    // Small calls on pinned memory skip the copies altogether: pinned host memory is addressable from the device (unified
+    // addressing), so the kernel reads the tracks and writes the results straight over the link.  One launch and one
+    // synchronisation instead of copy + launch + copy; worth it while the transfer is latency, not bandwidth.
+    if (n <= kZeroCopyMax) {
+        bool pinned = true;
+        const void *ptrs[12] = { h[0], h[1], h[2], dir ? h[3] : nullptr, dir ? h[4] : nullptr, dir ? h[5] : nullptr, out, hit,
+                                 all ? all[0] : nullptr, all ? all[1] : nullptr, all ? all[2] : nullptr, all ? all[3] : nullptr };
+        const void *last = all ? all[4] : nullptr;
+        for (int a = 0; a < 13 && pinned; ++a) {
+            const void *q = a < 12 ? ptrs[a] : last;
+            if (!q) continue;
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, q) != cudaSuccess) {
+                cudaGetLastError();
+                pinned = false;
+            } else {
+                pinned = at.type == cudaMemoryTypeHost && at.devicePointer == q;
+            }
+        }
+        if (pinned) {
+            cudaStream_t st = p->st[0];
+            int rc0;
+            if (volume) rc0 = vg_compute_step(volume, h[0], h[1], h[2], h[3], h[4], h[5], step_max, n, static_cast<double *>(out), hit, st);
+            else if (q == qAll)
+                rc0 = vg_query_all(shape, h[0], h[1], h[2], h[3], h[4], h[5], step_max, n, static_cast<int32_t *>(all[0]),
+                                   static_cast<double *>(all[1]), static_cast<double *>(all[2]), static_cast<double *>(all[3]),
+                                   static_cast<double *>(all[4]), st);
+            else if (q == qInside) rc0 = vg_inside(shape, h[0], h[1], h[2], n, static_cast<int32_t *>(out), st);
+            else if (q == qDistIn) rc0 = vg_distance_to_in(shape, h[0], h[1], h[2], h[3], h[4], h[5], step_max, n, static_cast<double *>(out), st);
+            else if (q == qDistOut) rc0 = vg_distance_to_out(shape, h[0], h[1], h[2], h[3], h[4], h[5], step_max, n, static_cast<double *>(out), st);
+            else if (q == qSafeIn) rc0 = vg_safety_to_in(shape, h[0], h[1], h[2], n, static_cast<double *>(out), st);
+            else rc0 = vg_safety_to_out(shape, h[0], h[1], h[2], n, static_cast<double *>(out), st);
+            if (rc0 != VG_OK) return rc0;
+            e = cudaStreamSynchronize(st);
+            return e == cudaSuccess ? VG_OK : cuda_fail(e, fn);
+        }
+    }
     int64_t chunk = pick_chunk(n);
     // Host arrays that sit at one constant distance from each other (rows of one allocation) travel as one 2-D copy per
     // chunk: every copy costs a few microseconds of set-up, which is most of the time of a small call.
