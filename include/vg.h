@@ -11,9 +11,11 @@
  * competes with the physics step; "coordinate transformations and distance calculations")
  *                                                                                      -> vg_compute_step.
  * The paper defines no solid and no formula; the exact meaning of every query is the reading
- * R1-R21 of SURVEY.md sec. 8(c), restated in DESIGN.md sec. 3.  In one line each:
+ * R1-R21 of SURVEY.md sec. 8(c), restated in DESIGN.md sec. 3 together with R22-R31 (the tree of volumes
+ * vg_world_*, polycone z steps, boolean solids and CSG trees vg_boolean_create).  In one line each:
  *   Inside        VG_INSIDE if sdf(p) < -kTol, VG_OUTSIDE if sdf(p) > +kTol, else VG_SURFACE (kTol = 1e-9)
- *   SafetyToIn    +sdf(p), SafetyToOut  -sdf(p): exact signed Euclidean distance to the surface
+ *   SafetyToIn    +sdf(p), SafetyToOut  -sdf(p): exact signed Euclidean distance to the surface (for a
+ *                 boolean: the composed bound of R29, which never over-estimates it)
  *   DistanceToIn  -1 if p is inside; else the first t > 0 with p + t d on the surface; +inf if none or > step_max
  *   DistanceToOut -1 if p is outside; else likewise
  *   ComputeStep   lexicographic min of (distance, index) over the mother's DistanceToOut (index -1) and every
