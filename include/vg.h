@@ -280,6 +280,13 @@ const char *vg_last_error(void);
 int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *stream);
 /* Enqueues `launches` empty kernels (launch-latency floor for the small-N end of configs[3]). */
 int vg_probe_empty_launch(int launches, void *stream);
+/* Host-only: the candidate grids vg_shape_create builds for the safeties of a polycone, recomputed
+ * into caller memory so that the host logic can be checked without a device.  masks: HOST uint64[rows * cols] of the
+ * surface grid; face_masks: HOST uint64[rows * 2 cols] of the phi-face grid (may be NULL); row_section: HOST
+ * uint8[rows]; geom: HOST double[3] = {1 / cell width in rho, 1 / cell height in z, z of the grid's lower edge};
+ * dims: HOST int[2] = {rows, cols}.  Any output pointer may be NULL.  VG_ERR_ARG if the shape is not a polycone. */
+int vg_debug_polycone_grid(const vg_shape *shape, uint64_t *masks, uint64_t *face_masks, unsigned char *row_section,
+                           double *geom, int *dims);
 /* Number of kernel launches the library has made in this process (all threads). */
 int64_t vg_launch_count(void);
 

@@ -833,6 +833,25 @@ extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const dou
     return VG_OK;
 }
 
+extern "C" int vg_debug_polycone_grid(const vg_shape *s, uint64_t *masks, uint64_t *face_masks, unsigned char *row_section,
+                                      double *geom, int *dims)
+{
+    if (!s || s->kind != VG_POLYCONE) return fail(VG_ERR_ARG, "vg_debug_polycone_grid: not a polycone");
+    std::vector<unsigned long long> m;
+    std::vector<unsigned char> rows;
+    PconGridGeom g;
+    pcon_grid_build(s->u.pcon, false, &g, &m, &rows);
+    if (masks) std::memcpy(masks, m.data(), m.size() * sizeof(unsigned long long));
+    if (row_section) std::memcpy(row_section, rows.data(), rows.size());
+    if (geom) geom[0] = g.inv_cr, geom[1] = g.inv_cz, geom[2] = g.zg0;
+    if (dims) dims[0] = kPconGridZ, dims[1] = kPconGridR;
+    if (face_masks) {
+        pcon_grid_build(s->u.pcon, true, &g, &m, &rows);
+        std::memcpy(face_masks, m.data(), m.size() * sizeof(unsigned long long));
+    }
+    return VG_OK;
+}
+
 // -------------------------------------------------------------------------------------------------- probes
 
 extern "C" int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *stream)

@@ -7,6 +7,7 @@ import os
 import re
 import socket
 
+import numpy as np
 import pytest
 import torch
 import torch.distributed as dist
@@ -211,3 +212,86 @@ def test_two_ranks_shard_without_exchange_and_reduce_the_timing():
     assert got[0][1] == 0 and got[0][2] == got[1][1] and got[1][2] == n
     assert np.array_equal(np.concatenate([got[0][3], got[1][3]]), whole)
     assert all(r[4] == 1.5 for r in got) and all(r[5] == n for r in got)
+
+
+# ------------------------------------------------------- host logic: the candidate grids of the polycone safeties
+
+def _polycone_segments(par, face):
+    """(r0, z0, r1, z1, bit) of every edge of the (r, z) outline with the bit it has in the masks (vg_params.h): caps 0 / 1,
+    outer / inner edge of section k at 2 + 2k / 3 + 2k, the faces of the j-th z step after the sections.  `face`: the
+    phi-face grid holds every edge; the surface grid leaves out edges on the axis (both radii 0)."""
+    nz = int(par[2])
+    pl = [(par[3 + 3 * i], par[4 + 3 * i], par[5 + 3 * i]) for i in range(nz)]
+    secs, steps = [], []
+    for a, b in zip(pl, pl[1:]):
+        if b[0] == a[0]:
+            steps.append((len(secs) - 1, a, b))
+        else:
+            secs.append((a, b))
+    segs = []
+    for k, (a, b) in enumerate(secs):
+        segs.append((a[2], a[0], b[2], b[0], 2 + 2 * k))
+        if face or a[1] > 0 or b[1] > 0:
+            segs.append((a[1], a[0], b[1], b[0], 3 + 2 * k))
+    for j, (_, a, b) in enumerate(steps):
+        base = 2 + 2 * len(secs) + 2 * j
+        if a[2] != b[2]:
+            segs.append((min(a[2], b[2]), a[0], max(a[2], b[2]), a[0], base))
+        if a[1] != b[1]:
+            segs.append((min(a[1], b[1]), a[0], max(a[1], b[1]), a[0], base + 1))
+    segs.append((pl[0][1], pl[0][0], pl[0][2], pl[0][0], 0))
+    segs.append((pl[-1][1], pl[-1][0], pl[-1][2], pl[-1][0], 1))
+    return segs, secs
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+def test_polycone_candidate_grid_holds_the_nearest_edge_of_every_point(seed):
+    """vg_pcon_grid.h builds, per cell of a (rho, z) grid, the set of outline edges that can be nearest to a point of the
+    cell.  Checked here on the host (no device): for random points the edge that IS nearest (distances written out in
+    numpy) has its bit in the mask of the point's cell, for the surface grid and for the phi-face grid; the per-row section
+    index never exceeds the section of any point of the row."""
+    import paper_1512_06637_b200 as vg
+    rng = np.random.default_rng(seed)
+    nz = int(rng.integers(3, 20))
+    z = np.sort(rng.uniform(-50, 50, nz)) + np.arange(nz) * 1e-3
+    par = [0.3, float(rng.choice([7.0, 4.0])), float(nz)]
+    for i in range(nz):
+        a = float(rng.choice([0.0, rng.uniform(0, 5)]))
+        par += [float(z[i]), a, a + float(rng.uniform(5, 25))]
+    if seed % 2 == 0:  # add a z step
+        i = nz // 2
+        zi, a, b = par[3 + 3 * i: 6 + 3 * i]
+        par[6 + 3 * i: 6 + 3 * i] = [zi, 0.0, 0.5 * (a + b) + 6.0]
+        par[2] += 1.0
+    s = vg.Shape(vg.POLYCONE, par)
+    dims = (C.c_int * 2)()
+    geom = (C.c_double * 3)()
+    vg._lib.vg_debug_polycone_grid.argtypes = [C.c_void_p] * 6
+    assert vg._lib.vg_debug_polycone_grid(s._h, None, None, None, geom, dims) == vg.OK
+    rows, cols = dims[0], dims[1]
+    masks = np.zeros(rows * cols, dtype=np.uint64)
+    fmasks = np.zeros(rows * 2 * cols, dtype=np.uint64)
+    rowsec = np.zeros(rows, dtype=np.uint8)
+    assert vg._lib.vg_debug_polycone_grid(s._h, masks.ctypes.data, fmasks.ctypes.data, rowsec.ctypes.data, geom, dims) == vg.OK
+    inv_cr, inv_cz, zg0 = geom[0], geom[1], geom[2]
+    R = cols / inv_cr
+    for face, m, ncol, ulo in ((False, masks, cols, 0.0), (True, fmasks, 2 * cols, -R)):
+        segs, secs = _polycone_segments(par, face)
+        n = 200000
+        u = rng.uniform(ulo, R, n)
+        v = rng.uniform(zg0, zg0 + rows / inv_cz, n)
+        d2 = np.full((len(segs), n), np.inf)
+        for j, (r0, z0, r1, z1, _) in enumerate(segs):
+            eu, ev = r1 - r0, z1 - z0
+            t = np.clip(((u - r0) * eu + (v - z0) * ev) / (eu * eu + ev * ev), 0, 1)
+            d2[j] = (u - r0 - t * eu) ** 2 + (v - z0 - t * ev) ** 2
+        nearest = np.argmin(d2, axis=0)
+        bits = np.array([sg[4] for sg in segs], dtype=np.uint64)[nearest]
+        cell = np.minimum((v - zg0) * inv_cz, rows - 1).astype(int) * ncol + np.minimum((u - ulo) * inv_cr, ncol - 1).astype(int)
+        assert np.all((m[cell] >> bits) & np.uint64(1) == 1), "a nearest edge is missing from its cell's mask (face=%s)" % face
+        pop = np.array([bin(int(w)).count("1") for w in m])
+        assert pop.min() >= 1 and pop.mean() < 0.5 * len(segs)  # every cell has a candidate; the masks do prune
+    planes = np.array([sc[0][0] for sc in secs[1:]])
+    zrow = zg0 + np.arange(rows) / inv_cz
+    assert np.all(rowsec <= np.array([(planes <= zz).sum() for zz in zrow]))
+    assert np.all(rowsec >= np.array([(planes <= zz - 1e-3).sum() for zz in zrow]))
