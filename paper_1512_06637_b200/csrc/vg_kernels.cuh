@@ -94,6 +94,19 @@ template <int F> struct Tune<TubeT<F>, qSafeOut> {
     static constexpr bool stream = false;
     static constexpr int block = VG_TUBE_SAFE_BLOCK;
 };
+#ifndef VG_CONE_SAFE_BLOCK
+#define VG_CONE_SAFE_BLOCK 128
+#endif
+template <int F> struct Tune<ConeT<F>, qSafeIn> {
+    static constexpr int minb = VG_MINB;
+    static constexpr bool stream = false;
+    static constexpr int block = VG_CONE_SAFE_BLOCK;
+};
+template <int F> struct Tune<ConeT<F>, qSafeOut> {
+    static constexpr int minb = VG_MINB;
+    static constexpr bool stream = false;
+    static constexpr int block = VG_CONE_SAFE_BLOCK;
+};
 template <> struct Tune<Trd, qSafeIn> {
     static constexpr int minb = VG_MINB;
     static constexpr bool stream = true;
