@@ -583,10 +583,11 @@ struct Trd {
     {
         double ax = fabs(x), ay = fabs(y), gx, gy;
         double g = gmax(p, ax, ay, z, gx, gy);
-        // the two z faces: rectangles
-        double zx1 = dmax(ax - p.dx1, 0.0), zy1 = dmax(ay - p.dy1, 0.0), zz1 = z + p.dz;
-        double zx2 = dmax(ax - p.dx2, 0.0), zy2 = dmax(ay - p.dy2, 0.0), zz2 = z - p.dz;
-        double D2 = dmin(fma(zx1, zx1, fma(zy1, zy1, zz1 * zz1)), fma(zx2, zx2, fma(zy2, zy2, zz2 * zz2)));
+        // the z face on the point's side of the mid-plane (a rectangle).  The other one cannot hold the nearest point in its
+        // interior (that needs the point beyond it), and its edges belong to the slanted faces below as well.
+        const bool top = not_neg(z);
+        double zx = dmax(ax - (top ? p.dx2 : p.dx1), 0.0), zy = dmax(ay - (top ? p.dy2 : p.dy1), 0.0), zz = fabs(z) - p.dz;
+        double D2 = fma(zx, zx, fma(zy, zy, zz * zz));
         // +x face: foot of the perpendicular, in-plane coordinates (|y|, slant coordinate)
         {
             double zf = fma(gx * p.icx, p.fx, z);
