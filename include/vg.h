@@ -287,6 +287,12 @@ int vg_probe_empty_launch(int launches, void *stream);
  * dims: HOST int[2] = {rows, cols}.  Any output pointer may be NULL.  VG_ERR_ARG if the shape is not a polycone. */
 int vg_debug_polycone_grid(const vg_shape *shape, uint64_t *masks, uint64_t *face_masks, unsigned char *row_section,
                            double *geom, int *dims);
+/* Host-only: a boolean as vg_boolean_create flattened it: the kinds of its primitives in tree order
+ * (kinds: HOST int[8]), the 3x4 transforms from the frame of the boolean to the frame of each primitive (xforms: HOST
+ * double[8 * 12]) and the postfix program (prog: HOST uint8[16]; a token < 0x80 pushes that primitive, 0x80 | op combines
+ * the two on top).  Returns the number of primitives (2 for a boolean of two primitives), *nprog receives the program
+ * length; VG_ERR_ARG if the shape is not a boolean.  Any output pointer may be NULL. */
+int vg_debug_boolean_program(const vg_shape *shape, int *kinds, double *xforms, unsigned char *prog, int *nprog);
 /* Number of kernel launches the library has made in this process (all threads). */
 int64_t vg_launch_count(void);
 

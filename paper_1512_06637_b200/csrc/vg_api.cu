@@ -833,6 +833,21 @@ extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const dou
     return VG_OK;
 }
 
+extern "C" int vg_debug_boolean_program(const vg_shape *s, int *kinds, double *xforms, unsigned char *prog, int *nprog)
+{
+    if (!s || (s->kind != VG_BOOLEAN && s->kind != kCsg)) return fail(VG_ERR_ARG, "vg_debug_boolean_program: not a boolean");
+    CsgOperand o;
+    int rc = csg_operand(s, &o);
+    if (rc != VG_OK) return rc;
+    for (int i = 0; i < o.nleaf; ++i) {
+        if (kinds) kinds[i] = o.leaf[i].kind;
+        if (xforms) std::memcpy(xforms + 12 * i, o.X[i], 12 * sizeof(double));
+    }
+    if (prog) std::memcpy(prog, o.prog, size_t(o.nprog));
+    if (nprog) *nprog = o.nprog;
+    return o.nleaf;
+}
+
 extern "C" int vg_debug_polycone_grid(const vg_shape *s, uint64_t *masks, uint64_t *face_masks, unsigned char *row_section,
                                       double *geom, int *dims)
 {

@@ -295,3 +295,53 @@ def test_polycone_candidate_grid_holds_the_nearest_edge_of_every_point(seed):
     zrow = zg0 + np.arange(rows) / inv_cz
     assert np.all(rowsec <= np.array([(planes <= zz).sum() for zz in zrow]))
     assert np.all(rowsec >= np.array([(planes <= zz - 1e-3).sum() for zz in zrow]))
+
+
+# ------------------------------------------------------------------- host logic: flattening of a CSG tree
+
+def test_boolean_trees_are_flattened_in_tree_order_with_composed_transforms():
+    """vg_boolean_create turns a tree into primitives + transforms + a postfix program (no device needed).  Checked
+    against the same tree walked in Python: primitive kinds in tree order, every transform == the product of the
+    placements on the way down (4x4 matrices in numpy), and the program evaluates to the tree's set expression on all
+    2^n assignments of its primitives."""
+    import paper_1512_06637_b200 as vg
+    import workloads as W
+    vg._lib.vg_debug_boolean_program.argtypes = [C.c_void_p] * 5
+    for cc in W.csg_cases() + [W.CsgCase("two", ("op", W.SUBTRACTION, ("leaf", W.BOX, [1.0, 2.0, 3.0]), ("leaf", W.ORB, [1.5]),
+                                                 W.placement(W.quaternion_to_matrix((0.5, 0.5, 0.5, 0.5)), (0.1, 0.2, 0.3))), (0, 0, 0), (1, 1, 1), 1)]:
+        shape = cc.build(vg)
+        kinds = (C.c_int * 8)()
+        xf = (C.c_double * 96)()
+        prog = (C.c_ubyte * 16)()
+        nprog = C.c_int(0)
+        nleaf = vg._lib.vg_debug_boolean_program(shape._h, kinds, xf, prog, C.byref(nprog))
+        want = []  # (kind, 4x4 frame of the tree -> frame of the primitive), tree order
+
+        def walk(t, pre):
+            if t[0] == "leaf":
+                want.append((t[1], pre))
+                return ("leaf", len(want) - 1)
+            a = walk(t[2], pre)
+            b = walk(t[3], np.vstack([np.asarray(t[4]).reshape(3, 4), [0, 0, 0, 1]]) @ pre)
+            return ("op", t[1], a, b)
+        expr = walk(cc.tree, np.eye(4))
+        assert nleaf == len(want) and [kinds[i] for i in range(nleaf)] == [k for k, _ in want]
+        X = np.array(xf[:12 * nleaf]).reshape(nleaf, 3, 4)
+        for i, (_, M) in enumerate(want):
+            assert np.max(np.abs(X[i] - M[:3])) < 1e-14, (cc.name, i)
+
+        def ev(e, bits):
+            if e[0] == "leaf":
+                return bool((bits >> e[1]) & 1)
+            a, b = ev(e[2], bits), ev(e[3], bits)
+            return {W.UNION: a or b, W.INTERSECTION: a and b, W.SUBTRACTION: a and not b}[e[1]]
+        for bits in range(1 << nleaf):
+            st = []
+            for tok in prog[:nprog.value]:
+                if tok < 0x80:
+                    st.append(bool((bits >> tok) & 1))
+                else:
+                    b, a = st.pop(), st.pop()
+                    st.append({W.UNION: a or b, W.INTERSECTION: a and b, W.SUBTRACTION: a and not b}[tok & 0x7f])
+            assert len(st) == 1 and st[0] == ev(expr, bits), (cc.name, bits)
+    assert vg._lib.vg_debug_boolean_program(vg.Shape(vg.BOX, [1, 1, 1])._h, None, None, None, None) == vg.ERR_ARG
