@@ -1,17 +1,26 @@
 #!/usr/bin/env python
 """bench.py -- tracks/s per query on one B200 (BASELINE.json `metric`) for the geometry hot path.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-detail]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-detail] [--min-ms M]
 
-A "step" is one pass of the hot path over one batch of synthetic tracks of BASELINE.json configs[1] (tube segment
-rmin 5, rmax 10, dz 15, phi 0..4pi/3, N = 1,048,576 tracks): Inside, DistanceToIn, DistanceToOut, SafetyToIn and
-SafetyToOut, five kernel launches through the C ABI.  `value` = tracks x queries / second with the tracks resident
-in HBM; every launch reads a different copy of the batch (rotating buffer sets whose total size is several times
-the 126 MB L2), so no launch finds its inputs in L2.  The K timed steps are replays of CUDA graphs captured from
-the same C-ABI calls (the launches are microseconds long; eager launches would time the Python interpreter).
-`e2e` is the same step through the host-buffer entry points (pinned host arrays in, host arrays out, copies
-inside the timed region).  `detail` adds every (config, shape, query) of BASELINE.json with its roofline fraction.
-`--impl reference` times the oracle (oracle/, plain scalar CPU code) on the host cores for the same step.
+Workload of the headline: BASELINE.json configs[2], the largest single-GPU configuration -- a cone segment
+(rmin1 2, rmax1 6, rmin2 4, rmax2 12, dz 20, full phi) AND a trd (5, 10, 7, 3, 15), N = 4,194,304 tracks each, all five
+queries (Inside, DistanceToIn, DistanceToOut, SafetyToIn, SafetyToOut) on both: one *pass* = ten kernel launches through
+the C ABI.  A *step* is `config.passes_per_step` passes, chosen so that the timed region (exactly --steps steps) lasts at
+least --min-ms (200 ms); the region is timed five times and the median is reported.  `value` =
+tracks x queries / second with the tracks resident in HBM; every launch reads a different copy of the batch (rotating
+buffer sets, each 201 MB > the 126 MB L2), so no launch finds its inputs in L2.  The steps are replays of a CUDA graph
+captured from the same C-ABI calls.  `e2e` is the same pass through the host-buffer entry points (pinned host arrays in,
+host arrays out, copies inside the timed region).
+
+Output: the LAST stdout line is one compact JSON object (< 2 KB: the driver keeps only the tail of stdout).  Everything
+else -- one row per (config, shape, query) of BASELINE.json configs[0..4] with its roofline fractions, the hot / cold
+variants, the 8(f) rows, the Fig. 4 protocol, the oracle timed on every config -- is printed on EARLIER lines (one JSON
+object per line) and written to `bench_detail.json` beside this file.
+
+`--gpus N` without torchrun starts N ranks itself (torch.distributed.run, one rank per GPU, NCCL only for the timing
+reductions); under torchrun (WORLD_SIZE set) it runs as the rank it is.
+`--impl reference` times the oracle (oracle/, plain scalar CPU code) on the host cores on the same workload.
 """
 import argparse
 import json
@@ -35,6 +44,9 @@ BYTES = {"inside": 24 + 4, "safety_to_in": 24 + 8, "safety_to_out": 24 + 8, "dis
          "distance_to_out": 48 + 8, "compute_step": 48 + 12, "all": 48 + 4 + 4 * 8}
 BYTES.update({"world_locate": 24 + 4, "world_step": 48 + 4 + 8 + 4, "world_safety": 24 + 4 + 8})
 L2_BYTES = 126e6
+COLD_ROTATION_BYTES = 4 * 126e6  # bytes of track arrays in rotation (>= 256 MB): even Inside, which reads half
+                                 # of a set, comes back to a set only after >= 2 x L2 of other reads
+MAX_SETS = 192
 HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
 
 
@@ -176,7 +188,9 @@ class Case:
             band = lambda x, y, z: np.abs(self._gpu3(self.handle.safety_to_in, x, y, z)) < W.SURFACE_BAND
         self.host = world.tracks(self.n, band) if world is not None else W.draw_tracks(seed, self.n, center, half, band)
         per_set = 48 * self.n
-        self.nsets = int(min(16, max(2, -(-int(4 * L2_BYTES) // per_set))))
+        # rotation >= 256 MB and >= 2 x L2 (SURVEY 8(d) cold variant), at most MAX_SETS copies (N <= 2^14 stays L2-resident:
+        # there a launch is two orders of magnitude longer than its bytes take, cold or not)
+        self.nsets = int(min(MAX_SETS, max(2, -(-int(COLD_ROTATION_BYTES) // per_set))))
         self.cold = self.nsets * per_set >= 2 * L2_BYTES
         base = [torch.from_numpy(a).to(dev) for a in self.host]
         self.sets = [base] + [[a.clone() for a in base] for _ in range(self.nsets - 1)]
@@ -248,37 +262,44 @@ def capture_steps(torch, case, with_events):
     return graphs, events
 
 
-def time_query_alone(torch, case, q, min_ms=30.0, hot=False):
-    """Average duration of one launch of `q` (cold inputs): a graph of nsets launches over the rotating sets,
-    replayed between two CUDA events on the launching stream until >= min_ms have been timed.  hot = True: every
-    launch reads the SAME buffer set (what the paper's 5000 repetitions on fixed particles did): the
-    batch stays in the 126 MB L2 if it fits."""
+def time_query_alone(torch, case, q, min_ms=100.0, hot=False, trials=5, want_trials=False):
+    """Duration of one launch of `q` (cold inputs): a graph of nsets launches over the rotating sets, replayed between
+    two CUDA events on the launching stream until >= min_ms have been timed; median of `trials` such regions (SURVEY
+    8(d) protocol).  hot = True: every launch reads the SAME buffer set (what the paper's 5000 repetitions on fixed
+    particles did): the batch stays in the 126 MB L2 if it fits."""
     case.cursor = 0
     case.launch(q)
     torch.cuda.synchronize()
     case.cursor = 0
+    per_graph = case.nsets if not hot else max(case.nsets, 8)
     g = torch.cuda.CUDAGraph()
     with torch.cuda.graph(g):
-        for _ in range(case.nsets):
+        for _ in range(per_graph):
             if hot:
                 case.cursor = 0
             case.launch(q)
     for _ in range(3):
         g.replay()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps, ms = 4, 0.0
-    while True:
+
+    def region(reps):
         torch.cuda.synchronize()
         e0.record()
         for _ in range(reps):
             g.replay()
         e1.record()
         torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1)
-        if ms >= min_ms or reps >= 4096:
-            break
-        reps *= 4
-    return ms * 1e-3 / (reps * case.nsets)
+        return e0.elapsed_time(e1)
+
+    reps = 2
+    ms = region(reps)
+    while ms < min_ms and reps < (1 << 20):  # grow the region to >= min_ms
+        reps = int(max(reps * 2, reps * 1.15 * min_ms / max(ms, 1e-3))) if ms < 0.5 * min_ms else reps * 2
+        ms = region(reps)
+    vals = sorted([ms] + [region(reps) for _ in range(trials - 1)])
+    sec = [v * 1e-3 / (reps * per_graph) for v in vals]
+    med = sec[len(sec) // 2]
+    return (med, sec) if want_trials else med
 
 
 # ------------------------------------------------------------------------------------------ the oracle legs
@@ -291,23 +312,102 @@ def oracle_step(O, shape, tracks, queries):
             getattr(shape, q)(*tracks[:3])
 
 
-def cpu_baseline(seconds=10.0):
-    """The oracle as it stands, timed on this box's host cores on the tracks of configs[1] (all five queries)."""
+HEADLINE_CFG = 2  # BASELINE.json configs[2]: the largest single-GPU configuration (cone + trd, 4,194,304 tracks each)
+HEADLINE_WORKLOAD = "configs[2]: cone(2,6,4,12,20,full phi) + trd(5,10,7,3,15), N=4194304 tracks each, all 5 queries on both"
+
+
+def oracle_headline_inputs(O, n=None):
+    """[(oracle shape, tracks, queries)] of the headline workload, the first n tracks of each shape (None: all)."""
+    out = []
+    for sc in W.shape_cases(HEADLINE_CFG):
+        s = O.Shape(sc.kind, sc.params)
+        m = sc.sizes[-1] if n is None else int(n)
+        out.append((s, sc.tracks(m, band=lambda x, y, z, s=s: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND), sc.queries))
+    return out
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+ORACLE_BUILD = "gcc -O2 -ffp-contract=off -fopenmp, schedule(static)"
+
+
+def cpu_baseline(seconds=10.0, n=1048576):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the headline workload: the first
+    `n` tracks of each of the two configs[2] solids, all five queries, repeated for ~`seconds`."""
     import oracle as O
-    sc = W.shape_cases(1)[0]
-    s = O.Shape(sc.kind, sc.params)
-    t = sc.tracks(sc.sizes[-1], band=lambda x, y, z: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND)
-    oracle_step(O, s, t, sc.queries)  # warm-up (thread pool, page faults)
+    inp = oracle_headline_inputs(O, n)
+    for s, t, qs in inp:
+        oracle_step(O, s, t, qs)  # warm-up (thread pool, page faults)
     reps, t0 = 0, time.perf_counter()
     while True:
-        oracle_step(O, s, t, sc.queries)
+        for s, t, qs in inp:
+            oracle_step(O, s, t, qs)
         reps += 1
         el = time.perf_counter() - t0
         if el >= seconds:
             break
-    return {"value": len(sc.queries) * len(t[0]) * reps / el, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-            "sample": "%d repetitions of the five queries over all %d tracks of configs[1] (%.1f s of wall time, "
-                      "gcc -O2 -ffp-contract=off, OpenMP static)" % (reps, len(t[0]), el)}
+    units = sum(len(qs) * len(t[0]) for _, t, qs in inp)
+    return {"value": units * reps / el, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": "%d x (5 queries on the first %d tracks of each configs[2] solid), %.1f s wall" % (reps, n, el),
+            "cpu": cpu_model(), "build": ORACLE_BUILD}
+
+
+def cpu_per_config(budget_s=6.0):
+    """The oracle on every config of BASELINE.json: one thread and all cores, full N
+    unless one pass at full N would exceed `budget_s` seconds (then a prefix whose size is stated; the oracle's cost
+    per track does not depend on N).  Rows go to the side file; the compact line carries the two rates per config."""
+    import oracle as O
+    all_threads = O.num_threads()
+    plan = []
+    for k in (0, 1, 2, 3):
+        for sc in W.shape_cases(k):
+            s = O.Shape(sc.kind, sc.params)
+            plan.append((k, sc.name, sc.sizes[-1], sc.queries, s,
+                         lambda m, sc=sc, s=s: sc.tracks(m, band=lambda x, y, z: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND)))
+    nav = W.navigator_case()
+    vo = O.Volume(O.Shape(nav.mother_kind, nav.mother_params),
+                  [O.Shape(kk, pp) for kk, pp in zip(nav.daughter_kinds, nav.daughter_params)], nav.xforms)
+    plan.append((4, "navigator", nav.sizes[-1], ("compute_step",), vo,
+                 lambda m: nav.tracks(m, band=lambda x, y, z: vo.safety(x, y, z) < W.SURFACE_BAND)))
+
+    def one_pass(obj, t, qs):
+        if qs == ("compute_step",):
+            obj.compute_step(*t, W.STEP_MAX)
+        else:
+            oracle_step(O, obj, t, qs)
+
+    rows = []
+    try:
+        for k, name, nfull, qs, obj, draw in plan:
+            probe = draw(16384)
+            O.set_num_threads(1)
+            one_pass(obj, probe, qs)
+            t0 = time.perf_counter()
+            one_pass(obj, probe, qs)
+            per_track_1 = (time.perf_counter() - t0) / 16384
+            for threads in (1, all_threads):
+                O.set_num_threads(threads)
+                n = int(min(nfull, max(16384, budget_s / (per_track_1 / threads * (1.0 if threads == 1 else 1.5)))))
+                t = draw(n)
+                one_pass(obj, t, qs)  # warm-up: page faults of the result arrays, thread pool
+                t0 = time.perf_counter()
+                one_pass(obj, t, qs)
+                el = time.perf_counter() - t0
+                rows.append({"row": "cpu_oracle", "config": k, "shape": name, "queries": list(qs), "n": n, "n_full": nfull,
+                             "threads": threads, "seconds_per_pass": el, "ns_per_track_query": el * 1e9 / (n * len(qs)),
+                             "track_queries_per_s": n * len(qs) / el, "cpu": cpu_model(), "build": ORACLE_BUILD})
+    finally:
+        O.set_num_threads(all_threads)
+    return rows
 
 
 # ---- the paper's own measurement (Fig. 4, PAPER.md:120-136): DistanceToOut on a Box and a Tube, particles placed at
@@ -400,35 +500,39 @@ def fig4_gpu(vg, torch, reps=5000):
 
 
 def run_reference(args, rank):
-    """--impl reference: the oracle on the host cores, same config / metric / unit (rank 0 only)."""
+    """--impl reference: the oracle on the host cores, same workload / metric / unit (rank 0 only).  Each step is one
+    pass (five queries, both configs[2] solids) over a prefix of the tracks sized so that the run ends within ~2 min."""
     if rank != 0:
         return
     import oracle as O
-    sc = W.shape_cases(1)[0]
-    s = O.Shape(sc.kind, sc.params)
-    full = sc.tracks(sc.sizes[-1], band=lambda x, y, z: np.abs(s.sdf(x, y, z)) < W.SURFACE_BAND)
-    probe = [a[:65536] for a in full]
-    oracle_step(O, s, probe, sc.queries)
+    probe = oracle_headline_inputs(O, 65536)
+    for s, t, qs in probe:
+        oracle_step(O, s, t, qs)
     t0 = time.perf_counter()
-    oracle_step(O, s, probe, sc.queries)
-    per_track = (time.perf_counter() - t0) / 65536
-    budget = 120.0  # seconds for the whole --steps + --warmup run
-    n = int(min(len(full[0]), max(4096, budget / ((args.steps + args.warmup) * per_track))))
-    t = [np.ascontiguousarray(a[:n]) for a in full]
+    for s, t, qs in probe:
+        oracle_step(O, s, t, qs)
+    per_track = (time.perf_counter() - t0) / 65536  # seconds per track of BOTH solids, five queries each
+    budget = 100.0  # seconds for the whole --steps + --warmup run
+    nfull = W.shape_cases(HEADLINE_CFG)[0].sizes[-1]
+    n = int(min(nfull, max(4096, budget / ((args.steps + args.warmup) * per_track))))
+    inp = oracle_headline_inputs(O, n)
     for _ in range(args.warmup):
-        oracle_step(O, s, t, sc.queries)
+        for s, t, qs in inp:
+            oracle_step(O, s, t, qs)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_step(O, s, t, sc.queries)
+        for s, t, qs in inp:
+            oracle_step(O, s, t, qs)
     el = time.perf_counter() - t0
-    value = len(sc.queries) * n * args.steps / el
-    sample = "each step = the five queries over the first %d of the %d tracks of configs[1]" % (n, len(full[0]))
+    units = sum(len(qs) * len(t[0]) for _, t, qs in inp)
+    value = units * args.steps / el
+    sample = "each step = 5 queries on the first %d of the %d tracks of each configs[2] solid" % (n, nfull)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": el * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[1]: tube segment rmin=5 rmax=10 dz=15 phi 0..4pi/3, five queries", "n_tracks": n,
-                       "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+            "config": {"workload": HEADLINE_WORKLOAD, "n_tracks_per_solid_per_step": n, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample,
+                             "cpu": cpu_model(), "build": ORACLE_BUILD},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -473,9 +577,18 @@ def launch_floor(vg, torch, per_graph=64, reps=50):
     return e0.elapsed_time(e1) * 1e-3 / (reps * per_graph)
 
 
-def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
-    """Every (config, shape, query) of BASELINE.json configs[0..4], each launch timed alone on cold inputs."""
+def detail_sweep(vg, torch, hbm_peak, fma_rate, have, headline_rows, min_ms, emit):
+    """Every (config, shape, query) of BASELINE.json configs[0..4], each launch timed alone on cold inputs (and hot, where
+    a batch fits L2), then the SURVEY 8(f) rows.  `have` = the headline's cases by shape name (reused, not re-drawn),
+    `headline_rows` = their rows already timed with the full protocol."""
     rows = []
+
+    def add(e):
+        rows.append(e)
+        emit(e)
+
+    tq = lambda case, q, **kw: time_query_alone(torch, case, q, min_ms=min_ms, **kw)
+    tq3 = lambda case, q: time_query_alone(torch, case, q, min_ms=min_ms / 2, trials=3)  # 8(f) rows
     floor_s = launch_floor(vg, torch)
     plan = []
     for k in (0, 1, 2, 3):
@@ -483,31 +596,38 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
             for n in sc.sizes:
                 plan.append((k, sc, n))
     for k, sc, n in plan:
-        case = main_case if (k == 1) else Case(vg, torch, sc.name, n, sc.queries, shape=sc)
+        mine = sc.name not in have
+        case = Case(vg, torch, sc.name, n, sc.queries, shape=sc) if mine else have[sc.name]
         for q in sc.queries:
-            sec = time_query_alone(torch, case, q)
-            e = roofline_entry(case.kind, q, n, sec, hbm_peak, fma_rate)
-            e.update({"config": k, "shape": sc.name, "query": q, "n": n, "cold_inputs": case.cold})
+            if not mine:
+                e = dict(headline_rows[(sc.name, q)])
+            else:
+                sec = tq(case, q)
+                e = roofline_entry(case.kind, q, n, sec, hbm_peak, fma_rate)
+            e.update({"config": k, "shape": sc.name, "query": q, "n": n, "cold_inputs": case.cold, "sets_in_rotation": case.nsets})
+            if 48 * n <= 0.5 * L2_BYTES:  # the hot variant: same buffers every launch, the batch stays in L2
+                hot_s = tq(case, q, hot=True)
+                e.update({"hot_us_per_launch": hot_s * 1e6, "hot_tracks_per_s": n / hot_s})
             if n <= 262144:  # launch-bound sizes: the bound a single launch can reach is max(bytes / BW, empty launch)
                 ideal = max(BYTES[q] * n / (hbm_peak * 1e9), floor_s)
                 e.update({"empty_launch_us": floor_s * 1e6, "latency_adjusted_bound_us": ideal * 1e6,
-                          "latency_adjusted_frac": ideal / sec})
-            rows.append(e)
+                          "latency_adjusted_frac": ideal / (e["us_per_launch"] * 1e-6)})
+            add(e)
         if len(sc.queries) == 5 and sc.kind != W.POLYCONE:  # the fused five-query kernel on the same tracks
-            sec = time_query_alone(torch, case, "all")
+            sec = tq(case, "all")
             e = roofline_entry(case.kind, "all", n, sec, hbm_peak, fma_rate)
             e.update({"config": k, "shape": sc.name, "query": "all five (vg_query_all, one kernel)", "n": n, "cold_inputs": case.cold,
                       "track_queries_per_s": 5 * n / sec})
-            rows.append(e)
-        if case is not main_case:
+            add(e)
+        if mine:
             del case
             torch.cuda.empty_cache()
     nav = W.navigator_case()
     case = Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step",), nav=nav)
-    sec = time_query_alone(torch, case, "compute_step")
+    sec = tq(case, "compute_step")
     e = roofline_entry("navigator", "compute_step", case.n, sec, hbm_peak, fma_rate)
     e.update({"config": 4, "shape": "box(100)+64 daughters", "query": "compute_step", "n": case.n, "cold_inputs": case.cold})
-    rows.append(e)
+    add(e)
     del case
     torch.cuda.empty_cache()
     # polycone variants -- the configs[3] polycone cut to phi in [0, 4 pi / 3], and one with two z steps
@@ -518,53 +638,53 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, main_case):
                          ("distance_to_in", "safety_to_in"))
         case = Case(vg, torch, sc.name, 4194304, sc.queries, shape=sc)
         for q in sc.queries:
-            sec = time_query_alone(torch, case, q)
+            sec = tq3(case, q)
             e = roofline_entry("polycone_variant", q, case.n, sec, hbm_peak, fma_rate)
             e.update({"config": "8(f) f2", "shape": vname, "query": q, "n": case.n, "cold_inputs": case.cold, "bound": "alu"})
-            rows.append(e)
+            add(e)
         del case
         torch.cuda.empty_cache()
     # boolean solids of two primitives (one of each operation)
     for bc in [b for b in W.boolean_cases() if b.name in ("tube_union_box", "cone_intersection_orb", "box_minus_tube")]:
         case = Case(vg, torch, bc.name, 4194304, W.QUERIES5, boolean=bc)
         for q in case.queries:
-            sec = time_query_alone(torch, case, q)
+            sec = tq3(case, q)
             e = roofline_entry("boolean", q, case.n, sec, hbm_peak, fma_rate)
             e.update({"config": "8(f) f2", "shape": bc.name, "query": q, "n": case.n, "cold_inputs": case.cold})
             if q.startswith("distance"):
                 e["bound"] = "alu"
-            rows.append(e)
+            add(e)
         del case
         torch.cuda.empty_cache()
     cc = [c for c in W.csg_cases() if c.name == "twice_drilled_block_in_a_sphere"][0]  # a tree of four primitives (R31)
     case = Case(vg, torch, cc.name, 4194304, W.QUERIES5, csg=cc)
     for q in case.queries:
-        sec = time_query_alone(torch, case, q)
+        sec = tq3(case, q)
         e = roofline_entry("boolean", q, case.n, sec, hbm_peak, fma_rate)
         e.update({"config": "8(f) f2", "shape": "csg tree: " + cc.name, "query": q, "n": case.n, "cold_inputs": case.cold, "bound": "alu"})
-        rows.append(e)
+        add(e)
     del case
     torch.cuda.empty_cache()
     # the three-level tree of placed solids (193 nodes), every track in its own node
     wc = W.world_case()
     case = Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc)
     for q in case.queries:
-        sec = time_query_alone(torch, case, q)
+        sec = tq3(case, q)
         e = roofline_entry("world", q, case.n, sec, hbm_peak, fma_rate)
         e.update({"config": "8(f) f3", "shape": "box(100) > 64 daughters > 128 grand-daughters", "query": q, "n": case.n,
                   "cold_inputs": case.cold, "bound": "alu", "track_order": "as drawn (nodes mixed within a warp)"})
-        rows.append(e)
+        add(e)
     # the same tracks in basket order (sorted by node, what the paper's scheduler hands to the geometry)
     for k in range(case.nsets):
         order = torch.argsort(case.nodes[k].to(torch.int64), stable=True)
         case.sets[k] = [a[order].contiguous() for a in case.sets[k]]
         case.nodes[k] = case.nodes[k][order].contiguous()
     for q in case.queries:
-        sec = time_query_alone(torch, case, q)
+        sec = tq3(case, q)
         e = roofline_entry("world", q, case.n, sec, hbm_peak, fma_rate)
         e.update({"config": "8(f) f3", "shape": "box(100) > 64 daughters > 128 grand-daughters", "query": q, "n": case.n,
                   "cold_inputs": case.cold, "bound": "alu", "track_order": "sorted by node (baskets)"})
-        rows.append(e)
+        add(e)
     return rows
 
 
@@ -605,6 +725,52 @@ def run_profile(args):
     print(json.dumps({"profile_mode": True, "launches": vg.vg_launch_count()}))
 
 
+def _sig(v, digits=4):
+    """Floats of the compact line rounded to `digits` significant digits (the line must stay under 2 KB)."""
+    if isinstance(v, float):
+        return float("%.*g" % (digits, v)) if v == v and abs(v) != float("inf") else None
+    if isinstance(v, dict):
+        return {k: _sig(x, digits) for k, x in v.items()}
+    if isinstance(v, (list, tuple)):
+        return [_sig(x, digits) for x in v]
+    return v
+
+
+KERNEL_NAME = {  # launch form of AUTO for the headline kernels (csrc/vg_kernels.cuh Tune<S, Q>); ncu names in profiles/
+    "cone": "query_kernel<ConeT<1>,%s>", "trd": "query_kernel<Trd,%s>"}
+NCU_SOLID = {"cone": "Cone", "trd": "Trd", "tube": "Tube", "box": "Box", "orb": "Orb", "polycone": "Polycone"}
+SHORT_Q = {"inside": "in", "distance_to_in": "dti", "distance_to_out": "dto", "safety_to_in": "sti", "safety_to_out": "sto",
+           "compute_step": "step"}
+HBM_NOMINAL_GBS = 8000.0  # BASELINE.json north_star: "~8 TB/s peak"; the 70 % target is read against this (SURVEY 8(d))
+
+
+def per_config_rows(detail, fma_rate):
+    """<= 10 short rows for the compact line: per (config, shape) the query FURTHEST below its bound.  us = one launch
+    (cold inputs), f = fraction of the measured HBM copy rate, f8 = fraction of the nominal 8 TB/s, fp64 = SURVEY 8(d)'s
+    algorithmic FP64 operations / s over the FP64 rate measured in this run (ALU-bound rows), lat = latency-adjusted
+    fraction max(bytes / BW, empty launch) / measured (launch-bound sizes)."""
+    groups = {}
+    for e in detail:
+        if e.get("row") or not isinstance(e.get("config"), int) or str(e["query"]).startswith("all five"):
+            continue
+        groups.setdefault((e["config"], e["shape"], e["n"]), []).append(e)
+    keep = []
+    for (k, shape, n), es in sorted(groups.items(), key=lambda kv: (kv[0][0], kv[0][1], kv[0][2])):
+        if k == 3 and n not in (1024, 16777216):
+            continue
+        score = lambda e: e["latency_adjusted_frac"] if n <= 262144 else (e.get("fp64_frac") if e["bound"] == "alu" else e["hbm_frac"])
+        w = min(es, key=score)
+        r = {"c": "%d %s 2^%d" % (k, shape.split("(")[0][:8], n.bit_length() - 1), "q": SHORT_Q.get(w["query"], w["query"]), "us": w["us_per_launch"]}
+        if n <= 262144:
+            r["lat"] = w["latency_adjusted_frac"]
+        elif w["bound"] == "alu":
+            r["fp64"] = w["fp64_frac"]
+        else:
+            r["f"], r["f8"] = w["hbm_frac"], w["hbm_gbs"] / HBM_NOMINAL_GBS
+        keep.append(_sig(r, 3))
+    return keep
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     if not torch.cuda.is_available():
@@ -623,161 +789,236 @@ def run_ours(args, rank, world, local_rank):
     if args.no_pdl:
         vg.vg_set_option(vg.OPT_PDL, 0)
 
+    side = []  # every row of the side file, in the order it is produced
+
+    def emit(row):
+        side.append(row)
+        if rank == 0:
+            print(json.dumps(_sig(row, 6)), flush=True)
+
     hbm_peak, hbm_src = measured_peaks()
     sampler = ClockSampler(local_rank)
     sampler.start()
     load0 = time.time()
-    fma_rate = 1.0  # measured below, AFTER the timed region and the per-query timings: the probe drives the FP64 pipe at full
-                    # power for ~70 ms and would leave the board power-capped for the measurements that matter
+    warmup = max(args.warmup, 3)
 
-    # weak scaling: every rank owns one full configs[1] batch (its own seed); no data-path collective
-    sc = W.shape_cases(1)[0]
-    case = Case(vg, torch, sc.name, sc.sizes[-1], sc.queries, seed_shift=1000 * rank, shape=sc)
-    graphs, _ = capture_steps(torch, case, False)
-    for i in range(max(args.warmup, 3)):
-        graphs[i % len(graphs)].replay()
+    # weak scaling: every rank owns one full configs[2] batch (its own seeds); no data-path collective
+    cases = [Case(vg, torch, sc.name, sc.sizes[-1], sc.queries, seed_shift=1000 * rank, shape=sc)
+             for sc in W.shape_cases(HEADLINE_CFG)]
+    launches = [(c, q) for c in cases for q in c.queries]  # one pass = ten launches
+    nsets = max(c.nsets for c in cases)
+    for c, q in launches:  # eager warm-up before capture (lazy attribute / occupancy queries happen here)
+        c.launch(q)
     torch.cuda.synchronize()
-    barrier()
+    for c in cases:
+        c.cursor = 0
+    graph = torch.cuda.CUDAGraph()  # nsets passes: after them every launch position has used every buffer set
+    with torch.cuda.graph(graph):
+        for _ in range(nsets):
+            for c, q in launches:
+                c.launch(q)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0 = time.time()
+    graph.replay()
+    torch.cuda.synchronize()
     e0.record()
-    for i in range(args.steps):
-        graphs[i % len(graphs)].replay()
+    graph.replay()
     e1.record()
     torch.cuda.synchronize()
+    replay_ms = max_over_ranks(e0.elapsed_time(e1), "cuda")
+    replays_per_step = max(1, int(-(-args.min_ms // (args.steps * replay_ms)))) if args.min_ms > 0 else 1
+    passes_per_step = replays_per_step * nsets
+    for _ in range(warmup):
+        for _ in range(replays_per_step):
+            graph.replay()
+    torch.cuda.synchronize()
+    trial_ms, t0 = [], time.time()
+    for _ in range(args.trials):  # the timed region (exactly --steps steps), `trials` times; the median is reported
+        barrier()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps * replays_per_step):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        barrier()
+        trial_ms.append(max_over_ranks(e0.elapsed_time(e1), "cuda"))
     t1 = time.time()
-    barrier()
-    ms = max_over_ranks(e0.elapsed_time(e1), "cuda")
-    tracks_all = sum_over_ranks(case.n, "cuda")
-    nq = len(case.queries)
-    value = tracks_all * nq * args.steps / (ms * 1e-3)
+    ms = sorted(trial_ms)[len(trial_ms) // 2]
+    units_per_pass = sum_over_ranks(sum(c.n * len(c.queries) for c in cases), "cuda")  # track-queries, all ranks
+    value = units_per_pass * passes_per_step * args.steps / (ms * 1e-3)
+    pass_us = ms * 1e3 / (args.steps * passes_per_step)
+    algo_bytes_per_pass = sum(BYTES[q] * c.n for c, q in launches)
 
-    # per-kernel durations, same process, right after the timed region: event-record nodes between the kernel nodes
-    # of the timed graphs cost ~5 us each (measured) and would distort `value`, so every query is timed alone as a
-    # graph of nsets back-to-back launches (cold inputs) between two CUDA events on the launching stream
-    kernel_timing = "each query alone: graph of %d back-to-back launches over the rotating buffer sets between two CUDA events" % case.nsets
-    per_q = {q: time_query_alone(torch, case, q) for q in case.queries}
-
-    per_query = {q: roofline_entry(case.kind, q, case.n, per_q[q], hbm_peak, fma_rate) for q in case.queries}
-    for q in case.queries:  # the hot variant: same buffers every launch, the 48 MB batch stays in L2
-        hot_s = time_query_alone(torch, case, q, hot=True)
-        per_query[q]["hot_us_per_launch"] = hot_s * 1e6
-        per_query[q]["hot_tracks_per_s"] = case.n / hot_s
-    dom = max(case.queries, key=lambda q: per_q[q])
-    kname = ("query_stream_kernel<TubeT<hollow, wide phi>, %s>" if dom == "distance_to_in" else "query_kernel<TubeT<hollow, wide phi>, %s>") % dom
-    roof = {"bound": "hbm", "kernel": kname, "achieved": per_query[dom]["hbm_gbs"],
-            "peak": hbm_peak, "unit": "GB/s", "frac": per_query[dom]["hbm_gbs"] / hbm_peak, "peak_source": hbm_src,
-            "traffic": (ncu_traffic("Tube", dom, case.n) or {}).get("bytes"), "traffic_detail": ncu_traffic("Tube", dom, case.n),
-            "algorithmic_bytes_per_launch": BYTES[dom] * case.n,
-            "us_per_launch": per_q[dom] * 1e6, "share_of_step": per_q[dom] / sum(per_q.values()),
-            "sum_of_kernels_us": sum(per_q.values()) * 1e6,
-            "kernel_timing": kernel_timing,
-            "step_hbm_frac": sum(BYTES[q] for q in case.queries) * case.n / (ms * 1e-3 / args.steps) / 1e9 / hbm_peak}
-
-    # the same step as ONE fused kernel (vg_query_all): 48 B read + 36 B written per track instead of 168 + 36
-    fused_s = time_query_alone(torch, case, "all")
-    fused = {"us_per_step": fused_s * 1e6, "value": nq * case.n / fused_s, "unit": UNIT, "api": "vg_query_all (one kernel, five results)",
-             "hbm_gbs": BYTES["all"] * case.n / fused_s / 1e9, "hbm_frac": BYTES["all"] * case.n / fused_s / 1e9 / hbm_peak,
-             "algorithmic_bytes_per_track": BYTES["all"], "speedup_vs_five_launches": sum(per_q.values()) / fused_s,
-             "note": "reported beside `value`, which stays the five per-query launches BASELINE.json's metric names"}
+    # per-kernel durations, same process, right after the timed region: event-record nodes between the kernel nodes of
+    # the timed graph cost ~5 us each (measured) and would distort `value`, so every query is timed alone as a graph of
+    # back-to-back launches over the rotating sets (cold inputs) between two CUDA events on the launching stream
+    head_rows, per_q = {}, {}
+    for c, q in launches:
+        sec, tr = time_query_alone(torch, c, q, min_ms=args.min_ms, trials=args.trials, want_trials=True)
+        per_q[(c.name, q)] = sec
+        e = roofline_entry(c.kind, q, c.n, sec, hbm_peak, 1.0)
+        e.update({"hbm_frac_of_8TBs": e["hbm_gbs"] / HBM_NOMINAL_GBS, "trials_us": [x * 1e6 for x in tr]})
+        head_rows[(c.name, q)] = e
+    dom = max(per_q, key=per_q.get)
+    dcase = [c for c in cases if c.name == dom[0]][0]
+    tr = ncu_traffic(NCU_SOLID.get(dcase.kind, dcase.kind), dom[1], dcase.n)
+    sum_k = sum(per_q.values())
+    roof = {"bound": "hbm", "kernel": KERNEL_NAME.get(dcase.kind, "%s") % dom[1], "achieved": head_rows[dom]["hbm_gbs"],
+            "peak": hbm_peak, "unit": "GB/s", "frac": head_rows[dom]["hbm_gbs"] / hbm_peak,
+            "peak_source": hbm_src, "frac_of_8TBs": head_rows[dom]["hbm_gbs"] / HBM_NOMINAL_GBS,
+            "traffic": (tr or {}).get("bytes"), "traffic_capture": (tr or {}).get("capture"),
+            "algorithmic_bytes_per_launch": BYTES[dom[1]] * dcase.n, "us_per_launch": per_q[dom] * 1e6,
+            "share_of_pass": per_q[dom] / sum_k, "sum_of_kernels_us": sum_k * 1e6, "pass_us": pass_us,
+            "pass_hbm_frac": algo_bytes_per_pass / (pass_us * 1e-6) / 1e9 / hbm_peak}
 
     # end to end: pinned host arrays -> C-ABI host entry point -> pinned host results, copies inside the timed region.
-    # The call a user makes for one step over host tracks is vg_query_all_host (the tracks cross the host link once);
-    # the five single-query host calls are timed beside it.
-    # the host basket is ONE pinned [6][n] allocation (and the four FP64 results one [4][n]): equally spaced arrays cross
-    # the link as one strided copy per chunk (vg_host.cu); separately allocated arrays work too, with six copies per chunk
-    hblock = torch.empty((6, case.n), dtype=torch.float64).pin_memory()
-    for i, a in enumerate(case.host):
-        hblock[i].copy_(torch.from_numpy(a))
-    host = [hblock[i] for i in range(6)]
-    oblock = torch.empty((4, case.n), dtype=torch.float64).pin_memory()
-    hout_d = [oblock[i] for i in range(4)]
-    hout_i = torch.empty(case.n, dtype=torch.int32).pin_memory()
+    # The call a user makes for one pass over host tracks is vg_query_all_host per solid (the tracks cross the host link
+    # once for all five answers).  Each host basket is ONE pinned [6][n] allocation (and the four FP64 results one
+    # [4][n]): equally spaced arrays cross the link as one strided copy per chunk (vg_host.cu).
+    hostbuf = []
+    for c in cases:
+        hb = torch.empty((6, c.n), dtype=torch.float64).pin_memory()
+        for i, a in enumerate(c.host):
+            hb[i].copy_(torch.from_numpy(a))
+        ob = torch.empty((4, c.n), dtype=torch.float64).pin_memory()
+        hostbuf.append((c, [hb[i] for i in range(6)], [torch.empty(c.n, dtype=torch.int32).pin_memory()] + [ob[i] for i in range(4)]))
 
-    def e2e_step():
-        case.handle.query_all_host(*host, step_max=W.STEP_MAX, out=[hout_i] + hout_d)
+    def e2e_pass():
+        for c, hin, hout in hostbuf:
+            c.handle.query_all_host(*hin, step_max=W.STEP_MAX, out=hout)
 
-    def e2e_step5():
-        for q in case.queries:
-            case.handle.query_host(q, *host, step_max=W.STEP_MAX, out=hout_i if q == "inside" else hout_d[0])
-
-    def time_e2e(fn):
-        for _ in range(3):
-            fn()
+    for _ in range(2):
+        e2e_pass()
+    w0 = time.perf_counter()
+    e2e_pass()
+    one = time.perf_counter() - w0
+    ke = max(3, int(-(-args.min_ms * 1e-3 // one))) if args.min_ms > 0 else 3
+    e2e_trials = []
+    for _ in range(3):
         barrier()
         w0 = time.perf_counter()
         for _ in range(ke):
-            fn()
+            e2e_pass()
         w1 = time.perf_counter()
         barrier()
-        return max_over_ranks(w1 - w0, "cuda")
+        e2e_trials.append(max_over_ranks(w1 - w0, "cuda"))
+    e2e_s = sorted(e2e_trials)[1]
+    h2d = sum(48 * c.n for c in cases)
+    d2h = sum(36 * c.n for c in cases)
+    e2e = {"value": units_per_pass * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+           "steps": ke, "ms_per_step": e2e_s * 1e3 / ke, "passes_per_step": 1,
+           "host_link_gbs": (h2d + d2h) / (e2e_s / ke) / 1e9, "api": "vg_query_all_host per solid, pinned [6][n] baskets"}
+    del hostbuf
 
-    ke = max(3, min(args.steps, 20))
-    e2e_s = time_e2e(e2e_step)
-    e2e5_s = time_e2e(e2e_step5)
-    h2d5 = sum((48 if q.startswith("distance") else 24) for q in case.queries) * case.n
-    d2h = sum((4 if q == "inside" else 8) for q in case.queries) * case.n
-    e2e = {"value": tracks_all * nq * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 48 * case.n, "d2h_bytes_per_step": d2h,
-           "steps": ke, "ms_per_step": e2e_s * 1e3 / ke,
-           "api": "vg_query_all_host (one pinned [6][n] host basket in, pinned results out, chunked copy/compute overlap)",
-           "host_link_gbs": (48 * case.n + d2h) / (e2e_s / ke) / 1e9,
-           "five_single_query_calls": {"value": tracks_all * nq * ke / e2e5_s, "ms_per_step": e2e5_s * 1e3 / ke,
-                                       "h2d_bytes_per_step": h2d5, "d2h_bytes_per_step": d2h, "api": "vg_query_host x5"}}
-
-    fma_rate = vg.vg_probe_fp64_fma_rate(30)  # the ALU-bound rows of `detail` are the only users (configs[1] is HBM-bound)
-    launches_per_step = nq
+    # FP64 rate probe AFTER the timed regions above: it drives the FP64 pipe at full power for ~70 ms and would leave the
+    # board power-capped for the measurements that matter; the ALU-bound rows of the sweep are its only users
+    fma_rate = vg.vg_probe_fp64_fma_rate(30)
     detail, fig4 = None, None
+    have = {c.name: c for c in cases}
     if world == 1 and not args.no_detail:
-        detail = detail_sweep(vg, torch, hbm_peak, fma_rate, case)
+        emit({"row": "header", "note": "one JSON object per line; the LAST line is the compact bench record", "hbm_peak_gbs": hbm_peak,
+              "hbm_peak_source": hbm_src, "fp64_fma_per_s": fma_rate, "fp64_tflops": 2 * fma_rate / 1e12,
+              "fp64_how": "register-resident DFMA chains, vg_probe_fp64_fma_rate, same run",
+              "timing": "each launch alone: graph of back-to-back launches over rotating buffer sets, >= %g ms per region, median of %d" % (args.min_ms, args.trials)})
+        detail = detail_sweep(vg, torch, hbm_peak, fma_rate, have, head_rows, args.min_ms * args.detail_scale, emit)
         fig4 = fig4_gpu(vg, torch)
+    else:
+        for (name, q), e in head_rows.items():
+            e.update({"config": HEADLINE_CFG, "shape": name, "query": q, "n": have[name].n, "cold_inputs": have[name].cold})
+            emit(e)
+        detail = list(head_rows.values())
     load1 = time.time()
     sampler.stop()
     clocks = sampler.summary(t0, t1, load0, load1)
 
     if rank == 0:
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
                 "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": "configs[1]: tube segment rmin=5 rmax=10 dz=15 phi 0..4pi/3, N=%d tracks per GPU, "
-                                       "Inside + DistanceToIn + DistanceToOut + SafetyToIn + SafetyToOut per step" % case.n,
-                           "n_tracks_per_gpu": case.n, "queries_per_step": nq, "step_max": W.STEP_MAX,
-                           "l2_policy": "inputs larger than L2: every launch reads the next of %d copies of the batch "
-                                        "(%d MB of inputs in rotation, L2 = 126 MB)" % (case.nsets, case.nsets * 48 * case.n // 10 ** 6),
-                           "launch": "CUDA graphs captured from the C-ABI calls, one graph per step",
-                           "pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N), "form": vg.vg_get_option(vg.OPT_FORM), "pdl": vg.vg_get_option(vg.OPT_PDL),
-                           "parallelism": "tracks sharded over ranks, no collective" if world > 1 else "1 GPU"},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
-                "roofline": roof, "per_query": per_query, "fused": fused,
-                "fp64_peak": {"fma_per_s": fma_rate, "tflops": 2 * fma_rate / 1e12,
-                              "how": "register-resident DFMA chains, vg_probe_fp64_fma_rate, same run"}}
+                "config": {"workload": HEADLINE_WORKLOAD, "n_tracks": cases[0].n, "launches_per_pass": len(launches),
+                           "passes_per_step": passes_per_step, "trials": "median of %d" % args.trials, "timed_ms": ms,
+                           "l2": "inputs > L2: %d rotating copies of 201 MB per solid" % nsets,
+                           "parallelism": "tracks sharded, no collective" if world > 1 else "1 GPU"},
+                "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+                "gpu_launches": len(launches) * passes_per_step * args.steps,
+                "roofline": {k: roof[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "frac_of_8TBs", "traffic",
+                                                  "algorithmic_bytes_per_launch", "us_per_launch", "share_of_pass", "pass_hbm_frac")},
+                "e2e": {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step")},
+                "fp64_tflops_measured": 2 * fma_rate / 1e12}
+        emit({"row": "headline", "trial_ms": trial_ms, "roofline": roof, "e2e": e2e, "clocks": clocks,
+              "options": {"pipe_min_n": vg.vg_get_option(vg.OPT_PIPE_MIN_N), "form": vg.vg_get_option(vg.OPT_FORM), "pdl": vg.vg_get_option(vg.OPT_PDL)}})
         if world == 1:
-            line["cpu_baseline"] = cpu_baseline()
+            cb = cpu_baseline(seconds=args.cpu_seconds)
+            line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            emit(dict(cb, row="cpu_baseline"))
             if fig4 is not None:  # the serial-CPU leg of the Fig. 4 protocol and the speed relative to it
-                cpu4 = fig4_cpu()
-                line["cpu_baseline"]["fig4_serial"] = cpu4
-                ref = {(r["shape"], r["n"]): r["us_per_call"] for r in cpu4}
+                ref = {(r["shape"], r["n"]): r["us_per_call"] for r in fig4_cpu()}
                 for r in fig4:
                     r["serial_oracle_us_per_call"] = ref[(r["shape"], r["n"])]
                     r["speedup_device_resident"] = r["serial_oracle_us_per_call"] / r["device_resident_us_per_launch"]
                     r["speedup_host_fed"] = r["serial_oracle_us_per_call"] / r["host_fed_us_per_call"]
-                line["fig4_protocol"] = {"what": "PAPER.md:120-136 (Fig. 4): DistanceToOut, Box and Tube, particles inside the body, "
-                                                 "speed relative to a serial CPU code (here: the oracle on one thread; the paper's "
-                                                 "own curve is not in the text, BASELINE.md)", "rows": fig4}
-        if detail is not None:
-            line["detail"] = detail
-        print(json.dumps(line), flush=True)
+                    emit(dict(r, row="fig4_protocol", what="PAPER.md:120-136 (Fig. 4): DistanceToOut, particles inside the body, speed "
+                              "relative to a serial CPU code (here the oracle on one thread; the paper's curve is not in the text)"))
+            if not args.no_detail:
+                cpu_rows = cpu_per_config()
+                for r in cpu_rows:
+                    emit(r)
+                # per config: [one thread, all cores] in 1e6 track-queries/s, all shapes of the config pooled
+                pool = {}
+                for r in cpu_rows:
+                    a = pool.setdefault((r["config"], r["threads"]), [0.0, 0.0])
+                    a[0] += r["n"] * len(r["queries"])
+                    a[1] += r["seconds_per_pass"]
+                line["cpu_Mtq_s_1thr_allcores"] = {str(k): [pool[(k, t)][0] / pool[(k, t)][1] / 1e6 for t in sorted({t for kk, t in pool if kk == k})]
+                                                   for k in sorted({kk for kk, _ in pool})}
+                line["per_config"] = per_config_rows(detail, fma_rate)
+        line["detail"] = "bench_detail.json"
+        try:
+            with open(os.path.join(ROOT, "bench_detail.json"), "w") as f:
+                json.dump({"line": line, "rows": side}, f, indent=1)
+        except OSError:
+            line["detail"] = "earlier stdout lines"
+        out = json.dumps(_sig(line), separators=(",", ":"))
+        for drop in ("cpu_Mtq_s_1thr_allcores", "fp64_tflops_measured"):  # never let the record outgrow the driver's tail
+            if len(out) > 2000 and drop in line:
+                del line[drop]
+                out = json.dumps(_sig(line), separators=(",", ":"))
+        while len(out) > 2000 and line.get("per_config"):
+            line["per_config"].pop()
+            out = json.dumps(_sig(line), separators=(",", ":"))
+        print(out, flush=True)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` as a plain command: start one rank per GPU under torch.distributed.run (what the driver
+    does itself for N > 1) and pass this process's arguments through."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")  # the driver counts ranks from NCCL's own log
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5000)
-    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--no-detail", action="store_true", help="skip the per-config sweep (configs[0..4])")
+    ap.add_argument("--min-ms", type=float, default=200.0,
+                    help="minimum length of every timed region in ms (SURVEY 8(d): >= 200 ms; 0 = one graph replay per step, for ncu)")
+    ap.add_argument("--trials", type=int, default=5, help="timed regions per number; the median is reported")
+    ap.add_argument("--detail-scale", type=float, default=0.5,
+                    help="timed-region length of the per-config sweep as a fraction of --min-ms (1.0 = the full SURVEY protocol)")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="wall time of the cpu_baseline leg")
+    ap.add_argument("--no-detail", action="store_true", help="skip the per-config sweep (configs[0..4]) and the 8(f) rows")
     ap.add_argument("--pipe-min-n", type=int, default=None,
                     help="vg_set_option(VG_OPT_PIPE_MIN_N): batch size from which the TMA-pipelined kernel runs "
                          "(default: the library's); for A/B runs of the two kernel forms")
@@ -786,6 +1027,8 @@ def main():
     ap.add_argument("--no-pdl", action="store_true", help="vg_set_option(VG_OPT_PDL, 0): launch without programmatic dependent launch")
     ap.add_argument("--profile", action="store_true", help="eager launches of every kernel, for ncu; no timing")
     args = ap.parse_args()
+    if args.impl == "ours" and not args.profile and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(spawn_ranks(args))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -795,8 +1038,6 @@ def main():
     if args.profile:
         run_profile(args)
         return
-    if world != args.gpus and world == 1 and args.gpus > 1:
-        raise SystemExit("bench.py: --gpus %d needs torchrun (one rank per GPU); see the module docstring" % args.gpus)
     run_ours(args, rank, world, local_rank)
 
 
