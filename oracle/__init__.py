@@ -47,6 +47,10 @@ def _load(path):
     lib.orc_boolean_distance.argtypes = [C.c_void_p, C.c_int, _P, _P, _P, _P, _P, _P, C.c_double, C.c_int64, _P]
     lib.orc_all_crossings.restype = C.c_int
     lib.orc_all_crossings.argtypes = [C.c_void_p] + [C.c_double] * 6 + [_P, C.c_int]
+    lib.orc_line_crossings.restype = C.c_int
+    lib.orc_line_crossings.argtypes = [C.c_void_p] + [C.c_double] * 6 + [_P, C.c_int]
+    lib.orc_boolean_events.restype = C.c_int
+    lib.orc_boolean_events.argtypes = [C.c_void_p] + [C.c_double] * 6 + [_P, C.c_int]
     lib.orc_world_create.restype = C.c_void_p
     lib.orc_world_create.argtypes = [C.c_int, C.POINTER(C.c_void_p), _PI, _P]
     lib.orc_world_create_mixed.restype = C.c_void_p
@@ -151,6 +155,12 @@ class Shape:
         n = self._l.orc_all_crossings(self._h, *[float(v) for v in p], *[float(v) for v in d], _ptr(out), out.size)
         return out[:n].copy()
 
+    def line_crossings(self, p, d):
+        """Every crossing of the boundary by the whole line p + t d, t of either sign, ascending (reading R32)."""
+        out = np.empty(512, dtype=np.float64)
+        n = self._l.orc_line_crossings(self._h, *[float(v) for v in p], *[float(v) for v in d], _ptr(out), out.size)
+        return out[:n].copy()
+
 
 class Volume:
     """Mother solid + placed daughters; `xforms` is (nd, 12) row-major [R | b], mother -> local."""
@@ -246,6 +256,12 @@ class Boolean:
 
     def distance_to_out(self, x, y, z, dx, dy, dz, step_max=np.inf):
         return self._dist(1, x, y, z, dx, dy, dz, step_max)
+
+    def events(self, p, d):
+        """Every t (either sign) at which the membership of the boolean flips along the whole line p + t d (R28)."""
+        out = np.empty(8 * 272, dtype=np.float64)
+        n = self._l.orc_boolean_events(self._h, *[float(v) for v in p], *[float(v) for v in d], _ptr(out), out.size)
+        return out[:n].copy()
 
 
 class World:

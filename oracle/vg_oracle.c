@@ -42,8 +42,9 @@
  * to one primitive and the never-over-estimating property of their composed
  * safety (tests/test_oracle_boolean.py), and
  * the 80-bit long-double build of this same file (-DORC_LONG_DOUBLE).
- * Parity unpinned: nothing under readings R1-R21; behaviour INSIDE the
- * kTol surface band (R7) is outside the parity contract.
+ * Start points INSIDE the kTol surface band follow reading R32 (stated above
+ * surface_cross below; pins in tests/test_oracle_surface.py); it replaces R7.
+ * Parity unpinned: nothing under readings R1-R32.
  */
 #include <math.h>
 #include <stdint.h>
@@ -504,18 +505,49 @@ static real cross(const orc_shape *s, int is_inside, const real p[3], const real
     }
 }
 
-/* c.2: DistanceToIn / DistanceToOut (readings R4, R5) */
+/*
+ * Reading R32 (SURVEY.md 8(c) R7 left start points in the surface band undefined; 8(f) f2 asks for them): a particle
+ * whose geometric step won "is transported to the border" and starts its next step ON a surface.
+ *   For a start point of class SURFACE the ray is read as starting on the crossing it sits on: let t_0 < t_1 < ... be
+ *   ALL crossings of the whole line p + t d, t in (-inf, +inf), by the boundary (c.4 without the t > 0 filter, see
+ *   line_crossings below); the solid is bounded, so along the line the even-numbered crossings enter it and the
+ *   odd-numbered leave it.  Let t_s be the crossing nearest to t = 0 (the later one on a tie).
+ *     DistanceToIn  = max(t_s, 0) if t_s is entering, else max(t_{s+1}, 0) (the next entry; +inf if there is none);
+ *     DistanceToOut = max(t_s, 0) if t_s is leaving,  else max(t_{s+1}, 0) (the exit that follows the entry at t_s).
+ *   A line that does not cross the boundary at all (a tangent start in the band): DistanceToIn = +inf, DistanceToOut = 0.
+ * So a surface point moving inward has DistanceToIn 0 and DistanceToOut = its chord; moving outward DistanceToOut 0 and
+ * DistanceToIn = the next entry.  For start points outside the band nothing changes (c.2).
+ */
+static int line_crossings(const orc_shape *s, const real p[3], const real d[3], real *out);
+
+static real surface_cross(const orc_shape *s, const real p[3], const real d[3], int want_leaving)
+{
+    real t[4 * ORC_MAXV + 8];
+    int n = line_crossings(s, p, d, t); /* t[0], t[2], ... enter, t[1], t[3], ... leave */
+    if (n == 0) return want_leaving ? (real)0 : ORC_INF;
+    int k = 0;
+    for (int i = 1; i < n; ++i)
+        if (R_FABS(t[i]) <= R_FABS(t[k])) k = i;
+    int leaving = k & 1;
+    if (leaving != want_leaving) ++k; /* the next crossing has the wanted sense */
+    if (k >= n) return ORC_INF;
+    return rmax2(t[k], 0);
+}
+
+/* c.2: DistanceToIn / DistanceToOut (readings R4, R5; R32 in the surface band) */
 static real distance_to_in(const orc_shape *s, const real p[3], const real d[3], real step_max)
 {
-    if (inside(s, p[0], p[1], p[2]) == ORC_INSIDE) return -1;
-    real t = cross(s, 0, p, d);
+    int cls = inside(s, p[0], p[1], p[2]);
+    if (cls == ORC_INSIDE) return -1;
+    real t = cls == ORC_SURFACE ? surface_cross(s, p, d, 0) : cross(s, 0, p, d);
     return t <= step_max ? t : ORC_INF;
 }
 
 static real distance_to_out(const orc_shape *s, const real p[3], const real d[3], real step_max)
 {
-    if (inside(s, p[0], p[1], p[2]) == ORC_OUTSIDE) return -1;
-    real t = cross(s, 1, p, d);
+    int cls = inside(s, p[0], p[1], p[2]);
+    if (cls == ORC_OUTSIDE) return -1;
+    real t = cls == ORC_SURFACE ? surface_cross(s, p, d, 1) : cross(s, 1, p, d);
     return t <= step_max ? t : ORC_INF;
 }
 
@@ -704,7 +736,7 @@ void orc_volume_safety(const orc_volume *v, const double *x, const double *y, co
 typedef struct orc_boolean_s orc_boolean;
 static int bool_inside(const orc_boolean *c, const real p[3]);
 static real bool_sdf(const orc_boolean *c, const real p[3]);
-static real bool_cross(const orc_boolean *c, const real p[3], const real d[3]);
+static real bool_cross(const orc_boolean *c, int cls, int want_leaving, const real p[3], const real d[3]);
 
 typedef struct {
     int nn;
@@ -727,13 +759,15 @@ static real node_sdf(const orc_world *w, int i, const real p[3])
 static real node_distance_to_in(const orc_world *w, int i, const real p[3], const real d[3])
 {
     if (!w->boolean[i]) return distance_to_in(w->shape[i], p, d, ORC_INF);
-    return bool_inside(w->boolean[i], p) == ORC_INSIDE ? (real)-1 : bool_cross(w->boolean[i], p, d);
+    int cls = bool_inside(w->boolean[i], p);
+    return cls == ORC_INSIDE ? (real)-1 : bool_cross(w->boolean[i], cls, 0, p, d);
 }
 
 static real node_distance_to_out(const orc_world *w, int i, const real p[3], const real d[3])
 {
     if (!w->boolean[i]) return distance_to_out(w->shape[i], p, d, ORC_INF);
-    return bool_inside(w->boolean[i], p) == ORC_OUTSIDE ? (real)-1 : bool_cross(w->boolean[i], p, d);
+    int cls = bool_inside(w->boolean[i], p);
+    return cls == ORC_OUTSIDE ? (real)-1 : bool_cross(w->boolean[i], cls, 1, p, d);
 }
 
 /* exactly one of shapes[i], booleans[i] is given per node (booleans may be NULL: no boolean nodes) */
@@ -871,10 +905,10 @@ void orc_world_safety(const orc_world *w, const int32_t *node, const double *x, 
  *        operation on the closed sets.  Inside(p) combines the two classes: union: INSIDE if either is INSIDE,
  *        OUTSIDE if both are OUTSIDE; intersection: INSIDE if both, OUTSIDE if either is OUTSIDE; subtraction:
  *        INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A OUTSIDE or B INSIDE; SURFACE otherwise.
- *   R28  Distances: along the ray each solid is a union of intervals bounded by its crossings (ALL crossings of
- *        c.4, not only the first); C's membership along the ray is the set operation on the two interval sets;
- *        DistanceToIn / DistanceToOut is the first t > 0 at which C's membership differs from its value at the
- *        start point (strict membership of A and B at p, R6), +inf if it never does; -1 on the wrong side as R4.
+ *   R28  Distances: along the WHOLE line each solid is a union of intervals bounded by its crossings (ALL crossings of
+ *        c.4, not only the first, t of either sign); C's membership along the line is the set operation on the two
+ *        interval sets (outside both far behind the start point); DistanceToIn / DistanceToOut is the first t > 0 at
+ *        which C's membership flips, +inf if it never does; -1 on the wrong side as R4; R32 for a start of class SURFACE.
  *   R29  Safeties: the usual composition sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB).  This is
  *        NOT the exact distance of R2: it never over-estimates the distance to the surface of C, is exact where
  *        only one operand matters, and has the sign of the membership (pinned as such).
@@ -922,8 +956,9 @@ void orc_boolean_destroy(orc_boolean *c) { free(c); }
 
 #define ORC_MAXX (4 * ORC_MAXV + 8)
 
-/* every crossing t > 0 of the boundary of one solid by the ray, ascending (c.4 with "collect" in place of "min") */
-static int all_crossings(const orc_shape *s, const real p[3], const real d[3], real *out)
+/* every crossing of the boundary of one solid by the ray, ascending (c.4 with "collect" in place of "min"):
+ * whole = 0: the crossings t > 0; whole = 1: those of the whole line, t of either sign (R32, R28) */
+static int crossings(const orc_shape *s, const real p[3], const real d[3], real *out, int whole)
 {
     int n = 0;
     if (s->kind == ORC_BOX || s->kind == ORC_TRD) { /* convex: the interval [tin, tout] of the clip */
@@ -949,8 +984,8 @@ static int all_crossings(const orc_shape *s, const real p[3], const real d[3], r
             }
         }
         if (!(tin < tout)) return 0;
-        if (tin > 0) out[n++] = tin;
-        if (tout > 0) out[n++] = tout;
+        if (whole || tin > 0) out[n++] = tin;
+        if (whole || tout > 0) out[n++] = tout;
         return n;
     }
     if (s->kind == ORC_ORB) {
@@ -959,7 +994,7 @@ static int all_crossings(const orc_shape *s, const real p[3], const real d[3], r
         real c = p[0] * p[0] + p[1] * p[1] + p[2] * p[2] - s->r * s->r;
         int m = quad_roots(1, b, c, t);
         for (int i = 0; i < m; ++i)
-            if (t[i] > 0) out[n++] = t[i];
+            if (whole || t[i] > 0) out[n++] = t[i];
     } else { /* RZ polygon + phi wedge: the candidate loops of cross_rz */
         real x = p[0], y = p[1], z = p[2], dx = d[0], dy = d[1], dz = d[2];
         for (int i = 0; i < s->nv; ++i) {
@@ -971,7 +1006,7 @@ static int all_crossings(const orc_shape *s, const real p[3], const real d[3], r
                 real t[2];
                 int m = quad_roots(dx * dx + dy * dy - B * B * dz * dz, x * dx + y * dy - B * dz * k, x * x + y * y - k * k, t);
                 for (int q = 0; q < m; ++q) {
-                    if (!(t[q] > 0)) continue;
+                    if (!whole && !(t[q] > 0)) continue;
                     real zh = z + t[q] * dz;
                     if (zh < rmin2(z0, z1) || zh > rmax2(z0, z1)) continue;
                     if (!in_phi(s, x + t[q] * dx, y + t[q] * dy)) continue;
@@ -979,7 +1014,7 @@ static int all_crossings(const orc_shape *s, const real p[3], const real d[3], r
                 }
             } else if (dz != 0) {
                 real t = (z0 - z) / dz;
-                if (!(t > 0)) continue;
+                if (!whole && !(t > 0)) continue;
                 real hx = x + t * dx, hy = y + t * dy, rh2 = hx * hx + hy * hy;
                 real rlo = rmin2(r0, r1), rhi = rmax2(r0, r1);
                 if (rh2 < rlo * rlo || rh2 > rhi * rhi) continue;
@@ -993,7 +1028,7 @@ static int all_crossings(const orc_shape *s, const real p[3], const real d[3], r
                 real nd = nx * dx + ny * dy;
                 if (nd == 0) continue;
                 real t = -(nx * x + ny * y) / nd;
-                if (!(t > 0)) continue;
+                if (!whole && !(t > 0)) continue;
                 real hx = x + t * dx, hy = y + t * dy;
                 if (!in_poly(s, ex * hx + ey * hy, z + t * dz)) continue;
                 out[n++] = t;
@@ -1007,6 +1042,33 @@ static int all_crossings(const orc_shape *s, const real p[3], const real d[3], r
         out[j + 1] = v;
     }
     return n;
+}
+
+static int all_crossings(const orc_shape *s, const real p[3], const real d[3], real *out) { return crossings(s, p, d, out, 0); }
+
+/* The crossings of the WHOLE line at which the membership of the solid really flips, ascending (R32, R28).  The patch
+ * loops above deliver every intersection with a boundary patch; a line through an edge of the solid meets two patches
+ * at one point, and one that clips an edge by less than the tolerance meets them within kTol of each other, so raw
+ * values within kTol of the first of their cluster are ONE candidate.  A candidate is a crossing iff the sign of the
+ * exact sdf differs between the midpoints of the gaps before and after it (outside before the first candidate and
+ * after the last: the solid is bounded).  So out[0], out[2], ... enter the solid and out[1], out[3], ... leave it. */
+static int line_crossings(const orc_shape *s, const real p[3], const real d[3], real *out)
+{
+    real raw[ORC_MAXX], c[ORC_MAXX];
+    int n = crossings(s, p, d, raw, 1), m = 0, k = 0;
+    for (int i = 0; i < n; ++i)
+        if (m == 0 || raw[i] - c[m - 1] > ORC_KTOL) c[m++] = raw[i];
+    int prev_in = 0;
+    for (int j = 0; j < m; ++j) {
+        int next_in = 0;
+        if (j + 1 < m) {
+            real tm = (c[j] + c[j + 1]) / 2;
+            next_in = sdf(s, p[0] + tm * d[0], p[1] + tm * d[1], p[2] + tm * d[2]) < 0;
+        }
+        if (next_in != prev_in) out[k++] = c[j];
+        prev_in = next_in;
+    }
+    return k;
 }
 
 static int bool_member(int op, int ina, int inb)
@@ -1029,10 +1091,10 @@ static real operand_sdf(const orc_shape *s, const orc_boolean *c, const real p[3
 
 static int bool_events(const orc_boolean *c, const real p[3], const real d[3], real *out);
 
-/* every t > 0 at which the operand's membership flips along the ray, ascending */
+/* every t (either sign) at which the operand's membership flips along the whole line, ascending */
 static int operand_events(const orc_shape *s, const orc_boolean *c, const real p[3], const real d[3], real *out)
 {
-    return s ? all_crossings(s, p, d, out) : bool_events(c, p, d, out);
+    return s ? line_crossings(s, p, d, out) : bool_events(c, p, d, out);
 }
 
 /* R27 */
@@ -1060,15 +1122,17 @@ static real bool_sdf(const orc_boolean *c, const real p[3])
     return rmax2(sa, -sb);
 }
 
-/* R28: every t > 0 at which the membership of C along the ray flips (merge of the operands' flips, a tie goes to A) */
+/* R28: every t, of either sign, at which the membership of C along the WHOLE line flips, ascending: the merge of the
+ * operands' flips (a tie goes to A).  Both operands are bounded, so far behind the start point the line is outside
+ * both and the memberships are counted on from there; no class of the start point enters (a start point in the
+ * surface band of an operand would make that class ambiguous). */
 static int bool_events(const orc_boolean *c, const real p[3], const real d[3], real *out)
 {
     real pb[3], db[3];
     real *ta = (real *)malloc(sizeof(real) * 2 * ORC_MAXLEAF * ORC_MAXX), *tb = ta + ORC_MAXLEAF * ORC_MAXX;
     to_local(c->xf, p, d, pb, db);
     int na = operand_events(c->a, c->ca, p, d, ta), nb = operand_events(c->b, c->cb, pb, db, tb);
-    int ina = operand_inside(c->a, c->ca, p) == ORC_INSIDE, inb = operand_inside(c->b, c->cb, pb) == ORC_INSIDE;
-    int cur = bool_member(c->op, ina, inb);
+    int ina = 0, inb = 0, cur = 0;
     int i = 0, j = 0, n = 0;
     while (i < na || j < nb) {
         real t;
@@ -1081,14 +1145,27 @@ static int bool_events(const orc_boolean *c, const real p[3], const real d[3], r
     return n;
 }
 
-/* R28: the first of them */
-static real bool_cross(const orc_boolean *c, const real p[3], const real d[3])
+/* R28: the first flip ahead of a start point of class INSIDE or OUTSIDE; R32 (read with "crossing" = flip of C's
+ * membership) for a start point of class SURFACE: want_leaving = 0 DistanceToIn, 1 DistanceToOut */
+static real bool_cross(const orc_boolean *c, int cls, int want_leaving, const real p[3], const real d[3])
 {
     real *t = (real *)malloc(sizeof(real) * ORC_MAXLEAF * ORC_MAXX);
     int n = bool_events(c, p, d, t);
-    real first = n > 0 ? t[0] : ORC_INF;
+    real r = ORC_INF;
+    if (cls != ORC_SURFACE) {
+        for (int i = 0; i < n; ++i)
+            if (t[i] > 0) { r = t[i]; break; }
+    } else if (n == 0) {
+        r = want_leaving ? (real)0 : ORC_INF;
+    } else {
+        int k = 0;
+        for (int i = 1; i < n; ++i)
+            if (R_FABS(t[i]) <= R_FABS(t[k])) k = i;
+        if ((k & 1) != want_leaving) ++k;
+        if (k < n) r = rmax2(t[k], 0);
+    }
     free(t);
-    return first;
+    return r;
 }
 
 void orc_boolean_inside(const orc_boolean *c, const double *x, const double *y, const double *z, int64_t n, int32_t *out)
@@ -1118,7 +1195,7 @@ void orc_boolean_distance(const orc_boolean *c, int which, const double *x, cons
         real p[3] = { x[i], y[i], z[i] }, d[3] = { dx[i], dy[i], dz[i] };
         int cls = bool_inside(c, p);
         if ((which == 0 && cls == ORC_INSIDE) || (which == 1 && cls == ORC_OUTSIDE)) { out[i] = -1; continue; }
-        real t = bool_cross(c, p, d);
+        real t = bool_cross(c, cls, which, p, d);
         out[i] = (double)(t <= step_max ? t : ORC_INF);
     }
 }
@@ -1129,5 +1206,25 @@ int orc_all_crossings(const orc_shape *s, double x, double y, double z, double d
     real p[3] = { x, y, z }, d[3] = { dx, dy, dz }, t[ORC_MAXX];
     int n = all_crossings(s, p, d, t);
     for (int i = 0; i < n && i < max; ++i) out[i] = (double)t[i];
+    return n;
+}
+
+/* the crossings of the whole line (t of either sign, R32), exposed for the pins */
+int orc_line_crossings(const orc_shape *s, double x, double y, double z, double dx, double dy, double dz, double *out, int max)
+{
+    real p[3] = { x, y, z }, d[3] = { dx, dy, dz }, t[ORC_MAXX];
+    int n = line_crossings(s, p, d, t);
+    for (int i = 0; i < n && i < max; ++i) out[i] = (double)t[i];
+    return n;
+}
+
+/* the membership flips of a boolean along the whole line (R28), exposed for the pins */
+int orc_boolean_events(const orc_boolean *c, double x, double y, double z, double dx, double dy, double dz, double *out, int max)
+{
+    real p[3] = { x, y, z }, d[3] = { dx, dy, dz };
+    real *t = (real *)malloc(sizeof(real) * ORC_MAXLEAF * ORC_MAXX);
+    int n = bool_events(c, p, d, t);
+    for (int i = 0; i < n && i < max; ++i) out[i] = (double)t[i];
+    free(t);
     return n;
 }

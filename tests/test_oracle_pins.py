@@ -52,8 +52,8 @@ def tracks_for(name, n, seed=11):
 
 # ------------------------------------------------------------------ worked examples (golden file)
 
-def _parse_golden():
-    path = os.path.join(os.path.dirname(__file__), "golden", "worked_examples.txt")
+def _parse_golden(name="worked_examples.txt"):
+    path = os.path.join(os.path.dirname(__file__), "golden", name)
     names = {"box": O.BOX, "orb": O.ORB, "tube": O.TUBE, "cone": O.CONE, "trd": O.TRD}
     val = lambda t: {"4PI3": 4 * PI / 3, "2PI": 2 * PI, "inf": math.inf}.get(t, None) if t in ("4PI3", "2PI", "inf") else float(t)
     rows = []
