@@ -11,13 +11,21 @@
  * competes with the physics step; "coordinate transformations and distance calculations")
  *                                                                                      -> vg_compute_step.
  * The paper defines no solid and no formula; the exact meaning of every query is the reading
- * R1-R21 of SURVEY.md sec. 8(c), restated in DESIGN.md sec. 3 together with R22-R31 (the tree of volumes
- * vg_world_*, polycone z steps, boolean solids and CSG trees vg_boolean_create).  In one line each:
+ * R1-R21 of SURVEY.md sec. 8(c), restated in DESIGN.md sec. 3 together with R22-R32 (the tree of volumes
+ * vg_world_*, polycone z steps, boolean solids and CSG trees vg_boolean_create, start points on a surface).
+ * In one line each:
  *   Inside        VG_INSIDE if sdf(p) < -kTol, VG_OUTSIDE if sdf(p) > +kTol, else VG_SURFACE (kTol = 1e-9)
  *   SafetyToIn    +sdf(p), SafetyToOut  -sdf(p): exact signed Euclidean distance to the surface (for a
  *                 boolean: the composed bound of R29, which never over-estimates it)
  *   DistanceToIn  -1 if p is inside; else the first t > 0 with p + t d on the surface; +inf if none or > step_max
  *   DistanceToOut -1 if p is outside; else likewise
+ *   ... from a start point of class VG_SURFACE (R32; a particle "transported to the border" starts its
+ *                 next step there): the ray starts ON the crossing it sits on -- moving inward DistanceToIn = 0 and
+ *                 DistanceToOut = the chord to the exit; moving outward DistanceToOut = 0 and DistanceToIn = the
+ *                 next entry (+inf for a convex solid).  Every distance returned is -1, >= 0 or +inf.  The kernels
+ *                 count a crossing of the wanted sense as lying at the start when its ray parameter is > -5e-7
+ *                 (VG_KRAYTOL) and clamp at 0: exact for a band point unless the ray grazes the surface it sits on
+ *                 at |n.d| < 2e-3 or another surface lies within 1e-6.
  *   ComputeStep   lexicographic min of (distance, index) over the mother's DistanceToOut (index -1) and every
  *                 daughter's DistanceToIn in its local frame p_i = R_i p + b_i, d_i = R_i d; (step_max, -2)
  *                 if the physics step step_max is shorter.
@@ -66,6 +74,7 @@ typedef enum {
 } vg_status;
 
 #define VG_KTOLERANCE 1e-9   /* BASELINE.json: kTolerance; half-width of the surface band (R6)        */
+#define VG_KRAYTOL 5e-7      /* R32: a crossing this little behind the start point lies AT it         */
 #define VG_MAX_ZPLANES 32    /* polycone                                                              */
 #define VG_MAX_DAUGHTERS 256 /* per volume                                                            */
 #define VG_HIT_MOTHER (-1)   /* vg_compute_step: the mother's boundary limits the step                */
@@ -104,8 +113,10 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  *   Inside       combines the operands' classes: union INSIDE if either is, OUTSIDE if both are; intersection INSIDE if
  *                both are, OUTSIDE if either is; subtraction (A minus B) INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A
  *                OUTSIDE or B INSIDE; SURFACE otherwise (R27);
- *   distances    the first t > 0 at which the membership of C along the ray differs from its value at the start point,
- *                +inf if none, -1 on the wrong side (R28);
+ *   distances    the first t > 0 at which the membership of C along the ray flips, +inf if none, -1 on the wrong side
+ *                (R28; the operands' memberships follow from their crossings along the whole line, so a start point on
+ *                an operand's surface that is hidden inside the other operand is an ordinary inside point of C); R32
+ *                from a start point of class SURFACE;
  *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
  *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
  *                safeties it is not the exact distance everywhere (R29).

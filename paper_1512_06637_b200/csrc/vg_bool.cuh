@@ -10,7 +10,9 @@ namespace vg {
 constexpr int kBoolBlock = 128;
 constexpr int kBoolMaxEvents = 64; // an operand has at most ~10 crossings with a line; the loop ends long before
 
-// next crossing of the operand's boundary at t > 0 in the given sense (leaving: the track is inside it), +inf if none.
+// next crossing of the operand's boundary in the given sense (leaving: the track is inside it) that lies ahead of the
+// point or at it (R32: t > -kRayTol, clamped at 0), +inf if none.  The crossing is picked by its SENSE, so the one just
+// taken (the point sits on it to rounding) is never taken again: it has the other sense now.
 // K = the operand's kind at compile time (the distance kernels are instantiated per pair of kinds: straight-line code,
 // no divergence between lanes over the kind), or -1 to read it from the record.
 template <int K>
@@ -30,19 +32,16 @@ VG_DEV double solid_next(const SolidU &s, bool inside, double x, double y, doubl
         t = inside ? tout : ((tin < tout) ? tin : inf());
         break;
     }
-    case kOrb: { // a = 1: the entering root is the smaller one, the leaving root the larger
+    case kOrb: { // a = 1: the entering root is -b - s, the leaving root -b + s
         const double pp = fma(x, x, fma(y, y, z * z)), b = fma(x, dx, fma(y, dy, z * dz));
         const double c = pp - s.u.orb.r2, D = fma(b, b, -c);
-        const double sq = sqrt_pos(D);
-        const double q = -(b + copysign_bits(sq, b));
-        const double t1 = q, t2 = c * rcp(q);
-        t = D > 0.0 ? (inside ? dmax(t1, t2) : dmin(t1, t2)) : inf();
+        t = D > 0.0 ? quad_root(1.0, b, c, sqrt_pos(D), inside) : inf();
         break;
     }
     case kTube: t = inside ? Tube::dist_out(s.u.tube, x, y, z, dx, dy, dz) : Tube::dist_in(s.u.tube, x, y, z, dx, dy, dz); break;
     default: t = inside ? Cone::dist_out(s.u.cone, x, y, z, dx, dy, dz) : Cone::dist_in(s.u.cone, x, y, z, dx, dy, dz); break;
     }
-    return t > 0.0 ? t : inf(); // a crossing behind the point, a wrong-side -1 or a NaN is "no crossing"
+    return ahead(t) ? dmax(t, 0.0) : inf(); // a crossing behind the point, a wrong-side -1 or a NaN is "no crossing"
 }
 
 VG_DEV bool bool_member(int op, bool ina, bool inb)
@@ -85,7 +84,14 @@ VG_DEV double bool_sdf_pt(const BoolP &p, double x, double y, double z) // R29
     return p.op == kUnion ? dmin(sa, sb) : (p.op == kIntersection ? dmax(sa, sb) : dmax(sa, -sb));
 }
 
-// R28: DistanceToIn (to_out = false) or DistanceToOut (true): -1 on the wrong side, +inf if the membership never changes
+// R28 / R32: DistanceToIn (to_out = false) or DistanceToOut (true): -1 on the wrong side, +inf if the membership never
+// changes.  A state machine over (inside A, inside B, t): each operand is asked for its next crossing in the sense its
+// state calls for, the nearer one is taken and flips that state; the answer is the first event after which C's
+// membership is what the query looks for (a member for DistanceToIn, a non-member for DistanceToOut -- the class test
+// has already sent the wrong side home, so the start value need not be read off the operands).  An operand whose class
+// at the start is SURFACE has no state yet: it starts as "outside", and if its entering crossing is not AT the start
+// (t <= kRayTol after the clamp) the crossing the point sits on is a leaving one and the operand was inside (R32: the
+// sense of motion decides); that operand's event at t ~ 0 then runs through the loop like any other.
 template <int KA, int KB>
 VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, double z, double dx, double dy, double dz)
 {
@@ -99,19 +105,26 @@ VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, dou
     const double bdy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
     const double bdz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
     bool ina = ca == cInside, inb = cb == cInside;
-    const bool start = bool_member(p.op, ina, inb);
+    bool pend_a = ca == cSurface, pend_b = cb == cSurface;
     double tt = 0.0;
 #pragma unroll 1
     for (int it = 0; it < kBoolMaxEvents; ++it) {
         const double ea = solid_next<KA>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
         const double eb = solid_next<KB>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
+        if (pend_a || pend_b) { // first pass only, and only for a start on an operand's surface
+            const bool fix_a = pend_a && !(ea <= kRayTol), fix_b = pend_b && !(eb <= kRayTol);
+            pend_a = pend_b = false;
+            ina = ina || fix_a;
+            inb = inb || fix_b;
+            if (fix_a || fix_b) continue;
+        }
         const bool a_first = ea <= eb; // a tie goes to A, as in the oracle's merge
         const double e = a_first ? ea : eb;
         if (!(e < inf())) break;
         tt += e;
         ina = a_first ? !ina : ina;
         inb = a_first ? inb : !inb;
-        if (bool_member(p.op, ina, inb) != start) return tt;
+        if (bool_member(p.op, ina, inb) != to_out) return tt;
     }
     return inf();
 }

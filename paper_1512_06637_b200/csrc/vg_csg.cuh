@@ -98,7 +98,8 @@ VG_DEV double csg_sdf(const CsgP &p, double x, double y, double z)
     return st[0];
 }
 
-// R28 read recursively
+// R28 / R32 read recursively: the state machine of bool_distance over one "inside" bit per primitive; primitives whose
+// class at the start is SURFACE get their bit from the sense of motion in the first pass
 VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, double z, double dx, double dy, double dz)
 {
     unsigned in, out;
@@ -106,12 +107,13 @@ VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, doubl
     const int cls = csg_classify(p, in, out);
     if ((!to_out && cls == cInside) || (to_out && cls == cOutside)) return -1.0;
     unsigned bits = in;
-    const bool start = csg_member(p, bits);
+    unsigned pend = ~(in | out) & ((1u << p.nleaf) - 1u);
     double tt = 0.0;
 #pragma unroll 1
     for (int it = 0; it < kCsgMaxEvents; ++it) {
         double emin = inf();
         int imin = -1;
+        unsigned fix = 0;
         const double px = fma(tt, dx, x), py = fma(tt, dy, y), pz = fma(tt, dz, z);
 #pragma unroll 1
         for (int i = 0; i < p.nleaf; ++i) {
@@ -122,12 +124,18 @@ VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, doubl
             const double ldy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
             const double ldz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
             const double e = solid_next<-1>(p.leaf[i], (bits >> i) & 1u, lx, ly, lz, ldx, ldy, ldz);
+            fix |= unsigned(((pend >> i) & 1u) && !(e <= kRayTol)) << i;
             if (e < emin) emin = e, imin = i; // strict: the lowest leaf wins a tie
+        }
+        pend = 0;
+        if (fix) { // those primitives are being left, not entered: they were inside
+            bits |= fix;
+            continue;
         }
         if (imin < 0) break;
         tt += emin;
         bits ^= 1u << imin;
-        if (csg_member(p, bits) != start) return tt;
+        if (csg_member(p, bits) != to_out) return tt;
     }
     return inf();
 }

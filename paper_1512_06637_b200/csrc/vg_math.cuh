@@ -14,12 +14,21 @@ namespace vg {
 
 constexpr double kTol = 1e-9;   // BASELINE.json kTolerance, SURVEY.md 8(c) R6
 constexpr double kTiny = 1e-300; // stands in for an exactly-zero direction component / denominator
+// Reading R32 ("transported to the border"): a start point in the surface band is read as
+// starting ON the crossing it sits on.  The kernels take every crossing of the wanted sense with t > -kRayTol and clamp
+// the result at 0.  For a start point >= 1e-6 from every surface (the parity generators) no crossing lies within 1e-6
+// of t = 0, so nothing changes there; for a band point the crossing it sits on is within kTol / |n.d| <= kRayTol of
+// t = 0 unless the ray grazes the surface at |n.d| < 2e-3.
+constexpr double kRayTol = 5e-7;
 
 #define VG_DEV __device__ __forceinline__
 
 VG_DEV double inf() { return __longlong_as_double(0x7ff0000000000000LL); }
 
 VG_DEV double sel(bool c, double a, double b) { return c ? a : b; }
+
+// R32: is a crossing at ray parameter t ahead of, or at, the start point?  (NaN: no)
+VG_DEV bool ahead(double t) { return t > -kRayTol; }
 
 // max / min that compile to one DSETP + selects; NaN in `b` keeps `a`
 VG_DEV double dmax(double a, double b) { return b > a ? b : a; }

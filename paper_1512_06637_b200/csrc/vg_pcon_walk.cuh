@@ -85,7 +85,7 @@ VG_DEV double pcon_step_enter(const PolyconeP &p, int k, const RayRZ &r, double 
     const bool up = dz > 0.0;
     const bool on_o = rh2 >= st.olo * st.olo && rh2 <= st.ohi * st.ohi && st.ohi > st.olo && (st.oup != 0) != up;
     const bool on_i = rh2 >= st.ilo * st.ilo && rh2 <= st.ihi * st.ihi && st.ihi > st.ilo && (st.iup != 0) != up;
-    return (t > 0.0 && (on_o || on_i)) ? t : inf();
+    return (ahead(t) && (on_o || on_i)) ? t : inf();
 }
 
 // squared distance from (u, v) to the horizontal edges of step k (the running minimum d2 goes in and comes out)
@@ -172,7 +172,7 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
     const double tc = up ? ta : tb;
     const double rc2 = fma(tc, fma(tc, a, b + b), r.rho2);
     const double clo = up ? p.cap_lo_rmin : p.cap_hi_rmin, chi = up ? p.cap_lo_rmax : p.cap_hi_rmax;
-    const bool beyond = up ? z < p.zlo : z > p.zhi;
+    const bool beyond = ahead(tc); // beyond the end plane, or on it (R32); NaN for a horizontal ray
     bool cap_hit = beyond && !horizontal && rc2 >= clo * clo && rc2 <= chi * chi;
     if (WEDGE) cap_hit = cap_hit && wedge_member_at<kWmRuntime>(p.w, ep, ed, tc);
 
@@ -212,18 +212,18 @@ VG_DEV double pcon_walk_dist_in(const PolyconeP &p, const PconWalkSec *tab, doub
     if (WEDGE) { // the two phi faces, entering sense; the hit point must lie in the (r, z) outline (R1: closed)
         {
             const double t = -ep.c0 * rcp(ed.c0);
-            const bool ok = ed.c0 > 0.0 && t > 0.0 && t < best &&
+            const bool ok = ed.c0 > 0.0 && ahead(t) && t < best &&
                             pcon_in_outline(p, tab, fma(t, ed.u0, ep.u0), fma(t, dz, z));
             best = ok ? t : best;
         }
         {
             const double t = -ep.c1 * rcp(ed.c1);
-            const bool ok = ed.c1 > 0.0 && t > 0.0 && t < best &&
+            const bool ok = ed.c1 > 0.0 && ahead(t) && t < best &&
                             pcon_in_outline(p, tab, fma(t, ed.u1, ep.u1), fma(t, dz, z));
             best = ok ? t : best;
         }
     }
-    return in ? -1.0 : best;
+    return in ? -1.0 : dmax(best, 0.0);
 }
 
 // exact signed distance of the full-phi polycone; same segments as PolyconeT::safety
@@ -433,7 +433,7 @@ VG_DEV double pcon_step_leave(const PolyconeP &p, int k, const RayRZ &r, double 
     const bool up = dz > 0.0;
     const bool on_o = rh2 >= st.olo * st.olo && rh2 <= st.ohi * st.ohi && st.ohi > st.olo && (st.oup != 0) == up;
     const bool on_i = rh2 >= st.ilo * st.ilo && rh2 <= st.ihi * st.ihi && st.ihi > st.ilo && (st.iup != 0) == up;
-    return (t > 0.0 && (on_o || on_i)) ? t : inf();
+    return (ahead(t) && (on_o || on_i)) ? t : inf();
 }
 
 // DistanceToOut: from the point's own section the ray stays in the material until it leaves through a patch of the
@@ -458,6 +458,12 @@ VG_DEV double pcon_walk_dist_out(const PolyconeP &p, const PconWalkSec *tab, dou
     int k = pcon_section_of(p, z);
     double best = inf();
     bool go = !out;
+    if (go && p.step_mask) { // a start ON a step face (R32): the plane just behind the point's section, leaving sense, t ~ 0
+        const double tb = pcon_step_leave(p, up ? k - 1 : k, r, z, dz, idz);
+        const bool okb = tb < inf() && (!WEDGE || wedge_member_at<kWmRuntime>(p.w, ep, ed, tb));
+        best = okb ? tb : best;
+        go = !okb;
+    }
     while (go) {
         const PconWalkSec w = tab[k];
         Frustum f;
@@ -478,7 +484,7 @@ VG_DEV double pcon_walk_dist_out(const PolyconeP &p, const PconWalkSec *tab, dou
         const int kn = k + step;
         if (kn < 0 || kn >= p.nsec) { // the end cap
             const double tc = ((up ? p.zhi : p.zlo) - z) * idz;
-            const bool okc = tc > 0.0 && (!WEDGE || wedge_member_at<kWmRuntime>(p.w, ep, ed, tc));
+            const bool okc = ahead(tc) && (!WEDGE || wedge_member_at<kWmRuntime>(p.w, ep, ed, tc));
             best = okc ? tc : best;
             break;
         }
@@ -493,16 +499,16 @@ VG_DEV double pcon_walk_dist_out(const PolyconeP &p, const PconWalkSec *tab, dou
     if (WEDGE && !out) { // the phi faces in the leaving sense
         {
             const double t = -ep.c0 * rcp(ed.c0);
-            const bool ok = ed.c0 < 0.0 && t > 0.0 && t < best && pcon_in_outline(p, tab, fma(t, ed.u0, ep.u0), fma(t, dz, z));
+            const bool ok = ed.c0 < 0.0 && ahead(t) && t < best && pcon_in_outline(p, tab, fma(t, ed.u0, ep.u0), fma(t, dz, z));
             best = ok ? t : best;
         }
         {
             const double t = -ep.c1 * rcp(ed.c1);
-            const bool ok = ed.c1 < 0.0 && t > 0.0 && t < best && pcon_in_outline(p, tab, fma(t, ed.u1, ep.u1), fma(t, dz, z));
+            const bool ok = ed.c1 < 0.0 && ahead(t) && t < best && pcon_in_outline(p, tab, fma(t, ed.u1, ep.u1), fma(t, dz, z));
             best = ok ? t : best;
         }
     }
-    return out ? -1.0 : best;
+    return out ? -1.0 : dmax(best, 0.0);
 }
 
 template <int Q, bool GRID, bool WEDGE>

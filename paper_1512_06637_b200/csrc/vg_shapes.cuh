@@ -11,7 +11,10 @@
 //     replaced by +-1e-300 so that no 0/0 or inf-inf can arise (R9, hard part H4);
 //   * `valid` flags are conjunctions of positive comparisons, so a NaN candidate is always discarded.
 // Inside uses per-surface tolerance tests (an L-infinity band); it equals the oracle's Euclidean band except
-// for points within [kTol, sqrt(3) kTol] of an edge, which the parity contract excludes (R6, R7).
+// for points within [kTol, sqrt(3) kTol] of an edge, which the parity contract excludes (R6).
+// Start points in the surface band (R32): a crossing of the wanted sense counts when ahead(t) (t > -kRayTol) and every
+// distance is clamped at 0, so a surface point moving inward has DistanceToIn 0 and DistanceToOut = its chord, and
+// one moving outward DistanceToOut 0 and DistanceToIn = the next entry.
 #pragma once
 #include "vg_math.cuh"
 #include "vg_params.h"
@@ -144,7 +147,7 @@ struct Box {
         double m, s2, tin, tout;
         slack(p, x, y, z, m, s2);
         slabs(p, x, y, z, dx, dy, dz, tin, tout);
-        double t = (tin < tout && tout > 0.0) ? tin : inf();
+        double t = (tin < tout && ahead(tin)) ? dmax(tin, 0.0) : inf(); // an outside point with tin < tout has tin > 0
         return m < -kTol ? -1.0 : t;
     }
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
@@ -152,7 +155,7 @@ struct Box {
         double m, s2, tin, tout;
         slack(p, x, y, z, m, s2);
         slabs(p, x, y, z, dx, dy, dz, tin, tout);
-        return s2 > kTol * kTol ? -1.0 : tout;
+        return s2 > kTol * kTol ? -1.0 : dmax(tout, 0.0);
     }
 };
 
@@ -171,30 +174,28 @@ struct Orb {
         double pp = fma(x, x, fma(y, y, z * z));
         return sqrt_nn(pp) - p.r;
     }
-    // c.4: a = 1, b = p.d, c = p.p - r^2; smallest root > 0
-    VG_DEV static double first_root(const P &p, double pp, double b)
+    // c.4: a = 1, b = p.d, c = p.p - r^2.  The crossing is picked by its SENSE, not as the smallest positive root: the
+    // entering root is -b - s, the leaving root -b + s (evaluated as q or c/q, whichever does not cancel), so a track that
+    // sits on the sphere to rounding sees the crossing it sits on only in the query whose sense it has (R32).
+    VG_DEV static double root(const P &p, double pp, double b, bool leaving)
     {
         double c = pp - p.r2;
         double D = fma(b, b, -c);
-        double s = sqrt_pos(D);
-        double q = -(b + copysign_bits(s, b));
-        double t1 = q, t2 = c * rcp(q);
-        double lo = dmin(t1, t2), hi = dmax(t1, t2);
-        double t = lo > 0.0 ? lo : (hi > 0.0 ? hi : inf());
-        return D > 0.0 ? t : inf();
+        double t = quad_root(1.0, b, c, sqrt_pos(D), leaving);
+        return (D > 0.0 && ahead(t)) ? dmax(t, 0.0) : inf();
     }
     VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {
         double pp = fma(x, x, fma(y, y, z * z));
         double b = fma(x, dx, fma(y, dy, z * dz));
-        double t = first_root(p, pp, b);
+        double t = root(p, pp, b, false);
         return pp < p.rin2 ? -1.0 : t;
     }
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {
         double pp = fma(x, x, fma(y, y, z * z));
         double b = fma(x, dx, fma(y, dy, z * dz));
-        double t = first_root(p, pp, b);
+        double t = root(p, pp, b, true);
         return pp > p.rout2 ? -1.0 : t;
     }
 };
@@ -276,7 +277,7 @@ template <int F> struct TubeT {
         {
             double D = fma(b, b, -a * (rho2 - p.rmax2));
             double t = (-b - sqrt_pos(D)) * inv_a;
-            bool ok = D > 0.0 && t > 0.0 && fabs(fma(t, dz, z)) <= p.dz;
+            bool ok = D > 0.0 && ahead(t) && fabs(fma(t, dz, z)) <= p.dz;
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = ok ? t : best;
         }
@@ -284,36 +285,35 @@ template <int F> struct TubeT {
         if (hollow(p)) {
             double D = fma(b, b, -a * (rho2 - p.rmin2));
             double t = (sqrt_pos(D) - b) * inv_a;
-            bool ok = D > 0.0 && t > 0.0 && fabs(fma(t, dz, z)) <= p.dz;
+            bool ok = D > 0.0 && ahead(t) && fabs(fma(t, dz, z)) <= p.dz;
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
-        // the cap the ray moves towards, only from beyond it (then t > 0 by construction);
-        // rho_hit^2 = rho^2 + 2 b t + a t^2
+        // the cap the ray moves towards, from beyond it or from on it (R32); rho_hit^2 = rho^2 + 2 b t + a t^2
         {
             double az = fabs(z);
             double t = (az - p.dz) * rcp(fabs(dz));
             double rh2 = fma(t, fma(t, a, b + b), rho2);
-            bool ok = az > p.dz && sign_differs(z, dz) && rh2 >= p.rmin2 && rh2 <= p.rmax2;
+            bool ok = ahead(t) && sign_differs(z, dz) && rh2 >= p.rmin2 && rh2 <= p.rmax2;
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
-        // phi faces, entering sense: c_k(p) < 0 and c_k(d) > 0 (then t > 0 by construction)
+        // phi faces, entering sense: c_k(d) > 0, from behind the plane or from on it (R32)
         if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 double uh = fma(t, ed.u0, ep.u0);
-                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(fma(t, dz, z)) <= p.dz;
+                bool ok = ed.c0 > 0.0 && ahead(t) && uh >= p.rmin && uh <= p.rmax && fabs(fma(t, dz, z)) <= p.dz;
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
                 double uh = fma(t, ed.u1, ep.u1);
-                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && uh >= p.rmin && uh <= p.rmax && fabs(fma(t, dz, z)) <= p.dz;
+                bool ok = ed.c1 > 0.0 && ahead(t) && uh >= p.rmin && uh <= p.rmax && fabs(fma(t, dz, z)) <= p.dz;
                 best = (ok && t < best) ? t : best;
             }
         }
-        return in ? -1.0 : best;
+        return in ? -1.0 : dmax(best, 0.0);
     }
 
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
@@ -330,30 +330,30 @@ template <int F> struct TubeT {
         {
             double D = fma(b, b, -a * (rho2 - p.rmax2));
             double t = (sqrt_pos(D) - b) * inv_a;
-            best = (D > 0.0 && t > 0.0) ? t : best;
+            best = (D > 0.0 && ahead(t)) ? t : best;
         }
-        if (hollow(p)) {
+        if (hollow(p)) { // the ray leaves the material where it ENTERS the bore: (-b - s)/a, which needs b < 0 to lie ahead
             double D = fma(b, b, -a * (rho2 - p.rmin2));
             double t = (-b - sqrt_pos(D)) * inv_a;
-            best = (D > 0.0 && b < 0.0 && t > 0.0 && t < best) ? t : best;
+            best = (D > 0.0 && b < 0.0 && ahead(t) && t < best) ? t : best;
         }
         {
             double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(dz));
-            best = (t > 0.0 && t < best) ? t : best;
+            best = (ahead(t) && t < best) ? t : best;
         }
         if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
-                bool ok = ed.c0 < 0.0 && t > 0.0 && fma(t, ed.u0, ep.u0) >= 0.0;
+                bool ok = ed.c0 < 0.0 && ahead(t) && fma(t, ed.u0, ep.u0) >= 0.0;
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
-                bool ok = ed.c1 < 0.0 && t > 0.0 && fma(t, ed.u1, ep.u1) >= 0.0;
+                bool ok = ed.c1 < 0.0 && ahead(t) && fma(t, ed.u1, ep.u1) >= 0.0;
                 best = (ok && t < best) ? t : best;
             }
         }
-        return out ? -1.0 : best;
+        return out ? -1.0 : dmax(best, 0.0);
     }
 };
 using Tube = TubeT<kFlagsRuntime>;
@@ -374,7 +374,7 @@ VG_DEV double frustum_root(const Frustum &f, const RayRZ &r, double z, double dz
     double c = fma(-k, k, r.rho2);
     double D = fma(b, b, -a * c);
     double t = quad_root(a, b, c, sqrt_pos(D), leaving);
-    ok = D > 0.0 && t > 0.0;
+    ok = D > 0.0 && ahead(t);
     return t;
 }
 
@@ -477,11 +477,11 @@ template <int F> struct ConeT {
         }
         {
             double az = fabs(z);
-            double t = (az - p.dz) * rcp(fabs(dz)); // > 0 from beyond the cap; NaN (rejected) for dz = 0
+            double t = (az - p.dz) * rcp(fabs(dz)); // > 0 from beyond the cap, ~0 from on it (R32); NaN (rejected) for dz = 0
             double rh2 = fma(t, fma(t, r.a_xy, r.b_xy + r.b_xy), r.rho2);
             bool top = z > 0.0;
             double rlo = top ? p.rmin2 : p.rmin1, rhi = top ? p.rmax2 : p.rmax1;
-            bool ok = az > p.dz && sign_differs(z, dz) && rh2 >= rlo * rlo && rh2 <= rhi * rhi;
+            bool ok = ahead(t) && sign_differs(z, dz) && rh2 >= rlo * rlo && rh2 <= rhi * rhi;
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
@@ -489,19 +489,19 @@ template <int F> struct ConeT {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 double uh = fma(t, ed.u0, ep.u0), zh = fma(t, dz, z);
-                bool ok = ed.c0 > 0.0 && ep.c0 < 0.0 && fabs(zh) <= p.dz &&
+                bool ok = ed.c0 > 0.0 && ahead(t) && fabs(zh) <= p.dz &&
                           uh >= fma(p.in.B, zh, p.in.A) && uh <= fma(p.out.B, zh, p.out.A);
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
                 double uh = fma(t, ed.u1, ep.u1), zh = fma(t, dz, z);
-                bool ok = ed.c1 > 0.0 && ep.c1 < 0.0 && fabs(zh) <= p.dz &&
+                bool ok = ed.c1 > 0.0 && ahead(t) && fabs(zh) <= p.dz &&
                           uh >= fma(p.in.B, zh, p.in.A) && uh <= fma(p.out.B, zh, p.out.A);
                 best = (ok && t < best) ? t : best;
             }
         }
-        return in ? -1.0 : best;
+        return in ? -1.0 : dmax(best, 0.0);
     }
 
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
@@ -529,21 +529,21 @@ template <int F> struct ConeT {
         }
         {
             double t = (p.dz - flipsign_bits(z, dz)) * rcp(fabs(dz));
-            best = (t > 0.0 && t < best) ? t : best;
+            best = (ahead(t) && t < best) ? t : best;
         }
         if (!full(p)) {
             {
                 double t = -ep.c0 * rcp(ed.c0);
-                bool ok = ed.c0 < 0.0 && t > 0.0 && fma(t, ed.u0, ep.u0) >= 0.0;
+                bool ok = ed.c0 < 0.0 && ahead(t) && fma(t, ed.u0, ep.u0) >= 0.0;
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
-                bool ok = ed.c1 < 0.0 && t > 0.0 && fma(t, ed.u1, ep.u1) >= 0.0;
+                bool ok = ed.c1 < 0.0 && ahead(t) && fma(t, ed.u1, ep.u1) >= 0.0;
                 best = (ok && t < best) ? t : best;
             }
         }
-        return out ? -1.0 : best;
+        return out ? -1.0 : dmax(best, 0.0);
     }
 };
 using Cone = ConeT<kFlagsRuntime>;
@@ -626,7 +626,7 @@ struct Trd {
         double gx, gy, tin, tout;
         double g = gmax(p, fabs(x), fabs(y), z, gx, gy);
         clip_all(p, x, y, z, dx, dy, dz, tin, tout);
-        double t = (tin < tout && tout > 0.0) ? tin : inf();
+        double t = (tin < tout && ahead(tin)) ? dmax(tin, 0.0) : inf();
         return g < -kTol ? -1.0 : t;
     }
     VG_DEV static double dist_out(const P &p, double x, double y, double z, double dx, double dy, double dz)
@@ -634,7 +634,7 @@ struct Trd {
         double gx, gy, tin, tout;
         double g = gmax(p, fabs(x), fabs(y), z, gx, gy);
         clip_all(p, x, y, z, dx, dy, dz, tin, tout);
-        return g > kTol ? -1.0 : tout;
+        return g > kTol ? -1.0 : dmax(tout, 0.0);
     }
 };
 
@@ -778,7 +778,7 @@ template <int F> struct PolyconeT {
             bool up = dz > 0.0;
             bool on_o = rh2 >= st.olo * st.olo && rh2 <= st.ohi * st.ohi && st.ohi > st.olo && (leaving ? (st.oup != 0) == up : (st.oup != 0) != up);
             bool on_i = rh2 >= st.ilo * st.ilo && rh2 <= st.ihi * st.ihi && st.ihi > st.ilo && (leaving ? (st.iup != 0) == up : (st.iup != 0) != up);
-            bool ok = t > 0.0 && (on_o || on_i);
+            bool ok = ahead(t) && (on_o || on_i);
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
@@ -787,7 +787,7 @@ template <int F> struct PolyconeT {
             double t = (p.zlo - z) * idz;
             double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);
             bool sense = leaving ? dz < 0.0 : dz > 0.0;
-            bool ok = sense && t > 0.0 && rh2 >= p.cap_lo_rmin * p.cap_lo_rmin && rh2 <= p.cap_lo_rmax * p.cap_lo_rmax;
+            bool ok = sense && ahead(t) && rh2 >= p.cap_lo_rmin * p.cap_lo_rmin && rh2 <= p.cap_lo_rmax * p.cap_lo_rmax;
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
@@ -795,7 +795,7 @@ template <int F> struct PolyconeT {
             double t = (p.zhi - z) * idz;
             double hx = fma(t, dx, x), hy = fma(t, dy, y), rh2 = fma(hx, hx, hy * hy);
             bool sense = leaving ? dz > 0.0 : dz < 0.0;
-            bool ok = sense && t > 0.0 && rh2 >= p.cap_hi_rmin * p.cap_hi_rmin && rh2 <= p.cap_hi_rmax * p.cap_hi_rmax;
+            bool ok = sense && ahead(t) && rh2 >= p.cap_hi_rmin * p.cap_hi_rmin && rh2 <= p.cap_hi_rmax * p.cap_hi_rmax;
             if (!full(p)) ok = ok && wedge_member_at<WM>(p.w, ep, ed, t);
             best = (ok && t < best) ? t : best;
         }
@@ -803,17 +803,17 @@ template <int F> struct PolyconeT {
             {
                 double t = -ep.c0 * rcp(ed.c0);
                 bool sense = leaving ? ed.c0 < 0.0 : ed.c0 > 0.0;
-                bool ok = sense && t > 0.0 && in_outline(p, fma(t, ed.u0, ep.u0), fma(t, dz, z));
+                bool ok = sense && ahead(t) && in_outline(p, fma(t, ed.u0, ep.u0), fma(t, dz, z));
                 best = (ok && t < best) ? t : best;
             }
             {
                 double t = -ep.c1 * rcp(ed.c1);
                 bool sense = leaving ? ed.c1 < 0.0 : ed.c1 > 0.0;
-                bool ok = sense && t > 0.0 && in_outline(p, fma(t, ed.u1, ep.u1), fma(t, dz, z));
+                bool ok = sense && ahead(t) && in_outline(p, fma(t, ed.u1, ep.u1), fma(t, dz, z));
                 best = (ok && t < best) ? t : best;
             }
         }
-        return best;
+        return dmax(best, 0.0);
     }
     VG_DEV static double dist_in(const P &p, double x, double y, double z, double dx, double dy, double dz)
     {

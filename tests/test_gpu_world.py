@@ -79,27 +79,8 @@ def test_points_outside_the_world_and_bad_nodes(vg, worlds):
     assert bool((wg.safety(bad, *dt[:3]) == -1).all())
 
 
-def test_walk_through_the_world(vg, worlds):
-    """Propagate tracks step by step on the GPU alone (step, move a hair beyond the border, take `next` as the new node) and
-    check every state against the oracle's Locate: the relocation of PAPER.md:98 done by vg_world_step itself."""
-    wc, wo, wg, band = worlds
-    t = wc.tracks(40000, band)
-    x, y, z, dx, dy, dz = dev(t)
-    node = wg.locate(x, y, z)
-    eps = 1e-6
-    agree = []
-    for _ in range(6):
-        step, nxt = wg.step(node, x, y, z, dx, dy, dz)
-        alive = nxt >= 0
-        x = torch.where(alive, x + (step + eps) * dx, x)
-        y = torch.where(alive, y + (step + eps) * dy, y)
-        z = torch.where(alive, z + (step + eps) * dz, z)
-        node = torch.where(alive, nxt, node)
-        loc = wo.locate(x.cpu().numpy(), y.cpu().numpy(), z.cpu().numpy())
-        a = alive.cpu().numpy()
-        agree.append((loc[a] == node.cpu().numpy()[a]).mean())
-    # grazing crossings (within eps of an edge, or a border closer than eps behind the new point) are the only disagreements
-    assert min(agree) > 0.995, agree
+# The walk through the world (step, move onto the border, take `next` as the new node) lives in tests/test_gpu_surface.py
+# now: it is exact (no nudge beyond the border), in lockstep with the oracle and on the GPU alone (reading R32).
 
 
 def test_world_create_rejects_bad_input(vg):
