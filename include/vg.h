@@ -291,6 +291,12 @@ const char *vg_last_error(void);
 int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *stream);
 /* Enqueues `launches` empty kernels (launch-latency floor for the small-N end of configs[3]). */
 int vg_probe_empty_launch(int launches, void *stream);
+/* Enqueues ONE launch of the query kernel of `query` (0 Inside, 1 DistanceToIn, 2 DistanceToOut, 3 SafetyToIn,
+ * 4 SafetyToOut) instantiated with an arithmetic-free pseudo-solid: the loads, the store, the grid shape and the
+ * launch form of a real query on n tracks, one add per coordinate.  Its duration is the size-matched memory ceiling
+ * bench.py quotes beside the small batches.  Arrays as for the queries (dx, dy, dz unused for 0, 3, 4). */
+int vg_probe_stream(int query, const double *x, const double *y, const double *z, const double *dx, const double *dy,
+                    const double *dz, int64_t n, void *out, void *stream);
 /* Host-only: the candidate grids vg_shape_create builds for the safeties of a polycone, recomputed
  * into caller memory so that the host logic can be checked without a device.  masks: HOST uint64[rows * cols] of the
  * surface grid; face_masks: HOST uint64[rows * 2 cols] of the phi-face grid (may be NULL); row_section: HOST

@@ -65,6 +65,7 @@ def _load():
     lib.vg_compute_step_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP]
     lib.vg_probe_fp64_fma_rate.argtypes = [C.c_int, _PD, _VP]
     lib.vg_probe_empty_launch.argtypes = [C.c_int, _VP]
+    lib.vg_probe_stream.argtypes = [C.c_int] + [_VP] * 6 + [C.c_int64, _VP, _VP]
     lib.vg_launch_count.restype = C.c_int64
     lib.vg_set_option.argtypes = [C.c_int, C.c_int64]
     lib.vg_get_option.argtypes = [C.c_int]
@@ -372,6 +373,16 @@ def vg_probe_fp64_fma_rate(launches=20, stream=None):
 
 def vg_probe_empty_launch(launches, stream=None):
     _check(_lib.vg_probe_empty_launch(int(launches), _stream(stream)))
+
+
+def vg_probe_stream(query, x, y, z, dx=None, dy=None, dz=None, out=None, stream=None):
+    """One launch of the arithmetic-free query kernel (same loads, store, grid and form as query `query` on these arrays)."""
+    q = QUERY_ID[query] if isinstance(query, str) else int(query)
+    n = x.numel()
+    need6 = q in (1, 2)
+    arrs = [x, y, z] + ([dx, dy, dz] if need6 else [None, None, None])
+    _check(_lib.vg_probe_stream(q, *[(_p(a) if a is not None else None) for a in arrs], n, _p(out), _stream(stream)))
+    return out
 
 
 def vg_launch_count():

@@ -878,6 +878,21 @@ extern "C" int vg_probe_fp64_fma_rate(int launches, double *fma_per_s, void *str
     return VG_OK;
 }
 
+extern "C" int vg_probe_stream(int query, const double *x, const double *y, const double *z, const double *dx, const double *dy,
+                               const double *dz, int64_t n, void *out, void *stream)
+{
+    if (query < qInside || query > qSafeOut) return fail(VG_ERR_ARG, "vg_probe_stream: unknown query");
+    const bool dir = (query == qDistIn || query == qDistOut);
+    const void *ptrs[6] = { x, y, z, dx, dy, dz };
+    bool vec = false;
+    int rc = check_arrays("vg_probe_stream", ptrs, dir ? 6 : 3, query == qInside ? 4 : 8, out, n, &vec);
+    if (rc != VG_OK || n == 0) return rc;
+    Tracks t{ x, y, z, dx, dy, dz };
+    cudaError_t e = probe_stream(query, t, n, out, vec, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return fail_cuda(e, "vg_probe_stream");
+    return VG_OK;
+}
+
 extern "C" int vg_probe_empty_launch(int launches, void *stream)
 {
     if (launches < 0) return fail(VG_ERR_ARG, "vg_probe_empty_launch: launches < 0");

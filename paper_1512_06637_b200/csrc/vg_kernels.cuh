@@ -607,5 +607,6 @@ cudaError_t launch_world_safety(const WorldTab &w, const int32_t *node, const Tr
 // probes (vg_probe.cu)
 cudaError_t probe_fp64_fma_rate(int launches, double *fma_per_s, cudaStream_t s);
 cudaError_t probe_empty_launch(int launches, cudaStream_t s);
+cudaError_t probe_stream(int q, const Tracks &t, int64_t n, void *out, bool vec, cudaStream_t s);
 
 } // namespace vg
