@@ -304,6 +304,17 @@ int vg_probe_stream(int query, const double *x, const double *y, const double *z
  * dims: HOST int[2] = {rows, cols}.  Any output pointer may be NULL.  VG_ERR_ARG if the shape is not a polycone. */
 int vg_debug_polycone_grid(const vg_shape *shape, uint64_t *masks, uint64_t *face_masks, unsigned char *row_section,
                            double *geom, int *dims);
+/* Host-only: the conservative cull of ComputeStep (which daughters can this ray touch?) evaluated on
+ * the CPU by the very code the kernel runs (csrc/vg_nav_cull.h is compiled for both sides and rounds identically), so
+ * that its soundness can be checked without a device.  mother / daughters / xforms as for vg_volume_create (primitives
+ * only); x .. dz: HOST arrays of n tracks in the mother frame; t_lim: HOST array of the ray-parameter limit per track
+ * (the mother's exit or the physics step; NULL = +inf); masks: HOST uint64[4 n], bit j of masks[4 i + c] set = daughter
+ * 64 c + j survives for track i.  stage 0: both stages as the kernel runs them; 1: the grid walk alone; 2: the FP32
+ * bounding-sphere test alone, applied to every daughter.  grid: HOST double[9] or NULL, receives the candidate grid's
+ * origin, cell size and cells per axis (x, y, z each).  No CUDA call is made. */
+int vg_debug_nav_cull(const vg_shape *mother, int ndaughters, const vg_shape *const *daughters, const double *xforms,
+                      const double *x, const double *y, const double *z, const double *dx, const double *dy,
+                      const double *dz, const double *t_lim, int64_t n, uint64_t *masks, int stage, double *grid);
 /* Host-only: a boolean as vg_boolean_create flattened it: the kinds of its primitives in tree order
  * (kinds: HOST int[8]), the 3x4 transforms from the frame of the boolean to the frame of each primitive (xforms: HOST
  * double[8 * 12]) and the postfix program (prog: HOST uint8[16]; a token < 0x80 pushes that primitive, 0x80 | op combines

@@ -66,6 +66,7 @@ def _load():
     lib.vg_probe_fp64_fma_rate.argtypes = [C.c_int, _PD, _VP]
     lib.vg_probe_empty_launch.argtypes = [C.c_int, _VP]
     lib.vg_probe_stream.argtypes = [C.c_int] + [_VP] * 6 + [C.c_int64, _VP, _VP]
+    lib.vg_debug_nav_cull.argtypes = [_VP, C.c_int, C.POINTER(_VP), _PD] + [_VP] * 7 + [C.c_int64, _VP, C.c_int, _VP]
     lib.vg_launch_count.restype = C.c_int64
     lib.vg_set_option.argtypes = [C.c_int, C.c_int64]
     lib.vg_get_option.argtypes = [C.c_int]
@@ -221,6 +222,24 @@ def vg_volume_create(mother, daughters, xforms):
     h = _VP()
     _check(_lib.vg_volume_create(_handle(mother), nd, arr, xf, C.byref(h)))
     return h
+
+
+def vg_debug_nav_cull(mother, daughters, xforms, x, y, z, dx, dy, dz, t_lim=None, stage=0):
+    """Host-only (numpy float64 arrays in, no device): the candidate masks of ComputeStep's conservative cull as
+    uint64 (n, 4), and the candidate grid's geometry (origin[3], cell size[3], cells per axis[3])."""
+    import numpy as np
+    nd = len(daughters)
+    arr = (_VP * max(1, nd))(*[_handle(d) for d in daughters])
+    flat = [float(v) for row in xforms for v in row]
+    xf = (C.c_double * max(1, len(flat)))(*flat)
+    a = [np.ascontiguousarray(v, dtype=np.float64) for v in (x, y, z, dx, dy, dz)]
+    n = a[0].size
+    tl = None if t_lim is None else np.ascontiguousarray(t_lim, dtype=np.float64)
+    masks = np.zeros((n, 4), dtype=np.uint64)
+    grid = np.zeros(9, dtype=np.float64)
+    _check(_lib.vg_debug_nav_cull(_handle(mother), nd, arr, xf, *[v.ctypes.data for v in a],
+                                  None if tl is None else tl.ctypes.data, n, masks.ctypes.data, int(stage), grid.ctypes.data))
+    return masks, grid
 
 
 def vg_volume_destroy(h):

@@ -3,6 +3,7 @@
 // path runs in the kernels of vg_k_*.cu / vg_nav.cu.
 #include "../../include/vg.h"
 #include "vg_kernels.cuh"
+#include "vg_nav_cull.h"
 
 #include <atomic>
 #include <cmath>
@@ -19,6 +20,8 @@ struct vg_volume {
     SolidU mother;
     NavMeta meta;
     unsigned char *table_dev; // the blob described in vg_params.h
+    unsigned char *table_host; // its host copy (vg_debug_nav_cull evaluates the cull predicate on the CPU)
+    int device;
     vg_world *general;        // mother or a daughter is a polycone / boolean: the volume is held as a one-level world instead
 };
 
@@ -382,46 +385,28 @@ static int to_solid(const vg_shape *s, SolidU *o, const char *what)
     }
 }
 
-extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
-                                vg_volume **out)
+// Host side of vg_volume_create for a volume of primitives: validation, the mother and daughter records, the FP32
+// bounding spheres and the candidate grid, as one blob in host memory (layout: vg_params.h).  No CUDA call.
+static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
+                          vg_volume *v, unsigned char **host_out)
 {
-    if (!out) return fail(VG_ERR_ARG, "vg_volume_create: out is NULL");
-    *out = nullptr;
-    if (!mother) return fail(VG_ERR_ARG, "vg_volume_create: mother is NULL");
-    if (nd < 0 || nd > VG_MAX_DAUGHTERS)
-        return fail(VG_ERR_PARAM, "vg_volume_create: ndaughters must be in [0, %d]", VG_MAX_DAUGHTERS);
-    if (nd > 0 && (!daughters || !xforms)) return fail(VG_ERR_ARG, "vg_volume_create: NULL daughters or xforms");
-    vg_volume *v = new (std::nothrow) vg_volume;
-    if (!v) return fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
-    std::memset(v, 0, sizeof *v);
-    bool general = mother->kind >= VG_POLYCONE;
-    for (int i = 0; i < nd && !general; ++i) general = daughters[i] && daughters[i]->kind >= VG_POLYCONE;
-    if (general) { // polycones / booleans do not fit the fixed-size daughter records: a one-level world serves the volume
-        std::vector<const vg_shape *> shapes(1, mother);
-        std::vector<int32_t> parent(1, -1);
-        std::vector<double> xf = { 1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0 };
-        for (int i = 0; i < nd; ++i) {
-            shapes.push_back(daughters[i]);
-            parent.push_back(0);
-            xf.insert(xf.end(), xforms + 12 * i, xforms + 12 * i + 12);
-        }
-        int rcw = vg_world_create(nd + 1, shapes.data(), parent.data(), xf.data(), &v->general);
-        if (rcw != VG_OK) {
-            delete v;
-            return rcw;
-        }
-        v->meta.nd = nd;
-        *out = v;
-        return VG_OK;
-    }
     int rc = to_solid(mother, &v->mother, "mother");
     NavMeta &mt = v->meta;
     mt.nd = nd;
     mt.nchunks = (nd + 63) / 64;
     int ndp = (nd + kCullUnroll - 1) / kCullUnroll * kCullUnroll;
     mt.off_d = unsigned(16 * ndp);
-    mt.bytes = (mt.off_d + unsigned(nd) * unsigned(kDaughterStride) + 15u) / 16u * 16u;
-    if (mt.bytes == 0) mt.bytes = 16;
+    // the candidate grid (vg_nav_cull.h): about one cell per daughter, at most kNavGridMax cells per axis
+    int gdim = 1;
+    while (gdim < kNavGridMax && gdim * gdim * gdim < nd) ++gdim;
+    NavGrid &gr = mt.grid;
+    gr.g[0] = gr.g[1] = gr.g[2] = gdim;
+    gr.off_g = (mt.off_d + unsigned(nd) * unsigned(kDaughterStride) + 15u) / 16u * 16u;
+    const unsigned ncell = unsigned(gdim * gdim * gdim);
+    const unsigned nchunks_alloc = mt.nchunks == 3 ? 4u : unsigned(mt.nchunks); // kernels exist for 1, 2 and 4 chunks
+    mt.bytes = (gr.off_g + 8u * ncell * (nchunks_alloc ? nchunks_alloc : 1u) + 15u) / 16u * 16u;
+    if (nchunks_alloc) mt.nchunks = int(nchunks_alloc);
+    std::vector<double> sph; // bounding spheres of the daughters in the mother frame: cx, cy, cz, r (FP64)
     unsigned char *host = nullptr;
     if (rc == VG_OK) {
         host = new (std::nothrow) unsigned char[mt.bytes];
@@ -471,7 +456,91 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
         double r2 = r * r * (1.0 + 1e-6) + 64.0 * std::ldexp(1.0, -24) * S * S;
         float e[4] = { float(cx), float(cy), float(cz), std::nextafterf(float(r2), INFINITY) };
         std::memcpy(host + 16 * i, e, 16);
+        mt.all[i / 64] |= 1ull << (i % 64);
+        sph.insert(sph.end(), { cx, cy, cz, std::sqrt(double(e[3])) });
     }
+    if (rc == VG_OK) { // the grid over the bounding box of the spheres; each cell lists the spheres (inflated) that meet it
+        double lo[3] = { 0, 0, 0 }, hi[3] = { 0, 0, 0 };
+        for (int i = 0; i < nd; ++i)
+            for (int a = 0; a < 3; ++a) {
+                double l = sph[4 * i + a] - sph[4 * i + 3], h = sph[4 * i + a] + sph[4 * i + 3];
+                lo[a] = i == 0 ? l : std::fmin(lo[a], l);
+                hi[a] = i == 0 ? h : std::fmax(hi[a], h);
+            }
+        double diag = 0;
+        for (int a = 0; a < 3; ++a) {
+            double ext = hi[a] - lo[a];
+            if (!(ext > 0)) ext = 1.0;
+            lo[a] -= 1e-6 * ext, ext *= 1.0 + 2e-6;
+            gr.o[a] = lo[a], gr.len[a] = ext, gr.cs[a] = ext / gdim, gr.ics[a] = gdim / ext;
+            diag += ext * ext;
+        }
+        diag = std::sqrt(diag);
+        const double pad = 1e-6 * (diag + r_mother); // see vg_nav_cull.h: covers the rounding of the walk
+        gr.tpad = pad;
+        gr.rm2 = r_mother * r_mother * (1.0 + 1e-9);
+        unsigned long long *cells = reinterpret_cast<unsigned long long *>(host + gr.off_g);
+        for (int i = 0; i < nd; ++i) {
+            const double *c = &sph[4 * i];
+            const double rr = c[3] * (1.0 + 1e-6) + pad;
+            for (int iz = 0; iz < gdim; ++iz)
+                for (int iy = 0; iy < gdim; ++iy)
+                    for (int ix = 0; ix < gdim; ++ix) {
+                        const int ic[3] = { ix, iy, iz };
+                        double d2 = 0;
+                        for (int a = 0; a < 3; ++a) { // distance from the sphere centre to the closed cell
+                            double l = gr.o[a] + ic[a] * gr.cs[a], h = l + gr.cs[a];
+                            double d = c[a] < l ? l - c[a] : (c[a] > h ? c[a] - h : 0.0);
+                            d2 += d * d;
+                        }
+                        if (d2 <= rr * rr)
+                            cells[size_t((iz * gdim + iy) * gdim + ix) * mt.nchunks + i / 64] |= 1ull << (i % 64);
+                    }
+        }
+    }
+    if (rc != VG_OK) {
+        delete[] host;
+        host = nullptr;
+    }
+    *host_out = host;
+    return rc;
+}
+
+extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
+                                vg_volume **out)
+{
+    if (!out) return fail(VG_ERR_ARG, "vg_volume_create: out is NULL");
+    *out = nullptr;
+    if (!mother) return fail(VG_ERR_ARG, "vg_volume_create: mother is NULL");
+    if (nd < 0 || nd > VG_MAX_DAUGHTERS)
+        return fail(VG_ERR_PARAM, "vg_volume_create: ndaughters must be in [0, %d]", VG_MAX_DAUGHTERS);
+    if (nd > 0 && (!daughters || !xforms)) return fail(VG_ERR_ARG, "vg_volume_create: NULL daughters or xforms");
+    vg_volume *v = new (std::nothrow) vg_volume;
+    if (!v) return fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
+    std::memset(v, 0, sizeof *v);
+    bool general = mother->kind >= VG_POLYCONE;
+    for (int i = 0; i < nd && !general; ++i) general = daughters[i] && daughters[i]->kind >= VG_POLYCONE;
+    if (general) { // polycones / booleans do not fit the fixed-size daughter records: a one-level world serves the volume
+        std::vector<const vg_shape *> shapes(1, mother);
+        std::vector<int32_t> parent(1, -1);
+        std::vector<double> xf = { 1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0 };
+        for (int i = 0; i < nd; ++i) {
+            shapes.push_back(daughters[i]);
+            parent.push_back(0);
+            xf.insert(xf.end(), xforms + 12 * i, xforms + 12 * i + 12);
+        }
+        int rcw = vg_world_create(nd + 1, shapes.data(), parent.data(), xf.data(), &v->general);
+        if (rcw != VG_OK) {
+            delete v;
+            return rcw;
+        }
+        v->meta.nd = nd;
+        *out = v;
+        return VG_OK;
+    }
+    unsigned char *host = nullptr;
+    int rc = nav_build_host(mother, nd, daughters, xforms, v, &host);
+    NavMeta &mt = v->meta;
     if (rc == VG_OK) {
         cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&v->table_dev), mt.bytes);
         if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMalloc");
@@ -480,12 +549,14 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
             if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMemcpy");
         }
     }
-    delete[] host;
+    if (rc == VG_OK && cudaGetDevice(&v->device) != cudaSuccess) v->device = -1;
     if (rc != VG_OK) {
+        delete[] host;
         if (v->table_dev) cudaFree(v->table_dev);
         delete v;
         return rc;
     }
+    v->table_host = host;
     *out = v;
     return VG_OK;
 }
@@ -495,6 +566,7 @@ extern "C" void vg_volume_destroy(vg_volume *v)
     if (!v) return;
     if (v->general) vg_world_destroy(v->general);
     if (v->table_dev) cudaFree(v->table_dev);
+    delete[] v->table_host;
     delete v;
 }
 
@@ -830,6 +902,50 @@ extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const dou
     Tracks t{ x, y, z, nullptr, nullptr, nullptr };
     cudaError_t e = launch_world_safety(w->tab, node, t, n, safety, static_cast<cudaStream_t>(stream));
     if (e != cudaSuccess) return fail_cuda(e, fn);
+    return VG_OK;
+}
+
+extern "C" int vg_debug_nav_cull(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
+                                 const double *x, const double *y, const double *z, const double *dx, const double *dy,
+                                 const double *dz, const double *t_lim, int64_t n, uint64_t *masks, int stage,
+                                 double *grid)
+{
+    const char *fn = "vg_debug_nav_cull";
+    if (!mother || nd < 1 || nd > VG_MAX_DAUGHTERS || !daughters || !xforms || !x || !y || !z || !dx || !dy || !dz || !masks || n < 0)
+        return fail(VG_ERR_ARG, "%s: bad argument", fn);
+    if (mother->kind >= VG_POLYCONE) return fail(VG_ERR_ARG, "%s: the mother must be a primitive", fn);
+    for (int i = 0; i < nd; ++i)
+        if (!daughters[i] || daughters[i]->kind >= VG_POLYCONE) return fail(VG_ERR_ARG, "%s: daughter %d is not a primitive", fn, i);
+    vg_volume v;
+    std::memset(&v, 0, sizeof v);
+    unsigned char *host = nullptr;
+    int rc = nav_build_host(mother, nd, daughters, xforms, &v, &host);
+    if (rc != VG_OK) return rc;
+    const NavMeta &mt = v.meta;
+    const float4 *cull = reinterpret_cast<const float4 *>(host);
+    const unsigned long long *cells = reinterpret_cast<const unsigned long long *>(host + mt.grid.off_g);
+    if (grid)
+        for (int a = 0; a < 3; ++a) grid[a] = mt.grid.o[a], grid[3 + a] = mt.grid.cs[a], grid[6 + a] = double(mt.grid.g[a]);
+    for (int64_t i = 0; i < n; ++i) {
+        unsigned long long m[4] = { 0, 0, 0, 0 };
+        const double tl = t_lim ? t_lim[i] : INFINITY;
+        if (stage == 0) { // both stages, as the kernel runs them
+            if (mt.nchunks == 1) nav_cull<1>(mt.grid, cull, cells, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m));
+            else if (mt.nchunks == 2) nav_cull<2>(mt.grid, cull, cells, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m));
+            else nav_cull<4>(mt.grid, cull, cells, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m);
+        } else if (stage == 1) { // the grid walk alone
+            if (mt.nchunks == 1) nav_grid_walk<1>(mt.grid, cells, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m));
+            else if (mt.nchunks == 2) nav_grid_walk<2>(mt.grid, cells, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m));
+            else nav_grid_walk<4>(mt.grid, cells, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m);
+        } else { // the FP32 sphere test alone, applied to every daughter
+            for (int c = 0; c < 4; ++c) m[c] = c < mt.nchunks ? mt.all[c] : 0ull;
+            if (mt.nchunks == 1) nav_sphere_refine<1>(cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], reinterpret_cast<unsigned long long(&)[1]>(m));
+            else if (mt.nchunks == 2) nav_sphere_refine<2>(cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], reinterpret_cast<unsigned long long(&)[2]>(m));
+            else nav_sphere_refine<4>(cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], m);
+        }
+        for (int c = 0; c < 4; ++c) masks[4 * i + c] = m[c];
+    }
+    delete[] host;
     return VG_OK;
 }
 

@@ -2,21 +2,23 @@
 // the distance to the geometric border against the physics step, "coordinate
 // transformations and distance calculations").
 //
-// Design: persistent CTAs (a multiple of the SM count), each stages the daughter table blob (vg_params.h) into
-// shared memory ONCE with a TMA bulk copy (cp.async.bulk.shared::cluster.global + mbarrier complete_tx) and then
-// strides over track tiles, one thread per track.  Per track:
-//   phase 1 (FP32 pipe, warp-uniform loop): ray against the bounding sphere of EVERY daughter in the mother
-//           frame -> a 64-bit candidate mask per lane.  The sphere radii carry the FP32 error bound, so the test
-//           can only keep too many daughters, never drop one the ray can touch: a culled daughter's DistanceToIn
-//           is +inf by construction and the result is bit-identical to evaluating all daughters.
-//   phase 2 (FP64 pipe, per-lane loop): each lane walks ITS OWN candidates (typically 0-2 of 64), one loop per solid
-//           kind so that the lanes of a warp execute the same DistanceToIn code on different daughters: transform
-//           p, d with the daughter's 3x4 matrix, DistanceToIn, lexicographic min of (distance, index).
-// The tie-break of R13 (lowest index, mother first) is kept by comparing (t, k) pairs explicitly, because
-// candidates are not visited in index order.
+// Design: persistent CTAs (a multiple of the SM count), each stages the volume's blob (vg_params.h: FP32 bounding
+// spheres, daughter records, candidate grid) into shared memory ONCE with a TMA bulk copy (cp.async.bulk.shared::cluster
+// .global + mbarrier complete_tx) and then strides over track tiles, one thread per track.  Per track:
+//   phase 1 (per lane; vg_nav_cull.h): FP64 walk of the candidate grid along the ray up to the mother's exit, then an
+//           FP32 ray / bounding-sphere test of the few daughters listed in the cells crossed -> a 64-bit candidate
+//           mask per chunk of 64 daughters.  Both tests only ever keep too many daughters: a culled daughter's
+//           DistanceToIn is +inf by construction, the result is bit-identical to evaluating all daughters.
+//   phase 2 (per warp): the candidates of the warp's 32 tracks, pooled per solid kind, are evaluated as one dense work
+//           list -- transform p, d with the daughter's 3x4 matrix, DistanceToIn -- and every owner lane takes the
+//           lexicographic min of (distance, index) over its own.
+// The tie-break of R13 (lowest index, mother first) is kept by comparing (t, k) pairs explicitly.
 #include "vg_kernels.cuh"
+#include "vg_nav_cull.h"
 #include "vg_solid.cuh"
 #include "vg_tma.cuh"
+
+#include <mutex>
 
 namespace vg {
 
@@ -41,40 +43,153 @@ VG_DEV const Daughter &daughter_at(const unsigned char *dtab, int k)
     return *reinterpret_cast<const Daughter *>(dtab + size_t(k) * kDaughterStride);
 }
 
-// phase 2 for the candidates of one kind: every lane walks its own bit mask
-template <class S>
-VG_DEV void eval_candidates(unsigned long long mk, int base, const unsigned char *dtab, double x, double y, double z,
-                            double dx, double dy, double dz, double &best, int &who)
+// ---- phase 2, warp-cooperative: the candidates of the 32 tracks of a warp are evaluated as one dense work list ----
+//
+// After the cull a lane holds 0-3 candidates and most lanes hold none (22 % of the tracks of configs[4] hit anything):
+// with every lane walking its own list the warp runs max-over-lanes iterations at 1-2 active lanes each.  Here the
+// lanes pool their candidates of one solid kind in a shared-memory queue (one (lane, daughter) code per entry, places
+// from a warp prefix sum), then ALL lanes take one entry each, fetch the owner's track with shuffles, transform it
+// into the daughter's frame and run that kind's DistanceToIn -- the same code on 32 different (track, daughter) pairs.
+// The distances go back through shared memory; every owner folds its own, in ascending daughter order, into the
+// lexicographic minimum of R13.  (BASELINE.json north_star: "warp-level ... where a warp cooperates over daughters".)
+constexpr int kCoopPerLane = 2;               // candidates a lane may enqueue per pass (unrolled: no per-lane loops)
+constexpr int kCoopQueue = 32 * kCoopPerLane; // entries per warp
+constexpr unsigned kFullWarp = 0xffffffffu;
+
+// lowest set bit of the 64-bit mask held as two words, removed from it; 64 if the mask is empty
+VG_DEV int pop_lowest(unsigned &lo, unsigned &hi)
 {
-    while (mk) {
-        int k = base + __ffsll((long long)mk) - 1;
-        mk &= mk - 1;
-        const Daughter &D = daughter_at(dtab, k);
-        double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
-        double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
-        double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
-        double ldx = fma(D.m[0], dx, fma(D.m[1], dy, D.m[2] * dz));
-        double ldy = fma(D.m[4], dx, fma(D.m[5], dy, D.m[6] * dz));
-        double ldz = fma(D.m[8], dx, fma(D.m[9], dy, D.m[10] * dz));
-        double tk = S::dist_in(Pick<S>::of(D.s), lx, ly, lz, ldx, ldy, ldz);
-        // R13: lexicographic min of (distance, index); a daughter the track is inside of (-1) is skipped
-        bool take = tk >= 0.0 && (tk < best || (tk == best && k < who));
-        best = take ? tk : best;
-        who = take ? k : who;
+    const bool in_lo = lo != 0u;
+    const unsigned w = in_lo ? lo : hi;
+    const int b = (in_lo ? 0 : 32) + __ffs(int(w)) - 1;
+    lo = in_lo ? (lo & (lo - 1u)) : lo;
+    hi = in_lo ? hi : (hi & (hi - 1u));
+    return w ? b : 64;
+}
+
+template <class S>
+VG_DEV void coop_candidates(unsigned long long mk, int base, const unsigned char *dtab, double x, double y, double z,
+                            double dx, double dy, double dz, double &best, int &who, int *q, double *res)
+{
+    const unsigned lane = threadIdx.x & 31u, lt = (1u << lane) - 1u;
+    unsigned lo = unsigned(mk), hi = unsigned(mk >> 32);
+    while (true) {
+        const int b0 = pop_lowest(lo, hi), b1 = pop_lowest(lo, hi);
+        const unsigned B0 = __ballot_sync(kFullWarp, b0 < 64), B1 = __ballot_sync(kFullWarp, b1 < 64);
+        if (B0 == 0u) break;
+        const int n0 = __popc(B0), total = n0 + __popc(B1);
+        const int off0 = __popc(B0 & lt), off1 = n0 + __popc(B1 & lt);
+        if (b0 < 64) q[off0] = int(lane << 6) | b0;
+        if (b1 < 64) q[off1] = int(lane << 6) | b1;
+        __syncwarp();
+        for (int r0 = 0; r0 < total; r0 += 32) {
+            const int it = r0 + int(lane);
+            const bool act = it < total;
+            const int code = act ? q[it] : int(lane << 6);
+            const int src = code >> 6, k = base + (code & 63);
+            const double sx = __shfl_sync(kFullWarp, x, src), sy = __shfl_sync(kFullWarp, y, src),
+                         sz = __shfl_sync(kFullWarp, z, src), sdx = __shfl_sync(kFullWarp, dx, src),
+                         sdy = __shfl_sync(kFullWarp, dy, src), sdz = __shfl_sync(kFullWarp, dz, src);
+            if (act) {
+                const Daughter &D = daughter_at(dtab, k);
+                double lx = fma(D.m[0], sx, fma(D.m[1], sy, fma(D.m[2], sz, D.m[3])));
+                double ly = fma(D.m[4], sx, fma(D.m[5], sy, fma(D.m[6], sz, D.m[7])));
+                double lz = fma(D.m[8], sx, fma(D.m[9], sy, fma(D.m[10], sz, D.m[11])));
+                double ldx = fma(D.m[0], sdx, fma(D.m[1], sdy, D.m[2] * sdz));
+                double ldy = fma(D.m[4], sdx, fma(D.m[5], sdy, D.m[6] * sdz));
+                double ldz = fma(D.m[8], sdx, fma(D.m[9], sdy, D.m[10] * sdz));
+                res[it] = S::dist_in(Pick<S>::of(D.s), lx, ly, lz, ldx, ldy, ldz);
+            }
+        }
+        __syncwarp();
+        // R13: lexicographic min of (distance, index), own candidates in ascending index order; a daughter the track
+        // is inside of (-1) is skipped
+        const double t0 = b0 < 64 ? res[off0] : -1.0, t1 = b1 < 64 ? res[off1] : -1.0;
+        const int k0 = base + b0, k1 = base + b1;
+        const bool take0 = t0 >= 0.0 && (t0 < best || (t0 == best && k0 < who));
+        best = take0 ? t0 : best;
+        who = take0 ? k0 : who;
+        const bool take1 = t1 >= 0.0 && (t1 < best || (t1 == best && k1 < who));
+        best = take1 ? t1 : best;
+        who = take1 ? k1 : who;
+        if (!__any_sync(kFullWarp, (lo | hi) != 0u)) break;
+        __syncwarp(); // the next pass reuses q and res
     }
 }
 
-// kStep = true: ComputeStep; false: volume safety (directions unused)
-template <bool kStep>
-__global__ void __launch_bounds__(kNavBlock) nav_kernel(const __grid_constant__ SolidU mother,
-                                                        const __grid_constant__ NavMeta meta,
-                                                        const unsigned char *__restrict__ table, Tracks t,
-                                                        double step_max, int64_t n, double *__restrict__ out,
-                                                        int32_t *__restrict__ hit)
+// ComputeStep; NC = chunks of 64 daughters (1, 2 or 4)
+template <int NC>
+__global__ void __launch_bounds__(kNavBlock) nav_step_kernel(const __grid_constant__ SolidU mother,
+                                                             const __grid_constant__ NavMeta meta,
+                                                             const unsigned char *__restrict__ table, Tracks t,
+                                                             double step_max, int64_t n, double *__restrict__ out,
+                                                             int32_t *__restrict__ hit)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
+    __shared__ int q_all[kNavBlock / 32][kCoopQueue];
+    __shared__ double res_all[kNavBlock / 32][kCoopQueue];
     const float4 *cull = reinterpret_cast<const float4 *>(smem_raw);
+    const unsigned char *dtab = smem_raw + meta.off_d;
+    const unsigned long long *cells = reinterpret_cast<const unsigned long long *>(smem_raw + meta.grid.off_g);
+    const int nd = meta.nd;
+    int *q = q_all[threadIdx.x >> 5];
+    double *res = res_all[threadIdx.x >> 5];
+
+    if (threadIdx.x == 0) {
+        mbar_init(&bar, 1);
+        mbar_fence_init();
+    }
+    pdl_launch_dependents();
+    __syncthreads();
+    pdl_wait();
+    if (threadIdx.x == 0 && nd > 0) tma_load_table(smem_raw, table, meta.bytes, &bar);
+    bool waited = (nd == 0);
+
+    // warp-uniform trip count: the lanes past n take part in the warp's collectives with an empty candidate list
+    for (int64_t tile = int64_t(blockIdx.x) * kNavBlock; tile < n; tile += int64_t(gridDim.x) * kNavBlock) {
+        const int64_t i = tile + threadIdx.x;
+        const bool valid = i < n;
+        double x = 0, y = 0, z = 0, dx = 0, dy = 0, dz = 1;
+        if (valid) {
+            x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+            dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+        }
+        if (!waited) { // the track loads above are already in flight while the table lands
+            mbar_wait(&bar, 0);
+            waited = true;
+        }
+        double best = solid_dist_out(mother, x, y, z, dx, dy, dz);
+        int who = -1;
+        if (nd > 0) {
+            unsigned long long m[NC];
+            nav_cull<NC>(meta.grid, cull, cells, meta.all, x, y, z, dx, dy, dz, best < step_max ? best : step_max, m);
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const unsigned long long mc = valid ? m[c] : 0ull;
+                if (meta.kmask[kBox][c]) coop_candidates<Box>(mc & meta.kmask[kBox][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
+                if (meta.kmask[kTube][c]) coop_candidates<Tube>(mc & meta.kmask[kTube][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
+                if (meta.kmask[kOrb][c]) coop_candidates<Orb>(mc & meta.kmask[kOrb][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
+                if (meta.kmask[kCone][c]) coop_candidates<Cone>(mc & meta.kmask[kCone][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
+                if (meta.kmask[kTrd][c]) coop_candidates<Trd>(mc & meta.kmask[kTrd][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
+            }
+        }
+        if (valid) {
+            bool phys = best > step_max; // PAPER.md:98: the physics step is shorter than the geometric one
+            stg1(out + i, phys ? step_max : best);
+            stg1i(hit + i, phys ? -2 : who);
+        }
+    }
+}
+
+// volume safety: min over the mother and every daughter of the exact distance
+__global__ void __launch_bounds__(kNavBlock) nav_safety_kernel(const __grid_constant__ SolidU mother,
+                                                               const __grid_constant__ NavMeta meta,
+                                                               const unsigned char *__restrict__ table, Tracks t,
+                                                               int64_t n, double *__restrict__ out)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar;
     const unsigned char *dtab = smem_raw + meta.off_d;
     const int nd = meta.nd;
 
@@ -90,114 +205,92 @@ __global__ void __launch_bounds__(kNavBlock) nav_kernel(const __grid_constant__ 
 
     for (int64_t i = int64_t(blockIdx.x) * kNavBlock + threadIdx.x; i < n; i += int64_t(gridDim.x) * kNavBlock) {
         double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
-        double dx = 0, dy = 0, dz = 0;
-        if (kStep) {
-            dx = ldg1(t.dx + i);
-            dy = ldg1(t.dy + i);
-            dz = ldg1(t.dz + i);
-        }
-        if (!waited) { // the track loads above are already in flight while the table lands
+        if (!waited) {
             mbar_wait(&bar, 0);
             waited = true;
         }
-        if (kStep) {
-            double best = solid_dist_out(mother, x, y, z, dx, dy, dz);
-            int who = -1;
-            const float xf = float(x), yf = float(y), zf = float(z), dxf = float(dx), dyf = float(dy), dzf = float(dz);
+        double best = -solid_sdf(mother, x, y, z);
 #pragma unroll 1
-            for (int c = 0; c < meta.nchunks; ++c) {
-                const int base = 64 * c;
-                const int lim = min(64, ((nd - base) + kCullUnroll - 1) / kCullUnroll * kCullUnroll);
-                unsigned long long m = 0;
-#pragma unroll 1
-                for (int j0 = 0; j0 < lim; j0 += kCullUnroll) {
-#pragma unroll
-                    for (int u = 0; u < kCullUnroll; ++u) {
-                        float4 s = cull[base + j0 + u]; // warp-uniform address: shared-memory broadcast
-                        float vx = s.x - xf, vy = s.y - yf, vz = s.z - zf;
-                        float vv = fmaf(vx, vx, fmaf(vy, vy, vz * vz));
-                        float tca = fmaf(vx, dxf, fmaf(vy, dyf, vz * dzf));
-                        float d2 = fmaf(-tca, tca, vv);
-                        bool keep = d2 <= s.w && (tca >= 0.f || vv <= s.w);
-                        m |= (unsigned long long)keep << (j0 + u);
-                    }
-                }
-                if (meta.kmask[kBox][c]) eval_candidates<Box>(m & meta.kmask[kBox][c], base, dtab, x, y, z, dx, dy, dz, best, who);
-                if (meta.kmask[kTube][c]) eval_candidates<Tube>(m & meta.kmask[kTube][c], base, dtab, x, y, z, dx, dy, dz, best, who);
-                if (meta.kmask[kOrb][c]) eval_candidates<Orb>(m & meta.kmask[kOrb][c], base, dtab, x, y, z, dx, dy, dz, best, who);
-                if (meta.kmask[kCone][c]) eval_candidates<Cone>(m & meta.kmask[kCone][c], base, dtab, x, y, z, dx, dy, dz, best, who);
-                if (meta.kmask[kTrd][c]) eval_candidates<Trd>(m & meta.kmask[kTrd][c], base, dtab, x, y, z, dx, dy, dz, best, who);
-            }
-            bool phys = best > step_max; // PAPER.md:98: the physics step is shorter than the geometric one
-            stg1(out + i, phys ? step_max : best);
-            stg1i(hit + i, phys ? -2 : who);
-        } else {
-            double best = -solid_sdf(mother, x, y, z);
-#pragma unroll 1
-            for (int k = 0; k < nd; ++k) {
-                const Daughter &D = daughter_at(dtab, k);
-                double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
-                double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
-                double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
-                best = dmin(best, solid_sdf(D.s, lx, ly, lz));
-            }
-            stg1(out + i, best);
+        for (int k = 0; k < nd; ++k) {
+            const Daughter &D = daughter_at(dtab, k);
+            double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
+            double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
+            double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
+            best = dmin(best, solid_sdf(D.s, lx, ly, lz));
         }
+        stg1(out + i, best);
     }
 }
 
-template <bool kStep>
-static cudaError_t launch_nav(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
-                              double step_max, int64_t n, double *out, int32_t *hit, cudaStream_t s)
+// Per-device launch state, process-wide: the shared-memory opt-in of a kernel is a per-device attribute that
+// cudaFuncSetAttribute SETS (it does not max), so it is only ever raised, under a lock, and the occupancy is cached
+// for the size it was computed for.
+struct NavDevState {
+    std::mutex mu;
+    int sm_count = 0;
+    size_t granted = 32 * 1024; // the kernels also hold static shared memory: opt in early
+    size_t occ_smem = size_t(-1);
+    int per_sm = 0;
+};
+
+template <class Kern>
+static cudaError_t nav_grid_size(Kern kern, NavDevState *states, size_t smem, int64_t n, unsigned *grid)
 {
-    if (n <= 0) return cudaSuccess;
-    size_t smem = meta.bytes;
-    // caches of the device queries, per host thread AND per device (the shared-memory opt-in is a per-device attribute of
-    // the kernel): after the first launch on a device the path makes no CUDA call but cudaGetDevice and the launch
     constexpr int kMaxDev = 64;
-    struct DevCache {
-        int sm_count = 0, per_sm = 0;
-        size_t smem_granted = 48 * 1024, smem_occ = size_t(-1);
-    };
-    static thread_local DevCache cache[kMaxDev];
-    cudaError_t err;
     int dev = 0;
+    cudaError_t err;
     if ((err = cudaGetDevice(&dev)) != cudaSuccess) return err;
     if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
-    int &sm_count = cache[dev].sm_count, &per_sm = cache[dev].per_sm;
-    size_t &smem_granted = cache[dev].smem_granted, &smem_occ = cache[dev].smem_occ;
-    if (sm_count == 0) {
-        if ((err = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return err;
-    }
-    if (smem > smem_granted) {
-        if ((err = cudaFuncSetAttribute(nav_kernel<kStep>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem))) !=
-            cudaSuccess)
+    NavDevState &st = states[dev];
+    std::lock_guard<std::mutex> lock(st.mu);
+    if (st.sm_count == 0 &&
+        (err = cudaDeviceGetAttribute(&st.sm_count, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+        return err;
+    if (smem > st.granted) {
+        if ((err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem))) != cudaSuccess)
             return err;
-        smem_granted = smem;
+        st.granted = smem;
     }
-    if (smem != smem_occ) {
-        if ((err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nav_kernel<kStep>, kNavBlock, smem)) !=
-            cudaSuccess)
-            return err;
-        if (per_sm < 1) per_sm = 1;
-        smem_occ = smem;
+    if (smem != st.occ_smem) {
+        if ((err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&st.per_sm, kern, kNavBlock, smem)) != cudaSuccess) return err;
+        if (st.per_sm < 1) st.per_sm = 1;
+        st.occ_smem = smem;
     }
-    int64_t want = (n + kNavBlock - 1) / kNavBlock;
-    int64_t cap = int64_t(sm_count) * per_sm; // persistent: one resident wave, a multiple of the SM count
-    unsigned grid = unsigned(want < cap ? want : cap);
-    return launch_kernel(nav_kernel<kStep>, grid, kNavBlock, smem, s, mother, meta, table_dev, t, step_max, n, out, hit);
+    const int64_t want = (n + kNavBlock - 1) / kNavBlock;
+    const int64_t cap = int64_t(st.sm_count) * st.per_sm; // persistent: one resident wave, a multiple of the SM count
+    *grid = unsigned(want < cap ? want : cap);
+    return cudaSuccess;
+}
+
+template <int NC>
+static cudaError_t launch_step_nc(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
+                                  double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
+{
+    static NavDevState states[64];
+    unsigned grid = 0;
+    cudaError_t err = nav_grid_size(nav_step_kernel<NC>, states, meta.bytes, n, &grid);
+    if (err != cudaSuccess) return err;
+    return launch_kernel(nav_step_kernel<NC>, grid, kNavBlock, meta.bytes, s, mother, meta, table_dev, t, step_max, n, step, hit);
 }
 
 cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                 double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
 {
-    return launch_nav<true>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    if (n <= 0) return cudaSuccess;
+    if (meta.nchunks <= 1) return launch_step_nc<1>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    if (meta.nchunks == 2) return launch_step_nc<2>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    return launch_step_nc<4>(mother, table_dev, meta, t, step_max, n, step, hit, s);
 }
 
 cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                  int64_t n, double *safety, cudaStream_t s)
 {
-    return launch_nav<false>(mother, table_dev, meta, t, 0.0, n, safety, nullptr, s);
+    if (n <= 0) return cudaSuccess;
+    static NavDevState states[64];
+    unsigned grid = 0;
+    cudaError_t err = nav_grid_size(nav_safety_kernel, states, meta.bytes, n, &grid);
+    if (err != cudaSuccess) return err;
+    return launch_kernel(nav_safety_kernel, grid, kNavBlock, meta.bytes, s, mother, meta, table_dev, t, n, safety);
 }
 
 } // namespace vg

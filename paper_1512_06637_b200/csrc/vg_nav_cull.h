@@ -1,0 +1,162 @@
+// vg_nav_cull.h -- which daughters of a volume can a ray touch?  (ComputeStep)
+//
+// ComputeStep is "every placed daughter" (BASELINE.json): DistanceToIn of each of the nd daughters and the lexicographic
+// minimum.  A daughter the ray cannot touch has DistanceToIn = +inf and never wins, so the kernel may skip it as long as
+// the skip is CONSERVATIVE: it may keep a daughter the ray misses, it must never drop one the ray touches.  This header
+// holds that predicate, in one place and compiled for BOTH sides: the device code of nav_kernel (vg_nav.cu) and the
+// host-only debug export vg_debug_nav_cull (vg_api.cu), which tests/test_nav_cull.py runs on the CPU over adversarial
+// rays against the oracle's DistanceToIn.  Every operation is written with an explicit rounding (fma / fmaf, IEEE
+// reciprocal), so host and device evaluate it bit for bit the same.
+//
+// Two stages per track:
+//  1. FP64 walk of a coarse uniform grid laid over the bounding box of all daughter spheres in the mother frame (3-D
+//     DDA).  Each cell holds the bit mask of the daughters whose bounding sphere, inflated by `pad`, meets the closed
+//     cell; the candidate mask of the ray is the OR over the cells it crosses between the start point and t_lim (the
+//     mother's exit or the physics step, whichever is nearer: a daughter crossed later cannot win).  Rounding can make
+//     the walk cut a corner the exact ray passes (or the other way round) only within ~1e-13 of the grid's size from a
+//     cell edge; `pad` = 1e-6 of the grid diagonal, so a sphere that meets the exact ray inside the skipped cell also
+//     meets a visited neighbour.
+//  2. FP32 test of the ray against the bounding sphere of each remaining candidate.  With S >= |c - p| + r the FP32
+//     evaluation of |c - p|^2 - ((c - p).d)^2 is off by < 30 u S^2 (u = 2^-24); the squared radius in the table is
+//     inflated by 64 u S^2 + 1e-6 relative and rounded up (vg_volume_create), S taken for p anywhere in the mother's
+//     bounding sphere.  Start points outside that sphere (contract violations) skip both stages and keep every daughter.
+#pragma once
+#include "vg_params.h"
+
+#if defined(__CUDA_ARCH__)
+#define VG_HD __host__ __device__ __forceinline__
+#define VG_RCP_RN(a) __drcp_rn(a)
+#define VG_CLZ32(m) __clz(int(m))
+#elif defined(__CUDACC__)
+#define VG_HD __host__ __device__ inline
+#define VG_RCP_RN(a) (1.0 / (a))
+#define VG_CLZ32(m) __builtin_clz(m)
+#else
+#define VG_HD inline
+#define VG_RCP_RN(a) (1.0 / (a))
+#define VG_CLZ32(m) __builtin_clz(m)
+#endif
+
+#include <math.h>
+
+namespace vg {
+
+// one axis of the walk: clip [t0, t1] to the slab [0, L] of the grid
+VG_HD bool nav_axis_clip(double p, double d, double L, double &t0, double &t1, double &inv)
+{
+    if (fabs(d) < 1e-300) { // parallel to the slab: inside it for all t or never
+        inv = 0.0;
+        return p >= 0.0 && p <= L;
+    }
+    inv = VG_RCP_RN(d);
+    double ta = -p * inv, tb = (L - p) * inv;
+    double tn = ta < tb ? ta : tb, tf = ta < tb ? tb : ta;
+    t0 = tn > t0 ? tn : t0;
+    t1 = tf < t1 ? tf : t1;
+    return true;
+}
+
+// ... and set up the stepping: ray parameter of the next cell border on this axis (tmax), its increment per cell
+// (tdelta), the cells left before the walk leaves the grid, the cell index
+VG_HD void nav_axis_init(double p, double d, double inv, double t0, double cs, double ics, int g, double &tmax,
+                         double &tdelta, int &left, int &i)
+{
+    double e = fma(t0, d, p); // entry coordinate relative to the grid origin
+    i = int(floor(e * ics));
+    i = i < 0 ? 0 : (i > g - 1 ? g - 1 : i);
+    const bool up = d > 0.0, still = inv == 0.0;
+    tmax = still ? INFINITY : fma(double(i + (up ? 1 : 0)), cs, -p) * inv;
+    tdelta = still ? 0.0 : cs * fabs(inv);
+    left = still ? 0 : (up ? g - 1 - i : i);
+}
+
+// Stage 1.  m[c] |= candidates of chunk c (64 daughters per chunk).  `cells`: [gz][gy][gx][NC] masks.
+// The loop body is branch-free (selects), so the lanes of a warp stay converged while they walk different cells.
+template <int NC>
+VG_HD void nav_grid_walk(const NavGrid &G, const unsigned long long *cells, double x, double y, double z, double dx,
+                         double dy, double dz, double t_lim, unsigned long long (&m)[NC])
+{
+#pragma unroll
+    for (int c = 0; c < NC; ++c) m[c] = 0ull;
+    const double px = x - G.o[0], py = y - G.o[1], pz = z - G.o[2];
+    double t0 = 0.0, t1 = fma(t_lim, 1e-9, t_lim) + G.tpad; // a crossing at t_lim itself still counts
+    double ivx, ivy, ivz;
+    bool ok = nav_axis_clip(px, dx, G.len[0], t0, t1, ivx);
+    ok = nav_axis_clip(py, dy, G.len[1], t0, t1, ivy) && ok;
+    ok = nav_axis_clip(pz, dz, G.len[2], t0, t1, ivz) && ok;
+    if (!ok || !(t0 <= t1)) return;
+    double tmx, tmy, tmz, tdx, tdy, tdz;
+    int lx, ly, lz, ix, iy, iz;
+    nav_axis_init(px, dx, ivx, t0, G.cs[0], G.ics[0], G.g[0], tmx, tdx, lx, ix);
+    nav_axis_init(py, dy, ivy, t0, G.cs[1], G.ics[1], G.g[1], tmy, tdy, ly, iy);
+    nav_axis_init(pz, dz, ivz, t0, G.cs[2], G.ics[2], G.g[2], tmz, tdz, lz, iz);
+    int idx = ix + G.g[0] * (iy + G.g[1] * iz);
+    const int stx = dx > 0.0 ? 1 : -1, sty = dy > 0.0 ? G.g[0] : -G.g[0], stz = dz > 0.0 ? G.g[0] * G.g[1] : -G.g[0] * G.g[1];
+    const int max_cells = G.g[0] + G.g[1] + G.g[2];
+    for (int it = 0; it < max_cells; ++it) { // a straight line crosses at most gx + gy + gz - 2 cells
+#pragma unroll
+        for (int c = 0; c < NC; ++c) m[c] |= cells[idx * NC + c];
+        const bool sx = tmx <= tmy && tmx <= tmz, sy = !sx && tmy <= tmz, sz = !sx && !sy;
+        const double tsel = sx ? tmx : (sy ? tmy : tmz);
+        const int left = sx ? lx : (sy ? ly : lz);
+        if (tsel > t1 || left == 0) break;
+        idx += sx ? stx : (sy ? sty : stz);
+        tmx += sx ? tdx : 0.0, tmy += sy ? tdy : 0.0, tmz += sz ? tdz : 0.0;
+        lx -= sx ? 1 : 0, ly -= sy ? 1 : 0, lz -= sz ? 1 : 0;
+    }
+}
+
+// Stage 2: the ray against the inflated bounding sphere {cx, cy, cz, r2} of one daughter, in FP32.
+VG_HD bool nav_sphere_keep(const float4 s, float xf, float yf, float zf, float dxf, float dyf, float dzf)
+{
+    float vx = s.x - xf, vy = s.y - yf, vz = s.z - zf;
+    float vv = fmaf(vx, vx, fmaf(vy, vy, vz * vz));
+    float tca = fmaf(vx, dxf, fmaf(vy, dyf, vz * dzf));
+    float d2 = fmaf(-tca, tca, vv);
+    return d2 <= s.w && (tca >= 0.f || vv <= s.w);
+}
+
+// ... for every candidate of a 32-bit half of a mask (32-bit words: a 64-bit find-first-set costs three times as much)
+VG_HD unsigned nav_sphere_refine32(const float4 *cull32, unsigned in, float xf, float yf, float zf, float dxf, float dyf,
+                                   float dzf)
+{
+    unsigned out = 0u;
+    while (in) {
+        const unsigned low = in & (0u - in);
+        in ^= low;
+        const int j = 31 - VG_CLZ32(low);
+        if (nav_sphere_keep(cull32[j], xf, yf, zf, dxf, dyf, dzf)) out |= low;
+    }
+    return out;
+}
+
+template <int NC>
+VG_HD void nav_sphere_refine(const float4 *cull, double x, double y, double z, double dx, double dy, double dz,
+                             unsigned long long (&m)[NC])
+{
+    const float xf = float(x), yf = float(y), zf = float(z), dxf = float(dx), dyf = float(dy), dzf = float(dz);
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+        const unsigned lo = nav_sphere_refine32(cull + 64 * c, unsigned(m[c]), xf, yf, zf, dxf, dyf, dzf);
+        const unsigned hi = nav_sphere_refine32(cull + 64 * c + 32, unsigned(m[c] >> 32), xf, yf, zf, dxf, dyf, dzf);
+        m[c] = (unsigned long long)hi << 32 | lo;
+    }
+}
+
+// Both stages.  `all[c]` = every daughter of chunk c (what a start point outside the mother's bounding sphere keeps).
+template <int NC>
+VG_HD void nav_cull(const NavGrid &G, const float4 *cull, const unsigned long long *cells, const unsigned long long *all,
+                    double x, double y, double z, double dx, double dy, double dz, double t_lim,
+                    unsigned long long (&m)[NC])
+{
+    const double pp = fma(x, x, fma(y, y, z * z));
+    if (!(pp <= G.rm2)) { // outside the mother's bounding sphere (or NaN): the error bounds above do not cover it
+#pragma unroll
+        for (int c = 0; c < NC; ++c) m[c] = all[c];
+        return;
+    }
+    nav_grid_walk<NC>(G, cells, x, y, z, dx, dy, dz, t_lim, m);
+    nav_sphere_refine<NC>(cull, x, y, z, dx, dy, dz, m);
+}
+
+} // namespace vg

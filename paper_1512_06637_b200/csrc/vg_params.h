@@ -162,16 +162,30 @@ struct Daughter {
 //                              ndp = nd rounded up to a multiple of kCullUnroll, padding entries have r2 = -1
 //   [off_d, off_d + nd stride) the Daughter records, stride = sizeof(Daughter) rounded up to an ODD number of 8-byte
 //                              words so that lanes reading different daughters spread over the shared-memory banks
+//   [off_g, off_g + 8 ncell nchunks)  candidate masks of the grid cells (NavGrid below), off_g a multiple of 16
 //   total rounded up to a multiple of 16 bytes (bulk-copy granularity)
 constexpr int kCullUnroll = 8;
 constexpr int kDaughterStride = int(sizeof(Daughter)) + (((sizeof(Daughter) / 8) % 2 == 0) ? 8 : 0);
 constexpr int kNavChunks = 4; // 64 daughters per chunk, VG_MAX_DAUGHTERS = 256
 constexpr int kNavKinds = 5;  // every kind except the polycone
 
+// Uniform grid over the bounding box of all daughter spheres in the mother frame (vg_nav_cull.h): g[0] x g[1] x g[2]
+// cells of size cs, each with one 64-bit candidate mask per chunk at blob offset off_g ([gz][gy][gx][nchunks]).
+constexpr int kNavGridMax = 8; // cells per axis
+struct NavGrid {
+    double o[3], len[3], cs[3], ics[3]; // origin, extent, cell size and its inverse per axis
+    double tpad;                        // absolute slack added to the ray-parameter limit of the walk
+    double rm2;                         // squared radius of the mother's bounding sphere about its origin, inflated
+    int g[3];
+    unsigned off_g;
+};
+
 struct NavMeta {
     int nd, nchunks;
     unsigned off_d, bytes;
     unsigned long long kmask[kNavKinds][kNavChunks]; // bit j of kmask[kind][c]: daughter 64 c + j is of that kind
+    unsigned long long all[kNavChunks];              // every daughter of the chunk
+    NavGrid grid;
 };
 
 // hierarchy of volumes (vg_world.cu): one record per node, plus the child lists as one int32 array

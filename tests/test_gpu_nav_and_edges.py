@@ -311,6 +311,42 @@ def test_mixed_daughter_kinds_and_mothers(vg):
         assert_real_close(sg, vo.safety(*t[:3]), "volume safety mother=%d" % mk)
 
 
+@pytest.mark.parametrize("nd, size, spread", [(65, 6.0, 40.0), (100, 20.0, 30.0), (130, 8.0, 45.0), (256, 12.0, 40.0),
+                                              (64, 30.0, 10.0)])
+def test_many_overlapping_daughters_of_all_kinds(vg, nd, size, spread):
+    """More than one chunk of 64 daughters (two- and four-chunk kernels), five kinds, heavy overlap: a track has many
+    candidates of one kind, so the warp's shared work list takes several passes; tracks start anywhere in the mother
+    (inside a daughter: that daughter is skipped, R13).  Every step and hit index against the oracle."""
+    rng = np.random.default_rng(nd * 31 + int(size))
+    kinds, pars, xf = [], [], []
+    for _ in range(nd):
+        kind = [W.BOX, W.ORB, W.TUBE, W.CONE, W.TRD][rng.integers(0, 5)]
+        a, b, c = size * rng.uniform(0.3, 1.0, 3)
+        par = {W.BOX: [a, b, c], W.ORB: [a], W.TUBE: [0.3 * a, a, b, 0.5, 4.0],
+               W.CONE: [0.2 * a, a, 0.3 * b, 1.2 * b, c, 0.0, TWO_PI], W.TRD: [a, 0.5 * a, b, 1.3 * b, c]}[kind]
+        q = rng.normal(size=4)
+        q /= np.linalg.norm(q)
+        kinds.append(kind)
+        pars.append(par)
+        xf.append(W.placement(W.quaternion_to_matrix(tuple(q)), rng.uniform(-spread, spread, 3)))
+    xf = np.stack(xf)
+    vo = O.Volume(O.Shape(W.BOX, [60, 60, 60]), [O.Shape(k, p) for k, p in zip(kinds, pars)], xf)
+    vgv = vg.Volume(vg.Shape(W.BOX, [60, 60, 60]), [vg.Shape(k, p) for k, p in zip(kinds, pars)], xf)
+
+    def band(x, y, z):
+        near = np.abs(vo.mother.sdf(x, y, z)) < 1e-6
+        for d, m in zip(vo.daughters, vo.xforms):
+            M = m.reshape(3, 4)
+            lx, ly, lz = (M[i, 0] * x + M[i, 1] * y + M[i, 2] * z + M[i, 3] for i in range(3))
+            near |= np.abs(d.sdf(lx, ly, lz)) < 1e-6
+        return near
+
+    t = W.draw_tracks(77 + nd, 100003, (0, 0, 0), (60, 60, 60), band)
+    for step_max in (W.STEP_MAX, 25.0):
+        so, ho = check_step(vo, vgv, t, step_max, "nd=%d step_max=%g" % (nd, step_max))
+    assert len(set(ho.tolist())) > min(nd, 40) // 2
+
+
 def test_volume_safety_config4(vg):
     nav = W.navigator_case()
     vo, vgv = build_volumes(vg, nav)
