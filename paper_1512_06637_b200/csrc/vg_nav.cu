@@ -22,7 +22,13 @@
 
 namespace vg {
 
-constexpr int kNavBlock = 128;
+#ifndef VG_NAV_BLOCK
+#define VG_NAV_BLOCK 256
+#endif
+#ifndef VG_NAV_MINB
+#define VG_NAV_MINB 3
+#endif
+constexpr int kNavBlock = VG_NAV_BLOCK;
 
 // one elected thread: arm the barrier with the byte count and issue the bulk copy global -> shared
 VG_DEV void tma_load_table(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
@@ -119,7 +125,7 @@ VG_DEV void coop_candidates(unsigned long long mk, int base, const unsigned char
 
 // ComputeStep; NC = chunks of 64 daughters (1, 2 or 4)
 template <int NC>
-__global__ void __launch_bounds__(kNavBlock) nav_step_kernel(const __grid_constant__ SolidU mother,
+__global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const __grid_constant__ SolidU mother,
                                                              const __grid_constant__ NavMeta meta,
                                                              const unsigned char *__restrict__ table, Tracks t,
                                                              double step_max, int64_t n, double *__restrict__ out,

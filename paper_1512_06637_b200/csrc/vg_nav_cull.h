@@ -25,7 +25,11 @@
 
 #if defined(__CUDA_ARCH__)
 #define VG_HD __host__ __device__ __forceinline__
+#ifdef VG_NAV_FAST_RCP
+#define VG_RCP_RN(a) vg::rcp(a)
+#else
 #define VG_RCP_RN(a) __drcp_rn(a)
+#endif
 #define VG_CLZ32(m) __clz(int(m))
 #elif defined(__CUDACC__)
 #define VG_HD __host__ __device__ inline
@@ -116,20 +120,8 @@ VG_HD bool nav_sphere_keep(const float4 s, float xf, float yf, float zf, float d
     return d2 <= s.w && (tca >= 0.f || vv <= s.w);
 }
 
-// ... for every candidate of a 32-bit half of a mask (32-bit words: a 64-bit find-first-set costs three times as much)
-VG_HD unsigned nav_sphere_refine32(const float4 *cull32, unsigned in, float xf, float yf, float zf, float dxf, float dyf,
-                                   float dzf)
-{
-    unsigned out = 0u;
-    while (in) {
-        const unsigned low = in & (0u - in);
-        in ^= low;
-        const int j = 31 - VG_CLZ32(low);
-        if (nav_sphere_keep(cull32[j], xf, yf, zf, dxf, dyf, dzf)) out |= low;
-    }
-    return out;
-}
-
+// ... for every candidate of one chunk.  The 64-bit mask is walked as two 32-bit words inside ONE loop (a 64-bit
+// find-first-set costs three times a 32-bit one, and two loops would each run to the slowest lane of the warp).
 template <int NC>
 VG_HD void nav_sphere_refine(const float4 *cull, double x, double y, double z, double dx, double dy, double dz,
                              unsigned long long (&m)[NC])
@@ -137,9 +129,18 @@ VG_HD void nav_sphere_refine(const float4 *cull, double x, double y, double z, d
     const float xf = float(x), yf = float(y), zf = float(z), dxf = float(dx), dyf = float(dy), dzf = float(dz);
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
-        const unsigned lo = nav_sphere_refine32(cull + 64 * c, unsigned(m[c]), xf, yf, zf, dxf, dyf, dzf);
-        const unsigned hi = nav_sphere_refine32(cull + 64 * c + 32, unsigned(m[c] >> 32), xf, yf, zf, dxf, dyf, dzf);
-        m[c] = (unsigned long long)hi << 32 | lo;
+        unsigned lo = unsigned(m[c]), hi = unsigned(m[c] >> 32), olo = 0u, ohi = 0u;
+        while (lo | hi) {
+            const bool in_lo = lo != 0u;
+            const unsigned w = in_lo ? lo : hi, low = w & (0u - w);
+            lo = in_lo ? lo ^ low : lo;
+            hi = in_lo ? hi : hi ^ low;
+            const int j = (in_lo ? 31 : 63) - VG_CLZ32(low);
+            const bool keep = nav_sphere_keep(cull[64 * c + j], xf, yf, zf, dxf, dyf, dzf);
+            olo |= (keep && in_lo) ? low : 0u;
+            ohi |= (keep && !in_lo) ? low : 0u;
+        }
+        m[c] = (unsigned long long)ohi << 32 | olo;
     }
 }
 
