@@ -274,8 +274,12 @@ int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, c
  * next pair of tracks while it evaluates the current one (16-byte aligned arrays only).  AUTO takes, per (solid,
  * query), the form that measured fastest (profiles/).
  * VG_OPT_HOST_CHUNK (default 0 = chosen from n): tracks per chunk of the host-buffer entry points' copy / compute
- * pipeline (clamped to 2^20). */
-typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2, VG_OPT_HOST_CHUNK = 3 } vg_option;
+ * pipeline (clamped to 2^20).
+ * VG_OPT_COOP_MAX_N (default VG_COOP_MAX_N_DEFAULT): queries of a full-phi polycone over at most this many tracks run as
+ *   the lanes-per-track kernel (a group of 4..32 lanes shares one track and splits its sections):
+ *   lowest latency for small batches, same results.  0 switches the form off. */
+typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2, VG_OPT_HOST_CHUNK = 3, VG_OPT_COOP_MAX_N = 4 } vg_option;
+#define VG_COOP_MAX_N_DEFAULT 32768
 enum { VG_FORM_AUTO = 0, VG_FORM_DIRECT = 1, VG_FORM_PIPELINED = 2, VG_FORM_STREAMING = 3 };
 int vg_set_option(int option, int64_t value);
 int64_t vg_get_option(int option); /* the value, or VG_ERR_ARG for an unknown option */

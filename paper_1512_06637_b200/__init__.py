@@ -82,6 +82,7 @@ OPT_PIPE_MIN_N = 0
 OPT_PDL = 1
 OPT_FORM = 2
 OPT_HOST_CHUNK = 3
+OPT_COOP_MAX_N = 4
 FORM_AUTO, FORM_DIRECT, FORM_PIPELINED, FORM_STREAMING = 0, 1, 2, 3
 INT64_MAX = 2 ** 63 - 1
 

@@ -55,6 +55,7 @@ std::atomic<int64_t> g_pipe_min_n{ int64_t(1) << 17 };
 std::atomic<int64_t> g_pdl{ 1 };
 std::atomic<int64_t> g_form{ VG_FORM_AUTO };
 std::atomic<int64_t> g_host_chunk{ 0 };
+std::atomic<int64_t> g_coop_max_n{ VG_COOP_MAX_N_DEFAULT };
 }
 extern "C" int64_t vg_launch_count(void) { return vg::g_launches.load(); }
 
@@ -76,6 +77,10 @@ extern "C" int vg_set_option(int option, int64_t value)
         if (value < VG_FORM_AUTO || value > VG_FORM_STREAMING) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_FORM must be 0..3");
         vg::g_form.store(value);
         return VG_OK;
+    case VG_OPT_COOP_MAX_N:
+        if (value < 0) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_COOP_MAX_N must be >= 0");
+        vg::g_coop_max_n.store(value);
+        return VG_OK;
     }
     return fail(VG_ERR_ARG, "vg_set_option: unknown option %d", option);
 }
@@ -87,6 +92,7 @@ extern "C" int64_t vg_get_option(int option)
     case VG_OPT_PDL: return vg::g_pdl.load();
     case VG_OPT_FORM: return vg::g_form.load();
     case VG_OPT_HOST_CHUNK: return vg::g_host_chunk.load();
+    case VG_OPT_COOP_MAX_N: return vg::g_coop_max_n.load();
     }
     return fail(VG_ERR_ARG, "vg_get_option: unknown option %d", option);
 }
@@ -106,11 +112,29 @@ static void upload_pcon_grid(vg_shape *s)
     pcon_grid_build(s->u.pcon, false, &geom, &masks, &rows);
     if (!s->u.pcon.w.full) pcon_grid_build(s->u.pcon, true, &geom2, &fmasks, &rows2); // same geometry, twice the columns
     const size_t mbytes = masks.size() * sizeof(unsigned long long), fbytes = fmasks.size() * sizeof(unsigned long long);
+    // the per-section records of the lanes-per-track kernels (vg_pcon_coop.cuh), in the same allocation
+    const PolyconeP &pc = s->u.pcon;
+    std::vector<PconCoopSec> coop(pc.nsec);
+    for (int k = 0; k < pc.nsec; ++k) {
+        const PconSec &c = pc.sec[k];
+        PconCoopSec &w = coop[k];
+        std::memset(&w, 0, sizeof w);
+        w.z0 = c.z0, w.z1 = c.z1, w.Ao = c.out.A, w.Bo = c.out.B, w.Ai = c.in.A, w.Bi = c.in.B, w.seco = c.out.sec, w.seci = c.in.sec;
+        w.ro0 = c.out.r0, w.ero = c.out.er, w.ilo = c.out.inv_l2, w.ri0 = c.in.r0, w.eri = c.in.er, w.ili = c.in.inv_l2;
+        w.flags = (pc.inner_mask >> k) & 1u;
+        if (k + 1 < pc.nsec && ((pc.step_mask >> k) & 1u)) {
+            const PconStep &t = pc.step[k];
+            w.sz = t.z, w.solo = t.olo, w.sohi = t.ohi, w.silo = t.ilo, w.sihi = t.ihi;
+            w.flags |= 2 | (t.oup ? 4 : 0) | (t.iup ? 8 : 0);
+        }
+    }
+    const size_t cbytes = coop.size() * sizeof(PconCoopSec), roff = (rows.size() + 15) / 16 * 16;
     unsigned char *blob = nullptr;
-    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + rows.size()) == cudaSuccess &&
+    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + roff + cbytes) == cudaSuccess &&
               cudaMemcpy(blob, masks.data(), mbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
               (fbytes == 0 || cudaMemcpy(blob + mbytes, fmasks.data(), fbytes, cudaMemcpyHostToDevice) == cudaSuccess) &&
-              cudaMemcpy(blob + mbytes + fbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) == cudaSuccess;
+              cudaMemcpy(blob + mbytes + fbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(blob + mbytes + fbytes + roff, coop.data(), cbytes, cudaMemcpyHostToDevice) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         if (blob) cudaFree(blob);
@@ -119,6 +143,7 @@ static void upload_pcon_grid(vg_shape *s)
     s->grid.masks = reinterpret_cast<const unsigned long long *>(blob);
     s->grid.face_masks = fbytes ? reinterpret_cast<const unsigned long long *>(blob + mbytes) : nullptr;
     s->grid.rows = blob + mbytes + fbytes;
+    s->grid.coop = reinterpret_cast<const PconCoopSec *>(blob + mbytes + fbytes + roff);
     s->grid.g = geom;
     s->grid_device = dev;
 }

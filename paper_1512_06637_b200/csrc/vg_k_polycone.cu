@@ -1,6 +1,7 @@
 // vg_k_polycone.cu -- instantiates the query kernels of the polycone: the run-time-flag form, the full-phi
 // specialisation, and the ordered-walk kernels (vg_pcon_walk.cuh) that serve DistanceToIn and the safeties of a
 // full-phi polycone when the arrays are 16-byte aligned (VG_FORM_AUTO; any forced form runs the generic kernels).
+#include "vg_pcon_coop.cuh"
 #include "vg_pcon_walk.cuh"
 
 namespace vg {
@@ -10,6 +11,16 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
 {
     if (n <= 0) return cudaSuccess;
     if (p.w.full) {
+        // small batches: a group of lanes per track (vg_pcon_coop.cuh), any alignment
+        if (g.coop && g_form.load(std::memory_order_relaxed) == 0 && n <= g_coop_max_n.load(std::memory_order_relaxed)) {
+            switch (q) {
+            case qInside: return launch_pcon_coop<qInside>(p, g, t, step_max, n, out, s);
+            case qDistIn: return launch_pcon_coop<qDistIn>(p, g, t, step_max, n, out, s);
+            case qDistOut: return launch_pcon_coop<qDistOut>(p, g, t, step_max, n, out, s);
+            case qSafeIn: return launch_pcon_coop<qSafeIn>(p, g, t, step_max, n, out, s);
+            case qSafeOut: return launch_pcon_coop<qSafeOut>(p, g, t, step_max, n, out, s);
+            }
+        }
         if (vec && g_form.load(std::memory_order_relaxed) == 0) {
             double *o = static_cast<double *>(out);
             if (q == qDistIn) return launch_pcon_walk<qDistIn, false>(p, g, t, step_max, n, o, s);

@@ -109,7 +109,17 @@ struct PconGridGeom {
     double inv_cr, inv_cz, zg0;
 };
 
+// One record per section for the lanes-per-track kernels (vg_pcon_coop.cuh), in device memory: a lane reads the record of
+// ITS section, so the table cannot live in the constant bank (divergent indices serialise there).  20 doubles.
+struct alignas(16) PconCoopSec {
+    double z0, z1, Ao, Bo, Ai, Bi, seco, seci; // slab, generators r = A + B z of the outer / inner patch, sqrt(1 + B^2)
+    double ro0, ero, ilo, ri0, eri, ili;       // outline edges: (r0, z0) -> (r0 + er, z1), 1 / |edge|^2
+    double sz, solo, sohi, silo, sihi;         // the z step on top of this section (flags & 2): PconStep z, olo, ohi, ilo, ihi
+    int flags, pad;                            // 1: inner surface, 2: step above, 4: step.oup, 8: step.iup
+};
+
 struct PconGrid {
+    const PconCoopSec *coop;         // [nsec]; NULL: not uploaded, the thread-per-track kernels serve every batch size
     const unsigned long long *masks; // [kPconGridZ][kPconGridR]; NULL: no grid, the ordered walk serves the safeties
     const unsigned long long *face_masks; // phi cut only: [kPconGridZ][2 kPconGridR] over u in [-R, R), every outline edge
     const unsigned char *rows;       // [kPconGridZ]

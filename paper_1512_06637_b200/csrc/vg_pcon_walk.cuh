@@ -545,8 +545,13 @@ __global__ void __launch_bounds__(kWalkBlock, VG_WALK_MINB)
     pdl_launch_dependents();
     __syncthreads();
     pdl_wait();
+    // every CTA owns ONE contiguous range of track pairs, the same number for all (rounded to a warp's row of 32): with
+    // whole 512-track tiles handed out round-robin, a batch of 1.15 resident waves (n = 2^18) took two full wave times
     const int64_t npairs = (n + 1) >> 1;
-    for (int64_t j = int64_t(blockIdx.x) * kWalkBlock + threadIdx.x; j < npairs; j += int64_t(gridDim.x) * kWalkBlock) {
+    int64_t per = (npairs + gridDim.x - 1) / gridDim.x;
+    per = (per + 31) / 32 * 32;
+    const int64_t lo = int64_t(blockIdx.x) * per, hi = lo + per < npairs ? lo + per : npairs;
+    for (int64_t j = lo + threadIdx.x; j < hi; j += kWalkBlock) {
         const int64_t i = 2 * j;
         if (i + 1 < n) {
             double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
