@@ -6,6 +6,7 @@ host numpy arrays out.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_
 --impl reference legs may import this package; it imports nothing of the CUDA path.
 """
 import ctypes as C
+import os
 
 import numpy as np
 
@@ -68,6 +69,8 @@ _LIBS = {}
 def _lib(long_double=False):
     if long_double not in _LIBS:
         paths = _build.build()
+        if not long_double and os.environ.get("ORACLE_SANITIZE") == "1":  # ASan + UBSan build (tests/test_oracle_sanitizers.py)
+            paths = (_build.build_sanitized(), paths[1])
         _LIBS[long_double] = _load(paths[1] if long_double else paths[0])
     return _LIBS[long_double]
 

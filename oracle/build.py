@@ -10,6 +10,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "vg_oracle.c")
 LIB = os.path.join(HERE, "liboracle.so")
 LIB_LD = os.path.join(HERE, "liboracle_ld.so")
+LIB_SAN = os.path.join(HERE, "liboracle_san.so")  # AddressSanitizer + UndefinedBehaviorSanitizer build
+SAN_FLAGS = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+             "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall", "-Wextra"]
 CFLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c99", "-Wall", "-Wextra"]
 
 
@@ -23,6 +26,18 @@ def build(force=False):
             cmd = ["gcc"] + CFLAGS + extra + [SRC, "-o", lib, "-lm"]
             subprocess.run(cmd, check=True)
     return LIB, LIB_LD
+
+
+def build_sanitized(force=False):
+    """The same source with ASan + UBSan.  A process that loads it must have the ASan runtime loaded first
+    (LD_PRELOAD=$(gcc -print-file-name=libasan.so)); oracle/__init__.py loads it when ORACLE_SANITIZE=1."""
+    if force or _stale(LIB_SAN):
+        subprocess.run(["gcc"] + SAN_FLAGS + [SRC, "-o", LIB_SAN, "-lm"], check=True)
+    return LIB_SAN
+
+
+def asan_runtime():
+    return subprocess.run(["gcc", "-print-file-name=libasan.so"], check=True, capture_output=True, text=True).stdout.strip()
 
 
 if __name__ == "__main__":

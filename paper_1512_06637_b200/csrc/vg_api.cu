@@ -227,7 +227,7 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
     case VG_POLYCONE: {
         PconGrid g = s->grid;
         int dev = -1;
-        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr;
         e = launch_polycone(q, s->u.pcon, g, t, step_max, n, out, vec, st);
         break;
     }
@@ -289,7 +289,7 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
         if (rcp != VG_OK) return rcp;
         PconGrid g = s->grid;
         int dev = -1;
-        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr;
         Tracks t{ x, y, z, dx, dy, dz };
         AllOut o{ cls, dist_in, dist_out, safety_in, safety_out };
         cudaError_t e = launch_polycone_all(s->u.pcon, g, t, step_max, n, o, vec, static_cast<cudaStream_t>(stream));
@@ -595,12 +595,26 @@ extern "C" void vg_volume_destroy(vg_volume *v)
     delete v;
 }
 
+// a volume / world lives on the device it was created on: a query made while another device is current would hand
+// that device foreign pointers
+static int check_device(int created_on, const char *fn)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(VG_ERR_CUDA, "%s: no current CUDA device", fn);
+    if (dev != created_on) return fail(VG_ERR_ARG, "%s: the handle was created on device %d, the current device is %d", fn, created_on, dev);
+    return VG_OK;
+}
+
 extern "C" int vg_compute_step(const vg_volume *v, const double *x, const double *y, const double *z, const double *dx,
                                const double *dy, const double *dz, double step_max, int64_t n, double *step,
                                int32_t *hit, void *stream)
 {
     const char *fn = "vg_compute_step";
     if (!v) return fail(VG_ERR_ARG, "%s: volume is NULL", fn);
+    if (n > 0 && !v->general) {
+        int rcd = check_device(v->device, fn);
+        if (rcd != VG_OK) return rcd;
+    }
     const void *ptrs[6] = { x, y, z, dx, dy, dz };
     bool vec = false;
     int rc = check_arrays(fn, ptrs, 6, 8, step, n, &vec);
@@ -621,6 +635,10 @@ extern "C" int vg_volume_safety(const vg_volume *v, const double *x, const doubl
 {
     const char *fn = "vg_volume_safety";
     if (!v) return fail(VG_ERR_ARG, "%s: volume is NULL", fn);
+    if (n > 0 && !v->general) {
+        int rcd = check_device(v->device, fn);
+        if (rcd != VG_OK) return rcd;
+    }
     const void *ptrs[3] = { x, y, z };
     bool vec = false;
     int rc = check_arrays(fn, ptrs, 3, 8, safety, n, &vec);
@@ -885,6 +903,10 @@ extern "C" int vg_world_locate(const vg_world *w, const double *x, const double 
 {
     const char *fn = "vg_world_locate";
     if (!w) return fail(VG_ERR_ARG, "%s: world is NULL", fn);
+    if (n > 0) {
+        int rcd = check_device(w->device, fn);
+        if (rcd != VG_OK) return rcd;
+    }
     const void *ptrs[3] = { x, y, z };
     bool vec = false;
     int rc = check_arrays(fn, ptrs, 3, 4, node, n, &vec);
@@ -901,6 +923,10 @@ extern "C" int vg_world_step(const vg_world *w, const int32_t *node, const doubl
 {
     const char *fn = "vg_world_step";
     if (!w) return fail(VG_ERR_ARG, "%s: world is NULL", fn);
+    if (n > 0) {
+        int rcd = check_device(w->device, fn);
+        if (rcd != VG_OK) return rcd;
+    }
     const void *ptrs[6] = { x, y, z, dx, dy, dz };
     bool vec = false;
     int rc = check_arrays(fn, ptrs, 6, 8, step, n, &vec);
@@ -919,6 +945,10 @@ extern "C" int vg_world_safety(const vg_world *w, const int32_t *node, const dou
 {
     const char *fn = "vg_world_safety";
     if (!w) return fail(VG_ERR_ARG, "%s: world is NULL", fn);
+    if (n > 0) {
+        int rcd = check_device(w->device, fn);
+        if (rcd != VG_OK) return rcd;
+    }
     const void *ptrs[3] = { x, y, z };
     bool vec = false;
     int rc = check_arrays(fn, ptrs, 3, 8, safety, n, &vec);
