@@ -225,6 +225,13 @@ class Case:
             self.handle.safety(self.nodes[k], *s[:3], out=self.outd[k])
         elif q == "compute_step":
             self.handle.compute_step(*s, step_max=W.STEP_MAX, step=self.outd[k], hit=self.outi[k])
+        elif q.startswith("probe:"):  # the arithmetic-free kernel of the same loads, store, grid and form (vg_probe_stream)
+            pq = q[6:]
+            out = self.outi[k] if pq == "inside" else self.outd[k]
+            if pq in ("distance_to_in", "distance_to_out"):
+                self.vg.vg_probe_stream(pq, *s, out=out)
+            else:
+                self.vg.vg_probe_stream(pq, *s[:3], out=out)
         elif q == "inside":
             self.handle.inside(*s[:3], out=self.outi[k])
         elif q in ("distance_to_in", "distance_to_out"):
@@ -608,6 +615,9 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, have, headline_rows, min_ms, emi
             if 48 * n <= 0.5 * L2_BYTES:  # the hot variant: same buffers every launch, the batch stays in L2
                 hot_s = tq(case, q, hot=True)
                 e.update({"hot_us_per_launch": hot_s * 1e6, "hot_tracks_per_s": n / hot_s})
+            if k in (0, 1) or n <= 262144:  # the size-matched memory ceiling: the same loads and store without the arithmetic
+                ceil_s = tq3(case, "probe:" + q)
+                e.update({"mem_ceiling_us": ceil_s * 1e6, "frac_of_mem_ceiling": ceil_s / (e["us_per_launch"] * 1e-6)})
             if n <= 262144:  # launch-bound sizes: the bound a single launch can reach is max(bytes / BW, empty launch)
                 ideal = max(BYTES[q] * n / (hbm_peak * 1e9), floor_s)
                 e.update({"empty_launch_us": floor_s * 1e6, "latency_adjusted_bound_us": ideal * 1e6,
@@ -748,7 +758,8 @@ def per_config_rows(detail, fma_rate):
     """<= 10 short rows for the compact line: per (config, shape) the query FURTHEST below its bound.  us = one launch
     (cold inputs), f = fraction of the measured HBM copy rate, f8 = fraction of the nominal 8 TB/s, fp64 = SURVEY 8(d)'s
     algorithmic FP64 operations / s over the FP64 rate measured in this run (ALU-bound rows), lat = latency-adjusted
-    fraction max(bytes / BW, empty launch) / measured (launch-bound sizes)."""
+    fraction max(bytes / BW, empty launch) / measured (launch-bound sizes), cl = duration of the arithmetic-free kernel
+    with the same loads, store, grid and form on the same buffers (vg_probe_stream) / measured."""
     groups = {}
     for e in detail:
         if e.get("row") or not isinstance(e.get("config"), int) or str(e["query"]).startswith("all five"):
@@ -767,6 +778,8 @@ def per_config_rows(detail, fma_rate):
             r["fp64"] = w["fp64_frac"]
         else:
             r["f"], r["f8"] = w["hbm_frac"], w["hbm_gbs"] / HBM_NOMINAL_GBS
+        if "frac_of_mem_ceiling" in w:  # cl = the size-matched memory ceiling (same loads / store / grid, no arithmetic) / measured
+            r["cl"] = w["frac_of_mem_ceiling"]
         keep.append(_sig(r, 3))
     return keep
 

@@ -107,8 +107,11 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  * "logical operations"; readings R27-R29 in DESIGN.md).  A sits in the frame of C; `xform_b` (HOST,
  * 12 doubles, row-major 3x4 [R | b], orthonormal R) maps the frame of C to the frame of B.  A and B: box, orb, tube,
  * cone, trd, or a boolean made by this call (reading R31: a CSG tree; at most 8 primitives per tree, VG_ERR_PARAM
- * beyond; a polycone operand gives VG_ERR_ARG); their constants are copied.  Two primitives run kernels specialised
- * per pair of kinds, a tree is flattened into a program over its primitives and runs the general kernel (vg_csg.cu).
+ * beyond); their constants are copied.  Two primitives run kernels specialised per pair of kinds, a tree is flattened
+ * into a program over its primitives and runs the general kernel (vg_csg.cu).  A or B may also be a POLYCONE when the
+ * other one is a primitive or a polycone: its constants are placed in memory of the CURRENT device (VG_ERR_CUDA
+ * without one; queries must run on that device) and the general two-operand kernel answers (vg_boolx.cu); such a
+ * boolean is neither an operand of another boolean nor a node of a world / daughter of a volume (VG_ERR_ARG).
  * The result is a vg_shape of kind VG_BOOLEAN that every query below accepts ("operand" read recursively for a tree):
  *   Inside       combines the operands' classes: union INSIDE if either is, OUTSIDE if both are; intersection INSIDE if
  *                both are, OUTSIDE if either is; subtraction (A minus B) INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A

@@ -171,13 +171,14 @@ extern "C" void vg_shape_destroy(vg_shape *s)
 {
     if (!s) return;
     if (s->grid.masks) cudaFree(const_cast<unsigned long long *>(s->grid.masks)); // rows live in the same allocation
+    if (s->ext_blob) cudaFree(s->ext_blob);
     delete s;
 }
 
 extern "C" int vg_shape_kind(const vg_shape *s)
 {
     if (!s) return fail(VG_ERR_ARG, "vg_shape_kind: NULL");
-    return s->kind == kCsg ? int(VG_BOOLEAN) : s->kind; // a nested boolean is a boolean to the caller
+    return (s->kind == kCsg || s->kind == kBoolX) ? int(VG_BOOLEAN) : s->kind; // every form of boolean is a boolean to the caller
 }
 
 // ------------------------------------------------------------------------------------------------- queries
@@ -200,6 +201,16 @@ static int check_arrays(const char *fn, const void *const *ptrs, int count, size
     if (!aligned(out, out_align)) return fail(VG_ERR_ARG, "%s: output array misaligned", fn);
     v = v && aligned(out, 2 * out_align);
     *vec = v;
+    return VG_OK;
+}
+
+// a volume / world lives on the device it was created on: a query made while another device is current would hand
+// that device foreign pointers
+static int check_device(int created_on, const char *fn)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return fail(VG_ERR_CUDA, "%s: no current CUDA device", fn);
+    if (dev != created_on) return fail(VG_ERR_ARG, "%s: the handle was created on device %d, the current device is %d", fn, created_on, dev);
     return VG_OK;
 }
 
@@ -233,6 +244,12 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
     }
     case VG_BOOLEAN: e = launch_boolean(q, s->u.boolean, t, step_max, n, out, st); break;
     case kCsg: e = launch_csg(q, s->u.csg, t, step_max, n, out, st); break;
+    case kBoolX: {
+        int rcd = check_device(s->ext_device, fn);
+        if (rcd != VG_OK) return rcd;
+        e = launch_boolx(q, s->u.boolean, t, step_max, n, out, st);
+        break;
+    }
     }
     if (e != cudaSuccess) return fail_cuda(e, fn);
     return VG_OK;
@@ -595,16 +612,6 @@ extern "C" void vg_volume_destroy(vg_volume *v)
     delete v;
 }
 
-// a volume / world lives on the device it was created on: a query made while another device is current would hand
-// that device foreign pointers
-static int check_device(int created_on, const char *fn)
-{
-    int dev = -1;
-    if (cudaGetDevice(&dev) != cudaSuccess) return fail(VG_ERR_CUDA, "%s: no current CUDA device", fn);
-    if (dev != created_on) return fail(VG_ERR_ARG, "%s: the handle was created on device %d, the current device is %d", fn, created_on, dev);
-    return VG_OK;
-}
-
 extern "C" int vg_compute_step(const vg_volume *v, const double *x, const double *y, const double *z, const double *dx,
                                const double *dy, const double *dz, double step_max, int64_t n, double *step,
                                int32_t *hit, void *stream)
@@ -732,7 +739,34 @@ extern "C" int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, c
     if (!s) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
     std::memset(s, 0, sizeof *s);
     int rc = VG_OK;
-    if (a->kind < VG_POLYCONE && b->kind < VG_POLYCONE) { // two primitives: the specialised kernels of vg_bool.cu
+    if ((a->kind == VG_POLYCONE && b->kind <= VG_POLYCONE) || (b->kind == VG_POLYCONE && a->kind <= VG_POLYCONE)) {
+        // a polycone operand (vg_boolx.cu): its constants go to device memory, the operand record points at them
+        s->kind = kBoolX;
+        BoolP &c = s->u.boolean;
+        c.op = op;
+        std::memcpy(c.X, xform_b, sizeof c.X);
+        const vg_shape *opnd[2] = { a, b };
+        SolidU *rec[2] = { &c.a, &c.b };
+        const int npc = (a->kind == VG_POLYCONE) + (b->kind == VG_POLYCONE);
+        PolyconeP *blob = nullptr;
+        cudaError_t e = cudaGetDevice(&s->ext_device);
+        if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), size_t(npc) * sizeof(PolyconeP));
+        if (e != cudaSuccess) rc = fail_cuda(e, "vg_boolean_create: a polycone operand needs device memory");
+        s->ext_blob = blob;
+        for (int i = 0, k = 0; i < 2 && rc == VG_OK; ++i) {
+            if (opnd[i]->kind == VG_POLYCONE) {
+                e = cudaMemcpy(blob + k, &opnd[i]->u.pcon, sizeof(PolyconeP), cudaMemcpyHostToDevice);
+                if (e != cudaSuccess) rc = fail_cuda(e, "vg_boolean_create: cudaMemcpy");
+                rec[i]->kind = kPolycone;
+                rec[i]->u.pcon = blob + k++;
+            } else {
+                rc = to_solid(opnd[i], rec[i], "operand");
+            }
+        }
+        if (rc != VG_OK && blob) cudaFree(blob);
+    } else if (a->kind == kBoolX || b->kind == kBoolX || a->kind == VG_POLYCONE || b->kind == VG_POLYCONE) {
+        rc = fail(VG_ERR_ARG, "%s: a polycone may be an operand of a boolean of two solids, not a leaf of a nested tree", fn);
+    } else if (a->kind < VG_POLYCONE && b->kind < VG_POLYCONE) { // two primitives: the specialised kernels of vg_bool.cu
         s->kind = VG_BOOLEAN;
         BoolP &c = s->u.boolean;
         c.op = op;
@@ -800,6 +834,8 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         const double *m = xforms + 12 * i;
         if (!all_finite(m, 12)) return fail(VG_ERR_PARAM, "%s: non-finite transform of node %d", fn, i);
         if (!rigid(m)) return fail(VG_ERR_PARAM, "%s: rotation of node %d is not orthonormal", fn, i);
+        if (shapes[i]->kind == kBoolX)
+            return fail(VG_ERR_ARG, "%s: node %d is a boolean with a polycone operand: not supported as a placed solid", fn, i);
         if (shapes[i]->kind == VG_POLYCONE) { // R30: constants in a side array, the record keeps kind + index
             N.s.kind = kPolycone;
             N.ext = int(pcons.size());

@@ -44,6 +44,29 @@ VG_DEV double solid_next(const SolidU &s, bool inside, double x, double y, doubl
     return ahead(t) ? dmax(t, 0.0) : inf(); // a crossing behind the point, a wrong-side -1 or a NaN is "no crossing"
 }
 
+// ---- operands that may be polycones (X = true: vg_boolx.cu): kind == kPolycone reads the constants through u.pcon ----
+template <bool X> VG_DEV int opnd_inside(const SolidU &s, double x, double y, double z)
+{
+    if (X && s.kind == kPolycone) return Polycone::inside(*s.u.pcon, x, y, z);
+    return solid_inside(s, x, y, z);
+}
+
+template <bool X> VG_DEV double opnd_sdf(const SolidU &s, double x, double y, double z)
+{
+    if (X && s.kind == kPolycone) return Polycone::safety(*s.u.pcon, x, y, z);
+    return solid_sdf(s, x, y, z);
+}
+
+template <int K, bool X>
+VG_DEV double opnd_next(const SolidU &s, bool inside, double x, double y, double z, double dx, double dy, double dz)
+{
+    if (X && s.kind == kPolycone) { // the polycone's distances pick crossings by their sense, like every solid's (R32)
+        const double t = inside ? Polycone::dist_out(*s.u.pcon, x, y, z, dx, dy, dz) : Polycone::dist_in(*s.u.pcon, x, y, z, dx, dy, dz);
+        return ahead(t) ? dmax(t, 0.0) : inf();
+    }
+    return solid_next<K>(s, inside, x, y, z, dx, dy, dz);
+}
+
 VG_DEV bool bool_member(int op, bool ina, bool inb)
 {
     return op == kUnion ? (ina || inb) : (op == kIntersection ? (ina && inb) : (ina && !inb));
@@ -69,18 +92,18 @@ VG_DEV void bool_to_b(const BoolP &p, double x, double y, double z, double &bx, 
     bz = fma(m[8], x, fma(m[9], y, fma(m[10], z, m[11])));
 }
 
-VG_DEV int bool_inside_pt(const BoolP &p, double x, double y, double z) // R27
+template <bool X = false> VG_DEV int bool_inside_pt(const BoolP &p, double x, double y, double z) // R27
 {
     double bx, by, bz;
     bool_to_b(p, x, y, z, bx, by, bz);
-    return bool_classify(p.op, solid_inside(p.a, x, y, z), solid_inside(p.b, bx, by, bz));
+    return bool_classify(p.op, opnd_inside<X>(p.a, x, y, z), opnd_inside<X>(p.b, bx, by, bz));
 }
 
-VG_DEV double bool_sdf_pt(const BoolP &p, double x, double y, double z) // R29
+template <bool X = false> VG_DEV double bool_sdf_pt(const BoolP &p, double x, double y, double z) // R29
 {
     double bx, by, bz;
     bool_to_b(p, x, y, z, bx, by, bz);
-    const double sa = solid_sdf(p.a, x, y, z), sb = solid_sdf(p.b, bx, by, bz);
+    const double sa = opnd_sdf<X>(p.a, x, y, z), sb = opnd_sdf<X>(p.b, bx, by, bz);
     return p.op == kUnion ? dmin(sa, sb) : (p.op == kIntersection ? dmax(sa, sb) : dmax(sa, -sb));
 }
 
@@ -92,13 +115,13 @@ VG_DEV double bool_sdf_pt(const BoolP &p, double x, double y, double z) // R29
 // at the start is SURFACE has no state yet: it starts as "outside", and if its entering crossing is not AT the start
 // (t <= kRayTol after the clamp) the crossing the point sits on is a leaving one and the operand was inside (R32: the
 // sense of motion decides); that operand's event at t ~ 0 then runs through the loop like any other.
-template <int KA, int KB>
+template <int KA, int KB, bool X = false>
 VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, double z, double dx, double dy, double dz)
 {
     const double *m = p.X;
     double bx, by, bz;
     bool_to_b(p, x, y, z, bx, by, bz);
-    const int ca = solid_inside(p.a, x, y, z), cb = solid_inside(p.b, bx, by, bz);
+    const int ca = opnd_inside<X>(p.a, x, y, z), cb = opnd_inside<X>(p.b, bx, by, bz);
     const int cls = bool_classify(p.op, ca, cb);
     if ((!to_out && cls == cInside) || (to_out && cls == cOutside)) return -1.0;
     const double bdx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
@@ -109,8 +132,8 @@ VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, dou
     double tt = 0.0;
 #pragma unroll 1
     for (int it = 0; it < kBoolMaxEvents; ++it) {
-        const double ea = solid_next<KA>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
-        const double eb = solid_next<KB>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
+        const double ea = opnd_next<KA, X>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
+        const double eb = opnd_next<KB, X>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
         if (pend_a || pend_b) { // first pass only, and only for a start on an operand's surface
             const bool fix_a = pend_a && !(ea <= kRayTol), fix_b = pend_b && !(eb <= kRayTol);
             pend_a = pend_b = false;
@@ -133,7 +156,7 @@ VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, dou
 #define VG_BOOL_MINB 3
 #endif
 
-template <int Q, int KA, int KB>
+template <int Q, int KA, int KB, bool X = false>
 __global__ void __launch_bounds__(kBoolBlock, (Q == qDistIn || Q == qDistOut) ? VG_BOOL_MINB : 1)
     bool_kernel(const __grid_constant__ BoolP p, Tracks t, double step_max, int64_t n, void *out)
 {
@@ -143,13 +166,13 @@ __global__ void __launch_bounds__(kBoolBlock, (Q == qDistIn || Q == qDistOut) ? 
     if (i >= n) return;
     const double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
     if (Q == qSafeIn || Q == qSafeOut) {
-        const double s = bool_sdf_pt(p, x, y, z);
+        const double s = bool_sdf_pt<X>(p, x, y, z);
         stg1(static_cast<double *>(out) + i, Q == qSafeIn ? s : -s);
     } else if (Q == qInside) {
-        stg1i(static_cast<int32_t *>(out) + i, bool_inside_pt(p, x, y, z));
+        stg1i(static_cast<int32_t *>(out) + i, bool_inside_pt<X>(p, x, y, z));
     } else {
         const double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
-        const double r = bool_distance<KA, KB>(p, Q == qDistOut, x, y, z, dx, dy, dz);
+        const double r = bool_distance<KA, KB, X>(p, Q == qDistOut, x, y, z, dx, dy, dz);
         stg1(static_cast<double *>(out) + i, r <= step_max ? r : inf());
     }
 }

@@ -26,6 +26,10 @@ struct vg_shape {
     // no device was available at create; the safeties then run the ordered walk)
     PconGrid grid;
     int grid_device;
+    // kBoolX only: the polycone operands' constants in device memory of `ext_device` (u.boolean's operand records point
+    // into it); owned by the shape
+    void *ext_blob;
+    int ext_device;
 };
 
 // ------------------------------------------------------------------------------------------- derived constants

@@ -595,6 +595,9 @@ cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *tabl
 // boolean solids (vg_bool.cu)
 cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
 
+// booleans with a polycone operand (vg_boolx.cu)
+cudaError_t launch_boolx(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
+
 // nested booleans (vg_csg.cu)
 cudaError_t launch_csg(int q, const CsgP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
 

@@ -11,7 +11,8 @@ constexpr int kMaxZ = 32;       // polycone z-planes
 constexpr int kMaxSec = kMaxZ - 1;
 
 enum Kind : int { kBox = 0, kOrb = 1, kTube = 2, kCone = 3, kTrd = 4, kPolycone = 5, kBoolean = 6,
-                  kCsg = 7 /* internal: a boolean whose operands include booleans (reading R31); reported as VG_BOOLEAN */ };
+                  kCsg = 7 /* internal: a boolean whose operands include booleans (reading R31); reported as VG_BOOLEAN */,
+                  kBoolX = 8 /* internal: a boolean of two solids of which at least one is a polycone; reported as VG_BOOLEAN */ };
 enum Query : int { qInside = 0, qDistIn = 1, qDistOut = 2, qSafeIn = 3, qSafeOut = 4 };
 
 // phi segment [sphi, sphi + dphi]; e0, e1 = unit vectors of the two bounding half-planes (reading R11)
@@ -126,7 +127,9 @@ struct PconGrid {
     PconGridGeom g;
 };
 
-// a solid that may be a mother or a daughter of a volume (every kind except the polycone)
+// a solid that may be a mother or a daughter of a volume (every kind except the polycone), or an operand of a boolean
+// (there a polycone too: kind == kPolycone and u.pcon points at its constants in device memory, vg_boolx.cu)
+struct PolyconeP;
 struct SolidU {
     int kind;
     int pad;
@@ -136,6 +139,7 @@ struct SolidU {
         TubeP tube;
         ConeP cone;
         TrdP trd;
+        const PolyconeP *pcon;
     } u;
 };
 

@@ -102,9 +102,14 @@ def test_boolean_create_rejects_bad_input(vg):
     with pytest.raises(vg.VgError):
         vg.Boolean(vg.UNION, a, a, [2, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0])
     pc = vg.Shape(W.POLYCONE, W.polycone_params(1))
-    with pytest.raises(vg.VgError):
-        vg.Boolean(vg.UNION, a, pc, ident)
     c = vg.Boolean(vg.UNION, a, a, ident)
+    bp = vg.Boolean(vg.UNION, a, pc, ident)  # a polycone may be an operand of a boolean of two solids ...
+    assert bp.kind == vg.BOOLEAN
+    for bad in ((c, pc), (pc, c), (bp, a), (a, bp)):  # ... but not a leaf of a nested tree
+        with pytest.raises(vg.VgError):
+            vg.Boolean(vg.UNION, bad[0], bad[1], ident)
+    with pytest.raises(vg.VgError):  # ... and such a boolean is not a placed solid
+        vg.Volume(vg.Shape(W.BOX, [100, 100, 100]), [bp], [ident])
     assert vg.Boolean(vg.UNION, a, c, ident).kind == vg.BOOLEAN  # a boolean operand makes a nested boolean (R31)
     vg.Volume(vg.Shape(W.BOX, [10, 10, 10]), [c], [ident])  # a boolean daughter is served by the world kernels (R30)
 
@@ -281,3 +286,60 @@ def test_nested_boolean_as_a_world_node_and_a_daughter(vg):
     sv, hv = vol.compute_step(*dev(tr), W.STEP_MAX)
     assert_real_close(sv.cpu().numpy(), so[root], "tree daughter step")
     assert_int_equal(hv.cpu().numpy(), np.where(no[root] < 0, -1, no[root] - 1), "tree daughter hit")
+
+
+# ---------------------------------------------------------------------------------- polycone operands (vg_boolx.cu)
+
+def _pcon_cases():
+    two_pi = 2 * np.pi
+    pc10 = W.polycone_params(W.config_seed(3, 0))                       # the configs[3] polycone, rmax 10..30, z in +-50
+    pcw = [0.4, 4.0] + pc10[2:]                                        # the same with a phi cut
+    small = [0.0, two_pi, 4.0, -8.0, 1.0, 4.0, -2.0, 2.0, 7.0, 3.0, 0.5, 5.0, 9.0, 0.0, 3.0]
+    q = np.array([0.18, -0.31, 0.22, 0.9])
+    Q = W.quaternion_to_matrix(tuple(q / np.linalg.norm(q)))
+    return [
+        ("pcon_minus_box", W.SUBTRACTION, (W.POLYCONE, pc10), (W.BOX, [12.0, 40.0, 30.0]), W.placement(Q, (8.0, 3.0, -5.0)), 60.0),
+        ("box_intersection_pcon", W.INTERSECTION, (W.BOX, [25.0, 18.0, 45.0]), (W.POLYCONE, pc10), W.placement(Q, (4.0, -3.0, 6.0)), 60.0),
+        ("pcon_union_pcon", W.UNION, (W.POLYCONE, small), (W.POLYCONE, small), W.placement(Q, (3.0, 2.0, 4.0)), 16.0),
+        ("tube_minus_pcon_wedge", W.SUBTRACTION, (W.TUBE, [0.0, 28.0, 45.0, 0.0, two_pi]), (W.POLYCONE, pcw), W.placement(np.eye(3), (0.0, 0.0, 0.0)), 60.0),
+        ("pcon_step_union_orb", W.UNION, (W.POLYCONE, W.STEPPED_POLYCONE), (W.ORB, [7.0]), W.placement(Q, (6.0, 0.0, 9.0)), 22.0),
+    ]
+
+
+@pytest.mark.parametrize("case", _pcon_cases(), ids=lambda c: c[0])
+def test_boolean_with_polycone_operands_matches_the_oracle(vg, case):
+    """boolean operations over the elementary bodies -- the polycone included.  All five queries, a finite
+    physics step, the fused call and tracks that start ON the boolean's surface (R32), against the oracle."""
+    name, op, (ka, pa), (kb, pb), xf, half = case
+    co = O.Boolean(op, O.Shape(ka, pa), O.Shape(kb, pb), xf)
+    cg = vg.Boolean(op, vg.Shape(ka, pa), vg.Shape(kb, pb), xf)
+    assert cg.kind == vg.BOOLEAN
+    M = np.asarray(xf).reshape(3, 4)
+
+    def band(x, y, z):
+        L = M[:, :3] @ np.stack([x, y, z]) + M[:, 3:4]
+        return (np.abs(co.a.sdf(x, y, z)) < W.SURFACE_BAND) | (np.abs(co.b.sdf(L[0], L[1], L[2])) < W.SURFACE_BAND)
+
+    t = W.draw_tracks(900 + len(name), 100003, (0.0, 0.0, 0.0), (half, half, half), band)
+    dt = dev(t)
+    cls = co.inside(*t[:3])
+    assert (cls == O.INSIDE).any() and (cls == O.OUTSIDE).any()
+    assert_int_equal(cg.inside(*dt[:3]).cpu().numpy(), cls, name + " inside")
+    for q in ("distance_to_in", "distance_to_out"):
+        for step_max in (W.STEP_MAX, 9.0):
+            assert_real_close(getattr(cg, q)(*dt, step_max).cpu().numpy(), getattr(co, q)(*t, step_max), "%s %s" % (name, q))
+    for q in ("safety_to_in", "safety_to_out"):
+        assert_real_close(getattr(cg, q)(*dt[:3]).cpu().numpy(), getattr(co, q)(*t[:3]), "%s %s" % (name, q))
+    fused = cg.query_all(*dt, W.STEP_MAX)
+    assert_int_equal(fused[0].cpu().numpy(), cls, name + " fused inside")
+    assert_real_close(fused[1].cpu().numpy(), co.distance_to_in(*t, W.STEP_MAX), name + " fused din")
+    # border starts: move the outside tracks that hit onto their crossing and ask again (no nudge)
+    x, y, z, dx, dy, dz = t
+    din = co.distance_to_in(x, y, z, dx, dy, dz)
+    hit = np.isfinite(din) & (din > 0)
+    ts = tuple(np.ascontiguousarray(a) for a in (x[hit] + din[hit] * dx[hit], y[hit] + din[hit] * dy[hit], z[hit] + din[hit] * dz[hit],
+                                                 dx[hit], dy[hit], dz[hit]))
+    ds = dev(ts)
+    assert_int_equal(cg.inside(*ds[:3]).cpu().numpy(), co.inside(*ts[:3]), name + " border inside")
+    for q in ("distance_to_in", "distance_to_out"):
+        assert_real_close(getattr(cg, q)(*ds, W.STEP_MAX).cpu().numpy(), getattr(co, q)(*ts, W.STEP_MAX), "%s border %s" % (name, q))
