@@ -280,8 +280,13 @@ int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, c
  * pipeline (clamped to 2^20).
  * VG_OPT_COOP_MAX_N (default VG_COOP_MAX_N_DEFAULT): queries of a full-phi polycone over at most this many tracks run as
  *   the lanes-per-track kernel (a group of 4..32 lanes shares one track and splits its sections):
- *   lowest latency for small batches, same results.  0 switches the form off. */
-typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2, VG_OPT_HOST_CHUNK = 3, VG_OPT_COOP_MAX_N = 4 } vg_option;
+ *   lowest latency for small batches, same results.  0 switches the form off.
+ * VG_OPT_NAV_FORM (default 0 = chosen per volume): how vg_compute_step evaluates the daughters that survive its cull
+ *   (same results).  1: every lane walks its own candidates.  2: the candidates of a warp's 32 tracks are pooled and
+ *   evaluated as one dense work list (a warp cooperates over daughters).  0 takes 2 for volumes whose candidate grid
+ *   lists more than 24 daughters per cell, else 1 (DESIGN.md sec. 6.4 has the measurements). */
+typedef enum { VG_OPT_PIPE_MIN_N = 0, VG_OPT_PDL = 1, VG_OPT_FORM = 2, VG_OPT_HOST_CHUNK = 3, VG_OPT_COOP_MAX_N = 4,
+               VG_OPT_NAV_FORM = 5 } vg_option;
 #define VG_COOP_MAX_N_DEFAULT 32768
 enum { VG_FORM_AUTO = 0, VG_FORM_DIRECT = 1, VG_FORM_PIPELINED = 2, VG_FORM_STREAMING = 3 };
 int vg_set_option(int option, int64_t value);

@@ -83,6 +83,7 @@ OPT_PDL = 1
 OPT_FORM = 2
 OPT_HOST_CHUNK = 3
 OPT_COOP_MAX_N = 4
+OPT_NAV_FORM = 5
 FORM_AUTO, FORM_DIRECT, FORM_PIPELINED, FORM_STREAMING = 0, 1, 2, 3
 INT64_MAX = 2 ** 63 - 1
 

@@ -55,6 +55,7 @@ std::atomic<int64_t> g_pipe_min_n{ int64_t(1) << 17 };
 std::atomic<int64_t> g_pdl{ 1 };
 std::atomic<int64_t> g_form{ VG_FORM_AUTO };
 std::atomic<int64_t> g_host_chunk{ 0 };
+std::atomic<int64_t> g_nav_form{ 0 };
 std::atomic<int64_t> g_coop_max_n{ VG_COOP_MAX_N_DEFAULT };
 }
 extern "C" int64_t vg_launch_count(void) { return vg::g_launches.load(); }
@@ -77,6 +78,10 @@ extern "C" int vg_set_option(int option, int64_t value)
         if (value < VG_FORM_AUTO || value > VG_FORM_STREAMING) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_FORM must be 0..3");
         vg::g_form.store(value);
         return VG_OK;
+    case VG_OPT_NAV_FORM:
+        if (value < 0 || value > 2) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_NAV_FORM must be 0 (auto), 1 (per lane) or 2 (cooperative)");
+        vg::g_nav_form.store(value);
+        return VG_OK;
     case VG_OPT_COOP_MAX_N:
         if (value < 0) return fail(VG_ERR_ARG, "vg_set_option: VG_OPT_COOP_MAX_N must be >= 0");
         vg::g_coop_max_n.store(value);
@@ -93,6 +98,7 @@ extern "C" int64_t vg_get_option(int option)
     case VG_OPT_FORM: return vg::g_form.load();
     case VG_OPT_HOST_CHUNK: return vg::g_host_chunk.load();
     case VG_OPT_COOP_MAX_N: return vg::g_coop_max_n.load();
+    case VG_OPT_NAV_FORM: return vg::g_nav_form.load();
     }
     return fail(VG_ERR_ARG, "vg_get_option: unknown option %d", option);
 }
@@ -427,6 +433,8 @@ static int to_solid(const vg_shape *s, SolidU *o, const char *what)
     }
 }
 
+constexpr double kNavDenseCell = 24.0; // measured: pooling pays only where nearly every daughter is a candidate of every ray
+
 // Host side of vg_volume_create for a volume of primitives: validation, the mother and daughter records, the FP32
 // bounding spheres and the candidate grid, as one blob in host memory (layout: vg_params.h).  No CUDA call.
 static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
@@ -539,6 +547,15 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
                             cells[size_t((iz * gdim + iy) * gdim + ix) * mt.nchunks + i / 64] |= 1ull << (i % 64);
                     }
         }
+        // mean number of daughters listed per non-empty cell: above kNavDenseCell a ray meets many candidates and the warp
+        // pools phase 2 (vg_nav.cu)
+        size_t listed = 0, nonempty = 0;
+        for (unsigned ic = 0; ic < ncell; ++ic) {
+            int pc = 0;
+            for (int c = 0; c < mt.nchunks; ++c) pc += __builtin_popcountll(cells[size_t(ic) * mt.nchunks + c]);
+            listed += size_t(pc), nonempty += pc ? 1 : 0;
+        }
+        mt.dense = nonempty && double(listed) / double(nonempty) > kNavDenseCell;
     }
     if (rc != VG_OK) {
         delete[] host;

@@ -265,6 +265,7 @@ constexpr int kPipeTile = 64 * kPipeWarps;         // tracks per tile: two per c
 
 extern std::atomic<int64_t> g_pipe_min_n; // vg_set_option(VG_OPT_PIPE_MIN_N)
 extern std::atomic<int64_t> g_host_chunk; // vg_set_option(VG_OPT_HOST_CHUNK): tracks per chunk of the host-fed pipeline, 0 = auto
+extern std::atomic<int64_t> g_nav_form;   // vg_set_option(VG_OPT_NAV_FORM): 0 auto, 1 per-lane, 2 warp-cooperative phase 2 of ComputeStep
 extern std::atomic<int64_t> g_form;       // vg_set_option(VG_OPT_FORM): 0 auto, 1 direct, 2 pipelined, 3 streaming
 
 // VG_FORM_AUTO: the pairs whose pipelined form measured faster than the direct one at n >= 2^22 (profiles/):

@@ -49,6 +49,35 @@ VG_DEV const Daughter &daughter_at(const unsigned char *dtab, int k)
     return *reinterpret_cast<const Daughter *>(dtab + size_t(k) * kDaughterStride);
 }
 
+// ---- phase 2, per lane: every lane walks ITS OWN candidates, one loop per solid kind so that the lanes of a warp run the
+// same DistanceToIn code on different daughters.  The form for sparse volumes (a ray meets the bounding sphere of 0-2
+// daughters: configs[4]), where pooling the work costs more than the idle lanes it saves (A/B in DESIGN.md sec. 6.4).
+template <class S>
+VG_DEV void lane_candidates(unsigned long long mk, int base, const unsigned char *dtab, double x, double y, double z,
+                            double dx, double dy, double dz, double &best, int &who)
+{
+    unsigned lo = unsigned(mk), hi = unsigned(mk >> 32);
+    while (lo | hi) {
+        const bool in_lo = lo != 0u;
+        const unsigned w = in_lo ? lo : hi;
+        const int k = base + (in_lo ? 0 : 32) + __ffs(int(w)) - 1;
+        lo = in_lo ? (lo & (lo - 1u)) : lo;
+        hi = in_lo ? hi : (hi & (hi - 1u));
+        const Daughter &D = daughter_at(dtab, k);
+        double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
+        double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
+        double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
+        double ldx = fma(D.m[0], dx, fma(D.m[1], dy, D.m[2] * dz));
+        double ldy = fma(D.m[4], dx, fma(D.m[5], dy, D.m[6] * dz));
+        double ldz = fma(D.m[8], dx, fma(D.m[9], dy, D.m[10] * dz));
+        double tk = S::dist_in(Pick<S>::of(D.s), lx, ly, lz, ldx, ldy, ldz);
+        // R13: lexicographic min of (distance, index); a daughter the track is inside of (-1) is skipped
+        bool take = tk >= 0.0 && (tk < best || (tk == best && k < who));
+        best = take ? tk : best;
+        who = take ? k : who;
+    }
+}
+
 // ---- phase 2, warp-cooperative: the candidates of the 32 tracks of a warp are evaluated as one dense work list ----
 //
 // After the cull a lane holds 0-3 candidates and most lanes hold none (22 % of the tracks of configs[4] hit anything):
@@ -123,8 +152,8 @@ VG_DEV void coop_candidates(unsigned long long mk, int base, const unsigned char
     }
 }
 
-// ComputeStep; NC = chunks of 64 daughters (1, 2 or 4)
-template <int NC>
+// ComputeStep; NC = chunks of 64 daughters (1, 2 or 4); COOP = phase 2 pooled over the warp, else per lane
+template <int NC, bool COOP>
 __global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const __grid_constant__ SolidU mother,
                                                              const __grid_constant__ NavMeta meta,
                                                              const unsigned char *__restrict__ table, Tracks t,
@@ -173,11 +202,11 @@ __global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const 
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const unsigned long long mc = valid ? m[c] : 0ull;
-                if (meta.kmask[kBox][c]) coop_candidates<Box>(mc & meta.kmask[kBox][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
-                if (meta.kmask[kTube][c]) coop_candidates<Tube>(mc & meta.kmask[kTube][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
-                if (meta.kmask[kOrb][c]) coop_candidates<Orb>(mc & meta.kmask[kOrb][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
-                if (meta.kmask[kCone][c]) coop_candidates<Cone>(mc & meta.kmask[kCone][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
-                if (meta.kmask[kTrd][c]) coop_candidates<Trd>(mc & meta.kmask[kTrd][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res);
+                if (meta.kmask[kBox][c]) { if (COOP) coop_candidates<Box>(mc & meta.kmask[kBox][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res); else lane_candidates<Box>(mc & meta.kmask[kBox][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who); }
+                if (meta.kmask[kTube][c]) { if (COOP) coop_candidates<Tube>(mc & meta.kmask[kTube][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res); else lane_candidates<Tube>(mc & meta.kmask[kTube][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who); }
+                if (meta.kmask[kOrb][c]) { if (COOP) coop_candidates<Orb>(mc & meta.kmask[kOrb][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res); else lane_candidates<Orb>(mc & meta.kmask[kOrb][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who); }
+                if (meta.kmask[kCone][c]) { if (COOP) coop_candidates<Cone>(mc & meta.kmask[kCone][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res); else lane_candidates<Cone>(mc & meta.kmask[kCone][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who); }
+                if (meta.kmask[kTrd][c]) { if (COOP) coop_candidates<Trd>(mc & meta.kmask[kTrd][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who, q, res); else lane_candidates<Trd>(mc & meta.kmask[kTrd][c], 64 * c, dtab, x, y, z, dx, dy, dz, best, who); }
             }
         }
         if (valid) {
@@ -268,24 +297,35 @@ static cudaError_t nav_grid_size(Kern kern, NavDevState *states, size_t smem, in
     return cudaSuccess;
 }
 
-template <int NC>
+template <int NC, bool COOP>
 static cudaError_t launch_step_nc(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                   double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
 {
     static NavDevState states[64];
     unsigned grid = 0;
-    cudaError_t err = nav_grid_size(nav_step_kernel<NC>, states, meta.bytes, n, &grid);
+    cudaError_t err = nav_grid_size(nav_step_kernel<NC, COOP>, states, meta.bytes, n, &grid);
     if (err != cudaSuccess) return err;
-    return launch_kernel(nav_step_kernel<NC>, grid, kNavBlock, meta.bytes, s, mother, meta, table_dev, t, step_max, n, step, hit);
+    return launch_kernel(nav_step_kernel<NC, COOP>, grid, kNavBlock, meta.bytes, s, mother, meta, table_dev, t, step_max, n, step, hit);
+}
+
+template <bool COOP>
+static cudaError_t launch_step_form(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
+                                    double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
+{
+    if (meta.nchunks <= 1) return launch_step_nc<1, COOP>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    if (meta.nchunks == 2) return launch_step_nc<2, COOP>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    return launch_step_nc<4, COOP>(mother, table_dev, meta, t, step_max, n, step, hit, s);
 }
 
 cudaError_t launch_compute_step(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                 double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
-    if (meta.nchunks <= 1) return launch_step_nc<1>(mother, table_dev, meta, t, step_max, n, step, hit, s);
-    if (meta.nchunks == 2) return launch_step_nc<2>(mother, table_dev, meta, t, step_max, n, step, hit, s);
-    return launch_step_nc<4>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    // phase 2: pooled over the warp where the candidate grid says a ray meets many daughters, per lane where it meets few
+    const int64_t form = g_nav_form.load(std::memory_order_relaxed);
+    const bool coop = form == 2 || (form == 0 && meta.dense);
+    return coop ? launch_step_form<true>(mother, table_dev, meta, t, step_max, n, step, hit, s)
+                : launch_step_form<false>(mother, table_dev, meta, t, step_max, n, step, hit, s);
 }
 
 cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,

@@ -196,6 +196,7 @@ struct NavGrid {
 
 struct NavMeta {
     int nd, nchunks;
+    int dense, pad; // the grid's cells list many daughters each (vg_volume_create): phase 2 of ComputeStep pools the warp's work
     unsigned off_d, bytes;
     unsigned long long kmask[kNavKinds][kNavChunks]; // bit j of kmask[kind][c]: daughter 64 c + j is of that kind
     unsigned long long all[kNavChunks];              // every daughter of the chunk

@@ -342,9 +342,27 @@ def test_many_overlapping_daughters_of_all_kinds(vg, nd, size, spread):
         return near
 
     t = W.draw_tracks(77 + nd, 100003, (0, 0, 0), (60, 60, 60), band)
-    for step_max in (W.STEP_MAX, 25.0):
-        so, ho = check_step(vo, vgv, t, step_max, "nd=%d step_max=%g" % (nd, step_max))
+    try:
+        for form in (1, 2, 0):  # every lane walks its own candidates / the warp pools them / the library's choice
+            vg.vg_set_option(vg.OPT_NAV_FORM, form)
+            for step_max in (W.STEP_MAX, 25.0):
+                so, ho = check_step(vo, vgv, t, step_max, "nd=%d step_max=%g form=%d" % (nd, step_max, form))
+    finally:
+        vg.vg_set_option(vg.OPT_NAV_FORM, 0)
     assert len(set(ho.tolist())) > min(nd, 40) // 2
+
+
+@pytest.mark.parametrize("form", [1, 2])
+def test_config4_both_forms_of_phase_two(vg, form):
+    nav = W.navigator_case()
+    vo, vgv = build_volumes(vg, nav)
+    t = nav_tracks(nav, vo, 300007, seed=nav.seed + 9)
+    try:
+        vg.vg_set_option(vg.OPT_NAV_FORM, form)
+        check_step(vo, vgv, t, W.STEP_MAX, "cfg4 form=%d" % form)
+        check_step(vo, vgv, t, 30.0, "cfg4 form=%d step_max=30" % form)
+    finally:
+        vg.vg_set_option(vg.OPT_NAV_FORM, 0)
 
 
 def test_volume_safety_config4(vg):
