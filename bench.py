@@ -67,6 +67,7 @@ def ncu_traffic(solid, query, n):
                 c = line.strip().split(",")
                 if len(c) >= 7 and c[1] == solid and c[2] == query and c[3] == str(n):
                     return {"bytes": int(c[4]) + int(c[5]), "dram_read": int(c[4]), "dram_write": int(c[5]),
+                            "fp64_pipe_pct": float(c[7]) if len(c) > 7 and c[7] else None,
                             "capture": "profiles/%s_full_capture.md" % c[6],
                             "note": "results still sit in the 126 MB L2 when the kernel ends, so DRAM writes read low"}
     except OSError:
@@ -714,6 +715,9 @@ def run_profile(args):
     for k in (1, 2, 3):
         for sc in W.shape_cases(k):
             cases.append(Case(vg, torch, sc.name, min(sc.sizes[-1], 4194304), sc.queries, shape=sc))
+    pc = W.shape_cases(3)[0]  # the small batches of configs[3]: the lanes-per-track kernels (vg_pcon_coop.cuh)
+    for n_small in (1024, 16384):
+        cases.append(Case(vg, torch, pc.name, n_small, pc.queries, shape=pc))
     nav = W.navigator_case()
     cases.append(Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step",), nav=nav))
     wc = W.world_case()
@@ -759,7 +763,8 @@ def per_config_rows(detail, fma_rate):
     (cold inputs), f = fraction of the measured HBM copy rate, f8 = fraction of the nominal 8 TB/s, fp64 = SURVEY 8(d)'s
     algorithmic FP64 operations / s over the FP64 rate measured in this run (ALU-bound rows), lat = latency-adjusted
     fraction max(bytes / BW, empty launch) / measured (launch-bound sizes), cl = duration of the arithmetic-free kernel
-    with the same loads, store, grid and form on the same buffers (vg_probe_stream) / measured."""
+    with the same loads, store, grid and form on the same buffers (vg_probe_stream) / measured, pipe = ncu's
+    sm__inst_executed_pipe_fp64 (fraction of peak while active) of that kernel in the committed capture."""
     groups = {}
     for e in detail:
         if e.get("row") or not isinstance(e.get("config"), int) or str(e["query"]).startswith("all five"):
@@ -775,7 +780,10 @@ def per_config_rows(detail, fma_rate):
         if n <= 262144:
             r["lat"] = w["latency_adjusted_frac"]
         elif w["bound"] == "alu":
-            r["fp64"] = w["fp64_frac"]
+            r["fp64"] = w["fp64_frac"]  # SURVEY 8(d)'s numerator (every segment / every daughter) over the measured FP64 rate
+            tr = ncu_traffic("navigator" if k == 4 else NCU_SOLID.get(shape, shape), w["query"], min(n, 4194304))
+            if tr and tr.get("fp64_pipe_pct") is not None:  # what the hardware counted in the committed capture (n = 2^22)
+                r["pipe"] = tr["fp64_pipe_pct"] / 100.0
         else:
             r["f"], r["f8"] = w["hbm_frac"], w["hbm_gbs"] / HBM_NOMINAL_GBS
         if "frac_of_mem_ceiling" in w:  # cl = the size-matched memory ceiling (same loads / store / grid, no arithmetic) / measured

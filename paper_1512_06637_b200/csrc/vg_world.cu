@@ -14,6 +14,7 @@
 // are identical to visiting every child.  Children are visited in ascending node index, so the strict `<` scan is
 // the tie-break of R13.
 #include "vg_csg.cuh"
+#include "vg_nav_cull.h"
 
 namespace vg {
 
@@ -169,12 +170,9 @@ __global__ void __launch_bounds__(kWorldBlock)
 #pragma unroll 4
             for (int j = 0; j < lim; ++j) {
                 // phase 1, FP32: ray against the bounding sphere (closest approach of the line; sphere not behind the start)
+                // (the predicate of ComputeStep's cull, vg_nav_cull.h: pinned on the CPU by tests/test_nav_cull.py, stage 2)
                 const float4 sp = __ldg(cull + c0 + base + j);
-                const float vx = sp.x - xf, vy = sp.y - yf, vz = sp.z - zf;
-                const float vv = fmaf(vx, vx, fmaf(vy, vy, vz * vz));
-                const float tca = fmaf(vx, dxf, fmaf(vy, dyf, vz * dzf));
-                const float d2 = fmaf(-tca, tca, vv);
-                m |= (unsigned long long)(d2 <= sp.w && (tca >= 0.f || vv <= sp.w)) << j;
+                m |= (unsigned long long)nav_sphere_keep(sp, xf, yf, zf, dxf, dyf, dzf) << j;
             }
             while (m) { // phase 2, FP64, ascending child index: the strict < is R13's tie-break
                 const int c = kids[c0 + base + __ffsll((long long)m) - 1];
