@@ -134,13 +134,23 @@ static void upload_pcon_grid(vg_shape *s)
             w.flags |= 2 | (t.oup ? 4 : 0) | (t.iup ? 8 : 0);
         }
     }
+    std::vector<PconWalkSec> wtab(pc.nsec); // the ordered walks' records (what pcon_stage builds in shared memory)
+    for (int k = 0; k < pc.nsec; ++k) {
+        const PconSec &c = pc.sec[k];
+        PconWalkSec &w = wtab[k];
+        w.z0 = c.z0, w.z1 = c.z1, w.Ao = c.out.A, w.Bo = c.out.B, w.Ai = c.in.A, w.Bi = c.in.B;
+        w.ro0 = c.out.r0, w.ero = c.out.er, w.ilo = c.out.inv_l2, w.ri0 = c.in.r0, w.eri = c.in.er, w.ili = c.in.inv_l2;
+        w.seco = c.out.sec, w.seci = c.in.sec;
+    }
+    const size_t wbytes = wtab.size() * sizeof(PconWalkSec);
     const size_t cbytes = coop.size() * sizeof(PconCoopSec), roff = (rows.size() + 15) / 16 * 16;
     unsigned char *blob = nullptr;
-    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + roff + cbytes) == cudaSuccess &&
+    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + roff + cbytes + wbytes) == cudaSuccess &&
               cudaMemcpy(blob, masks.data(), mbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
               (fbytes == 0 || cudaMemcpy(blob + mbytes, fmasks.data(), fbytes, cudaMemcpyHostToDevice) == cudaSuccess) &&
               cudaMemcpy(blob + mbytes + fbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
-              cudaMemcpy(blob + mbytes + fbytes + roff, coop.data(), cbytes, cudaMemcpyHostToDevice) == cudaSuccess;
+              cudaMemcpy(blob + mbytes + fbytes + roff, coop.data(), cbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(blob + mbytes + fbytes + roff + cbytes, wtab.data(), wbytes, cudaMemcpyHostToDevice) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         if (blob) cudaFree(blob);
@@ -150,6 +160,7 @@ static void upload_pcon_grid(vg_shape *s)
     s->grid.face_masks = fbytes ? reinterpret_cast<const unsigned long long *>(blob + mbytes) : nullptr;
     s->grid.rows = blob + mbytes + fbytes;
     s->grid.coop = reinterpret_cast<const PconCoopSec *>(blob + mbytes + fbytes + roff);
+    s->grid.wtab = reinterpret_cast<const PconWalkSec *>(blob + mbytes + fbytes + roff + cbytes);
     s->grid.g = geom;
     s->grid_device = dev;
 }
@@ -244,7 +255,7 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
     case VG_POLYCONE: {
         PconGrid g = s->grid;
         int dev = -1;
-        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr, g.wtab = nullptr;
         e = launch_polycone(q, s->u.pcon, g, t, step_max, n, out, vec, st);
         break;
     }
@@ -312,7 +323,7 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
         if (rcp != VG_OK) return rcp;
         PconGrid g = s->grid;
         int dev = -1;
-        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr, g.wtab = nullptr;
         Tracks t{ x, y, z, dx, dy, dz };
         AllOut o{ cls, dist_in, dist_out, safety_in, safety_out };
         cudaError_t e = launch_polycone_all(s->u.pcon, g, t, step_max, n, o, vec, static_cast<cudaStream_t>(stream));

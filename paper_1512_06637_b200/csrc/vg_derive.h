@@ -99,6 +99,7 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         t.rmax_in2 = (rmax - kTol) * (rmax - kTol);
         t.rmin_out2 = rmin > kTol ? (rmin - kTol) * (rmin - kTol) : 0.0;
         t.rmax_out2 = (rmax + kTol) * (rmax + kTol);
+        t.rc = 0.5 * (rmin + rmax), t.rh = 0.5 * (rmax - rmin);
         t.w = make_wedge(p[3], p[4]);
         t.hollow = rmin > 0;
         return VG_OK;
@@ -118,6 +119,8 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         c.rmax2 = rmax2;
         c.w = make_wedge(p[5], p[6]);
         c.hollow = rmin1 > 0 || rmin2 > 0;
+        c.cap_c1 = 0.5 * (rmin1 + rmax1), c.cap_h1 = 0.5 * (rmax1 - rmin1);
+        c.cap_c2 = 0.5 * (rmin2 + rmax2), c.cap_h2 = 0.5 * (rmax2 - rmin2);
         return VG_OK;
     }
     case VG_TRD: {

@@ -21,6 +21,12 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
             case qSafeOut: return launch_pcon_coop<qSafeOut>(p, g, t, step_max, n, out, s);
             }
         }
+        // medium batches: one track per thread, section table in device memory (vg_pcon_walk.cuh), any alignment
+        if (g.wtab && g_form.load(std::memory_order_relaxed) == 0 && n <= kWalkSmallMaxN && g_coop_max_n.load(std::memory_order_relaxed) > 0) {
+            if (q == qInside) return launch_pcon_walk_small<qInside>(p, g, t, step_max, n, out, s);
+            if (q == qDistIn) return launch_pcon_walk_small<qDistIn>(p, g, t, step_max, n, out, s);
+            if (q == qDistOut) return launch_pcon_walk_small<qDistOut>(p, g, t, step_max, n, out, s);
+        }
         if (vec && g_form.load(std::memory_order_relaxed) == 0) {
             double *o = static_cast<double *>(out);
             if (q == qDistIn) return launch_pcon_walk<qDistIn, false>(p, g, t, step_max, n, o, s);

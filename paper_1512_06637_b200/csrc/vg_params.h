@@ -36,6 +36,7 @@ struct TubeP {
     double rmin2, rmax2;
     double rmin_in2, rmax_in2;   // (rmin + kTol)^2, (rmax - kTol)^2 : strictly-inside tests
     double rmin_out2, rmax_out2; // (rmin - kTol)^2 (0 if rmin <= kTol), (rmax + kTol)^2
+    double rc, rh;               // (rmin + rmax) / 2, (rmax - rmin) / 2: distance to [rmin, rmax] = max(|rho - rc| - rh, 0)
     Wedge w;
     int hollow; // rmin > 0
 };
@@ -52,6 +53,7 @@ struct ConeP {
     double dz;
     Frustum out, in;
     double rmin1, rmax1, rmin2, rmax2;
+    double cap_c1, cap_h1, cap_c2, cap_h2; // centre (rmin + rmax) / 2 and half-width (rmax - rmin) / 2 of the two cap annuli
     Wedge w;
     int hollow; // rmin1 > 0 || rmin2 > 0 : the inner patch is a surface
 };
@@ -119,7 +121,18 @@ struct alignas(16) PconCoopSec {
     int flags, pad;                            // 1: inner surface, 2: step above, 4: step.oup, 8: step.iup
 };
 
+// One compact record per section for the ordered walks (vg_pcon_walk.cuh): staged in shared memory by the persistent
+// kernels, read from device memory by the medium-batch kernel.  14 doubles, 16-byte aligned.
+struct alignas(16) PconWalkSec {
+    double z0, z1;
+    double Ao, Bo, Ai, Bi;    // generators r = A + B z of the outer / inner patch
+    double ro0, ero, ilo;     // outer edge (r0, z0) -> (r0 + er, z1), 1 / |edge|^2
+    double ri0, eri, ili;     // inner edge
+    double seco, seci;        // sqrt(1 + B^2) of both patches (tolerance band of the Inside test)
+};
+
 struct PconGrid {
+    const PconWalkSec *wtab;         // [nsec] in device memory; NULL: not uploaded
     const PconCoopSec *coop;         // [nsec]; NULL: not uploaded, the thread-per-track kernels serve every batch size
     const unsigned long long *masks; // [kPconGridZ][kPconGridR]; NULL: no grid, the ordered walk serves the safeties
     const unsigned long long *face_masks; // phi cut only: [kPconGridZ][2 kPconGridR] over u in [-R, R), every outline edge

@@ -17,14 +17,6 @@
 
 namespace vg {
 
-struct PconWalkSec {          // 14 doubles, 16-byte aligned
-    double z0, z1;
-    double Ao, Bo, Ai, Bi;    // generators r = A + B z of the outer / inner patch
-    double ro0, ero, ilo;     // outer edge (r0, z0) -> (r0 + er, z1), 1 / |edge|^2
-    double ri0, eri, ili;     // inner edge
-    double seco, seci;        // sqrt(1 + B^2) of both patches (tolerance band of the Inside test)
-};
-
 constexpr int kWalkBlock = 256;
 
 VG_DEV void pcon_stage(const PolyconeP &p, PconWalkSec *tab)
@@ -635,6 +627,46 @@ __global__ void __launch_bounds__(kWalkBlock, 2)
             stg1(o.sout + i, -s0);
         }
     }
+}
+
+// ---- medium batches (VG_OPT_COOP_MAX_N < n <= kWalkSmallMaxN): the same ordered walks, one track per thread in 64-thread
+// CTAs that read the section table from device memory (built at vg_shape_create) instead of staging it: no barrier, four
+// times as many CTAs as the persistent form has at these sizes, half the dependent work per thread.  Full phi; the
+// safeties keep the candidate-grid kernel above.
+constexpr int kWalkSmallBlock = 64;
+#ifndef VG_WALK_SMALL_MAX_N
+#define VG_WALK_SMALL_MAX_N 524288
+#endif
+constexpr int64_t kWalkSmallMaxN = VG_WALK_SMALL_MAX_N;
+
+template <int Q>
+__global__ void __launch_bounds__(kWalkSmallBlock)
+    pcon_walk_small_kernel(const __grid_constant__ PolyconeP p, const PconWalkSec *__restrict__ tab, Tracks t, double step_max,
+                           int64_t n, void *out_any)
+{
+    const int64_t i = int64_t(blockIdx.x) * kWalkSmallBlock + threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
+    if (i >= n) return;
+    const double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+    if (Q == qInside) {
+        bool in, out;
+        pcon_walk_classify<false>(p, tab, x, y, z, in, out);
+        stg1i(static_cast<int32_t *>(out_any) + i, classify(in, out));
+        return;
+    }
+    const double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+    const double r = Q == qDistOut ? pcon_walk_dist_out<false>(p, tab, x, y, z, dx, dy, dz)
+                                   : pcon_walk_dist_in<false>(p, tab, x, y, z, dx, dy, dz);
+    stg1(static_cast<double *>(out_any) + i, r <= step_max ? r : inf());
+}
+
+template <int Q>
+cudaError_t launch_pcon_walk_small(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, void *out,
+                                   cudaStream_t s)
+{
+    const unsigned grid = unsigned((n + kWalkSmallBlock - 1) / kWalkSmallBlock);
+    return launch_kernel(pcon_walk_small_kernel<Q>, grid, kWalkSmallBlock, 0, s, p, g.wtab, t, step_max, n, out);
 }
 
 template <bool GRID, bool WEDGE>

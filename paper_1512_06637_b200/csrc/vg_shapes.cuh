@@ -237,11 +237,13 @@ template <int F> struct TubeT {
     {
         double rho2 = fma(x, x, y * y);
         double rho = sqrt_nn(rho2);
-        double qr = rho - p.rmax;
-        if (hollow(p)) qr = dmax(qr, p.rmin - rho);
+        // distance to an interval [lo, hi] as max(|u - c| - h, 0) (one compare less than max(lo - u, u - hi, 0)); the square
+        // of max(q, 0) as (q + |q|)^2 / 4 (no compare at all)
+        double qr = hollow(p) ? fabs(rho - p.rc) - p.rh : rho - p.rmax;
         double qz = fabs(z) - p.dz;
-        double ar = dmax(qr, 0.0), az = dmax(qz, 0.0);
-        double out2 = fma(ar, ar, az * az);
+        double sr = qr + fabs(qr), sz = qz + fabs(qz);
+        double az2 = 0.25 * sz * sz;
+        double out2 = fma(0.25 * sr, sr, az2);
         double m = dmax(qr, qz);
         bool in_rect = m < 0.0;
         if (full(p)) return in_rect ? m : sqrt_nn(out2);
@@ -250,11 +252,10 @@ template <int F> struct TubeT {
         bool mem = wedge_member<WM>(p.w, e.c0, e.c1);
         D2 = mem ? D2 : inf();
         // the two phi faces: filled rectangle [rmin, rmax] x [-dz, dz] in the half-plane (u >= 0)
-        double q0 = dmax(dmax(e.u0 - p.rmax, p.rmin - e.u0), 0.0);
-        double q1 = dmax(dmax(e.u1 - p.rmax, p.rmin - e.u1), 0.0);
-        double az2 = az * az;
-        D2 = dmin(D2, fma(e.c0, e.c0, fma(q0, q0, az2)));
-        D2 = dmin(D2, fma(e.c1, e.c1, fma(q1, q1, az2)));
+        double q0 = fabs(e.u0 - p.rc) - p.rh, q1 = fabs(e.u1 - p.rc) - p.rh;
+        double s0 = q0 + fabs(q0), s1 = q1 + fabs(q1);
+        D2 = dmin(D2, fma(e.c0, e.c0, fma(0.25 * s0, s0, az2)));
+        D2 = dmin(D2, fma(e.c1, e.c1, fma(0.25 * s1, s1, az2)));
         double D = sqrt_nn(D2);
         return (mem && in_rect) ? -D : D;
     }
@@ -417,10 +418,14 @@ template <int F> struct ConeT {
         double ez = 2.0 * p.dz;
         double d2 = seg_d2(u, v, p.out.r0, -p.dz, p.out.er, ez, p.out.inv_l2);
         if (hollow(p) || axis) d2 = dmin(d2, seg_d2(u, v, p.in.r0, -p.dz, p.in.er, ez, p.in.inv_l2));
-        double b1 = dmax(dmax(p.rmin1 - u, u - p.rmax1), 0.0), v1 = v + p.dz;
-        double b2 = dmax(dmax(p.rmin2 - u, u - p.rmax2), 0.0), v2 = v - p.dz;
-        d2 = dmin(d2, fma(b1, b1, v1 * v1));
-        d2 = dmin(d2, fma(b2, b2, v2 * v2));
+        // The cap on the point's side of the mid-plane only: the other cap cannot hold the nearest point in its interior
+        // (the vertical segment to it comes from inside the outline, so it has crossed a nearer edge), and its rims are
+        // end points of the two edges above.  Distance to the annulus [rmin, rmax] as max(|u - c| - h, 0); its square
+        // from s = q + |q| = 2 max(q, 0) without a compare.
+        const bool top = not_neg(v);
+        double q = fabs(u - (top ? p.cap_c2 : p.cap_c1)) - (top ? p.cap_h2 : p.cap_h1);
+        double s = q + fabs(q), vc = fabs(v) - p.dz;
+        d2 = dmin(d2, fma(0.25 * s, s, vc * vc));
         return d2;
     }
     VG_DEV static bool in_quad(const P &p, double u, double v)

@@ -24,10 +24,12 @@ def vg():
     return m
 
 
-@pytest.fixture(params=["lanes", "threads"])
+@pytest.fixture(params=["lanes", "medium", "threads"])
 def form(request, vg):
+    """lanes: a group of lanes per track whatever n; medium: one track per thread, section table in device memory (what
+    batches between VG_OPT_COOP_MAX_N and 2^19 tracks run as; here every n > 1); threads: the persistent walk kernels."""
     old = vg.vg_get_option(vg.OPT_COOP_MAX_N)
-    vg.vg_set_option(vg.OPT_COOP_MAX_N, 1 << 40 if request.param == "lanes" else 0)
+    vg.vg_set_option(vg.OPT_COOP_MAX_N, {"lanes": 1 << 40, "medium": 1, "threads": 0}[request.param])
     yield request.param
     vg.vg_set_option(vg.OPT_COOP_MAX_N, old)
 
@@ -66,8 +68,8 @@ def test_every_group_width_and_z_steps(vg, form, seed, nz, rmin_hi, steps):
 
 
 def test_threshold_switches_the_form_and_both_sides_agree_with_the_oracle(vg):
-    """n = threshold - 1, threshold, threshold + 1 with the default policy: the first two run as lane groups, the third
-    as the thread-per-track walk (counted through the launch counter: one launch each, results identical in meaning)."""
+    """n = threshold - 1, threshold, threshold + 1: the first two run as lane groups, the third as the one-track-per-thread
+    walk (one launch each through the launch counter; every answer against the oracle)."""
     sc = W.shape_cases(3)[0]
     so, sg = O.Shape(sc.kind, sc.params), vg.Shape(sc.kind, sc.params)
     old = vg.vg_get_option(vg.OPT_COOP_MAX_N)
