@@ -143,14 +143,18 @@ static void upload_pcon_grid(vg_shape *s)
         w.seco = c.out.sec, w.seci = c.in.sec;
     }
     const size_t wbytes = wtab.size() * sizeof(PconWalkSec);
+    std::vector<double> segs(64 * kPconSegStride); // the candidate grids' segment records
+    for (int b = 0; b < 64; ++b) pcon_seg_record(pc, b, &segs[size_t(b) * kPconSegStride]);
+    const size_t sbytes = segs.size() * sizeof(double);
     const size_t cbytes = coop.size() * sizeof(PconCoopSec), roff = (rows.size() + 15) / 16 * 16;
     unsigned char *blob = nullptr;
-    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + roff + cbytes + wbytes) == cudaSuccess &&
+    bool ok = cudaMalloc(reinterpret_cast<void **>(&blob), mbytes + fbytes + roff + cbytes + wbytes + sbytes) == cudaSuccess &&
               cudaMemcpy(blob, masks.data(), mbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
               (fbytes == 0 || cudaMemcpy(blob + mbytes, fmasks.data(), fbytes, cudaMemcpyHostToDevice) == cudaSuccess) &&
               cudaMemcpy(blob + mbytes + fbytes, rows.data(), rows.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
               cudaMemcpy(blob + mbytes + fbytes + roff, coop.data(), cbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
-              cudaMemcpy(blob + mbytes + fbytes + roff + cbytes, wtab.data(), wbytes, cudaMemcpyHostToDevice) == cudaSuccess;
+              cudaMemcpy(blob + mbytes + fbytes + roff + cbytes, wtab.data(), wbytes, cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(blob + mbytes + fbytes + roff + cbytes + wbytes, segs.data(), sbytes, cudaMemcpyHostToDevice) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
         if (blob) cudaFree(blob);
@@ -161,6 +165,7 @@ static void upload_pcon_grid(vg_shape *s)
     s->grid.rows = blob + mbytes + fbytes;
     s->grid.coop = reinterpret_cast<const PconCoopSec *>(blob + mbytes + fbytes + roff);
     s->grid.wtab = reinterpret_cast<const PconWalkSec *>(blob + mbytes + fbytes + roff + cbytes);
+    s->grid.segs = reinterpret_cast<const double *>(blob + mbytes + fbytes + roff + cbytes + wbytes);
     s->grid.g = geom;
     s->grid_device = dev;
 }
@@ -255,7 +260,7 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
     case VG_POLYCONE: {
         PconGrid g = s->grid;
         int dev = -1;
-        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr, g.wtab = nullptr;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr, g.wtab = nullptr, g.segs = nullptr;
         e = launch_polycone(q, s->u.pcon, g, t, step_max, n, out, vec, st);
         break;
     }
@@ -323,7 +328,7 @@ extern "C" int vg_query_all(const vg_shape *s, const double *x, const double *y,
         if (rcp != VG_OK) return rcp;
         PconGrid g = s->grid;
         int dev = -1;
-        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr, g.wtab = nullptr;
+        if (g.masks && (cudaGetDevice(&dev) != cudaSuccess || dev != s->grid_device)) g.masks = nullptr, g.face_masks = nullptr, g.coop = nullptr, g.wtab = nullptr, g.segs = nullptr;
         Tracks t{ x, y, z, dx, dy, dz };
         AllOut o{ cls, dist_in, dist_out, safety_in, safety_out };
         cudaError_t e = launch_polycone_all(s->u.pcon, g, t, step_max, n, o, vec, static_cast<cudaStream_t>(stream));

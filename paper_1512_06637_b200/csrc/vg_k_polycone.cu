@@ -21,11 +21,14 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
             case qSafeOut: return launch_pcon_coop<qSafeOut>(p, g, t, step_max, n, out, s);
             }
         }
-        // medium batches: one track per thread, section table in device memory (vg_pcon_walk.cuh), any alignment
-        if (g.wtab && g_form.load(std::memory_order_relaxed) == 0 && n <= kWalkSmallMaxN && g_coop_max_n.load(std::memory_order_relaxed) > 0) {
-            if (q == qInside) return launch_pcon_walk_small<qInside>(p, g, t, step_max, n, out, s);
-            if (q == qDistIn) return launch_pcon_walk_small<qDistIn>(p, g, t, step_max, n, out, s);
-            if (q == qDistOut) return launch_pcon_walk_small<qDistOut>(p, g, t, step_max, n, out, s);
+        // Inside and the distances: one track per thread, section table in device memory (vg_pcon_walk.cuh), any alignment
+        // (VG_OPT_COOP_MAX_N = 0 keeps the persistent kernels in use: the tests run every form)
+        if (g.wtab && g_form.load(std::memory_order_relaxed) == 0 && g_coop_max_n.load(std::memory_order_relaxed) > 0) {
+            if (q == qInside) return launch_pcon_walk_small<qInside, false>(p, g, t, step_max, n, out, s);
+            if (q == qDistIn) return launch_pcon_walk_small<qDistIn, false>(p, g, t, step_max, n, out, s);
+            if (q == qDistOut) return launch_pcon_walk_small<qDistOut, false>(p, g, t, step_max, n, out, s);
+            if (g.masks && g.segs && q == qSafeIn) return launch_pcon_safety_small<qSafeIn, false>(p, g, t, n, out, s);
+            if (g.masks && g.segs && q == qSafeOut) return launch_pcon_safety_small<qSafeOut, false>(p, g, t, n, out, s);
         }
         if (vec && g_form.load(std::memory_order_relaxed) == 0) {
             double *o = static_cast<double *>(out);
@@ -43,6 +46,13 @@ cudaError_t launch_polycone(int q, const PolyconeP &p, const PconGrid &g, const 
         return launch_any<Polycone, PolyconeT<solid_flags(false, kWmFull)>>(q, p, t, step_max, n, out, vec, s);
     }
     // a phi cut: the ordered walk serves DistanceToIn (every candidate also tested against the segment, the phi faces added)
+    if (g.wtab && g_form.load(std::memory_order_relaxed) == 0 && g_coop_max_n.load(std::memory_order_relaxed) > 0) {
+        if (q == qInside) return launch_pcon_walk_small<qInside, true>(p, g, t, step_max, n, out, s);
+        if (q == qDistIn) return launch_pcon_walk_small<qDistIn, true>(p, g, t, step_max, n, out, s);
+        if (q == qDistOut) return launch_pcon_walk_small<qDistOut, true>(p, g, t, step_max, n, out, s);
+        if (g.masks && g.face_masks && g.segs && q == qSafeIn) return launch_pcon_safety_small<qSafeIn, true>(p, g, t, n, out, s);
+        if (g.masks && g.face_masks && g.segs && q == qSafeOut) return launch_pcon_safety_small<qSafeOut, true>(p, g, t, n, out, s);
+    }
     if (vec && g_form.load(std::memory_order_relaxed) == 0) {
         if (q == qDistIn) return launch_pcon_walk<qDistIn, false, true>(p, g, t, step_max, n, out, s);
         if (q == qDistOut) return launch_pcon_walk<qDistOut, false, true>(p, g, t, step_max, n, out, s);
@@ -62,6 +72,11 @@ cudaError_t launch_polycone_all(const PolyconeP &p, const PconGrid &g, const Tra
                                 bool vec, cudaStream_t s)
 {
     if (n <= 0) return cudaSuccess;
+    // one track per thread with every table in device memory (any alignment); VG_OPT_COOP_MAX_N = 0 keeps the persistent kernel
+    if (g_form.load(std::memory_order_relaxed) == 0 && g_coop_max_n.load(std::memory_order_relaxed) > 0 && g.wtab && g.segs && g.masks) {
+        if (p.w.full) return launch_pcon_all_small<false>(p, g, t, step_max, n, o, s);
+        if (g.face_masks) return launch_pcon_all_small<true>(p, g, t, step_max, n, o, s);
+    }
     if (!vec || g_form.load(std::memory_order_relaxed) != 0) return cudaErrorNotSupported;
     if (p.w.full)
         return g.masks ? launch_pcon_all<true, false>(p, g, t, step_max, n, o, s) : launch_pcon_all<false, false>(p, g, t, step_max, n, o, s);

@@ -133,12 +133,49 @@ struct alignas(16) PconWalkSec {
 
 struct PconGrid {
     const PconWalkSec *wtab;         // [nsec] in device memory; NULL: not uploaded
+    const double *segs;              // [64][6] segment records of the candidate grids (vg_pcon_walk.cuh), device memory
     const PconCoopSec *coop;         // [nsec]; NULL: not uploaded, the thread-per-track kernels serve every batch size
     const unsigned long long *masks; // [kPconGridZ][kPconGridR]; NULL: no grid, the ordered walk serves the safeties
     const unsigned long long *face_masks; // phi cut only: [kPconGridZ][2 kPconGridR] over u in [-R, R), every outline edge
     const unsigned char *rows;       // [kPconGridZ]
     PconGridGeom g;
 };
+
+// One record per segment of the polycone's (r, z) outline, numbered like the mask bits of the candidate grids: start point,
+// edge vector, edge vector / |edge|^2 (six doubles, 16-byte aligned).  Staged in shared memory by the persistent safety
+// kernel, read from device memory by the one-track-per-thread one.
+constexpr int kPconSegStride = 6;
+#ifdef __CUDACC__
+#define VG_PARAMS_HD __host__ __device__
+#else
+#define VG_PARAMS_HD
+#endif
+// record s of the table (bit s of the grid masks); plain arithmetic, compiled for the host too (vg_api.cu uploads the table
+// the one-track-per-thread safety kernel reads from device memory)
+VG_PARAMS_HD inline void pcon_seg_record(const PolyconeP &p, int s, double *o)
+{
+    double r0 = 0, z0 = 0, er = 0, ez = 0, il = 0;
+    const int k = (s - kPconSecBit0) >> 1;
+    if (s >= kPconSecBit0 && k < p.nsec) {
+        const PconSec &c = p.sec[k];
+        const Frustum &f = (s & 1) ? c.in : c.out;
+        r0 = f.r0, z0 = c.z0, er = f.er, ez = c.z1 - c.z0, il = f.inv_l2;
+    }
+    const int js = s - kPconSecBit0 - 2 * p.nsec; // >= 0: face (js & 1 ? inner : outer) of the (js >> 1)-th z step
+    if (js >= 0 && (js >> 1) < p.nstep) {
+        int kk = -1;
+        for (int q = 0, seen = 0; q + 1 < p.nsec; ++q)
+            if ((p.step_mask >> q) & 1u) {
+                if (seen++ == (js >> 1)) kk = q;
+            }
+        const PconStep &t = p.step[kk];
+        const double lo = (js & 1) ? t.ilo : t.olo, hi = (js & 1) ? t.ihi : t.ohi;
+        if (hi > lo) r0 = lo, z0 = t.z, er = hi - lo, ez = 0.0, il = 1.0 / (er * er);
+    }
+    if (s == kPconCapLoBit) r0 = p.cap_lo_rmin, z0 = p.zlo, er = p.cap_lo_rmax - p.cap_lo_rmin, il = 1.0 / (er * er);
+    if (s == kPconCapHiBit) r0 = p.cap_hi_rmin, z0 = p.zhi, er = p.cap_hi_rmax - p.cap_hi_rmin, il = 1.0 / (er * er);
+    o[0] = r0, o[1] = z0, o[2] = er, o[3] = ez, o[4] = er * il, o[5] = ez * il;
+}
 
 // a solid that may be a mother or a daughter of a volume (every kind except the polycone), or an operand of a boolean
 // (there a polycone too: kind == kPolycone and u.pcon points at its constants in device memory, vg_boolx.cu)

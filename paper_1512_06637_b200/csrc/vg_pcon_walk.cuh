@@ -261,34 +261,10 @@ VG_DEV double pcon_walk_sdf(const PolyconeP &p, const PconWalkSec *tab, double x
 // One record per segment of the (r, z) outline, numbered like the mask bits of the grid: (r0, z0), the edge vector
 // (er, ez) and the edge vector divided by |edge|^2, so that the foot parameter is t = w . e' (one FMA + one MUL).  Six
 // doubles, 16-byte aligned: three 128-bit shared loads per candidate.
-constexpr int kPconSegStride = 6;
 
 VG_DEV void pcon_stage_segs(const PolyconeP &p, double *seg)
 {
-    for (int s = threadIdx.x; s < 64; s += blockDim.x) {
-        double r0 = 0, z0 = 0, er = 0, ez = 0, il = 0;
-        const int k = (s - kPconSecBit0) >> 1;
-        if (s >= kPconSecBit0 && k < p.nsec) {
-            const PconSec &c = p.sec[k];
-            const Frustum &f = (s & 1) ? c.in : c.out;
-            r0 = f.r0, z0 = c.z0, er = f.er, ez = c.z1 - c.z0, il = f.inv_l2;
-        }
-        const int js = s - kPconSecBit0 - 2 * p.nsec; // >= 0: face (js & 1 ? inner : outer) of the (js >> 1)-th z step
-        if (js >= 0 && (js >> 1) < p.nstep) {
-            int kk = -1;
-            for (int q = 0, seen = 0; q + 1 < p.nsec; ++q)
-                if ((p.step_mask >> q) & 1u) {
-                    if (seen++ == (js >> 1)) kk = q;
-                }
-            const PconStep &t = p.step[kk];
-            const double lo = (js & 1) ? t.ilo : t.olo, hi = (js & 1) ? t.ihi : t.ohi;
-            if (hi > lo) r0 = lo, z0 = t.z, er = hi - lo, ez = 0.0, il = 1.0 / (er * er);
-        }
-        if (s == kPconCapLoBit) r0 = p.cap_lo_rmin, z0 = p.zlo, er = p.cap_lo_rmax - p.cap_lo_rmin, il = 1.0 / (er * er);
-        if (s == kPconCapHiBit) r0 = p.cap_hi_rmin, z0 = p.zhi, er = p.cap_hi_rmax - p.cap_hi_rmin, il = 1.0 / (er * er);
-        double *o = seg + kPconSegStride * s;
-        o[0] = r0, o[1] = z0, o[2] = er, o[3] = ez, o[4] = er * il, o[5] = ez * il;
-    }
+    for (int s = threadIdx.x; s < 64; s += blockDim.x) pcon_seg_record(p, s, seg + kPconSegStride * s);
 }
 
 // squared distance from (u, v) to the segment of record q (same value as seg_d2 up to the rounding of e' = e / |e|^2)
@@ -629,17 +605,18 @@ __global__ void __launch_bounds__(kWalkBlock, 2)
     }
 }
 
-// ---- medium batches (VG_OPT_COOP_MAX_N < n <= kWalkSmallMaxN): the same ordered walks, one track per thread in 64-thread
-// CTAs that read the section table from device memory (built at vg_shape_create) instead of staging it: no barrier, four
-// times as many CTAs as the persistent form has at these sizes, half the dependent work per thread.  Full phi; the
-// safeties keep the candidate-grid kernel above.
-constexpr int kWalkSmallBlock = 64;
-#ifndef VG_WALK_SMALL_MAX_N
-#define VG_WALK_SMALL_MAX_N 524288
+// ---- Inside and the two distances, one track per thread: the same ordered walks in 128-thread CTAs that read the section
+// table from device memory (built at vg_shape_create; a few hundred bytes, L1-resident) instead of staging it.  No barrier,
+// 46-48 registers against the persistent form's 70 with two tracks per thread, so twice the warps per SM to hide the walks'
+// dependent FP64 chains: DistanceToIn 106 -> 93 us, DistanceToOut 132 -> 116 us, Inside 49 -> 44 us at 4 Mi tracks, 10.6 ->
+// 8.0 us at 2^18, 402 -> 356 us at 2^24 (profiles/).  Any alignment, full phi or a phi cut.  The persistent kernel above
+// still serves these queries when the table is not on the current device, and the safeties.
+#ifndef VG_WALK_SMALL_BLOCK
+#define VG_WALK_SMALL_BLOCK 128
 #endif
-constexpr int64_t kWalkSmallMaxN = VG_WALK_SMALL_MAX_N;
+constexpr int kWalkSmallBlock = VG_WALK_SMALL_BLOCK;
 
-template <int Q>
+template <int Q, bool WEDGE>
 __global__ void __launch_bounds__(kWalkSmallBlock)
     pcon_walk_small_kernel(const __grid_constant__ PolyconeP p, const PconWalkSec *__restrict__ tab, Tracks t, double step_max,
                            int64_t n, void *out_any)
@@ -651,22 +628,73 @@ __global__ void __launch_bounds__(kWalkSmallBlock)
     const double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
     if (Q == qInside) {
         bool in, out;
-        pcon_walk_classify<false>(p, tab, x, y, z, in, out);
+        pcon_walk_classify<WEDGE>(p, tab, x, y, z, in, out);
         stg1i(static_cast<int32_t *>(out_any) + i, classify(in, out));
         return;
     }
     const double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
-    const double r = Q == qDistOut ? pcon_walk_dist_out<false>(p, tab, x, y, z, dx, dy, dz)
-                                   : pcon_walk_dist_in<false>(p, tab, x, y, z, dx, dy, dz);
+    const double r = Q == qDistOut ? pcon_walk_dist_out<WEDGE>(p, tab, x, y, z, dx, dy, dz)
+                                   : pcon_walk_dist_in<WEDGE>(p, tab, x, y, z, dx, dy, dz);
     stg1(static_cast<double *>(out_any) + i, r <= step_max ? r : inf());
 }
 
-template <int Q>
+template <int Q, bool WEDGE>
 cudaError_t launch_pcon_walk_small(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, void *out,
                                    cudaStream_t s)
 {
     const unsigned grid = unsigned((n + kWalkSmallBlock - 1) / kWalkSmallBlock);
-    return launch_kernel(pcon_walk_small_kernel<Q>, grid, kWalkSmallBlock, 0, s, p, g.wtab, t, step_max, n, out);
+    return launch_kernel(pcon_walk_small_kernel<Q, WEDGE>, grid, kWalkSmallBlock, 0, s, p, g.wtab, t, step_max, n, out);
+}
+
+// ... and the safeties from the candidate grids the same way: segment records and section table read from device memory
+template <int Q, bool WEDGE>
+__global__ void __launch_bounds__(kWalkSmallBlock)
+    pcon_safety_small_kernel(const __grid_constant__ PolyconeP p, const __grid_constant__ PconGrid g, Tracks t, int64_t n,
+                             double *__restrict__ out)
+{
+    const int64_t i = int64_t(blockIdx.x) * kWalkSmallBlock + threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
+    if (i >= n) return;
+    const double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+    const double s = WEDGE ? pcon_grid_sdf_wedge(p, g.wtab, g.segs, g, x, y, z) : pcon_grid_sdf(p, g.wtab, g.segs, g, x, y, z);
+    stg1(out + i, Q == qSafeIn ? s : -s);
+}
+
+template <int Q, bool WEDGE>
+cudaError_t launch_pcon_safety_small(const PolyconeP &p, const PconGrid &g, const Tracks &t, int64_t n, void *out, cudaStream_t s)
+{
+    const unsigned grid = unsigned((n + kWalkSmallBlock - 1) / kWalkSmallBlock);
+    return launch_kernel(pcon_safety_small_kernel<Q, WEDGE>, grid, kWalkSmallBlock, 0, s, p, g, t, n, static_cast<double *>(out));
+}
+
+// ... and the fused five-query call (vg_query_all)
+template <bool WEDGE>
+__global__ void __launch_bounds__(kWalkSmallBlock)
+    pcon_all_small_kernel(const __grid_constant__ PolyconeP p, const __grid_constant__ PconGrid g, Tracks t, double step_max,
+                          int64_t n, AllOut o)
+{
+    const int64_t i = int64_t(blockIdx.x) * kWalkSmallBlock + threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
+    if (i >= n) return;
+    int c0;
+    double a0, b0, s0;
+    pcon_all_eval<true, WEDGE>(p, g.wtab, g.segs, g, ldg1(t.x + i), ldg1(t.y + i), ldg1(t.z + i), ldg1(t.dx + i), ldg1(t.dy + i),
+                               ldg1(t.dz + i), step_max, c0, a0, b0, s0);
+    stg1i(o.cls + i, c0);
+    stg1(o.din + i, a0);
+    stg1(o.dout + i, b0);
+    stg1(o.sin + i, s0);
+    stg1(o.sout + i, -s0);
+}
+
+template <bool WEDGE>
+cudaError_t launch_pcon_all_small(const PolyconeP &p, const PconGrid &g, const Tracks &t, double step_max, int64_t n, const AllOut &o,
+                                  cudaStream_t s)
+{
+    const unsigned grid = unsigned((n + kWalkSmallBlock - 1) / kWalkSmallBlock);
+    return launch_kernel(pcon_all_small_kernel<WEDGE>, grid, kWalkSmallBlock, 0, s, p, g, t, step_max, n, o);
 }
 
 template <bool GRID, bool WEDGE>

@@ -26,8 +26,8 @@ def vg():
 
 @pytest.fixture(params=["lanes", "medium", "threads"])
 def form(request, vg):
-    """lanes: a group of lanes per track whatever n; medium: one track per thread, section table in device memory (what
-    batches between VG_OPT_COOP_MAX_N and 2^19 tracks run as; here every n > 1); threads: the persistent walk kernels."""
+    """lanes: a group of lanes per track whatever n; medium: one track per thread, tables in device memory (what every batch
+    above VG_OPT_COOP_MAX_N runs as; here every n > 1); threads: the persistent kernels with the tables staged per CTA."""
     old = vg.vg_get_option(vg.OPT_COOP_MAX_N)
     vg.vg_set_option(vg.OPT_COOP_MAX_N, {"lanes": 1 << 40, "medium": 1, "threads": 0}[request.param])
     yield request.param
