@@ -468,7 +468,7 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
     NavGrid &gr = mt.grid;
     gr.g[0] = gr.g[1] = gr.g[2] = gdim;
     gr.off_g = (mt.off_d + unsigned(nd) * unsigned(kDaughterStride) + 15u) / 16u * 16u;
-    const unsigned ncell = unsigned(gdim * gdim * gdim);
+    const unsigned ncell = unsigned((gdim + 2) * (gdim + 2) * (gdim + 2)); // with a ring of empty cells (vg_nav_cull.h)
     const unsigned nchunks_alloc = mt.nchunks == 3 ? 4u : unsigned(mt.nchunks); // kernels exist for 1, 2 and 4 chunks
     mt.bytes = (gr.off_g + 8u * ncell * (nchunks_alloc ? nchunks_alloc : 1u) + 15u) / 16u * 16u;
     if (nchunks_alloc) mt.nchunks = int(nchunks_alloc);
@@ -560,7 +560,7 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
                             d2 += d * d;
                         }
                         if (d2 <= rr * rr)
-                            cells[size_t((iz * gdim + iy) * gdim + ix) * mt.nchunks + i / 64] |= 1ull << (i % 64);
+                            cells[size_t(((iz + 1) * (gdim + 2) + iy + 1) * (gdim + 2) + ix + 1) * mt.nchunks + i / 64] |= 1ull << (i % 64);
                     }
         }
         // mean number of daughters listed per non-empty cell: above kNavDenseCell a ray meets many candidates and the warp

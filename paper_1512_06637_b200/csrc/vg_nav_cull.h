@@ -61,9 +61,9 @@ VG_HD bool nav_axis_clip(double p, double d, double L, double &t0, double &t1, d
 }
 
 // ... and set up the stepping: ray parameter of the next cell border on this axis (tmax), its increment per cell
-// (tdelta), the cells left before the walk leaves the grid, the cell index
+// (tdelta), the cell index
 VG_HD void nav_axis_init(double p, double d, double inv, double t0, double cs, double ics, int g, double &tmax,
-                         double &tdelta, int &left, int &i)
+                         double &tdelta, int &i)
 {
     double e = fma(t0, d, p); // entry coordinate relative to the grid origin
     i = int(floor(e * ics));
@@ -71,11 +71,12 @@ VG_HD void nav_axis_init(double p, double d, double inv, double t0, double cs, d
     const bool up = d > 0.0, still = inv == 0.0;
     tmax = still ? INFINITY : fma(double(i + (up ? 1 : 0)), cs, -p) * inv;
     tdelta = still ? 0.0 : cs * fabs(inv);
-    left = still ? 0 : (up ? g - 1 - i : i);
 }
 
-// Stage 1.  m[c] |= candidates of chunk c (64 daughters per chunk).  `cells`: [gz][gy][gx][NC] masks.
-// The loop body is branch-free (selects), so the lanes of a warp stay converged while they walk different cells.
+// Stage 1.  m[c] |= candidates of chunk c (64 daughters per chunk).  `cells`: [gz + 2][gy + 2][gx + 2][NC] masks: the grid
+// with a ring of EMPTY cells around it, so the walk needs no bounds test -- it stops when the next border lies beyond
+// t1 <= (the ray's exit from the grid) + slack, i.e. at the latest one step per axis into the ring.  The loop body is
+// branch-free (selects), so the lanes of a warp stay converged while they walk different cells.
 template <int NC>
 VG_HD void nav_grid_walk(const NavGrid &G, const unsigned long long *cells, double x, double y, double z, double dx,
                          double dy, double dz, double t_lim, unsigned long long (&m)[NC])
@@ -90,23 +91,22 @@ VG_HD void nav_grid_walk(const NavGrid &G, const unsigned long long *cells, doub
     ok = nav_axis_clip(pz, dz, G.len[2], t0, t1, ivz) && ok;
     if (!ok || !(t0 <= t1)) return;
     double tmx, tmy, tmz, tdx, tdy, tdz;
-    int lx, ly, lz, ix, iy, iz;
-    nav_axis_init(px, dx, ivx, t0, G.cs[0], G.ics[0], G.g[0], tmx, tdx, lx, ix);
-    nav_axis_init(py, dy, ivy, t0, G.cs[1], G.ics[1], G.g[1], tmy, tdy, ly, iy);
-    nav_axis_init(pz, dz, ivz, t0, G.cs[2], G.ics[2], G.g[2], tmz, tdz, lz, iz);
-    int idx = ix + G.g[0] * (iy + G.g[1] * iz);
-    const int stx = dx > 0.0 ? 1 : -1, sty = dy > 0.0 ? G.g[0] : -G.g[0], stz = dz > 0.0 ? G.g[0] * G.g[1] : -G.g[0] * G.g[1];
-    const int max_cells = G.g[0] + G.g[1] + G.g[2];
-    for (int it = 0; it < max_cells; ++it) { // a straight line crosses at most gx + gy + gz - 2 cells
+    int ix, iy, iz;
+    nav_axis_init(px, dx, ivx, t0, G.cs[0], G.ics[0], G.g[0], tmx, tdx, ix);
+    nav_axis_init(py, dy, ivy, t0, G.cs[1], G.ics[1], G.g[1], tmy, tdy, iy);
+    nav_axis_init(pz, dz, ivz, t0, G.cs[2], G.ics[2], G.g[2], tmz, tdz, iz);
+    const int sy_ = G.g[0] + 2, sz_ = sy_ * (G.g[1] + 2); // strides of the ringed array
+    int idx = (ix + 1) + sy_ * (iy + 1) + sz_ * (iz + 1);
+    const int stx = dx > 0.0 ? 1 : -1, sty = dy > 0.0 ? sy_ : -sy_, stz = dz > 0.0 ? sz_ : -sz_;
+    const int max_cells = G.g[0] + G.g[1] + G.g[2] + 3; // a straight line crosses at most gx + gy + gz - 2 cells (+ the ring)
+    for (int it = 0; it < max_cells; ++it) {
 #pragma unroll
         for (int c = 0; c < NC; ++c) m[c] |= cells[idx * NC + c];
         const bool sx = tmx <= tmy && tmx <= tmz, sy = !sx && tmy <= tmz, sz = !sx && !sy;
         const double tsel = sx ? tmx : (sy ? tmy : tmz);
-        const int left = sx ? lx : (sy ? ly : lz);
-        if (tsel > t1 || left == 0) break;
+        if (tsel >= t1) break; // (>= also ends a ray that moves along no axis: inf >= inf)
         idx += sx ? stx : (sy ? sty : stz);
         tmx += sx ? tdx : 0.0, tmy += sy ? tdy : 0.0, tmz += sz ? tdz : 0.0;
-        lx -= sx ? 1 : 0, ly -= sy ? 1 : 0, lz -= sz ? 1 : 0;
     }
 }
 

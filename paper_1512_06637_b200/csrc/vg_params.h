@@ -234,7 +234,8 @@ constexpr int kNavChunks = 4; // 64 daughters per chunk, VG_MAX_DAUGHTERS = 256
 constexpr int kNavKinds = 5;  // every kind except the polycone
 
 // Uniform grid over the bounding box of all daughter spheres in the mother frame (vg_nav_cull.h): g[0] x g[1] x g[2]
-// cells of size cs, each with one 64-bit candidate mask per chunk at blob offset off_g ([gz][gy][gx][nchunks]).
+// cells of size cs, each with one 64-bit candidate mask per chunk at blob offset off_g, stored with a ring of empty cells
+// around the grid ([gz + 2][gy + 2][gx + 2][nchunks]).
 constexpr int kNavGridMax = 8; // cells per axis
 struct NavGrid {
     double o[3], len[3], cs[3], ics[3]; // origin, extent, cell size and its inverse per axis
