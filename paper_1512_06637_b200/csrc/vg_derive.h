@@ -144,6 +144,8 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         // slanted edge of the +x face: half-widths dy1 -> dy2 over the slant height 2 dz cx; likewise +y
         t.inv_kx = 1 / ((t.dy2 - t.dy1) * (t.dy2 - t.dy1) + 4 * t.dz * t.dz * t.cx * t.cx);
         t.inv_ky = 1 / ((t.dx2 - t.dx1) * (t.dx2 - t.dx1) + 4 * t.dz * t.dz * t.cy * t.cy);
+        t.hex = t.dz * t.cx, t.hey = t.dz * t.cy;
+        t.sfx = t.icx * t.fx, t.sfy = t.icy * t.fy;
         return VG_OK;
     }
     case VG_POLYCONE: {

@@ -63,6 +63,8 @@ struct TrdP {
     double fx, mx, icx, cx; // X(z) = mx + fx z; cx = sqrt(1 + fx^2)
     double fy, my, icy, cy;
     double inv_kx, inv_ky;  // 1 / ((d2 - d1)^2 + (2 dz c)^2) for the slanted edge of the +x / +y face
+    double hex, hey;        // dz cx, dz cy: half-heights of the +x / +y face along its slant
+    double sfx, sfy;        // icx fx, icy fy: z shift of the foot of the perpendicular per unit plane distance
 };
 
 struct PconSec {

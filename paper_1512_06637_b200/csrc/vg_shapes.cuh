@@ -595,12 +595,12 @@ struct Trd {
         double D2 = fma(zx, zx, fma(zy, zy, zz * zz));
         // +x face: foot of the perpendicular, in-plane coordinates (|y|, slant coordinate)
         {
-            double zf = fma(gx * p.icx, p.fx, z);
-            D2 = dmin(D2, fma(gx, gx, trapezoid_d2(ay, zf * p.cx, p.dy1, p.dy2, p.dz * p.cx, p.inv_kx)));
+            double zf = fma(gx, p.sfx, z);
+            D2 = dmin(D2, fma(gx, gx, trapezoid_d2(ay, zf * p.cx, p.dy1, p.dy2, p.hex, p.inv_kx)));
         }
         {
-            double zf = fma(gy * p.icy, p.fy, z);
-            D2 = dmin(D2, fma(gy, gy, trapezoid_d2(ax, zf * p.cy, p.dx1, p.dx2, p.dz * p.cy, p.inv_ky)));
+            double zf = fma(gy, p.sfy, z);
+            D2 = dmin(D2, fma(gy, gy, trapezoid_d2(ax, zf * p.cy, p.dx1, p.dx2, p.hey, p.inv_ky)));
         }
         return g > 0.0 ? sqrt_nn(D2) : g;
     }
