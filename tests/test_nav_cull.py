@@ -19,7 +19,8 @@ import workloads as W
 
 
 def unit(v):
-    return v / np.linalg.norm(v, axis=-1, keepdims=True)
+    with np.errstate(divide="ignore", invalid="ignore"):  # a zero vector stays non-finite: the callers replace or reject it
+        return v / np.linalg.norm(v, axis=-1, keepdims=True)
 
 
 def isotropic(rng, n):
