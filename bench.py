@@ -993,6 +993,10 @@ def run_ours(args, rank, world, local_rank):
                 line["cpu_Mtq_s_1thr_allcores"] = {str(k): [pool[(k, t)][0] / pool[(k, t)][1] / 1e6 for t in sorted({t for kk, t in pool if kk == k})]
                                                    for k in sorted({kk for kk, _ in pool})}
                 line["per_config"] = per_config_rows(detail, fma_rate)
+                # the same ten answers per track pair from the two fused calls (vg_query_all) instead of ten launches
+                fused = [e for e in detail if e.get("config") == HEADLINE_CFG and str(e.get("query", "")).startswith("all five")]
+                if len(fused) == 2:
+                    line["value_fused_calls"] = sum(5 * e["n"] for e in fused) / sum(e["us_per_launch"] * 1e-6 for e in fused)
         line["detail"] = "bench_detail.json"
         try:
             with open(os.path.join(ROOT, "bench_detail.json"), "w") as f:
