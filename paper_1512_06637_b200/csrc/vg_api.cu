@@ -470,7 +470,8 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
     gr.off_g = (mt.off_d + unsigned(nd) * unsigned(kDaughterStride) + 15u) / 16u * 16u;
     const unsigned ncell = unsigned((gdim + 2) * (gdim + 2) * (gdim + 2)); // with a ring of empty cells (vg_nav_cull.h)
     const unsigned nchunks_alloc = mt.nchunks == 3 ? 4u : unsigned(mt.nchunks); // kernels exist for 1, 2 and 4 chunks
-    mt.bytes = (gr.off_g + 8u * ncell * (nchunks_alloc ? nchunks_alloc : 1u) + 15u) / 16u * 16u;
+    gr.off_p = (gr.off_g + 8u * ncell * (nchunks_alloc ? nchunks_alloc : 1u) + 15u) / 16u * 16u;
+    mt.bytes = (gr.off_p + 4u * ncell + 15u) / 16u * 16u;
     if (nchunks_alloc) mt.nchunks = int(nchunks_alloc);
     std::vector<double> sph; // bounding spheres of the daughters in the mother frame: cx, cy, cz, r (FP64)
     unsigned char *host = nullptr;
@@ -563,6 +564,22 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
                             cells[size_t(((iz + 1) * (gdim + 2) + iy + 1) * (gdim + 2) + ix + 1) * mt.nchunks + i / 64] |= 1ull << (i % 64);
                     }
         }
+        int *prim = reinterpret_cast<int *>(host + gr.off_p); // the only daughter of a cell, for the fused sphere test of the walk
+        unsigned singles = 0, filled = 0;
+        for (unsigned ic = 0; ic < ncell; ++ic) {
+            int pc = 0, only = -1;
+            for (int c = 0; c < mt.nchunks; ++c) {
+                const unsigned long long w = cells[size_t(ic) * mt.nchunks + c];
+                pc += __builtin_popcountll(w);
+                if (w) only = 64 * c + __builtin_ctzll(w);
+            }
+            prim[ic] = pc == 1 ? only : -1;
+            singles += pc == 1, filled += pc > 0;
+        }
+        // the fused test pays where nearly every cell the rays cross lists one daughter (configs[4]: all of them); in a mixed
+        // grid the lanes of a warp would split over both paths in every step of the walk, so it is switched off there
+        if (singles * 10 < filled * 9)
+            for (unsigned ic = 0; ic < ncell; ++ic) prim[ic] = -1;
         // mean number of daughters listed per non-empty cell: above kNavDenseCell a ray meets many candidates and the warp
         // pools phase 2 (vg_nav.cu)
         size_t listed = 0, nonempty = 0;
@@ -1048,19 +1065,20 @@ extern "C" int vg_debug_nav_cull(const vg_shape *mother, int nd, const vg_shape 
     const NavMeta &mt = v.meta;
     const float4 *cull = reinterpret_cast<const float4 *>(host);
     const unsigned long long *cells = reinterpret_cast<const unsigned long long *>(host + mt.grid.off_g);
+    const int *prim = reinterpret_cast<const int *>(host + mt.grid.off_p);
     if (grid)
         for (int a = 0; a < 3; ++a) grid[a] = mt.grid.o[a], grid[3 + a] = mt.grid.cs[a], grid[6 + a] = double(mt.grid.g[a]);
     for (int64_t i = 0; i < n; ++i) {
-        unsigned long long m[4] = { 0, 0, 0, 0 };
+        unsigned long long m[4] = { 0, 0, 0, 0 }, hit[4] = { 0, 0, 0, 0 };
         const double tl = t_lim ? t_lim[i] : INFINITY;
         if (stage == 0) { // both stages, as the kernel runs them
-            if (mt.nchunks == 1) nav_cull<1>(mt.grid, cull, cells, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m));
-            else if (mt.nchunks == 2) nav_cull<2>(mt.grid, cull, cells, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m));
-            else nav_cull<4>(mt.grid, cull, cells, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m);
+            if (mt.nchunks == 1) nav_cull<1>(mt.grid, cull, cells, prim, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m));
+            else if (mt.nchunks == 2) nav_cull<2>(mt.grid, cull, cells, prim, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m));
+            else nav_cull<4>(mt.grid, cull, cells, prim, mt.all, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m);
         } else if (stage == 1) { // the grid walk alone
-            if (mt.nchunks == 1) nav_grid_walk<1>(mt.grid, cells, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m));
-            else if (mt.nchunks == 2) nav_grid_walk<2>(mt.grid, cells, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m));
-            else nav_grid_walk<4>(mt.grid, cells, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m);
+            if (mt.nchunks == 1) nav_grid_walk<1, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m), reinterpret_cast<unsigned long long(&)[1]>(hit));
+            else if (mt.nchunks == 2) nav_grid_walk<2, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m), reinterpret_cast<unsigned long long(&)[2]>(hit));
+            else nav_grid_walk<4, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m, hit);
         } else { // the FP32 sphere test alone, applied to every daughter
             for (int c = 0; c < 4; ++c) m[c] = c < mt.nchunks ? mt.all[c] : 0ull;
             if (mt.nchunks == 1) nav_sphere_refine<1>(cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], reinterpret_cast<unsigned long long(&)[1]>(m));

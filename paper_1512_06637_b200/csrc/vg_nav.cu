@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const 
     const float4 *cull = reinterpret_cast<const float4 *>(smem_raw);
     const unsigned char *dtab = smem_raw + meta.off_d;
     const unsigned long long *cells = reinterpret_cast<const unsigned long long *>(smem_raw + meta.grid.off_g);
+    const int *prim = reinterpret_cast<const int *>(smem_raw + meta.grid.off_p);
     const int nd = meta.nd;
     int *q = q_all[threadIdx.x >> 5];
     double *res = res_all[threadIdx.x >> 5];
@@ -198,7 +199,7 @@ __global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const 
         int who = -1;
         if (nd > 0) {
             unsigned long long m[NC];
-            nav_cull<NC>(meta.grid, cull, cells, meta.all, x, y, z, dx, dy, dz, best < step_max ? best : step_max, m);
+            nav_cull<NC>(meta.grid, cull, cells, prim, meta.all, x, y, z, dx, dy, dz, best < step_max ? best : step_max, m);
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const unsigned long long mc = valid ? m[c] : 0ull;

@@ -229,6 +229,7 @@ struct Daughter {
 //   [off_d, off_d + nd stride) the Daughter records, stride = sizeof(Daughter) rounded up to an ODD number of 8-byte
 //                              words so that lanes reading different daughters spread over the shared-memory banks
 //   [off_g, off_g + 8 ncell nchunks)  candidate masks of the grid cells (NavGrid below), off_g a multiple of 16
+//   [off_p, off_p + 4 ncell)          the only daughter of each cell or -1
 //   total rounded up to a multiple of 16 bytes (bulk-copy granularity)
 constexpr int kCullUnroll = 8;
 constexpr int kDaughterStride = int(sizeof(Daughter)) + (((sizeof(Daughter) / 8) % 2 == 0) ? 8 : 0);
@@ -245,6 +246,8 @@ struct NavGrid {
     double rm2;                         // squared radius of the mother's bounding sphere about its origin, inflated
     int g[3];
     unsigned off_g;
+    unsigned off_p; // int32 per cell (same ringed layout): the cell's only daughter, -1 if it lists none or several
+    int pad;
 };
 
 struct NavMeta {
