@@ -18,6 +18,11 @@ else -- one row per (config, shape, query) of BASELINE.json configs[0..4] with i
 variants, the 8(f) rows, the Fig. 4 protocol, the oracle timed on every config -- is printed on EARLIER lines (one JSON
 object per line) and written to `bench_detail.json` beside this file.
 
+Extra keys of the compact line: `per_config` (<= 10 rows, one per (config, shape, N): the query furthest below its bound
+with us per launch and f / f8 / fp64 / lat fractions, `cl` = size-matched memory ceiling / measured, `pipe` = ncu's FP64-pipe
+utilisation of that kernel from the committed capture), `value_fused_calls` (the same ten answers per track pair from the
+two fused vg_query_all calls instead of ten launches), `cpu_Mtq_s_1thr_allcores` (the oracle per config).
+
 `--gpus N` without torchrun starts N ranks itself (torch.distributed.run, one rank per GPU, NCCL only for the timing
 reductions); under torchrun (WORLD_SIZE set) it runs as the rank it is.
 `--impl reference` times the oracle (oracle/, plain scalar CPU code) on the host cores on the same workload.

@@ -226,6 +226,7 @@ __global__ void __launch_bounds__(kNavBlock) nav_safety_kernel(const __grid_cons
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
+    const float4 *cull = reinterpret_cast<const float4 *>(smem_raw);
     const unsigned char *dtab = smem_raw + meta.off_d;
     const int nd = meta.nd;
 
@@ -252,6 +253,12 @@ __global__ void __launch_bounds__(kNavBlock) nav_safety_kernel(const __grid_cons
             double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
             double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
             double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
+            // the daughter lies inside the sphere of radius r about its local origin (r: the table's FP32 radius, which is
+            // inflated, so not smaller than the true one): sdf >= |l| - r.  A daughter with |l| - r >= best cannot lower
+            // the minimum and is skipped; the slack keeps the comparison on the safe side of its own rounding.
+            const double reach = best + double(sqrtf(cull[k].w)) * (1.0 + 1e-6);
+            const double l2 = fma(lx, lx, fma(ly, ly, lz * lz));
+            if (best > 0.0 && l2 >= reach * reach * (1.0 + 1e-12)) continue;
             best = dmin(best, solid_sdf(D.s, lx, ly, lz));
         }
         stg1(out + i, best);
