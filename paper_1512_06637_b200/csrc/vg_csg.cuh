@@ -98,8 +98,24 @@ VG_DEV double csg_sdf(const CsgP &p, double x, double y, double z)
     return st[0];
 }
 
+// next crossing of primitive i in the sense of its bit, seen from the point at ray parameter tt; +inf if none
+VG_DEV double csg_leaf_next(const CsgP &p, int i, bool inside, double tt, double x, double y, double z, double dx, double dy,
+                            double dz)
+{
+    const double *m = p.X[i];
+    double lx, ly, lz;
+    csg_to_leaf(m, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), lx, ly, lz);
+    const double ldx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
+    const double ldy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
+    const double ldz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
+    return solid_next<-1>(p.leaf[i], inside, lx, ly, lz, ldx, ldy, ldz);
+}
+
 // R28 / R32 read recursively: the state machine of bool_distance over one "inside" bit per primitive; primitives whose
-// class at the start is SURFACE get their bit from the sense of motion in the first pass
+// class at the start is SURFACE get their bit from the sense of motion in the first pass.  Every primitive's NEXT
+// crossing (an absolute ray parameter) is kept: an event flips one primitive, and only that one is asked again -- the
+// others' next crossings lie at or beyond the event and stay valid.  nleaf + events solid evaluations instead of
+// nleaf x events (698 -> 417 us for the four-primitive tree of bench.py at 4 Mi tracks).
 VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, double z, double dx, double dy, double dz)
 {
     unsigned in, out;
@@ -107,35 +123,32 @@ VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, doubl
     const int cls = csg_classify(p, in, out);
     if ((!to_out && cls == cInside) || (to_out && cls == cOutside)) return -1.0;
     unsigned bits = in;
-    unsigned pend = ~(in | out) & ((1u << p.nleaf) - 1u);
-    double tt = 0.0;
+    const unsigned pend = ~(in | out) & ((1u << p.nleaf) - 1u);
+    double tn[kCsgMaxLeaf];
+    unsigned fix = 0;
+#pragma unroll 1
+    for (int i = 0; i < p.nleaf; ++i) {
+        const double e = csg_leaf_next(p, i, (bits >> i) & 1u, 0.0, x, y, z, dx, dy, dz);
+        fix |= unsigned(((pend >> i) & 1u) && !(e <= kRayTol)) << i;
+        tn[i] = e;
+    }
+    if (fix) { // those primitives are being left, not entered: they were inside; ask them for the crossing they sit on
+        bits |= fix;
+#pragma unroll 1
+        for (int i = 0; i < p.nleaf; ++i)
+            if ((fix >> i) & 1u) tn[i] = csg_leaf_next(p, i, true, 0.0, x, y, z, dx, dy, dz);
+    }
 #pragma unroll 1
     for (int it = 0; it < kCsgMaxEvents; ++it) {
         double emin = inf();
         int imin = -1;
-        unsigned fix = 0;
-        const double px = fma(tt, dx, x), py = fma(tt, dy, y), pz = fma(tt, dz, z);
 #pragma unroll 1
-        for (int i = 0; i < p.nleaf; ++i) {
-            const double *m = p.X[i];
-            double lx, ly, lz;
-            csg_to_leaf(m, px, py, pz, lx, ly, lz);
-            const double ldx = fma(m[0], dx, fma(m[1], dy, m[2] * dz));
-            const double ldy = fma(m[4], dx, fma(m[5], dy, m[6] * dz));
-            const double ldz = fma(m[8], dx, fma(m[9], dy, m[10] * dz));
-            const double e = solid_next<-1>(p.leaf[i], (bits >> i) & 1u, lx, ly, lz, ldx, ldy, ldz);
-            fix |= unsigned(((pend >> i) & 1u) && !(e <= kRayTol)) << i;
-            if (e < emin) emin = e, imin = i; // strict: the lowest leaf wins a tie
-        }
-        pend = 0;
-        if (fix) { // those primitives are being left, not entered: they were inside
-            bits |= fix;
-            continue;
-        }
+        for (int i = 0; i < p.nleaf; ++i)
+            if (tn[i] < emin) emin = tn[i], imin = i; // strict: the lowest leaf wins a tie
         if (imin < 0) break;
-        tt += emin;
         bits ^= 1u << imin;
-        if (csg_member(p, bits) != to_out) return tt;
+        if (csg_member(p, bits) != to_out) return emin;
+        tn[imin] = emin + csg_leaf_next(p, imin, (bits >> imin) & 1u, emin, x, y, z, dx, dy, dz);
     }
     return inf();
 }
