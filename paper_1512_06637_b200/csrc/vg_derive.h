@@ -146,6 +146,8 @@ static int fill_shape(vg_shape *s, vg_kind kind, const double *p, int np)
         t.inv_ky = 1 / ((t.dx2 - t.dx1) * (t.dx2 - t.dx1) + 4 * t.dz * t.dz * t.cy * t.cy);
         t.hex = t.dz * t.cx, t.hey = t.dz * t.cy;
         t.sfx = t.icx * t.fx, t.sfy = t.icy * t.fy;
+        t.kxx = t.dy2 - t.dy1, t.kyx = 2.0 * t.hex, t.kxx_s = t.kxx * t.inv_kx, t.kyx_s = t.kyx * t.inv_kx;
+        t.kxy = t.dx2 - t.dx1, t.kyy = 2.0 * t.hey, t.kxy_s = t.kxy * t.inv_ky, t.kyy_s = t.kyy * t.inv_ky;
         return VG_OK;
     }
     case VG_POLYCONE: {

@@ -65,6 +65,8 @@ struct TrdP {
     double inv_kx, inv_ky;  // 1 / ((d2 - d1)^2 + (2 dz c)^2) for the slanted edge of the +x / +y face
     double hex, hey;        // dz cx, dz cy: half-heights of the +x / +y face along its slant
     double sfx, sfy;        // icx fx, icy fy: z shift of the foot of the perpendicular per unit plane distance
+    double kxx, kyx, kxx_s, kyx_s; // +x face: edge vector of its slanted side (dy2 - dy1, 2 hex), and the same / |edge|^2
+    double kxy, kyy, kxy_s, kyy_s; // +y face: (dx2 - dx1, 2 hey), and the same / |edge|^2
 };
 
 struct PconSec {

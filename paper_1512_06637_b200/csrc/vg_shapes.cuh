@@ -572,16 +572,18 @@ struct Trd {
         return classify(g < -kTol, g > kTol);
     }
     // squared in-plane distance from (v, s), v >= 0, to the filled symmetric trapezoid with half-widths r1 at
-    // s = -he and r2 at s = +he; 0 inside.  inv_k = 1 / ((r2-r1)^2 + (2 he)^2).
-    VG_DEV static double trapezoid_d2(double v, double s, double r1, double r2, double he, double inv_k)
+    // s = -he and r2 at s = +he; 0 inside.  (kx, ky) = the slanted side's edge vector (r2 - r1, 2 he), (kxs, kys) = the
+    // same divided by its squared length: the foot parameter is one FMA + one MUL, the offsets reuse (r2 - v), (he - s).
+    VG_DEV static double trapezoid_d2(double v, double s, double r1, double r2, double he, double kx, double ky, double kxs,
+                                      double kys)
     {
         double rc = s < 0.0 ? r1 : r2;
-        double cax = dmax(v - rc, 0.0), cay = fabs(s) - he;
-        double k2x = r2 - r1, k2y = 2.0 * he;
-        double h = fma(r2 - v, k2x, (he - s) * k2y) * inv_k;
+        double qa = v - rc, sa = qa + fabs(qa), cay = fabs(s) - he; // max(v - rc, 0)^2 = (qa + |qa|)^2 / 4
+        double wv = r2 - v, ws = he - s;
+        double h = fma(wv, kxs, ws * kys);
         h = dmin(dmax(h, 0.0), 1.0);
-        double cbx = fma(k2x, h, v - r2), cby = fma(k2y, h, s - he);
-        double d2 = dmin(fma(cax, cax, cay * cay), fma(cbx, cbx, cby * cby));
+        double cbx = fma(kx, h, -wv), cby = fma(ky, h, -ws);
+        double d2 = dmin(fma(0.25 * sa, sa, cay * cay), fma(cbx, cbx, cby * cby));
         return (cbx < 0.0 && cay < 0.0) ? 0.0 : d2;
     }
     VG_DEV static double safety(const P &p, double x, double y, double z)
@@ -596,11 +598,11 @@ struct Trd {
         // +x face: foot of the perpendicular, in-plane coordinates (|y|, slant coordinate)
         {
             double zf = fma(gx, p.sfx, z);
-            D2 = dmin(D2, fma(gx, gx, trapezoid_d2(ay, zf * p.cx, p.dy1, p.dy2, p.hex, p.inv_kx)));
+            D2 = dmin(D2, fma(gx, gx, trapezoid_d2(ay, zf * p.cx, p.dy1, p.dy2, p.hex, p.kxx, p.kyx, p.kxx_s, p.kyx_s)));
         }
         {
             double zf = fma(gy, p.sfy, z);
-            D2 = dmin(D2, fma(gy, gy, trapezoid_d2(ax, zf * p.cy, p.dx1, p.dx2, p.hey, p.inv_ky)));
+            D2 = dmin(D2, fma(gy, gy, trapezoid_d2(ax, zf * p.cy, p.dx1, p.dx2, p.hey, p.kxy, p.kyy, p.kxy_s, p.kyy_s)));
         }
         return g > 0.0 ? sqrt_nn(D2) : g;
     }
