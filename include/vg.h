@@ -280,7 +280,9 @@ int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, c
  * pipeline (clamped to 2^20).
  * VG_OPT_COOP_MAX_N (default VG_COOP_MAX_N_DEFAULT): queries of a full-phi polycone over at most this many tracks run as
  *   the lanes-per-track kernel (a group of 4..32 lanes shares one track and splits its sections):
- *   lowest latency for small batches, same results.  0 switches the form off.
+ *   lowest latency for small batches, same results.  0 switches the form off, and with it the one-track-per-thread
+ *   polycone kernels that serve larger batches (the persistent kernels with per-CTA staged tables run instead: the
+ *   tests use this to keep every form under parity).
  * VG_OPT_NAV_FORM (default 0 = chosen per volume): how vg_compute_step evaluates the daughters that survive its cull
  *   (same results).  1: every lane walks its own candidates.  2: the candidates of a warp's 32 tracks are pooled and
  *   evaluated as one dense work list (a warp cooperates over daughters).  0 takes 2 for volumes whose candidate grid

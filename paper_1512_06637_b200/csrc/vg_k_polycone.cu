@@ -1,6 +1,11 @@
-// vg_k_polycone.cu -- instantiates the query kernels of the polycone: the run-time-flag form, the full-phi
-// specialisation, and the ordered-walk kernels (vg_pcon_walk.cuh) that serve DistanceToIn and the safeties of a
-// full-phi polycone when the arrays are 16-byte aligned (VG_FORM_AUTO; any forced form runs the generic kernels).
+// vg_k_polycone.cu -- instantiates the query kernels of the polycone and picks the form a call runs as (VG_FORM_AUTO; any
+// forced form runs the generic streaming kernels over all sections):
+//   n <= VG_OPT_COOP_MAX_N, full phi   a group of lanes per track (vg_pcon_coop.cuh)
+//   above it                            one track per thread, section / segment tables in device memory
+//                                       (vg_pcon_walk.cuh: ordered walks for Inside and the distances, candidate grids
+//                                       for the safeties; full phi or a phi cut, any alignment)
+//   tables not on the current device,   the persistent kernels with the tables staged per CTA (16-byte aligned arrays),
+//   or VG_OPT_COOP_MAX_N = 0            else the generic kernels
 #include "vg_pcon_coop.cuh"
 #include "vg_pcon_walk.cuh"
 
