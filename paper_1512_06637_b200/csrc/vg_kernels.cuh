@@ -174,7 +174,7 @@ struct AllOut {
 };
 
 #ifndef VG_ALL_MINB
-#define VG_ALL_MINB 3
+#define VG_ALL_MINB 4
 #endif
 
 template <class S>
@@ -188,53 +188,38 @@ VG_DEV void eval_all(const typename S::P &p, double x, double y, double z, doubl
     dout = b <= step_max ? b : inf();
 }
 
-template <class S, int TPT>
+// One track per thread, capped at 64 registers (4 CTAs of 256 threads per SM): the five answers are ~400 instructions of
+// dependent FP64 work per track, and what bounds the kernel is the number of warps there are to overlap those chains,
+// not its loads.  Two tracks per thread with 128-bit loads (80 registers, 3 CTAs) measured 4-6 % slower for the tube and
+// the cone (20.7 -> 19.4 us at 1 Mi, 74.2 -> 71.2 us at 4 Mi tracks) and the same for the trd.
+template <class S>
 __global__ void __launch_bounds__(kBlock, VG_ALL_MINB)
     query_all_kernel(const __grid_constant__ typename S::P p, Tracks t, double step_max, int64_t n, AllOut o)
 {
-    int64_t i = (int64_t(blockIdx.x) * kBlock + threadIdx.x) * TPT;
+    const int64_t i = int64_t(blockIdx.x) * kBlock + threadIdx.x;
     pdl_launch_dependents();
     pdl_wait();
     if (i >= n) return;
-    if (TPT == 2 && i + 1 < n) {
-        double2 x = ldg2(t.x + i), y = ldg2(t.y + i), z = ldg2(t.z + i);
-        double2 dx = ldg2(t.dx + i), dy = ldg2(t.dy + i), dz = ldg2(t.dz + i);
-        int c0, c1;
-        double a0, a1, b0, b1, s0, s1;
-        eval_all<S>(p, x.x, y.x, z.x, dx.x, dy.x, dz.x, step_max, c0, a0, b0, s0);
-        eval_all<S>(p, x.y, y.y, z.y, dx.y, dy.y, dz.y, step_max, c1, a1, b1, s1);
-        stg2i(o.cls + i, c0, c1);
-        stg2(o.din + i, a0, a1);
-        stg2(o.dout + i, b0, b1);
-        stg2(o.sin + i, s0, s1);
-        stg2(o.sout + i, -s0, -s1);
-    } else {
-        double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
-        double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
-        int c0;
-        double a0, b0, s0;
-        eval_all<S>(p, x, y, z, dx, dy, dz, step_max, c0, a0, b0, s0);
-        stg1i(o.cls + i, c0);
-        stg1(o.din + i, a0);
-        stg1(o.dout + i, b0);
-        stg1(o.sin + i, s0);
-        stg1(o.sout + i, -s0);
-    }
+    double x = ldg1(t.x + i), y = ldg1(t.y + i), z = ldg1(t.z + i);
+    double dx = ldg1(t.dx + i), dy = ldg1(t.dy + i), dz = ldg1(t.dz + i);
+    int c0;
+    double a0, b0, s0;
+    eval_all<S>(p, x, y, z, dx, dy, dz, step_max, c0, a0, b0, s0);
+    stg1i(o.cls + i, c0);
+    stg1(o.din + i, a0);
+    stg1(o.dout + i, b0);
+    stg1(o.sin + i, s0);
+    stg1(o.sout + i, -s0);
 }
 
 template <class S>
 cudaError_t launch_all(const typename S::P &p, const Tracks &t, double step_max, int64_t n, const AllOut &o, bool vec,
                        cudaStream_t stream)
 {
+    (void)vec; // any alignment
     if (n <= 0) return cudaSuccess;
-    if (n < kSmallBatchTpt1) vec = false; // see launch_query
-    if (vec) {
-        int64_t threads = (n + 1) / 2;
-        unsigned grid = unsigned((threads + kBlock - 1) / kBlock);
-        return launch_kernel(query_all_kernel<S, 2>, grid, kBlock, 0, stream, p, t, step_max, n, o);
-    }
     unsigned grid = unsigned((n + kBlock - 1) / kBlock);
-    return launch_kernel(query_all_kernel<S, 1>, grid, kBlock, 0, stream, p, t, step_max, n, o);
+    return launch_kernel(query_all_kernel<S>, grid, kBlock, 0, stream, p, t, step_max, n, o);
 }
 
 // ---- the pipelined form of the same kernel (the default for 16-byte aligned arrays and n >= g_pipe_min_n) ----
