@@ -1,5 +1,6 @@
 """Launches every kernel of libvg once on small odd-sized inputs (all solids, all queries, every kernel form, 8-byte-only
-alignment, the fused call, ComputeStep, the world, a boolean of every operand kind, the host entry points).  Not a test
+alignment, the three polycone forms, the fused call, ComputeStep in both phase-2 forms, the world, a boolean of every
+operand kind, the host entry points).  Not a test
 by itself (`python tests/exercise_all_kernels.py` on a GPU box; tests/test_gpu_nav_and_edges.py runs it as one).  compute-sanitizer
 is closed on this pool, so the script brings its own bounds check: every result array sits between guard words that must
 come back untouched, sizes are odd, and every result is compared with the oracle."""
@@ -68,7 +69,26 @@ def check_shape(kind, par, what):
             assert_real_close(sg.safety_to_in(*dt[:3]).cpu().numpy(), so.safety_to_in(*t[:3]), what)
             assert_real_close(sg.safety_to_out(*dt[:3]).cpu().numpy(), so.safety_to_out(*t[:3]), what)
     vg.vg_set_option(vg.OPT_FORM, vg.FORM_AUTO)
-    fused = sg.query_all(*dev(t), W.STEP_MAX)
+    if kind == W.POLYCONE:  # the three polycone forms: a group of lanes per track, one track per thread, persistent CTAs
+        old = vg.vg_get_option(vg.OPT_COOP_MAX_N)
+        for coop in (1 << 40, 1, 0):
+            vg.vg_set_option(vg.OPT_COOP_MAX_N, coop)
+            for mis in (False, True):
+                dt = dev(t, mis)
+                sh = 1 if mis else 0
+                bi, oi = guarded(N, torch.int32, sh)
+                assert_int_equal(sg.inside(*dt[:3], out=oi).cpu().numpy(), so.inside(*t[:3]), what + " form %d" % coop)
+                assert guards_intact(bi, N, sh), what + " inside form %d: write outside the result array" % coop
+                for q in ("distance_to_in", "distance_to_out", "safety_to_in", "safety_to_out"):
+                    bd, od = guarded(N, torch.float64, sh)
+                    g = sg.query(q, *dt, step_max=W.STEP_MAX, out=od) if q.startswith("distance") else sg.query(q, *dt[:3], out=od)
+                    o = getattr(so, q)(*t, W.STEP_MAX) if q.startswith("distance") else getattr(so, q)(*t[:3])
+                    assert_real_close(g.cpu().numpy(), o, what + " %s form %d" % (q, coop))
+                    assert guards_intact(bd, N, sh), what + " %s form %d: write outside the result array" % (q, coop)
+        vg.vg_set_option(vg.OPT_COOP_MAX_N, old)
+    gb = [guarded(N, torch.int32)] + [guarded(N, torch.float64) for _ in range(4)]  # the fused call, every output guarded
+    fused = sg.query_all(*dev(t), W.STEP_MAX, out=[g[1] for g in gb])
+    assert all(guards_intact(g[0], N) for g in gb), what + " fused: write outside a result array"
     assert_real_close(fused[1].cpu().numpy(), so.distance_to_in(*t, W.STEP_MAX), what + " fused")
     ht = [torch.from_numpy(a).pin_memory() for a in t]
     assert_real_close(sg.query_host("distance_to_out", *ht, step_max=W.STEP_MAX).numpy(), so.distance_to_out(*t, W.STEP_MAX), what + " host")
@@ -93,9 +113,15 @@ def main():
     vgv = vg.Volume(vg.Shape(nav.mother_kind, nav.mother_params), [vg.Shape(k, p) for k, p in zip(nav.daughter_kinds, nav.daughter_params)], nav.xforms)
     t = nav.tracks(N, band=lambda x, y, z: vo.safety(x, y, z) < W.SURFACE_BAND)
     so, ho = vo.compute_step(*t, W.STEP_MAX)
-    sg, hg = vgv.compute_step(*dev(t), W.STEP_MAX)
-    assert_int_equal(hg.cpu().numpy(), ho, "compute_step hit")
-    assert_real_close(sg.cpu().numpy(), so, "compute_step")
+    for form in (1, 2, 0):  # phase 2 per lane, pooled over the warp, the library's choice
+        vg.vg_set_option(vg.OPT_NAV_FORM, form)
+        bs, os_ = guarded(N, torch.float64)
+        bh, oh = guarded(N, torch.int32)
+        sg, hg = vgv.compute_step(*dev(t), W.STEP_MAX, step=os_, hit=oh)
+        assert_int_equal(hg.cpu().numpy(), ho, "compute_step hit form %d" % form)
+        assert_real_close(sg.cpu().numpy(), so, "compute_step form %d" % form)
+        assert guards_intact(bs, N) and guards_intact(bh, N), "compute_step form %d: write outside a result array" % form
+    vg.vg_set_option(vg.OPT_NAV_FORM, 0)
     assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), vo.safety(*t[:3]), "volume safety")
     wc = W.world_case()
     wo = O.World([O.Shape(k, p) for k, p in zip(wc.kinds, wc.params)], wc.parents, wc.xforms)
