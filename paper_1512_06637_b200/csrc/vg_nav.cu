@@ -29,6 +29,11 @@ namespace vg {
 #define VG_NAV_MINB 3
 #endif
 constexpr int kNavBlock = VG_NAV_BLOCK;
+#ifndef VG_NAV_SMALL_N
+#define VG_NAV_SMALL_N (148 * 64)
+#endif
+constexpr int kNavSmallBlock = 64;          // CTA size of ComputeStep for batches below kNavSmallN tracks
+constexpr int64_t kNavSmallN = VG_NAV_SMALL_N;
 
 // one elected thread: arm the barrier with the byte count and issue the bulk copy global -> shared
 VG_DEV void tma_load_table(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
@@ -152,9 +157,11 @@ VG_DEV void coop_candidates(unsigned long long mk, int base, const unsigned char
     }
 }
 
-// ComputeStep; NC = chunks of 64 daughters (1, 2 or 4); COOP = phase 2 pooled over the warp, else per lane
-template <int NC, bool COOP>
-__global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const __grid_constant__ SolidU mother,
+// ComputeStep; NC = chunks of 64 daughters (1, 2 or 4); COOP = phase 2 pooled over the warp, else per lane; BLOCK = CTA
+// size: kNavBlock for batches that fill the GPU, kNavSmallBlock for small ones (four times the CTAs: a 1,024-track call
+// runs on 16 SMs instead of 4)
+template <int NC, bool COOP, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, BLOCK == kNavBlock ? VG_NAV_MINB : 1) nav_step_kernel(const __grid_constant__ SolidU mother,
                                                              const __grid_constant__ NavMeta meta,
                                                              const unsigned char *__restrict__ table, Tracks t,
                                                              double step_max, int64_t n, double *__restrict__ out,
@@ -162,8 +169,8 @@ __global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const 
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar;
-    __shared__ int q_all[kNavBlock / 32][kCoopQueue];
-    __shared__ double res_all[kNavBlock / 32][kCoopQueue];
+    __shared__ int q_all[BLOCK / 32][kCoopQueue];
+    __shared__ double res_all[BLOCK / 32][kCoopQueue];
     const float4 *cull = reinterpret_cast<const float4 *>(smem_raw);
     const unsigned char *dtab = smem_raw + meta.off_d;
     const unsigned long long *cells = reinterpret_cast<const unsigned long long *>(smem_raw + meta.grid.off_g);
@@ -183,7 +190,7 @@ __global__ void __launch_bounds__(kNavBlock, VG_NAV_MINB) nav_step_kernel(const 
     bool waited = (nd == 0);
 
     // warp-uniform trip count: the lanes past n take part in the warp's collectives with an empty candidate list
-    for (int64_t tile = int64_t(blockIdx.x) * kNavBlock; tile < n; tile += int64_t(gridDim.x) * kNavBlock) {
+    for (int64_t tile = int64_t(blockIdx.x) * BLOCK; tile < n; tile += int64_t(gridDim.x) * BLOCK) {
         const int64_t i = tile + threadIdx.x;
         const bool valid = i < n;
         double x = 0, y = 0, z = 0, dx = 0, dy = 0, dz = 1;
@@ -277,7 +284,7 @@ struct NavDevState {
 };
 
 template <class Kern>
-static cudaError_t nav_grid_size(Kern kern, NavDevState *states, size_t smem, int64_t n, unsigned *grid)
+static cudaError_t nav_grid_size(Kern kern, NavDevState *states, size_t smem, int64_t n, unsigned *grid, int block = kNavBlock)
 {
     constexpr int kMaxDev = 64;
     int dev = 0;
@@ -295,25 +302,33 @@ static cudaError_t nav_grid_size(Kern kern, NavDevState *states, size_t smem, in
         st.granted = smem;
     }
     if (smem != st.occ_smem) {
-        if ((err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&st.per_sm, kern, kNavBlock, smem)) != cudaSuccess) return err;
+        if ((err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&st.per_sm, kern, block, smem)) != cudaSuccess) return err;
         if (st.per_sm < 1) st.per_sm = 1;
         st.occ_smem = smem;
     }
-    const int64_t want = (n + kNavBlock - 1) / kNavBlock;
+    const int64_t want = (n + block - 1) / block;
     const int64_t cap = int64_t(st.sm_count) * st.per_sm; // persistent: one resident wave, a multiple of the SM count
     *grid = unsigned(want < cap ? want : cap);
     return cudaSuccess;
+}
+
+template <int NC, bool COOP, int BLOCK>
+static cudaError_t launch_step_nc_b(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
+                                    double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
+{
+    static NavDevState states[64];
+    unsigned grid = 0;
+    cudaError_t err = nav_grid_size(nav_step_kernel<NC, COOP, BLOCK>, states, meta.bytes, n, &grid, BLOCK);
+    if (err != cudaSuccess) return err;
+    return launch_kernel(nav_step_kernel<NC, COOP, BLOCK>, grid, BLOCK, meta.bytes, s, mother, meta, table_dev, t, step_max, n, step, hit);
 }
 
 template <int NC, bool COOP>
 static cudaError_t launch_step_nc(const SolidU &mother, const unsigned char *table_dev, const NavMeta &meta, const Tracks &t,
                                   double step_max, int64_t n, double *step, int32_t *hit, cudaStream_t s)
 {
-    static NavDevState states[64];
-    unsigned grid = 0;
-    cudaError_t err = nav_grid_size(nav_step_kernel<NC, COOP>, states, meta.bytes, n, &grid);
-    if (err != cudaSuccess) return err;
-    return launch_kernel(nav_step_kernel<NC, COOP>, grid, kNavBlock, meta.bytes, s, mother, meta, table_dev, t, step_max, n, step, hit);
+    if (n < kNavSmallN) return launch_step_nc_b<NC, COOP, kNavSmallBlock>(mother, table_dev, meta, t, step_max, n, step, hit, s);
+    return launch_step_nc_b<NC, COOP, kNavBlock>(mother, table_dev, meta, t, step_max, n, step, hit, s);
 }
 
 template <bool COOP>
