@@ -451,6 +451,74 @@ static int to_solid(const vg_shape *s, SolidU *o, const char *what)
 
 constexpr double kNavDenseCell = 24.0; // measured: pooling pays only where nearly every daughter is a candidate of every ray
 
+// Fills the candidate grid of vg_nav_cull.h for nd bounding spheres (`sph`: cx, cy, cz, r per sphere, in the frame the rays
+// are in; r already carries the inflation of the FP32 test): geometry into `gr` (gdim cells per axis over the bounding box
+// of the spheres), the cells' masks (ringed layout, `nchunks` 64-bit words per cell, zero-initialised by the caller),
+// `prim` (the only sphere of a cell, or -1) and whether the cells list many spheres each.  `r_frame` = radius of the
+// sphere about the frame's origin that holds every start point the error bounds are stated for.
+static void nav_grid_fill(const std::vector<double> &sph, int nd, int nchunks, int gdim, double r_frame, NavGrid &gr,
+                          unsigned long long *cells, int *prim, bool *dense_out)
+{
+    gr.g[0] = gr.g[1] = gr.g[2] = gdim;
+    const unsigned ncell = unsigned((gdim + 2) * (gdim + 2) * (gdim + 2));
+    double lo[3] = { 0, 0, 0 }, hi[3] = { 0, 0, 0 };
+    for (int i = 0; i < nd; ++i)
+        for (int a = 0; a < 3; ++a) {
+            double l = sph[4 * i + a] - sph[4 * i + 3], h = sph[4 * i + a] + sph[4 * i + 3];
+            lo[a] = i == 0 ? l : std::fmin(lo[a], l);
+            hi[a] = i == 0 ? h : std::fmax(hi[a], h);
+        }
+    double diag = 0;
+    for (int a = 0; a < 3; ++a) {
+        double ext = hi[a] - lo[a];
+        if (!(ext > 0)) ext = 1.0;
+        lo[a] -= 1e-6 * ext, ext *= 1.0 + 2e-6;
+        gr.o[a] = lo[a], gr.len[a] = ext, gr.cs[a] = ext / gdim, gr.ics[a] = gdim / ext;
+        diag += ext * ext;
+    }
+    diag = std::sqrt(diag);
+    const double pad = 1e-6 * (diag + r_frame); // see vg_nav_cull.h: covers the rounding of the walk
+    gr.tpad = pad;
+    gr.rm2 = r_frame * r_frame * (1.0 + 1e-9);
+    for (int i = 0; i < nd; ++i) {
+        const double *c = &sph[4 * i];
+        const double rr = c[3] * (1.0 + 1e-6) + pad;
+        for (int iz = 0; iz < gdim; ++iz)
+            for (int iy = 0; iy < gdim; ++iy)
+                for (int ix = 0; ix < gdim; ++ix) {
+                    const int ic[3] = { ix, iy, iz };
+                    double d2 = 0;
+                    for (int a = 0; a < 3; ++a) { // distance from the sphere centre to the closed cell
+                        double l = gr.o[a] + ic[a] * gr.cs[a], h = l + gr.cs[a];
+                        double d = c[a] < l ? l - c[a] : (c[a] > h ? c[a] - h : 0.0);
+                        d2 += d * d;
+                    }
+                    if (d2 <= rr * rr)
+                        cells[size_t(((iz + 1) * (gdim + 2) + iy + 1) * (gdim + 2) + ix + 1) * nchunks + i / 64] |= 1ull << (i % 64);
+                }
+    }
+    unsigned singles = 0, filled = 0;
+    size_t listed = 0;
+    for (unsigned ic = 0; ic < ncell; ++ic) {
+        int pc = 0, only = -1;
+        for (int c = 0; c < nchunks; ++c) {
+            const unsigned long long w = cells[size_t(ic) * nchunks + c];
+            pc += __builtin_popcountll(w);
+            if (w) only = 64 * c + __builtin_ctzll(w);
+        }
+        prim[ic] = pc == 1 ? only : -1;
+        singles += pc == 1, filled += pc > 0;
+        listed += size_t(pc);
+    }
+    // the fused test pays where nearly every cell the rays cross lists one sphere (configs[4]: all of them); in a mixed
+    // grid the lanes of a warp would split over both paths in every step of the walk, so it is switched off there
+    if (singles * 10 < filled * 9)
+        for (unsigned ic = 0; ic < ncell; ++ic) prim[ic] = -1;
+    // mean number of spheres listed per non-empty cell: above kNavDenseCell a ray meets many candidates and the warp
+    // pools phase 2 (vg_nav.cu)
+    *dense_out = filled && double(listed) / double(filled) > kNavDenseCell;
+}
+
 // Host side of vg_volume_create for a volume of primitives: validation, the mother and daughter records, the FP32
 // bounding spheres and the candidate grid, as one blob in host memory (layout: vg_params.h).  No CUDA call.
 static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
@@ -466,7 +534,6 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
     int gdim = 1;
     while (gdim < kNavGridMax && gdim * gdim * gdim < nd) ++gdim;
     NavGrid &gr = mt.grid;
-    gr.g[0] = gr.g[1] = gr.g[2] = gdim;
     gr.off_g = (mt.off_d + unsigned(nd) * unsigned(kDaughterStride) + 15u) / 16u * 16u;
     const unsigned ncell = unsigned((gdim + 2) * (gdim + 2) * (gdim + 2)); // with a ring of empty cells (vg_nav_cull.h)
     const unsigned nchunks_alloc = mt.nchunks == 3 ? 4u : unsigned(mt.nchunks); // kernels exist for 1, 2 and 4 chunks
@@ -526,69 +593,11 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
         mt.all[i / 64] |= 1ull << (i % 64);
         sph.insert(sph.end(), { cx, cy, cz, std::sqrt(double(e[3])) });
     }
-    if (rc == VG_OK) { // the grid over the bounding box of the spheres; each cell lists the spheres (inflated) that meet it
-        double lo[3] = { 0, 0, 0 }, hi[3] = { 0, 0, 0 };
-        for (int i = 0; i < nd; ++i)
-            for (int a = 0; a < 3; ++a) {
-                double l = sph[4 * i + a] - sph[4 * i + 3], h = sph[4 * i + a] + sph[4 * i + 3];
-                lo[a] = i == 0 ? l : std::fmin(lo[a], l);
-                hi[a] = i == 0 ? h : std::fmax(hi[a], h);
-            }
-        double diag = 0;
-        for (int a = 0; a < 3; ++a) {
-            double ext = hi[a] - lo[a];
-            if (!(ext > 0)) ext = 1.0;
-            lo[a] -= 1e-6 * ext, ext *= 1.0 + 2e-6;
-            gr.o[a] = lo[a], gr.len[a] = ext, gr.cs[a] = ext / gdim, gr.ics[a] = gdim / ext;
-            diag += ext * ext;
-        }
-        diag = std::sqrt(diag);
-        const double pad = 1e-6 * (diag + r_mother); // see vg_nav_cull.h: covers the rounding of the walk
-        gr.tpad = pad;
-        gr.rm2 = r_mother * r_mother * (1.0 + 1e-9);
-        unsigned long long *cells = reinterpret_cast<unsigned long long *>(host + gr.off_g);
-        for (int i = 0; i < nd; ++i) {
-            const double *c = &sph[4 * i];
-            const double rr = c[3] * (1.0 + 1e-6) + pad;
-            for (int iz = 0; iz < gdim; ++iz)
-                for (int iy = 0; iy < gdim; ++iy)
-                    for (int ix = 0; ix < gdim; ++ix) {
-                        const int ic[3] = { ix, iy, iz };
-                        double d2 = 0;
-                        for (int a = 0; a < 3; ++a) { // distance from the sphere centre to the closed cell
-                            double l = gr.o[a] + ic[a] * gr.cs[a], h = l + gr.cs[a];
-                            double d = c[a] < l ? l - c[a] : (c[a] > h ? c[a] - h : 0.0);
-                            d2 += d * d;
-                        }
-                        if (d2 <= rr * rr)
-                            cells[size_t(((iz + 1) * (gdim + 2) + iy + 1) * (gdim + 2) + ix + 1) * mt.nchunks + i / 64] |= 1ull << (i % 64);
-                    }
-        }
-        int *prim = reinterpret_cast<int *>(host + gr.off_p); // the only daughter of a cell, for the fused sphere test of the walk
-        unsigned singles = 0, filled = 0;
-        for (unsigned ic = 0; ic < ncell; ++ic) {
-            int pc = 0, only = -1;
-            for (int c = 0; c < mt.nchunks; ++c) {
-                const unsigned long long w = cells[size_t(ic) * mt.nchunks + c];
-                pc += __builtin_popcountll(w);
-                if (w) only = 64 * c + __builtin_ctzll(w);
-            }
-            prim[ic] = pc == 1 ? only : -1;
-            singles += pc == 1, filled += pc > 0;
-        }
-        // the fused test pays where nearly every cell the rays cross lists one daughter (configs[4]: all of them); in a mixed
-        // grid the lanes of a warp would split over both paths in every step of the walk, so it is switched off there
-        if (singles * 10 < filled * 9)
-            for (unsigned ic = 0; ic < ncell; ++ic) prim[ic] = -1;
-        // mean number of daughters listed per non-empty cell: above kNavDenseCell a ray meets many candidates and the warp
-        // pools phase 2 (vg_nav.cu)
-        size_t listed = 0, nonempty = 0;
-        for (unsigned ic = 0; ic < ncell; ++ic) {
-            int pc = 0;
-            for (int c = 0; c < mt.nchunks; ++c) pc += __builtin_popcountll(cells[size_t(ic) * mt.nchunks + c]);
-            listed += size_t(pc), nonempty += pc ? 1 : 0;
-        }
-        mt.dense = nonempty && double(listed) / double(nonempty) > kNavDenseCell;
+    if (rc == VG_OK) { // the candidate grid over the bounding box of the spheres (vg_nav_cull.h)
+        bool dense = false;
+        nav_grid_fill(sph, nd, mt.nchunks, gdim, r_mother, gr, reinterpret_cast<unsigned long long *>(host + gr.off_g),
+                      reinterpret_cast<int *>(host + gr.off_p), &dense);
+        mt.dense = dense;
     }
     if (rc != VG_OK) {
         delete[] host;
