@@ -948,17 +948,48 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
             float *e = &cull[4 * size_t(nodes[p].child0 + j)];
             e[0] = float(N.bs[0]), e[1] = float(N.bs[1]), e[2] = float(N.bs[2]), e[3] = std::nextafterf(float(r2), INFINITY);
         }
+    // candidate grids (vg_nav_cull.h) for the nodes with many children: Step walks the grid along the ray, Locate looks up
+    // the point's cell, instead of testing the bounding sphere of every child
+    std::vector<WorldGrid> grids;
+    std::vector<unsigned long long> gcells;
+    std::vector<int> gprim;
+    for (int p = 0; p < nn; ++p) {
+        WorldNode &P = nodes[p];
+        P.grid = -1;
+        if (P.nchild < kWorldGridMin || P.nchild > 64) continue;
+        std::vector<double> sph;
+        for (int j = 0; j < P.nchild; ++j) {
+            const WorldNode &C = nodes[kids[P.child0 + j]];
+            sph.insert(sph.end(), { C.bs[0], C.bs[1], C.bs[2], std::sqrt(double(cull[4 * size_t(P.child0 + j) + 3])) });
+        }
+        int gdim = 1;
+        while (gdim < kNavGridMax && gdim * gdim * gdim < P.nchild) ++gdim;
+        const size_t ncell = size_t(gdim + 2) * (gdim + 2) * (gdim + 2);
+        WorldGrid wg;
+        std::memset(&wg, 0, sizeof wg);
+        wg.cells0 = unsigned(gcells.size()), wg.prim0 = unsigned(gprim.size());
+        wg.all = P.nchild == 64 ? ~0ull : ((1ull << P.nchild) - 1ull);
+        gcells.resize(gcells.size() + ncell, 0ull);
+        gprim.resize(gprim.size() + ncell, -1);
+        bool dense = false;
+        nav_grid_fill(sph, P.nchild, 1, gdim, radius[p], wg.g, gcells.data() + wg.cells0, gprim.data() + wg.prim0, &dense);
+        P.grid = int(grids.size());
+        grids.push_back(wg);
+    }
     vg_world *w = new (std::nothrow) vg_world;
     if (!w) return fail(VG_ERR_NOMEM, "%s: out of host memory", fn);
     std::memset(w, 0, sizeof *w);
     w->nn = nn;
     auto up16 = [](size_t v) { return (v + 15) / 16 * 16; };
+    const size_t wgbytes = up16(grids.size() * sizeof(WorldGrid)), gcbytes = up16(gcells.size() * sizeof(unsigned long long)),
+                 gpbytes = up16(gprim.size() * sizeof(int));
     const size_t nbytes = size_t(nn) * sizeof(WorldNode), cbytes = cull.size() * sizeof(float), kbytes = up16(kids.size() * sizeof(int32_t));
     const size_t pbytes = up16(pcons.size() * sizeof(PolyconeP)), bbytes = up16(bools.size() * sizeof(BoolP)), gbytes = csgs.size() * sizeof(CsgP);
     static_assert(sizeof(WorldNode) % 16 == 0, "the float4 array follows the node records");
     unsigned char *blob = nullptr;
     cudaError_t e = cudaGetDevice(&w->device);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), nbytes + cbytes + kbytes + pbytes + bbytes + gbytes + 16);
+    const size_t goff = up16(nbytes + cbytes + kbytes + pbytes + bbytes + gbytes); // the grids follow everything else
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), goff + wgbytes + gcbytes + gpbytes + 16);
     if (e == cudaSuccess) e = cudaMemcpy(blob, nodes.data(), nbytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes, cull.data(), cbytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes + cbytes, kids.data(), kids.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
@@ -968,12 +999,20 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes, bools.data(), bools.size() * sizeof(BoolP), cudaMemcpyHostToDevice);
     if (e == cudaSuccess && !csgs.empty())
         e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes + bbytes, csgs.data(), gbytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && !grids.empty()) {
+        e = cudaMemcpy(blob + goff, grids.data(), grids.size() * sizeof(WorldGrid), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(blob + goff + wgbytes, gcells.data(), gcells.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(blob + goff + wgbytes + gcbytes, gprim.data(), gprim.size() * sizeof(int), cudaMemcpyHostToDevice);
+    }
     if (e != cudaSuccess) {
         if (blob) cudaFree(blob);
         delete w;
         return fail_cuda(e, fn);
     }
     w->blob = blob;
+    w->tab.grids = reinterpret_cast<WorldGrid *>(blob + goff);
+    w->tab.gcells = reinterpret_cast<unsigned long long *>(blob + goff + wgbytes);
+    w->tab.gprim = reinterpret_cast<int *>(blob + goff + wgbytes + gcbytes);
     w->tab.nodes = reinterpret_cast<WorldNode *>(blob);
     w->tab.cull = reinterpret_cast<float4 *>(blob + nbytes);
     w->tab.kids = reinterpret_cast<int32_t *>(blob + nbytes + cbytes);

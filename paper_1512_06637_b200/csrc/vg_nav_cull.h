@@ -156,6 +156,19 @@ VG_HD void nav_sphere_refine(const float4 *cull, double x, double y, double z, d
     }
 }
 
+// The candidates of a POINT (Locate in a tree of volumes): the mask of the cell that holds it; empty outside the grid's
+// box, which holds every sphere.  A point that rounding puts into the neighbouring cell is within ~1e-13 of the border,
+// and a sphere that holds it reaches across the border by its pad.
+VG_HD unsigned long long nav_point_cell(const NavGrid &G, const unsigned long long *cells, double x, double y, double z)
+{
+    const double px = x - G.o[0], py = y - G.o[1], pz = z - G.o[2];
+    if (!(px >= 0.0 && px <= G.len[0] && py >= 0.0 && py <= G.len[1] && pz >= 0.0 && pz <= G.len[2])) return 0ull;
+    int ix = int(floor(px * G.ics[0])), iy = int(floor(py * G.ics[1])), iz = int(floor(pz * G.ics[2]));
+    ix = ix > G.g[0] - 1 ? G.g[0] - 1 : ix, iy = iy > G.g[1] - 1 ? G.g[1] - 1 : iy, iz = iz > G.g[2] - 1 ? G.g[2] - 1 : iz;
+    const int sy_ = G.g[0] + 2, sz_ = sy_ * (G.g[1] + 2);
+    return cells[(ix + 1) + sy_ * (iy + 1) + sz_ * (iz + 1)];
+}
+
 // Both stages.  `all[c]` = every daughter of chunk c (what a start point outside the mother's bounding sphere keeps).
 template <int NC>
 VG_HD void nav_cull(const NavGrid &G, const float4 *cull, const unsigned long long *cells, const int *prim,

@@ -270,6 +270,17 @@ struct alignas(16) WorldNode {
     SolidU s;
     int parent, child0, nchild; // children: child_list[child0 .. child0 + nchild), ascending node index
     int ext;                    // s.kind == kPolycone / kBoolean: index into the world's polycone / boolean array
+    int grid;                   // >= 0: index of the node's candidate grid over its children (WorldGrid), -1: none
+    int pad_[3];
+};
+
+// Candidate grid of a node with kWorldGridMin..64 children (vg_nav_cull.h; bit j = the j-th child of the node's list): Step
+// walks it along the ray and Locate looks the point's cell up instead of testing every child's bounding sphere.
+constexpr int kWorldGridMin = 12;
+struct WorldGrid {
+    NavGrid g;
+    unsigned cells0, prim0; // first element of the node's cells / prim arrays in the world's pools
+    unsigned long long all; // every child of the node
 };
 
 // everything a world kernel needs, by value in kernel-parameter space
@@ -280,6 +291,9 @@ struct WorldTab {
     const struct PolyconeP *pcons; // nodes that are polycones (reading R30)
     const struct BoolP *bools;     // nodes that are booleans of two primitives
     const struct CsgP *csgs;       // nodes that are nested booleans (reading R31)
+    const WorldGrid *grids;        // candidate grids of the nodes with many children
+    const unsigned long long *gcells; // their cells' masks (one 64-bit word per cell, ringed layout)
+    const int *gprim;              // ... and the only child of each cell or -1
     int nnodes;
     int has_ext;                   // any polycone / boolean node: the kernels with their code are launched
 };

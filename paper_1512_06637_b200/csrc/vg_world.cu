@@ -102,16 +102,21 @@ __global__ void __launch_bounds__(kWorldBlock)
         bool moved = true;
         while (moved) {
             moved = false;
-            const int c0 = nodes[cur].child0, nc = nodes[cur].nchild;
+            const int c0 = nodes[cur].child0, nc = nodes[cur].nchild, gi = nodes[cur].grid;
             const float xf = float(x), yf = float(y), zf = float(z);
             for (int base = 0; base < nc && !moved; base += 64) {
                 const int lim = min(64, nc - base);
                 unsigned long long m = 0;
+                if (gi >= 0) { // a node with many children: the candidates of the point's grid cell (vg_nav_cull.h)
+                    const WorldGrid &G = w.grids[gi];
+                    m = nav_point_cell(G.g, w.gcells + G.cells0, x, y, z);
+                } else {
 #pragma unroll 4
-                for (int j = 0; j < lim; ++j) { // phase 1, FP32: inside the child's bounding sphere?
-                    const float4 sp = __ldg(cull + c0 + base + j);
-                    const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
-                    m |= (unsigned long long)(fmaf(vx, vx, fmaf(vy, vy, vz * vz)) <= sp.w) << j;
+                    for (int j = 0; j < lim; ++j) { // phase 1, FP32: inside the child's bounding sphere?
+                        const float4 sp = __ldg(cull + c0 + base + j);
+                        const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                        m |= (unsigned long long)(fmaf(vx, vx, fmaf(vy, vy, vz * vz)) <= sp.w) << j;
+                    }
                 }
                 while (m) { // phase 2, FP64, ascending child index
                     const int c = kids[c0 + base + __ffsll((long long)m) - 1];
@@ -167,12 +172,20 @@ __global__ void __launch_bounds__(kWorldBlock)
         for (int base = 0; base < nc; base += 64) {
             const int lim = min(64, nc - base);
             unsigned long long m = 0;
+            if (N.grid >= 0) { // a node with many children: ComputeStep's cull (grid walk + sphere test, vg_nav_cull.h)
+                const WorldGrid &G = w.grids[N.grid];
+                unsigned long long mm[1];
+                nav_cull<1>(G.g, cull + c0, w.gcells + G.cells0, w.gprim + G.prim0, &G.all, x, y, z, dx, dy, dz,
+                            best < step_max ? best : step_max, mm);
+                m = mm[0];
+            } else {
 #pragma unroll 4
-            for (int j = 0; j < lim; ++j) {
-                // phase 1, FP32: ray against the bounding sphere (closest approach of the line; sphere not behind the start)
-                // (the predicate of ComputeStep's cull, vg_nav_cull.h: pinned on the CPU by tests/test_nav_cull.py, stage 2)
-                const float4 sp = __ldg(cull + c0 + base + j);
-                m |= (unsigned long long)nav_sphere_keep(sp, xf, yf, zf, dxf, dyf, dzf) << j;
+                for (int j = 0; j < lim; ++j) {
+                    // phase 1, FP32: ray against the bounding sphere (closest approach of the line; sphere not behind the start)
+                    // (the predicate of ComputeStep's cull, vg_nav_cull.h: pinned on the CPU by tests/test_nav_cull.py, stage 2)
+                    const float4 sp = __ldg(cull + c0 + base + j);
+                    m |= (unsigned long long)nav_sphere_keep(sp, xf, yf, zf, dxf, dyf, dzf) << j;
+                }
             }
             while (m) { // phase 2, FP64, ascending child index: the strict < is R13's tie-break
                 const int c = kids[c0 + base + __ffsll((long long)m) - 1];
