@@ -324,7 +324,8 @@ int vg_debug_polycone_grid(const vg_shape *shape, uint64_t *masks, uint64_t *fac
  * only); x .. dz: HOST arrays of n tracks in the mother frame; t_lim: HOST array of the ray-parameter limit per track
  * (the mother's exit or the physics step; NULL = +inf); masks: HOST uint64[4 n], bit j of masks[4 i + c] set = daughter
  * 64 c + j survives for track i.  stage 0: both stages as the kernel runs them; 1: the grid walk alone; 2: the FP32
- * bounding-sphere test alone, applied to every daughter.  grid: HOST double[9] or NULL, receives the candidate grid's
+ * bounding-sphere test alone, applied to every daughter; 3: the candidates of the POINT x, y, z (the mask of its grid
+ * cell, what vg_world_locate tests in a node with many children; at most 64 daughters).  grid: HOST double[9] or NULL, receives the candidate grid's
  * origin, cell size and cells per axis (x, y, z each).  No CUDA call is made. */
 int vg_debug_nav_cull(const vg_shape *mother, int ndaughters, const vg_shape *const *daughters, const double *xforms,
                       const double *x, const double *y, const double *z, const double *dx, const double *dy,

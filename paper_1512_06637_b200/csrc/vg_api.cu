@@ -1127,6 +1127,12 @@ extern "C" int vg_debug_nav_cull(const vg_shape *mother, int nd, const vg_shape 
             if (mt.nchunks == 1) nav_grid_walk<1, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m), reinterpret_cast<unsigned long long(&)[1]>(hit));
             else if (mt.nchunks == 2) nav_grid_walk<2, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m), reinterpret_cast<unsigned long long(&)[2]>(hit));
             else nav_grid_walk<4, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m, hit);
+        } else if (stage == 3) { // the candidates of the POINT (world Locate): the mask of its grid cell; one chunk only
+            if (mt.nchunks != 1) {
+                delete[] host;
+                return fail(VG_ERR_ARG, "%s: stage 3 needs at most 64 daughters", fn);
+            }
+            m[0] = nav_point_cell(mt.grid, cells, x[i], y[i], z[i]);
         } else { // the FP32 sphere test alone, applied to every daughter
             for (int c = 0; c < 4; ++c) m[c] = c < mt.nchunks ? mt.all[c] : 0ull;
             if (mt.nchunks == 1) nav_sphere_refine<1>(cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], reinterpret_cast<unsigned long long(&)[1]>(m));

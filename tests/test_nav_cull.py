@@ -264,3 +264,26 @@ def test_flat_scenes_and_start_points_outside_the_mother():
     assert np.all(m[:, 0] == np.uint64(0xFFFFFFFFFFFFFFFF)) and np.all(m[:, 1:] == 0)
     tin = sc.oracle_tin(P, D)
     assert np.isfinite(tin).any()
+
+
+def test_the_cell_of_a_point_lists_every_daughter_that_holds_it():
+    """World Locate in a node with many children tests only the daughters listed in the point's grid cell: every daughter
+    whose Inside (oracle) is INSIDE or SURFACE at the point must be in that mask -- random points, points on the daughters'
+    surfaces and points on the grid's own cell planes, edges and corners."""
+    rng = np.random.default_rng(11)
+    for sc, half in (config4_scene(), random_scene(4242, 40, 50.0, 12.0, 35.0), random_scene(77, 64, 1e3, 60.0, 800.0)):
+        _, grid = sc.masks(np.zeros((1, 3)), np.array([[0.0, 0.0, 1.0]]))
+        o, cs, g = grid[:3], grid[3:6], grid[6:9].astype(int)
+        n = 200000
+        P = rng.uniform(-1, 1, (n, 3)) * np.asarray(half)
+        _, Q = surface_points(sc, rng, n)
+        node = o + cs * np.stack([rng.integers(0, g[a] + 1, n) for a in range(3)], axis=1)
+        snapped = np.where(rng.random((n, 3)) < 0.6, node, rng.uniform(-1, 1, (n, 3)) * np.asarray(half))
+        for pts, what in ((P, "random"), (Q, "on a daughter's surface"), (snapped, "on the grid's planes")):
+            pts = np.ascontiguousarray(pts)
+            m, _ = sc.masks(pts, np.tile([0.0, 0.0, 1.0], (len(pts), 1)), None, 3)
+            for k, s in enumerate(sc.o_d):
+                L = pts @ sc.R[k].T + sc.b[k]
+                holds = s.inside(L[:, 0], L[:, 1], L[:, 2]) != O.OUTSIDE
+                bit = (m[:, 0] >> np.uint64(k)) & np.uint64(1) == 1
+                assert not (holds & ~bit).any(), "%s: daughter %d holds %d points that its cell does not list" % (what, k, (holds & ~bit).sum())
