@@ -111,7 +111,8 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  * into a program over its primitives and runs the general kernel (vg_csg.cu).  A or B may also be a POLYCONE when the
  * other one is a primitive or a polycone: its constants are placed in memory of the CURRENT device (VG_ERR_CUDA
  * without one; queries must run on that device) and the general two-operand kernel answers (vg_boolx.cu); such a
- * boolean is neither an operand of another boolean nor a node of a world / daughter of a volume (VG_ERR_ARG).
+ * boolean is not an operand of another boolean (VG_ERR_ARG), but it is a placed solid like any other: a node of a
+ * world, the mother or a daughter of a volume (the world / volume copies the polycones' constants once more).
  * The result is a vg_shape of kind VG_BOOLEAN that every query below accepts ("operand" read recursively for a tree):
  *   Inside       combines the operands' classes: union INSIDE if either is, OUTSIDE if both are; intersection INSIDE if
  *                both are, OUTSIDE if either is; subtraction (A minus B) INSIDE if A INSIDE and B OUTSIDE, OUTSIDE if A

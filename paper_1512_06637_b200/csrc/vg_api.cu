@@ -194,6 +194,7 @@ extern "C" void vg_shape_destroy(vg_shape *s)
     if (!s) return;
     if (s->grid.masks) cudaFree(const_cast<unsigned long long *>(s->grid.masks)); // rows live in the same allocation
     if (s->ext_blob) cudaFree(s->ext_blob);
+    delete[] s->ext_host;
     delete s;
 }
 
@@ -401,6 +402,25 @@ static double shape_radius(const vg_shape *s)
         const PolyconeP &c = s->u.pcon;
         double zm = std::fmax(std::fabs(c.zlo), std::fabs(c.zhi));
         return std::sqrt(c.rb2 + zm * zm);
+    }
+    if (s->kind == kBoolX) { // a polycone operand: its radius from the host copy kept with the shape
+        const BoolP &c = s->u.boolean;
+        const SolidU *rec[2] = { &c.a, &c.b };
+        double r[2];
+        for (int o = 0, k = 0; o < 2; ++o) {
+            if (rec[o]->kind == kPolycone) {
+                const PolyconeP &pc = s->ext_host[k++];
+                const double zm = std::fmax(std::fabs(pc.zlo), std::fabs(pc.zhi));
+                r[o] = std::sqrt(pc.rb2 + zm * zm);
+            } else {
+                r[o] = bounding_radius(*rec[o]);
+            }
+        }
+        if (c.op != kUnion) return r[0]; // an intersection and a subtraction lie inside A
+        const double *m = c.X;           // centre of B in the frame of C: -R^T b
+        const double cx = -(m[0] * m[3] + m[4] * m[7] + m[8] * m[11]), cy = -(m[1] * m[3] + m[5] * m[7] + m[9] * m[11]),
+                     cz = -(m[2] * m[3] + m[6] * m[7] + m[10] * m[11]);
+        return std::fmax(r[0], std::sqrt(cx * cx + cy * cy + cz * cz) + r[1]);
     }
     if (s->kind == kCsg) { // any tree lies inside the union of its primitives
         const CsgP &c = s->u.csg;
@@ -812,10 +832,13 @@ extern "C" int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, c
         if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&blob), size_t(npc) * sizeof(PolyconeP));
         if (e != cudaSuccess) rc = fail_cuda(e, "vg_boolean_create: a polycone operand needs device memory");
         s->ext_blob = blob;
+        s->ext_host = new (std::nothrow) PolyconeP[2];
+        if (!s->ext_host && rc == VG_OK) rc = fail(VG_ERR_NOMEM, "vg_boolean_create: out of host memory");
         for (int i = 0, k = 0; i < 2 && rc == VG_OK; ++i) {
             if (opnd[i]->kind == VG_POLYCONE) {
                 e = cudaMemcpy(blob + k, &opnd[i]->u.pcon, sizeof(PolyconeP), cudaMemcpyHostToDevice);
                 if (e != cudaSuccess) rc = fail_cuda(e, "vg_boolean_create: cudaMemcpy");
+                s->ext_host[k] = opnd[i]->u.pcon;
                 rec[i]->kind = kPolycone;
                 rec[i]->u.pcon = blob + k++;
             } else {
@@ -823,6 +846,7 @@ extern "C" int vg_boolean_create(int op, const vg_shape *a, const vg_shape *b, c
             }
         }
         if (rc != VG_OK && blob) cudaFree(blob);
+        if (rc != VG_OK) delete[] s->ext_host;
     } else if (a->kind == kBoolX || b->kind == kBoolX || a->kind == VG_POLYCONE || b->kind == VG_POLYCONE) {
         rc = fail(VG_ERR_ARG, "%s: a polycone may be an operand of a boolean of two solids, not a leaf of a nested tree", fn);
     } else if (a->kind < VG_POLYCONE && b->kind < VG_POLYCONE) { // two primitives: the specialised kernels of vg_bool.cu
@@ -879,6 +903,7 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     std::vector<int> count(nn, 0), fill(nn, 0);
     std::vector<PolyconeP> pcons;
     std::vector<BoolP> bools;
+    std::vector<int> boolx; // entries of `bools` whose polycone operands still hold an index into `pcons`
     std::vector<CsgP> csgs;
     std::vector<double> radius(nn, 0.0);
     for (int i = 1; i < nn; ++i) {
@@ -893,9 +918,20 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         const double *m = xforms + 12 * i;
         if (!all_finite(m, 12)) return fail(VG_ERR_PARAM, "%s: non-finite transform of node %d", fn, i);
         if (!rigid(m)) return fail(VG_ERR_PARAM, "%s: rotation of node %d is not orthonormal", fn, i);
-        if (shapes[i]->kind == kBoolX)
-            return fail(VG_ERR_ARG, "%s: node %d is a boolean with a polycone operand: not supported as a placed solid", fn, i);
-        if (shapes[i]->kind == VG_POLYCONE) { // R30: constants in a side array, the record keeps kind + index
+        if (shapes[i]->kind == kBoolX) { // a boolean with polycone operands: its polycones join the world's side array
+            N.s.kind = kBoolX;
+            N.ext = int(bools.size());
+            BoolP b = shapes[i]->u.boolean;
+            SolidU *rec[2] = { &b.a, &b.b };
+            for (int o = 0, k = 0; o < 2; ++o)
+                if (rec[o]->kind == kPolycone) {
+                    // the index for now; becomes the device address once the world's blob exists (below)
+                    rec[o]->u.pcon = reinterpret_cast<const PolyconeP *>(uintptr_t(pcons.size()));
+                    pcons.push_back(shapes[i]->ext_host[k++]);
+                }
+            bools.push_back(b);
+            boolx.push_back(int(bools.size()) - 1);
+        } else if (shapes[i]->kind == VG_POLYCONE) { // R30: constants in a side array, the record keeps kind + index
             N.s.kind = kPolycone;
             N.ext = int(pcons.size());
             pcons.push_back(shapes[i]->u.pcon);
@@ -995,6 +1031,14 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
     if (e == cudaSuccess) e = cudaMemcpy(blob + nbytes + cbytes, kids.data(), kids.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
     if (e == cudaSuccess && !pcons.empty())
         e = cudaMemcpy(blob + nbytes + cbytes + kbytes, pcons.data(), pcons.size() * sizeof(PolyconeP), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) { // polycone operands of boolean nodes: index -> address in this world's polycone array
+        const PolyconeP *pc0 = reinterpret_cast<const PolyconeP *>(blob + nbytes + cbytes + kbytes);
+        for (int k : boolx) {
+            SolidU *rec[2] = { &bools[k].a, &bools[k].b };
+            for (int o = 0; o < 2; ++o)
+                if (rec[o]->kind == kPolycone) rec[o]->u.pcon = pc0 + reinterpret_cast<uintptr_t>(rec[o]->u.pcon);
+        }
+    }
     if (e == cudaSuccess && !bools.empty())
         e = cudaMemcpy(blob + nbytes + cbytes + kbytes + pbytes, bools.data(), bools.size() * sizeof(BoolP), cudaMemcpyHostToDevice);
     if (e == cudaSuccess && !csgs.empty())

@@ -30,6 +30,7 @@ struct vg_shape {
     // into it); owned by the shape
     void *ext_blob;
     int ext_device;
+    PolyconeP *ext_host; // ... and their host copies, in operand order (a world that places the boolean uploads its own)
 };
 
 // ------------------------------------------------------------------------------------------- derived constants

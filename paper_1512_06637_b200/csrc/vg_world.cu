@@ -44,12 +44,14 @@ __device__ __noinline__ int ext_inside(const WorldTab &w, const WorldNode &N, do
         csg_classes(w.csgs[N.ext], x, y, z, in, out);
         return csg_classify(w.csgs[N.ext], in, out);
     }
+    if (N.s.kind == kBoolX) return bool_inside_pt<true>(w.bools[N.ext], x, y, z); // a polycone operand: constants in w.pcons
     return N.s.kind == kPolycone ? Polycone::inside(w.pcons[N.ext], x, y, z) : bool_inside_pt(w.bools[N.ext], x, y, z);
 }
 
 __device__ __noinline__ double ext_sdf(const WorldTab &w, const WorldNode &N, double x, double y, double z)
 {
     if (N.s.kind == kCsg) return csg_sdf(w.csgs[N.ext], x, y, z);
+    if (N.s.kind == kBoolX) return bool_sdf_pt<true>(w.bools[N.ext], x, y, z);
     return N.s.kind == kPolycone ? Polycone::safety(w.pcons[N.ext], x, y, z) : bool_sdf_pt(w.bools[N.ext], x, y, z);
 }
 
@@ -59,6 +61,7 @@ __device__ __noinline__ double ext_distance(const WorldTab &w, const WorldNode &
     if (N.s.kind == kPolycone)
         return to_out ? Polycone::dist_out(w.pcons[N.ext], x, y, z, dx, dy, dz) : Polycone::dist_in(w.pcons[N.ext], x, y, z, dx, dy, dz);
     if (N.s.kind == kCsg) return csg_distance(w.csgs[N.ext], to_out, x, y, z, dx, dy, dz);
+    if (N.s.kind == kBoolX) return bool_distance<-1, -1, true>(w.bools[N.ext], to_out, x, y, z, dx, dy, dz);
     return bool_distance<-1, -1>(w.bools[N.ext], to_out, x, y, z, dx, dy, dz);
 }
 

@@ -387,12 +387,19 @@ def test_volume_with_polycone_and_boolean_solids(vg):
     b1 = bools["box_minus_tube"]
     specs = [("shape", W.POLYCONE, W.STEPPED_POLYCONE, (-40.0, -40.0, 0.0)), ("boolean", b1, None, (40.0, -40.0, 5.0)),
              ("shape", W.TUBE, [5.0, 10.0, 15.0, 0.0, 4 * PI / 3], (-40.0, 40.0, -5.0)),
-             ("shape", W.POLYCONE, [0.5, 4.0] + W.STEPPED_POLYCONE[2:], (40.0, 40.0, 0.0))]
+             ("shape", W.POLYCONE, [0.5, 4.0] + W.STEPPED_POLYCONE[2:], (40.0, 40.0, 0.0)),
+             # a boolean with a polycone operand (vg_boolx.cu) as a placed solid: stepped polycone minus an off-centre box
+             # (faces at z = -2.9 and 5.5: none in a plane of the polycone, where the two operands' crossings would tie)
+             ("pair", (W.SUBTRACTION, W.POLYCONE, W.STEPPED_POLYCONE, W.BOX, [3.0, 20.0, 4.2], W.placement(np.eye(3), (5.0, 0.0, 1.3))),
+              None, (0.0, 0.0, 0.0))]
     rng = np.random.default_rng(12)
 
     def mk(mod, sp):
         if sp[0] == "shape":
             return mod.Shape(sp[1], sp[2])
+        if sp[0] == "pair":
+            op, ka, pa, kb, pb, xb = sp[1]
+            return mod.Boolean(op, mod.Shape(ka, pa), mod.Shape(kb, pb), xb)
         b = sp[1]
         return mod.Boolean(b.op, mod.Shape(b.kind_a, b.par_a), mod.Shape(b.kind_b, b.par_b), b.xform)
     xf = []
@@ -402,7 +409,7 @@ def test_volume_with_polycone_and_boolean_solids(vg):
     ident = W.placement(np.eye(3), (0, 0, 0))
     for mother in (("shape", W.BOX, [80.0, 80.0, 40.0]), ("boolean", bools["box_union_orb"].__class__(
             "m", W.SUBTRACTION, W.BOX, [80.0, 80.0, 40.0], W.ORB, [6.0], (0.0, 0.0, 0.0), (0.0, 0.0, 0.0, 1.0), 1), None)):
-        wo = O.World([mk(O, mother)] + [mk(O, sp) for sp in specs], [-1, 0, 0, 0, 0], [ident] + xf)
+        wo = O.World([mk(O, mother)] + [mk(O, sp) for sp in specs], [-1] + [0] * len(specs), [ident] + xf)
         vgv = vg.Volume(mk(vg, mother), [mk(vg, sp) for sp in specs], xf)
 
         def band(x, y, z):
@@ -417,8 +424,18 @@ def test_volume_with_polycone_and_boolean_solids(vg):
             want_hit = np.where(no == 0, -2, np.where(no < 0, -1, no - 1))
             assert_int_equal(hg.cpu().numpy(), want_hit, "general volume hit")
             assert_real_close(sg.cpu().numpy(), so, "general volume step")
-        assert set(np.unique(want_hit)) >= {-2, -1, 0, 1, 2, 3}
+        assert set(np.unique(want_hit)) >= {-2, -1, 0, 1, 2, 3, 4}
         assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), wo.safety(zero, *t[:3]), "general volume safety")
+        # the same solids as a world: Locate of points anywhere (inside the daughters too), node indices bit-exact
+        wg = vg.World([mk(vg, mother)] + [mk(vg, sp) for sp in specs], [-1] + [0] * len(specs), [ident] + xf)
+        p = W.draw_tracks(92, 150001, (0, 0, 0), (80, 80, 40), lambda x, y, z: np.zeros(x.size, dtype=bool))[:3]
+        node_o = wo.locate(*p)
+        clear = np.ones(p[0].size, dtype=bool)
+        for nd in range(len(specs) + 1):  # keep points clear of every node's surface band (R7)
+            clear &= np.abs(wo.safety(np.full(p[0].size, nd, dtype=np.int32), *p)) > 1e-6
+        pc = tuple(np.ascontiguousarray(a[clear]) for a in p)
+        assert_int_equal(wg.locate(*dev(pc)).cpu().numpy(), node_o[clear], "world locate with a polycone-operand boolean")
+        assert (node_o[clear] == len(specs)).any()
 
 
 # ------------------------------------------------------------------------------- host-buffer entry points
