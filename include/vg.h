@@ -326,8 +326,12 @@ int vg_debug_polycone_grid(const vg_shape *shape, uint64_t *masks, uint64_t *fac
  * (the mother's exit or the physics step; NULL = +inf); masks: HOST uint64[4 n], bit j of masks[4 i + c] set = daughter
  * 64 c + j survives for track i.  stage 0: both stages as the kernel runs them; 1: the grid walk alone; 2: the FP32
  * bounding-sphere test alone, applied to every daughter; 3: the candidates of the POINT x, y, z (the mask of its grid
- * cell, what vg_world_locate tests in a node with many children; at most 64 daughters).  grid: HOST double[9] or NULL, receives the candidate grid's
- * origin, cell size and cells per axis (x, y, z each).  No CUDA call is made. */
+ * cell, what vg_world_locate tests in a node with many children); 4: the candidates of the
+ * SAFETY of the point x, y, z (the daughters that can be the nearest one anywhere in its cell of the safety grid, what
+ * vg_volume_safety / vg_world_safety evaluate; every daughter outside the grid or without one).  grid: HOST double[9]
+ * (stage 4: double[10]) or NULL, receives the candidate grid's origin, cell size and cells per axis (x, y, z each;
+ * stage 4: the SAFETY grid's, laid over the mother's bounding box, and its cells per axis once more as the tenth
+ * value; 0 = none).  No CUDA call is made. */
 int vg_debug_nav_cull(const vg_shape *mother, int ndaughters, const vg_shape *const *daughters, const double *xforms,
                       const double *x, const double *y, const double *z, const double *dx, const double *dy,
                       const double *dz, const double *t_lim, int64_t n, uint64_t *masks, int stage, double *grid);

@@ -228,7 +228,8 @@ def vg_volume_create(mother, daughters, xforms):
 
 def vg_debug_nav_cull(mother, daughters, xforms, x, y, z, dx, dy, dz, t_lim=None, stage=0):
     """Host-only (numpy float64 arrays in, no device): the candidate masks of ComputeStep's conservative cull as
-    uint64 (n, 4), and the candidate grid's geometry (origin[3], cell size[3], cells per axis[3])."""
+    uint64 (n, 4), and the candidate grid's geometry (origin[3], cell size[3], cells per axis[3]; stage 4 appends the
+    safety grid's cells per axis)."""
     import numpy as np
     nd = len(daughters)
     arr = (_VP * max(1, nd))(*[_handle(d) for d in daughters])
@@ -238,7 +239,7 @@ def vg_debug_nav_cull(mother, daughters, xforms, x, y, z, dx, dy, dz, t_lim=None
     n = a[0].size
     tl = None if t_lim is None else np.ascontiguousarray(t_lim, dtype=np.float64)
     masks = np.zeros((n, 4), dtype=np.uint64)
-    grid = np.zeros(9, dtype=np.float64)
+    grid = np.zeros(10 if int(stage) == 4 else 9, dtype=np.float64)
     _check(_lib.vg_debug_nav_cull(_handle(mother), nd, arr, xf, *[v.ctypes.data for v in a],
                                   None if tl is None else tl.ctypes.data, n, masks.ctypes.data, int(stage), grid.ctypes.data))
     return masks, grid

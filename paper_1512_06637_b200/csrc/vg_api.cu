@@ -20,6 +20,7 @@ struct vg_volume {
     SolidU mother;
     NavMeta meta;
     unsigned char *table_dev; // the blob described in vg_params.h
+    size_t table_bytes;       // all of it (meta.bytes: the part the kernels stage in shared memory)
     unsigned char *table_host; // its host copy (vg_debug_nav_cull evaluates the cull predicate on the CPU)
     int device;
     vg_world *general;        // mother or a daughter is a polycone / boolean: the volume is held as a one-level world instead
@@ -539,6 +540,64 @@ static void nav_grid_fill(const std::vector<double> &sph, int nd, int nchunks, i
     *dense_out = filled && double(listed) / double(filled) > kNavDenseCell;
 }
 
+// The safety grid over the box nav_grid_fill laid out (vg_nav_cull.h, nav_safety_cell): gs^3 cells, nchunks mask words
+// each.  `bounded[i]`: daughter i is never empty, so |p - c| + r bounds its SafetyToIn from above.
+static int nav_safe_dim(int nd)
+{
+    if (nd < kNavSafeGridMin) return 0;
+    int gs = 4;
+    while (gs < kNavSafeGridMax && gs * gs * gs < 64 * nd) gs += 4; // about 64 cells per daughter
+    return gs;
+}
+
+// half-extents of the axis-aligned bounding box of a solid about its local origin
+static void bounding_half(const SolidU &s, double h[3])
+{
+    switch (s.kind) {
+    case kBox: h[0] = s.u.box.hx, h[1] = s.u.box.hy, h[2] = s.u.box.hz; break;
+    case kOrb: h[0] = h[1] = h[2] = s.u.orb.r; break;
+    case kTube: h[0] = h[1] = std::sqrt(s.u.tube.rmax2), h[2] = s.u.tube.dz; break;
+    case kCone: h[0] = h[1] = std::fmax(s.u.cone.rmax1, s.u.cone.rmax2), h[2] = s.u.cone.dz; break;
+    default: h[0] = std::fmax(s.u.trd.dx1, s.u.trd.dx2), h[1] = std::fmax(s.u.trd.dy1, s.u.trd.dy2), h[2] = s.u.trd.dz; break;
+    }
+}
+
+// `fh`: half-extents of the mother's bounding box about its origin (the grid's box, a little larger)
+static void nav_safe_grid_fill(const std::vector<double> &sph, const std::vector<char> &bounded, int nd, int nchunks,
+                               const double fh[3], NavGrid &gr, unsigned long long *scells)
+{
+    const int gs = gr.gs;
+    double cs[3];
+    for (int a = 0; a < 3; ++a) {
+        const double h = fh[a] > 0 ? fh[a] * (1.0 + 1e-6) : 1.0;
+        gr.so[a] = -h, gr.slen[a] = 2.0 * h, cs[a] = gr.slen[a] / gs, gr.sics[a] = gs / gr.slen[a];
+    }
+    gr.spad = gr.tpad;
+    std::vector<double> dn(nd), df(nd);
+    for (int iz = 0; iz < gs; ++iz)
+        for (int iy = 0; iy < gs; ++iy)
+            for (int ix = 0; ix < gs; ++ix) {
+                const int ic[3] = { ix, iy, iz };
+                double U = INFINITY;
+                for (int i = 0; i < nd; ++i) {
+                    const double *c = &sph[4 * i];
+                    double n2 = 0, f2 = 0;
+                    for (int a = 0; a < 3; ++a) { // nearest and farthest point of the padded closed cell from the centre
+                        const double l = gr.so[a] + ic[a] * cs[a] - gr.spad, h = gr.so[a] + (ic[a] + 1) * cs[a] + gr.spad;
+                        const double d = c[a] < l ? l - c[a] : (c[a] > h ? c[a] - h : 0.0);
+                        const double f = std::fmax(std::fabs(c[a] - l), std::fabs(c[a] - h));
+                        n2 += d * d, f2 += f * f;
+                    }
+                    dn[i] = std::sqrt(n2), df[i] = std::sqrt(f2);
+                    if (bounded[i]) U = std::fmin(U, df[i] + c[3]);
+                }
+                U = U * (1.0 + 1e-9) + gr.spad;
+                unsigned long long *m = scells + size_t((iz * gs + iy) * gs + ix) * size_t(nchunks);
+                for (int i = 0; i < nd; ++i)
+                    if (dn[i] - sph[4 * i + 3] <= U) m[i / 64] |= 1ull << (i % 64);
+            }
+}
+
 // Host side of vg_volume_create for a volume of primitives: validation, the mother and daughter records, the FP32
 // bounding spheres and the candidate grid, as one blob in host memory (layout: vg_params.h).  No CUDA call.
 static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
@@ -560,12 +619,16 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
     gr.off_p = (gr.off_g + 8u * ncell * (nchunks_alloc ? nchunks_alloc : 1u) + 15u) / 16u * 16u;
     mt.bytes = (gr.off_p + 4u * ncell + 15u) / 16u * 16u;
     if (nchunks_alloc) mt.nchunks = int(nchunks_alloc);
+    // the safety grid's masks follow the part of the blob the kernels stage in shared memory (vg_params.h)
+    gr.gs = nav_safe_dim(nd);
+    gr.off_s = mt.bytes;
+    v->table_bytes = size_t(mt.bytes) + 8u * size_t(gr.gs) * gr.gs * gr.gs * size_t(mt.nchunks);
     std::vector<double> sph; // bounding spheres of the daughters in the mother frame: cx, cy, cz, r (FP64)
     unsigned char *host = nullptr;
     if (rc == VG_OK) {
-        host = new (std::nothrow) unsigned char[mt.bytes];
+        host = new (std::nothrow) unsigned char[v->table_bytes];
         if (!host) rc = fail(VG_ERR_NOMEM, "vg_volume_create: out of host memory");
-        else std::memset(host, 0, mt.bytes);
+        else std::memset(host, 0, v->table_bytes);
     }
     double r_mother = rc == VG_OK ? bounding_radius(v->mother) : 0.0;
     for (int i = 0; rc == VG_OK && i < ndp; ++i) { // padding entries of the cull table: never hit
@@ -618,6 +681,13 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
         nav_grid_fill(sph, nd, mt.nchunks, gdim, r_mother, gr, reinterpret_cast<unsigned long long *>(host + gr.off_g),
                       reinterpret_cast<int *>(host + gr.off_p), &dense);
         mt.dense = dense;
+        if (gr.gs > 0) // primitives are never empty: every daughter bounds the minimum from above
+        {
+            double fh[3];
+            bounding_half(v->mother, fh);
+            nav_safe_grid_fill(sph, std::vector<char>(size_t(nd), 1), nd, mt.nchunks, fh, gr,
+                               reinterpret_cast<unsigned long long *>(host + gr.off_s));
+        }
     }
     if (rc != VG_OK) {
         delete[] host;
@@ -663,10 +733,10 @@ extern "C" int vg_volume_create(const vg_shape *mother, int nd, const vg_shape *
     int rc = nav_build_host(mother, nd, daughters, xforms, v, &host);
     NavMeta &mt = v->meta;
     if (rc == VG_OK) {
-        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&v->table_dev), mt.bytes);
+        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&v->table_dev), v->table_bytes);
         if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMalloc");
         if (rc == VG_OK) {
-            e = cudaMemcpy(v->table_dev, host, mt.bytes, cudaMemcpyHostToDevice);
+            e = cudaMemcpy(v->table_dev, host, v->table_bytes, cudaMemcpyHostToDevice);
             if (e != cudaSuccess) rc = fail_cuda(e, "vg_volume_create: cudaMemcpy");
         }
     }
@@ -1009,6 +1079,17 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         gprim.resize(gprim.size() + ncell, -1);
         bool dense = false;
         nav_grid_fill(sph, P.nchild, 1, gdim, radius[p], wg.g, gcells.data() + wg.cells0, gprim.data() + wg.prim0, &dense);
+        // the safety grid (nav_safety_cell): a boolean can be empty, so only the other kinds bound the minimum from above
+        wg.g.gs = nav_safe_dim(P.nchild);
+        wg.g.off_s = unsigned(gcells.size());
+        if (wg.g.gs > 0) {
+            std::vector<char> bounded;
+            for (int j = 0; j < P.nchild; ++j) bounded.push_back(shapes[kids[P.child0 + j]]->kind != VG_BOOLEAN);
+            gcells.resize(gcells.size() + size_t(wg.g.gs) * wg.g.gs * wg.g.gs, 0ull);
+            double fh[3] = { radius[p], radius[p], radius[p] }; // a polycone or boolean node: the cube about its sphere
+            if (P.s.kind < kPolycone) bounding_half(P.s, fh);
+            nav_safe_grid_fill(sph, bounded, P.nchild, 1, fh, wg.g, gcells.data() + wg.g.off_s);
+        }
         P.grid = int(grids.size());
         grids.push_back(wg);
     }
@@ -1160,6 +1241,10 @@ extern "C" int vg_debug_nav_cull(const vg_shape *mother, int nd, const vg_shape 
     const int *prim = reinterpret_cast<const int *>(host + mt.grid.off_p);
     if (grid)
         for (int a = 0; a < 3; ++a) grid[a] = mt.grid.o[a], grid[3 + a] = mt.grid.cs[a], grid[6 + a] = double(mt.grid.g[a]);
+    if (grid && stage == 4) { // the safety grid's own box
+        for (int a = 0; a < 3; ++a) grid[a] = mt.grid.so[a], grid[3 + a] = mt.grid.gs ? mt.grid.slen[a] / mt.grid.gs : 0.0, grid[6 + a] = double(mt.grid.gs);
+        grid[9] = double(mt.grid.gs);
+    }
     for (int64_t i = 0; i < n; ++i) {
         unsigned long long m[4] = { 0, 0, 0, 0 }, hit[4] = { 0, 0, 0, 0 };
         const double tl = t_lim ? t_lim[i] : INFINITY;
@@ -1171,12 +1256,13 @@ extern "C" int vg_debug_nav_cull(const vg_shape *mother, int nd, const vg_shape 
             if (mt.nchunks == 1) nav_grid_walk<1, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[1]>(m), reinterpret_cast<unsigned long long(&)[1]>(hit));
             else if (mt.nchunks == 2) nav_grid_walk<2, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, reinterpret_cast<unsigned long long(&)[2]>(m), reinterpret_cast<unsigned long long(&)[2]>(hit));
             else nav_grid_walk<4, false>(mt.grid, cells, prim, cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], tl, m, hit);
-        } else if (stage == 3) { // the candidates of the POINT (world Locate): the mask of its grid cell; one chunk only
-            if (mt.nchunks != 1) {
-                delete[] host;
-                return fail(VG_ERR_ARG, "%s: stage 3 needs at most 64 daughters", fn);
-            }
-            m[0] = nav_point_cell(mt.grid, cells, x[i], y[i], z[i]);
+        } else if (stage == 3) { // the candidates of the POINT (world Locate, the volume safety of a point inside a daughter): its grid cell
+            const unsigned long long *cell = nav_point_cell_masks(mt.grid, cells, mt.nchunks, x[i], y[i], z[i]);
+            for (int c = 0; c < mt.nchunks; ++c) m[c] = cell ? cell[c] : 0ull;
+        } else if (stage == 4) { // the candidates of the point's SAFETY: its cell of the safety grid, else every daughter
+            const unsigned long long *cell = nav_safety_cell(
+                mt.grid, reinterpret_cast<const unsigned long long *>(host + mt.grid.off_s), mt.nchunks, x[i], y[i], z[i]);
+            for (int c = 0; c < mt.nchunks; ++c) m[c] = cell ? cell[c] : mt.all[c];
         } else { // the FP32 sphere test alone, applied to every daughter
             for (int c = 0; c < 4; ++c) m[c] = c < mt.nchunks ? mt.all[c] : 0ull;
             if (mt.nchunks == 1) nav_sphere_refine<1>(cull, x[i], y[i], z[i], dx[i], dy[i], dz[i], reinterpret_cast<unsigned long long(&)[1]>(m));

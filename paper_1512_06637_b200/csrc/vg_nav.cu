@@ -254,19 +254,77 @@ __global__ void __launch_bounds__(kNavBlock) nav_safety_kernel(const __grid_cons
             waited = true;
         }
         double best = -solid_sdf(mother, x, y, z);
-#pragma unroll 1
-        for (int k = 0; k < nd; ++k) {
-            const Daughter &D = daughter_at(dtab, k);
-            double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
-            double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
-            double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
-            // the daughter lies inside the sphere of radius r about its local origin (r: the table's FP32 radius, which is
-            // inflated, so not smaller than the true one): sdf >= |l| - r.  A daughter with |l| - r >= best cannot lower
-            // the minimum and is skipped; the slack keeps the comparison on the safe side of its own rounding.
-            const double reach = best + double(sqrtf(cull[k].w)) * (1.0 + 1e-6);
-            const double l2 = fma(lx, lx, fma(ly, ly, lz * lz));
-            if (best > 0.0 && l2 >= reach * reach * (1.0 + 1e-12)) continue;
-            best = dmin(best, solid_sdf(D.s, lx, ly, lz));
+        // A daughter lies inside the sphere of radius r about its local origin (the table's FP32 sphere, centre in the
+        // mother's frame, r^2 inflated by the rounding bound of the FP32 test: vg_volume_create), so its
+        // SafetyToIn >= |p - c| - r and a daughter whose bound is not below the running minimum is skipped.  The
+        // candidates: the daughters that can be nearest to a point of the safety grid's cell (vg_nav_cull.h,
+        // nav_safety_cell; read from device memory: 64 cells per daughter are too many to stage), else every daughter.
+        // The one whose sphere looks nearest (|p - c|^2 - r^2 in FP32, a heuristic with no bearing on the result: the
+        // minimum is order-independent) is evaluated first, exactly; the others meet the bound in FP32, then -- after
+        // the FP64 transform only they pay for -- in FP64 against the running minimum.
+        if (best > 0.0 && nd > 0) {
+            const float xf = float(x), yf = float(y), zf = float(z);
+            const unsigned long long *cell =
+                nav_safety_cell(meta.grid, reinterpret_cast<const unsigned long long *>(table + meta.grid.off_s), meta.nchunks, x, y, z);
+            const unsigned long long *cand = cell ? cell : meta.all;
+            int probe = -1;
+            float key = 3.0e38f;
+            for (int c = 0; c < meta.nchunks; ++c)
+                for (unsigned long long mm = cand[c]; mm; mm &= mm - 1) {
+                    const int k = 64 * c + __ffsll((long long)mm) - 1;
+                    const float4 sp = cull[k];
+                    const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                    const float q = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, -sp.w)));
+                    probe = q < key ? k : probe;
+                    key = fminf(q, key);
+                }
+            if (probe >= 0) {
+                const Daughter &D = daughter_at(dtab, probe);
+                const double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
+                const double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
+                const double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
+                best = dmin(best, solid_sdf(D.s, lx, ly, lz));
+            }
+            const float bf = float(best);
+            for (int c = 0; c < meta.nchunks && best > 0.0; ++c) { // (best <= 0: inside the probe, the branch below)
+                unsigned long long m = cand[c];
+                if ((probe >> 6) == c) m &= ~(1ull << (probe & 63)); // already counted
+                while (m) {
+                    const int k = 64 * c + __ffsll((long long)m) - 1;
+                    m &= m - 1;
+                    const float4 sp = cull[k];
+                    const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                    const float rf = sqrtf(sp.w), reachf = bf + rf;
+                    if (!(fmaf(vx, vx, fmaf(vy, vy, vz * vz)) <= reachf * reachf)) continue;
+                    const Daughter &D = daughter_at(dtab, k);
+                    const double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
+                    const double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
+                    const double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
+                    // the slack keeps the comparison on the safe side of its own rounding
+                    const double reach = best + double(rf) * (1.0 + 1e-6);
+                    const double l2 = fma(lx, lx, fma(ly, ly, lz * lz));
+                    if (best > 0.0 && l2 >= reach * reach * (1.0 + 1e-12)) continue;
+                    best = dmin(best, solid_sdf(D.s, lx, ly, lz));
+                }
+            }
+        }
+        if (best <= 0.0 && nd > 0) {
+            // Outside the mother, on a surface or inside a daughter: only a daughter that HOLDS the point (SafetyToIn
+            // < 0) can lower a minimum that is not positive, and its bounding sphere then holds the point too: the
+            // candidates are the daughters listed in the point's cell of the candidate grid (vg_nav_cull.h,
+            // nav_point_cell; none outside the grid's box, which holds every sphere).  For volumes that keep the
+            // containment contract this is at most the daughter the point is in; for the others the result stays the
+            // plain minimum over every daughter.
+            const unsigned long long *cell =
+                nav_point_cell_masks(meta.grid, reinterpret_cast<const unsigned long long *>(smem_raw + meta.grid.off_g), meta.nchunks, x, y, z);
+            for (int c = 0; cell && c < meta.nchunks; ++c)
+                for (unsigned long long m = cell[c]; m; m &= m - 1) {
+                    const Daughter &D = daughter_at(dtab, 64 * c + __ffsll((long long)m) - 1);
+                    const double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));
+                    const double ly = fma(D.m[4], x, fma(D.m[5], y, fma(D.m[6], z, D.m[7])));
+                    const double lz = fma(D.m[8], x, fma(D.m[9], y, fma(D.m[10], z, D.m[11])));
+                    best = dmin(best, solid_sdf(D.s, lx, ly, lz));
+                }
         }
         stg1(out + i, best);
     }

@@ -159,14 +159,43 @@ VG_HD void nav_sphere_refine(const float4 *cull, double x, double y, double z, d
 // The candidates of a POINT (Locate in a tree of volumes): the mask of the cell that holds it; empty outside the grid's
 // box, which holds every sphere.  A point that rounding puts into the neighbouring cell is within ~1e-13 of the border,
 // and a sphere that holds it reaches across the border by its pad.
-VG_HD unsigned long long nav_point_cell(const NavGrid &G, const unsigned long long *cells, double x, double y, double z)
+// (nchunks mask words per cell; NULL outside the box)
+VG_HD const unsigned long long *nav_point_cell_masks(const NavGrid &G, const unsigned long long *cells, int nchunks, double x,
+                                                     double y, double z)
 {
     const double px = x - G.o[0], py = y - G.o[1], pz = z - G.o[2];
-    if (!(px >= 0.0 && px <= G.len[0] && py >= 0.0 && py <= G.len[1] && pz >= 0.0 && pz <= G.len[2])) return 0ull;
+    if (!(px >= 0.0 && px <= G.len[0] && py >= 0.0 && py <= G.len[1] && pz >= 0.0 && pz <= G.len[2])) return nullptr;
     int ix = int(floor(px * G.ics[0])), iy = int(floor(py * G.ics[1])), iz = int(floor(pz * G.ics[2]));
     ix = ix > G.g[0] - 1 ? G.g[0] - 1 : ix, iy = iy > G.g[1] - 1 ? G.g[1] - 1 : iy, iz = iz > G.g[2] - 1 ? G.g[2] - 1 : iz;
     const int sy_ = G.g[0] + 2, sz_ = sy_ * (G.g[1] + 2);
-    return cells[(ix + 1) + sy_ * (iy + 1) + sz_ * (iz + 1)];
+    return cells + size_t((ix + 1) + sy_ * (iy + 1) + sz_ * (iz + 1)) * size_t(nchunks);
+}
+
+// ... of a grid with one word per cell (at most 64 daughters)
+VG_HD unsigned long long nav_point_cell(const NavGrid &G, const unsigned long long *cells, double x, double y, double z)
+{
+    const unsigned long long *c = nav_point_cell_masks(G, cells, 1, x, y, z);
+    return c ? *c : 0ull;
+}
+
+// The candidates of a point's SAFETY (min over the daughters of SafetyToIn): the mask of the safety grid's cell that
+// holds it.  A daughter lies inside its bounding sphere (c, r), so for every point p of a cell
+//   |p - c| - r  <=  SafetyToIn(daughter)  <=  |p - c| + r,
+// and with U = min over the daughters of (farthest distance from the cell to c) + r, a daughter whose
+// (nearest distance from the cell to c) - r exceeds U is strictly farther than some other daughter everywhere in the
+// cell: it is never the minimum, and the cell's mask leaves it out (vg_volume_create / vg_world_create; a solid that can
+// be empty -- a boolean -- gives no upper bound and does not enter U).  The cells are taken `spad` larger than they
+// are, so a point that rounding puts into the neighbouring cell still finds its nearest daughter.  Returns the cell's
+// nchunks mask words, or NULL outside the grid's box -- the mother's bounding box: such a point is outside the mother --
+// or without a grid: the caller then keeps every daughter.
+VG_HD const unsigned long long *nav_safety_cell(const NavGrid &G, const unsigned long long *scells, int nchunks, double x,
+                                                double y, double z)
+{
+    const double px = x - G.so[0], py = y - G.so[1], pz = z - G.so[2];
+    if (G.gs <= 0 || !(px >= 0.0 && px <= G.slen[0] && py >= 0.0 && py <= G.slen[1] && pz >= 0.0 && pz <= G.slen[2])) return nullptr;
+    int ix = int(floor(px * G.sics[0])), iy = int(floor(py * G.sics[1])), iz = int(floor(pz * G.sics[2]));
+    ix = ix > G.gs - 1 ? G.gs - 1 : ix, iy = iy > G.gs - 1 ? G.gs - 1 : iy, iz = iz > G.gs - 1 ? G.gs - 1 : iz;
+    return scells + size_t((iz * G.gs + iy) * G.gs + ix) * size_t(nchunks);
 }
 
 // Both stages.  `all[c]` = every daughter of chunk c (what a start point outside the mother's bounding sphere keeps).

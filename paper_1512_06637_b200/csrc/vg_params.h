@@ -232,7 +232,8 @@ struct Daughter {
 //                              words so that lanes reading different daughters spread over the shared-memory banks
 //   [off_g, off_g + 8 ncell nchunks)  candidate masks of the grid cells (NavGrid below), off_g a multiple of 16
 //   [off_p, off_p + 4 ncell)          the only daughter of each cell or -1
-//   total rounded up to a multiple of 16 bytes (bulk-copy granularity)
+//   total (NavMeta::bytes) rounded up to a multiple of 16 bytes (bulk-copy granularity)
+//   [off_s, off_s + 8 gs^3 nchunks)   behind the staged part, read from device memory: the safety grid's masks
 constexpr int kCullUnroll = 8;
 constexpr int kDaughterStride = int(sizeof(Daughter)) + (((sizeof(Daughter) / 8) % 2 == 0) ? 8 : 0);
 constexpr int kNavChunks = 4; // 64 daughters per chunk, VG_MAX_DAUGHTERS = 256
@@ -242,6 +243,11 @@ constexpr int kNavKinds = 5;  // every kind except the polycone
 // cells of size cs, each with one 64-bit candidate mask per chunk at blob offset off_g, stored with a ring of empty cells
 // around the grid ([gz + 2][gy + 2][gx + 2][nchunks]).
 constexpr int kNavGridMax = 8; // cells per axis
+// The safety grid (vg_nav_cull.h, nav_safety_cell): a finer grid over the mother's own bounding box (every point with a
+// positive SafetyToOut lies in it) whose cells list the daughters that can be the NEAREST one of a point of the cell
+// (bounding-sphere bounds, taken at create time).
+constexpr int kNavSafeGridMax = 16;
+constexpr int kNavSafeGridMin = 8; // daughters from which the grid is built
 struct NavGrid {
     double o[3], len[3], cs[3], ics[3]; // origin, extent, cell size and its inverse per axis
     double tpad;                        // absolute slack added to the ray-parameter limit of the walk
@@ -249,7 +255,11 @@ struct NavGrid {
     int g[3];
     unsigned off_g;
     unsigned off_p; // int32 per cell (same ringed layout): the cell's only daughter, -1 if it lists none or several
-    int pad;
+    int gs;         // the SAFETY grid: gs^3 cells (no ring) over the bounding box of the MOTHER, 0 = none
+    double so[3], slen[3], sics[3]; // its origin, extent and inverse cell size per axis
+    double spad;    // how far outside its cell a point may sit and still find its nearest daughter in the cell's list
+    unsigned off_s; // its masks (nchunks words per cell): daughters that can be the nearest one of a point of the cell
+    unsigned pad;
 };
 
 struct NavMeta {
@@ -279,7 +289,8 @@ struct alignas(16) WorldNode {
 constexpr int kWorldGridMin = 12;
 struct WorldGrid {
     NavGrid g;
-    unsigned cells0, prim0; // first element of the node's cells / prim arrays in the world's pools
+    unsigned cells0, prim0; // first element of the node's cells / prim arrays in the world's pools (safety cells: g.off_s,
+                            // an element index into the cells pool)
     unsigned long long all; // every child of the node
 };
 

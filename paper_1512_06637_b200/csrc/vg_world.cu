@@ -208,20 +208,37 @@ __global__ void __launch_bounds__(kWorldBlock)
         stg1i(next + i, vol ? (phys ? -2 : (who < 0 ? -1 : who - 1)) : (phys ? nd : who));
     } else {
         double best = -node_sdf<EXT>(w, N, x, y, z);
-        // SafetyToIn of a child >= |p - c| - r.  Phase 1, FP32: children whose bound can undercut the node's own
-        // SafetyToOut (the spheres carry the FP32 error bound, see vg_world_create); a point outside its node (best <= 0)
-        // is outside every child, whose SafetyToIn is then positive and never the minimum.  Phase 2, FP64: the same
-        // bound against the running minimum, then the child's exact distance.
-        const float xf = float(x), yf = float(y), zf = float(z), bf = float(best);
+        // SafetyToIn of a child >= |p - c| - r: a child whose bound is not below the running minimum is skipped.  A point
+        // outside its node (best <= 0) is outside every child, whose SafetyToIn is then positive and never the minimum.
+        // The candidates: for a node with a safety grid, the children that can be nearest to a point of its cell
+        // (vg_nav_cull.h, nav_safety_cell), else every child.  The one whose sphere looks nearest (|p - c|^2 - r^2 in
+        // FP32, a heuristic with no bearing on the result: the minimum is order-independent) is evaluated first, so
+        // that the bound, taken in FP64 against the running minimum, leaves few of the others.
+        const float xf = float(x), yf = float(y), zf = float(z);
         for (int base = 0; base < nc && best > 0.0; base += 64) {
             const int lim = min(64, nc - base);
-            unsigned long long m = 0;
-#pragma unroll 4
-            for (int j = 0; j < lim; ++j) {
+            unsigned long long m = lim == 64 ? ~0ull : ((1ull << lim) - 1ull);
+            if (N.grid >= 0) {
+                const WorldGrid &G = w.grids[N.grid];
+                const unsigned long long *cell = nav_safety_cell(G.g, w.gcells + G.g.off_s, 1, x, y, z);
+                m = cell ? *cell : m;
+            }
+            int probe = -1;
+            float key = 3.0e38f;
+            for (unsigned long long mm = m; mm; mm &= mm - 1) {
+                const int j = __ffsll((long long)mm) - 1;
                 const float4 sp = __ldg(cull + c0 + base + j);
                 const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
-                const float reach = bf + sqrtf(sp.w);
-                m |= (unsigned long long)(fmaf(vx, vx, fmaf(vy, vy, vz * vz)) <= reach * reach) << j;
+                const float k = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, -sp.w)));
+                probe = k < key ? j : probe;
+                key = fminf(k, key);
+            }
+            if (probe >= 0) {
+                const WorldNode &C = nodes[kids[c0 + base + probe]];
+                double lx, ly, lz;
+                xf_point(C.X, x, y, z, lx, ly, lz);
+                best = dmin(best, node_sdf<EXT>(w, C, lx, ly, lz));
+                m &= ~(1ull << probe);
             }
             while (m) {
                 const int c = kids[c0 + base + __ffsll((long long)m) - 1];

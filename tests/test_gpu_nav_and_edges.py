@@ -350,6 +350,14 @@ def test_many_overlapping_daughters_of_all_kinds(vg, nd, size, spread):
     finally:
         vg.vg_set_option(vg.OPT_NAV_FORM, 0)
     assert len(set(ho.tolist())) > min(nd, 40) // 2
+    # vg_volume_safety is the plain minimum over the mother and EVERY daughter whatever the containment contract says:
+    # points inside several overlapping daughters, and points up to 1.3 half-lengths out (beyond the mother, beyond the
+    # safety grid's box and, for some, beyond the bounding box of the daughters' spheres)
+    assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), vo.safety(*t[:3]), "volume safety nd=%d, anywhere in the mother" % nd)
+    p = W.draw_tracks(78 + nd, 100003, (0, 0, 0), (78, 78, 78), band)[:3]
+    so_ = vo.safety(*p)
+    assert (so_ < -1.0).sum() > 1000 and (so_ > 1.0).sum() > 1000
+    assert_real_close(vgv.safety(*dev(p)).cpu().numpy(), so_, "volume safety nd=%d, beyond the mother" % nd)
 
 
 @pytest.mark.parametrize("form", [1, 2])

@@ -267,11 +267,13 @@ def test_flat_scenes_and_start_points_outside_the_mother():
 
 
 def test_the_cell_of_a_point_lists_every_daughter_that_holds_it():
-    """World Locate in a node with many children tests only the daughters listed in the point's grid cell: every daughter
+    """World Locate in a node with many children -- and vg_volume_safety for a point inside a daughter or outside the
+    mother -- test only the daughters listed in the point's grid cell: every daughter
     whose Inside (oracle) is INSIDE or SURFACE at the point must be in that mask -- random points, points on the daughters'
     surfaces and points on the grid's own cell planes, edges and corners."""
     rng = np.random.default_rng(11)
-    for sc, half in (config4_scene(), random_scene(4242, 40, 50.0, 12.0, 35.0), random_scene(77, 64, 1e3, 60.0, 800.0)):
+    for sc, half in (config4_scene(), random_scene(4242, 40, 50.0, 12.0, 35.0), random_scene(77, 64, 1e3, 60.0, 800.0),
+                     random_scene(99, 200, 100.0, 6.0, 90.0)):  # (four chunks of 64: what vg_volume_safety looks up)
         _, grid = sc.masks(np.zeros((1, 3)), np.array([[0.0, 0.0, 1.0]]))
         o, cs, g = grid[:3], grid[3:6], grid[6:9].astype(int)
         n = 200000
@@ -285,5 +287,55 @@ def test_the_cell_of_a_point_lists_every_daughter_that_holds_it():
             for k, s in enumerate(sc.o_d):
                 L = pts @ sc.R[k].T + sc.b[k]
                 holds = s.inside(L[:, 0], L[:, 1], L[:, 2]) != O.OUTSIDE
-                bit = (m[:, 0] >> np.uint64(k)) & np.uint64(1) == 1
+                bit = (m[:, k // 64] >> np.uint64(k % 64)) & np.uint64(1) == 1
                 assert not (holds & ~bit).any(), "%s: daughter %d holds %d points that its cell does not list" % (what, k, (holds & ~bit).sum())
+
+
+def test_the_safety_cell_of_a_point_lists_its_nearest_daughter():
+    """vg_volume_safety / vg_world_safety evaluate only the daughters listed in the point's cell of the safety grid
+    (vg_nav_cull.h, nav_safety_cell; stage 4): the minimum over the LISTED daughters of the oracle's SafetyToIn must be
+    the minimum over ALL of them, bit for bit -- random points, points on the daughters' surfaces, on the planes, edges
+    and corners of the safety grid itself, and points outside the grid's box (every daughter kept).  The lists must
+    also prune, and a grid must exist where this test means to exercise one."""
+    rng = np.random.default_rng(2027)
+    scenes = (config4_scene(), random_scene(4242, 40, 50.0, 12.0, 35.0), random_scene(77, 64, 1e3, 60.0, 800.0),
+              random_scene(99, 200, 100.0, 6.0, 90.0), random_scene(5, 100, 50.0, 20.0, 30.0), random_scene(8, 8, 1e4, 1e-2, 0.9e4),
+              random_scene(3, 5, 10.0, 2.0, 6.0))
+    for si, (sc, half) in enumerate(scenes):
+        nd = len(sc.kinds)
+        _, grid = sc.masks(np.zeros((1, 3)), np.array([[0.0, 0.0, 1.0]]), None, 4)
+        o, ext, gs = grid[:3], grid[3:6] * grid[6:9], int(grid[9])
+        assert (gs > 0) == (nd >= 8), "scene %d: %d daughters, safety grid of %d cells per axis" % (si, nd, gs)
+        n = 60000
+        P = rng.uniform(-1, 1, (n, 3)) * np.asarray(half)
+        _, Q = surface_points(sc, rng, n)
+        g1 = max(gs, 1)
+        node = o + ext / g1 * np.stack([rng.integers(0, g1 + 1, n) for a in range(3)], axis=1)
+        node = node * (1 + rng.choice([0.0, 1e-16, -1e-16, 1e-13, -1e-13], (n, 1)))
+        snapped = np.where(rng.random((n, 3)) < 0.6, node, rng.uniform(-1, 1, (n, 3)) * np.asarray(half))
+        outside = (o + ext * rng.uniform(-0.2, 1.2, (n, 3)))
+        listed = 0
+        for pts, what in ((P, "random"), (Q, "on a daughter's surface"), (snapped, "on the safety grid's planes"), (outside, "around the box")):
+            pts = np.ascontiguousarray(pts)
+            m, _ = sc.masks(pts, np.tile([0.0, 0.0, 1.0], (len(pts), 1)), None, 4)
+            s_all = np.empty((nd, len(pts)))
+            bits = np.zeros((nd, len(pts)), dtype=bool)
+            for k, s in enumerate(sc.o_d):
+                L = pts @ sc.R[k].T + sc.b[k]
+                s_all[k] = s.safety_to_in(L[:, 0], L[:, 1], L[:, 2])
+                bits[k] = (m[:, k // 64] >> np.uint64(k % 64)) & np.uint64(1) == 1
+            assert not (m[:, (nd + 63) // 64:] != 0).any() and bits.any(axis=0).all()
+            want = s_all.min(axis=0)
+            got = np.where(bits, s_all, np.inf).min(axis=0)
+            bad = got != want
+            assert not bad.any(), "scene %d, %s: the nearest daughter of %d points is not listed, first %s (listed min %r, min %r)" % (
+                si, what, bad.sum(), pts[bad][0].tolist(), got[bad][0], want[bad][0])
+            inbox = np.all((pts >= o) & (pts <= o + ext), axis=1)
+            if gs == 0:
+                assert bits.all()
+            else:
+                assert bits[:, ~inbox].all()  # outside the box: no cell, every daughter
+            if what == "random":
+                listed = bits[:, inbox].sum() / max(1, inbox.sum())
+        if si == 0:
+            assert listed < 12.0, "configs[4]: %.1f of 64 daughters listed per cell: the grid does not prune" % listed
