@@ -264,6 +264,27 @@ int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, c
                       const double *dy, const double *dz, double step_max, int64_t n, int32_t *cls, double *dist_in,
                       double *dist_out, double *safety_in, double *safety_out);
 
+/* vg_query_host_static -- vg_query_host for callers that must not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc; same operation as vg_query_host).  The device
+ * staging area is a static array inside the library's device image (7 x VG_STATIC_MAX_TRACKS doubles = 3.5 MiB, held
+ * by every GPU that loads the library until the process exits) instead of memory allocated on first use, and the call
+ * makes no cudaMalloc / cudaFree / cudaHostAlloc and creates no stream or event: the host -> device copies, the same
+ * kernel as the other entry points and the device -> host copy are enqueued on `stream` (a cudaStream_t, NULL = the
+ * default stream) and the call returns when `out` is complete (it synchronises that stream).
+ *   x, y, z (and dx, dy, dz for the two distance queries; may be NULL otherwise): HOST double[n], pageable or pinned;
+ *   out: HOST int32[n] for VG_Q_INSIDE, double[n] otherwise; the caller owns every array.
+ *   n > VG_STATIC_MAX_TRACKS: VG_ERR_PARAM and nothing is enqueued (split the batch, or call vg_query_host);
+ *   n = 0: VG_OK, no array is touched.
+ * All calls on a device share the one array: calls through this entry point are serialised by a lock and each waits
+ * for its own work, so they never overlap each other, but any other way of having two of them on the GPU at once
+ * (none is offered) would race.  The array keeps the previous call's contents; nothing in it needs to start at zero
+ * (a call overwrites the first n elements of each array its kernel reads, and only the first n results are copied
+ * out). */
+#define VG_STATIC_MAX_TRACKS 65536
+int vg_query_host_static(const vg_shape *shape, int query, const double *x, const double *y, const double *z,
+                         const double *dx, const double *dy, const double *dz, double step_max, int64_t n, void *out,
+                         void *stream);
+
 /* ---- launch policy (process-wide; does not change any result) ----
  * VG_OPT_PIPE_MIN_N: queries over at least this many tracks whose arrays are all 16-byte aligned run as the
  * persistent TMA-pipelined kernel (track tiles staged global -> shared memory by bulk copies);

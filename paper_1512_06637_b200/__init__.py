@@ -61,6 +61,7 @@ def _load():
     lib.vg_world_step.argtypes = [_VP, _VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP, _VP]
     lib.vg_world_safety.argtypes = [_VP, _VP, _VP, _VP, _VP, C.c_int64, _VP, _VP]
     lib.vg_query_host.argtypes = [_VP, C.c_int] + [_VP] * 6 + [C.c_double, C.c_int64, _VP]
+    lib.vg_query_host_static.argtypes = [_VP, C.c_int] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP]
     lib.vg_query_all_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64] + [_VP] * 5
     lib.vg_compute_step_host.argtypes = [_VP] + [_VP] * 6 + [C.c_double, C.c_int64, _VP, _VP]
     lib.vg_probe_fp64_fma_rate.argtypes = [C.c_int, _PD, _VP]
@@ -354,6 +355,27 @@ def vg_query_host(shape, query, x, y, z, dx=None, dy=None, dz=None, step_max=mat
     return out
 
 
+STATIC_MAX_TRACKS = 65536  # include/vg.h VG_STATIC_MAX_TRACKS
+
+
+def vg_query_host_static(shape, query, x, y, z, dx=None, dy=None, dz=None, step_max=math.inf, out=None, stream=None):
+    """vg_query_host without any allocation inside the library (include/vg.h): at most STATIC_MAX_TRACKS tracks, staged in
+    a static device array that all calls share.  `out` is a CPU tensor the caller owns (created here if None)."""
+    q = QUERY_ID[query] if isinstance(query, str) else int(query)
+    needs_dir = q in (1, 2)
+    arrs = (x, y, z, dx, dy, dz) if needs_dir else (x, y, z)
+    n = _host_tracks(arrs)
+    dtype = torch.int32 if q == 0 else torch.float64
+    if out is None:
+        out = torch.empty(n, dtype=dtype)
+    elif out.is_cuda or out.dtype != dtype or out.numel() != n or not out.is_contiguous():
+        raise TypeError("out: wrong dtype, length, device or layout")
+    null = C.c_void_p(0)
+    ptrs = [_p(a) for a in arrs] + ([] if needs_dir else [null] * 3)
+    _check(_lib.vg_query_host_static(_handle(shape), q, *ptrs, float(step_max), n, _p(out), _stream(stream)))
+    return out
+
+
 def vg_query_all_host(shape, x, y, z, dx, dy, dz, step_max=math.inf, out=None):
     """All five answers over HOST track arrays (one pass of the tracks over the host link).  `out`: optional tuple of
     CPU tensors (cls int32, dist_in, dist_out, safety_in, safety_out).  Returns that tuple when complete."""
@@ -454,6 +476,9 @@ class Shape:
 
     def query_host(self, name, x, y, z, dx=None, dy=None, dz=None, step_max=math.inf, out=None):
         return vg_query_host(self, name, x, y, z, dx, dy, dz, step_max, out)
+
+    def query_host_static(self, name, x, y, z, dx=None, dy=None, dz=None, step_max=math.inf, out=None, stream=None):
+        return vg_query_host_static(self, name, x, y, z, dx, dy, dz, step_max, out, stream)
 
 
 class Boolean(Shape):

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libvg.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-UNITS = ["vg_api", "vg_host", "vg_nav", "vg_world", "vg_bool", "vg_boolx", "vg_csg", "vg_bool_k0", "vg_bool_k1", "vg_bool_k2", "vg_bool_k3", "vg_bool_k4", "vg_probe", "vg_k_box", "vg_k_orb", "vg_k_tube", "vg_k_cone", "vg_k_trd", "vg_k_polycone"]
+UNITS = ["vg_api", "vg_host", "vg_static", "vg_nav", "vg_world", "vg_bool", "vg_boolx", "vg_csg", "vg_bool_k0", "vg_bool_k1", "vg_bool_k2", "vg_bool_k3", "vg_bool_k4", "vg_probe", "vg_k_box", "vg_k_orb", "vg_k_tube", "vg_k_cone", "vg_k_trd", "vg_k_polycone"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
          "-Xptxas", "-v", "-I", INCLUDE]
