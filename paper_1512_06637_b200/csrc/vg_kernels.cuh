@@ -98,25 +98,40 @@ template <int F> struct Tune<TubeT<F>, qSafeOut> {
 #ifndef VG_CONE_SAFE_BLOCK
 #define VG_CONE_SAFE_BLOCK 128
 #endif
+#ifndef VG_CONE_SAFE_MINB
+#define VG_CONE_SAFE_MINB VG_MINB
+#endif
 template <int F> struct Tune<ConeT<F>, qSafeIn> {
-    static constexpr int minb = VG_MINB;
+    static constexpr int minb = VG_CONE_SAFE_MINB;
     static constexpr bool stream = false;
     static constexpr int block = VG_CONE_SAFE_BLOCK;
 };
 template <int F> struct Tune<ConeT<F>, qSafeOut> {
-    static constexpr int minb = VG_MINB;
+    static constexpr int minb = VG_CONE_SAFE_MINB;
     static constexpr bool stream = false;
     static constexpr int block = VG_CONE_SAFE_BLOCK;
 };
+// The exact Trd safeties are bound by their FP64 instruction count (about 84 of 134 instructions per track), not by
+// the launch shape: the streaming form (128 registers, one resident wave) took 30.9 / 31.5 us at 4 Mi tracks, 256-thread
+// direct CTAs 33.0 / 33.9 us, 128-thread direct CTAs capped at 64 registers (8 CTAs per SM, no spills) 28.9 / 30.6 us.
+#ifndef VG_TRD_SAFE_BLOCK
+#define VG_TRD_SAFE_BLOCK 128
+#endif
+#ifndef VG_TRD_SAFE_MINB
+#define VG_TRD_SAFE_MINB 8
+#endif
+#ifndef VG_TRD_SAFE_STREAM
+#define VG_TRD_SAFE_STREAM false
+#endif
 template <> struct Tune<Trd, qSafeIn> {
-    static constexpr int minb = VG_MINB;
-    static constexpr bool stream = true;
-    static constexpr int block = kBlock;
+    static constexpr int minb = VG_TRD_SAFE_MINB;
+    static constexpr bool stream = VG_TRD_SAFE_STREAM;
+    static constexpr int block = VG_TRD_SAFE_BLOCK;
 };
 template <> struct Tune<Trd, qSafeOut> {
-    static constexpr int minb = VG_MINB;
-    static constexpr bool stream = true;
-    static constexpr int block = kBlock;
+    static constexpr int minb = VG_TRD_SAFE_MINB;
+    static constexpr bool stream = VG_TRD_SAFE_STREAM;
+    static constexpr int block = VG_TRD_SAFE_BLOCK;
 };
 
 template <class S, int Q, int TPT>
