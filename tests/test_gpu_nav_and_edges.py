@@ -446,6 +446,74 @@ def test_volume_with_polycone_and_boolean_solids(vg):
         assert (node_o[clear] == len(specs)).any()
 
 
+def test_volume_of_many_mixed_solids_uses_the_grids(vg):
+    """27 daughters on a 3 x 3 x 3 lattice -- primitives, polycones, booleans, CSG trees and three EMPTY booleans (a box minus
+    a far larger box: SafetyToIn > 0 everywhere and larger than |p - c| + r, so it must not bound the nearest-daughter
+    search) -- in one volume: more than 12 children, so the world kernels behind it take the candidate grid (Step, Locate)
+    and the safety grid (Safety).  Steps, hit indices, safeties and Locate against the oracle."""
+    bools = {b.name: b for b in W.boolean_cases()}
+    rng = np.random.default_rng(2718)
+    # (B far larger than A: the empty solid's SafetyToIn is ~500 everywhere, far above |p - c| + r of its bounding sphere)
+    empty = ("pair", (W.SUBTRACTION, W.BOX, [3.0, 3.0, 3.0], W.BOX, [500.0, 500.0, 500.0], W.placement(np.eye(3), (0.5, 0.0, 0.0))))
+    menu = [("shape", W.BOX, [5.0, 7.0, 4.0]), ("shape", W.ORB, [7.0]), ("shape", W.TUBE, [2.0, 6.0, 7.0, 0.3, 4.0]),
+            ("shape", W.CONE, [1.0, 4.0, 2.0, 7.0, 6.0, 0.0, TWO_PI]), ("shape", W.TRD, [3.0, 6.0, 5.0, 2.0, 6.0]),
+            ("shape", W.POLYCONE, [0.0, TWO_PI, 4.0, -7.0, 0.0, 3.0, -2.0, 1.0, 7.0, 3.0, 2.0, 5.0, 7.0, 0.0, 2.0]),
+            ("boolean", bools["box_union_orb"]), ("pair", (W.SUBTRACTION, W.ORB, [8.0], W.TUBE, [0.0, 3.0, 9.0, 0.0, TWO_PI],
+                                                              W.placement(np.eye(3), (1.0, 0.5, 0.0)))), empty,
+            ("tree", bools["box_union_orb"], (W.SUBTRACTION, W.TUBE, [0.0, 2.5, 12.0, 0.0, TWO_PI], W.placement(np.eye(3), (-1.0, 0.0, 0.0))))]
+    specs, xf = [], []
+    k = 0
+    for ix in (-1, 0, 1):
+        for iy in (-1, 0, 1):
+            for iz in (-1, 0, 1):
+                specs.append(menu[k % len(menu)])
+                k += 1
+                q = rng.normal(size=4)
+                c = np.array([ix, iy, iz]) * 26.0 + rng.uniform(-2.0, 2.0, 3)
+                xf.append(W.placement(W.quaternion_to_matrix(tuple(q / np.linalg.norm(q))), tuple(c)))
+
+    def mk(mod, sp):
+        if sp[0] == "shape":
+            return mod.Shape(sp[1], sp[2])
+        if sp[0] == "pair":
+            op, ka, pa, kb, pb, xb = sp[1]
+            return mod.Boolean(op, mod.Shape(ka, pa), mod.Shape(kb, pb), xb)
+        b = sp[1]
+        inner = mod.Boolean(b.op, mod.Shape(b.kind_a, b.par_a), mod.Shape(b.kind_b, b.par_b), b.xform)
+        if sp[0] == "tree":  # (A op B) op2 C: a CSG tree of three primitives (R31)
+            op2, kc, pc, xc = sp[2]
+            return mod.Boolean(op2, inner, mod.Shape(kc, pc), xc)
+        return inner
+    ident = W.placement(np.eye(3), (0, 0, 0))
+    mother = ("shape", W.BOX, [42.0, 42.0, 42.0])
+    wo = O.World([mk(O, mother)] + [mk(O, sp) for sp in specs], [-1] + [0] * len(specs), [ident] + xf)
+    vgv = vg.Volume(mk(vg, mother), [mk(vg, sp) for sp in specs], xf)
+    wg = vg.World([mk(vg, mother)] + [mk(vg, sp) for sp in specs], [-1] + [0] * len(specs), [ident] + xf)
+    n_nodes = len(specs) + 1
+
+    def near_a_surface(x, y, z):
+        near = np.zeros(x.size, dtype=bool)
+        for nd in range(n_nodes):
+            near |= np.abs(wo.safety(np.full(x.size, nd, dtype=np.int32), x, y, z)) < 1e-4
+        return near
+    t = W.draw_tracks(93, 120001, (0, 0, 0), (42, 42, 42), lambda x, y, z: (wo.locate(x, y, z) != 0) | near_a_surface(x, y, z))
+    zero = np.zeros(t[0].size, dtype=np.int32)
+    for step_max in (W.STEP_MAX, 15.0):
+        so, no = wo.step(zero, *t, step_max)
+        sg, hg = vgv.compute_step(*dev(t), step_max)
+        want_hit = np.where(no == 0, -2, np.where(no < 0, -1, no - 1))
+        assert_int_equal(hg.cpu().numpy(), want_hit, "many mixed solids hit step_max=%g" % step_max)
+        assert_real_close(sg.cpu().numpy(), so, "many mixed solids step step_max=%g" % step_max)
+    hits = set(np.unique(want_hit).tolist())
+    assert len(hits) >= 20 and not any(specs[h] is empty for h in hits if h >= 0)  # nothing ever hits an empty solid
+    assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), wo.safety(zero, *t[:3]), "many mixed solids safety")
+    # points anywhere (inside the daughters, outside the mother): Locate bit-exact, per-node safety of the mother
+    p = W.draw_tracks(94, 120001, (0, 0, 0), (50, 50, 50), near_a_surface)[:3]
+    assert_int_equal(wg.locate(*dev(p)).cpu().numpy(), wo.locate(*p), "many mixed solids locate")
+    zp = np.zeros(p[0].size, dtype=np.int32)
+    assert_real_close(wg.safety(torch.from_numpy(zp).cuda(), *dev(p)).cpu().numpy(), wo.safety(zp, *p), "many mixed solids safety anywhere")
+
+
 # ------------------------------------------------------------------------------- host-buffer entry points
 
 @pytest.mark.parametrize("n", [1, 4097, 65536, 1048576 + 3, 3 * 1048576 + 11])
