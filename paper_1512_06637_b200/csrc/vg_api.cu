@@ -1084,7 +1084,7 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         wg.g.off_s = unsigned(gcells.size());
         if (wg.g.gs > 0) {
             std::vector<char> bounded;
-            for (int j = 0; j < P.nchild; ++j) bounded.push_back(shapes[kids[P.child0 + j]]->kind != VG_BOOLEAN);
+            for (int j = 0; j < P.nchild; ++j) bounded.push_back(shapes[kids[P.child0 + j]]->kind < VG_BOOLEAN); // (a tree or a polycone-operand boolean: kind > VG_BOOLEAN)
             gcells.resize(gcells.size() + size_t(wg.g.gs) * wg.g.gs * wg.g.gs, 0ull);
             double fh[3] = { radius[p], radius[p], radius[p] }; // a polycone or boolean node: the cube about its sphere
             if (P.s.kind < kPolycone) bounding_half(P.s, fh);

@@ -447,7 +447,7 @@ def test_volume_with_polycone_and_boolean_solids(vg):
 
 
 def test_volume_of_many_mixed_solids_uses_the_grids(vg):
-    """27 daughters on a 3 x 3 x 3 lattice -- primitives, polycones, booleans, CSG trees and three EMPTY booleans (a box minus
+    """27 daughters on a 3 x 3 x 3 lattice -- primitives, polycones, booleans, CSG trees and EMPTY booleans of all three record kinds (a solid minus
     a far larger box: SafetyToIn > 0 everywhere and larger than |p - c| + r, so it must not bound the nearest-daughter
     search) -- in one volume: more than 12 children, so the world kernels behind it take the candidate grid (Step, Locate)
     and the safety grid (Safety).  Steps, hit indices, safeties and Locate against the oracle."""
@@ -460,7 +460,13 @@ def test_volume_of_many_mixed_solids_uses_the_grids(vg):
             ("shape", W.POLYCONE, [0.0, TWO_PI, 4.0, -7.0, 0.0, 3.0, -2.0, 1.0, 7.0, 3.0, 2.0, 5.0, 7.0, 0.0, 2.0]),
             ("boolean", bools["box_union_orb"]), ("pair", (W.SUBTRACTION, W.ORB, [8.0], W.TUBE, [0.0, 3.0, 9.0, 0.0, TWO_PI],
                                                               W.placement(np.eye(3), (1.0, 0.5, 0.0)))), empty,
-            ("tree", bools["box_union_orb"], (W.SUBTRACTION, W.TUBE, [0.0, 2.5, 12.0, 0.0, TWO_PI], W.placement(np.eye(3), (-1.0, 0.0, 0.0))))]
+            ("tree", bools["box_union_orb"], (W.SUBTRACTION, W.TUBE, [0.0, 2.5, 12.0, 0.0, TWO_PI], W.placement(np.eye(3), (-1.0, 0.0, 0.0)))),
+            # ... an empty CSG tree and an empty boolean with a polycone operand (other record kinds inside the library)
+            # (small, so that their bounding spheres would be a tight -- and wrong -- upper bound)
+            ("tree", W.BooleanCase("tiny", W.UNION, W.BOX, [2.0, 2.0, 2.0], W.ORB, [2.0], (1.0, 0.0, 0.0), (0.0, 0.0, 0.0, 1.0), 1),
+             (W.SUBTRACTION, W.BOX, [500.0, 500.0, 500.0], W.placement(np.eye(3), (0.0, 0.0, 0.0)))),
+            ("pair", (W.SUBTRACTION, W.POLYCONE, [0.0, TWO_PI, 3.0, -2.0, 0.0, 1.0, 0.0, 0.5, 2.0, 2.0, 0.0, 1.0], W.BOX, [500.0, 500.0, 500.0],
+                      W.placement(np.eye(3), (0.0, 0.0, 0.0))))]
     specs, xf = [], []
     k = 0
     for ix in (-1, 0, 1):
@@ -485,7 +491,7 @@ def test_volume_of_many_mixed_solids_uses_the_grids(vg):
             return mod.Boolean(op2, inner, mod.Shape(kc, pc), xc)
         return inner
     ident = W.placement(np.eye(3), (0, 0, 0))
-    mother = ("shape", W.BOX, [42.0, 42.0, 42.0])
+    mother = ("shape", W.BOX, [60.0, 60.0, 60.0])  # well clear of the lattice: near a daughter, its neighbours are nearer than the mother
     wo = O.World([mk(O, mother)] + [mk(O, sp) for sp in specs], [-1] + [0] * len(specs), [ident] + xf)
     vgv = vg.Volume(mk(vg, mother), [mk(vg, sp) for sp in specs], xf)
     wg = vg.World([mk(vg, mother)] + [mk(vg, sp) for sp in specs], [-1] + [0] * len(specs), [ident] + xf)
@@ -496,7 +502,7 @@ def test_volume_of_many_mixed_solids_uses_the_grids(vg):
         for nd in range(n_nodes):
             near |= np.abs(wo.safety(np.full(x.size, nd, dtype=np.int32), x, y, z)) < 1e-4
         return near
-    t = W.draw_tracks(93, 120001, (0, 0, 0), (42, 42, 42), lambda x, y, z: (wo.locate(x, y, z) != 0) | near_a_surface(x, y, z))
+    t = W.draw_tracks(93, 120001, (0, 0, 0), (60, 60, 60), lambda x, y, z: (wo.locate(x, y, z) != 0) | near_a_surface(x, y, z))
     zero = np.zeros(t[0].size, dtype=np.int32)
     for step_max in (W.STEP_MAX, 15.0):
         so, no = wo.step(zero, *t, step_max)
@@ -505,13 +511,26 @@ def test_volume_of_many_mixed_solids_uses_the_grids(vg):
         assert_int_equal(hg.cpu().numpy(), want_hit, "many mixed solids hit step_max=%g" % step_max)
         assert_real_close(sg.cpu().numpy(), so, "many mixed solids step step_max=%g" % step_max)
     hits = set(np.unique(want_hit).tolist())
-    assert len(hits) >= 20 and not any(specs[h] is empty for h in hits if h >= 0)  # nothing ever hits an empty solid
+    is_empty = lambda sp: sp is empty or (sp[0] in ("pair", "tree") and 500.0 in (sp[1][4] if sp[0] == "pair" else sp[2][2]))
+    assert sum(is_empty(sp) for sp in specs) >= 6
+    assert len(hits) >= 17 and not any(is_empty(specs[h]) for h in hits if h >= 0)  # nothing ever hits an empty solid
     assert_real_close(vgv.safety(*dev(t[:3])).cpu().numpy(), wo.safety(zero, *t[:3]), "many mixed solids safety")
     # points anywhere (inside the daughters, outside the mother): Locate bit-exact, per-node safety of the mother
-    p = W.draw_tracks(94, 120001, (0, 0, 0), (50, 50, 50), near_a_surface)[:3]
+    p = W.draw_tracks(94, 120001, (0, 0, 0), (70, 70, 70), near_a_surface)[:3]
     assert_int_equal(wg.locate(*dev(p)).cpu().numpy(), wo.locate(*p), "many mixed solids locate")
     zp = np.zeros(p[0].size, dtype=np.int32)
     assert_real_close(wg.safety(torch.from_numpy(zp).cuda(), *dev(p)).cpu().numpy(), wo.safety(zp, *p), "many mixed solids safety anywhere")
+    # points around the centres of the empty solids: the nearest daughter is a NEIGHBOUR, 15-20 away, although the empty
+    # solid's bounding sphere is right there
+    rng = np.random.default_rng(5)
+    cs = np.stack([-(np.asarray(m).reshape(3, 4)[:, :3].T @ np.asarray(m).reshape(3, 4)[:, 3]) for sp, m in zip(specs, xf) if is_empty(sp)])
+    q = cs[rng.integers(0, len(cs), 60000)] + rng.uniform(-9.0, 9.0, (60000, 3))
+    q = tuple(np.ascontiguousarray(q[:, a]) for a in range(3))
+    zq = np.zeros(60000, dtype=np.int32)
+    want = wo.safety(zq, *q)
+    assert (want > 5.0).sum() > 20000
+    assert_real_close(vgv.safety(*dev(q)).cpu().numpy(), want, "safety around the empty solids (volume)")
+    assert_real_close(wg.safety(torch.from_numpy(zq).cuda(), *dev(q)).cpu().numpy(), want, "safety around the empty solids (world)")
 
 
 # ------------------------------------------------------------------------------- host-buffer entry points
