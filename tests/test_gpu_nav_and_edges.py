@@ -360,6 +360,57 @@ def test_many_overlapping_daughters_of_all_kinds(vg, nd, size, spread):
     assert_real_close(vgv.safety(*dev(p)).cpu().numpy(), so_, "volume safety nd=%d, beyond the mother" % nd)
 
 
+def test_random_volumes_step_and_safety_soak(vg):
+    """Seeded random volumes (VG_STRESS_REPS of them, default 12): 1..256 daughters of the five kinds, sizes from a
+    hundredth to a third of the mother, clustered or spread, in a box / orb / tube mother -- every geometry gives the
+    candidate grid and the safety grid other cells, lists and margins.  ComputeStep (steps, hit indices) for tracks
+    anywhere in the mother, the volume safety for points up to 1.3 half-lengths out, against the oracle."""
+    reps = int(os.environ.get("VG_STRESS_REPS", "12"))
+    for rep in range(reps):
+        rng = np.random.default_rng(9000 + rep)
+        nd = int(rng.choice([1, 2, 7, 8, 9, 13, 40, 63, 64, 65, 128, 129, 200, 256]))
+        H = float(rng.choice([10.0, 60.0, 1000.0]))
+        size = H * float(rng.choice([0.01, 0.05, 0.15, 0.33]))
+        spread = H * float(rng.choice([0.2, 0.6, 0.85]))
+        kinds, pars, xf = [], [], []
+        for _ in range(nd):
+            kind = [W.BOX, W.ORB, W.TUBE, W.CONE, W.TRD][rng.integers(0, 5)]
+            a, b, c = size * rng.uniform(0.3, 1.0, 3)
+            par = {W.BOX: [a, b, c], W.ORB: [a], W.TUBE: [0.3 * a, a, b, 0.5, 4.0],
+                   W.CONE: [0.2 * a, a, 0.3 * b, 1.2 * b, c, 0.0, TWO_PI], W.TRD: [a, 0.5 * a, b, 1.3 * b, c]}[kind]
+            q = rng.normal(size=4)
+            kinds.append(kind)
+            pars.append(par)
+            xf.append(W.placement(W.quaternion_to_matrix(tuple(q / np.linalg.norm(q))), rng.uniform(-spread, spread, 3)))
+        xf = np.stack(xf)
+        mk, mp = [(W.BOX, [H, H, H]), (W.ORB, [1.6 * H]), (W.TUBE, [0.0, 1.5 * H, H, 0.0, TWO_PI])][rep % 3]
+        vo = O.Volume(O.Shape(mk, mp), [O.Shape(k, p) for k, p in zip(kinds, pars)], xf)
+        vgv = vg.Volume(vg.Shape(mk, mp), [vg.Shape(k, p) for k, p in zip(kinds, pars)], xf)
+        band_w = 1e-6 * max(1.0, H / 60.0)
+
+        def band(x, y, z):
+            near = np.abs(vo.mother.sdf(x, y, z)) < band_w
+            for d, m in zip(vo.daughters, vo.xforms):
+                M = m.reshape(3, 4)
+                lx, ly, lz = (M[i, 0] * x + M[i, 1] * y + M[i, 2] * z + M[i, 3] for i in range(3))
+                near |= np.abs(d.sdf(lx, ly, lz)) < band_w
+            return near
+        what = "soak %d: nd=%d H=%g size=%g spread=%g mother=%d" % (rep, nd, H, size, spread, mk)
+        t = W.draw_tracks(9100 + rep, 20011, (0, 0, 0), (H, H, H), lambda x, y, z: band(x, y, z) | (vo.mother.sdf(x, y, z) > 0))
+        for step_max in (W.STEP_MAX, 0.4 * H):
+            check_step(vo, vgv, t, step_max, what + " step_max=%g" % step_max)
+        p = W.draw_tracks(9200 + rep, 30011, (0, 0, 0), (1.3 * H,) * 3, band)[:3]
+        assert_real_close(vgv.safety(*dev(p)).cpu().numpy(), vo.safety(*p), what + " safety")
+        # ... and around the daughters, where the lists of the safety grid's cells matter most
+        k = rng.integers(0, nd, 20011)
+        c = -np.einsum("nji,nj->ni", xf.reshape(-1, 3, 4)[k][:, :, :3], xf.reshape(-1, 3, 4)[k][:, :, 3])
+        q3 = c + rng.uniform(-2.5 * size, 2.5 * size, (20011, 3))
+        q3 = tuple(np.ascontiguousarray(q3[:, a]) for a in range(3))
+        keep = ~band(*q3)
+        q3 = tuple(np.ascontiguousarray(a[keep]) for a in q3)
+        assert_real_close(vgv.safety(*dev(q3)).cpu().numpy(), vo.safety(*q3), what + " safety around the daughters")
+
+
 @pytest.mark.parametrize("form", [1, 2])
 def test_config4_both_forms_of_phase_two(vg, form):
     nav = W.navigator_case()
