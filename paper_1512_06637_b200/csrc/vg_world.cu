@@ -208,14 +208,14 @@ __global__ void __launch_bounds__(kWorldBlock)
         stg1i(next + i, vol ? (phys ? -2 : (who < 0 ? -1 : who - 1)) : (phys ? nd : who));
     } else {
         double best = -node_sdf<EXT>(w, N, x, y, z);
-        // SafetyToIn of a child >= |p - c| - r: a child whose bound is not below the running minimum is skipped.  A point
-        // outside its node (best <= 0) is outside every child, whose SafetyToIn is then positive and never the minimum.
+        // SafetyToIn of a child >= |p - c| - r: a child whose bound is not below the running minimum is skipped (valid for
+        // a minimum of either sign, so trees whose children overlap or stick out of their parent get the plain minimum too).
         // The candidates: for a node with a safety grid, the children that can be nearest to a point of its cell
         // (vg_nav_cull.h, nav_safety_cell), else every child.  The one whose sphere looks nearest (|p - c|^2 - r^2 in
         // FP32, a heuristic with no bearing on the result: the minimum is order-independent) is evaluated first, so
         // that the bound, taken in FP64 against the running minimum, leaves few of the others.
         const float xf = float(x), yf = float(y), zf = float(z);
-        for (int base = 0; base < nc && best > 0.0; base += 64) {
+        for (int base = 0; base < nc; base += 64) { // (every chunk whatever the sign so far: the result is the plain minimum)
             const int lim = min(64, nc - base);
             unsigned long long m = lim == 64 ? ~0ull : ((1ull << lim) - 1ull);
             if (N.grid >= 0) {

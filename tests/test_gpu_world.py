@@ -173,3 +173,70 @@ def test_mixed_world_matches_the_oracle(vg, mixed_worlds, n):
     if n > 100000:
         counts = np.bincount(node_o, minlength=13)
         assert np.all(counts[:9] > 1000) and counts[9:].sum() > 50
+
+
+# ------------------------------------------------------------------------------------- random trees (soak)
+
+def _random_tree(rng):
+    """Root box (100) > k1 children of random kinds, sizes and rotations (they may overlap: Locate takes the first in index
+    order, Step and Safety are minima) > for some box / orb children, k2 grand-children inside them."""
+    TWO_PI = 2 * np.pi
+    H = 100.0
+
+    def solid(size):
+        kind = [W.BOX, W.ORB, W.TUBE, W.CONE, W.TRD, W.POLYCONE][rng.integers(0, 6)]
+        a, b, c = size * rng.uniform(0.4, 1.0, 3)
+        par = {W.BOX: [a, b, c], W.ORB: [a], W.TUBE: [0.3 * a, a, b, 0.5, 4.0],
+               W.CONE: [0.2 * a, a, 0.3 * b, 1.2 * b, c, 0.0, TWO_PI], W.TRD: [a, 0.5 * a, b, 1.3 * b, c],
+               W.POLYCONE: [0.0, TWO_PI, 4.0, -c, 0.0, 0.5 * a, -0.3 * c, 0.2 * a, a, 0.3 * c, 0.2 * a, 0.6 * a, c, 0.0, 0.4 * a]}[kind]
+        return kind, [float(v) for v in par]
+
+    def place(spread):
+        q = rng.normal(size=4)
+        return W.placement(W.quaternion_to_matrix(tuple(q / np.linalg.norm(q))), rng.uniform(-spread, spread, 3))
+    kinds, pars, parents, xf = [W.BOX], [[H, H, H]], [-1], [W.placement(np.eye(3), (0, 0, 0))]
+    k1 = int(rng.choice([3, 11, 12, 13, 30, 64, 70]))
+    size = H * float(rng.choice([0.06, 0.12, 0.2]))
+    for _ in range(k1):
+        k, p = solid(size)
+        kinds.append(k), pars.append(p), parents.append(0), xf.append(place(H - 1.8 * size))
+    for i in range(1, k1 + 1):
+        if kinds[i] in (W.BOX, W.ORB) and rng.random() < 0.5:
+            inner = min(pars[i])
+            for _ in range(int(rng.choice([1, 2, 12, 20]))):
+                k, p = solid(0.22 * inner)
+                kinds.append(k), pars.append(p), parents.append(i), xf.append(place(0.45 * inner))
+    return kinds, pars, parents, np.stack(xf)
+
+
+def test_random_trees_soak(vg):
+    """VG_STRESS_REPS seeded random trees (default 8): Locate of points anywhere, Step and Safety in the located nodes and
+    in the root, against the oracle.  Nodes with 12..64 children take the candidate and safety grids, the others the
+    sphere loops."""
+    import os
+    for rep in range(int(os.environ.get("VG_STRESS_REPS", "8"))):
+        rng = np.random.default_rng(7000 + rep)
+        kinds, pars, parents, xf = _random_tree(rng)
+        nn = len(kinds)
+        wo = O.World([O.Shape(k, p) for k, p in zip(kinds, pars)], parents, xf)
+        wg = vg.World([vg.Shape(k, p) for k, p in zip(kinds, pars)], parents, xf)
+
+        def band(x, y, z):  # clear of the surface of EVERY node (children overlap: a point may be near a sibling's surface)
+            bad = wo.locate(x, y, z) < 0
+            for nd in range(nn):
+                bad |= np.abs(wo.safety(np.full(x.size, nd, dtype=np.int32), x, y, z)) < 1e-6
+            return bad
+        t = W.draw_tracks(7100 + rep, 20011, (0, 0, 0), (100, 100, 100), band)
+        dt = dev(t)
+        what = "random tree %d (%d nodes, %d under the root)" % (rep, nn, parents.count(0))
+        node_o = wo.locate(*t[:3])
+        node_g = wg.locate(*dt[:3])
+        assert_int_equal(node_g.cpu().numpy(), node_o, what + " locate")
+        for nodes in (node_o, np.zeros_like(node_o)):
+            ng_in = torch.from_numpy(nodes).cuda()
+            for step_max in (W.STEP_MAX, 12.0):
+                so, no = wo.step(nodes, *t, step_max)
+                sg, ng = wg.step(ng_in, *dt, step_max)
+                assert_int_equal(ng.cpu().numpy(), no, what + " next")
+                assert_real_close(sg.cpu().numpy(), so, what + " step")
+            assert_real_close(wg.safety(ng_in, *dt[:3]).cpu().numpy(), wo.safety(nodes, *t[:3]), what + " safety")
