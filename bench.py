@@ -47,7 +47,7 @@ UNIT = "track-queries/s"
 # algorithmic bytes per track: SoA inputs read once + one result written once
 BYTES = {"inside": 24 + 4, "safety_to_in": 24 + 8, "safety_to_out": 24 + 8, "distance_to_in": 48 + 8,
          "distance_to_out": 48 + 8, "compute_step": 48 + 12, "all": 48 + 4 + 4 * 8}
-BYTES.update({"world_locate": 24 + 4, "world_step": 48 + 4 + 8 + 4, "world_safety": 24 + 4 + 8})
+BYTES.update({"world_locate": 24 + 4, "world_step": 48 + 4 + 8 + 4, "world_safety": 24 + 4 + 8, "volume_safety": 24 + 8})
 L2_BYTES = 126e6
 COLD_ROTATION_BYTES = 4 * 126e6  # bytes of track arrays in rotation (>= 256 MB): even Inside, which reads half
                                  # of a set, comes back to a set only after >= 2 x L2 of other reads
@@ -231,6 +231,8 @@ class Case:
             self.handle.safety(self.nodes[k], *s[:3], out=self.outd[k])
         elif q == "compute_step":
             self.handle.compute_step(*s, step_max=W.STEP_MAX, step=self.outd[k], hit=self.outi[k])
+        elif q == "volume_safety":
+            self.handle.safety(*s[:3], out=self.outd[k])
         elif q.startswith("probe:"):  # the arithmetic-free kernel of the same loads, store, grid and form (vg_probe_stream)
             pq = q[6:]
             out = self.outi[k] if pq == "inside" else self.outd[k]
@@ -643,6 +645,10 @@ def detail_sweep(vg, torch, hbm_peak, fma_rate, have, headline_rows, min_ms, emi
     sec = tq(case, "compute_step")
     e = roofline_entry("navigator", "compute_step", case.n, sec, hbm_peak, fma_rate)
     e.update({"config": 4, "shape": "box(100)+64 daughters", "query": "compute_step", "n": case.n, "cold_inputs": case.cold})
+    add(e)
+    sec = tq(case, "volume_safety")  # vg_volume_safety (an addition of this build): not part of any step
+    e = roofline_entry("navigator", "volume_safety", case.n, sec, hbm_peak, fma_rate)
+    e.update({"config": "4 (+)", "shape": "box(100)+64 daughters", "query": "volume_safety", "n": case.n, "cold_inputs": case.cold})
     add(e)
     del case
     torch.cuda.empty_cache()
