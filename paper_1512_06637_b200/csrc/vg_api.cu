@@ -266,7 +266,7 @@ static int run_query(const char *fn, int q, const vg_shape *s, const double *x, 
         e = launch_polycone(q, s->u.pcon, g, t, step_max, n, out, vec, st);
         break;
     }
-    case VG_BOOLEAN: e = launch_boolean(q, s->u.boolean, t, step_max, n, out, st); break;
+    case VG_BOOLEAN: e = launch_boolean(q, s->u.boolean, t, step_max, n, out, st, vec); break;
     case kCsg: e = launch_csg(q, s->u.csg, t, step_max, n, out, st); break;
     case kBoolX: {
         int rcd = check_device(s->ext_device, fn);

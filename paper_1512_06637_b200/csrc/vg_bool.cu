@@ -14,10 +14,16 @@
 
 namespace vg {
 
-cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s)
+cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s, bool vec)
 {
     if (n <= 0) return cudaSuccess;
     const unsigned grid = unsigned((n + kBoolBlock - 1) / kBoolBlock);
+    if (vec && n >= 2 * 148 * VG_BOOL_PT_BLOCK) // (smaller batches: one track per thread fills more SMs)
+        switch (q) {
+        case qInside: return launch_bool_point2<qInside>(p, t, n, out, s);
+        case qSafeIn: return launch_bool_point2<qSafeIn>(p, t, n, out, s);
+        case qSafeOut: return launch_bool_point2<qSafeOut>(p, t, n, out, s);
+        }
     switch (q) {
     case qInside: return launch_kernel(bool_kernel<qInside, -1, -1>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);
     case qSafeIn: return launch_kernel(bool_kernel<qSafeIn, -1, -1>, grid, kBoolBlock, 0, s, p, t, step_max, n, out);

@@ -599,7 +599,8 @@ cudaError_t launch_volume_safety(const SolidU &mother, const unsigned char *tabl
                                  double *safety, cudaStream_t s);
 
 // boolean solids (vg_bool.cu)
-cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
+cudaError_t launch_boolean(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s,
+                           bool vec = false);
 
 // booleans with a polycone operand (vg_boolx.cu)
 cudaError_t launch_boolx(int q, const BoolP &p, const Tracks &t, double step_max, int64_t n, void *out, cudaStream_t s);
