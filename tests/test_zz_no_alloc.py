@@ -87,3 +87,33 @@ def test_sizes_beyond_the_static_array_are_rejected(vg):
         sg.query_host_static("safety_to_in", a, a, a, out=out)
     assert bool((out == 7.0).all())  # nothing was enqueued
     assert sg.query_host_static("safety_to_in", a[:0], a[:0], a[:0]).numel() == 0  # n = 0: nothing to do
+
+
+def test_two_host_threads_share_the_array_without_racing(vg):
+    """All calls use ONE staging array; the entry point serialises them with a lock and waits for its own work, so two host
+    threads on two streams, each with its own tracks, must both get their own answers (ctypes drops the GIL in the call)."""
+    import threading
+    sc = W.shape_cases(1)[0]
+    so, sg = O.Shape(sc.kind, sc.params), vg.Shape(sc.kind, sc.params)
+    c, h = W.bounding_half(sc.kind, sc.params)
+    jobs = []
+    for k in range(2):
+        t = W.draw_tracks(300 + k, 30000 + 5000 * k, c, tuple(1.5 * v for v in h), band(so))
+        jobs.append((t, host(t, True), so.distance_to_in(*t, W.STEP_MAX), torch.cuda.Stream()))
+    errors = []
+
+    def work(k):
+        t, ht, want, st = jobs[k]
+        try:
+            torch.cuda.set_device(0)
+            for _ in range(40):
+                got = sg.query_host_static("distance_to_in", *ht, step_max=W.STEP_MAX, stream=st).numpy()
+                assert_real_close(got, want, "thread %d" % k)
+        except Exception as e:  # noqa: BLE001 (reported by the main thread)
+            errors.append(e)
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    for th in threads:
+        th.start()
+    for th in threads:
+        th.join()
+    assert not errors, errors[0]
