@@ -153,6 +153,27 @@ def main():
         assert_real_close(cg.distance_to_in(*dt, W.STEP_MAX).cpu().numpy(), co.distance_to_in(*t, W.STEP_MAX), bc.name)
         assert_real_close(cg.distance_to_out(*dt, W.STEP_MAX).cpu().numpy(), co.distance_to_out(*t, W.STEP_MAX), bc.name)
         assert_real_close(cg.safety_to_in(*dt[:3]).cpu().numpy(), co.safety_to_in(*t[:3]), bc.name)
+    # the two-tracks-per-thread point kernels of the booleans (aligned arrays, >= 2 x 148 x 256 tracks): odd size, guarded outputs
+    bc = W.boolean_cases()[0]
+    co = O.Boolean(bc.op, O.Shape(bc.kind_a, bc.par_a), O.Shape(bc.kind_b, bc.par_b), bc.xform)
+    cg = vg.Boolean(bc.op, vg.Shape(bc.kind_a, bc.par_a), vg.Shape(bc.kind_b, bc.par_b), bc.xform)
+    M = np.asarray(bc.xform).reshape(3, 4)
+
+    def bband2(x, y, z):
+        L = M[:, :3] @ np.stack([x, y, z]) + M[:, 3:4]
+        return (np.abs(co.a.sdf(x, y, z)) < W.SURFACE_BAND) | (np.abs(co.b.sdf(L[0], L[1], L[2])) < W.SURFACE_BAND)
+    nb = 2 * 148 * 256 + 5
+    t = bc.tracks(nb, bband2)
+    dt = dev(t)
+    bi, oi = guarded(nb, torch.int32)
+    cg.inside(*dt[:3], out=oi)
+    assert guards_intact(bi, nb), "boolean inside (two tracks per thread) wrote outside its array"
+    assert_int_equal(oi.cpu().numpy(), co.inside(*t[:3]), "boolean inside, two tracks per thread")
+    for q in ("safety_to_in", "safety_to_out"):
+        bd, od = guarded(nb, torch.float64)
+        getattr(cg, q)(*dt[:3], out=od)
+        assert guards_intact(bd, nb), "boolean %s (two tracks per thread) wrote outside its array" % q
+        assert_real_close(od.cpu().numpy(), getattr(co, q)(*t[:3]), "boolean %s, two tracks per thread" % q)
     vg.vg_probe_fp64_fma_rate(1)
     vg.vg_probe_empty_launch(2)
     torch.cuda.synchronize()
