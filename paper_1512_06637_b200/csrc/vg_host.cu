@@ -62,7 +62,7 @@ static int64_t pick_chunk(int64_t n)
     const int64_t forced = g_host_chunk.load(std::memory_order_relaxed); // vg_set_option(VG_OPT_HOST_CHUNK)
     if (forced > 0) return forced < kMaxChunk ? (forced + 1) / 2 * 2 : kMaxChunk;
     // One chunk per slot, between 64 Ki and 512 Ki tracks: every cudaMemcpyAsync costs ~5 us of engine set-up, so copies
-    // under ~2 MB per array leave the link idle (measured, profiles/r1g_host_chunk.md: 1 Mi tracks 1.70 ms with 128 Ki
+    // under ~2 MB per array leave the link idle (measured, DESIGN.md Appendix A.2: 1 Mi tracks 1.70 ms with 128 Ki
     // chunks, 1.41 ms with 256-512 Ki), while fewer than three chunks cannot overlap H2D with D2H.
     int64_t c = (n + kSlots - 1) / kSlots;
     c = (c + 4095) / 4096 * 4096;

@@ -65,7 +65,7 @@ VG_DEV void eval_store(const typename S::P &p, double x, double y, double z, dou
     }
 }
 
-// Per-(solid, query) launch tuning, from the sweeps recorded in profiles/ (r1c_tuning.md):
+// Per-(solid, query) launch tuning, from the sweeps recorded in DESIGN.md, Appendix A.1:
 //   minb   -- minimum resident CTAs per SM of the direct kernel, i.e. its register cap (65536 / (256 minb)).  The
 //             straight-line distance code takes ~100 registers if allowed to, which leaves 2 CTAs per SM and too
 //             few warps to cover the FP64 latencies; capped at 64 registers (4 CTAs) it runs 15-25 % faster.
