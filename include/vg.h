@@ -275,6 +275,10 @@ int vg_query_all_host(const vg_shape *shape, const double *x, const double *y, c
  *   out: HOST int32[n] for VG_Q_INSIDE, double[n] otherwise; the caller owns every array.
  *   n > VG_STATIC_MAX_TRACKS: VG_ERR_PARAM and nothing is enqueued (split the batch, or call vg_query_host);
  *   n = 0: VG_OK, no array is touched.
+ * If `stream` is being captured into a CUDA graph, the call records its copies and its kernel as nodes of that graph and
+ * returns without waiting (host arrays must then be pinned, stay alive and hold the tracks at replay time; make one
+ * direct call on the device before the capture, which looks up the array's address).  Replays of such graphs must not
+ * overlap each other or a direct call.
  * All calls on a device share the one array: calls through this entry point are serialised by a lock and each waits
  * for its own work, so they never overlap each other, but any other way of having two of them on the GPU at once
  * (none is offered) would race.  The array keeps the previous call's contents; nothing in it needs to start at zero

@@ -13,7 +13,8 @@
 //    the array's name is a host-side stand-in, not a device address);
 //  * every call on a device uses the SAME array: two calls that overlap on the GPU (different streams, or threads)
 //    race.  Calls are serialised on the host by a lock and each call waits for its own work before it returns, so
-//    calls through this entry point cannot overlap each other;
+//    calls through this entry point cannot overlap each other.  On a stream under CUDA graph capture the call only
+//    records its copies and its kernel (it cannot wait): keeping replays apart is then the graph owner's job;
 //  * the array keeps the previous call's contents.  Nothing in it has to start at zero: a call overwrites the first n
 //    elements of every array its kernel reads and the kernel writes the first n results, which are all that is
 //    copied out.
@@ -108,7 +109,12 @@ extern "C" int vg_query_host_static(const vg_shape *shape, int query, const doub
         if ((e = cudaMemcpyAsync(out, res, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
             rc = static_cuda_fail(e, "device -> host copy");
     }
-    // always wait: the array must be free again when the lock is released, also after an error half-way
+    // A stream that is being CAPTURED into a CUDA graph cannot be waited for (and has run nothing yet): the copies and the
+    // kernel are now nodes of the caller's graph, which owns the ordering from here on -- replays of such graphs must not
+    // overlap each other or a direct call (the array is shared), and the host arrays must be pinned and alive at replay.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusActive) return rc;
+    // otherwise always wait: the array must be free again when the lock is released, also after an error half-way
     e = cudaStreamSynchronize(st);
     if (e != cudaSuccess && rc == VG_OK) rc = static_cuda_fail(e, "cudaStreamSynchronize");
     return rc;

@@ -117,3 +117,29 @@ def test_two_host_threads_share_the_array_without_racing(vg):
     for th in threads:
         th.join()
     assert not errors, errors[0]
+
+
+def test_the_call_can_be_captured_into_a_cuda_graph(vg):
+    """The caller the entry point exists for: under graph capture nothing may allocate or synchronise.  One direct call
+    first (it looks up the array's address), then the call is captured on pinned arrays; every replay answers for the
+    tracks that sit in those arrays at that moment."""
+    sc = W.shape_cases(1)[0]
+    so, sg = O.Shape(sc.kind, sc.params), vg.Shape(sc.kind, sc.params)
+    c, h = W.bounding_half(sc.kind, sc.params)
+    n = 20000
+    sets = [W.draw_tracks(500 + k, n, c, tuple(1.5 * v for v in h), band(so)) for k in range(3)]
+    ht = host(sets[0], True)
+    out = torch.empty(n, dtype=torch.float64).pin_memory()
+    sg.query_host_static("distance_to_in", *ht, step_max=W.STEP_MAX, out=out)
+    assert_real_close(out.numpy(), so.distance_to_in(*sets[0], W.STEP_MAX), "direct call before the capture")
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        sg.query_host_static("distance_to_in", *ht, step_max=W.STEP_MAX, out=out)
+    for k in (1, 2, 0):
+        for a, src in zip(ht, sets[k]):
+            a.copy_(torch.from_numpy(src))
+        out.fill_(-7.0)
+        g.replay()
+        torch.cuda.synchronize()
+        assert_real_close(out.numpy(), so.distance_to_in(*sets[k], W.STEP_MAX), "graph replay on track set %d" % k)
