@@ -545,8 +545,13 @@ static void nav_grid_fill(const std::vector<double> &sph, int nd, int nchunks, i
 static int nav_safe_dim(int nd)
 {
     if (nd < kNavSafeGridMin) return 0;
+    // about 512 cells per daughter, at most 32^3: measured at 4 Mi tracks of configs[4] (64 daughters; volume safety /
+    // world safety of the 193-node tree), 12^3 cells 242 / 348 us, 16^3 208 / 316, 24^3 193 / 302, 32^3 181 / 293
+#ifndef VG_NAV_SAFE_DENSITY
+#define VG_NAV_SAFE_DENSITY 512
+#endif
     int gs = 4;
-    while (gs < kNavSafeGridMax && gs * gs * gs < 64 * nd) gs += 4; // about 64 cells per daughter
+    while (gs < kNavSafeGridMax && gs * gs * gs < VG_NAV_SAFE_DENSITY * nd) gs += 4;
     return gs;
 }
 
@@ -579,6 +584,7 @@ static void nav_safe_grid_fill(const std::vector<double> &sph, const std::vector
             for (int ix = 0; ix < gs; ++ix) {
                 const int ic[3] = { ix, iy, iz };
                 double U = INFINITY;
+                long long first = -1; // the daughter that attains U
                 for (int i = 0; i < nd; ++i) {
                     const double *c = &sph[4 * i];
                     double n2 = 0, f2 = 0;
@@ -589,12 +595,13 @@ static void nav_safe_grid_fill(const std::vector<double> &sph, const std::vector
                         n2 += d * d, f2 += f * f;
                     }
                     dn[i] = std::sqrt(n2), df[i] = std::sqrt(f2);
-                    if (bounded[i]) U = std::fmin(U, df[i] + c[3]);
+                    if (bounded[i] && df[i] + c[3] < U) U = df[i] + c[3], first = i;
                 }
                 U = U * (1.0 + 1e-9) + gr.spad;
-                unsigned long long *m = scells + size_t((iz * gs + iy) * gs + ix) * size_t(nchunks);
+                unsigned long long *m = scells + size_t((iz * gs + iy) * gs + ix) * size_t(nchunks + 1);
                 for (int i = 0; i < nd; ++i)
                     if (dn[i] - sph[4 * i + 3] <= U) m[i / 64] |= 1ull << (i % 64);
+                m[nchunks] = first >= 0 ? (unsigned long long)first : ~0ull;
             }
 }
 
@@ -622,7 +629,7 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
     // the safety grid's masks follow the part of the blob the kernels stage in shared memory (vg_params.h)
     gr.gs = nav_safe_dim(nd);
     gr.off_s = mt.bytes;
-    v->table_bytes = size_t(mt.bytes) + 8u * size_t(gr.gs) * gr.gs * gr.gs * size_t(mt.nchunks);
+    v->table_bytes = size_t(mt.bytes) + 8u * size_t(gr.gs) * gr.gs * gr.gs * size_t(mt.nchunks + 1); // (+ 1: vg_nav_cull.h)
     std::vector<double> sph; // bounding spheres of the daughters in the mother frame: cx, cy, cz, r (FP64)
     unsigned char *host = nullptr;
     if (rc == VG_OK) {
@@ -1085,7 +1092,7 @@ extern "C" int vg_world_create(int nn, const vg_shape *const *shapes, const int3
         if (wg.g.gs > 0) {
             std::vector<char> bounded;
             for (int j = 0; j < P.nchild; ++j) bounded.push_back(shapes[kids[P.child0 + j]]->kind < VG_BOOLEAN); // (a tree or a polycone-operand boolean: kind > VG_BOOLEAN)
-            gcells.resize(gcells.size() + size_t(wg.g.gs) * wg.g.gs * wg.g.gs, 0ull);
+            gcells.resize(gcells.size() + 2 * size_t(wg.g.gs) * wg.g.gs * wg.g.gs, 0ull); // a mask and the first child per cell
             double fh[3] = { radius[p], radius[p], radius[p] }; // a polycone or boolean node: the cube about its sphere
             if (P.s.kind < kPolycone) bounding_half(P.s, fh);
             nav_safe_grid_fill(sph, bounded, P.nchild, 1, fh, wg.g, gcells.data() + wg.g.off_s);

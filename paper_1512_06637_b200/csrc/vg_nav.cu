@@ -259,25 +259,30 @@ __global__ void __launch_bounds__(kNavBlock) nav_safety_kernel(const __grid_cons
         // SafetyToIn >= |p - c| - r and a daughter whose bound is not below the running minimum is skipped.  The
         // candidates: the daughters that can be nearest to a point of the safety grid's cell (vg_nav_cull.h,
         // nav_safety_cell; read from device memory: 64 cells per daughter are too many to stage), else every daughter.
-        // The one whose sphere looks nearest (|p - c|^2 - r^2 in FP32, a heuristic with no bearing on the result: the
-        // minimum is order-independent) is evaluated first, exactly; the others meet the bound in FP32, then -- after
-        // the FP64 transform only they pay for -- in FP64 against the running minimum.
+        // One daughter is evaluated first, exactly -- the one with the smallest upper bound over the cell, stored behind
+        // the cell's masks; a heuristic with no bearing on the result, the minimum is order-independent -- and the
+        // others meet the bound against that value in FP32, then -- after the FP64 transform only they pay for -- in
+        // FP64 against the running minimum.
         if (best > 0.0 && nd > 0) {
             const float xf = float(x), yf = float(y), zf = float(z);
             const unsigned long long *cell =
                 nav_safety_cell(meta.grid, reinterpret_cast<const unsigned long long *>(table + meta.grid.off_s), meta.nchunks, x, y, z);
             const unsigned long long *cand = cell ? cell : meta.all;
             int probe = -1;
-            float key = 3.0e38f;
-            for (int c = 0; c < meta.nchunks; ++c)
-                for (unsigned long long mm = cand[c]; mm; mm &= mm - 1) {
-                    const int k = 64 * c + __ffsll((long long)mm) - 1;
-                    const float4 sp = cull[k];
-                    const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
-                    const float q = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, -sp.w)));
-                    probe = q < key ? k : probe;
-                    key = fminf(q, key);
-                }
+            if (cell) { // the daughter with the smallest upper bound over the cell (vg_volume_create)
+                probe = int(cell[meta.nchunks]);
+            } else {    // no grid (fewer than 8 daughters): the one whose sphere looks nearest to the point
+                float key = 3.0e38f;
+                for (int c = 0; c < meta.nchunks; ++c)
+                    for (unsigned long long mm = cand[c]; mm; mm &= mm - 1) {
+                        const int k = 64 * c + __ffsll((long long)mm) - 1;
+                        const float4 sp = cull[k];
+                        const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                        const float q = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, -sp.w)));
+                        probe = q < key ? k : probe;
+                        key = fminf(q, key);
+                    }
+            }
             if (probe >= 0) {
                 const Daughter &D = daughter_at(dtab, probe);
                 const double lx = fma(D.m[0], x, fma(D.m[1], y, fma(D.m[2], z, D.m[3])));

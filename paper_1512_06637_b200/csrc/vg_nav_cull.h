@@ -186,7 +186,8 @@ VG_HD unsigned long long nav_point_cell(const NavGrid &G, const unsigned long lo
 // cell: it is never the minimum, and the cell's mask leaves it out (vg_volume_create / vg_world_create; a solid that can
 // be empty -- a boolean -- gives no upper bound and does not enter U).  The cells are taken `spad` larger than they
 // are, so a point that rounding puts into the neighbouring cell still finds its nearest daughter.  Returns the cell's
-// nchunks mask words, or NULL outside the grid's box -- the mother's bounding box: such a point is outside the mother --
+// nchunks mask words -- followed by one more word: the daughter that attains U, which the kernels evaluate first (any
+// choice gives the same minimum; ~0 if no daughter bounds the cell) -- or NULL outside the grid's box -- the mother's bounding box: such a point is outside the mother --
 // or without a grid: the caller then keeps every daughter.
 VG_HD const unsigned long long *nav_safety_cell(const NavGrid &G, const unsigned long long *scells, int nchunks, double x,
                                                 double y, double z)
@@ -195,7 +196,7 @@ VG_HD const unsigned long long *nav_safety_cell(const NavGrid &G, const unsigned
     if (G.gs <= 0 || !(px >= 0.0 && px <= G.slen[0] && py >= 0.0 && py <= G.slen[1] && pz >= 0.0 && pz <= G.slen[2])) return nullptr;
     int ix = int(floor(px * G.sics[0])), iy = int(floor(py * G.sics[1])), iz = int(floor(pz * G.sics[2]));
     ix = ix > G.gs - 1 ? G.gs - 1 : ix, iy = iy > G.gs - 1 ? G.gs - 1 : iy, iz = iz > G.gs - 1 ? G.gs - 1 : iz;
-    return scells + size_t((iz * G.gs + iy) * G.gs + ix) * size_t(nchunks);
+    return scells + size_t((iz * G.gs + iy) * G.gs + ix) * size_t(nchunks + 1);
 }
 
 // Both stages.  `all[c]` = every daughter of chunk c (what a start point outside the mother's bounding sphere keeps).

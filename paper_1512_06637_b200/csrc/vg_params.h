@@ -233,7 +233,8 @@ struct Daughter {
 //   [off_g, off_g + 8 ncell nchunks)  candidate masks of the grid cells (NavGrid below), off_g a multiple of 16
 //   [off_p, off_p + 4 ncell)          the only daughter of each cell or -1
 //   total (NavMeta::bytes) rounded up to a multiple of 16 bytes (bulk-copy granularity)
-//   [off_s, off_s + 8 gs^3 nchunks)   behind the staged part, read from device memory: the safety grid's masks
+//   [off_s, off_s + 8 gs^3 (nchunks + 1))  behind the staged part, read from device memory: the safety grid's cells
+//                                     (nchunks masks + the daughter to evaluate first)
 constexpr int kCullUnroll = 8;
 constexpr int kDaughterStride = int(sizeof(Daughter)) + (((sizeof(Daughter) / 8) % 2 == 0) ? 8 : 0);
 constexpr int kNavChunks = 4; // 64 daughters per chunk, VG_MAX_DAUGHTERS = 256
@@ -246,7 +247,10 @@ constexpr int kNavGridMax = 8; // cells per axis
 // The safety grid (vg_nav_cull.h, nav_safety_cell): a finer grid over the mother's own bounding box (every point with a
 // positive SafetyToOut lies in it) whose cells list the daughters that can be the NEAREST one of a point of the cell
 // (bounding-sphere bounds, taken at create time).
-constexpr int kNavSafeGridMax = 16;
+#ifndef VG_NAV_SAFE_MAX
+#define VG_NAV_SAFE_MAX 32
+#endif
+constexpr int kNavSafeGridMax = VG_NAV_SAFE_MAX;
 constexpr int kNavSafeGridMin = 8; // daughters from which the grid is built
 struct NavGrid {
     double o[3], len[3], cs[3], ics[3]; // origin, extent, cell size and its inverse per axis

@@ -211,27 +211,33 @@ __global__ void __launch_bounds__(kWorldBlock)
         // SafetyToIn of a child >= |p - c| - r: a child whose bound is not below the running minimum is skipped (valid for
         // a minimum of either sign, so trees whose children overlap or stick out of their parent get the plain minimum too).
         // The candidates: for a node with a safety grid, the children that can be nearest to a point of its cell
-        // (vg_nav_cull.h, nav_safety_cell), else every child.  The one whose sphere looks nearest (|p - c|^2 - r^2 in
-        // FP32, a heuristic with no bearing on the result: the minimum is order-independent) is evaluated first, so
-        // that the bound, taken in FP64 against the running minimum, leaves few of the others.
+        // (vg_nav_cull.h, nav_safety_cell), else every child.  One child is evaluated first -- the one with the smallest
+        // upper bound over the cell, stored with the cell, else the one whose sphere looks nearest in FP32; a heuristic
+        // with no bearing on the result, the minimum is order-independent -- so that the bound, taken in FP64 against
+        // the running minimum, leaves few of the others.
         const float xf = float(x), yf = float(y), zf = float(z);
         for (int base = 0; base < nc; base += 64) { // (every chunk whatever the sign so far: the result is the plain minimum)
             const int lim = min(64, nc - base);
             unsigned long long m = lim == 64 ? ~0ull : ((1ull << lim) - 1ull);
+            int probe = -1;
+            const unsigned long long *cell = nullptr;
             if (N.grid >= 0) {
                 const WorldGrid &G = w.grids[N.grid];
-                const unsigned long long *cell = nav_safety_cell(G.g, w.gcells + G.g.off_s, 1, x, y, z);
-                m = cell ? *cell : m;
+                cell = nav_safety_cell(G.g, w.gcells + G.g.off_s, 1, x, y, z);
             }
-            int probe = -1;
-            float key = 3.0e38f;
-            for (unsigned long long mm = m; mm; mm &= mm - 1) {
-                const int j = __ffsll((long long)mm) - 1;
-                const float4 sp = __ldg(cull + c0 + base + j);
-                const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
-                const float k = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, -sp.w)));
-                probe = k < key ? j : probe;
-                key = fminf(k, key);
+            if (cell) { // the cell's list, and the child with the smallest upper bound over the cell
+                m = cell[0];
+                probe = int(cell[1]);
+            } else {
+                float key = 3.0e38f;
+                for (unsigned long long mm = m; mm; mm &= mm - 1) {
+                    const int j = __ffsll((long long)mm) - 1;
+                    const float4 sp = __ldg(cull + c0 + base + j);
+                    const float vx = xf - sp.x, vy = yf - sp.y, vz = zf - sp.z;
+                    const float k = fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, -sp.w)));
+                    probe = k < key ? j : probe;
+                    key = fminf(k, key);
+                }
             }
             if (probe >= 0) {
                 const WorldNode &C = nodes[kids[c0 + base + probe]];
