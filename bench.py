@@ -730,7 +730,7 @@ def run_profile(args):
     for n_small in (1024, 16384):
         cases.append(Case(vg, torch, pc.name, n_small, pc.queries, shape=pc))
     nav = W.navigator_case()
-    cases.append(Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step",), nav=nav))
+    cases.append(Case(vg, torch, "navigator", nav.sizes[-1], ("compute_step", "volume_safety"), nav=nav))
     wc = W.world_case()
     cases.append(Case(vg, torch, "world", wc.sizes[-1], ("world_locate", "world_step", "world_safety"), world=wc))
     bc = [b for b in W.boolean_cases() if b.name == "box_minus_tube"][0]
