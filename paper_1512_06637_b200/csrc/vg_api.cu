@@ -607,8 +607,9 @@ static void nav_safe_grid_fill(const std::vector<double> &sph, const std::vector
 
 // Host side of vg_volume_create for a volume of primitives: validation, the mother and daughter records, the FP32
 // bounding spheres and the candidate grid, as one blob in host memory (layout: vg_params.h).  No CUDA call.
+// `with_safe` = false leaves the safety grid out (vg_debug_nav_cull for the stages that do not read it).
 static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const *daughters, const double *xforms,
-                          vg_volume *v, unsigned char **host_out)
+                          vg_volume *v, unsigned char **host_out, bool with_safe = true)
 {
     int rc = to_solid(mother, &v->mother, "mother");
     NavMeta &mt = v->meta;
@@ -627,7 +628,7 @@ static int nav_build_host(const vg_shape *mother, int nd, const vg_shape *const 
     mt.bytes = (gr.off_p + 4u * ncell + 15u) / 16u * 16u;
     if (nchunks_alloc) mt.nchunks = int(nchunks_alloc);
     // the safety grid's masks follow the part of the blob the kernels stage in shared memory (vg_params.h)
-    gr.gs = nav_safe_dim(nd);
+    gr.gs = with_safe ? nav_safe_dim(nd) : 0;
     gr.off_s = mt.bytes;
     v->table_bytes = size_t(mt.bytes) + 8u * size_t(gr.gs) * gr.gs * gr.gs * size_t(mt.nchunks + 1); // (+ 1: vg_nav_cull.h)
     std::vector<double> sph; // bounding spheres of the daughters in the mother frame: cx, cy, cz, r (FP64)
@@ -1240,7 +1241,7 @@ extern "C" int vg_debug_nav_cull(const vg_shape *mother, int nd, const vg_shape 
     vg_volume v;
     std::memset(&v, 0, sizeof v);
     unsigned char *host = nullptr;
-    int rc = nav_build_host(mother, nd, daughters, xforms, &v, &host);
+    int rc = nav_build_host(mother, nd, daughters, xforms, &v, &host, stage == 4);
     if (rc != VG_OK) return rc;
     const NavMeta &mt = v.meta;
     const float4 *cull = reinterpret_cast<const float4 *>(host);
