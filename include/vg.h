@@ -170,6 +170,9 @@ int vg_query_all(const vg_shape *shape, const double *x, const double *y, const 
  * daughter table staged in shared memory by TMA); a polycone or boolean among them (reading R30) makes the volume a
  * one-level world served by the world kernels, with the same results and conventions.
  * The shapes' constants are copied; the vg_shape handles may be destroyed afterwards.
+ * Built here, once, on the host and placed on the current device: the daughters' bounding spheres, the candidate grid of
+ * ComputeStep and -- for 8 daughters or more -- the grid of nearest-daughter lists that vg_volume_safety reads (up to
+ * 32^3 cells): about 40 ms for 64 daughters, 160 ms for 256, and 0.5 / 1.3 MiB of device memory.
  */
 int vg_volume_create(const vg_shape *mother, int ndaughters, const vg_shape *const *daughters, const double *xforms,
                      vg_volume **out);
