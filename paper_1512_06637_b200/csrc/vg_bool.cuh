@@ -130,16 +130,32 @@ VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, dou
     bool ina = ca == cInside, inb = cb == cInside;
     bool pend_a = ca == cSurface, pend_b = cb == cSurface;
     double tt = 0.0;
+    int last = 0;                 // the operand whose crossing the previous event was: 1 = A, 2 = B
+    double offa = 0.0, offb = 0.0; // see below
 #pragma unroll 1
     for (int it = 0; it < kBoolMaxEvents; ++it) {
-        const double ea = opnd_next<KA, X>(p.a, ina, fma(tt, dx, x), fma(tt, dy, y), fma(tt, dz, z), dx, dy, dz);
-        const double eb = opnd_next<KB, X>(p.b, inb, fma(tt, bdx, bx), fma(tt, bdy, by), fma(tt, bdz, bz), bdx, bdy, bdz);
+        const double ta = tt + offa, tb = tt + offb;
+        const double ea = offa + opnd_next<KA, X>(p.a, ina, fma(ta, dx, x), fma(ta, dy, y), fma(ta, dz, z), dx, dy, dz);
+        const double eb = offb + opnd_next<KB, X>(p.b, inb, fma(tb, bdx, bx), fma(tb, bdy, by), fma(tb, bdz, bz), bdx, bdy, bdz);
+        // An operand asked again from the very crossing it has just taken must answer with a LATER one.  It answers 0
+        // when it has just been left through a chord shorter than kRayTol: the entering crossing, that little behind,
+        // counts as lying at the start (R32), and the machine would enter and leave on the spot until the event limit.
+        // A zero from the operand of the last event is asked again, once, from 2 kRayTol further on (a rare extra trip).
+        if (last == 1 && offa == 0.0 && !(ea > 0.0)) {
+            offa = 2.0 * kRayTol;
+            continue;
+        }
+        if (last == 2 && offb == 0.0 && !(eb > 0.0)) {
+            offb = 2.0 * kRayTol;
+            continue;
+        }
+        offa = offb = 0.0;
         if (pend_a || pend_b) { // first pass only, and only for a start on an operand's surface
             const bool fix_a = pend_a && !(ea <= kRayTol), fix_b = pend_b && !(eb <= kRayTol);
             pend_a = pend_b = false;
             ina = ina || fix_a;
             inb = inb || fix_b;
-            if (fix_a || fix_b) continue;
+            if (fix_a || fix_b) continue; // (last stays 0: no event yet)
         }
         const bool a_first = ea <= eb; // a tie goes to A, as in the oracle's merge
         const double e = a_first ? ea : eb;
@@ -147,6 +163,7 @@ VG_DEV double bool_distance(const BoolP &p, bool to_out, double x, double y, dou
         tt += e;
         ina = a_first ? !ina : ina;
         inb = a_first ? inb : !inb;
+        last = a_first ? 1 : 2;
         if (bool_member(p.op, ina, inb) != to_out) return tt;
     }
     return inf();

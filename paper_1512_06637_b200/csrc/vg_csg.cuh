@@ -148,7 +148,12 @@ VG_DEV double csg_distance(const CsgP &p, bool to_out, double x, double y, doubl
         if (imin < 0) break;
         bits ^= 1u << imin;
         if (csg_member(p, bits) != to_out) return emin;
-        tn[imin] = emin + csg_leaf_next(p, imin, (bits >> imin) & 1u, emin, x, y, z, dx, dy, dz);
+        // the primitive's next crossing must lie beyond the one just taken: a zero (it has just been left through a chord
+        // shorter than kRayTol, and the entering crossing that little behind counts as lying at the start, R32) is asked
+        // again from 2 kRayTol further on, or the machine would enter and leave on the spot until the event limit
+        double nx = csg_leaf_next(p, imin, (bits >> imin) & 1u, emin, x, y, z, dx, dy, dz);
+        if (!(nx > 0.0)) nx = 2.0 * kRayTol + csg_leaf_next(p, imin, (bits >> imin) & 1u, emin + 2.0 * kRayTol, x, y, z, dx, dy, dz);
+        tn[imin] = emin + nx;
     }
     return inf();
 }

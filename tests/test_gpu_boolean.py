@@ -342,3 +342,47 @@ def test_boolean_with_polycone_operands_matches_the_oracle(vg, case):
     assert_int_equal(cg.inside(*ds[:3]).cpu().numpy(), co.inside(*ts[:3]), name + " border inside")
     for q in ("distance_to_in", "distance_to_out"):
         assert_real_close(getattr(cg, q)(*ds, W.STEP_MAX).cpu().numpy(), getattr(co, q)(*ts, W.STEP_MAX), "%s border %s" % (name, q))
+
+
+@pytest.mark.parametrize("eps", [2e-8, 7e-8, 2e-7, 3e-7, 1e-6, 1e-3])
+def test_a_chord_shorter_than_the_ray_tolerance_does_not_stall_the_state_machine(vg, eps):
+    """A ray that clips an edge of an operand through a chord of ~1e-7 (shorter than VG_KRAYTOL) leaves that operand with
+    its entering crossing still 'at the start' (R32): asked for its next entering crossing it answered 0, and the state
+    machines of the booleans entered and left it on the spot until their event limit and returned +inf (found by the
+    8000-tree soak: one track in 10^8).  B = the unit cube, clipped at its edge x = y = 1 along d = (1, -1, 0) / sqrt 2;
+    A = a box 8 further along the ray; E = a large box around everything; D = an orb far away.  The clip must not decide
+    anything: DistanceToIn of A - B, (A - B) u D and (B n D) u A is A's entry; DistanceToOut of E u B and (E u B) u D from
+    a start inside E is E's exit."""
+    s0 = 5.0
+    d = np.array([1.0, -1.0, 0.0]) / np.sqrt(2.0)
+    mid = np.array([1.0 - eps / 2, 1.0 - eps / 2, 0.0])   # middle of the chord: the line x + y = 2 - eps cuts the corner
+    n = 64
+    z0 = np.random.default_rng(3).uniform(-0.5, 0.5, n)    # the same clip at 64 heights
+    P = mid[None, :] - s0 * d[None, :] + np.stack([0 * z0, 0 * z0, z0], axis=1)
+    ca = mid + 8.0 * d                                     # centre of A
+
+    def tracks(origin):  # the rays in the frame whose origin sits at `origin` (no rotation)
+        Q = P - np.asarray(origin)[None, :]
+        return tuple(np.ascontiguousarray(a) for a in (Q[:, 0], Q[:, 1], Q[:, 2], np.full(n, d[0]), np.full(n, d[1]), np.full(n, d[2])))
+    to_b_from_a = W.placement(np.eye(3), tuple(-ca))       # B as seen from the frame of A: centred at -ca (B sits at the world's origin)
+    far = W.placement(np.eye(3), (0.0, 0.0, -40.0))
+    ident = W.placement(np.eye(3), (0.0, 0.0, 0.0))
+
+    def build(mod):
+        A, B, D, E = (lambda: mod.Shape(W.BOX, [1.0, 1.0, 2.0])), (lambda: mod.Shape(W.BOX, [1.0, 1.0, 1.0])), \
+                     (lambda: mod.Shape(W.ORB, [1.0])), (lambda: mod.Shape(W.BOX, [30.0, 30.0, 30.0]))
+        a_minus_b = lambda: mod.Boolean(W.SUBTRACTION, A(), B(), to_b_from_a)
+        return {  # name: (solid, origin of its frame, query)
+            "A - B": (a_minus_b(), ca, "distance_to_in"),
+            "(A - B) u D": (mod.Boolean(W.UNION, a_minus_b(), D(), far), ca, "distance_to_in"),
+            "(B n D) u A": (mod.Boolean(W.UNION, mod.Boolean(W.INTERSECTION, B(), D(), far), A(), W.placement(np.eye(3), tuple(ca))), (0, 0, 0), "distance_to_in"),
+            "E u B": (mod.Boolean(W.UNION, E(), B(), ident), (0, 0, 0), "distance_to_out"),
+            "(E u B) u D": (mod.Boolean(W.UNION, mod.Boolean(W.UNION, E(), B(), ident), D(), far), (0, 0, 0), "distance_to_out"),
+        }
+    so, sg = build(O), build(vg)
+    for name, (co, origin, q) in so.items():
+        t = tracks(origin)
+        want = getattr(co, q)(*t, W.STEP_MAX)
+        assert np.isfinite(want).all() and (want > s0 + 1.0).all(), name  # the answer lies beyond the clip
+        got = getattr(sg[name][0], q)(*dev(t), W.STEP_MAX).cpu().numpy()
+        assert_real_close(got, want, "%s %s, chord %g" % (name, q, eps * np.sqrt(2.0)))

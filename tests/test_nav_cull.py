@@ -339,3 +339,51 @@ def test_the_safety_cell_of_a_point_lists_its_nearest_daughter():
                 listed = bits[:, inbox].sum() / max(1, inbox.sum())
         if si == 0:
             assert listed < 12.0, "configs[4]: %.1f of 64 daughters listed per cell: the grid does not prune" % listed
+
+
+def test_the_walk_lists_every_daughter_whose_bounding_sphere_the_ray_meets():
+    """The grid walk on its own (stage 1), against geometry written out here: every daughter whose TRUE bounding sphere
+    (centre -R^T b, radius of the solid about its origin, no inflation) is met by the ray between the start point and
+    the limit must be in the walk's mask -- a tighter statement than 'no hit is culled' (the spheres are much larger
+    than the solids), and the one the walk's rounding margins (FP32 stepping, padded cells) have to deliver.  Rays along
+    the grid's planes, edges and diagonals, tangent rays, rays with tiny components, limits set exactly at the sphere."""
+    for si, (sc, half) in enumerate((config4_scene(), random_scene(4242, 40, 50.0, 12.0, 35.0), random_scene(8, 64, 1e4, 1e-2, 0.9e4),
+                                     random_scene(99, 200, 100.0, 6.0, 90.0), random_scene(5, 100, 50.0, 20.0, 30.0))):
+        nd = len(sc.kinds)
+        rad = np.zeros(nd)
+        for j, (kind, par) in enumerate(zip(sc.kinds, sc.params)):
+            if kind == W.BOX:
+                rad[j] = np.linalg.norm(par[:3])
+            elif kind == W.TRD:
+                rad[j] = np.linalg.norm([max(par[0], par[1]), max(par[2], par[3]), par[4]])
+            elif kind == W.ORB:
+                rad[j] = par[0]
+            elif kind == W.TUBE:
+                rad[j] = math.hypot(par[1], par[2])
+            else:
+                rad[j] = math.hypot(max(par[1], par[3]), par[4])
+        rng = np.random.default_rng(31 + si)
+        _, grid = sc.masks(np.zeros((1, 3)), np.array([[0.0, 0.0, 1.0]]))
+        for name, gen in (("random", random_rays), ("aimed", aimed_rays), ("tangent", tangent_rays),
+                          ("tiny component", tiny_component_rays), ("grid", lambda s, r, n, h: grid_rays(s, r, n, h, grid))):
+            P, D = gen(sc, rng, 40000, half)
+            P, D = np.ascontiguousarray(P), np.ascontiguousarray(D)
+            inside_mother = sc.o_mother.inside(P[:, 0], P[:, 1], P[:, 2]) != O.OUTSIDE
+            P, D = P[inside_mother], D[inside_mother]
+            V = sc.centers[:, None, :] - P[None, :, :]                      # (nd, n, 3)
+            tca = np.einsum("knj,nj->kn", V, D)
+            d2 = np.einsum("knj,knj->kn", V, V) - tca * tca
+            r2 = (rad * rad)[:, None]
+            thc = np.sqrt(np.maximum(r2 - d2, 0.0))
+            t_in, t_out = tca - thc, tca + thc                               # the ray is inside the sphere for t in [t_in, t_out]
+            met = (d2 <= r2 * (1 - 1e-12)) & (t_out >= 0)
+            first = np.where(met, np.maximum(t_in, 0.0), np.inf)
+            for t_lim in (None, np.where(np.isfinite(first.min(axis=0)), first.min(axis=0), 1.0)):
+                must = met if t_lim is None else met & (first <= t_lim[None, :])
+                m, _ = sc.masks(P, D, t_lim, 1)
+                bits = np.zeros((nd, len(P)), dtype=bool)
+                for k in range(nd):
+                    bits[k] = (m[:, k // 64] >> np.uint64(k % 64)) & np.uint64(1) == 1
+                lost = must & ~bits
+                assert not lost.any(), "scene %d, %s rays, limit %s: the walk misses %d (daughter, ray) pairs whose sphere the ray meets, first %s" % (
+                    si, name, "none" if t_lim is None else "at the nearest sphere", lost.sum(), np.argwhere(lost)[:3].tolist())
