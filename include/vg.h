@@ -120,7 +120,8 @@ int vg_shape_create(vg_kind kind, const double *params, int nparams, vg_shape **
  *   distances    the first t > 0 at which the membership of C along the ray flips, +inf if none, -1 on the wrong side
  *                (R28; the operands' memberships follow from their crossings along the whole line, so a start point on
  *                an operand's surface that is hidden inside the other operand is an ordinary inside point of C); R32
- *                from a start point of class SURFACE;
+ *                from a start point of class SURFACE; a ray that clips an operand through a chord shorter than
+ *                VG_KRAYTOL passes that operand's two crossings like any others (it is never held there);
  *   safeties     the composed bound sdf_C = min(sdfA, sdfB) / max(sdfA, sdfB) / max(sdfA, -sdfB): it has the sign of the
  *                membership and never over-estimates the distance to the surface of C, but unlike the primitives'
  *                safeties it is not the exact distance everywhere (R29).
